@@ -1,0 +1,168 @@
+/*
+ * modal.h -- C ABI of libmodal.so: B200 (sm_100a) time-stepping of N_q coupled modal
+ * oscillators (arXiv 2505.05940), batched over parameter sets.
+ *
+ * The library implements the data-parallel hot path of the paper:
+ *   q''_k + 2 gamma_k q'_k + omega_k^2 q_k = fext_k - fnl_k(q)        (Eq. 12)
+ * advanced by the explicit two-step schemes of PAPER.md:138-167 (Eq. 15-23), with
+ *   fnl = 0                                   MODAL_LINEAR
+ *   fnl_k = c lambda_k q_k sum_v lambda_v q_v^2   MODAL_TENSION  (Eq. 8)
+ *   fnl_k = sum_n eta_n sum_r H^n_kr q_r,  eta_n = s_n sum_pq H^n_pq q_p q_q
+ *                                             MODAL_VK       (Eq. 9-11;
+ *                                             C eliminated by H^k_ij = C^j_ik)
+ * and a point read-out out[b][n] = sum_k w_k q_k^n.
+ *
+ * Every step of the path runs in hand-written CUDA kernels; there is no CPU fallback:
+ * modal_simulate() on a plan created without a device returns MODAL_ECUDA.
+ *
+ * Conventions
+ *  - All descriptor quantities are SI, fp64.  Host arrays are fp64; the device keeps the
+ *    coupling tensor, s_n, w_k, lambda_k in fp32 and the oscillator state and update
+ *    coefficients in fp64.
+ *  - Ownership: the caller owns every buffer it passes; the library copies what it needs
+ *    before returning.  The library owns the plan and its device storage.
+ *  - Errors: every call returns a modal_status and never aborts or throws.  All validation
+ *    messages of the last failing (or warning) call on a plan are available, '\n'-separated,
+ *    from modal_last_error(); for a failed modal_plan_create (*out == NULL) pass NULL.
+ *  - Modes beyond the stability limit of the scheme are masked (q_k == 0, excluded from
+ *    force, projection and read-out; reading R11); masking is a warning.
+ *  - Thread safety: calls on different plans may run concurrently; calls on one plan may not.
+ */
+#ifndef MODAL_H_
+#define MODAL_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct modal_plan modal_plan; /* opaque, owned by the library */
+
+typedef enum {
+    MODAL_OK = 0,
+    MODAL_EINVAL = 1,    /* descriptor / argument validation failed                        */
+    MODAL_EINCOMPAT = 2, /* valid request this build cannot run (size limits)              */
+    MODAL_EUNSTABLE = 3, /* a sample went non-finite; first_bad_step says where            */
+    MODAL_ECUDA = 4,     /* CUDA runtime error, or no device attached to the plan          */
+    MODAL_ENOMEM = 5
+} modal_status;
+
+typedef enum { MODAL_LINEAR = 0, MODAL_TENSION = 1, MODAL_VK = 2 } modal_model;
+typedef enum { MODAL_SV = 0, MODAL_FTM = 1 } modal_scheme;
+typedef enum { MODAL_STRING = 0, MODAL_RECT = 1 } modal_geom;
+typedef enum { MODAL_BC_FIXED_SS = 0 } modal_bc; /* fixed string / simply supported plate */
+
+/* Reference geometry, material and sizes of a plan (Eq. 1-4). */
+typedef struct {
+    int model, scheme, geom, bc; /* the enums above                                            */
+    double Lx, Ly, h;            /* string: Lx = L; Ly, h unused                               */
+    double E, rho, nu;           /* rho: kg/m^3 (plate) or kg/m (string)  (reading R3)         */
+    double T0, D;                /* tension; bending stiffness. RECT with D <= 0 => E h^3/(12(1-nu^2)) */
+    double area;                 /* string cross-section A for tau = E A / (2 L)  (Eq. 4)      */
+    double sigma0, sigma1;       /* gamma_k = sigma0 + sigma1 lambda_k  (Eq. 14, reading R9)   */
+    double pickup_x, pickup_y;   /* read-out point, metres (string: pickup_x only)             */
+    int n_q, n_phi;              /* transverse / in-plane mode counts; n_phi = 0 unless VK     */
+    double sample_rate;          /* Hz                                                         */
+    int max_batch, max_steps;    /* sizes the plan's device storage                            */
+} modal_plan_desc;
+
+/* Create a plan: validates the descriptor (all violations are reported), derives the mode
+ * index sets, lambda_k, omega_k, gamma_k, the stability mask, s_n / tau/rho, the pickup
+ * weights and (VK) the coupling tensor H of the simply supported plate in closed form, packs
+ * H into its device layout and allocates device storage on `cuda_device`.
+ * cuda_device < 0 creates a host-only plan (queries work, modal_simulate returns MODAL_ECUDA).
+ * `desc` stays owned by the caller.  On failure *out = NULL. */
+modal_status modal_plan_create(const modal_plan_desc *desc, int cuda_device, modal_plan **out);
+
+/* Replace coefficients (Eq. 13-14; Eq. 9-11).  Any pointer may be NULL =
+ * keep the plan's current value.  All pointers are HOST pointers; the library copies.
+ * Per-sample arrays have coeff_batch rows: 1 (broadcast to every sample) or the batch of the
+ * following modal_simulate calls (<= max_batch).  All non-NULL per-sample arrays of one call
+ * share coeff_batch; arrays left NULL keep their previous rows only if coeff_batch is
+ * unchanged, otherwise row 0 of the previous value is broadcast. */
+typedef struct {
+    int coeff_batch;
+    const double *omega;    /* [coeff_batch][n_q]  rad/s                                          */
+    const double *sigma;    /* [coeff_batch][n_q]  1/s   (gamma_k)                                */
+    const double *nl_scale; /* VK: s_n = E/(2 rho zeta_n^4) (x geometry scale, reading R14)       */
+                            /*     [coeff_batch][n_phi];  TENSION: tau/rho_m  [coeff_batch]       */
+    const double *lambda;   /* TENSION: [coeff_batch][n_q]                                        */
+    const double *pickup;   /* [coeff_batch][n_q]                                                 */
+    const double *H_full;   /* VK: [n_phi][n_q][n_q] row-major, shared by the whole batch.  The   */
+                            /* library checks |H[n][p][q]-H[n][q][p]| <= 1e-12 max|H| and packs.  */
+} modal_coeffs;
+modal_status modal_coeffs_upload(modal_plan *plan, const modal_coeffs *coeffs);
+
+typedef struct {
+    const double *q0;        /* host [batch][n_q]: modal displacement at n = 0                    */
+    const double *qm1;       /* host [batch][n_q]: displacement at n = -1; NULL => zero initial   */
+                             /* velocity, q^-1 = q^0 + (T^2/2)(-omega^2 q^0 - fnl(q^0)) (R8),     */
+                             /* evaluated on the device                                            */
+    const float *fext_signal;/* optional DEVICE [batch][n_steps] scalar force signal, NULL = none */
+    const double *fext_gain; /* optional host [batch][n_q]: Phi_k(x_e)/mass; required with signal */
+    double *traj_dev;        /* optional DEVICE [batch][n_steps][n_q]: receives q^n (diagnostics) */
+} modal_init;
+
+/* Run n_steps of the recurrence for `batch` samples (Eq. 19/20):
+ *   out_audio_dev[b][n] = sum_k w_k q_k^n,  n = 0 .. n_steps-1   (n = 0 is the initial state, R10)
+ * out_audio_dev: DEVICE pointer, [batch][n_steps] fp32 row-major, caller-allocated.
+ * first_bad_step: host [batch] or NULL.  When non-NULL the call synchronises the stream and
+ *   fills first_bad_step[b] with the first n at which sample b's state was non-finite (-1 if
+ *   none) and returns MODAL_EUNSTABLE iff any is >= 0; the finite prefix of the output is valid.
+ *   When NULL the work is only enqueued on `cuda_stream` (a cudaStream_t, NULL = default).
+ * Errors: MODAL_EINVAL (batch/steps outside the plan, missing q0), MODAL_ECUDA. */
+modal_status modal_simulate(modal_plan *plan, int batch, int n_steps, const modal_init *init,
+                            float *out_audio_dev, int *first_bad_step, void *cuda_stream);
+
+/* Same, with a HOST output buffer [batch][n_steps]; the library stages through plan-owned
+ * device memory (host<->device copies included).  Always synchronous. */
+modal_status modal_simulate_host(modal_plan *plan, int batch, int n_steps, const modal_init *init,
+                                 float *out_audio_host, int *first_bad_step);
+
+void modal_plan_destroy(modal_plan *plan);
+const char *modal_last_error(const modal_plan *plan);
+
+/* ---- host-side helpers (no device needed) --------------------------------------------- */
+
+typedef enum {
+    MODAL_Q_MODE_M = 0,      /* int    [n_q]    transverse mode index m_k                          */
+    MODAL_Q_MODE_N = 1,      /* int    [n_q]    transverse mode index n_k (string: all 0)          */
+    MODAL_Q_PHI_M = 2,       /* int    [n_phi]                                                      */
+    MODAL_Q_PHI_N = 3,       /* int    [n_phi]                                                      */
+    MODAL_Q_LAMBDA = 4,      /* double [n_q]    lambda_k of the reference geometry                  */
+    MODAL_Q_OMEGA = 5,       /* double [coeff_batch][n_q]                                           */
+    MODAL_Q_SIGMA = 6,       /* double [coeff_batch][n_q]                                           */
+    MODAL_Q_NL_SCALE = 7,    /* double [coeff_batch][n_phi] (VK) or [coeff_batch] (TENSION)         */
+    MODAL_Q_PICKUP = 8,      /* double [coeff_batch][n_q]   (before masking)                        */
+    MODAL_Q_ACTIVE = 9,      /* int    [coeff_batch][n_q]   1 = active, 0 = masked (R11)            */
+    MODAL_Q_H_FULL = 10,     /* double [n_phi][n_q][n_q]: the fp32 values the device holds, widened */
+    MODAL_Q_COEFF_BATCH = 11,/* int    [1]                                                          */
+    MODAL_Q_KERNEL_INFO = 12 /* int    [8]: kernel family, cluster size, clusters, threads, smem    */
+                             /*        bytes, resident flag, tiles per n, padded n_q (last launch)  */
+} modal_query;
+/* Copies the item into `dst` (capacity `dst_bytes`); returns MODAL_EINVAL if it does not fit. */
+modal_status modal_plan_query(const modal_plan *plan, int what, void *dst, unsigned long long dst_bytes);
+
+/* Per-sample coefficients for a geometry other than the plan's reference one, with the PLAN'S
+ * mode index sets (reading R14): for RECT fills omega, sigma [n_q], nl_scale [n_phi]
+ * (= E/(2 rho zeta^4) (c_b/c_ref)^2, c = (Lx Ly)^(-5/2)) and pickup [n_q] at
+ * (pickup_x_frac Lx, pickup_y_frac Ly); for STRING fills omega, sigma, lambda, pickup [n_q] and
+ * nl_scale [1] = tau/rho_lin.  Fields of `geom` that are <= 0 / NaN fall back to the plan's. */
+typedef struct {
+    double Lx, Ly, h;           /* RECT; STRING: Lx = L                                          */
+    double T0, D, rho, area;    /* STRING per-sample tension, stiffness, linear density, section */
+    double pickup_x_frac, pickup_y_frac;
+} modal_sample_geom;
+modal_status modal_derive_coeffs(const modal_plan *plan, const modal_sample_geom *geom,
+                                 double *omega, double *sigma, double *nl_scale,
+                                 double *lambda, double *pickup);
+
+/* q0[k] = int w0 Phi_k for the raised-cosine bump w0 = (A/2)(1 + cos(2 pi r / W)), r < W/2
+ * centred at (x0,y0) (string: x0) on a sample of size (Lx, Ly) with the plan's index sets
+ * (reading R13).  q0: host [n_q]. */
+modal_status modal_project_bump(const modal_plan *plan, double Lx, double Ly, double x0, double y0,
+                                double W, double A, double *q0);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MODAL_H_ */

@@ -1,0 +1,652 @@
+// modal_api.cu -- the C ABI of include/modal.h: plan, coefficient upload, launch logic.
+// Host-side derivations live in host_math.hpp, kernels in kernels.cuh.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/modal.h"
+#include "host_math.hpp"
+#include "kernels.cuh"
+
+namespace mh = modal_host;
+namespace md = modal_dev;
+
+static_assert(sizeof(mh::Unit) == sizeof(md::VkUnit), "schedule unit layout");
+
+namespace {
+
+thread_local std::string g_create_error;   // messages of a failed modal_plan_create
+
+constexpr size_t SMEM_LIMIT = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100
+
+struct DevBuf {
+    void *p = nullptr; size_t bytes = 0;
+    cudaError_t ensure(size_t n) {
+        if (n <= bytes) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; bytes = 0;
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e == cudaSuccess) bytes = n;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+    template <class T> T *as() const { return reinterpret_cast<T *>(p); }
+};
+
+struct VkConfig {
+    int CS = 1, NCL = 1, NW = 16, grid_team = 0, resident = 0, n_clusters = 1;
+    size_t smem = 0;
+    mh::Schedule sched;
+    DevBuf units, warp_ptr, cta_ptr, nlo;
+    bool uploaded = false;
+};
+
+}  // namespace
+
+struct modal_plan {
+    modal_plan_desc d{};
+    int device = -1;
+    double T = 0;
+    mh::ModeSet mq, mphi;
+    int NQP = 0;                 // padded mode count of the device layout
+    int coeff_batch = 1;
+    std::vector<double> omega, sigma, nl_scale, lambda_s, pickup;   // [coeff_batch][...]
+    std::vector<int> active;                                          // [coeff_batch][n_q]
+    std::vector<float> Ht;                                            // tile-packed H (VK)
+    bool coeffs_dirty = true, H_dirty = true;
+    std::string err;
+    int sm_count = 148;
+    // device storage
+    DevBuf dHt, dkv, dkq, dr, dast, ds, dw, dlam, dc, dq0, dv0, dgain, dbad, dout, dfbuf, dcounter;
+    std::map<long long, VkConfig> vk_cfgs;
+    int kinfo[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+
+namespace {
+
+#define CU(call)                                                                             \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess) {                                                             \
+            p->err += std::string("CUDA error: ") + cudaGetErrorString(e_) + " at " #call "\n"; \
+            return MODAL_ECUDA;                                                              \
+        }                                                                                    \
+    } while (0)
+
+int n_nl(const modal_plan *p) { return p->d.model == MODAL_VK ? p->d.n_phi : 1; }
+
+bool validate_desc(const modal_plan_desc &d, std::string &err)
+{
+    auto bad = [&](const char *m) { err += m; err += "\n"; };
+    if (d.model < MODAL_LINEAR || d.model > MODAL_VK) bad("model must be MODAL_LINEAR, MODAL_TENSION or MODAL_VK");
+    if (d.scheme != MODAL_SV && d.scheme != MODAL_FTM) bad("scheme must be MODAL_SV or MODAL_FTM");
+    if (d.geom != MODAL_STRING && d.geom != MODAL_RECT) bad("geom must be MODAL_STRING or MODAL_RECT");
+    if (d.bc != MODAL_BC_FIXED_SS) bad("bc must be MODAL_BC_FIXED_SS");
+    if (d.model == MODAL_VK && d.geom != MODAL_RECT) bad("MODAL_VK needs MODAL_RECT geometry");
+    if (!(d.Lx > 0)) bad("Lx must be positive");
+    if (d.geom == MODAL_RECT && !(d.Ly > 0)) bad("Ly must be positive");
+    if (d.geom == MODAL_RECT && !(d.h > 0)) bad("h must be positive");
+    if (!(d.rho > 0)) bad("rho must be positive");
+    if (!(d.E >= 0)) bad("E must be non-negative");
+    if (d.geom == MODAL_RECT && !(d.nu > -1.0 && d.nu < 0.5 + 1e-12)) bad("nu must lie in (-1, 0.5]");
+    if (!(d.T0 >= 0)) bad("T0 must be non-negative");
+    if (d.geom == MODAL_STRING && !(d.T0 > 0) && !(d.D > 0)) bad("degenerate dispersion: T0 and D both zero");
+    if (!(d.sigma0 >= 0) || !(d.sigma1 >= 0)) bad("sigma0 and sigma1 must be non-negative");
+    if (d.n_q < 1) bad("n_q must be at least 1");
+    if (d.model == MODAL_VK && d.n_phi < 1) bad("MODAL_VK needs n_phi >= 1");
+    if (d.model != MODAL_VK && d.n_phi != 0) bad("n_phi must be 0 unless MODAL_VK");
+    if (!(d.sample_rate > 0)) bad("sample_rate must be positive");
+    if (d.max_batch < 1) bad("max_batch must be at least 1");
+    if (d.max_steps < 1) bad("max_steps must be at least 1");
+    if (d.geom == MODAL_RECT) {
+        if (!(d.pickup_x >= 0 && d.pickup_x <= d.Lx) || !(d.pickup_y >= 0 && d.pickup_y <= d.Ly))
+            bad("pickup point must lie on the plate");
+    } else if (!(d.pickup_x >= 0 && d.pickup_x <= d.Lx)) bad("pickup point must lie on the string");
+    return err.empty();
+}
+
+double mode_value(const modal_plan *p, int k, double Lx, double Ly, double x, double y)
+{
+    if (p->d.geom == MODAL_STRING) return std::sqrt(2.0 / Lx) * std::sin(p->mq.m[k] * mh::PI * x / Lx);
+    return 2.0 / std::sqrt(Lx * Ly) * std::sin(p->mq.m[k] * mh::PI * x / Lx) * std::sin(p->mq.n[k] * mh::PI * y / Ly);
+}
+
+// Fill one row of per-sample coefficients for a geometry (plan index sets).
+void derive_row(const modal_plan *p, const modal_sample_geom &g, double *omega, double *sigma,
+                double *nl_scale, double *lambda, double *pickup)
+{
+    const modal_plan_desc &d = p->d;
+    const int nq = d.n_q;
+    std::vector<double> lam(nq);
+    if (d.geom == MODAL_RECT) {
+        for (int k = 0; k < nq; ++k) lam[k] = mh::rect_lambda(p->mq.m[k], p->mq.n[k], g.Lx, g.Ly);
+        const double D = (d.D > 0 && g.h == d.h) ? d.D : mh::plate_D(d.E, g.h, d.nu);
+        mh::omega_sigma(lam, D, d.T0, d.rho * g.h, d.sigma0, d.sigma1, omega, sigma);   // reading R3: rho h
+        if (d.model == MODAL_VK && nl_scale) {
+            const double cb = std::pow(g.Lx * g.Ly, -2.5), cref = std::pow(d.Lx * d.Ly, -2.5);
+            for (int n = 0; n < d.n_phi; ++n) {
+                const double z = mh::rect_lambda(p->mphi.m[n], p->mphi.n[n], g.Lx, g.Ly);   // zeta^4 = lambda^2 (R5)
+                nl_scale[n] = d.E / (2.0 * d.rho * z * z) * (cb / cref) * (cb / cref);       // reading R14
+            }
+        } else if (d.model == MODAL_TENSION && nl_scale) {
+            nl_scale[0] = d.E * g.h / (2.0 * g.Lx * g.Ly * (1.0 - d.nu * d.nu)) / (d.rho * g.h);   // Berger, Eq. 4
+        } else if (nl_scale) nl_scale[0] = 0.0;
+        if (pickup)
+            for (int k = 0; k < nq; ++k)
+                pickup[k] = mode_value(p, k, g.Lx, g.Ly, g.pickup_x_frac * g.Lx, g.pickup_y_frac * g.Ly);
+    } else {
+        for (int k = 0; k < nq; ++k) lam[k] = (p->mq.m[k] * mh::PI / g.Lx) * (p->mq.m[k] * mh::PI / g.Lx);
+        mh::omega_sigma(lam, g.D, g.T0, g.rho, d.sigma0, d.sigma1, omega, sigma);
+        if (nl_scale) nl_scale[0] = d.model == MODAL_TENSION ? d.E * g.area / (2.0 * g.Lx) / g.rho : 0.0;   // Eq. 4
+        if (pickup)
+            for (int k = 0; k < nq; ++k) pickup[k] = mode_value(p, k, g.Lx, 0, g.pickup_x_frac * g.Lx, 0);
+    }
+    if (lambda) for (int k = 0; k < nq; ++k) lambda[k] = lam[k];
+}
+
+modal_sample_geom fill_geom(const modal_plan *p, const modal_sample_geom *in)
+{
+    const modal_plan_desc &d = p->d;
+    modal_sample_geom g{};
+    auto pick = [](double v, double def) { return (v > 0) ? v : def; };
+    g.Lx = pick(in ? in->Lx : 0, d.Lx); g.Ly = pick(in ? in->Ly : 0, d.Ly); g.h = pick(in ? in->h : 0, d.h);
+    g.T0 = pick(in ? in->T0 : 0, d.T0); g.D = pick(in ? in->D : 0, d.D); g.rho = pick(in ? in->rho : 0, d.rho);
+    g.area = pick(in ? in->area : 0, d.area);
+    g.pickup_x_frac = (in && in->pickup_x_frac > 0) ? in->pickup_x_frac : d.pickup_x / d.Lx;
+    g.pickup_y_frac = (in && in->pickup_y_frac > 0) ? in->pickup_y_frac
+                                                    : (d.geom == MODAL_RECT ? d.pickup_y / d.Ly : 0.0);
+    return g;
+}
+
+// Recompute masks and delta-form coefficients from (omega, sigma, ...) and upload them.
+modal_status sync_coeffs(modal_plan *p)
+{
+    const modal_plan_desc &d = p->d;
+    const int cb = p->coeff_batch, nq = d.n_q, P = p->NQP, nnl = n_nl(p);
+    p->active.assign((size_t)cb * nq, 0);
+    std::vector<double> kv((size_t)cb * P, 0.0), kq(kv), r(kv), ast(kv);
+    std::vector<float> w((size_t)cb * P, 0.f), lam((size_t)cb * P, 0.f), s((size_t)cb * nnl, 0.f);
+    int masked = 0;
+    for (int b = 0; b < cb; ++b)
+        for (int k = 0; k < nq; ++k) {
+            const double om = p->omega[(size_t)b * nq + k], sg = p->sigma[(size_t)b * nq + k];
+            const bool act = mh::mode_active(d.scheme, om, sg, p->T) && std::isfinite(om) && std::isfinite(sg);
+            p->active[(size_t)b * nq + k] = act;
+            if (!act) { ++masked; continue; }
+            const mh::StepCoeffs c = mh::step_coeffs(d.scheme, om, sg, p->T);
+            const size_t o = (size_t)b * P + k;
+            kv[o] = c.kv; kq[o] = c.kq; r[o] = c.r; ast[o] = c.astart;
+            w[o] = (float)p->pickup[(size_t)b * nq + k];
+            if (d.model != MODAL_VK) lam[o] = (float)p->lambda_s[(size_t)b * nq + k];
+        }
+    for (size_t i = 0; i < s.size(); ++i) s[i] = (float)p->nl_scale[i];
+    if (masked) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "warning: %d mode-rows masked (beyond the stability limit of the scheme, reading R11)\n", masked);
+        p->err += buf;
+    }
+    if (p->device < 0) { p->coeffs_dirty = false; return MODAL_OK; }
+    CU(cudaSetDevice(p->device));
+    auto up = [&](DevBuf &b, const void *src, size_t bytes) -> cudaError_t {
+        cudaError_t e = b.ensure(bytes);
+        if (e != cudaSuccess) return e;
+        return cudaMemcpy(b.p, src, bytes, cudaMemcpyHostToDevice);
+    };
+    CU(up(p->dkv, kv.data(), kv.size() * 8)); CU(up(p->dkq, kq.data(), kq.size() * 8));
+    CU(up(p->dr, r.data(), r.size() * 8));    CU(up(p->dast, ast.data(), ast.size() * 8));
+    CU(up(p->dw, w.data(), w.size() * 4));
+    if (d.model == MODAL_VK) CU(up(p->ds, s.data(), s.size() * 4));
+    else { CU(up(p->dlam, lam.data(), lam.size() * 4)); CU(up(p->dc, s.data(), s.size() * 4)); }
+    p->coeffs_dirty = false;
+    return MODAL_OK;
+}
+
+modal_status sync_H(modal_plan *p)
+{
+    if (p->device >= 0 && p->d.model == MODAL_VK) {
+        CU(cudaSetDevice(p->device));
+        CU(p->dHt.ensure(p->Ht.size() * 4));
+        CU(cudaMemcpy(p->dHt.p, p->Ht.data(), p->Ht.size() * 4, cudaMemcpyHostToDevice));
+    }
+    p->H_dirty = false;
+    return MODAL_OK;
+}
+
+int env_int(const char *name, int def)
+{
+    const char *s = getenv(name);
+    return (s && *s) ? atoi(s) : def;
+}
+
+template <bool R>
+cudaError_t launch_vk(const md::VkArgs &a, int n_clusters, int CS, int threads, size_t smem, cudaStream_t st)
+{
+    auto kern = md::vk_team_kernel<R>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    if (CS > 8) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(n_clusters * CS); cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+template <bool R>
+int max_active_clusters(int CS, int threads, size_t smem)
+{
+    auto kern = md::vk_team_kernel<R>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (CS > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return 0;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(CS); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return n;
+}
+
+size_t vk_smem_bytes(const mh::Schedule &s, int NQP, int grid_team, int resident)
+{
+    size_t f = md::vk_smem_floats(NQP, s.NLOC_MAX, s.CS, grid_team, s.max_cta_units, s.max_tp);
+    size_t bytes = f * 4;
+    if (resident) bytes += (size_t)s.max_cta_tiles * md::TILE_ELEMS * 4;
+    return bytes + 16;
+}
+
+// Choose team shape and residency for this batch.
+modal_status configure_vk(modal_plan *p, int batch, VkConfig **out)
+{
+    const int nq = p->d.n_q, nphi = p->d.n_phi, P = p->NQP;
+    const int NW = env_int("MODAL_VK_NW", 16);
+    if (P > NW * 32) { p->err += "n_q too large for the vK kernel of this build (padded n_q <= 512)\n"; return MODAL_EINCOMPAT; }
+    const int force_cs = env_int("MODAL_VK_CS", 0);
+    const char *mode = getenv("MODAL_VK_MODE");   // "resident" | "cluster" | "grid"
+    const int tiles_total = nphi * mh::tiles_per_n(nq);
+    int CS = 0, grid_team = 0, resident = 0, NCL = 1;
+    mh::Schedule sch;
+    // 1. resident in one cluster's shared memory?
+    if (!mode || !strcmp(mode, "resident")) {
+        for (int cs : {1, 2, 4, 8, 16}) {
+            if (force_cs && cs != force_cs) continue;
+            mh::Schedule s = mh::build_schedule(nq, nphi, cs, 1, NW);
+            if (vk_smem_bytes(s, P, 0, 1) > SMEM_LIMIT) continue;
+            if (max_active_clusters<true>(cs, NW * 32, vk_smem_bytes(s, P, 0, 1)) < 1) continue;
+            // widen small-batch runs while every warp still has >= 2 tiles of work
+            const bool widen = !force_cs && cs < 16 && (long long)batch * cs * 2 <= p->sm_count &&
+                               tiles_total / (cs * 2 * NW) >= 2;
+            CS = cs; resident = 1; sch = s;
+            if (!widen) break;
+        }
+    }
+    if (!CS) {
+        const bool want_grid = mode ? !strcmp(mode, "grid") : batch <= 4;
+        CS = force_cs ? force_cs : 8;
+        grid_team = want_grid;
+        NCL = grid_team ? p->sm_count / CS : 1;
+        sch = mh::build_schedule(nq, nphi, CS, NCL, NW);
+    }
+    const long long key = ((long long)CS << 40) | ((long long)NCL << 20) | (grid_team << 1) | resident;
+    VkConfig &c = p->vk_cfgs[key];
+    if (!c.uploaded) {
+        c.CS = CS; c.NCL = NCL; c.NW = NW; c.grid_team = grid_team; c.resident = resident;
+        c.sched = sch;
+        c.smem = vk_smem_bytes(sch, P, grid_team, resident);
+        if (c.smem > SMEM_LIMIT) { p->err += "vK schedule does not fit shared memory\n"; return MODAL_EINCOMPAT; }
+        auto up = [&](DevBuf &b, const void *src, size_t bytes) -> cudaError_t {
+            cudaError_t e = b.ensure(bytes);
+            return e != cudaSuccess ? e : cudaMemcpy(b.p, src, bytes, cudaMemcpyHostToDevice);
+        };
+        CU(up(c.units, sch.units.data(), sch.units.size() * sizeof(mh::Unit)));
+        CU(up(c.warp_ptr, sch.warp_ptr.data(), sch.warp_ptr.size() * 4));
+        CU(up(c.cta_ptr, sch.cta_ptr.data(), sch.cta_ptr.size() * 4));
+        CU(up(c.nlo, sch.nlo.data(), sch.nlo.size() * 4));
+        c.uploaded = true;
+    }
+    if (grid_team) {
+        const int cap = resident ? max_active_clusters<true>(CS, NW * 32, c.smem)
+                                 : max_active_clusters<false>(CS, NW * 32, c.smem);
+        if (cap < NCL) {
+            char buf[128];
+            snprintf(buf, sizeof buf, "grid team of %d clusters of %d is not co-resident (capacity %d)\n", NCL, CS, cap);
+            p->err += buf;
+            return MODAL_EINCOMPAT;
+        }
+        c.n_clusters = NCL;
+    } else {
+        c.n_clusters = batch;
+    }
+    *out = &c;
+    return MODAL_OK;
+}
+
+template <int MPL>
+cudaError_t launch_tension(const md::TensionArgs &a, cudaStream_t st)
+{
+    const int warps_per_block = 4;
+    const int blocks = (a.batch + warps_per_block - 1) / warps_per_block;
+    md::tension_kernel<MPL><<<blocks, warps_per_block * 32, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, float *out_dev,
+                 int *first_bad, cudaStream_t st)
+{
+    const modal_plan_desc &d = p->d;
+    const int nq = d.n_q, P = p->NQP, cb = p->coeff_batch;
+    if (p->coeffs_dirty) { modal_status s = sync_coeffs(p); if (s != MODAL_OK) return s; }
+    if (p->H_dirty) { modal_status s = sync_H(p); if (s != MODAL_OK) return s; }
+    CU(cudaSetDevice(p->device));
+    // initial state, masked and padded:  v^0 = q^0 - q^-1
+    std::vector<double> q0((size_t)batch * P, 0.0), v0((size_t)batch * P, 0.0), gain;
+    for (int b = 0; b < batch; ++b)
+        for (int k = 0; k < nq; ++k) {
+            if (!p->active[(size_t)(cb == 1 ? 0 : b) * nq + k]) continue;
+            const double q = init->q0[(size_t)b * nq + k];
+            q0[(size_t)b * P + k] = q;
+            if (init->qm1) v0[(size_t)b * P + k] = q - init->qm1[(size_t)b * nq + k];
+        }
+    CU(p->dq0.ensure(q0.size() * 8)); CU(p->dv0.ensure(v0.size() * 8)); CU(p->dbad.ensure((size_t)batch * 4));
+    CU(cudaMemcpyAsync(p->dq0.p, q0.data(), q0.size() * 8, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(p->dv0.p, v0.data(), v0.size() * 8, cudaMemcpyHostToDevice, st));
+    if (init->fext_signal) {
+        gain.assign((size_t)batch * P, 0.0);
+        for (int b = 0; b < batch; ++b)
+            for (int k = 0; k < nq; ++k)
+                if (p->active[(size_t)(cb == 1 ? 0 : b) * nq + k]) gain[(size_t)b * P + k] = init->fext_gain[(size_t)b * nq + k];
+        CU(p->dgain.ensure(gain.size() * 8));
+        CU(cudaMemcpyAsync(p->dgain.p, gain.data(), gain.size() * 8, cudaMemcpyHostToDevice, st));
+    }
+    CU(cudaMemsetAsync(p->dbad.p, 0xff, (size_t)batch * 4, st));
+    const int auto_start = init->qm1 ? 0 : 1;
+    const double half_T2 = 0.5 * p->T * p->T;
+
+    if (d.model != MODAL_VK) {
+        md::TensionArgs a{};
+        a.batch = batch; a.n_steps = n_steps; a.n_modes_pad = P; a.coeff_stride = cb == 1 ? 0 : P;
+        a.kv = p->dkv.as<double>(); a.kq = p->dkq.as<double>(); a.r = p->dr.as<double>(); a.astart = p->dast.as<double>();
+        a.lambda = p->dlam.as<float>(); a.w = p->dw.as<float>(); a.c = p->dc.as<float>();
+        a.q0 = p->dq0.as<double>(); a.v0 = p->dv0.as<double>();
+        a.auto_start = auto_start; a.half_T2 = half_T2;
+        a.fext = init->fext_signal; a.gain = p->dgain.as<double>();
+        a.out = out_dev; a.traj = init->traj_dev; a.n_q = nq; a.first_bad = p->dbad.as<int>();
+        cudaError_t e;
+        switch (P / 32) {
+            case 1: e = launch_tension<1>(a, st); break;
+            case 2: e = launch_tension<2>(a, st); break;
+            case 3: e = launch_tension<3>(a, st); break;
+            case 4: e = launch_tension<4>(a, st); break;
+            case 5: e = launch_tension<5>(a, st); break;
+            case 6: e = launch_tension<6>(a, st); break;
+            case 7: e = launch_tension<7>(a, st); break;
+            case 8: e = launch_tension<8>(a, st); break;
+            case 12: e = launch_tension<12>(a, st); break;
+            case 16: e = launch_tension<16>(a, st); break;
+            default: p->err += "n_q not supported by the tension kernel (n_q <= 256, 353..384 or 481..512)\n"; return MODAL_EINCOMPAT;
+        }
+        CU(e);
+        p->kinfo[0] = 1; p->kinfo[1] = 1; p->kinfo[2] = (batch + 3) / 4; p->kinfo[3] = 128;
+        p->kinfo[4] = 0; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
+    } else {
+        VkConfig *c = nullptr;
+        modal_status s = configure_vk(p, batch, &c);
+        if (s != MODAL_OK) return s;
+        md::VkArgs a{};
+        a.Ht = p->dHt.as<float>(); a.units = c->units.as<md::VkUnit>();
+        a.warp_ptr = c->warp_ptr.as<int2>(); a.cta_ptr = c->cta_ptr.as<int2>(); a.nlo = c->nlo.as<int>();
+        a.NQP = P; a.n_q = nq; a.n_phi = d.n_phi; a.tiles_per_n = mh::tiles_per_n(nq);
+        a.NLOC_MAX = c->sched.NLOC_MAX; a.CS = c->CS; a.NCL = c->NCL; a.grid_team = c->grid_team; a.resident = c->resident;
+        a.max_cta_units = c->sched.max_cta_units; a.max_tp = c->sched.max_tp; a.max_cta_tiles = c->sched.max_cta_tiles;
+        a.batch = batch; a.n_steps = n_steps;
+        a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
+        a.kv = p->dkv.as<double>(); a.kq = p->dkq.as<double>(); a.r = p->dr.as<double>(); a.astart = p->dast.as<double>();
+        a.s = p->ds.as<float>(); a.w = p->dw.as<float>();
+        a.q0 = p->dq0.as<double>(); a.v0 = p->dv0.as<double>();
+        a.auto_start = auto_start; a.half_T2 = half_T2;
+        a.fext = init->fext_signal; a.gain = p->dgain.as<double>();
+        a.out = out_dev; a.traj = init->traj_dev; a.first_bad = p->dbad.as<int>();
+        if (c->grid_team) {
+            CU(p->dfbuf.ensure((size_t)2 * c->NCL * P * 4));
+            CU(p->dcounter.ensure(64));
+            CU(cudaMemsetAsync(p->dcounter.p, 0, 64, st));
+            a.fbuf = p->dfbuf.as<float>(); a.counter = p->dcounter.as<unsigned>();
+        }
+        const int threads = c->NW * 32;
+        cudaError_t e = c->resident ? launch_vk<true>(a, c->n_clusters, c->CS, threads, c->smem, st)
+                                    : launch_vk<false>(a, c->n_clusters, c->CS, threads, c->smem, st);
+        CU(e);
+        p->kinfo[0] = 2; p->kinfo[1] = c->CS; p->kinfo[2] = c->n_clusters; p->kinfo[3] = threads;
+        p->kinfo[4] = (int)c->smem; p->kinfo[5] = c->resident | (c->grid_team << 1); p->kinfo[6] = a.tiles_per_n; p->kinfo[7] = P;
+    }
+    if (first_bad) {
+        CU(cudaMemcpyAsync(first_bad, p->dbad.p, (size_t)batch * 4, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        for (int b = 0; b < batch; ++b)
+            if (first_bad[b] >= 0) {
+                char buf[96];
+                snprintf(buf, sizeof buf, "sample %d went non-finite at step %d\n", b, first_bad[b]);
+                p->err += buf;
+                return MODAL_EUNSTABLE;
+            }
+    }
+    return MODAL_OK;
+}
+
+modal_status check_sim_args(modal_plan *p, int batch, int n_steps, const modal_init *init, const void *out)
+{
+    if (!p) return MODAL_EINVAL;
+    p->err.clear();
+    if (p->device < 0) { p->err = "plan has no CUDA device (host-only plan): there is no CPU fallback\n"; return MODAL_ECUDA; }
+    if (batch < 1 || batch > p->d.max_batch) p->err += "batch outside [1, max_batch]\n";
+    if (n_steps < 1 || n_steps > p->d.max_steps) p->err += "n_steps outside [1, max_steps]\n";
+    if (!init || !init->q0) p->err += "init->q0 is required\n";
+    if (init && init->fext_signal && !init->fext_gain) p->err += "fext_signal needs fext_gain\n";
+    if (!out) p->err += "output buffer is NULL\n";
+    if (p->coeff_batch != 1 && p->coeff_batch != batch) p->err += "coeff_batch must be 1 or equal to batch\n";
+    return p->err.empty() ? MODAL_OK : MODAL_EINVAL;
+}
+
+}  // namespace
+
+// ============================================================================ C ABI ====
+
+extern "C" modal_status modal_plan_create(const modal_plan_desc *desc, int cuda_device, modal_plan **out)
+{
+    if (out) *out = nullptr;
+    g_create_error.clear();
+    if (!desc || !out) { g_create_error = "desc and out must not be NULL\n"; return MODAL_EINVAL; }
+    if (!validate_desc(*desc, g_create_error)) return MODAL_EINVAL;
+    modal_plan *p = new (std::nothrow) modal_plan;
+    if (!p) return MODAL_ENOMEM;
+    p->d = *desc; p->device = cuda_device; p->T = 1.0 / desc->sample_rate;
+    const modal_plan_desc &d = p->d;
+    const int nq = d.n_q;
+    if (d.geom == MODAL_RECT) {
+        p->mq = mh::rect_modes(d.Lx, d.Ly, nq);
+        if (d.model == MODAL_VK) p->mphi = mh::rect_modes(d.Lx, d.Ly, d.n_phi);   // reading R5
+    } else p->mq = mh::string_modes(d.Lx, nq);
+    p->NQP = d.model == MODAL_VK ? mh::padded_nq(nq) : ((nq + 31) / 32) * 32;
+    p->coeff_batch = 1;
+    p->omega.resize(nq); p->sigma.resize(nq); p->pickup.resize(nq); p->lambda_s.resize(nq);
+    p->nl_scale.resize(n_nl(p));
+    modal_sample_geom g = fill_geom(p, nullptr);
+    derive_row(p, g, p->omega.data(), p->sigma.data(), p->nl_scale.data(), p->lambda_s.data(), p->pickup.data());
+    if (d.model == MODAL_VK) {
+        const double geom = mh::H_geom(d.Lx, d.Ly);
+        const mh::ModeSet &q = p->mq, &f = p->mphi;
+        mh::pack_tiles(nq, d.n_phi, [&](int n, int a, int b) {
+            return geom * mh::H_bracket(q.m[a], q.n[a], q.m[b], q.n[b], f.m[n], f.n[n]);
+        }, p->Ht);
+    }
+    if (cuda_device >= 0) {
+        cudaError_t e = cudaSetDevice(cuda_device);
+        cudaDeviceProp prop{};
+        if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, cuda_device);
+        if (e != cudaSuccess) {
+            g_create_error = std::string("CUDA error: ") + cudaGetErrorString(e) + "\n";
+            delete p;
+            return MODAL_ECUDA;
+        }
+        if (prop.major != 10) {
+            g_create_error = "this library is built for sm_100a (B200) only\n";
+            delete p;
+            return MODAL_ECUDA;
+        }
+        p->sm_count = prop.multiProcessorCount;
+    }
+    modal_status s = sync_coeffs(p);
+    if (s == MODAL_OK) s = sync_H(p);
+    if (s != MODAL_OK) { g_create_error = p->err; modal_plan_destroy(p); return s; }
+    *out = p;
+    return MODAL_OK;
+}
+
+extern "C" modal_status modal_coeffs_upload(modal_plan *p, const modal_coeffs *c)
+{
+    if (!p || !c) return MODAL_EINVAL;
+    p->err.clear();
+    const modal_plan_desc &d = p->d;
+    const int nq = d.n_q, nnl = n_nl(p), cb = c->coeff_batch;
+    if (cb < 1 || cb > d.max_batch) { p->err = "coeff_batch outside [1, max_batch]\n"; return MODAL_EINVAL; }
+    if (c->H_full && d.model != MODAL_VK) { p->err = "H_full given but the plan is not MODAL_VK\n"; return MODAL_EINVAL; }
+    if (c->lambda && d.model == MODAL_VK) { p->err = "lambda is a MODAL_TENSION / MODAL_LINEAR coefficient\n"; return MODAL_EINVAL; }
+    auto finite = [&](const double *a, size_t n, const char *name) {
+        for (size_t i = 0; a && i < n; ++i)
+            if (!std::isfinite(a[i])) { p->err += std::string(name) + " contains non-finite values\n"; return; }
+    };
+    finite(c->omega, (size_t)cb * nq, "omega"); finite(c->sigma, (size_t)cb * nq, "sigma");
+    finite(c->nl_scale, (size_t)cb * nnl, "nl_scale"); finite(c->lambda, (size_t)cb * nq, "lambda");
+    finite(c->pickup, (size_t)cb * nq, "pickup"); finite(c->H_full, c->H_full ? (size_t)d.n_phi * nq * nq : 0, "H_full");
+    for (size_t i = 0; c->omega && i < (size_t)cb * nq; ++i) if (c->omega[i] < 0) { p->err += "omega must be non-negative\n"; break; }
+    for (size_t i = 0; c->sigma && i < (size_t)cb * nq; ++i) if (c->sigma[i] < 0) { p->err += "sigma must be non-negative\n"; break; }
+    if (c->H_full) {
+        double mx = 0, asym = 0;
+        for (size_t i = 0; i < (size_t)d.n_phi * nq * nq; ++i) mx = std::max(mx, std::fabs(c->H_full[i]));
+        for (int n = 0; n < d.n_phi; ++n)
+            for (int a = 0; a < nq; ++a)
+                for (int b = 0; b < a; ++b)
+                    asym = std::max(asym, std::fabs(c->H_full[((size_t)n * nq + a) * nq + b] - c->H_full[((size_t)n * nq + b) * nq + a]));
+        if (asym > 1e-12 * mx) p->err += "H_full is not symmetric in its two transverse indices\n";
+    }
+    if (!p->err.empty()) return MODAL_EINVAL;
+    // re-shape the per-sample arrays to the new coeff_batch (row 0 broadcast when it changes)
+    auto reshape = [&](std::vector<double> &v, int width, const double *src) {
+        if (src) { v.assign(src, src + (size_t)cb * width); return; }
+        if (cb == p->coeff_batch) return;
+        std::vector<double> row(v.begin(), v.begin() + width), nv((size_t)cb * width);
+        for (int b = 0; b < cb; ++b) std::copy(row.begin(), row.end(), nv.begin() + (size_t)b * width);
+        v.swap(nv);
+    };
+    reshape(p->omega, nq, c->omega); reshape(p->sigma, nq, c->sigma); reshape(p->nl_scale, nnl, c->nl_scale);
+    reshape(p->lambda_s, nq, c->lambda); reshape(p->pickup, nq, c->pickup);
+    p->coeff_batch = cb;
+    p->coeffs_dirty = true;
+    if (c->H_full) {
+        const double *H = c->H_full;
+        mh::pack_tiles(nq, d.n_phi, [&](int n, int a, int b) { return H[((size_t)n * nq + a) * nq + b]; }, p->Ht);
+        p->H_dirty = true;
+    }
+    modal_status s = sync_coeffs(p);
+    if (s == MODAL_OK && p->H_dirty) s = sync_H(p);
+    return s;
+}
+
+extern "C" modal_status modal_simulate(modal_plan *p, int batch, int n_steps, const modal_init *init,
+                                       float *out_audio_dev, int *first_bad_step, void *cuda_stream)
+{
+    modal_status s = check_sim_args(p, batch, n_steps, init, out_audio_dev);
+    if (s != MODAL_OK) return s;
+    return run(p, batch, n_steps, init, out_audio_dev, first_bad_step, (cudaStream_t)cuda_stream);
+}
+
+extern "C" modal_status modal_simulate_host(modal_plan *p, int batch, int n_steps, const modal_init *init,
+                                            float *out_audio_host, int *first_bad_step)
+{
+    modal_status s = check_sim_args(p, batch, n_steps, init, out_audio_host);
+    if (s != MODAL_OK) return s;
+    const size_t bytes = (size_t)batch * n_steps * 4;
+    CU(cudaSetDevice(p->device));
+    CU(p->dout.ensure(bytes));
+    std::vector<int> bad(batch, -1);
+    s = run(p, batch, n_steps, init, p->dout.as<float>(), bad.data(), nullptr);
+    if (s != MODAL_OK && s != MODAL_EUNSTABLE) return s;
+    CU(cudaMemcpy(out_audio_host, p->dout.p, bytes, cudaMemcpyDeviceToHost));
+    if (first_bad_step) memcpy(first_bad_step, bad.data(), (size_t)batch * 4);
+    return s;
+}
+
+extern "C" void modal_plan_destroy(modal_plan *p)
+{
+    if (!p) return;
+    if (p->device >= 0) {
+        cudaSetDevice(p->device);
+        for (DevBuf *b : {&p->dHt, &p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dw, &p->dlam, &p->dc, &p->dq0,
+                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter}) b->release();
+        for (auto &kv : p->vk_cfgs) { kv.second.units.release(); kv.second.warp_ptr.release(); kv.second.cta_ptr.release(); kv.second.nlo.release(); }
+    }
+    delete p;
+}
+
+extern "C" const char *modal_last_error(const modal_plan *p) { return p ? p->err.c_str() : g_create_error.c_str(); }
+
+extern "C" modal_status modal_plan_query(const modal_plan *p, int what, void *dst, unsigned long long cap)
+{
+    if (!p || !dst) return MODAL_EINVAL;
+    const modal_plan_desc &d = p->d;
+    const int nq = d.n_q, cb = p->coeff_batch;
+    auto put = [&](const void *src, size_t bytes) { if (bytes > cap) return MODAL_EINVAL; memcpy(dst, src, bytes); return MODAL_OK; };
+    switch (what) {
+        case MODAL_Q_MODE_M: return put(p->mq.m.data(), (size_t)nq * 4);
+        case MODAL_Q_MODE_N: return put(p->mq.n.data(), (size_t)nq * 4);
+        case MODAL_Q_PHI_M: return put(p->mphi.m.data(), p->mphi.m.size() * 4);
+        case MODAL_Q_PHI_N: return put(p->mphi.n.data(), p->mphi.n.size() * 4);
+        case MODAL_Q_LAMBDA: return put(p->mq.lambda.data(), (size_t)nq * 8);
+        case MODAL_Q_OMEGA: return put(p->omega.data(), p->omega.size() * 8);
+        case MODAL_Q_SIGMA: return put(p->sigma.data(), p->sigma.size() * 8);
+        case MODAL_Q_NL_SCALE: return put(p->nl_scale.data(), p->nl_scale.size() * 8);
+        case MODAL_Q_PICKUP: return put(p->pickup.data(), p->pickup.size() * 8);
+        case MODAL_Q_ACTIVE: return put(p->active.data(), p->active.size() * 4);
+        case MODAL_Q_COEFF_BATCH: return put(&cb, 4);
+        case MODAL_Q_KERNEL_INFO: return put(p->kinfo, sizeof p->kinfo);
+        case MODAL_Q_H_FULL: {
+            if (d.model != MODAL_VK) return MODAL_EINVAL;
+            const size_t bytes = (size_t)d.n_phi * nq * nq * 8;
+            if (bytes > cap) return MODAL_EINVAL;
+            mh::unpack_tiles(nq, d.n_phi, p->Ht, reinterpret_cast<double *>(dst));
+            return MODAL_OK;
+        }
+        default: return MODAL_EINVAL;
+    }
+}
+
+extern "C" modal_status modal_derive_coeffs(const modal_plan *p, const modal_sample_geom *geom, double *omega,
+                                            double *sigma, double *nl_scale, double *lambda, double *pickup)
+{
+    if (!p || !omega || !sigma) return MODAL_EINVAL;
+    modal_sample_geom g = fill_geom(p, geom);
+    derive_row(p, g, omega, sigma, nl_scale, lambda, pickup);
+    return MODAL_OK;
+}
+
+extern "C" modal_status modal_project_bump(const modal_plan *p, double Lx, double Ly, double x0, double y0,
+                                           double W, double A, double *q0)
+{
+    if (!p || !q0 || !(Lx > 0) || !(W > 0)) return MODAL_EINVAL;
+    if (p->d.geom == MODAL_RECT) {
+        if (!(Ly > 0)) return MODAL_EINVAL;
+        mh::project_bump_rect(p->mq, Lx, Ly, x0, y0, W, A, q0);
+    } else mh::project_bump_string(p->d.n_q, Lx, x0, W, A, q0);
+    return MODAL_OK;
+}

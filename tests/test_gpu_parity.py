@@ -1,0 +1,268 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's: pickup max error <= 1e-4 of the
+signal peak over the first 4096 samples; relative L2 <= 1e-3 over the full run in the weakly
+non-linear regime (V_nl(q0)/V_lin(q0) <= 0.05, R15); lossless energy drift <= 1e-5."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2505_05940_b200 import workloads as wlmod
+
+pytestmark = pytest.mark.gpu
+
+TOL_MAX, TOL_L2, TOL_E = 1e-4, 1e-3, 1e-5
+
+
+def _mods():
+    import torch
+    from paper_2505_05940_b200 import binding as mb
+    return torch, mb
+
+
+def gpu_run(plan, q0, qm1, n_steps, want_traj=False, fext=None, fext_gain=None):
+    torch, mb = _mods()
+    B = np.atleast_2d(q0).shape[0]
+    out = torch.empty((B, n_steps), dtype=torch.float32, device="cuda")
+    traj = torch.zeros((B, n_steps, plan.n_q), dtype=torch.float64, device="cuda") if want_traj else None
+    fdev = None if fext is None else torch.tensor(fext, dtype=torch.float32, device="cuda").contiguous()
+    st, fb = plan.simulate(q0, n_steps, out.data_ptr(), qm1=qm1,
+                           stream=torch.cuda.current_stream().cuda_stream,
+                           fext_dev_ptr=0 if fdev is None else fdev.data_ptr(), fext_gain=fext_gain,
+                           traj_dev_ptr=0 if traj is None else traj.data_ptr())
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64), fb, (None if traj is None else traj.cpu().numpy()), st
+
+
+def plan_with_oracle_inputs(wl, case, scheme=0, lossless=False):
+    """Plan whose coefficient arrays are the oracle's (fp32-rounded where the device stores fp32),
+    so that the comparison measures arithmetic, not input quantisation."""
+    torch, mb = _mods()
+    plan = mb.Plan(mb.desc_from_workload(wl, scheme=scheme, lossless=lossless), 0)
+    B = case.q0.shape[0]
+    # pickup: the oracle's w is already masked; the library masks again (same rule)
+    if case.model == orc.VK:
+        plan.coeffs_upload(B, omega=case.omega, sigma=case.gamma, nl_scale=case.nl_scale, pickup=case.w, H_full=case.H)
+    else:
+        plan.coeffs_upload(B, omega=case.omega, sigma=case.gamma, nl_scale=case.nl_scale, lam=case.lam, pickup=case.w)
+    assert np.array_equal(plan.query(mb.Q_ACTIVE).astype(bool), case.active)
+    return plan
+
+
+def nl_ratio(case, b):
+    vlin = 0.5 * np.sum(case.omega[b] ** 2 * case.q0[b] ** 2)
+    if case.model == orc.VK:
+        v = orc.potential_nl(orc.VK, None, case.nl_scale[b], case.H, case.q0[b])
+    elif case.model == orc.TENSION:
+        v = orc.potential_nl(orc.TENSION, case.lam[b], case.nl_scale[b], None, case.q0[b])
+    else:
+        v = 0.0
+    return v / vlin
+
+
+def check_parity(gpu, ref, case, weak_only_l2=True, first=4096):
+    for b in range(ref.shape[0]):
+        peak = np.max(np.abs(ref[b]))
+        k = min(first, ref.shape[1])
+        weak = nl_ratio(case, b) <= 0.05
+        kk = k if weak else min(256, k)           # strongly non-linear: first 256 samples (R15)
+        e_max = np.max(np.abs(gpu[b, :kk] - ref[b, :kk])) / peak
+        assert e_max <= TOL_MAX, (b, e_max, weak)
+        if weak or not weak_only_l2:
+            e_l2 = np.linalg.norm(gpu[b] - ref[b]) / np.linalg.norm(ref[b])
+            assert e_l2 <= TOL_L2, (b, e_l2)
+        assert np.all(np.isfinite(gpu[b]))
+
+
+# ------------------------------------------------------------------ C0 -----------
+def test_c0_full_run_parity():
+    wl = wlmod.c0()
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, wl["n_steps"])
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, wl["n_steps"])
+    assert st == 0 and fb[0] == -1 and ref["first_bad"][0] == -1
+    assert nl_ratio(case, 0) <= 0.05
+    check_parity(gpu, ref["out"], case)
+    # determinism: bit-identical on a second run
+    gpu2, _, _, _ = gpu_run(plan, case.q0, case.qm1, wl["n_steps"])
+    assert np.array_equal(gpu, gpu2)
+
+
+def test_c0_plan_defaults_without_oracle_inputs():
+    """The library's own derivations (closed-form H, coefficients, projection, device-side start)."""
+    torch, mb = _mods()
+    wl = wlmod.c0()
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    gpu, fb, _, st = gpu_run(plan, q0, None, wl["n_steps"])
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, wl["n_steps"])["out"]
+    check_parity(gpu, ref, case)
+
+
+@pytest.mark.parametrize("amp", [0.5, 2.0])
+def test_c0_lossless_energy_drift(amp):
+    wl = wlmod.c0()
+    wl["A"] = np.array([amp * wl["h"][0]]); wl["W"] = np.array([0.3]); wl["x0"] = np.array([0.27]); wl["y0"] = np.array([0.17])
+    case = orc.assemble(wl, lossless=True)
+    n = wl["n_steps"]
+    ref = orc.run_case(case, n, want_traj=True)
+    plan = plan_with_oracle_inputs(wl, case, lossless=True)
+    gpu, fb, traj, _ = gpu_run(plan, case.q0, case.qm1, n, want_traj=True)
+    e_ref = orc.energy(orc.VK, case.T, case.omega[0], ref["traj"][0], nl_scale=case.nl_scale[0], H=case.H)
+    e_gpu = orc.energy(orc.VK, case.T, case.omega[0], traj[0], nl_scale=case.nl_scale[0], H=case.H)
+    k = len(e_ref) // 10
+    drift = abs(e_gpu[-k:].mean() - e_gpu[:k].mean()) / e_gpu.mean()
+    assert drift <= TOL_E, drift
+    if amp <= 0.5:                                   # weakly non-linear: trace tracks the oracle's (R12)
+        assert np.max(np.abs(e_gpu - e_ref)) / e_ref.mean() <= TOL_E
+
+
+def test_linear_lossless_energy_is_flat_on_gpu():
+    wl = wlmod.c0()
+    case = orc.assemble(wl, lossless=True)
+    case.H = np.zeros_like(case.H)
+    case.qm1 = orc.start_state(orc.LINEAR, case.q0[0], case.omega[0], case.T)[None]
+    plan = plan_with_oracle_inputs(wl, case, lossless=True)
+    _, _, traj, _ = gpu_run(plan, case.q0, case.qm1, 11025, want_traj=True)
+    e = orc.energy(orc.LINEAR, case.T, case.omega[0], traj[0])
+    assert (e.max() - e.min()) / e.mean() <= TOL_E
+
+
+# -------------------------------------------- team shapes: several tiles, ragged tails ----
+def _small_vk_workload(n_q, n_phi, batch, n_steps, seed=11):
+    wl = wlmod.c3(batch=batch, n_steps=n_steps)
+    wl["n_q"], wl["n_phi"] = n_q, n_phi
+    wl["A"] = np.minimum(wl["A"], 1.5 * wl["h"])
+    return wl
+
+
+@pytest.mark.parametrize("n_q,n_phi,batch,mode,cs", [
+    (37, 13, 3, None, 0),          # 3 tile rows, ragged (37 = 2*16 + 5), resident, auto cluster size
+    (37, 13, 3, "resident", 1),
+    (37, 13, 3, "resident", 4),
+    (37, 13, 3, "cluster", 2),     # streamed from L2, cluster team
+    (37, 13, 2, "grid", 8),        # streamed, whole-grid team with the L2 exchange + grid barrier
+    (100, 50, 2, None, 0),         # C2 shape
+    (16, 1, 1, None, 0),           # exactly one tile, one in-plane mode
+    (1, 1, 2, None, 0),            # degenerate: single mode (Duffing)
+])
+def test_vk_team_shapes_parity(n_q, n_phi, batch, mode, cs, monkeypatch):
+    if mode: monkeypatch.setenv("MODAL_VK_MODE", mode)
+    if cs: monkeypatch.setenv("MODAL_VK_CS", str(cs))
+    wl = _small_vk_workload(n_q, n_phi, batch, 1500)
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, 1500)
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, 1500)
+    assert st == 0 and np.all(fb == -1)
+    check_parity(gpu, ref["out"], case)
+    torch, mb = _mods()
+    info = plan.query(mb.Q_KERNEL_INFO)
+    if cs: assert info[1] == cs
+    if mode == "grid": assert info[5] & 2
+    if mode == "resident": assert info[5] & 1
+
+
+def test_vk_ftm_scheme_and_auto_start_parity():
+    wl = _small_vk_workload(37, 13, 2, 2000)
+    case = orc.assemble(wl, scheme=orc.FTM)
+    ref = orc.run_case(case, 2000)
+    plan = plan_with_oracle_inputs(wl, case, scheme=1)
+    gpu, fb, _, _ = gpu_run(plan, case.q0, None, 2000)       # qm1 = NULL: second-order start on the device
+    check_parity(gpu, ref["out"], case)
+
+
+def test_c4_shape_grid_team_short_run():
+    wl = wlmod.c4(batch=2, n_steps=96)
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, 96)
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, _ = gpu_run(plan, case.q0, case.qm1, 96)
+    torch, mb = _mods()
+    assert plan.query(mb.Q_KERNEL_INFO)[5] & 2               # grid team, streamed
+    check_parity(gpu, ref["out"], case, first=96)
+
+
+# ------------------------------------------------------------------ tension / linear ----
+@pytest.mark.parametrize("batch,n_steps", [(32, 4096), (5, 333)])
+def test_c1_string_parity(batch, n_steps):
+    wl = wlmod.c1(batch=batch, n_steps=n_steps)
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, n_steps)
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, n_steps)
+    assert st == 0
+    check_parity(gpu, ref["out"], case)
+
+
+def test_string_plan_defaults_and_lossless_energy():
+    torch, mb = _mods()
+    wl = wlmod.c1(batch=16, n_steps=8192)
+    wl["A"] = np.minimum(wl["A"], 1e-3)
+    case = orc.assemble(wl, lossless=True)
+    plan = plan_with_oracle_inputs(wl, case, lossless=True)
+    gpu, fb, traj, _ = gpu_run(plan, case.q0, case.qm1, 8192, want_traj=True)
+    ref = orc.run_case(case, 8192, want_traj=True)
+    for b in range(16):
+        kw = dict(lam=case.lam[b], nl_scale=case.nl_scale[b])
+        e_ref = orc.energy(orc.TENSION, case.T, case.omega[b], ref["traj"][b], **kw)
+        e_gpu = orc.energy(orc.TENSION, case.T, case.omega[b], traj[b], **kw)
+        assert np.max(np.abs(e_gpu - e_ref)) / e_ref.mean() <= TOL_E
+
+
+def test_linear_model_with_external_force():
+    torch, mb = _mods()
+    wl = wlmod.c1(batch=3, n_steps=3000)
+    wl["model"] = "linear"
+    case = orc.assemble(wl)
+    rng = np.random.default_rng(2)
+    fext = np.zeros((3, 3000)); t = np.arange(40)
+    fext[:, 10:50] = 0.5 * (1 - np.cos(2 * np.pi * t / 40))[None] * rng.uniform(1, 3, (3, 1))   # raised-cosine strike
+    gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0)
+    z = np.zeros_like(case.q0)
+    ref = orc.simulate(orc.LINEAR, case.c1, case.c2, case.c3, case.w, z, z, 3000, fext=orc.f32(fext), fext_gain=gain)
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, _ = gpu_run(plan, z, z, 3000, fext=fext, fext_gain=gain)
+    peak = np.abs(ref["out"]).max(axis=1)
+    assert np.all(np.max(np.abs(gpu - ref["out"]), axis=1) <= TOL_MAX * peak)
+
+
+def test_instability_is_reported_with_step_index():
+    torch, mb = _mods()
+    wl = wlmod.c0(n_steps=4000)
+    case = orc.assemble(wl)
+    plan = plan_with_oracle_inputs(wl, case)
+    q0 = case.q0 * 4000.0                                   # 2 m "displacement": the explicit scheme blows up
+    qm1 = q0.copy()
+    ref = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, q0, qm1, 4000, nl_scale=case.nl_scale, H=case.H)
+    gpu, fb, _, st = gpu_run(plan, q0, qm1, 4000)
+    assert ref["first_bad"][0] > 0
+    assert st == mb.EUNSTABLE and 0 < fb[0] <= ref["first_bad"][0] and ref["first_bad"][0] - fb[0] <= 3
+    assert "non-finite" in plan.last_error()
+    k = fb[0] - 2
+    assert np.all(np.isfinite(gpu[0, :k]))
+
+
+def test_empty_and_limit_arguments():
+    torch, mb = _mods()
+    wl = wlmod.c0(n_steps=64)
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    out = torch.empty((1, 64), dtype=torch.float32, device="cuda")
+    with pytest.raises(mb.ModalError) as e:
+        plan.simulate(q0, 65, out.data_ptr())
+    assert e.value.status == mb.EINVAL and "n_steps" in e.value.message
+    with pytest.raises(mb.ModalError):
+        plan.simulate(np.zeros((2, 10)), 64, out.data_ptr())
+    # zero state -> identically zero output
+    gpu, fb, _, _ = gpu_run(plan, np.zeros((1, 10)), np.zeros((1, 10)), 64)
+    assert np.all(gpu == 0)
+    # one step: out[0] = w . q0
+    gpu, _, _, _ = gpu_run(plan, q0, q0, 1)
+    w = plan.query(mb.Q_PICKUP)[0]
+    assert abs(gpu[0, 0] - np.float32(w).astype(np.float64) @ q0[0]) <= 1e-6 * abs(w @ q0[0]) + 1e-12
+    # host-buffer entry point gives the same samples as the device one
+    g1, _, _, _ = gpu_run(plan, q0, None, 64)
+    g2, fb2, st2 = plan.simulate_host(q0, 64)
+    assert np.array_equal(g1.astype(np.float32), g2)

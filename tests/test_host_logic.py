@@ -1,0 +1,142 @@
+"""CPU tests of the C-ABI library: it loads, exports every symbol include/modal.h declares,
+validates descriptors, and its host-side derivations (mode sets, coefficients, closed-form H,
+stability mask, projection) agree with the independent oracle.  No compute call needs a GPU."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2505_05940_b200 import binding as mb
+from paper_2505_05940_b200 import workloads as wlmod
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "modal.h")).read()
+    declared = set(re.findall(r"\b(modal_[a-z_]+)\s*\(", hdr))
+    assert declared == set(mb.EXPORTS), declared ^ set(mb.EXPORTS)
+    for name in declared:
+        assert hasattr(mb.lib, name)
+
+
+def _c0_plan(n_q=10, n_phi=10, **over):
+    wl = wlmod.c0()
+    wl["n_q"], wl["n_phi"] = n_q, n_phi
+    d = mb.desc_from_workload(wl)
+    for k, v in over.items():
+        setattr(d, k, v)
+    return wl, mb.Plan(d, device=-1)
+
+
+def test_host_only_plan_refuses_to_simulate_no_cpu_fallback():
+    wl, plan = _c0_plan()
+    out = np.zeros((1, 8), np.float32)
+    with pytest.raises(mb.ModalError) as e:
+        plan.simulate_host(np.zeros((1, 10)), 8, out=out)
+    assert e.value.status == mb.ECUDA and "no CPU fallback" in e.value.message
+
+
+def test_validation_reports_all_violations():
+    wl = wlmod.c0()
+    d = mb.desc_from_workload(wl)
+    d.rho = -1.0; d.n_q = 0; d.sample_rate = 0.0; d.Lx = 0.0
+    with pytest.raises(mb.ModalError) as e:
+        mb.Plan(d, device=-1)
+    msg = e.value.message
+    assert e.value.status == mb.EINVAL
+    for frag in ("rho must be positive", "n_q must be at least 1", "sample_rate must be positive", "Lx must be positive"):
+        assert frag in msg
+    d = mb.desc_from_workload(wlmod.c1(batch=2))
+    d.T0 = 0.0; d.D = 0.0
+    with pytest.raises(mb.ModalError) as e:
+        mb.Plan(d, device=-1)
+    assert "degenerate dispersion" in e.value.message
+
+
+@pytest.mark.parametrize("n_q,n_phi", [(10, 10), (57, 23)])
+def test_plate_plan_defaults_match_oracle(n_q, n_phi):
+    wl, plan = _c0_plan(n_q, n_phi)
+    ref = wl["ref"]
+    m, n, lam = orc.rect_modes(ref["Lx"], ref["Ly"], n_q)
+    mp, np_, lamp = orc.rect_modes(ref["Lx"], ref["Ly"], n_phi)
+    assert np.array_equal(plan.query(mb.Q_MODE_M), m) and np.array_equal(plan.query(mb.Q_MODE_N), n)
+    assert np.array_equal(plan.query(mb.Q_PHI_M), mp) and np.array_equal(plan.query(mb.Q_PHI_N), np_)
+    assert np.allclose(plan.query(mb.Q_LAMBDA), lam, rtol=1e-14)
+    om, ga = orc.omega_gamma(lam, orc.plate_D(wl["E"], ref["h"], wl["nu"]), 0.0, wl["rho"] * ref["h"],
+                             wl["sigma0"], wl["sigma1"])
+    assert np.allclose(plan.query(mb.Q_OMEGA)[0], om, rtol=1e-13)
+    assert np.allclose(plan.query(mb.Q_SIGMA)[0], ga, rtol=1e-13)
+    s = wl["E"] / (2 * wl["rho"] * lamp ** 2)
+    assert np.allclose(plan.query(mb.Q_NL_SCALE)[0], s, rtol=1e-13)
+    w = [orc.rect_mode(m[k], n[k], ref["Lx"], ref["Ly"], 0.43 * ref["Lx"], 0.37 * ref["Ly"]) for k in range(n_q)]
+    assert np.allclose(plan.query(mb.Q_PICKUP)[0], w, rtol=1e-12, atol=1e-13)
+    H = orc.H_closed(ref["Lx"], ref["Ly"], m, n, mp, np_)
+    Hdev = plan.query(mb.Q_H_FULL)
+    # two independent closed forms (J-based vs 4-term product-to-sum), compared at fp32 resolution
+    assert np.allclose(Hdev, H, rtol=2e-7, atol=1e-7 * np.abs(H).max())
+    assert np.array_equal(Hdev == 0, H == 0)                       # parity zeros are exact on both sides
+    assert np.array_equal(Hdev, Hdev.transpose(0, 2, 1))
+    assert np.all(plan.query(mb.Q_ACTIVE) == 1)
+
+
+def test_H_upload_roundtrip_and_symmetry_check():
+    wl, plan = _c0_plan(21, 7)           # ragged: 21 = 16 + 5
+    rng = np.random.default_rng(3)
+    H = rng.normal(size=(7, 21, 21)); H = H + H.transpose(0, 2, 1)
+    plan.coeffs_upload(1, H_full=H)
+    assert np.array_equal(plan.query(mb.Q_H_FULL), orc.f32(H))
+    Hbad = H.copy(); Hbad[3, 2, 5] += 1e-3
+    with pytest.raises(mb.ModalError) as e:
+        plan.coeffs_upload(1, H_full=Hbad)
+    assert "not symmetric" in e.value.message
+
+
+def test_derive_coeffs_other_geometry_matches_oracle_scaling():
+    wl = wlmod.c3(batch=4)
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    case = orc.assemble(wl, round_fp32=False)
+    for b in range(4):
+        r = plan.derive_coeffs(Lx=wl["Lx"][b], Ly=wl["Ly"][b], h=wl["h"][b], pickup_x_frac=0.43, pickup_y_frac=0.37)
+        assert np.allclose(r["omega"], case.omega[b], rtol=1e-13)
+        assert np.allclose(r["sigma"], case.gamma[b], rtol=1e-13)
+        assert np.allclose(r["nl_scale"], case.nl_scale[b], rtol=1e-12)
+        wfull = np.array([orc.rect_mode(case.extra["mq"][k], case.extra["nq"][k], wl["Lx"][b], wl["Ly"][b],
+                                        0.43 * wl["Lx"][b], 0.37 * wl["Ly"][b]) for k in range(wl["n_q"])])
+        assert np.allclose(r["pickup"], wfull, rtol=1e-11, atol=1e-12)
+        q0 = plan.project_bump(wl["Lx"][b], wl["Ly"][b], wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
+        q0o = orc.project_bump_rect(case.extra["mq"], case.extra["nq"], wl["Lx"][b], wl["Ly"][b],
+                                    wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
+        assert np.max(np.abs(q0 - q0o)) < 1e-12 * np.abs(q0o).max()
+
+
+def test_string_plan_coeffs_mask_and_projection_match_oracle():
+    wl = wlmod.c1(batch=8)
+    plan, q0 = mb.plan_from_workload(wl, device=-1)
+    case = orc.assemble(wl, round_fp32=False)
+    assert np.allclose(plan.query(mb.Q_OMEGA), case.omega, rtol=1e-13)
+    assert np.allclose(plan.query(mb.Q_SIGMA), case.gamma, rtol=1e-13)
+    assert np.allclose(plan.query(mb.Q_NL_SCALE)[:, 0], case.nl_scale, rtol=1e-13)
+    assert np.array_equal(plan.query(mb.Q_ACTIVE).astype(bool), case.active)       # reading R11, decided in fp64
+    assert 0 < case.active.sum() < case.active.size                                # some strings do lose modes
+    assert "masked" in plan.last_error()
+    q0o = np.where(case.active, 0, 0) + np.array([orc.project_bump_string(wl["n_q"], wl["L"][b], wl["x0"][b], wl["W"][b], wl["A"][b]) for b in range(8)])
+    assert np.max(np.abs(q0 - q0o)) < 1e-13 * np.abs(q0o).max()
+
+
+def test_workloads_are_seeded_and_shaped_like_baseline_configs():
+    a, b = wlmod.c3(batch=16), wlmod.c3(batch=16)
+    for k in ("Lx", "Ly", "h", "A", "x0", "y0"):
+        assert np.array_equal(a[k], b[k])
+    assert np.all((a["Lx"] >= 0.4) & (a["Lx"] <= 0.8)) and np.all((a["Ly"] / a["Lx"] >= 0.5) & (a["Ly"] / a["Lx"] <= 1.0))
+    assert np.all((a["A"] / a["h"] >= 0.1) & (a["A"] / a["h"] <= 5.0))
+    assert np.all(a["x0"] - a["W"] / 2 >= 0) and np.all(a["x0"] + a["W"] / 2 <= a["Lx"])
+    c1 = wlmod.c1()
+    assert c1["batch"] == 1024 and c1["n_q"] == 200 and c1["n_steps"] == 44100
+    assert np.all((c1["T0s"] >= 40) & (c1["T0s"] <= 120)) and np.all((c1["A"] >= 0.5e-3) & (c1["A"] <= 3e-3))
+    assert (wlmod.c0()["n_steps"], wlmod.c2()["n_steps"], wlmod.c4()["n_steps"], wlmod.c3()["n_steps"]) == (11025, 44100, 4410, 22050)
+    sh = wlmod.shard(wlmod.c3(batch=10), 1, 4)
+    assert sh["batch"] == 3 and sh["shard"] == (2, 5) and len(sh["Lx"]) == 3
