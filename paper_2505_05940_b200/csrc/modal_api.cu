@@ -293,10 +293,30 @@ modal_status configure_vk(modal_plan *p, int batch, VkConfig **out)
     }
     if (!CS) {
         const bool want_grid = mode ? !strcmp(mode, "grid") : batch <= 4;
-        CS = force_cs ? force_cs : 8;
         grid_team = want_grid;
-        NCL = grid_team ? p->sm_count / CS : 1;
-        sch = mh::build_schedule(nq, nphi, CS, NCL, NW);
+        if (!grid_team) {
+            CS = force_cs ? force_cs : 8;
+            sch = mh::build_schedule(nq, nphi, CS, 1, NW);
+        } else {
+            // a cluster needs its CTAs in one GPC, so the co-resident capacity depends on the
+            // cluster size: take the shape that keeps the most SMs busy (ties -> larger cluster)
+            int best_ctas = 0;
+            for (int cs : {8, 4, 2, 1}) {
+                if (force_cs && cs != force_cs) continue;
+                int ncl = std::min(p->sm_count / cs, nphi);
+                for (int it = 0; it < 2 && ncl > 0; ++it) {
+                    mh::Schedule s = mh::build_schedule(nq, nphi, cs, ncl, NW);
+                    const size_t sm = vk_smem_bytes(s, P, 1, 0);
+                    const int cap = sm <= SMEM_LIMIT ? max_active_clusters<false>(cs, NW * 32, sm) : 0;
+                    if (cap >= ncl) {
+                        if (ncl * cs > best_ctas) { best_ctas = ncl * cs; CS = cs; NCL = ncl; sch = s; }
+                        break;
+                    }
+                    ncl = cap;
+                }
+            }
+            if (!CS) { p->err += "no co-resident grid team shape for the vK kernel\n"; return MODAL_EINCOMPAT; }
+        }
     }
     const long long key = ((long long)CS << 40) | ((long long)NCL << 20) | (grid_team << 1) | resident;
     VkConfig &c = p->vk_cfgs[key];

@@ -61,8 +61,20 @@ def nl_ratio(case, b):
     return v / vlin
 
 
-def check_parity(gpu, ref, case, weak_only_l2=True, first=4096):
+def check_parity(gpu, ref, case, weak_only_l2=True, first=4096, ref_bad=None, gpu_bad=None):
     for b in range(ref.shape[0]):
+        if ref_bad is not None and ref_bad[b] >= 0:
+            # the explicit scheme blows up on this sample in the oracle too (degenerate case of the
+            # method): the GPU must report it within a few steps of the oracle and
+            # agree on the early prefix; point-wise parity is meaningless close to the blow-up.
+            assert gpu_bad[b] >= 0 and abs(int(gpu_bad[b]) - int(ref_bad[b])) <= 8, (b, gpu_bad[b], ref_bad[b])
+            k = min(256, int(ref_bad[b]) - 64)
+            if k > 0:
+                peak = np.max(np.abs(ref[b, :k]))
+                assert np.max(np.abs(gpu[b, :k] - ref[b, :k])) <= TOL_MAX * peak, b
+            continue
+        if gpu_bad is not None:
+            assert gpu_bad[b] == -1, (b, gpu_bad[b])
         peak = np.max(np.abs(ref[b]))
         k = min(first, ref.shape[1])
         weak = nl_ratio(case, b) <= 0.05
@@ -193,8 +205,9 @@ def test_c1_string_parity(batch, n_steps):
     ref = orc.run_case(case, n_steps)
     plan = plan_with_oracle_inputs(wl, case)
     gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, n_steps)
-    assert st == 0
-    check_parity(gpu, ref["out"], case)
+    torch, mb = _mods()
+    assert st == (mb.EUNSTABLE if np.any(ref["first_bad"] >= 0) else 0)
+    check_parity(gpu, ref["out"], case, ref_bad=ref["first_bad"], gpu_bad=fb)
 
 
 def test_string_plan_defaults_and_lossless_energy():
