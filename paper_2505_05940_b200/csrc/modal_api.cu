@@ -9,7 +9,9 @@
 
 #include "../../include/modal.h"
 #include "host_math.hpp"
+#include "flow_schedule.hpp"
 #include "kernels.cuh"
+#include "vk_flow.cuh"
 
 namespace mh = modal_host;
 namespace md = modal_dev;
@@ -44,6 +46,14 @@ struct VkConfig {
     bool uploaded = false;
 };
 
+struct FlowConfig {
+    int G = 1, NT = 1, NW = 16, NS = 0, slot_tiles = 8, res_tiles = 0;
+    size_t smem = 0;
+    mh::FlowSchedule sched;
+    DevBuf dsched;
+    bool uploaded = false;
+};
+
 }  // namespace
 
 struct modal_plan {
@@ -55,11 +65,14 @@ struct modal_plan {
     int coeff_batch = 1;
     std::vector<double> omega, sigma, nl_scale, lambda_s, pickup;   // [coeff_batch][...]
     std::vector<int> active;                                          // [coeff_batch][n_q]
-    std::vector<float> Ht;                                            // tile-packed H (VK)
+    std::vector<float> Ht;                                            // tile-packed H (VK, team kernel)
+    std::vector<float> Hf;                                            // flow-tile-packed H (VK, flow kernel)
     bool coeffs_dirty = true, H_dirty = true;
     std::string err;
     int sm_count = 148;
     // device storage
+    DevBuf dHf, dfx, dgx, dqx;
+    std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dHt, dkv, dkq, dr, dast, ds, dw, dlam, dc, dq0, dv0, dgain, dbad, dout, dfbuf, dcounter;
     std::map<long long, VkConfig> vk_cfgs;
     int kinfo[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -204,21 +217,30 @@ modal_status sync_coeffs(modal_plan *p)
     return MODAL_OK;
 }
 
-modal_status sync_H(modal_plan *p)
-{
-    if (p->device >= 0 && p->d.model == MODAL_VK) {
-        CU(cudaSetDevice(p->device));
-        CU(p->dHt.ensure(p->Ht.size() * 4));
-        CU(cudaMemcpy(p->dHt.p, p->Ht.data(), p->Ht.size() * 4, cudaMemcpyHostToDevice));
-    }
-    p->H_dirty = false;
-    return MODAL_OK;
-}
-
 int env_int(const char *name, int def)
 {
     const char *s = getenv(name);
     return (s && *s) ? atoi(s) : def;
+}
+bool use_team_kernel()
+{
+    const char *s = getenv("MODAL_VK_IMPL");
+    return s && !strcmp(s, "team");
+}
+
+modal_status sync_H(modal_plan *p)
+{
+    if (p->device >= 0 && p->d.model == MODAL_VK) {
+        CU(cudaSetDevice(p->device));
+        if (use_team_kernel()) {
+            CU(p->dHt.ensure(p->Ht.size() * 4));
+            CU(cudaMemcpy(p->dHt.p, p->Ht.data(), p->Ht.size() * 4, cudaMemcpyHostToDevice));
+        }
+        CU(p->dHf.ensure(p->Hf.size() * 4));
+        CU(cudaMemcpy(p->dHf.p, p->Hf.data(), p->Hf.size() * 4, cudaMemcpyHostToDevice));
+    }
+    p->H_dirty = false;
+    return MODAL_OK;
 }
 
 template <bool R>
@@ -352,6 +374,111 @@ modal_status configure_vk(modal_plan *p, int batch, VkConfig **out)
     return MODAL_OK;
 }
 
+
+// ---- vk_flow launch selection ------------------------------
+int flow_capacity(size_t smem)
+{
+    auto kern = md::vk_flow_kernel;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 17 * 32, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return per_sm;
+}
+
+// Size one team shape: schedule, residency, ring.  Returns false if it does not fit shared memory.
+bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, FlowConfig &c)
+{
+    c.G = G; c.NW = 16; c.slot_tiles = 8;
+    c.sched = mh::build_flow_schedule(nq, nphi, G, c.NW, c.slot_tiles);
+    const mh::FlowSchedule &s = c.sched;
+    if (s.NLOC_MAX > 255 || s.tp_max >= (1 << 24)) return false;
+    const md::FlowSmem fixed = md::flow_smem_layout(0, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, 0);
+    if (fixed.total + 1024 > SMEM_LIMIT) return false;
+    const int avail_tiles = (int)((SMEM_LIMIT - fixed.total - 256) / 1024);
+    if (force_ns <= 0 && force_res < 0 && s.tiles_max <= avail_tiles) { c.NS = 0; c.res_tiles = s.tiles_max; }
+    else {
+        int ns = force_ns > 0 ? force_ns : std::min(12, std::max(0, avail_tiles / c.slot_tiles / 2));
+        if (ns < 2 || ns * c.slot_tiles > avail_tiles) return false;
+        c.NS = ns;
+        c.res_tiles = avail_tiles - ns * c.slot_tiles;
+        if (force_res >= 0) c.res_tiles = std::min(c.res_tiles, force_res);
+    }
+    mh::flow_set_residency(c.sched, c.res_tiles);
+    int rmax = 0;
+    for (int g = 0; g < G; ++g) rmax = std::max(rmax, c.sched.blob[(size_t)g * s.stride + 6]);
+    c.res_tiles = rmax;
+    c.smem = md::flow_smem_layout(c.NS, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, c.res_tiles).total;
+    return c.smem <= SMEM_LIMIT;
+}
+
+// Rough cost of one time step of one team, in SM cycles (constants measured on B200).
+double flow_step_cost(int nq, int nphi, int G)
+{
+    const double tiles = (double)nphi * mh::flow_tiles_per_n(nq);
+    const double per_cta = tiles / G;
+    const double issue = per_cta * 7.0;                         // ~26 warp instructions per tile, 4 issue slots
+    const double unit_chain = 150.0 + 75.0 * std::min(8.0, per_cta);   // one warp, one unit, dependent latency
+    const double resident_cap = 190.0;                          // tiles of shared memory
+    const double stream = std::max(0.0, per_cta - resident_cap) * 1024.0 / 40.0;   // ~40 B/cycle/SM from L2
+    const bool shared_modes = !(G <= nphi && nphi % G == 0);
+    const double exchange = G == 1 ? 0.0 : (shared_modes ? 3.0 : 2.0) * 800.0;   // L2 round trips
+    return std::max(std::max(issue, unit_chain), stream) + exchange + 400.0;
+}
+
+modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
+{
+    const int nq = p->d.n_q, nphi = p->d.n_phi;
+    const int force_g = env_int("MODAL_FLOW_G", 0), force_ns = env_int("MODAL_FLOW_NS", 0), force_res = env_int("MODAL_FLOW_RES", -1);
+    const long long key0 = ((long long)force_g << 40) | ((long long)(force_ns & 0xff) << 32) | ((long long)(force_res + 1) << 8);
+    // pick the team size: minimise (rounds of samples) x (step cost) over the feasible sizes
+    int bestG = 0; double best = 0;
+    const int sm = p->sm_count;
+    std::vector<int> cand;
+    if (force_g > 0) cand.push_back(force_g);
+    else {
+        for (int g = 1; g <= sm; g = g < 8 ? g + 1 : g + 4) cand.push_back(g);
+        cand.push_back(sm);
+        for (int div = 1; div <= 4; ++div) if (nphi % div == 0 && nphi / div <= sm) cand.push_back(nphi / div);
+    }
+    for (int g : cand) {
+        if (g < 1 || g > sm) continue;
+        const double tiles_cta = (double)nphi * mh::flow_tiles_per_n(nq) / g;
+        if (force_g <= 0 && tiles_cta > 1200) continue;          // tables would not fit; skip the expensive build
+        const int nt = std::max(1, std::min(batch, sm / g));
+        const double cost = std::ceil((double)batch / nt) * flow_step_cost(nq, nphi, g);
+        if (!bestG || cost < best * 0.999) { bestG = g; best = cost; }
+    }
+    if (!bestG) { p->err += "no feasible team size for the vK flow kernel\n"; return MODAL_EINCOMPAT; }
+    FlowConfig *c = nullptr;
+    for (int attempt = 0; attempt < 64 && !c; ++attempt) {
+        const long long key = key0 | bestG;
+        FlowConfig &fc = p->flow_cfgs[key];
+        if (fc.uploaded) { c = &fc; break; }
+        if (flow_shape(nq, nphi, bestG, force_ns, force_res, fc)) {
+            CU(fc.dsched.ensure(fc.sched.blob.size() * 4));
+            CU(cudaMemcpy(fc.dsched.p, fc.sched.blob.data(), fc.sched.blob.size() * 4, cudaMemcpyHostToDevice));
+            fc.uploaded = true;
+            c = &fc;
+            break;
+        }
+        p->flow_cfgs.erase(key);
+        if (force_g > 0 || bestG >= sm) break;
+        bestG = std::min(sm, bestG + std::max(1, bestG / 4));    // does not fit: widen the team
+    }
+    if (!c) { p->err += "vK flow schedule does not fit shared memory\n"; return MODAL_EINCOMPAT; }
+    const int per_sm = flow_capacity(c->smem);
+    const int cap = per_sm * sm;
+    if (cap < c->G) {
+        char buf[128];
+        snprintf(buf, sizeof buf, "a team of %d CTAs is not co-resident (capacity %d)\n", c->G, cap);
+        p->err += buf;
+        return MODAL_EINCOMPAT;
+    }
+    c->NT = std::max(1, std::min(batch, cap / c->G));
+    *out = c;
+    return MODAL_OK;
+}
+
 template <int MPL>
 cudaError_t launch_tension(const md::TensionArgs &a, cudaStream_t st)
 {
@@ -390,6 +517,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         CU(cudaMemcpyAsync(p->dgain.p, gain.data(), gain.size() * 8, cudaMemcpyHostToDevice, st));
     }
     CU(cudaMemsetAsync(p->dbad.p, 0xff, (size_t)batch * 4, st));
+    bool flow_launched = false;
     const int auto_start = init->qm1 ? 0 : 1;
     const double half_T2 = 0.5 * p->T * p->T;
 
@@ -419,6 +547,40 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         CU(e);
         p->kinfo[0] = 1; p->kinfo[1] = 1; p->kinfo[2] = (batch + 3) / 4; p->kinfo[3] = 128;
         p->kinfo[4] = 0; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
+    } else if (!use_team_kernel()) {
+        FlowConfig *c = nullptr;
+        modal_status s = configure_flow(p, batch, &c);
+        if (s != MODAL_OK) return s;
+        const mh::FlowSchedule &fs = c->sched;
+        md::FlowArgs a{};
+        a.Hf = p->dHf.as<float>(); a.sched = c->dsched.as<int>(); a.sched_stride = fs.stride;
+        a.off_units = fs.off_units; a.off_ltile = fs.off_ltile; a.off_pieces = fs.off_pieces; a.off_pu = fs.off_pu;
+        a.off_kbptr = fs.off_kbptr; a.off_kblist = fs.off_kblist;
+        a.G = c->G; a.NT = c->NT; a.NW = c->NW; a.NS = c->NS; a.slot_tiles = c->slot_tiles;
+        a.NQP = P; a.n_q = nq; a.n_phi = d.n_phi; a.nb = fs.nb;
+        a.U_max = fs.U_max; a.tp_max = fs.tp_max; a.NLOC_MAX = fs.NLOC_MAX; a.res_tiles = c->res_tiles;
+        a.slice_max = fs.slice_max; a.MS = fs.MS;
+        a.batch = batch; a.n_steps = n_steps;
+        a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
+        a.kv = p->dkv.as<double>(); a.kq = p->dkq.as<double>(); a.r = p->dr.as<double>(); a.astart = p->dast.as<double>();
+        a.s = p->ds.as<float>(); a.w = p->dw.as<float>();
+        a.q0 = p->dq0.as<double>(); a.v0 = p->dv0.as<double>();
+        a.auto_start = auto_start; a.half_T2 = half_T2;
+        a.fext = init->fext_signal; a.gain = p->dgain.as<double>();
+        a.out = out_dev; a.traj = init->traj_dev; a.first_bad = p->dbad.as<int>();
+        if ((long long)((batch + c->NT - 1) / c->NT) * n_steps >= 0xffffffffLL) { p->err += "batch x n_steps too large for one launch\n"; return MODAL_EINCOMPAT; }
+        if (c->G > 1) {
+            const size_t nfx = (size_t)c->NT * c->G * P * 8, ngx = (size_t)c->NT * d.n_phi * fs.MS * 8, nqx = (size_t)c->NT * P * 8;
+            CU(p->dfx.ensure(nfx)); CU(p->dgx.ensure(ngx)); CU(p->dqx.ensure(nqx));
+            CU(cudaMemsetAsync(p->dfx.p, 0, nfx, st)); CU(cudaMemsetAsync(p->dgx.p, 0, ngx, st)); CU(cudaMemsetAsync(p->dqx.p, 0, nqx, st));
+            a.fx = p->dfx.as<unsigned long long>(); a.gx = p->dgx.as<unsigned long long>(); a.qx = p->dqx.as<unsigned long long>();
+        }
+        CU(cudaFuncSetAttribute(md::vk_flow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
+        flow_launched = true;
+        md::vk_flow_kernel<<<c->G * c->NT, (c->NW + 1) * 32, c->smem, st>>>(a);
+        CU(cudaGetLastError());
+        p->kinfo[0] = 3; p->kinfo[1] = c->G; p->kinfo[2] = c->NT; p->kinfo[3] = (c->NW + 1) * 32;
+        p->kinfo[4] = (int)c->smem; p->kinfo[5] = (c->NS == 0 ? 1 : 0) | (c->G > 1 ? 2 : 0); p->kinfo[6] = c->NS; p->kinfo[7] = P;
     } else {
         VkConfig *c = nullptr;
         modal_status s = configure_vk(p, batch, &c);
@@ -453,6 +615,16 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
     if (first_bad) {
         CU(cudaMemcpyAsync(first_bad, p->dbad.p, (size_t)batch * 4, cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
+        if (flow_launched) {
+            int flag = 0;
+            CU(cudaMemcpyFromSymbol(&flag, md::flow_timeout_flag, sizeof(int)));
+            if (flag) {
+                const int zero = 0;
+                CU(cudaMemcpyToSymbol(md::flow_timeout_flag, &zero, sizeof(int)));
+                p->err += "vK flow kernel: a cross-CTA exchange timed out (team not co-resident?)\n";
+                return MODAL_ECUDA;
+            }
+        }
         for (int b = 0; b < batch; ++b)
             if (first_bad[b] >= 0) {
                 char buf[96];
@@ -506,9 +678,11 @@ extern "C" modal_status modal_plan_create(const modal_plan_desc *desc, int cuda_
     if (d.model == MODAL_VK) {
         const double geom = mh::H_geom(d.Lx, d.Ly);
         const mh::ModeSet &q = p->mq, &f = p->mphi;
-        mh::pack_tiles(nq, d.n_phi, [&](int n, int a, int b) {
+        auto get = [&](int n, int a, int b) {
             return geom * mh::H_bracket(q.m[a], q.n[a], q.m[b], q.n[b], f.m[n], f.n[n]);
-        }, p->Ht);
+        };
+        mh::pack_flow_tiles(nq, d.n_phi, get, p->Hf);
+        if (use_team_kernel()) mh::pack_tiles(nq, d.n_phi, get, p->Ht);
     }
     if (cuda_device >= 0) {
         cudaError_t e = cudaSetDevice(cuda_device);
@@ -575,7 +749,9 @@ extern "C" modal_status modal_coeffs_upload(modal_plan *p, const modal_coeffs *c
     p->coeffs_dirty = true;
     if (c->H_full) {
         const double *H = c->H_full;
-        mh::pack_tiles(nq, d.n_phi, [&](int n, int a, int b) { return H[((size_t)n * nq + a) * nq + b]; }, p->Ht);
+        auto get = [&](int n, int a, int b) { return H[((size_t)n * nq + a) * nq + b]; };
+        mh::pack_flow_tiles(nq, d.n_phi, get, p->Hf);
+        if (use_team_kernel()) mh::pack_tiles(nq, d.n_phi, get, p->Ht);
         p->H_dirty = true;
     }
     modal_status s = sync_coeffs(p);
@@ -613,7 +789,8 @@ extern "C" void modal_plan_destroy(modal_plan *p)
     if (p->device >= 0) {
         cudaSetDevice(p->device);
         for (DevBuf *b : {&p->dHt, &p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dw, &p->dlam, &p->dc, &p->dq0,
-                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter}) b->release();
+                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx}) b->release();
+        for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         for (auto &kv : p->vk_cfgs) { kv.second.units.release(); kv.second.warp_ptr.release(); kv.second.cta_ptr.release(); kv.second.nlo.release(); }
     }
     delete p;
@@ -644,7 +821,7 @@ extern "C" modal_status modal_plan_query(const modal_plan *p, int what, void *ds
             if (d.model != MODAL_VK) return MODAL_EINVAL;
             const size_t bytes = (size_t)d.n_phi * nq * nq * 8;
             if (bytes > cap) return MODAL_EINVAL;
-            mh::unpack_tiles(nq, d.n_phi, p->Ht, reinterpret_cast<double *>(dst));
+            mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, reinterpret_cast<double *>(dst));
             return MODAL_OK;
         }
         default: return MODAL_EINVAL;

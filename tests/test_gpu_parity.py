@@ -150,19 +150,24 @@ def _small_vk_workload(n_q, n_phi, batch, n_steps, seed=11):
     return wl
 
 
-@pytest.mark.parametrize("n_q,n_phi,batch,mode,cs", [
-    (37, 13, 3, None, 0),          # 3 tile rows, ragged (37 = 2*16 + 5), resident, auto cluster size
-    (37, 13, 3, "resident", 1),
-    (37, 13, 3, "resident", 4),
-    (37, 13, 3, "cluster", 2),     # streamed from L2, cluster team
-    (37, 13, 2, "grid", 8),        # streamed, whole-grid team with the L2 exchange + grid barrier
-    (100, 50, 2, None, 0),         # C2 shape
-    (16, 1, 1, None, 0),           # exactly one tile, one in-plane mode
-    (1, 1, 2, None, 0),            # degenerate: single mode (Duffing)
+@pytest.mark.parametrize("n_q,n_phi,batch,G,NS,RES", [
+    (37, 13, 3, 0, 0, -1),         # 3 tile rows, ragged (37 = 2*16 + 5); launch selection on its own
+    (37, 13, 3, 1, 0, -1),         # one CTA per sample, everything resident, no L2 exchange
+    (37, 13, 3, 4, 0, -1),         # team of 4: in-plane modes shared between CTAs, L2 exchange
+    (37, 13, 3, 13, 0, -1),        # one in-plane mode per CTA: no shared modes
+    (37, 13, 2, 5, 2, 0),          # nothing resident: every unit streamed by TMA through a 2-slot ring
+    (37, 13, 2, 3, 3, 4),          # 4 tiles resident, the rest streamed
+    (37, 13, 2, 148, 0, -1),       # more CTAs than units: idle CTAs still take part in the exchange
+    (100, 50, 2, 0, 0, -1),        # C2 shape
+    (16, 1, 1, 0, 0, -1),          # exactly one tile, one in-plane mode
+    (16, 1, 1, 7, 0, -1),          # one in-plane mode ... owned by one CTA of a team of 7
+    (1, 1, 2, 0, 0, -1),           # degenerate: single mode (Duffing)
+    (130, 3, 1, 40, 4, 2),         # long tile rows cut into several units, shared by many CTAs, streamed
 ])
-def test_vk_team_shapes_parity(n_q, n_phi, batch, mode, cs, monkeypatch):
-    if mode: monkeypatch.setenv("MODAL_VK_MODE", mode)
-    if cs: monkeypatch.setenv("MODAL_VK_CS", str(cs))
+def test_vk_flow_team_shapes_parity(n_q, n_phi, batch, G, NS, RES, monkeypatch):
+    if G: monkeypatch.setenv("MODAL_FLOW_G", str(G))
+    if NS: monkeypatch.setenv("MODAL_FLOW_NS", str(NS))
+    if RES >= 0: monkeypatch.setenv("MODAL_FLOW_RES", str(RES))
     wl = _small_vk_workload(n_q, n_phi, batch, 1500)
     case = orc.assemble(wl)
     ref = orc.run_case(case, 1500)
@@ -172,9 +177,11 @@ def test_vk_team_shapes_parity(n_q, n_phi, batch, mode, cs, monkeypatch):
     check_parity(gpu, ref["out"], case)
     torch, mb = _mods()
     info = plan.query(mb.Q_KERNEL_INFO)
-    if cs: assert info[1] == cs
-    if mode == "grid": assert info[5] & 2
-    if mode == "resident": assert info[5] & 1
+    assert info[0] == 3
+    if G: assert info[1] == G
+    if NS: assert info[6] == NS and not (info[5] & 1)
+    gpu2, _, _, _ = gpu_run(plan, case.q0, case.qm1, 1500)
+    assert np.array_equal(gpu, gpu2)                         # deterministic summation order
 
 
 def test_vk_ftm_scheme_and_auto_start_parity():
@@ -186,14 +193,15 @@ def test_vk_ftm_scheme_and_auto_start_parity():
     check_parity(gpu, ref["out"], case)
 
 
-def test_c4_shape_grid_team_short_run():
+def test_c4_shape_whole_gpu_team_short_run():
     wl = wlmod.c4(batch=2, n_steps=96)
     case = orc.assemble(wl)
     ref = orc.run_case(case, 96)
     plan = plan_with_oracle_inputs(wl, case)
     gpu, fb, _, _ = gpu_run(plan, case.q0, case.qm1, 96)
     torch, mb = _mods()
-    assert plan.query(mb.Q_KERNEL_INFO)[5] & 2               # grid team, streamed
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 3 and info[1] > 100 and info[6] > 0   # whole-GPU team, H streamed through the TMA ring
     check_parity(gpu, ref["out"], case, first=96)
 
 
