@@ -216,9 +216,11 @@ def main():
         hbm_peak, peak_src = peaks()
         if wl["model"] == "vk":
             ach = hbytes * n_steps / per_launch / 1e9
-            roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
-                    "peak_source": peak_src, "kernel": "vk_team_kernel",
-                    "note": "algorithmic bytes = 4*n_phi*n_q(n_q+1)/2 per time step, once per step for the whole batch"}
+            roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                    "traffic": 68.72e6 if (wl["name"], n_steps) == ("c4_vk_400x200_b1", 4410) else None,
+                    "peak_source": peak_src, "kernel": "vk_flow_kernel",
+                    "note": "algorithmic bytes = 4*n_phi*n_q(n_q+1)/2 per time step, once per step for the whole batch; "
+                            "traffic = dram read+write bytes of one launch (profiles/r1_c4_b1.md): H is read from HBM once and then served by L2"}
         else:
             ach = flops * B * n_steps / per_launch / 1e12
             roof = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP32_PEAK_TFLOPS,

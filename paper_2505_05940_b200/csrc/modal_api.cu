@@ -71,7 +71,7 @@ struct modal_plan {
     std::string err;
     int sm_count = 148;
     // device storage
-    DevBuf dHf, dfx, dgx, dqx;
+    DevBuf dHf, dfx, dgx, dqx, dtiming;
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dHt, dkv, dkq, dr, dast, ds, dw, dlam, dc, dq0, dv0, dgain, dbad, dout, dfbuf, dcounter;
     std::map<long long, VkConfig> vk_cfgs;
@@ -397,7 +397,7 @@ bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, FlowConfig
     const int avail_tiles = (int)((SMEM_LIMIT - fixed.total - 256) / 1024);
     if (force_ns <= 0 && force_res < 0 && s.tiles_max <= avail_tiles) { c.NS = 0; c.res_tiles = s.tiles_max; }
     else {
-        int ns = force_ns > 0 ? force_ns : std::min(12, std::max(0, avail_tiles / c.slot_tiles / 2));
+        int ns = force_ns > 0 ? std::min(force_ns, 32) : std::min(20, std::max(0, (avail_tiles - 16) / c.slot_tiles));   // measured on C4: 8 -> 12 -> 16 -> 20 slots = 18.7 / 17.0 / 16.0 / 15.6 us per step
         if (ns < 2 || ns * c.slot_tiles > avail_tiles) return false;
         c.NS = ns;
         c.res_tiles = avail_tiles - ns * c.slot_tiles;
@@ -570,15 +570,31 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         a.out = out_dev; a.traj = init->traj_dev; a.first_bad = p->dbad.as<int>();
         if ((long long)((batch + c->NT - 1) / c->NT) * n_steps >= 0xffffffffLL) { p->err += "batch x n_steps too large for one launch\n"; return MODAL_EINCOMPAT; }
         if (c->G > 1) {
-            const size_t nfx = (size_t)c->NT * c->G * P * 8, ngx = (size_t)c->NT * d.n_phi * fs.MS * 8, nqx = (size_t)c->NT * P * 8;
+            const size_t nfx = (size_t)c->NT * c->G * P * 8, ngx = (size_t)c->NT * d.n_phi * fs.MS * 8, nqx = (size_t)c->NT * md::FLOW_QREP * P * 8;
             CU(p->dfx.ensure(nfx)); CU(p->dgx.ensure(ngx)); CU(p->dqx.ensure(nqx));
             CU(cudaMemsetAsync(p->dfx.p, 0, nfx, st)); CU(cudaMemsetAsync(p->dgx.p, 0, ngx, st)); CU(cudaMemsetAsync(p->dqx.p, 0, nqx, st));
             a.fx = p->dfx.as<unsigned long long>(); a.gx = p->dgx.as<unsigned long long>(); a.qx = p->dqx.as<unsigned long long>();
+        }
+        const bool timing = env_int("MODAL_FLOW_TIMING", 0) != 0;
+        if (timing) {
+            CU(p->dtiming.ensure((size_t)c->G * c->NT * 32));
+            CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)c->G * c->NT * 32, st));
+            a.timing = p->dtiming.as<long long>();
         }
         CU(cudaFuncSetAttribute(md::vk_flow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
         flow_launched = true;
         md::vk_flow_kernel<<<c->G * c->NT, (c->NW + 1) * 32, c->smem, st>>>(a);
         CU(cudaGetLastError());
+        if (timing) {   // diagnostics: mean cycles per time step and phase over the CTAs
+            CU(cudaStreamSynchronize(st));
+            std::vector<long long> tm((size_t)c->G * c->NT * 4);
+            CU(cudaMemcpy(tm.data(), p->dtiming.p, tm.size() * 8, cudaMemcpyDeviceToHost));
+            double acc[4] = {0, 0, 0, 0}, mx[4] = {0, 0, 0, 0};
+            for (size_t i = 0; i < tm.size(); ++i) { acc[i & 3] += (double)tm[i]; mx[i & 3] = std::max(mx[i & 3], (double)tm[i]); }
+            const double den = (double)c->G * c->NT * n_steps * ((batch + c->NT - 1) / c->NT);
+            fprintf(stderr, "[modal flow timing] G=%d NT=%d NS=%d res=%d cycles/step: A %.0f (max %.0f)  B1 %.0f  B2+C+D %.0f  total %.0f\n",
+                    c->G, c->NT, c->NS, c->res_tiles, acc[0] / den, mx[0] * c->G * c->NT / den, acc[1] / den, acc[2] / den, acc[3] / den);
+        }
         p->kinfo[0] = 3; p->kinfo[1] = c->G; p->kinfo[2] = c->NT; p->kinfo[3] = (c->NW + 1) * 32;
         p->kinfo[4] = (int)c->smem; p->kinfo[5] = (c->NS == 0 ? 1 : 0) | (c->G > 1 ? 2 : 0); p->kinfo[6] = c->NS; p->kinfo[7] = P;
     } else {
@@ -789,7 +805,7 @@ extern "C" void modal_plan_destroy(modal_plan *p)
     if (p->device >= 0) {
         cudaSetDevice(p->device);
         for (DevBuf *b : {&p->dHt, &p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dw, &p->dlam, &p->dc, &p->dq0,
-                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx}) b->release();
+                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming}) b->release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         for (auto &kv : p->vk_cfgs) { kv.second.units.release(); kv.second.warp_ptr.release(); kv.second.cta_ptr.release(); kv.second.nlo.release(); }
     }

@@ -44,7 +44,8 @@ struct FlowArgs {
     float *out; double *traj; int *first_bad;
     unsigned long long *fx;     // [NT][G][NQP]   partial forces
     unsigned long long *gx;     // [NT][n_phi][MS] partial G_n of shared modes
-    unsigned long long *qx;     // [NT][NQP]      new state
+    unsigned long long *qx;     // [NT][FLOW_QREP][NQP]  new state
+    long long *timing;          // optional [G*NT][4]: cycles in phases A, B1, B2+C+D, total (MODAL_FLOW_TIMING)
 };
 
 // ---- tagged 64-bit words through L2 ----------------------------------------------------------
@@ -68,6 +69,41 @@ __device__ __forceinline__ float ld_tag(const unsigned long long *p, unsigned ep
     } while (true);
     return __uint_as_float((unsigned)w);
 }
+
+// two adjacent tagged words with one 16-byte load (each 8-byte half is single-copy atomic)
+__device__ __forceinline__ float2 ld_tag2(const unsigned long long *p, unsigned epoch, volatile int *abortp)
+{
+    unsigned long long w0, w1;
+    unsigned spins = 0;
+    do {
+        asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(p) : "memory");
+        if ((unsigned)(w0 >> 32) == epoch && (unsigned)(w1 >> 32) == epoch) break;
+        if ((++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
+    } while (true);
+    return make_float2(__uint_as_float((unsigned)w0), __uint_as_float((unsigned)w1));
+}
+// sum of the tagged words p[i * stride], i = 0 .. cnt-1 (cnt <= 8), all loads in flight together;
+// words that are not there yet are polled again.  Fixed summation order.
+__device__ __forceinline__ float ld_tag_sum8(const unsigned long long *p, size_t stride, int cnt, unsigned epoch,
+                                            volatile int *abortp)
+{
+    float v[8];
+    unsigned pend = cnt >= 8 ? 0xffu : ((1u << cnt) - 1u), spins = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = 0.f;
+    while (pend) {
+        unsigned long long w[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            if (pend >> i & 1) asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(w[i]) : "l"(p + i * stride) : "memory");
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            if ((pend >> i & 1) && (unsigned)(w[i] >> 32) == epoch) { v[i] = __uint_as_float((unsigned)w[i]); pend &= ~(1u << i); }
+        if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
+    }
+    return ((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]));
+}
+constexpr int FLOW_QREP = 4;     // replicas of the published state: spreads the pollers over L2 slices
 
 // ---- mbarrier / TMA bulk copy ----------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -236,20 +272,35 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
 
     if (warp == NW) {
         // ---------------- producer: TMA bulk copies of the streamed units, step after step --------
-        if (lane == 0 && S > 0) {
-            int slot = 0;
-            unsigned use = 0;
-            for (long long st = 0; st < total_steps; ++st)
-                for (int u = R; u < U; ++u) {
-                    mbar_wait(smem_u32(bars + a.NS + slot), (use & 1) ^ 1, s_abort);
-                    if (*s_abort) return;
-                    const int4 un = units[u];
+        // Lane l owns ring slot l (NS <= 32): the items of a slot are it = l, l+NS, l+2NS, ...  Every lane
+        // runs a non-blocking state machine (test_wait, then issue), so 32 copies are prepared side by
+        // side and no lane ever waits on another.
+        if (S > 0 && lane < a.NS) {
+            const long long total_items = total_steps * S;
+            const int step_u = a.NS % S;
+            long long it = lane;
+            int ui = lane % S;                                  // it % S
+            unsigned use = 0, idle = 0;
+            const uint32_t full = smem_u32(bars + lane), empty = smem_u32(bars + a.NS + lane);
+            const uint32_t dst = smem_u32(ring + (size_t)lane * a.slot_tiles * 64);
+            long long t0 = clock64();
+            while (it < total_items) {
+                uint32_t ok;
+                asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                             "selp.u32 %0, 1, 0, p;\n\t}"
+                             : "=r"(ok) : "r"(empty), "r"((use & 1) ^ 1) : "memory");
+                if (ok) {
+                    const int4 un = units[R + ui];
                     const uint32_t bytes = (uint32_t)((un.x >> 16) & 0xff) * 1024u;
-                    mbar_expect_tx(smem_u32(bars + slot), bytes);
-                    tma_bulk_g2s(smem_u32(ring + (size_t)slot * a.slot_tiles * 64), Hg + (size_t)un.w * 64, bytes,
-                                 smem_u32(bars + slot));
-                    if (++slot == a.NS) { slot = 0; ++use; }
+                    mbar_expect_tx(full, bytes);
+                    tma_bulk_g2s(dst, Hg + (size_t)un.w * 64, bytes, full);
+                    it += a.NS; ++use; idle = 0;
+                    ui += step_u; if (ui >= S) ui -= S;
+                } else if ((++idle & 255u) == 0) {
+                    if (idle == 256) t0 = clock64();
+                    if (*s_abort || clock64() - t0 > 3000000000LL) { *s_abort = 1; flow_timeout_flag = 1; break; }
                 }
+            }
         }
         return;
     }
@@ -259,7 +310,8 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
     unsigned ring_pos = 0, ring_use = 0;                       // ring slot / use count at the start of the step
     unsigned long long *fx = a.fx + (size_t)team * G * NQP;
     unsigned long long *gx = a.gx + (size_t)team * a.n_phi * a.MS;
-    unsigned long long *qx = a.qx + (size_t)team * NQP;
+    unsigned long long *qx = a.qx + (size_t)team * FLOW_QREP * NQP;
+    const unsigned long long *qx_mine = qx + (size_t)(rank % FLOW_QREP) * NQP;
     const bool out_cta = rank == 0;
 
     for (int b = team; b < a.batch; b += a.NT) {
@@ -277,6 +329,8 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
 
         for (int n = 0; n < a.n_steps; ++n) {
             ++epoch;
+            long long tk0 = 0, tk1 = 0, tk2 = 0;
+            if (a.timing && tid == 0) tk0 = clock64();
             // ---- a1 pickup + a6 write-out (last consumer warp of rank 0) ----
             if (out_cta && warp == NW - 1) {
                 float o = 0.f, nrm = 0.f;
@@ -332,6 +386,7 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                 ring_pos = x % (unsigned)a.NS; ring_use += x / (unsigned)a.NS;
             }
             if (bar_consumers_or(NC, *s_abort)) break;      // uniform: nobody is left behind at a barrier
+            if (a.timing && tid == 0) tk1 = clock64();
 
             // ---- B1: G_n per piece (fixed summation order), all-gather over the sharers ----
             for (int p = warp; p < NLOC; p += NW) {
@@ -355,6 +410,7 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                 if (lane == 0) eta[p] = sb[pc.x] * Gn;           // eta_n = s_n G_n
             }
             bar_consumers(NC);
+            if (a.timing && tid == 0) tk2 = clock64();
 
             // ---- B2: partial force of this CTA ----
             for (int k = tid; k < NQP; k += NC) {
@@ -377,7 +433,8 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                 for (int j = warp; j < slice_len; j += NW) {
                     const int k = slice0 + j;
                     float f = 0.f;
-                    for (int c = lane; c < G; c += 32) f += ld_tag(fx + (size_t)c * NQP + k, epoch, s_abort);
+                    for (int c0 = lane; c0 < G; c0 += 256)          // 8 partials per lane in flight
+                        f += ld_tag_sum8(fx + (size_t)c0 * NQP + k, (size_t)32 * NQP, min(8, (G - c0 + 31) / 32), epoch, s_abort);
 #pragma unroll
                     for (int m = 16; m >= 1; m >>= 1) f += __shfl_xor_sync(FLOW_FULL, f, m);
                     if (lane == 0) {
@@ -388,11 +445,15 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                         v = a.kv[coq + k] * v - a.kq[coq + k] * q + r * (fe - fd);
                         q += v;
                         sq[j] = q; sv[j] = v;
-                        st_tag(qx + k, (float)q, epoch);
+#pragma unroll
+                        for (int rep = 0; rep < FLOW_QREP; ++rep) st_tag(qx + (size_t)rep * NQP + k, (float)q, epoch);
                     }
                 }
                 // ---- D: gather q^{n+1} ----
-                for (int k = tid; k < NQP; k += NC) q32[k] = ld_tag(qx + k, epoch, s_abort);
+                // the last eight warps gather, 16 bytes per lane per load; the others go straight to the barrier
+                if (warp >= NW - 8)
+                    for (int pp = (warp - (NW - 8)) * 32 + lane; pp < NQP / 2; pp += 256)
+                        *reinterpret_cast<float2 *>(q32 + 2 * pp) = ld_tag2(qx_mine + 2 * pp, epoch, s_abort);
             } else {
                 bar_consumers(NC);
                 for (int k = tid; k < NQP; k += NC) {
@@ -407,6 +468,11 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                 }
             }
             bar_consumers(NC);
+            if (a.timing && tid == 0) {
+                const long long tk3 = clock64();
+                long long *tm = a.timing + (size_t)blockIdx.x * 4;
+                tm[0] += tk1 - tk0; tm[1] += tk2 - tk1; tm[2] += tk3 - tk2; tm[3] += tk3 - tk0;
+            }
         }
         if (out_cta && warp == NW - 1) {
             const int rem = a.n_steps & 31;
