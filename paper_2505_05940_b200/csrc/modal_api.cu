@@ -10,8 +10,10 @@
 #include "../../include/modal.h"
 #include "host_math.hpp"
 #include "flow_schedule.hpp"
+#include "mma_schedule.hpp"
 #include "kernels.cuh"
 #include "vk_flow.cuh"
+#include "vk_mma.cuh"
 
 namespace mh = modal_host;
 namespace md = modal_dev;
@@ -54,6 +56,13 @@ struct FlowConfig {
     bool uploaded = false;
 };
 
+struct MmaConfig {
+    bool tried = false, ok = false;
+    mh::MmaLayout L;
+    size_t smem = 0;
+    DevBuf dslabs, dn0, dQg, dqf, dGx, dfx, dflags;
+};
+
 }  // namespace
 
 struct modal_plan {
@@ -72,6 +81,7 @@ struct modal_plan {
     int sm_count = 148;
     // device storage
     DevBuf dHf, dfx, dgx, dqx, dtiming;
+    MmaConfig mma;
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dHt, dkv, dkq, dr, dast, ds, dw, dlam, dc, dq0, dv0, dgain, dbad, dout, dfbuf, dcounter;
     std::map<long long, VkConfig> vk_cfgs;
@@ -227,6 +237,14 @@ bool use_team_kernel()
     const char *s = getenv("MODAL_VK_IMPL");
     return s && !strcmp(s, "team");
 }
+// 1 = forced on, 0 = forced off, -1 = automatic (batch >= 64 and the layout fits)
+int mma_kernel_mode()
+{
+    const char *s = getenv("MODAL_VK_IMPL");
+    if (s && !strcmp(s, "mma")) return 1;
+    if (s && (!strcmp(s, "flow") || !strcmp(s, "team"))) return 0;
+    return -1;
+}
 
 modal_status sync_H(modal_plan *p)
 {
@@ -238,6 +256,7 @@ modal_status sync_H(modal_plan *p)
         }
         CU(p->dHf.ensure(p->Hf.size() * 4));
         CU(cudaMemcpy(p->dHf.p, p->Hf.data(), p->Hf.size() * 4, cudaMemcpyHostToDevice));
+        p->mma.tried = false; p->mma.ok = false;            // operand slabs are rebuilt from the new H on demand
     }
     p->H_dirty = false;
     return MODAL_OK;
@@ -479,6 +498,45 @@ modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
     return MODAL_OK;
 }
 
+// ---- vk_mma (batched tensor-core kernel) -------------------------------------------------------
+modal_status configure_mma(modal_plan *p)
+{
+    MmaConfig &m = p->mma;
+    if (m.tried) return MODAL_OK;
+    m.tried = true; m.ok = false;
+    const int nq = p->d.n_q, nphi = p->d.n_phi;
+    const size_t other = md::mma_smem_layout(0, 1).total + 1024;   // generous: state arrays sized for NGRP = 1
+    if (!mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, other, m.L)) return MODAL_OK;
+    m.smem = md::mma_smem_layout((int)m.L.slab_bytes, m.L.NGRP).total;
+    if (m.smem > SMEM_LIMIT) return MODAL_OK;
+    if (cudaFuncSetAttribute(md::vk_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, md::vk_mma_kernel, md::MMA_THREADS, m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
+    if (per_sm * p->sm_count < m.L.G) return MODAL_OK;
+    // operand slabs from the fp32 values the device holds (flow tiles)
+    const std::vector<float> &Hf = p->Hf;
+    const int tpn = mh::flow_tiles_per_n(nq);
+    auto get = [&](int n, int a, int b) -> double {
+        const int hi = std::max(a, b), lo = std::min(a, b), I = hi / 16, J = lo / 16;
+        const float t = Hf[((size_t)n * tpn + I * (I + 1) / 2 + J) * 256 + mh::flow_elem(hi % 16, lo % 16)];
+        return hi == lo ? 2.0 * (double)t : (double)t;
+    };
+    std::vector<uint16_t> slabs;
+    mh::pack_mma_slabs(m.L, get, slabs);
+    const mh::MmaLayout &L = m.L;
+    CU(m.dslabs.ensure(slabs.size() * 2));
+    CU(cudaMemcpy(m.dslabs.p, slabs.data(), slabs.size() * 2, cudaMemcpyHostToDevice));
+    CU(m.dn0.ensure(L.n0.size() * 4));
+    CU(cudaMemcpy(m.dn0.p, L.n0.data(), L.n0.size() * 4, cudaMemcpyHostToDevice));
+    CU(m.dQg.ensure((size_t)2 * L.KC * 8192));
+    CU(m.dqf.ensure((size_t)256 * L.KP * 4));
+    CU(m.dGx.ensure((size_t)L.G * 2 * 128 * L.NGP * 4));
+    CU(m.dfx.ensure((size_t)L.NGRP * 2 * 128 * L.KP * 4));
+    CU(m.dflags.ensure((size_t)3 * L.G * 2 * 4));
+    m.ok = true;
+    return MODAL_OK;
+}
+
 template <int MPL>
 cudaError_t launch_tension(const md::TensionArgs &a, cudaStream_t st)
 {
@@ -547,6 +605,39 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         CU(e);
         p->kinfo[0] = 1; p->kinfo[1] = 1; p->kinfo[2] = (batch + 3) / 4; p->kinfo[3] = 128;
         p->kinfo[4] = 0; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
+    } else if (!use_team_kernel() && mma_kernel_mode() != 0 && (mma_kernel_mode() == 1 || batch >= 64) &&
+               configure_mma(p) == MODAL_OK && p->mma.ok) {
+        MmaConfig &m = p->mma;
+        const mh::MmaLayout &L = m.L;
+        CU(cudaFuncSetAttribute(md::vk_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m.smem));
+        for (int b0 = 0; b0 < batch; b0 += 256) {       // up to two M tiles of 128 samples per launch
+            const int nb = std::min(256, batch - b0);
+            md::MmaArgs a{};
+            a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)L.slab_bytes;
+            a.NKB = L.NKB; a.NGRP = L.NGRP; a.NG = L.NG; a.NGP = L.NGP; a.NC = L.NC; a.KC = L.KC; a.KP = L.KP; a.G = L.G;
+            a.n0 = m.dn0.as<int>(); a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P;
+            a.batch = nb; a.n_steps = n_steps; a.MT = (nb + 127) / 128;
+            a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
+            const size_t oq = cb == 1 ? 0 : (size_t)b0 * P, on = cb == 1 ? 0 : (size_t)b0 * d.n_phi;
+            a.kv = p->dkv.as<double>() + oq; a.kq = p->dkq.as<double>() + oq; a.r = p->dr.as<double>() + oq;
+            a.astart = p->dast.as<double>() + oq; a.s = p->ds.as<float>() + on; a.w = p->dw.as<float>() + oq;
+            a.q0 = p->dq0.as<double>() + (size_t)b0 * P; a.v0 = p->dv0.as<double>() + (size_t)b0 * P;
+            a.auto_start = auto_start; a.half_T2 = half_T2;
+            a.fext = init->fext_signal ? init->fext_signal + (size_t)b0 * n_steps : nullptr;
+            a.gain = init->fext_signal ? p->dgain.as<double>() + (size_t)b0 * P : nullptr;
+            a.out = out_dev + (size_t)b0 * n_steps;
+            a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr;
+            a.first_bad = p->dbad.as<int>() + b0;
+            a.Qg = m.dQg.as<uint16_t>(); a.qf = m.dqf.as<float>(); a.Gx = m.dGx.as<float>(); a.fx = m.dfx.as<float>();
+            a.gflag = m.dflags.as<unsigned>(); a.fflag = a.gflag + L.G * 2; a.qflag = a.fflag + L.G * 2;
+            CU(cudaMemsetAsync(m.dQg.p, 0, (size_t)2 * L.KC * 8192, st));
+            CU(cudaMemsetAsync(m.dflags.p, 0, (size_t)3 * L.G * 2 * 4, st));
+            flow_launched = true;
+            md::vk_mma_kernel<<<L.G, md::MMA_THREADS, m.smem, st>>>(a);
+            CU(cudaGetLastError());
+        }
+        p->kinfo[0] = 4; p->kinfo[1] = L.G; p->kinfo[2] = L.NGRP; p->kinfo[3] = md::MMA_THREADS;
+        p->kinfo[4] = (int)m.smem; p->kinfo[5] = 1; p->kinfo[6] = L.NC; p->kinfo[7] = P;
     } else if (!use_team_kernel()) {
         FlowConfig *c = nullptr;
         modal_status s = configure_flow(p, batch, &c);
@@ -805,7 +896,8 @@ extern "C" void modal_plan_destroy(modal_plan *p)
     if (p->device >= 0) {
         cudaSetDevice(p->device);
         for (DevBuf *b : {&p->dHt, &p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dw, &p->dlam, &p->dc, &p->dq0,
-                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming}) b->release();
+                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming, &p->mma.dslabs, &p->mma.dn0, &p->mma.dQg,
+                          &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags}) b->release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         for (auto &kv : p->vk_cfgs) { kv.second.units.release(); kv.second.warp_ptr.release(); kv.second.cta_ptr.release(); kv.second.nlo.release(); }
     }

@@ -184,6 +184,30 @@ def test_vk_flow_team_shapes_parity(n_q, n_phi, batch, G, NS, RES, monkeypatch):
     assert np.array_equal(gpu, gpu2)                         # deterministic summation order
 
 
+@pytest.mark.parametrize("n_q,n_phi,batch,n_steps", [
+    (37, 13, 5, 1500),             # one M tile, ragged K (37 -> 48), 13 in-plane modes in groups
+    (37, 13, 130, 600),            # two M tiles, second one nearly empty
+    (100, 50, 256, 400),           # two full M tiles, C2 shape
+    (16, 1, 3, 800),               # one k block, one in-plane mode
+])
+def test_vk_mma_tensor_core_parity(n_q, n_phi, batch, n_steps, monkeypatch):
+    """Batched step on tcgen05 (bf16 hi/lo split, 3 MMAs) against the fp64 oracle."""
+    monkeypatch.setenv("MODAL_VK_IMPL", "mma")
+    wl = _small_vk_workload(n_q, n_phi, batch, n_steps)
+    sub = list(range(batch)) if batch <= 8 else sorted(set(np.linspace(0, batch - 1, 12).astype(int).tolist()))
+    case_all = orc.assemble(wl)
+    ref = orc.run_case(orc.assemble(wl, samples=sub), n_steps)
+    plan = plan_with_oracle_inputs(wl, case_all)
+    gpu, fb, _, st = gpu_run(plan, case_all.q0, case_all.qm1, n_steps)
+    torch, mb = _mods()
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 4
+    assert st == 0 and np.all(fb == -1)
+    sub_case = orc.assemble(wl, samples=sub)
+    check_parity(gpu[sub], ref["out"], sub_case)
+    gpu2, _, _, _ = gpu_run(plan, case_all.q0, case_all.qm1, n_steps)
+    assert np.array_equal(gpu, gpu2)
+
+
 def test_vk_ftm_scheme_and_auto_start_parity():
     wl = _small_vk_workload(37, 13, 2, 2000)
     case = orc.assemble(wl, scheme=orc.FTM)
