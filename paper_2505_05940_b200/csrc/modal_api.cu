@@ -505,7 +505,7 @@ modal_status configure_mma(modal_plan *p)
     if (m.tried) return MODAL_OK;
     m.tried = true; m.ok = false;
     const int nq = p->d.n_q, nphi = p->d.n_phi;
-    const size_t other = md::mma_smem_layout(0, 1).total + 1024;   // generous: state arrays sized for NGRP = 1
+    const size_t other = (size_t)md::MMA_NSTG * 8192 + 2048;       // ring + barriers; the exact total is checked below
     if (!mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, other, m.L)) return MODAL_OK;
     m.smem = md::mma_smem_layout((int)m.L.slab_bytes, m.L.NGRP).total;
     if (m.smem > SMEM_LIMIT) return MODAL_OK;
@@ -632,9 +632,26 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             a.gflag = m.dflags.as<unsigned>(); a.fflag = a.gflag + L.G * 2; a.qflag = a.fflag + L.G * 2;
             CU(cudaMemsetAsync(m.dQg.p, 0, (size_t)2 * L.KC * 8192, st));
             CU(cudaMemsetAsync(m.dflags.p, 0, (size_t)3 * L.G * 2 * 4, st));
+            const bool timing = env_int("MODAL_FLOW_TIMING", 0) != 0;
+            if (timing) {
+                CU(p->dtiming.ensure((size_t)L.G * 64));
+                CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)L.G * 64, st));
+                a.timing = p->dtiming.as<long long>();
+            }
             flow_launched = true;
             md::vk_mma_kernel<<<L.G, md::MMA_THREADS, m.smem, st>>>(a);
             CU(cudaGetLastError());
+            if (timing) {
+                CU(cudaStreamSynchronize(st));
+                std::vector<long long> tm((size_t)L.G * 8);
+                CU(cudaMemcpy(tm.data(), p->dtiming.p, tm.size() * 8, cudaMemcpyDeviceToHost));
+                double acc[8] = {0};
+                for (size_t x = 0; x < tm.size(); ++x) acc[x & 7] += (double)tm[x];
+                const double den = (double)L.G * n_steps;
+                fprintf(stderr, "[modal mma timing] G=%d NGRPxNKB=%dx%d NC=%d cycles/step (tile 0): wait q %.0f | wait mma %.0f | epi1 %.0f | G exch %.0f | "
+                        "eta %.0f | epi2 %.0f | f exch %.0f | update %.0f\n", L.G, L.NGRP, L.NKB, L.NC, acc[0] / den, acc[1] / den, acc[2] / den,
+                        acc[3] / den, acc[7] / den, acc[4] / den, acc[5] / den, acc[6] / den);
+            }
         }
         p->kinfo[0] = 4; p->kinfo[1] = L.G; p->kinfo[2] = L.NGRP; p->kinfo[3] = md::MMA_THREADS;
         p->kinfo[4] = (int)m.smem; p->kinfo[5] = 1; p->kinfo[6] = L.NC; p->kinfo[7] = P;

@@ -22,7 +22,7 @@
 namespace modal_dev {
 
 constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
-constexpr int MMA_THREADS = 384;     // warp 0 TMA producer, 1 MMA issuer, 2-3 pickup, 4-7 / 8-11 epilogue tile 0 / 1
+constexpr int MMA_THREADS = 320;     // warp 0 TMA producer, 1 MMA issuer, 2-5 / 6-9 epilogue + pickup of tile 0 / 1 (<= 204 registers)
 
 struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H
@@ -44,6 +44,7 @@ struct MmaArgs {
     float *Gx;                  // [G][2][128][NGP]    partial G
     float *fx;                  // [NGRP][2][128][KP]  partial f
     unsigned *gflag, *fflag, *qflag;   // [G][2] epochs
+    long long *timing;          // optional [G][8] cycle counters of tile 0 (MODAL_FLOW_TIMING)
 };
 
 __device__ __forceinline__ void poll_flag(const unsigned *p, unsigned epoch, volatile int *abortp)
@@ -78,16 +79,32 @@ __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16])
+__device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&u)[16])
 {
-    uint32_t u[16];
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
                  : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]),
                    "=r"(u[8]), "=r"(u[9]), "=r"(u[10]), "=r"(u[11]), "=r"(u[12]), "=r"(u[13]), "=r"(u[14]), "=r"(u[15])
                  : "r"(taddr));
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// flags p[idx * stride], idx = first, first + 32, ... < count: all loads of a lane in flight together
+__device__ __forceinline__ void poll_flags_strided(const unsigned *p, int stride, int first, int count, unsigned epoch,
+                                                   volatile int *abortp)
+{
+    for (int base = first; base < count; base += 256) {
+        unsigned pend = 0, spins = 0;
 #pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(u[i]);
+        for (int u = 0; u < 8; ++u) if (base + 32 * u < count) pend |= 1u << u;
+        while (pend) {
+            unsigned v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (pend >> u & 1) asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + (size_t)(base + 32 * u) * stride) : "memory");
+#pragma unroll
+            for (int u = 0; u < 8; ++u) if ((pend >> u & 1) && v[u] >= epoch) pend &= ~(1u << u);
+            if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
+        }
+    }
 }
 __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
 {
@@ -96,7 +113,7 @@ __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
     return (uint16_t)(u >> 16);
 }
 
-struct MmaSmem { size_t bars, sq, sv, sbad, slab, ring, total; };
+struct MmaSmem { size_t bars, sq, sv, sbad, cst, slab, ring, total; };
 __host__ __device__ inline int mma_nel_max(int NGRP) { return ((128 + NGRP - 1) / NGRP + 1) * 16; }
 __host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int NGRP)
 {
@@ -106,6 +123,7 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int NGRP)
     L.sq = o;   o += 2 * nel * 8;                          // owner state q [2 tiles][nel]
     L.sv = o;   o += 2 * nel * 8;
     L.sbad = o; o += 256 * 4;
+    L.cst = o;  o += 256 * 128;                            // per epilogue thread: s_n[16] floats + 8 doubles of update coefficients
     o = flow_align(o, 128);
     L.slab = o; o += (size_t)slab_bytes;
     o = flow_align(o, 128);
@@ -117,7 +135,8 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int NGRP)
 // One epilogue group = 128 threads = one M tile of 128 samples (thread <-> TMEM lane <-> sample).
 __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int mt, const int c, const int i, const int j,
                                                    const int r, uint64_t *bars, double *sq, double *sv,
-                                                   const uint32_t tbase, volatile int *s_abort, const int lane_base)
+                                                   const uint32_t tbase, volatile int *s_abort, const int lane_base,
+                                                   int *sbad, const int gw, const int lane, unsigned char *cst)
 {
     const int NC = a.NC, NG = a.NG, NGP = a.NGP, KP = a.KP, NKB = a.NKB, NGRP = a.NGRP, B = a.batch;
     const int b = mt * 128 + r;
@@ -146,10 +165,48 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
     bar_named(bar_id, 128);
     if (r == 0) set_flag(a.qflag + c * 2 + mt, 1u);
 
+    // per-thread constants, loaded once: __threadfence (gpu scope) invalidates L1, so anything re-read from
+    // global inside the step loop would pay an L2 round trip every time
+    float *sreg = reinterpret_cast<float *>(cst);                                // [16] s_n of this sample
+    double *ccf = reinterpret_cast<double *>(cst + 64);                         // [2][4] kv, kq, r, astart of the owned elements
+    for (int u = 0; u < 16; ++u) sreg[u] = (u < NG && n0 + u < a.n_phi) ? sb[n0 + u] : 0.f;
+    const bool fast = nel <= 256;                                               // <= 2 owned elements per thread
+    if (fast)
+        for (int h = 0; h < 2; ++h) {
+            const int e = r + 128 * h;
+            ccf[4 * h] = ccf[4 * h + 1] = ccf[4 * h + 2] = ccf[4 * h + 3] = 0.0;
+            if (e < nel) {
+                const int re = r0 + (e >> 4), be = mt * 128 + re, k = j * 16 + (e & 15);
+                if (be < B) {
+                    const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
+                    ccf[4 * h] = a.kv[co]; ccf[4 * h + 1] = a.kq[co]; ccf[4 * h + 2] = a.r[co]; ccf[4 * h + 3] = a.astart[co];
+                }
+            }
+        }
     const uint32_t taddr0 = tbase + ((uint32_t)lane_base << 16) + (uint32_t)(mt * NC);
+    const bool tmg = a.timing && r == 0 && mt == 0;
+    long long *tm = a.timing + (size_t)c * 8;
     for (int n = 0; n < a.n_steps; ++n) {
         const unsigned ep = (unsigned)n + 1u;
+        long long tk = tmg ? clock64() : 0;
         mbar_wait(smem_u32(bars + 16 + mt), n & 1, s_abort);                       // q^n published by everybody
+        if (tmg) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
+        // ---- a1 pickup + a6 write-out: out[b][n] = w . q^n for the samples b = c, c+G, ... of this tile ----
+        for (int m = gw, b2 = c + gw * a.G; b2 < B; m += 4, b2 += 4 * a.G) {
+            if (b2 / 128 != mt) continue;
+            const float *wb = a.w + (size_t)(a.coeff_stride_q ? b2 : 0) * a.NQP;
+            float o = 0.f, nrm = 0.f;
+            for (int k = lane; k < a.n_q; k += 32) {
+                const float qk = __ldcg(a.qf + (size_t)b2 * KP + k);
+                o = fmaf(wb[k], qk, o); nrm = fmaf(qk, qk, nrm);
+            }
+#pragma unroll
+            for (int sh = 16; sh >= 1; sh >>= 1) { o += __shfl_xor_sync(FLOW_FULL, o, sh); nrm += __shfl_xor_sync(FLOW_FULL, nrm, sh); }
+            if (lane == 0) {
+                a.out[(size_t)b2 * a.n_steps + n] = o;
+                if (sbad[m] < 0 && !(isfinite(o) && isfinite(nrm))) sbad[m] = n;
+            }
+        }
         float q16[16];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
@@ -158,54 +215,70 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
             q16[4 * u] = x.x; q16[4 * u + 1] = x.y; q16[4 * u + 2] = x.z; q16[4 * u + 3] = x.w;
         }
         mbar_wait(smem_u32(bars + 12 + mt), n & 1, s_abort);                       // t of this tile is in TMEM
+        if (tmg) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         // ---- epilogue 1: partial G over the 16 rows k of block j ----
         float4 *gout = reinterpret_cast<float4 *>(a.Gx + ((size_t)(c * 2 + mt) * 128 + r) * NGP);
         for (int n4 = 0; n4 < NGP / 4; ++n4) {
-            float g4[4];
+            float g4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int nl = n4 * 4 + u;
-                float g = 0.f;
-                if (nl < NG) {
-                    float v[16];
-                    tmem_ld16(taddr0 + nl * 16, v);
+            for (int h = 0; h < 2; ++h) {                                       // two modes per TMEM wait
+                const int nl = n4 * 4 + 2 * h;
+                uint32_t v0[16], v1[16];
+                if (nl < NG) tmem_ld16_nowait(taddr0 + nl * 16, v0);
+                if (nl + 1 < NG) tmem_ld16_nowait(taddr0 + (nl + 1) * 16, v1);
+                tmem_ld_wait();
 #pragma unroll
-                    for (int kk = 0; kk < 16; ++kk) g = fmaf(q16[kk], v[kk], g);
+                for (int kk = 0; kk < 16; ++kk) {
+                    if (nl < NG) g4[2 * h] = fmaf(q16[kk], __uint_as_float(v0[kk]), g4[2 * h]);
+                    if (nl + 1 < NG) g4[2 * h + 1] = fmaf(q16[kk], __uint_as_float(v1[kk]), g4[2 * h + 1]);
                 }
-                g4[u] = g;
             }
             gout[n4] = make_float4(g4[0], g4[1], g4[2], g4[3]);
         }
         bar_named(bar_id, 128);
         if (r == 0) set_flag(a.gflag + c * 2 + mt, ep);
-        for (int x = r; x < NKB; x += 128) poll_flag(a.gflag + (i * NKB + x) * 2 + mt, ep, s_abort);
+        if (tmg) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; }
+        if (r < 32) poll_flags_strided(a.gflag + (i * NKB) * 2 + mt, 2, r, NKB, ep, s_abort);
         bar_named(bar_id, 128);
+        if (tmg) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; }
         float eta[16];
 #pragma unroll
         for (int u = 0; u < 16; ++u) eta[u] = 0.f;
-        for (int jj = 0; jj < NKB; ++jj) {                                          // fixed order: deterministic
-            const float4 *gp = reinterpret_cast<const float4 *>(a.Gx + ((size_t)((i * NKB + jj) * 2 + mt) * 128 + r) * NGP);
+        {   // sum over the k blocks in fixed order (deterministic); 8 partial rows in flight per batch
+            const float4 *gp0 = reinterpret_cast<const float4 *>(a.Gx + ((size_t)((i * NKB) * 2 + mt) * 128 + r) * NGP);
+            const size_t gstride = (size_t)2 * 128 * NGP / 4;                       // float4 between consecutive k blocks
 #pragma unroll
             for (int n4 = 0; n4 < 4; ++n4)
-                if (n4 < NGP / 4) {
-                    const float4 x = __ldcg(gp + n4);
-                    eta[4 * n4] += x.x; eta[4 * n4 + 1] += x.y; eta[4 * n4 + 2] += x.z; eta[4 * n4 + 3] += x.w;
-                }
+                if (n4 < NGP / 4)
+                    for (int jj0 = 0; jj0 < NKB; jj0 += 8) {
+                        float4 x[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) if (jj0 + u < NKB) x[u] = __ldcg(gp0 + (size_t)(jj0 + u) * gstride + n4);
+#pragma unroll
+                        for (int u = 0; u < 8; ++u)
+                            if (jj0 + u < NKB) { eta[4 * n4] += x[u].x; eta[4 * n4 + 1] += x[u].y; eta[4 * n4 + 2] += x[u].z; eta[4 * n4 + 3] += x[u].w; }
+                    }
         }
 #pragma unroll
-        for (int u = 0; u < 16; ++u) eta[u] = (u < NG && n0 + u < a.n_phi) ? eta[u] * sb[n0 + u] : 0.f;   // eta_n = s_n G_n
+        for (int u = 0; u < 16; ++u) eta[u] *= sreg[u];                             // eta_n = s_n G_n
+        if (tmg) { const long long t_ = clock64(); tm[7] += t_ - tk; tk = t_; }
         // ---- epilogue 2: partial force over the modes n of group i ----
         float facc[16];
 #pragma unroll
         for (int kk = 0; kk < 16; ++kk) facc[kk] = 0.f;
 #pragma unroll
-        for (int nl = 0; nl < 16; ++nl)
+        for (int nl = 0; nl < 16; nl += 2)
             if (nl < NG) {
-                float v[16];
-                tmem_ld16(taddr0 + nl * 16, v);
+                uint32_t v0[16], v1[16];
+                tmem_ld16_nowait(taddr0 + nl * 16, v0);
+                if (nl + 1 < NG) tmem_ld16_nowait(taddr0 + (nl + 1) * 16, v1);
+                tmem_ld_wait();
 #pragma unroll
-                for (int kk = 0; kk < 16; ++kk) facc[kk] = fmaf(eta[nl], v[kk], facc[kk]);
+                for (int kk = 0; kk < 16; ++kk) {
+                    facc[kk] = fmaf(eta[nl], __uint_as_float(v0[kk]), facc[kk]);
+                    if (nl + 1 < NG) facc[kk] = fmaf(eta[nl + 1], __uint_as_float(v1[kk]), facc[kk]);
+                }
             }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         mbar_arrive(smem_u32(bars + 14 + mt));                                      // TMEM tile may be overwritten
@@ -214,21 +287,35 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
         for (int u = 0; u < 4; ++u) fout[u] = make_float4(facc[4 * u], facc[4 * u + 1], facc[4 * u + 2], facc[4 * u + 3]);
         bar_named(bar_id, 128);
         if (r == 0) set_flag(a.fflag + c * 2 + mt, ep);
-        for (int x = r; x < NGRP; x += 128) poll_flag(a.fflag + (x * NKB + j) * 2 + mt, ep, s_abort);
+        if (tmg) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; }
+        if (r < 32) poll_flags_strided(a.fflag + j * 2 + mt, 2 * NKB, r, NGRP, ep, s_abort);
         bar_named(bar_id, 128);
+        if (tmg) { const long long t_ = clock64(); tm[5] += t_ - tk; tk = t_; }
         // ---- owner update: group-ordered sum of the partial forces, a5 linear update (fp64, delta form) ----
         for (int e = r; e < nel; e += 128) {
             const int re = r0 + (e >> 4), kk = e & 15, be = mt * 128 + re, k = j * 16 + kk;
             if (be >= B) continue;
             float f = 0.f;
-            for (int ii = 0; ii < NGRP; ++ii) f += __ldcg(a.fx + ((size_t)(ii * 2 + mt) * 128 + re) * KP + k);
+            {
+                const float *fp0 = a.fx + ((size_t)mt * 128 + re) * KP + k;
+                const size_t fstride = (size_t)2 * 128 * KP;
+                for (int ii0 = 0; ii0 < NGRP; ii0 += 16) {                          // group order; 16 loads in flight
+                    float x[16];
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) if (ii0 + u < NGRP) x[u] = __ldcg(fp0 + (size_t)(ii0 + u) * fstride);
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) if (ii0 + u < NGRP) f += x[u];
+                }
+            }
             const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
-            const double fd = (double)f, rr = a.r[co];
+            const int h = e >= 128 ? 1 : 0;
+            const double fd = (double)f;
+            const double rr = fast ? ccf[4 * h + 2] : a.r[co], kvv = fast ? ccf[4 * h] : a.kv[co], kqq = fast ? ccf[4 * h + 1] : a.kq[co];
             double q = sq[e], v = sv[e];
             if (a.traj && k < a.n_q) a.traj[((size_t)be * a.n_steps + n) * a.n_q + k] = q;
-            if (n == 0 && a.auto_start) v = (rr != 0.0) ? a.astart[co] * q + a.half_T2 * fd : 0.0;
+            if (n == 0 && a.auto_start) v = (rr != 0.0) ? (fast ? ccf[4 * h + 3] : a.astart[co]) * q + a.half_T2 * fd : 0.0;
             const double fe = a.fext ? (double)a.fext[(size_t)be * a.n_steps + n] * a.gain[(size_t)be * a.NQP + k] : 0.0;
-            v = a.kv[co] * v - a.kq[co] * q + rr * (fe - fd);
+            v = kvv * v - kqq * q + rr * (fe - fd);
             q += v;
             sq[e] = q; sv[e] = v;
             const float qfl = (float)q;
@@ -239,7 +326,11 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
         }
         bar_named(bar_id, 128);
         if (r == 0) set_flag(a.qflag + c * 2 + mt, ep + 1u);
+        if (tmg) { const long long t_ = clock64(); tm[6] += t_ - tk; tk = t_; }
     }
+    if (lane == 0)
+        for (int m = gw, b2 = c + gw * a.G; b2 < B; m += 4, b2 += 4 * a.G)
+            if (b2 / 128 == mt) a.first_bad[b2] = sbad[m];
     (void)cq;
 }
 
@@ -254,6 +345,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     volatile int *s_abort = reinterpret_cast<volatile int *>(bars + 21);
     double *sq = reinterpret_cast<double *>(mma_smem + L.sq), *sv = reinterpret_cast<double *>(mma_smem + L.sv);
     int *sbad = reinterpret_cast<int *>(mma_smem + L.sbad);
+    unsigned char *cst = mma_smem + L.cst;
     unsigned char *slab = mma_smem + L.slab, *ring = mma_smem + L.ring;
     const int nel_max = mma_nel_max(a.NGRP);
 
@@ -288,10 +380,9 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
         int stage = 0; unsigned ph = 0;
         for (int n = 0; n < a.n_steps; ++n)
             for (int mt = 0; mt < MT; ++mt) {
-                for (int cc = lane; cc < a.G; cc += 32) poll_flag(a.qflag + cc * 2 + mt, (unsigned)n + 1u, s_abort);
+                poll_flags_strided(a.qflag + mt, 2, lane, a.G, (unsigned)n + 1u, s_abort);
                 __syncwarp();
                 if (lane == 0) {
-                    if (mt == 0 && n > 0) mbar_wait(smem_u32(bars + 18), (n - 1) & 1, s_abort);   // pickup of step n-1 done
                     mbar_arrive(smem_u32(bars + 16 + mt));
                     asm volatile("fence.proxy.async.global;" ::: "memory");
                     for (int kc = 0; kc < KC; ++kc) {
@@ -328,37 +419,11 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                     umma_commit(smem_u32(bars + 12 + mt));                                 // t of tile mt complete
                 }
         }
-    } else if (warp < 4) {
-        // ---------------- pickup: out[b][n] = w . q^n for the samples b = c, c+G, ... --------------------
-        for (int n = 0; n < a.n_steps; ++n) {
-            for (int mt = 0; mt < MT; ++mt) {
-                mbar_wait(smem_u32(bars + 16 + mt), n & 1, s_abort);
-                for (int m = warp - 2, b = c + (warp - 2) * a.G; b < a.batch; m += 2, b += 2 * a.G) {
-                    if (b / 128 != mt) continue;
-                    const float *wb = a.w + (size_t)(a.coeff_stride_q ? b : 0) * a.NQP;
-                    float o = 0.f, nrm = 0.f;
-                    for (int k = lane; k < a.n_q; k += 32) {
-                        const float qk = __ldcg(a.qf + (size_t)b * a.KP + k);
-                        o = fmaf(wb[k], qk, o); nrm = fmaf(qk, qk, nrm);
-                    }
-#pragma unroll
-                    for (int sh = 16; sh >= 1; sh >>= 1) { o += __shfl_xor_sync(FLOW_FULL, o, sh); nrm += __shfl_xor_sync(FLOW_FULL, nrm, sh); }
-                    if (lane == 0) {
-                        a.out[(size_t)b * a.n_steps + n] = o;
-                        if (sbad[m] < 0 && !(isfinite(o) && isfinite(nrm))) sbad[m] = n;
-                    }
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(bars + 18));
-        }
-        if (lane == 0)
-            for (int m = warp - 2, b = c + (warp - 2) * a.G; b < a.batch; m += 2, b += 2 * a.G) a.first_bad[b] = sbad[m];
     } else {
-        const int mt = (warp - 4) >> 2;
+        const int mt = (warp - 2) >> 2, gw = (warp - 2) & 3;
         if (mt < MT)
             mma_epilogue_group(a, mt, c, i, j, (warp & 3) * 32 + lane, bars, sq + (size_t)mt * nel_max, sv + (size_t)mt * nel_max,
-                               tbase, s_abort, (warp & 3) * 32);
+                               tbase, s_abort, (warp & 3) * 32, sbad, gw, lane, cst + (size_t)(tid - 64) * 128);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
