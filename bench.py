@@ -39,8 +39,8 @@ def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
-        return d.get("hbm_gbs", 6650.0), "measured (MEASURED_PEAKS.json)"
-    return 6650.0, "fallback (B200_PROFILING.md)"
+        return d.get("hbm_gbs", 6650.0), "measured (MEASURED_PEAKS.json)", d.get("bf16_tflops_sustained", 1400.0)
+    return 6650.0, "fallback (B200_PROFILING.md)", 1400.0
 
 
 def make_workload(name, batch, n_steps):
@@ -59,6 +59,42 @@ def algorithmic_work(wl):
         P = nq * (nq + 1) // 2
         return 2 * nphi * nq * nq + 4 * nphi * nq + 8 * nq, 4 * nphi * P
     return 12 * nq, 0
+
+
+def tensor_roofline(wl, B, n_steps, per_launch, bf16_peak, peak_src):
+    """vk_mma_kernel: algorithmic flops (F_alg per sample-step) against the measured bf16 peak.
+    The kernel issues three bf16 MMAs per algorithmic MAC (hi*hi + lo*hi + hi*lo) to meet the 1e-4 tolerance."""
+    flops, _ = algorithmic_work(wl)
+    ach = flops * B * n_steps / per_launch / 1e12
+    return {"bound": "tensor", "achieved": ach, "peak": bf16_peak, "unit": "TFLOP/s", "frac": ach / bf16_peak, "traffic": None,
+            "peak_source": peak_src + " bf16 sustained", "kernel": "vk_mma_kernel",
+            "note": "achieved = F_alg (2 N_phi N_q^2 + ...) x batch x steps / time; the tensor pipe executes 3x that "
+                    "(split-bf16), so frac x 3 is the pipe's own utilisation on useful MACs"}
+
+
+def secondary_c3(mb, torch, steps=2, warmup=1):
+    """C3 (batch 256, tensor-core kernel), device-timed only: reported beside the headline workload."""
+    wl = wlmod.by_name("c3")
+    B, n_steps = wl["batch"], wl["n_steps"]
+    plan, q0 = mb.plan_from_workload(wl, torch.cuda.current_device())
+    out = torch.empty((B, n_steps), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    for _ in range(warmup):
+        plan.simulate(q0, n_steps, out.data_ptr(), first_bad=False, stream=stream)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for s_, e_ in ev:
+        s_.record(); plan.simulate(q0, n_steps, out.data_ptr(), first_bad=False, stream=stream); e_.record()
+    torch.cuda.synchronize()
+    per_launch = sum(s_.elapsed_time(e_) for s_, e_ in ev) * 1e-3 / steps
+    info = plan.query(mb.Q_KERNEL_INFO)
+    _, src, bf16_peak = peaks()
+    res = {"workload": wl["name"], "value": B * n_steps / per_launch, "unit": UNIT, "us_per_time_step": 1e6 * per_launch / n_steps,
+           "mode_steps_per_s": B * n_steps * wl["n_q"] / per_launch, "kernel_family": int(info[0]), "ctas": int(info[1])}
+    if int(info[0]) == 4:
+        res["roofline"] = tensor_roofline(wl, B, n_steps, per_launch, bf16_peak, src)
+    plan.close()
+    return res
 
 
 class ClockSampler(threading.Thread):
@@ -147,6 +183,7 @@ def main():
     ap.add_argument("--batch", type=int, default=0)
     ap.add_argument("--n-steps", dest="n_steps", type=int, default=0, help="time steps per simulate call (default: the config's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the C3 (batch 256, tensor-core) line reported beside the headline")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -213,8 +250,10 @@ def main():
         units = world * B * n_steps * args.steps
         value = units / t_dev
         per_launch = t_dev / args.steps
-        hbm_peak, peak_src = peaks()
-        if wl["model"] == "vk":
+        hbm_peak, peak_src, bf16_peak = peaks()
+        if wl["model"] == "vk" and int(info[0]) == 4:
+            roof = tensor_roofline(wl, B, n_steps, per_launch, bf16_peak, peak_src)
+        elif wl["model"] == "vk":
             ach = hbytes * n_steps / per_launch / 1e9
             roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
                     "traffic": 68.72e6 if (wl["name"], n_steps) == ("c4_vk_400x200_b1", 4410) else None,
@@ -239,6 +278,8 @@ def main():
                 "e2e": {"value": units / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(2 * q0.size * 8),
                         "d2h_bytes_per_step": int(out_host.nbytes + 4 * B)},
                 "gpu_launches": args.steps, "clocks": sampler.summary(), "roofline": roof}
+        if not args.no_secondary and world == 1 and args.workload == "c4" and not args.batch and not args.n_steps:
+            line["secondary"] = secondary_c3(mb, torch)
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(wl)
         print(json.dumps(line), flush=True)

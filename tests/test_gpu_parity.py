@@ -208,6 +208,26 @@ def test_vk_mma_tensor_core_parity(n_q, n_phi, batch, n_steps, monkeypatch):
     assert np.array_equal(gpu, gpu2)
 
 
+def test_c3_full_shape_tensor_core_short_run():
+    """C3 at its full size (200 + 100 modes, 256 geometries) in the launch configuration bench.py times,
+    checked on a sample subset spanning the amplitude range (the oracle needs ~2 s per sample here)."""
+    n_steps = 300
+    wl = wlmod.c3(n_steps=n_steps)
+    order = np.argsort(wl["A"] / wl["h"])
+    sub = sorted(set(order[np.linspace(0, 255, 6).astype(int)].tolist()))
+    torch, mb = _mods()
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 4 and info[1] > 100                    # tensor-core kernel on > 100 SMs
+    sub_case = orc.assemble(wl, samples=sub)
+    ref = orc.run_case(sub_case, n_steps)
+    ok = ref["first_bad"] < 0
+    assert np.all(fb[np.array(sub)][ok] == -1)
+    check_parity(gpu[sub][ok], ref["out"][ok], orc.assemble(wl, samples=[s_ for s_, o in zip(sub, ok) if o]), first=n_steps)
+    assert np.all(np.isfinite(gpu[fb < 0]))
+
+
 def test_vk_ftm_scheme_and_auto_start_parity():
     wl = _small_vk_workload(37, 13, 2, 2000)
     case = orc.assemble(wl, scheme=orc.FTM)
