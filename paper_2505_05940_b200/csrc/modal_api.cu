@@ -49,7 +49,7 @@ struct VkConfig {
 };
 
 struct FlowConfig {
-    int G = 1, NT = 1, NW = 16, NS = 0, slot_tiles = 8, res_tiles = 0;
+    int G = 1, NT = 1, NW = 16, NS = 0, slot_tiles = 8, res_tiles = 0, direct = 0, streamed = 0;
     size_t smem = 0;
     mh::FlowSchedule sched;
     DevBuf dsched;
@@ -395,12 +395,12 @@ modal_status configure_vk(modal_plan *p, int batch, VkConfig **out)
 
 
 // ---- vk_flow launch selection ------------------------------
-int flow_capacity(size_t smem)
+int flow_capacity(size_t smem, bool ring)
 {
-    auto kern = md::vk_flow_kernel;
+    auto kern = ring ? md::vk_flow_kernel<true> : md::vk_flow_kernel<false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 17 * 32, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, ring ? 17 * 32 : 16 * 32, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
     return per_sm;
 }
 
@@ -415,14 +415,17 @@ bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, FlowConfig
     if (fixed.total + 1024 > SMEM_LIMIT) return false;
     const int avail_tiles = (int)((SMEM_LIMIT - fixed.total - 256) / 1024);
     if (force_ns <= 0 && force_res < 0 && s.tiles_max <= avail_tiles) { c.NS = 0; c.res_tiles = s.tiles_max; }
-    else {
+    else if (force_ns <= 0) {      // default: no ring; what is not resident is read directly from L2 by the consumers
+        c.NS = 0;
+        c.res_tiles = force_res >= 0 ? std::min(avail_tiles, force_res) : avail_tiles;
+    } else {
         int ns = force_ns > 0 ? std::min(force_ns, 32) : std::min(20, std::max(0, (avail_tiles - 16) / c.slot_tiles));   // measured on C4: 8 -> 12 -> 16 -> 20 slots = 18.7 / 17.0 / 16.0 / 15.6 us per step
         if (ns < 2 || ns * c.slot_tiles > avail_tiles) return false;
         c.NS = ns;
         c.res_tiles = avail_tiles - ns * c.slot_tiles;
         if (force_res >= 0) c.res_tiles = std::min(c.res_tiles, force_res);
     }
-    mh::flow_set_residency(c.sched, c.res_tiles);
+    c.streamed = mh::flow_set_residency(c.sched, c.res_tiles);
     int rmax = 0;
     for (int g = 0; g < G; ++g) rmax = std::max(rmax, c.sched.blob[(size_t)g * s.stride + 6]);
     c.res_tiles = rmax;
@@ -485,7 +488,7 @@ modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
         bestG = std::min(sm, bestG + std::max(1, bestG / 4));    // does not fit: widen the team
     }
     if (!c) { p->err += "vK flow schedule does not fit shared memory\n"; return MODAL_EINCOMPAT; }
-    const int per_sm = flow_capacity(c->smem);
+    const int per_sm = flow_capacity(c->smem, c->NS > 0);
     const int cap = per_sm * sm;
     if (cap < c->G) {
         char buf[128];
@@ -664,7 +667,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         a.Hf = p->dHf.as<float>(); a.sched = c->dsched.as<int>(); a.sched_stride = fs.stride;
         a.off_units = fs.off_units; a.off_ltile = fs.off_ltile; a.off_pieces = fs.off_pieces; a.off_pu = fs.off_pu;
         a.off_kbptr = fs.off_kbptr; a.off_kblist = fs.off_kblist;
-        a.G = c->G; a.NT = c->NT; a.NW = c->NW; a.NS = c->NS; a.slot_tiles = c->slot_tiles;
+        a.G = c->G; a.NT = c->NT; a.NW = c->NW; a.NS = c->NS; a.slot_tiles = c->slot_tiles; a.direct = c->NS == 0 ? 1 : 0;
         a.NQP = P; a.n_q = nq; a.n_phi = d.n_phi; a.nb = fs.nb;
         a.U_max = fs.U_max; a.tp_max = fs.tp_max; a.NLOC_MAX = fs.NLOC_MAX; a.res_tiles = c->res_tiles;
         a.slice_max = fs.slice_max; a.MS = fs.MS;
@@ -685,26 +688,31 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         }
         const bool timing = env_int("MODAL_FLOW_TIMING", 0) != 0;
         if (timing) {
-            CU(p->dtiming.ensure((size_t)c->G * c->NT * 32));
-            CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)c->G * c->NT * 32, st));
+            CU(p->dtiming.ensure((size_t)c->G * c->NT * 64));
+            CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)c->G * c->NT * 64, st));
             a.timing = p->dtiming.as<long long>();
         }
-        CU(cudaFuncSetAttribute(md::vk_flow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
         flow_launched = true;
-        md::vk_flow_kernel<<<c->G * c->NT, (c->NW + 1) * 32, c->smem, st>>>(a);
+        if (c->NS > 0) {
+            CU(cudaFuncSetAttribute(md::vk_flow_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
+            md::vk_flow_kernel<true><<<c->G * c->NT, (c->NW + 1) * 32, c->smem, st>>>(a);
+        } else {
+            CU(cudaFuncSetAttribute(md::vk_flow_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
+            md::vk_flow_kernel<false><<<c->G * c->NT, c->NW * 32, c->smem, st>>>(a);
+        }
         CU(cudaGetLastError());
         if (timing) {   // diagnostics: mean cycles per time step and phase over the CTAs
             CU(cudaStreamSynchronize(st));
-            std::vector<long long> tm((size_t)c->G * c->NT * 4);
+            std::vector<long long> tm((size_t)c->G * c->NT * 8);
             CU(cudaMemcpy(tm.data(), p->dtiming.p, tm.size() * 8, cudaMemcpyDeviceToHost));
-            double acc[4] = {0, 0, 0, 0}, mx[4] = {0, 0, 0, 0};
-            for (size_t i = 0; i < tm.size(); ++i) { acc[i & 3] += (double)tm[i]; mx[i & 3] = std::max(mx[i & 3], (double)tm[i]); }
+            double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, mx0 = 0;
+            for (size_t i = 0; i < tm.size(); ++i) { acc[i & 7] += (double)tm[i]; if ((i & 7) == 0) mx0 = std::max(mx0, (double)tm[i]); }
             const double den = (double)c->G * c->NT * n_steps * ((batch + c->NT - 1) / c->NT);
-            fprintf(stderr, "[modal flow timing] G=%d NT=%d NS=%d res=%d cycles/step: A %.0f (max %.0f)  B1 %.0f  B2+C+D %.0f  total %.0f\n",
-                    c->G, c->NT, c->NS, c->res_tiles, acc[0] / den, mx[0] * c->G * c->NT / den, acc[1] / den, acc[2] / den, acc[3] / den);
+            fprintf(stderr, "[modal flow timing] G=%d NT=%d NS=%d res=%d cycles/step: A %.0f (max %.0f)  B1 %.0f  B2 %.0f  C %.0f  D+barrier %.0f  total %.0f\n",
+                    c->G, c->NT, c->NS, c->res_tiles, acc[0] / den, mx0 * c->G * c->NT / den, acc[1] / den, acc[4] / den, acc[5] / den, acc[6] / den, acc[3] / den);
         }
-        p->kinfo[0] = 3; p->kinfo[1] = c->G; p->kinfo[2] = c->NT; p->kinfo[3] = (c->NW + 1) * 32;
-        p->kinfo[4] = (int)c->smem; p->kinfo[5] = (c->NS == 0 ? 1 : 0) | (c->G > 1 ? 2 : 0); p->kinfo[6] = c->NS; p->kinfo[7] = P;
+        p->kinfo[0] = 3; p->kinfo[1] = c->G; p->kinfo[2] = c->NT; p->kinfo[3] = (c->NW + (c->NS > 0 ? 1 : 0)) * 32;
+        p->kinfo[4] = (int)c->smem; p->kinfo[5] = (c->streamed == 0 ? 1 : 0) | (c->G > 1 ? 2 : 0); p->kinfo[6] = c->NS; p->kinfo[7] = P;
     } else {
         VkConfig *c = nullptr;
         modal_status s = configure_vk(p, batch, &c);

@@ -32,6 +32,7 @@ struct FlowArgs {
     int sched_stride;
     int off_units, off_ltile, off_pieces, off_pu, off_kbptr, off_kblist;
     int G, NT, NW, NS, slot_tiles;
+    int direct;                 // 1: units that are not resident are read straight from L2/HBM by the consumers (no ring)
     int NQP, n_q, n_phi, nb;
     int U_max, tp_max, NLOC_MAX, res_tiles, slice_max, MS;
     int batch, n_steps;
@@ -45,7 +46,7 @@ struct FlowArgs {
     unsigned long long *fx;     // [NT][G][NQP]   partial forces
     unsigned long long *gx;     // [NT][n_phi][MS] partial G_n of shared modes
     unsigned long long *qx;     // [NT][FLOW_QREP][NQP]  new state
-    long long *timing;          // optional [G*NT][4]: cycles in phases A, B1, B2+C+D, total (MODAL_FLOW_TIMING)
+    long long *timing;          // optional [G*NT][8]: cycles in phases A, B1, B2+C+D, total (MODAL_FLOW_TIMING)
 };
 
 // ---- tagged 64-bit words through L2 ----------------------------------------------------------
@@ -148,6 +149,33 @@ __device__ __forceinline__ void bar_consumers(int nthreads)
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
 
+// row sums of a unit: transposing butterfly over the 16 column lanes (bits 3,2,1 of j), then bit 0;
+// writes the 16 row sums after the column groups and returns the unit's share of G_n
+__device__ __forceinline__ float flow_unit_rows(float a0, float a1, float a2, float a3, float a4, float a5, float a6, float a7,
+                                                const int I, const int nt, const float *__restrict__ q32,
+                                                float *__restrict__ tp, const int lane)
+{
+    const int j = lane & 15, half = lane >> 4;
+    const bool b8 = j & 8, b4 = j & 4, b2 = j & 2;
+    float v0 = (b8 ? a4 : a0) + __shfl_xor_sync(FLOW_FULL, b8 ? a0 : a4, 8);
+    float v1 = (b8 ? a5 : a1) + __shfl_xor_sync(FLOW_FULL, b8 ? a1 : a5, 8);
+    float v2 = (b8 ? a6 : a2) + __shfl_xor_sync(FLOW_FULL, b8 ? a2 : a6, 8);
+    float v3 = (b8 ? a7 : a3) + __shfl_xor_sync(FLOW_FULL, b8 ? a3 : a7, 8);
+    float w0 = (b4 ? v2 : v0) + __shfl_xor_sync(FLOW_FULL, b4 ? v0 : v2, 4);
+    float w1 = (b4 ? v3 : v1) + __shfl_xor_sync(FLOW_FULL, b4 ? v1 : v3, 4);
+    float x = (b2 ? w1 : w0) + __shfl_xor_sync(FLOW_FULL, b2 ? w0 : w1, 2);
+    x += __shfl_xor_sync(FLOW_FULL, x, 1);
+    const int row = half * 8 + (b2 ? 1 : 0) + (b4 ? 2 : 0) + (b8 ? 4 : 0);
+    float g = 0.f;
+    if (!(j & 1)) {
+        tp[nt * 16 + row] = x;
+        g = q32[I * 16 + row] * x;
+    }
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) g += __shfl_xor_sync(FLOW_FULL, g, m);
+    return 2.f * g;
+}
+
 // ---- one unit: tiles (I, J0 .. J0+nt-1) of one H^n -------------------------------------------
 // tile : first tile of the unit in shared memory, 64 float4 per tile (flow layout)
 // tp   : the unit's output: nt*16 column sums (block J0+t at tp[t*16..]) then 16 row sums
@@ -173,25 +201,38 @@ __device__ __forceinline__ float flow_unit(const float4 *__restrict__ tile, cons
         c += __shfl_xor_sync(FLOW_FULL, c, 16);
         if (half == 0) tp[t * 16 + j] = c;
     }
-    // row sums: transposing butterfly over the 16 column lanes (bits 3,2,1 of j), then bit 0
-    const bool b8 = j & 8, b4 = j & 4, b2 = j & 2;
-    float v0 = (b8 ? a4 : a0) + __shfl_xor_sync(FLOW_FULL, b8 ? a0 : a4, 8);
-    float v1 = (b8 ? a5 : a1) + __shfl_xor_sync(FLOW_FULL, b8 ? a1 : a5, 8);
-    float v2 = (b8 ? a6 : a2) + __shfl_xor_sync(FLOW_FULL, b8 ? a2 : a6, 8);
-    float v3 = (b8 ? a7 : a3) + __shfl_xor_sync(FLOW_FULL, b8 ? a3 : a7, 8);
-    float w0 = (b4 ? v2 : v0) + __shfl_xor_sync(FLOW_FULL, b4 ? v0 : v2, 4);
-    float w1 = (b4 ? v3 : v1) + __shfl_xor_sync(FLOW_FULL, b4 ? v1 : v3, 4);
-    float x = (b2 ? w1 : w0) + __shfl_xor_sync(FLOW_FULL, b2 ? w0 : w1, 2);
-    x += __shfl_xor_sync(FLOW_FULL, x, 1);
-    const int row = half * 8 + (b2 ? 1 : 0) + (b4 ? 2 : 0) + (b8 ? 4 : 0);
-    float g = 0.f;
-    if (!(j & 1)) {
-        tp[nt * 16 + row] = x;
-        g = q32[I * 16 + row] * x;
-    }
+    return flow_unit_rows(a0, a1, a2, a3, a4, a5, a6, a7, I, nt, q32, tp, lane);
+}
+
+// Same unit with the tiles read straight from global memory (L2): all tiles of the unit (<= 16 LDG.128 per lane) are
+// issued before they are consumed; with 16 warps that keeps up to ~128 KB per SM in flight, which measures
+// ~20 TB/s from L2 on B200, against ~4 TB/s for the cp.async.bulk ring (profiles/r1_c4_b1.md).
+__device__ __forceinline__ float flow_unit_direct(const float4 *__restrict__ tile, const int I, const int J0, const int nt,
+                                                  const float *__restrict__ q32, float *__restrict__ tp, const int lane)
+{
+    const int j = lane & 15, half = lane >> 4;
+    const float4 qa = *reinterpret_cast<const float4 *>(q32 + I * 16 + half * 8);
+    const float4 qb = *reinterpret_cast<const float4 *>(q32 + I * 16 + half * 8 + 4);
+    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f, a5 = 0.f, a6 = 0.f, a7 = 0.f;
+    const float *qj = q32 + J0 * 16 + j;
+    float4 h[16];                                            // the whole unit (<= 8 tiles) in flight
 #pragma unroll
-    for (int m = 16; m >= 1; m >>= 1) g += __shfl_xor_sync(FLOW_FULL, g, m);
-    return 2.f * g;
+    for (int u = 0; u < 8; ++u)
+        if (u < nt) { h[2 * u] = __ldcg(tile + u * 64 + lane); h[2 * u + 1] = __ldcg(tile + u * 64 + 32 + lane); }
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+        if (u < nt) {
+            const float4 h0 = h[2 * u], h1 = h[2 * u + 1];
+            const float x = qj[u * 16];
+            float c = h0.x * qa.x;
+            c = fmaf(h0.y, qa.y, c); c = fmaf(h0.z, qa.z, c); c = fmaf(h0.w, qa.w, c);
+            c = fmaf(h1.x, qb.x, c); c = fmaf(h1.y, qb.y, c); c = fmaf(h1.z, qb.z, c); c = fmaf(h1.w, qb.w, c);
+            a0 = fmaf(h0.x, x, a0); a1 = fmaf(h0.y, x, a1); a2 = fmaf(h0.z, x, a2); a3 = fmaf(h0.w, x, a3);
+            a4 = fmaf(h1.x, x, a4); a5 = fmaf(h1.y, x, a5); a6 = fmaf(h1.z, x, a6); a7 = fmaf(h1.w, x, a7);
+            c += __shfl_xor_sync(FLOW_FULL, c, 16);
+            if (half == 0) tp[u * 16 + j] = c;
+        }
+    return flow_unit_rows(a0, a1, a2, a3, a4, a5, a6, a7, I, nt, q32, tp, lane);
 }
 
 __host__ __device__ inline size_t flow_align(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -221,7 +262,9 @@ __host__ __device__ inline FlowSmem flow_smem_layout(int NS, int slot_tiles, int
     return L;
 }
 
-__global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
+// RING = true: 16 consumer warps + the TMA producer warp; false: consumers only (resident and direct units)
+template <bool RING>
+__global__ void __launch_bounds__(RING ? 544 : 512, 1) vk_flow_kernel(const FlowArgs a)
 {
     extern __shared__ __align__(128) unsigned char flow_smem[];
     unsigned char *smem = flow_smem;
@@ -252,7 +295,7 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
     }
     __syncthreads();
     const int U = sch[0], R = sch[1], NLOC = sch[2], slice0 = sch[4], slice_len = sch[5];
-    const int S = U - R;                                       // streamed units per time step
+    const int S = a.direct ? 0 : U - R;                        // units per time step that go through the TMA ring
     const int4 *units = reinterpret_cast<const int4 *>(sch + a.off_units);
     const int *ltile = sch + a.off_ltile;
     const int4 *pieces = reinterpret_cast<const int4 *>(sch + a.off_pieces);
@@ -270,7 +313,7 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
     const int my_samples = team < a.batch ? (a.batch - team + a.NT - 1) / a.NT : 0;
     const long long total_steps = (long long)my_samples * a.n_steps;
 
-    if (warp == NW) {
+    if (RING && warp == NW) {
         // ---------------- producer: TMA bulk copies of the streamed units, step after step --------
         // Lane l owns ring slot l (NS <= 32): the items of a slot are it = l, l+NS, l+2NS, ...  Every lane
         // runs a non-blocking state machine (test_wait, then issue), so 32 copies are prepared side by
@@ -329,7 +372,7 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
 
         for (int n = 0; n < a.n_steps; ++n) {
             ++epoch;
-            long long tk0 = 0, tk1 = 0, tk2 = 0;
+            long long tk0 = 0, tk1 = 0, tk2 = 0, tkb = 0, tkc = 0;
             if (a.timing && tid == 0) tk0 = clock64();
             // ---- a1 pickup + a6 write-out (last consumer warp of rank 0) ----
             if (out_cta && warp == NW - 1) {
@@ -360,7 +403,11 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                 int slot = 0;
                 unsigned use = 0;
                 if (u < R) tile = res + (size_t)ltile[u] * 64;
-                else {
+                else if (a.direct) {
+                    const float g = flow_unit_direct(Hg + (size_t)un.w * 64, I, un.y, ntl, q32, tp + un.z, lane);
+                    if (lane == 0) gu[u] = g;
+                    continue;
+                } else {
                     const unsigned x = ring_pos + (unsigned)(u - R);
                     slot = (int)(x % (unsigned)a.NS);
                     use = ring_use + x / (unsigned)a.NS;
@@ -428,6 +475,7 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                 if (G > 1) st_tag(fx + (size_t)rank * NQP + k, f, epoch);
                 else fpart[k] = f;
             }
+            if (a.timing && tid == 0) tkb = clock64();
             // ---- C: owner of mode k: rank-ordered sum, a5 linear update (fp64, delta form) ----
             if (G > 1) {
                 for (int j = warp; j < slice_len; j += NW) {
@@ -449,6 +497,7 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
                         for (int rep = 0; rep < FLOW_QREP; ++rep) st_tag(qx + (size_t)rep * NQP + k, (float)q, epoch);
                     }
                 }
+                if (a.timing && tid == 0) tkc = clock64();
                 // ---- D: gather q^{n+1} ----
                 // the last eight warps gather, 16 bytes per lane per load; the others go straight to the barrier
                 if (warp >= NW - 8)
@@ -470,8 +519,9 @@ __global__ void __launch_bounds__(544, 1) vk_flow_kernel(const FlowArgs a)
             bar_consumers(NC);
             if (a.timing && tid == 0) {
                 const long long tk3 = clock64();
-                long long *tm = a.timing + (size_t)blockIdx.x * 4;
+                long long *tm = a.timing + (size_t)blockIdx.x * 8;
                 tm[0] += tk1 - tk0; tm[1] += tk2 - tk1; tm[2] += tk3 - tk2; tm[3] += tk3 - tk0;
+                tm[4] += tkb - tk2; tm[5] += tkc - tkb; tm[6] += tk3 - tkc;
             }
         }
         if (out_cta && warp == NW - 1) {
