@@ -210,6 +210,53 @@ def test_vk_mma_tensor_core_parity(n_q, n_phi, batch, n_steps, monkeypatch):
     assert np.array_equal(gpu, gpu2)
 
 
+def test_vk_mma_ftm_fext_traj(monkeypatch):
+    """Tensor-core kernel with the FTM coefficients, device-side second-order start, an external force signal
+    and the trajectory output; lossless energy of the weakly non-linear samples tracks the oracle's."""
+    monkeypatch.setenv("MODAL_VK_IMPL", "mma")
+    torch, mb = _mods()
+    n_steps, batch = 1200, 9
+    wl = _small_vk_workload(37, 13, batch, n_steps)
+    case = orc.assemble(wl, scheme=orc.FTM)
+    rng = np.random.default_rng(5)
+    fext = np.zeros((batch, n_steps)); t = np.arange(48)
+    fext[:, 20:68] = 0.5 * (1 - np.cos(2 * np.pi * t / 48))[None] * rng.uniform(0.5, 2.0, (batch, 1))
+    gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
+    ref = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, case.q0, case.qm1, n_steps, nl_scale=case.nl_scale,
+                       H=case.H, fext=orc.f32(fext), fext_gain=gain, want_traj=True)
+    plan = plan_with_oracle_inputs(wl, case, scheme=1)
+    gpu, fb, traj, st = gpu_run(plan, case.q0, None, n_steps, want_traj=True, fext=fext, fext_gain=gain)
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 4 and st == 0 and np.all(fb == -1)
+    check_parity(gpu, ref["out"], case)
+    assert np.max(np.abs(traj - ref["traj"])) <= 1e-4 * np.max(np.abs(ref["traj"]))
+    # lossless SV run: discrete energy of a weakly non-linear sample stays within 1e-5 of the oracle's trace
+    wl2 = _small_vk_workload(37, 13, 3, 3000)
+    wl2["A"] = 0.3 * wl2["h"]
+    c2 = orc.assemble(wl2, lossless=True)
+    r2 = orc.run_case(c2, 3000, want_traj=True)
+    p2 = plan_with_oracle_inputs(wl2, c2, lossless=True)
+    _, _, tr2, _ = gpu_run(p2, c2.q0, c2.qm1, 3000, want_traj=True)
+    for b in range(3):
+        e_ref = orc.energy(orc.VK, c2.T, c2.omega[b], r2["traj"][b], nl_scale=c2.nl_scale[b], H=c2.H)
+        e_gpu = orc.energy(orc.VK, c2.T, c2.omega[b], tr2[b], nl_scale=c2.nl_scale[b], H=c2.H)
+        k = len(e_ref) // 10
+        assert abs(e_gpu[-k:].mean() - e_gpu[:k].mean()) / e_gpu.mean() <= TOL_E
+        assert np.max(np.abs(e_gpu - e_ref)) / e_ref.mean() <= TOL_E
+
+
+def test_vk_mma_batch_beyond_one_launch(monkeypatch):
+    """More than 256 samples: the library splits the batch into launches of two M tiles."""
+    monkeypatch.setenv("MODAL_VK_IMPL", "mma")
+    wl = _small_vk_workload(16, 4, 300, 200)
+    case = orc.assemble(wl)
+    sub = [0, 127, 128, 255, 256, 299]
+    ref = orc.run_case(orc.assemble(wl, samples=sub), 200)
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, 200)
+    assert st == 0 and np.all(fb == -1)
+    check_parity(gpu[sub], ref["out"], orc.assemble(wl, samples=sub), first=200)
+
+
 def test_c3_full_shape_tensor_core_short_run():
     """C3 at its full size (200 + 100 modes, 256 geometries) in the launch configuration bench.py times,
     checked on a sample subset spanning the amplitude range (the oracle needs ~2 s per sample here)."""
