@@ -4,7 +4,8 @@
 // Per time step and sample the kernel forms t[n][k] = sum_r H^n[k][r] q[r] (Eq. 9 in
 // one pass, C eliminated by PAPER.md:283) as a GEMM  D[b][(n,k)] = Q[b][r] * Hs[(n,k)][r]^T  on
 // tcgen05 tensor cores: M = 128 samples per tile, K = padded N_q, N = the (n,k) columns of a CTA.
-// CTA (i,j) of the NGRP x NKB grid owns in-plane modes n of group i and the 16 rows k of block j.
+// CTA (i,j) of the NGRP x NKB grid owns in-plane modes n of group i and the RB rows k of block j
+// (B-operand row = local mode * RB + local k).
 // Operands are bf16 split hi + lo; three MMAs (hi*hi + lo*hi + hi*lo) per K chunk give ~2^-17
 // relative accuracy, which the 1e-4 parity tolerance needs.
 //
@@ -33,35 +34,65 @@ inline float bf16_to_float(uint16_t h) { uint32_t u = (uint32_t)h << 16; float f
 inline int umma_chunk_off(int r, int k) { return (r >> 3) * 256 + ((k >> 3) & 1) * 128 + (r & 7) * 16 + (k & 7) * 2; }
 
 struct MmaLayout {
-    int n_q = 0, n_phi = 0, KP = 0, KC = 0;     // padded K, K chunks of 16 (= k blocks of 16 rows)
-    int NKB = 0, NGRP = 0, NG = 0, NC = 0;      // k blocks, n groups, modes per group, columns per CTA (NG*16)
-    int NGP = 0;                                // NG padded to a multiple of 4 (float4 exchange rows)
+    int n_q = 0, n_phi = 0, KP = 0, KC = 0;     // padded K, K chunks of 16
+    int NKB = 0, RB = 0;                        // k blocks, rows k per block (multiple of 4, <= 32)
+    int NGRP = 0, NG = 0, NC = 0;               // n groups, modes per group, operand columns per CTA (>= NG*RB, multiple of 16)
+    int NG4 = 0;                                // float4 per partial-G row: ceil(NG / 4)
+    int QS = 0;                                 // row stride (floats) of the q / partial-f exchange rows: max(KP, NKB*RB)
     int G = 0;                                  // CTAs = NGRP * NKB
+    int nel_max = 0;                            // most (sample, k) elements one CTA owns per M tile
     size_t slab_bytes = 0;                      // per CTA: KC * 2 (hi, lo) * NC * 32
     std::vector<int> n0;                        // [NGRP+1] first in-plane mode of each group
 };
 
-// Returns false if the problem does not fit (grid of `sm` CTAs, `smem_limit` bytes each).
-inline bool mma_layout(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_other, MmaLayout &L)
+inline int mma_rows_owned_max(int NGRP) { return (128 + NGRP - 1) / NGRP; }
+
+// One candidate shape; false if it does not fit.  smem_fixed = bytes besides the slab and the owner state.
+inline bool mma_layout_try(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, int NKB, int rb_align, MmaLayout &L)
 {
     L.n_q = n_q; L.n_phi = n_phi;
-    L.KC = (n_q + 15) / 16; L.KP = L.KC * 16; L.NKB = L.KC;
-    if (L.NKB > sm) return false;
-    L.NGRP = std::min(n_phi, sm / L.NKB);
-    L.NG = (n_phi + L.NGRP - 1) / L.NGRP;
+    L.KC = (n_q + 15) / 16; L.KP = L.KC * 16;
+    L.NKB = NKB;
+    L.RB = ((n_q + NKB - 1) / NKB + rb_align - 1) / rb_align * rb_align;
+    if (L.RB > 32 || NKB > sm) return false;
+    if (NKB > 1 && (NKB - 1) * L.RB >= n_q) return false;          // an empty k block
+    const int max_groups = std::min(n_phi, sm / NKB);
+    L.NG = (n_phi + max_groups - 1) / max_groups;
     L.NGRP = (n_phi + L.NG - 1) / L.NG;
-    L.NC = L.NG * 16;
-    L.NGP = (L.NG + 3) / 4 * 4;
+    L.NC = (L.NG * L.RB + 15) / 16 * 16;
+    if (L.NG > 16 || L.NC > 256) return false;
+    L.NG4 = (L.NG + 3) / 4;
+    L.QS = std::max(L.KP, L.NKB * L.RB);
     L.G = L.NGRP * L.NKB;
+    L.nel_max = mma_rows_owned_max(L.NGRP) * L.RB;
     L.slab_bytes = (size_t)L.KC * 2 * L.NC * 32;
-    if (L.NC > 256 || 2 * L.NC > 512) return false;
-    if (L.slab_bytes + smem_other > smem_limit) return false;
+    if (L.slab_bytes + smem_fixed + (size_t)2 * L.nel_max * (L.nel_max <= 512 ? 40 : 16) > smem_limit) return false;
     L.n0.resize(L.NGRP + 1);
     for (int i = 0; i <= L.NGRP; ++i) L.n0[i] = std::min(n_phi, i * L.NG);
     return true;
 }
 
-// Per-CTA operand slabs: [G][KC][2][NC*32 bytes]; CTA c = i * NKB + j.
+// Shape choice: the MMA time of a tile is ~ KC * 3 * NC / 2 cycles; the G hop reads NKB * NG4 rows per
+// thread, the f hop NGRP partials per owned element.  force_nkb > 0 pins the number of k blocks
+// (MODAL_MMA_NKB, tests / sweeps); rb_align = 16 keeps every tcgen05.ld column offset 16-aligned.
+inline bool mma_layout(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, int force_nkb, int rb_align, MmaLayout &L)
+{
+    double best = 1e300; bool found = false;
+    const int KC = (n_q + 15) / 16;
+    for (int NKB = 1; NKB <= std::min(4 * KC, sm); ++NKB) {
+        if (force_nkb > 0 && NKB != force_nkb) continue;
+        MmaLayout T;
+        if (!mma_layout_try(n_q, n_phi, sm, smem_limit, smem_fixed, NKB, rb_align, T)) continue;
+        const double mma = (double)T.KC * 3.0 * T.NC / 2.0;
+        const double ghop = T.NKB > 1 ? 600.0 + 40.0 * T.NKB * T.NG4 : 0.0;
+        const double fhop = 600.0 + 12.0 * T.NGRP * ((T.nel_max + 127) / 128);
+        const double cost = mma + ghop + fhop;
+        if (cost < best) { best = cost; L = T; found = true; }
+    }
+    return found;
+}
+
+// Per-CTA operand slabs: [G][KC][2][NC*32 bytes]; CTA c = i * NKB + j; operand row = nl * RB + kk.
 template <class Get>   // Get(n,p,q) -> double (full symmetric H)
 inline void pack_mma_slabs(const MmaLayout &L, Get get, std::vector<uint16_t> &slabs)
 {
@@ -72,10 +103,10 @@ inline void pack_mma_slabs(const MmaLayout &L, Get get, std::vector<uint16_t> &s
             for (int nl = 0; nl < L.NG; ++nl) {
                 const int n = L.n0[i] + nl;
                 if (n >= L.n0[i + 1]) break;
-                for (int kk = 0; kk < 16; ++kk) {
-                    const int k = j * 16 + kk;
+                for (int kk = 0; kk < L.RB; ++kk) {
+                    const int k = j * L.RB + kk;
                     if (k >= L.n_q) break;
-                    const int row = nl * 16 + kk;
+                    const int row = nl * L.RB + kk;
                     for (int r = 0; r < L.n_q; ++r) {
                         const float x = (float)get(n, k, r);
                         const uint16_t hi = bf16_rn(x), lo = bf16_rn(x - bf16_to_float(hi));

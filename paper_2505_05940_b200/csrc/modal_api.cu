@@ -508,9 +508,9 @@ modal_status configure_mma(modal_plan *p)
     if (m.tried) return MODAL_OK;
     m.tried = true; m.ok = false;
     const int nq = p->d.n_q, nphi = p->d.n_phi;
-    const size_t other = (size_t)md::MMA_NSTG * 8192 + 2048;       // ring + barriers; the exact total is checked below
-    if (!mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, other, m.L)) return MODAL_OK;
-    m.smem = md::mma_smem_layout((int)m.L.slab_bytes, m.L.NGRP).total;
+    if (!mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, md::mma_smem_fixed(), env_int("MODAL_MMA_NKB", 0),
+                        env_int("MODAL_MMA_RBALIGN", 16) == 4 ? 4 : 16, m.L)) return MODAL_OK;
+    m.smem = md::mma_smem_layout((int)m.L.slab_bytes, m.L.nel_max).total;
     if (m.smem > SMEM_LIMIT) return MODAL_OK;
     if (cudaFuncSetAttribute(md::vk_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
     int per_sm = 0;
@@ -532,10 +532,10 @@ modal_status configure_mma(modal_plan *p)
     CU(m.dn0.ensure(L.n0.size() * 4));
     CU(cudaMemcpy(m.dn0.p, L.n0.data(), L.n0.size() * 4, cudaMemcpyHostToDevice));
     CU(m.dQg.ensure((size_t)2 * L.KC * 8192));
-    CU(m.dqf.ensure((size_t)256 * L.KP * 4));
-    CU(m.dGx.ensure((size_t)L.G * 2 * 128 * L.NGP * 4));
-    CU(m.dfx.ensure((size_t)L.NGRP * 2 * 128 * L.KP * 4));
-    CU(m.dflags.ensure((size_t)3 * L.G * 2 * 4));
+    CU(m.dqf.ensure((size_t)256 * L.QS * 4));
+    CU(m.dGx.ensure((size_t)L.G * 2 * 128 * 4 * L.NG4 * 4));
+    CU(m.dfx.ensure((size_t)L.NGRP * 2 * 128 * L.QS * 4));
+    CU(m.dflags.ensure((size_t)L.G * 2 * 4 * 4));
     m.ok = true;
     return MODAL_OK;
 }
@@ -617,7 +617,8 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             const int nb = std::min(256, batch - b0);
             md::MmaArgs a{};
             a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)L.slab_bytes;
-            a.NKB = L.NKB; a.NGRP = L.NGRP; a.NG = L.NG; a.NGP = L.NGP; a.NC = L.NC; a.KC = L.KC; a.KP = L.KP; a.G = L.G;
+            a.NKB = L.NKB; a.RB = L.RB; a.NGRP = L.NGRP; a.NG = L.NG; a.NG4 = L.NG4; a.NC = L.NC; a.KC = L.KC; a.KP = L.KP; a.QS = L.QS;
+            a.G = L.G; a.nel_max = L.nel_max;
             a.n0 = m.dn0.as<int>(); a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P;
             a.batch = nb; a.n_steps = n_steps; a.MT = (nb + 127) / 128;
             a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
@@ -631,10 +632,14 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             a.out = out_dev + (size_t)b0 * n_steps;
             a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr;
             a.first_bad = p->dbad.as<int>() + b0;
-            a.Qg = m.dQg.as<uint16_t>(); a.qf = m.dqf.as<float>(); a.Gx = m.dGx.as<float>(); a.fx = m.dfx.as<float>();
-            a.gflag = m.dflags.as<unsigned>(); a.fflag = a.gflag + L.G * 2; a.qflag = a.fflag + L.G * 2;
+            a.Qg = m.dQg.as<uint16_t>(); a.qf = m.dqf.as<float>(); a.Gx = m.dGx.as<uint32_t>(); a.fx = m.dfx.as<uint32_t>();
+            a.qflag = m.dflags.as<unsigned>(); a.dbg = env_int("MODAL_MMA_DBG", 0);
+            // exchange buffers start at tag / epoch 0 (the first step uses 1)
             CU(cudaMemsetAsync(m.dQg.p, 0, (size_t)2 * L.KC * 8192, st));
-            CU(cudaMemsetAsync(m.dflags.p, 0, (size_t)3 * L.G * 2 * 4, st));
+            CU(cudaMemsetAsync(m.dqf.p, 0, (size_t)256 * L.QS * 4, st));
+            CU(cudaMemsetAsync(m.dGx.p, 0, (size_t)L.G * 2 * 128 * 4 * L.NG4 * 4, st));
+            CU(cudaMemsetAsync(m.dfx.p, 0, (size_t)L.NGRP * 2 * 128 * L.QS * 4, st));
+            CU(cudaMemsetAsync(m.dflags.p, 0, (size_t)L.G * 2 * 4 * 4, st));
             const bool timing = env_int("MODAL_FLOW_TIMING", 0) != 0;
             if (timing) {
                 CU(p->dtiming.ensure((size_t)L.G * 64));
@@ -651,9 +656,9 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
                 double acc[8] = {0};
                 for (size_t x = 0; x < tm.size(); ++x) acc[x & 7] += (double)tm[x];
                 const double den = (double)L.G * n_steps;
-                fprintf(stderr, "[modal mma timing] G=%d NGRPxNKB=%dx%d NC=%d cycles/step (tile 0): wait q %.0f | wait mma %.0f | epi1 %.0f | G exch %.0f | "
-                        "eta %.0f | epi2 %.0f | f exch %.0f | update %.0f\n", L.G, L.NGRP, L.NKB, L.NC, acc[0] / den, acc[1] / den, acc[2] / den,
-                        acc[3] / den, acc[7] / den, acc[4] / den, acc[5] / den, acc[6] / den);
+                fprintf(stderr, "[modal mma timing] G=%d NGRPxNKB=%dx%d RB=%d NG=%d NC=%d cycles/step (tile 0): wait q %.0f | wait mma %.0f | epi1 %.0f | G hop %.0f | "
+                        "epi2 %.0f | f hop+update %.0f | bar+flag %.0f\n", L.G, L.NGRP, L.NKB, L.RB, L.NG, L.NC, acc[0] / den, acc[1] / den, acc[2] / den,
+                        acc[3] / den, acc[4] / den, acc[5] / den, acc[6] / den);
             }
         }
         p->kinfo[0] = 4; p->kinfo[1] = L.G; p->kinfo[2] = L.NGRP; p->kinfo[3] = md::MMA_THREADS;

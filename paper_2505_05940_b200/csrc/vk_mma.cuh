@@ -6,14 +6,23 @@
 //                                                A = q chunk streamed by TMA from L2, B = H slab resident in
 //                                                shared memory, D = t in TMEM (fp32), kept for both epilogues
 //   G[b][n]  = sum_k q[b][k] t[b][(n,k)]         epilogue 1 (tcgen05.ld, one thread per sample), partial over
-//                                                the CTA's 16 rows k; summed over the k blocks through L2
+//                                                the CTA's RB rows k; summed over the k blocks through L2
 //   eta      = s_n[b] G[b][n]                    (Eq. 9, C eliminated by PAPER.md:283)
 //   f[b][k]  = sum_n eta[b][n] t[b][(n,k)]       epilogue 2, partial over the CTA's modes n; summed over
 //                                                the n groups through L2 by the owner of (b, k)
 //   fp64 delta-form update of the owner's (q, v) (Eq. 19-23), q republished as fp32 and
 //   as bf16 hi/lo in operand layout; pickup out[b][n] = w . q^n.
-// CTA (i,j) owns in-plane modes of group i and rows k of block j.  CTAs synchronise with epoch
-// flags in global memory (writer: stores, fence, flag; reader: acquire flag, L2 loads): no grid barrier.
+// CTA (i,j) owns in-plane modes of group i and rows k of block j.
+//
+// Exchange between CTAs (no grid barrier, no atomics):
+//  * partial G and partial f travel as TAGGED fp32 words: the two low mantissa bits carry (step+1) & 3, the
+//    value is rounded to a multiple of 4 ulp (2^-22 relative, far below the 2^-17 of the split products).
+//    A reader polls the data words themselves (ld.relaxed.gpu) until every tag matches: one L2 round trip,
+//    no fence, no flag.  A word is only overwritten after q of the next step has been published by every
+//    owner, i.e. after every reader of the previous value has consumed it, so a tag can never be mistaken
+//    for the one written four steps earlier.
+//  * the new state q feeds the TMA (async proxy), which cannot poll: owners store, one thread per
+//    (CTA, tile) releases an epoch flag, the TMA warp of every CTA acquires the flags of all CTAs.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -22,12 +31,14 @@
 namespace modal_dev {
 
 constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
-constexpr int MMA_THREADS = 320;     // warp 0 TMA producer, 1 MMA issuer, 2-5 / 6-9 epilogue + pickup of tile 0 / 1 (<= 204 registers)
+constexpr int MMA_THREADS = 384;     // warpgroup 0: warp 0 TMA producer, warp 1 MMA issuer (40 registers after setmaxnreg);
+                                     // warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (232 registers)
+constexpr int MMA_FB = 16;           // partial-force words in flight per owned element while polling
 
 struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H
     int slab_bytes;
-    int NKB, NGRP, NG, NGP, NC, KC, KP, G;
+    int NKB, RB, NGRP, NG, NG4, NC, KC, KP, QS, G, nel_max;
     const int *n0;              // [NGRP+1]
     int n_q, n_phi, NQP;
     int batch, n_steps, MT;     // batch <= 256; MT = M tiles in use
@@ -39,27 +50,18 @@ struct MmaArgs {
     const float *fext; const double *gain;
     float *out; double *traj; int *first_bad;
     // exchange (global, L2 resident)
-    uint16_t *Qg;               // [2][KC][2][4096 B]  q as bf16 hi/lo operand chunks
-    float *qf;                  // [256][KP]           q fp32
-    float *Gx;                  // [G][2][128][NGP]    partial G
-    float *fx;                  // [NGRP][2][128][KP]  partial f
-    unsigned *gflag, *fflag, *qflag;   // [G][2] epochs
+    uint16_t *Qg;               // [2][KC][2][4096 B]   q as bf16 hi/lo operand chunks
+    float *qf;                  // [256][QS]            q fp32
+    uint32_t *Gx;               // [G][2][128][4*NG4]   partial G, tagged
+    uint32_t *fx;               // [NGRP][2][128][QS]   partial f, tagged
+    unsigned *qflag;            // [2][G][4] epochs, one per (tile, CTA, epilogue warp)
     long long *timing;          // optional [G][8] cycle counters of tile 0 (MODAL_FLOW_TIMING)
+    int dbg;                    // MODAL_MMA_DBG: timing experiments that break the results (0 in production)
 };
 
-__device__ __forceinline__ void poll_flag(const unsigned *p, unsigned epoch, volatile int *abortp)
-{
-    unsigned v, spins = 0;
-    do {
-        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-        if (v >= epoch) break;
-        if ((++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
-    } while (true);
-}
 __device__ __forceinline__ void set_flag(unsigned *p, unsigned epoch)
 {
-    __threadfence();
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(epoch) : "memory");
+    asm volatile("fence.acq_rel.gpu;\n\tst.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(epoch) : "memory");
 }
 __device__ __forceinline__ void bar_named(int id, int nthreads)
 {
@@ -87,24 +89,28 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&u)[1
                  : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// flags p[idx * stride], idx = first, first + 32, ... < count: all loads of a lane in flight together
-__device__ __forceinline__ void poll_flags_strided(const unsigned *p, int stride, int first, int count, unsigned epoch,
-                                                   volatile int *abortp)
+// The G uint4 flag groups p[0 .. G): relaxed 16-byte loads, all of a lane in flight together (one L2 round trip
+// per poll round), then ONE acquire fence once every word has reached the epoch.
+__device__ __forceinline__ void poll_flags4(const unsigned *p, int lane, int count, unsigned epoch, volatile int *abortp)
 {
-    for (int base = first; base < count; base += 256) {
+    for (int base = lane; base < count; base += 256) {
         unsigned pend = 0, spins = 0;
 #pragma unroll
         for (int u = 0; u < 8; ++u) if (base + 32 * u < count) pend |= 1u << u;
         while (pend) {
-            unsigned v[8];
+            uint4 v[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u)
-                if (pend >> u & 1) asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + (size_t)(base + 32 * u) * stride) : "memory");
+                if (pend >> u & 1)
+                    asm volatile("ld.relaxed.gpu.global.v4.b32 {%0,%1,%2,%3}, [%4];"
+                                 : "=r"(v[u].x), "=r"(v[u].y), "=r"(v[u].z), "=r"(v[u].w) : "l"(p + (size_t)(base + 32 * u) * 4) : "memory");
 #pragma unroll
-            for (int u = 0; u < 8; ++u) if ((pend >> u & 1) && v[u] >= epoch) pend &= ~(1u << u);
+            for (int u = 0; u < 8; ++u)
+                if ((pend >> u & 1) && v[u].x >= epoch && v[u].y >= epoch && v[u].z >= epoch && v[u].w >= epoch) pend &= ~(1u << u);
             if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
         }
     }
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
 }
 __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
 {
@@ -112,18 +118,46 @@ __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
     u += 0x7fffu + ((u >> 16) & 1u);
     return (uint16_t)(u >> 16);
 }
+// ---- tagged fp32 words -------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t tag_word(float x, uint32_t tag)
+{
+    uint32_t u = __float_as_uint(x);
+    if ((u & 0x7f800000u) != 0x7f800000u) u += 2u;          // round to a multiple of 4 ulp; inf / nan stay non-finite
+    return (u & ~3u) | tag;
+}
+__device__ __forceinline__ float untag(uint32_t w) { return __uint_as_float(w & ~3u); }
+__device__ __forceinline__ void st_tagged4(uint32_t *p, float a, float b, float c, float d, uint32_t tag)
+{
+    asm volatile("st.relaxed.gpu.global.v4.b32 [%0], {%1,%2,%3,%4};"
+                 ::"l"(p), "r"(tag_word(a, tag)), "r"(tag_word(b, tag)), "r"(tag_word(c, tag)), "r"(tag_word(d, tag)) : "memory");
+}
+__device__ __forceinline__ uint4 ld_relaxed4(const uint32_t *p)
+{
+    uint4 w;
+    asm volatile("ld.relaxed.gpu.global.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "l"(p) : "memory");
+    return w;
+}
+__device__ __forceinline__ uint32_t ld_relaxed1(const uint32_t *p)
+{
+    uint32_t w;
+    asm volatile("ld.relaxed.gpu.global.b32 %0, [%1];" : "=r"(w) : "l"(p) : "memory");
+    return w;
+}
+__device__ __forceinline__ bool tags_ok(const uint4 &w, uint32_t tag)
+{
+    return ((w.x & 3u) == tag) & ((w.y & 3u) == tag) & ((w.z & 3u) == tag) & ((w.w & 3u) == tag);
+}
 
-struct MmaSmem { size_t bars, sq, sv, sbad, cst, slab, ring, total; };
-__host__ __device__ inline int mma_nel_max(int NGRP) { return ((128 + NGRP - 1) / NGRP + 1) * 16; }
-__host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int NGRP)
+__host__ __device__ inline int mma_own_bytes(int nel_max) { return nel_max <= 512 ? 40 : 16; }
+struct MmaSmem { size_t bars, own, sbad, cst, slab, ring, total; };
+__host__ __device__ inline size_t mma_smem_fixed() { return 256 + 256 * 4 + 256 * 64 + (size_t)MMA_NSTG * 8192 + 384; }
+__host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int nel_max)
 {
     MmaSmem L; size_t o = 0;
-    const size_t nel = (size_t)mma_nel_max(NGRP);
     L.bars = o; o += 256;                                  // mbarriers, tmem pointer, abort word
-    L.sq = o;   o += 2 * nel * 8;                          // owner state q [2 tiles][nel]
-    L.sv = o;   o += 2 * nel * 8;
+    L.own = o;  o += (size_t)2 * nel_max * mma_own_bytes(nel_max);   // owner state per tile: q, v (+ kv, kq, r if they fit), fp64 [nel_max] each
     L.sbad = o; o += 256 * 4;
-    L.cst = o;  o += 256 * 128;                            // per epilogue thread: s_n[16] floats + 8 doubles of update coefficients
+    L.cst = o;  o += 256 * 64;                             // per epilogue thread: s_n[16] floats
     o = flow_align(o, 128);
     L.slab = o; o += (size_t)slab_bytes;
     o = flow_align(o, 128);
@@ -134,70 +168,74 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int NGRP)
 
 // One epilogue group = 128 threads = one M tile of 128 samples (thread <-> TMEM lane <-> sample).
 __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int mt, const int c, const int i, const int j,
-                                                   const int r, uint64_t *bars, double *sq, double *sv,
+                                                   const int r, uint64_t *bars, double *own,
                                                    const uint32_t tbase, volatile int *s_abort, const int lane_base,
-                                                   int *sbad, const int gw, const int lane, unsigned char *cst)
+                                                   int *sbad, const int gw, const int lane, float *sreg)
 {
-    const int NC = a.NC, NG = a.NG, NGP = a.NGP, KP = a.KP, NKB = a.NKB, NGRP = a.NGRP, B = a.batch;
+    const int NC = a.NC, NG = a.NG, NG4 = a.NG4, QS = a.QS, NKB = a.NKB, NGRP = a.NGRP, B = a.batch, RB = a.RB, KC = a.KC;
+    const int nch = (RB + 15) >> 4;
     const int b = mt * 128 + r;
     const bool valid = b < B;
-    const int bar_id = 2 + mt;
     const int n0 = a.n0[i];
-    const size_t cq = (size_t)(a.coeff_stride_q ? (valid ? b : 0) : 0) * a.NQP;
     const float *sb = a.s + (size_t)(a.coeff_stride_phi ? (valid ? b : 0) : 0) * a.n_phi;
-    // the (sample, k) elements this group owns for the update: rows r0..r1 of the tile, 16 modes of block j
-    const int r0 = 128 * i / NGRP, r1 = 128 * (i + 1) / NGRP, nel = (r1 - r0) * 16;
-    uint16_t *Qt = a.Qg + (size_t)mt * a.KC * 8192 / 2 + (size_t)j * 8192 / 2;     // chunk kc = j of this tile (hi; lo at +4096 B)
-    // ---- publish q^0 ----
+    // the (sample, k) elements this group owns for the update: rows r0..r1 of the tile, RB modes of block j
+    const int r0 = 128 * i / NGRP, r1 = 128 * (i + 1) / NGRP, nel = (r1 - r0) * RB;
+    double *sq = own, *sv = own + a.nel_max, *skv = own + 2 * a.nel_max, *skq = own + 3 * a.nel_max, *sr = own + 4 * a.nel_max;
+    const bool csm = mma_own_bytes(a.nel_max) == 40;                                // update coefficients held in shared memory
+    uint16_t *Qt = a.Qg + (size_t)mt * KC * 4096;                                  // chunk kc at + kc * 4096 (hi; lo at + 2048)
+    // ---- owner state, coefficients, publish q^0 ----
     for (int e = r; e < nel; e += 128) {
-        const int re = r0 + (e >> 4), kk = e & 15, be = mt * 128 + re, k = j * 16 + kk;
-        double q = 0.0, v = 0.0;
-        if (be < B) { q = a.q0[(size_t)be * a.NQP + k]; v = a.v0[(size_t)be * a.NQP + k]; }
-        sq[e] = q; sv[e] = v;
-        if (be < B) {
+        const int rr_ = e / RB, kk = e - rr_ * RB, re = r0 + rr_, be = mt * 128 + re, k = j * RB + kk;
+        double q = 0.0, v = 0.0, kv = 0.0, kq = 0.0, rc = 0.0;
+        if (be < B && k < a.n_q) {
+            q = a.q0[(size_t)be * a.NQP + k]; v = a.v0[(size_t)be * a.NQP + k];
+            const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
+            kv = a.kv[co]; kq = a.kq[co]; rc = a.r[co];
             const float qfl = (float)q;
-            a.qf[(size_t)be * KP + k] = qfl;
+            a.qf[(size_t)be * QS + k] = qfl;
             const uint16_t hi = bf16_rn_dev(qfl), lo = bf16_rn_dev(qfl - __uint_as_float((uint32_t)hi << 16));
-            const int off = ((re >> 3) * 256 + (kk >> 3) * 128 + (re & 7) * 16 + (kk & 7) * 2) >> 1;
-            Qt[off] = hi; Qt[2048 + off] = lo;
+            const int k16 = k & 15;
+            const int off = ((re >> 3) * 256 + (k16 >> 3) * 128 + (re & 7) * 16 + (k16 & 7) * 2) >> 1;
+            uint16_t *Qc = Qt + (size_t)(k >> 4) * 4096;
+            Qc[off] = hi; Qc[2048 + off] = lo;
         }
+        sq[e] = q; sv[e] = v;
+        if (csm) { skv[e] = kv; skq[e] = kq; sr[e] = rc; }
     }
-    bar_named(bar_id, 128);
-    if (r == 0) set_flag(a.qflag + c * 2 + mt, 1u);
+    __syncwarp();
+    if (lane == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * 4 + (r >> 5), 1u);
+    for (int u = 0; u < 16; ++u) sreg[u * 256] = (u < NG && n0 + u < a.n_phi) ? sb[n0 + u] : 0.f;   // [16][256]: conflict-free
 
-    // per-thread constants, loaded once: __threadfence (gpu scope) invalidates L1, so anything re-read from
-    // global inside the step loop would pay an L2 round trip every time
-    float *sreg = reinterpret_cast<float *>(cst);                                // [16] s_n of this sample
-    double *ccf = reinterpret_cast<double *>(cst + 64);                         // [2][4] kv, kq, r, astart of the owned elements
-    for (int u = 0; u < 16; ++u) sreg[u] = (u < NG && n0 + u < a.n_phi) ? sb[n0 + u] : 0.f;
-    const bool fast = nel <= 256;                                               // <= 2 owned elements per thread
-    if (fast)
-        for (int h = 0; h < 2; ++h) {
-            const int e = r + 128 * h;
-            ccf[4 * h] = ccf[4 * h + 1] = ccf[4 * h + 2] = ccf[4 * h + 3] = 0.0;
-            if (e < nel) {
-                const int re = r0 + (e >> 4), be = mt * 128 + re, k = j * 16 + (e & 15);
-                if (be < B) {
-                    const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
-                    ccf[4 * h] = a.kv[co]; ccf[4 * h + 1] = a.kq[co]; ccf[4 * h + 2] = a.r[co]; ccf[4 * h + 3] = a.astart[co];
-                }
-            }
-        }
     const uint32_t taddr0 = tbase + ((uint32_t)lane_base << 16) + (uint32_t)(mt * NC);
     const bool tmg = a.timing && r == 0 && mt == 0;
     long long *tm = a.timing + (size_t)c * 8;
+    uint32_t *grow = a.Gx + ((size_t)(c * 2 + mt) * 128 + r) * (4 * NG4);
+    const uint32_t *grd = a.Gx + ((size_t)((i * NKB) * 2 + mt) * 128 + r) * (4 * NG4);
+    const size_t gstride = (size_t)2 * 128 * 4 * NG4;                               // words between consecutive k blocks
+    uint32_t *frow = a.fx + ((size_t)(i * 2 + mt) * 128 + r) * QS + j * RB;
+    const size_t fstride = (size_t)2 * 128 * QS;                                    // words between consecutive n groups
+    const float *qrow = a.qf + (size_t)(valid ? b : 0) * QS + j * RB;
+
     for (int n = 0; n < a.n_steps; ++n) {
-        const unsigned ep = (unsigned)n + 1u;
+        const uint32_t tag = ((uint32_t)n + 1u) & 3u;
         long long tk = tmg ? clock64() : 0;
         mbar_wait(smem_u32(bars + 16 + mt), n & 1, s_abort);                       // q^n published by everybody
         if (tmg) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
+        // ---- this sample's q over the rows of block j (operand of epilogue 1) ----
+        float qb[32];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (4 * u < RB) x = __ldcg(reinterpret_cast<const float4 *>(qrow) + u);
+            qb[4 * u] = x.x; qb[4 * u + 1] = x.y; qb[4 * u + 2] = x.z; qb[4 * u + 3] = x.w;
+        }
         // ---- a1 pickup + a6 write-out: out[b][n] = w . q^n for the samples b = c, c+G, ... of this tile ----
-        for (int m = gw, b2 = c + gw * a.G; b2 < B; m += 4, b2 += 4 * a.G) {
+        for (int m = gw, b2 = c + gw * a.G; b2 < B && !(a.dbg & 4); m += 4, b2 += 4 * a.G) {
             if (b2 / 128 != mt) continue;
             const float *wb = a.w + (size_t)(a.coeff_stride_q ? b2 : 0) * a.NQP;
             float o = 0.f, nrm = 0.f;
             for (int k = lane; k < a.n_q; k += 32) {
-                const float qk = __ldcg(a.qf + (size_t)b2 * KP + k);
+                const float qk = __ldcg(a.qf + (size_t)b2 * QS + k);
                 o = fmaf(wb[k], qk, o); nrm = fmaf(qk, qk, nrm);
             }
 #pragma unroll
@@ -207,131 +245,173 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 if (sbad[m] < 0 && !(isfinite(o) && isfinite(nrm))) sbad[m] = n;
             }
         }
-        float q16[16];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (valid) x = __ldcg(reinterpret_cast<const float4 *>(a.qf + (size_t)b * KP + j * 16) + u);
-            q16[4 * u] = x.x; q16[4 * u + 1] = x.y; q16[4 * u + 2] = x.z; q16[4 * u + 3] = x.w;
-        }
         mbar_wait(smem_u32(bars + 12 + mt), n & 1, s_abort);                       // t of this tile is in TMEM
         if (tmg) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        // ---- epilogue 1: partial G over the 16 rows k of block j ----
-        float4 *gout = reinterpret_cast<float4 *>(a.Gx + ((size_t)(c * 2 + mt) * 128 + r) * NGP);
-        for (int n4 = 0; n4 < NGP / 4; ++n4) {
+        // ---- epilogue 1: partial G over the RB rows k of block j, four modes per pass ----
+        for (int n4 = 0; n4 < NG4; ++n4) {
             float g4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {                                       // two modes per TMEM wait
-                const int nl = n4 * 4 + 2 * h;
-                uint32_t v0[16], v1[16];
-                if (nl < NG) tmem_ld16_nowait(taddr0 + nl * 16, v0);
-                if (nl + 1 < NG) tmem_ld16_nowait(taddr0 + (nl + 1) * 16, v1);
-                tmem_ld_wait();
+            for (int u = 0; u < 4; ++u) {
+                const int nl = 4 * n4 + u;
+                if (nl < NG) {
+                    uint32_t v0[16], v1[16];
+                    if (!(a.dbg & 2)) {
+                    tmem_ld16_nowait(taddr0 + nl * RB, v0);
+                    if (nch > 1) tmem_ld16_nowait(taddr0 + nl * RB + 16, v1);
+                    tmem_ld_wait();
+                    } else {
 #pragma unroll
-                for (int kk = 0; kk < 16; ++kk) {
-                    if (nl < NG) g4[2 * h] = fmaf(q16[kk], __uint_as_float(v0[kk]), g4[2 * h]);
-                    if (nl + 1 < NG) g4[2 * h + 1] = fmaf(q16[kk], __uint_as_float(v1[kk]), g4[2 * h + 1]);
+                        for (int kk = 0; kk < 16; ++kk) { v0[kk] = 0; v1[kk] = 0; }
+                    }
+#pragma unroll
+                    for (int kk = 0; kk < 16; ++kk)
+                        if (kk < RB) g4[u] = fmaf(qb[kk], __uint_as_float(v0[kk]), g4[u]);
+                    if (nch > 1) {
+#pragma unroll
+                        for (int kk = 0; kk < 16; ++kk)
+                            if (16 + kk < RB) g4[u] = fmaf(qb[16 + kk], __uint_as_float(v1[kk]), g4[u]);
+                    }
                 }
             }
-            gout[n4] = make_float4(g4[0], g4[1], g4[2], g4[3]);
+            st_tagged4(grow + 4 * n4, g4[0], g4[1], g4[2], g4[3], tag);                   // G hop, send side
         }
-        bar_named(bar_id, 128);
-        if (r == 0) set_flag(a.gflag + c * 2 + mt, ep);
         if (tmg) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; }
-        if (r < 32) poll_flags_strided(a.gflag + (i * NKB) * 2 + mt, 2, r, NKB, ep, s_abort);
-        bar_named(bar_id, 128);
-        if (tmg) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; }
         float eta[16];
 #pragma unroll
         for (int u = 0; u < 16; ++u) eta[u] = 0.f;
-        {   // sum over the k blocks in fixed order (deterministic); 8 partial rows in flight per batch
-            const float4 *gp0 = reinterpret_cast<const float4 *>(a.Gx + ((size_t)((i * NKB) * 2 + mt) * 128 + r) * NGP);
-            const size_t gstride = (size_t)2 * 128 * NGP / 4;                       // float4 between consecutive k blocks
+        {
+            // ---- G hop, receive side: gather the partial rows of all k blocks of this mode group ----
 #pragma unroll
             for (int n4 = 0; n4 < 4; ++n4)
-                if (n4 < NGP / 4)
-                    for (int jj0 = 0; jj0 < NKB; jj0 += 8) {
-                        float4 x[8];
+                if (n4 < NG4)
+                    for (int jj0 = 0; jj0 < NKB; jj0 += 8) {                       // k-block order (deterministic); 8 rows in flight
+                        uint4 x[8];
+                        const int cnt = min(8, NKB - jj0);
+                        unsigned pend = cnt >= 8 ? 0xffu : ((1u << cnt) - 1u), spins = 0;
+                        if (a.dbg & 16) pend = 0;
+                        while (pend) {
 #pragma unroll
-                        for (int u = 0; u < 8; ++u) if (jj0 + u < NKB) x[u] = __ldcg(gp0 + (size_t)(jj0 + u) * gstride + n4);
+                            for (int u = 0; u < 8; ++u)
+                                if (pend >> u & 1) x[u] = ld_relaxed4(grd + (size_t)(jj0 + u) * gstride + 4 * n4);
+#pragma unroll
+                            for (int u = 0; u < 8; ++u)
+                                if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
+                            if (pend && (++spins & 1023u) == 0 && (*s_abort || spins > (1u << 21))) { *s_abort = 1; flow_timeout_flag = 1; break; }
+                        }
 #pragma unroll
                         for (int u = 0; u < 8; ++u)
-                            if (jj0 + u < NKB) { eta[4 * n4] += x[u].x; eta[4 * n4 + 1] += x[u].y; eta[4 * n4 + 2] += x[u].z; eta[4 * n4 + 3] += x[u].w; }
+                            if (u < cnt) {
+                                eta[4 * n4] += untag(x[u].x); eta[4 * n4 + 1] += untag(x[u].y);
+                                eta[4 * n4 + 2] += untag(x[u].z); eta[4 * n4 + 3] += untag(x[u].w);
+                            }
                     }
         }
 #pragma unroll
-        for (int u = 0; u < 16; ++u) eta[u] *= sreg[u];                             // eta_n = s_n G_n
-        if (tmg) { const long long t_ = clock64(); tm[7] += t_ - tk; tk = t_; }
-        // ---- epilogue 2: partial force over the modes n of group i ----
-        float facc[16];
+        for (int u = 0; u < 16; ++u) eta[u] *= sreg[u * 256];                             // eta_n = s_n G_n
+        if (tmg) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; }
+        // ---- epilogue 2: partial force over the modes n of group i, published as tagged words ----
+        for (int ch = 0; ch < nch; ++ch) {
+                float facc[16];
 #pragma unroll
-        for (int kk = 0; kk < 16; ++kk) facc[kk] = 0.f;
+                for (int kk = 0; kk < 16; ++kk) facc[kk] = 0.f;
 #pragma unroll
-        for (int nl = 0; nl < 16; nl += 2)
-            if (nl < NG) {
-                uint32_t v0[16], v1[16];
-                tmem_ld16_nowait(taddr0 + nl * 16, v0);
-                if (nl + 1 < NG) tmem_ld16_nowait(taddr0 + (nl + 1) * 16, v1);
-                tmem_ld_wait();
+                for (int nl = 0; nl < 16; nl += 2)
+                    if (nl < NG) {
+                        uint32_t v0[16], v1[16];
+                        if (!(a.dbg & 2)) {
+                        tmem_ld16_nowait(taddr0 + nl * RB + ch * 16, v0);
+                        if (nl + 1 < NG) tmem_ld16_nowait(taddr0 + (nl + 1) * RB + ch * 16, v1);
+                        tmem_ld_wait();
+                        } else {
 #pragma unroll
-                for (int kk = 0; kk < 16; ++kk) {
-                    facc[kk] = fmaf(eta[nl], __uint_as_float(v0[kk]), facc[kk]);
-                    if (nl + 1 < NG) facc[kk] = fmaf(eta[nl + 1], __uint_as_float(v1[kk]), facc[kk]);
-                }
+                            for (int kk = 0; kk < 16; ++kk) { v0[kk] = 0; v1[kk] = 0; }
+                        }
+#pragma unroll
+                        for (int kk = 0; kk < 16; ++kk) {
+                            facc[kk] = fmaf(eta[nl], __uint_as_float(v0[kk]), facc[kk]);
+                            if (nl + 1 < NG) facc[kk] = fmaf(eta[nl + 1], __uint_as_float(v1[kk]), facc[kk]);
+                        }
+                    }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (ch * 16 + 4 * u < RB)
+                        st_tagged4(frow + ch * 16 + 4 * u, facc[4 * u], facc[4 * u + 1], facc[4 * u + 2], facc[4 * u + 3], tag);
             }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         mbar_arrive(smem_u32(bars + 14 + mt));                                      // TMEM tile may be overwritten
-        float4 *fout = reinterpret_cast<float4 *>(a.fx + ((size_t)(i * 2 + mt) * 128 + r) * KP + j * 16);
-#pragma unroll
-        for (int u = 0; u < 4; ++u) fout[u] = make_float4(facc[4 * u], facc[4 * u + 1], facc[4 * u + 2], facc[4 * u + 3]);
-        bar_named(bar_id, 128);
-        if (r == 0) set_flag(a.fflag + c * 2 + mt, ep);
         if (tmg) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; }
-        if (r < 32) poll_flags_strided(a.fflag + j * 2 + mt, 2 * NKB, r, NGRP, ep, s_abort);
-        bar_named(bar_id, 128);
-        if (tmg) { const long long t_ = clock64(); tm[5] += t_ - tk; tk = t_; }
-        // ---- owner update: group-ordered sum of the partial forces, a5 linear update (fp64, delta form) ----
-        for (int e = r; e < nel; e += 128) {
-            const int re = r0 + (e >> 4), kk = e & 15, be = mt * 128 + re, k = j * 16 + kk;
-            if (be >= B) continue;
-            float f = 0.f;
-            {
-                const float *fp0 = a.fx + ((size_t)mt * 128 + re) * KP + k;
-                const size_t fstride = (size_t)2 * 128 * KP;
-                for (int ii0 = 0; ii0 < NGRP; ii0 += 16) {                          // group order; 16 loads in flight
-                    float x[16];
+        // ---- f hop + owner update: group-ordered sum of the partial forces, a5 linear update (fp64, delta form) ----
+        for (int e0 = r; e0 < nel; e0 += 256) {
+            int ee[2], re[2], k[2], be[2];
+            bool act[2];
+            const uint32_t *fp[2];
 #pragma unroll
-                    for (int u = 0; u < 16; ++u) if (ii0 + u < NGRP) x[u] = __ldcg(fp0 + (size_t)(ii0 + u) * fstride);
-#pragma unroll
-                    for (int u = 0; u < 16; ++u) if (ii0 + u < NGRP) f += x[u];
-                }
+            for (int h = 0; h < 2; ++h) {
+                ee[h] = e0 + 128 * h;
+                const int rr_ = ee[h] / RB, kk = ee[h] - rr_ * RB;
+                re[h] = r0 + rr_; k[h] = j * RB + kk; be[h] = mt * 128 + re[h];
+                act[h] = ee[h] < nel && be[h] < B && k[h] < a.n_q;
+                fp[h] = a.fx + ((size_t)mt * 128 + (act[h] ? re[h] : 0)) * QS + (act[h] ? k[h] : 0);
             }
-            const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
-            const int h = e >= 128 ? 1 : 0;
-            const double fd = (double)f;
-            const double rr = fast ? ccf[4 * h + 2] : a.r[co], kvv = fast ? ccf[4 * h] : a.kv[co], kqq = fast ? ccf[4 * h + 1] : a.kq[co];
-            double q = sq[e], v = sv[e];
-            if (a.traj && k < a.n_q) a.traj[((size_t)be * a.n_steps + n) * a.n_q + k] = q;
-            if (n == 0 && a.auto_start) v = (rr != 0.0) ? (fast ? ccf[4 * h + 3] : a.astart[co]) * q + a.half_T2 * fd : 0.0;
-            const double fe = a.fext ? (double)a.fext[(size_t)be * a.n_steps + n] * a.gain[(size_t)be * a.NQP + k] : 0.0;
-            v = kvv * v - kqq * q + rr * (fe - fd);
-            q += v;
-            sq[e] = q; sv[e] = v;
-            const float qfl = (float)q;
-            a.qf[(size_t)be * KP + k] = qfl;
-            const uint16_t hi = bf16_rn_dev(qfl), lo = bf16_rn_dev(qfl - __uint_as_float((uint32_t)hi << 16));
-            const int off = ((re >> 3) * 256 + (kk >> 3) * 128 + (re & 7) * 16 + (kk & 7) * 2) >> 1;
-            Qt[off] = hi; Qt[2048 + off] = lo;
+            float f[2] = {0.f, 0.f};
+            for (int ii0 = 0; ii0 < NGRP; ii0 += MMA_FB) {                          // group order (deterministic)
+                uint32_t x[2][MMA_FB];
+                const int cnt = min(MMA_FB, NGRP - ii0);
+                const unsigned full = (1u << cnt) - 1u;
+                unsigned pend0 = act[0] ? full : 0u, pend1 = act[1] ? full : 0u, spins = 0;
+                if (a.dbg & 32) pend0 = pend1 = 0;
+                while (pend0 | pend1) {
+#pragma unroll
+                    for (int u = 0; u < MMA_FB; ++u) {
+                        if (pend0 >> u & 1) x[0][u] = ld_relaxed1(fp[0] + (size_t)(ii0 + u) * fstride);
+                        if (pend1 >> u & 1) x[1][u] = ld_relaxed1(fp[1] + (size_t)(ii0 + u) * fstride);
+                    }
+#pragma unroll
+                    for (int u = 0; u < MMA_FB; ++u) {
+                        if ((pend0 >> u & 1) && (x[0][u] & 3u) == tag) pend0 &= ~(1u << u);
+                        if ((pend1 >> u & 1) && (x[1][u] & 3u) == tag) pend1 &= ~(1u << u);
+                    }
+                    if ((pend0 | pend1) && (++spins & 1023u) == 0 && (*s_abort || spins > (1u << 21))) { *s_abort = 1; flow_timeout_flag = 1; break; }
+                }
+#pragma unroll
+                for (int u = 0; u < MMA_FB; ++u)
+                    if (u < cnt) {
+                        if (act[0]) f[0] += untag(x[0][u]);
+                        if (act[1]) f[1] += untag(x[1][u]);
+                    }
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (!act[h]) continue;
+                const int e = ee[h];
+                const size_t co = (size_t)(a.coeff_stride_q ? be[h] : 0) * a.NQP + k[h];
+                const double fd = (double)f[h], rr = csm ? sr[e] : a.r[co], kvv = csm ? skv[e] : a.kv[co], kqq = csm ? skq[e] : a.kq[co];
+                double q = sq[e], v = sv[e];
+                if (a.traj) a.traj[((size_t)be[h] * a.n_steps + n) * a.n_q + k[h]] = q;
+                if (n == 0 && a.auto_start)
+                    v = (rr != 0.0) ? a.astart[co] * q + a.half_T2 * fd : 0.0;
+                const double fe = a.fext ? (double)a.fext[(size_t)be[h] * a.n_steps + n] * a.gain[(size_t)be[h] * a.NQP + k[h]] : 0.0;
+                v = kvv * v - kqq * q + rr * (fe - fd);
+                q += v;
+                sq[e] = q; sv[e] = v;
+                const float qfl = (float)q;
+                a.qf[(size_t)be[h] * QS + k[h]] = qfl;
+                const uint16_t hi = bf16_rn_dev(qfl), lo = bf16_rn_dev(qfl - __uint_as_float((uint32_t)hi << 16));
+                const int k16 = k[h] & 15;
+                const int off = ((re[h] >> 3) * 256 + (k16 >> 3) * 128 + (re[h] & 7) * 16 + (k16 & 7) * 2) >> 1;
+                uint16_t *Qc = Qt + (size_t)(k[h] >> 4) * 4096;
+                if (!(a.dbg & 8)) { Qc[off] = hi; Qc[2048 + off] = lo; }
+            }
         }
-        bar_named(bar_id, 128);
-        if (r == 0) set_flag(a.qflag + c * 2 + mt, ep + 1u);
+        if (tmg) { const long long t_ = clock64(); tm[5] += t_ - tk; tk = t_; }
+        __syncwarp();
+        if (lane == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * 4 + (r >> 5), (unsigned)n + 2u);
         if (tmg) { const long long t_ = clock64(); tm[6] += t_ - tk; tk = t_; }
     }
     if (lane == 0)
         for (int m = gw, b2 = c + gw * a.G; b2 < B; m += 4, b2 += 4 * a.G)
             if (b2 / 128 == mt) a.first_bad[b2] = sbad[m];
-    (void)cq;
 }
 
 __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
@@ -339,22 +419,20 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     extern __shared__ __align__(128) unsigned char mma_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int c = blockIdx.x, i = c / a.NKB, j = c - i * a.NKB;
-    const MmaSmem L = mma_smem_layout(a.slab_bytes, a.NGRP);
+    const MmaSmem L = mma_smem_layout(a.slab_bytes, a.nel_max);
     uint64_t *bars = reinterpret_cast<uint64_t *>(mma_smem + L.bars);      // full[0..5] empty[6..11] acc_full[12,13]
-    uint32_t *tptr = reinterpret_cast<uint32_t *>(bars + 20);              // acc_empty[14,15] qready[16,17] pick_done[18]
+    uint32_t *tptr = reinterpret_cast<uint32_t *>(bars + 20);              // acc_empty[14,15] qready[16,17]
     volatile int *s_abort = reinterpret_cast<volatile int *>(bars + 21);
-    double *sq = reinterpret_cast<double *>(mma_smem + L.sq), *sv = reinterpret_cast<double *>(mma_smem + L.sv);
+    double *own = reinterpret_cast<double *>(mma_smem + L.own);
     int *sbad = reinterpret_cast<int *>(mma_smem + L.sbad);
     unsigned char *cst = mma_smem + L.cst;
     unsigned char *slab = mma_smem + L.slab, *ring = mma_smem + L.ring;
-    const int nel_max = mma_nel_max(a.NGRP);
 
     if (tid == 0) {
         for (int s = 0; s < MMA_NSTG; ++s) { mbar_init(smem_u32(bars + s), 1); mbar_init(smem_u32(bars + 6 + s), 1); }
         for (int m = 0; m < 2; ++m) {
             mbar_init(smem_u32(bars + 12 + m), 1); mbar_init(smem_u32(bars + 14 + m), 128); mbar_init(smem_u32(bars + 16 + m), 1);
         }
-        mbar_init(smem_u32(bars + 18), 2);
         *s_abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -373,19 +451,29 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tbase = *tptr;
-    const int MT = a.MT, KC = a.KC, NC = a.NC;
+    const int MT = a.MT, KC = a.KC, NC = a.NC, KCX = (a.dbg & 1) ? 1 : a.KC;
 
+    const int kc0 = c % KC;                        // K chunks are walked from a per-CTA offset: spreads the q reads over the L2 slices
+    if (warp >= 4) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+        const int mt = (warp - 4) >> 2, gw = warp & 3;
+        if (mt < MT)
+            mma_epilogue_group(a, mt, c, i, j, (warp & 3) * 32 + lane, bars, own + (size_t)mt * (mma_own_bytes(a.nel_max) / 8) * a.nel_max,
+                               tbase, s_abort, (warp & 3) * 32, sbad, gw, lane, reinterpret_cast<float *>(cst) + (tid - 128));
+    } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
     if (warp == 0) {
         // ---------------- producer: wait for q^n of a tile, stream it through the ring by TMA ----------
         int stage = 0; unsigned ph = 0;
         for (int n = 0; n < a.n_steps; ++n)
             for (int mt = 0; mt < MT; ++mt) {
-                poll_flags_strided(a.qflag + mt, 2, lane, a.G, (unsigned)n + 1u, s_abort);
+                poll_flags4(a.qflag + (size_t)mt * a.G * 4, lane, a.G, (unsigned)n + 1u, s_abort);
                 __syncwarp();
                 if (lane == 0) {
                     mbar_arrive(smem_u32(bars + 16 + mt));
                     asm volatile("fence.proxy.async.global;" ::: "memory");
-                    for (int kc = 0; kc < KC; ++kc) {
+                    for (int kx = 0; kx < KCX; ++kx) {
+                        const int kc = kx + kc0 < KC ? kx + kc0 : kx + kc0 - KC;
                         mbar_wait(smem_u32(bars + 6 + stage), ph ^ 1, s_abort);
                         mbar_expect_tx(smem_u32(bars + stage), 8192);
                         tma_bulk_g2s(smem_u32(ring + stage * 8192), a.Qg + ((size_t)mt * KC + kc) * 4096, 8192, smem_u32(bars + stage));
@@ -404,13 +492,14 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                     mbar_wait(smem_u32(bars + 14 + mt), (n & 1) ^ 1, s_abort);              // epilogues of step n-1 left the tile
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint32_t td = tbase + (uint32_t)(mt * NC);
-                    for (int kc = 0; kc < KC; ++kc) {
+                    for (int kx = 0; kx < KCX; ++kx) {
+                        const int kc = kx + kc0 < KC ? kx + kc0 : kx + kc0 - KC;
                         mbar_wait(smem_u32(bars + stage), ph, s_abort);
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t qa = smem_u32(ring + stage * 8192), hb = smem_u32(slab + (size_t)kc * 2 * NC * 32);
                         const uint64_t qhi = umma_desc(qa), qlo = umma_desc(qa + 4096);
                         const uint64_t hhi = umma_desc(hb), hlo = umma_desc(hb + NC * 32);
-                        umma_bf16(td, qhi, hhi, idesc, kc > 0);
+                        umma_bf16(td, qhi, hhi, idesc, kx > 0);
                         umma_bf16(td, qlo, hhi, idesc, 1);
                         umma_bf16(td, qhi, hlo, idesc, 1);
                         umma_commit(smem_u32(bars + 6 + stage));                           // ring slot free when these MMAs retire
@@ -419,11 +508,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                     umma_commit(smem_u32(bars + 12 + mt));                                 // t of tile mt complete
                 }
         }
-    } else {
-        const int mt = (warp - 2) >> 2, gw = (warp - 2) & 3;
-        if (mt < MT)
-            mma_epilogue_group(a, mt, c, i, j, (warp & 3) * 32 + lane, bars, sq + (size_t)mt * nel_max, sv + (size_t)mt * nel_max,
-                               tbase, s_abort, (warp & 3) * 32, sbad, gw, lane, cst + (size_t)(tid - 64) * 128);
+    }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
