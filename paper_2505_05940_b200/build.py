@@ -16,7 +16,7 @@ DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "host_math.hpp"
 def nvcc_cmd(out: str, extra=()):
     return ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
             "-shared", "-Xcompiler", "-fPIC",
-            "--expt-relaxed-constexpr", *extra, "-o", out, *SOURCES]
+            "--expt-relaxed-constexpr", *os.environ.get("MODAL_NVCC_FLAGS", "").split(), *extra, "-o", out, *SOURCES]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

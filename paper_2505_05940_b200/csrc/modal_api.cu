@@ -633,7 +633,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr;
             a.first_bad = p->dbad.as<int>() + b0;
             a.Qg = m.dQg.as<uint16_t>(); a.qf = m.dqf.as<float>(); a.Gx = m.dGx.as<uint32_t>(); a.fx = m.dfx.as<uint32_t>();
-            a.qflag = m.dflags.as<unsigned>(); a.dbg = env_int("MODAL_MMA_DBG", 0);
+            a.qflag = m.dflags.as<unsigned>();
             // exchange buffers start at tag / epoch 0 (the first step uses 1)
             CU(cudaMemsetAsync(m.dQg.p, 0, (size_t)2 * L.KC * 8192, st));
             CU(cudaMemsetAsync(m.dqf.p, 0, (size_t)256 * L.QS * 4, st));

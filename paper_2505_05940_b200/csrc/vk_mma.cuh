@@ -33,7 +33,7 @@ namespace modal_dev {
 constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
 constexpr int MMA_THREADS = 384;     // warpgroup 0: warp 0 TMA producer, warp 1 MMA issuer (40 registers after setmaxnreg);
                                      // warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (232 registers)
-constexpr int MMA_FB = 16;           // partial-force words in flight per owned element while polling
+constexpr int MMA_FB = 20;           // partial-force words in flight per owned element while polling
 
 struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H
@@ -54,9 +54,8 @@ struct MmaArgs {
     float *qf;                  // [256][QS]            q fp32
     uint32_t *Gx;               // [G][2][128][4*NG4]   partial G, tagged
     uint32_t *fx;               // [NGRP][2][128][QS]   partial f, tagged
-    unsigned *qflag;            // [2][G][4] epochs, one per (tile, CTA, epilogue warp)
+    unsigned *qflag;            // [2][G] epochs, one per (tile, CTA)
     long long *timing;          // optional [G][8] cycle counters of tile 0 (MODAL_FLOW_TIMING)
-    int dbg;                    // MODAL_MMA_DBG: timing experiments that break the results (0 in production)
 };
 
 __device__ __forceinline__ void set_flag(unsigned *p, unsigned epoch)
@@ -89,28 +88,24 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&u)[1
                  : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// The G uint4 flag groups p[0 .. G): relaxed 16-byte loads, all of a lane in flight together (one L2 round trip
-// per poll round), then ONE acquire fence once every word has reached the epoch.
-__device__ __forceinline__ void poll_flags4(const unsigned *p, int lane, int count, unsigned epoch, volatile int *abortp)
+// The flags p[0 .. count), each polled with ld.acquire.gpu (a separate fence.acq_rel.gpu after relaxed polls
+// measured slower: the MEMBAR stalls the epilogue warps of the other tile).
+__device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int count, unsigned epoch, volatile int *abortp)
 {
     for (int base = lane; base < count; base += 256) {
         unsigned pend = 0, spins = 0;
 #pragma unroll
         for (int u = 0; u < 8; ++u) if (base + 32 * u < count) pend |= 1u << u;
         while (pend) {
-            uint4 v[8];
+            unsigned v[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u)
-                if (pend >> u & 1)
-                    asm volatile("ld.relaxed.gpu.global.v4.b32 {%0,%1,%2,%3}, [%4];"
-                                 : "=r"(v[u].x), "=r"(v[u].y), "=r"(v[u].z), "=r"(v[u].w) : "l"(p + (size_t)(base + 32 * u) * 4) : "memory");
+                if (pend >> u & 1) asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + base + 32 * u) : "memory");
 #pragma unroll
-            for (int u = 0; u < 8; ++u)
-                if ((pend >> u & 1) && v[u].x >= epoch && v[u].y >= epoch && v[u].z >= epoch && v[u].w >= epoch) pend &= ~(1u << u);
+            for (int u = 0; u < 8; ++u) if ((pend >> u & 1) && v[u] >= epoch) pend &= ~(1u << u);
             if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
         }
     }
-    asm volatile("fence.acq_rel.gpu;" ::: "memory");
 }
 __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
 {
@@ -202,8 +197,8 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
         sq[e] = q; sv[e] = v;
         if (csm) { skv[e] = kv; skq[e] = kq; sr[e] = rc; }
     }
-    __syncwarp();
-    if (lane == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * 4 + (r >> 5), 1u);
+    bar_named(2 + mt, 128);
+    if (r == 0) set_flag(a.qflag + (size_t)mt * a.G + c, 1u);
     for (int u = 0; u < 16; ++u) sreg[u * 256] = (u < NG && n0 + u < a.n_phi) ? sb[n0 + u] : 0.f;   // [16][256]: conflict-free
 
     const uint32_t taddr0 = tbase + ((uint32_t)lane_base << 16) + (uint32_t)(mt * NC);
@@ -230,7 +225,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
             qb[4 * u] = x.x; qb[4 * u + 1] = x.y; qb[4 * u + 2] = x.z; qb[4 * u + 3] = x.w;
         }
         // ---- a1 pickup + a6 write-out: out[b][n] = w . q^n for the samples b = c, c+G, ... of this tile ----
-        for (int m = gw, b2 = c + gw * a.G; b2 < B && !(a.dbg & 4); m += 4, b2 += 4 * a.G) {
+        for (int m = gw, b2 = c + gw * a.G; b2 < B; m += 4, b2 += 4 * a.G) {
             if (b2 / 128 != mt) continue;
             const float *wb = a.w + (size_t)(a.coeff_stride_q ? b2 : 0) * a.NQP;
             float o = 0.f, nrm = 0.f;
@@ -256,14 +251,9 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 const int nl = 4 * n4 + u;
                 if (nl < NG) {
                     uint32_t v0[16], v1[16];
-                    if (!(a.dbg & 2)) {
                     tmem_ld16_nowait(taddr0 + nl * RB, v0);
                     if (nch > 1) tmem_ld16_nowait(taddr0 + nl * RB + 16, v1);
                     tmem_ld_wait();
-                    } else {
-#pragma unroll
-                        for (int kk = 0; kk < 16; ++kk) { v0[kk] = 0; v1[kk] = 0; }
-                    }
 #pragma unroll
                     for (int kk = 0; kk < 16; ++kk)
                         if (kk < RB) g4[u] = fmaf(qb[kk], __uint_as_float(v0[kk]), g4[u]);
@@ -283,27 +273,31 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
         {
             // ---- G hop, receive side: gather the partial rows of all k blocks of this mode group ----
 #pragma unroll
-            for (int n4 = 0; n4 < 4; ++n4)
-                if (n4 < NG4)
-                    for (int jj0 = 0; jj0 < NKB; jj0 += 8) {                       // k-block order (deterministic); 8 rows in flight
-                        uint4 x[8];
+            for (int m = 0; m < 2; ++m)                                           // two float4 columns of the rows per batch
+                if (2 * m < NG4)
+                    for (int jj0 = 0; jj0 < NKB; jj0 += 8) {                        // k-block order (deterministic); 8 + 8 loads in flight
+                        uint4 x[16];
                         const int cnt = min(8, NKB - jj0);
-                        unsigned pend = cnt >= 8 ? 0xffu : ((1u << cnt) - 1u), spins = 0;
-                        if (a.dbg & 16) pend = 0;
+                        const unsigned lo8 = cnt >= 8 ? 0xffu : ((1u << cnt) - 1u);
+                        unsigned pend = lo8 | (2 * m + 1 < NG4 ? lo8 << 8 : 0u), spins = 0;
                         while (pend) {
 #pragma unroll
-                            for (int u = 0; u < 8; ++u)
-                                if (pend >> u & 1) x[u] = ld_relaxed4(grd + (size_t)(jj0 + u) * gstride + 4 * n4);
+                            for (int u = 0; u < 16; ++u)
+                                if (pend >> u & 1) x[u] = ld_relaxed4(grd + (size_t)(jj0 + (u & 7)) * gstride + 4 * (2 * m + (u >> 3)));
 #pragma unroll
-                            for (int u = 0; u < 8; ++u)
+                            for (int u = 0; u < 16; ++u)
                                 if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
                             if (pend && (++spins & 1023u) == 0 && (*s_abort || spins > (1u << 21))) { *s_abort = 1; flow_timeout_flag = 1; break; }
                         }
 #pragma unroll
                         for (int u = 0; u < 8; ++u)
                             if (u < cnt) {
-                                eta[4 * n4] += untag(x[u].x); eta[4 * n4 + 1] += untag(x[u].y);
-                                eta[4 * n4 + 2] += untag(x[u].z); eta[4 * n4 + 3] += untag(x[u].w);
+                                eta[8 * m] += untag(x[u].x); eta[8 * m + 1] += untag(x[u].y);
+                                eta[8 * m + 2] += untag(x[u].z); eta[8 * m + 3] += untag(x[u].w);
+                                if (2 * m + 1 < NG4) {
+                                    eta[8 * m + 4] += untag(x[u + 8].x); eta[8 * m + 5] += untag(x[u + 8].y);
+                                    eta[8 * m + 6] += untag(x[u + 8].z); eta[8 * m + 7] += untag(x[u + 8].w);
+                                }
                             }
                     }
         }
@@ -319,14 +313,9 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 for (int nl = 0; nl < 16; nl += 2)
                     if (nl < NG) {
                         uint32_t v0[16], v1[16];
-                        if (!(a.dbg & 2)) {
                         tmem_ld16_nowait(taddr0 + nl * RB + ch * 16, v0);
                         if (nl + 1 < NG) tmem_ld16_nowait(taddr0 + (nl + 1) * RB + ch * 16, v1);
                         tmem_ld_wait();
-                        } else {
-#pragma unroll
-                            for (int kk = 0; kk < 16; ++kk) { v0[kk] = 0; v1[kk] = 0; }
-                        }
 #pragma unroll
                         for (int kk = 0; kk < 16; ++kk) {
                             facc[kk] = fmaf(eta[nl], __uint_as_float(v0[kk]), facc[kk]);
@@ -360,7 +349,6 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 const int cnt = min(MMA_FB, NGRP - ii0);
                 const unsigned full = (1u << cnt) - 1u;
                 unsigned pend0 = act[0] ? full : 0u, pend1 = act[1] ? full : 0u, spins = 0;
-                if (a.dbg & 32) pend0 = pend1 = 0;
                 while (pend0 | pend1) {
 #pragma unroll
                     for (int u = 0; u < MMA_FB; ++u) {
@@ -401,12 +389,12 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 const int k16 = k[h] & 15;
                 const int off = ((re[h] >> 3) * 256 + (k16 >> 3) * 128 + (re[h] & 7) * 16 + (k16 & 7) * 2) >> 1;
                 uint16_t *Qc = Qt + (size_t)(k[h] >> 4) * 4096;
-                if (!(a.dbg & 8)) { Qc[off] = hi; Qc[2048 + off] = lo; }
+                Qc[off] = hi; Qc[2048 + off] = lo;
             }
         }
         if (tmg) { const long long t_ = clock64(); tm[5] += t_ - tk; tk = t_; }
-        __syncwarp();
-        if (lane == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * 4 + (r >> 5), (unsigned)n + 2u);
+        bar_named(2 + mt, 128);
+        if (r == 0) set_flag(a.qflag + (size_t)mt * a.G + c, (unsigned)n + 2u);
         if (tmg) { const long long t_ = clock64(); tm[6] += t_ - tk; tk = t_; }
     }
     if (lane == 0)
@@ -451,7 +439,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tbase = *tptr;
-    const int MT = a.MT, KC = a.KC, NC = a.NC, KCX = (a.dbg & 1) ? 1 : a.KC;
+    const int MT = a.MT, KC = a.KC, NC = a.NC;
 
     const int kc0 = c % KC;                        // K chunks are walked from a per-CTA offset: spreads the q reads over the L2 slices
     if (warp >= 4) {
@@ -467,12 +455,12 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
         int stage = 0; unsigned ph = 0;
         for (int n = 0; n < a.n_steps; ++n)
             for (int mt = 0; mt < MT; ++mt) {
-                poll_flags4(a.qflag + (size_t)mt * a.G * 4, lane, a.G, (unsigned)n + 1u, s_abort);
+                poll_flags(a.qflag + (size_t)mt * a.G, lane, a.G, (unsigned)n + 1u, s_abort);
                 __syncwarp();
                 if (lane == 0) {
                     mbar_arrive(smem_u32(bars + 16 + mt));
                     asm volatile("fence.proxy.async.global;" ::: "memory");
-                    for (int kx = 0; kx < KCX; ++kx) {
+                    for (int kx = 0; kx < KC; ++kx) {
                         const int kc = kx + kc0 < KC ? kx + kc0 : kx + kc0 - KC;
                         mbar_wait(smem_u32(bars + 6 + stage), ph ^ 1, s_abort);
                         mbar_expect_tx(smem_u32(bars + stage), 8192);
@@ -492,7 +480,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                     mbar_wait(smem_u32(bars + 14 + mt), (n & 1) ^ 1, s_abort);              // epilogues of step n-1 left the tile
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint32_t td = tbase + (uint32_t)(mt * NC);
-                    for (int kx = 0; kx < KCX; ++kx) {
+                    for (int kx = 0; kx < KC; ++kx) {
                         const int kc = kx + kc0 < KC ? kx + kc0 : kx + kc0 - KC;
                         mbar_wait(smem_u32(bars + stage), ph, s_abort);
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
