@@ -430,6 +430,30 @@ def assemble(wl: dict, samples=None, *, scheme=SV, lossless=False, round_fp32=Tr
             for k, v in zip(rows, (om, ga, act, c1, c2, c3, w, lam, s, q0, qm1)):
                 rows[k].append(v)
         extra = {"mq": mq, "nq": nq, "mphi": mphi, "nphi": nphi}
+    elif wl["model"] == "berger":
+        # Berger plate: tension modulation (Eq. 8) on the rectangular sine basis with
+        # tau_membrane of PAPER.md:85 (Eq. 4), per unit mass rho h (reading R3)
+        model, Nphi = TENSION, 0
+        ref = wl["ref"]
+        mq, nq, _ = rect_modes(ref["Lx"], ref["Ly"], Nq)
+        for b in samples:
+            Lx, Ly, h = wl["Lx"][b], wl["Ly"][b], wl["h"][b]
+            lam = rect_lambda(mq, nq, Lx, Ly)
+            om, ga = omega_gamma(lam, plate_D(wl["E"], h, wl["nu"]), wl["T0"], wl["rho"] * h, s0, s1)
+            act = active_mask(scheme, om, ga, T)
+            c = float(rnd(tau_membrane(wl["E"], h, Lx, Ly, wl["nu"]) / (wl["rho"] * h)))
+            lam_r = rnd(lam)
+            xp, yp = wl["pickup"][0] * Lx, wl["pickup"][1] * Ly
+            w = np.array([rect_mode(mq[k], nq[k], Lx, Ly, xp, yp) for k in range(Nq)])
+            w = rnd(np.where(act, w, 0.0))
+            q0 = project_bump_rect(mq, nq, Lx, Ly, wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
+            q0 = np.where(act, q0, 0.0)
+            c1, c2, c3 = scheme_coeffs(scheme, om, ga, T)
+            c3 = np.where(act, c3, 0.0)
+            qm1 = np.where(act, start_state(TENSION, q0, om, T, lam=lam_r, nl_scale=c), 0.0)
+            for k, v in zip(rows, (om, ga, act, c1, c2, c3, w, lam_r, c, q0, qm1)):
+                rows[k].append(v)
+        extra = {"mq": mq, "nq": nq}
     else:
         model = TENSION if wl["model"] == "tension" else LINEAR
         Nphi = 0

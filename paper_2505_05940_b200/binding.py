@@ -184,9 +184,9 @@ class Plan:
 def desc_from_workload(wl: dict, scheme=SV, lossless=False, max_batch=None, max_steps=None) -> PlanDesc:
     s0 = 0.0 if lossless else wl["sigma0"]
     s1 = 0.0 if lossless else wl["sigma1"]
-    if wl["model"] == "vk":
+    if wl["model"] in ("vk", "berger"):
         ref = wl["ref"]
-        return PlanDesc(model=VK, scheme=scheme, geom=RECT, bc=0, Lx=ref["Lx"], Ly=ref["Ly"], h=ref["h"],
+        return PlanDesc(model=VK if wl["model"] == "vk" else TENSION, scheme=scheme, geom=RECT, bc=0, Lx=ref["Lx"], Ly=ref["Ly"], h=ref["h"],
                         E=wl["E"], rho=wl["rho"], nu=wl["nu"], T0=wl["T0"], D=0.0, area=0.0,
                         sigma0=s0, sigma1=s1, pickup_x=wl["pickup"][0] * ref["Lx"], pickup_y=wl["pickup"][1] * ref["Ly"],
                         n_q=wl["n_q"], n_phi=wl["n_phi"], sample_rate=wl["sample_rate"],
@@ -205,14 +205,15 @@ def plan_from_workload(wl: dict, device=0, scheme=SV, lossless=False):
     plan = Plan(desc_from_workload(wl, scheme, lossless), device)
     B = wl["batch"]
     q0 = np.empty((B, wl["n_q"]))
-    if wl["model"] == "vk":
+    if wl["model"] in ("vk", "berger"):
         same = all(np.all(wl[k] == wl[k][0]) for k in ("Lx", "Ly", "h")) and \
             wl["Lx"][0] == wl["ref"]["Lx"] and wl["Ly"][0] == wl["ref"]["Ly"] and wl["h"][0] == wl["ref"]["h"]
         if not same:
             rows = [plan.derive_coeffs(Lx=wl["Lx"][b], Ly=wl["Ly"][b], h=wl["h"][b],
                                        pickup_x_frac=wl["pickup"][0], pickup_y_frac=wl["pickup"][1]) for b in range(B)]
+            lam = dict(lam=[r["lam"] for r in rows]) if wl["model"] == "berger" else {}
             plan.coeffs_upload(B, omega=[r["omega"] for r in rows], sigma=[r["sigma"] for r in rows],
-                               nl_scale=[r["nl_scale"] for r in rows], pickup=[r["pickup"] for r in rows])
+                               nl_scale=[r["nl_scale"] for r in rows], pickup=[r["pickup"] for r in rows], **lam)
         for b in range(B):
             q0[b] = plan.project_bump(wl["Lx"][b], wl["Ly"][b], wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
     else:

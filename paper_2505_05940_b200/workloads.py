@@ -11,7 +11,8 @@ one vectorised draw of ``batch`` values per parameter, in the order written
 below.  The paper's own benchmark is synthetic too (analytic plate modes, 10 /
 50 / 100 modes, 1 s at 44.1 kHz): C0 and C2 are its 10- and
 100-mode points, C1 its tension-modulated case scaled to dataset generation,
-C3 / C4 the batched and large-tensor extensions BASELINE.json asks for.
+C3 / C4 the batched and large-tensor extensions BASELINE.json asks for; ``berger`` is the paper's
+second benchmark model (tension-modulated plate) on the C0 plate.
 """
 from __future__ import annotations
 
@@ -105,8 +106,20 @@ def c1(batch=1024, n_steps=44100, n_q=200):
     return wl
 
 
+def berger(n_q=100, batch=1, n_steps=44100):
+    """Berger (tension-modulated) plate of the paper's second benchmark (Fig. 3 bottom; tau of
+    PAPER.md:85): the C0 plate with ``n_q`` modes (the paper times 10 / 50 / 100), bump 0.1 m wide, peak
+    a*h with a log-uniform in [0.2, 2] drawn from the seed."""
+    wl = _plate_common(f"berger_plate_{n_q}_b{batch}", 5, n_q, 0, n_steps, batch, dict(Lx=0.6, Ly=0.4, h=1.0e-3))
+    wl["model"] = "berger"
+    wl["bump_width"] = 0.1
+    rng = _rng(5)
+    a = np.exp(rng.uniform(np.log(0.2), np.log(2.0), batch))
+    return _fixed_plate(wl, rng, a)
+
+
 def by_name(name: str, **kw):
-    return {"c0": c0, "c1": c1, "c2": c2, "c3": c3, "c4": c4}[name](**kw)
+    return {"c0": c0, "c1": c1, "c2": c2, "c3": c3, "c4": c4, "berger": berger}[name](**kw)
 
 
 def shard(wl: dict, rank: int, world: int) -> dict:

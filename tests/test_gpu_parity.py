@@ -311,6 +311,25 @@ def test_c1_string_parity(batch, n_steps):
     check_parity(gpu, ref["out"], case, ref_bad=ref["first_bad"], gpu_bad=fb)
 
 
+@pytest.mark.parametrize("n_q,batch,n_steps", [(10, 1, 4410), (100, 6, 4410)])
+def test_berger_plate_parity(n_q, batch, n_steps):
+    """Berger (tension-modulated) plate, the model of the paper's second benchmark: fp32 kernel vs
+    the fp64 oracle, through the plan's own defaults (nothing uploaded) and with the oracle's rounded inputs."""
+    torch, mb = _mods()
+    wl = wlmod.berger(n_q=n_q, batch=batch, n_steps=n_steps)
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, n_steps)
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, n_steps)
+    assert st == 0 and np.all(fb == -1) and plan.query(mb.Q_KERNEL_INFO)[0] == 1
+    check_parity(gpu, ref["out"], case)
+    plan2, q0 = mb.plan_from_workload(wl, 0)
+    gpu2, fb2, _, st2 = gpu_run(plan2, q0, None, n_steps)
+    assert st2 == 0
+    peak = np.max(np.abs(ref["out"]), axis=1, keepdims=True)
+    assert np.max(np.abs(gpu2 - ref["out"]) / peak) <= 5e-4            # default path: fp64-exact vs fp32-rounded inputs
+
+
 def test_string_plan_defaults_and_lossless_energy():
     torch, mb = _mods()
     wl = wlmod.c1(batch=16, n_steps=8192)

@@ -140,3 +140,23 @@ def test_workloads_are_seeded_and_shaped_like_baseline_configs():
     assert (wlmod.c0()["n_steps"], wlmod.c2()["n_steps"], wlmod.c4()["n_steps"], wlmod.c3()["n_steps"]) == (11025, 44100, 4410, 22050)
     sh = wlmod.shard(wlmod.c3(batch=10), 1, 4)
     assert sh["batch"] == 3 and sh["shard"] == (2, 5) and len(sh["Lx"]) == 3
+
+
+def test_berger_plate_plan_defaults_match_oracle():
+    """Tension-modulated (Berger) plate, the paper's second benchmark model: the library's
+    default coefficients (lambda, omega, gamma, tau/(rho h), pickup) and its bump projection agree with the oracle."""
+    wl = wlmod.berger(n_q=50, batch=3, n_steps=64)
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    case = orc.assemble(wl, round_fp32=False)
+    assert np.array_equal(plan.query(mb.Q_ACTIVE).astype(bool)[0], case.active[0])
+    assert np.allclose(plan.query(mb.Q_LAMBDA), case.lam[0], rtol=1e-13)
+    assert np.allclose(plan.query(mb.Q_OMEGA)[0], case.omega[0], rtol=1e-12)
+    assert np.allclose(plan.query(mb.Q_SIGMA)[0], case.gamma[0], rtol=1e-12)
+    d = plan.derive_coeffs()
+    # tau / (rho h) with tau = E h / (2 Lx Ly (1 - nu^2)) written out from PAPER.md:85
+    tau_rho = 2.0e11 * 1e-3 / (2 * 0.6 * 0.4 * (1 - 0.09)) / (7860.0 * 1e-3)
+    assert abs(d["nl_scale"][0] / tau_rho - 1) < 1e-13 and abs(case.nl_scale[0] / tau_rho - 1) < 1e-13
+    assert np.allclose(d["pickup"], case.w[0], rtol=1e-11, atol=1e-12)
+    for b in range(3):
+        q0 = plan.project_bump(wl["Lx"][b], wl["Ly"][b], wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
+        assert np.max(np.abs(q0 - case.q0[b])) <= 1e-7 * np.max(np.abs(case.q0[b]))
