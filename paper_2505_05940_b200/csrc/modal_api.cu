@@ -433,18 +433,22 @@ bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, FlowConfig
     return c.smem <= SMEM_LIMIT;
 }
 
-// Rough cost of one time step of one team, in SM cycles (constants measured on B200).
-double flow_step_cost(int nq, int nphi, int G)
+// Rough cost of one time step of one team of G CTAs while NT teams run side by side, in SM cycles.  Calibrated on
+// B200 with MODAL_FLOW_TIMING: the pass over H costs ~1.5 k + 28 cycles per 1 KiB tile of a CTA; tiles
+// beyond the ~187 that stay in shared memory are streamed from L2, which delivers ~3.3 KB/cycle to ALL teams together;
+// the exchange phases cost 3.5 k + 70 G + 35 k / G cycles (C2: 6.3 k at G=25, 7.1 k at 50, 9.8 k at 100; C4: 15.4 k at
+// 148), plus one more hop when in-plane modes are shared between CTAs.
+double flow_step_cost(int nq, int nphi, int G, int NT)
 {
     const double tiles = (double)nphi * mh::flow_tiles_per_n(nq);
     const double per_cta = tiles / G;
-    const double issue = per_cta * 7.0;                         // ~26 warp instructions per tile, 4 issue slots
-    const double unit_chain = 150.0 + 75.0 * std::min(8.0, per_cta);   // one warp, one unit, dependent latency
-    const double resident_cap = 190.0;                          // tiles of shared memory
-    const double stream = std::max(0.0, per_cta - resident_cap) * 1024.0 / 40.0;   // ~40 B/cycle/SM from L2
+    const double pass = 1500.0 + 28.0 * per_cta;
+    const double resident_cap = 187.0;                          // tiles of shared memory
+    const double streamed = std::max(0.0, per_cta - resident_cap);
+    const double stream = (double)NT * G * streamed * 1024.0 / 3300.0;
     const bool shared_modes = !(G <= nphi && nphi % G == 0);
-    const double exchange = G == 1 ? 0.0 : (shared_modes ? 3.0 : 2.0) * 800.0;   // L2 round trips
-    return std::max(std::max(issue, unit_chain), stream) + exchange + 400.0;
+    const double exchange = G == 1 ? 0.0 : 3500.0 + 70.0 * G + 35000.0 / G + (shared_modes ? 1500.0 : 0.0);
+    return std::max(pass, stream) + exchange;
 }
 
 modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
@@ -465,9 +469,9 @@ modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
     for (int g : cand) {
         if (g < 1 || g > sm) continue;
         const double tiles_cta = (double)nphi * mh::flow_tiles_per_n(nq) / g;
-        if (force_g <= 0 && tiles_cta > 1200) continue;          // tables would not fit; skip the expensive build
+        if (force_g <= 0 && tiles_cta > 2000) continue;          // tables would not fit; skip the expensive build
         const int nt = std::max(1, std::min(batch, sm / g));
-        const double cost = std::ceil((double)batch / nt) * flow_step_cost(nq, nphi, g);
+        const double cost = std::ceil((double)batch / nt) * flow_step_cost(nq, nphi, g, nt);
         if (!bestG || cost < best * 0.999) { bestG = g; best = cost; }
     }
     if (!bestG) { p->err += "no feasible team size for the vK flow kernel\n"; return MODAL_EINCOMPAT; }

@@ -287,7 +287,7 @@ def test_vk_ftm_scheme_and_auto_start_parity():
 
 
 def test_c4_shape_whole_gpu_team_short_run():
-    wl = wlmod.c4(batch=2, n_steps=96)
+    wl = wlmod.c4(batch=1, n_steps=96)
     case = orc.assemble(wl)
     ref = orc.run_case(case, 96)
     plan = plan_with_oracle_inputs(wl, case)
@@ -296,6 +296,20 @@ def test_c4_shape_whole_gpu_team_short_run():
     info = plan.query(mb.Q_KERNEL_INFO)
     assert info[0] == 3 and info[1] > 100 and not (info[5] & 1)   # whole-GPU team, H only partly resident: streamed from L2
     check_parity(gpu, ref["out"], case, first=96)
+
+
+def test_c4_shape_batch_teams_side_by_side():
+    """C4 with a batch: several teams share the GPU (and the L2-resident H), each streaming its own pass; a ragged
+    last round (5 samples on 4 teams)."""
+    wl = wlmod.c4(batch=5, n_steps=64)
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, 64)
+    plan = plan_with_oracle_inputs(wl, case)
+    gpu, fb, _, _ = gpu_run(plan, case.q0, case.qm1, 64)
+    torch, mb = _mods()
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 3 and info[2] >= 2 and info[1] * info[2] > 100 and not (info[5] & 1)
+    check_parity(gpu, ref["out"], case, first=64)
 
 
 # ------------------------------------------------------------------ tension / linear ----
