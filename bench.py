@@ -33,6 +33,8 @@ METRIC = "von_karman_modal_sample_steps_per_s"
 UNIT = "sample-steps/s"
 # nominal FP32 pipe: 148 SMs x 128 FMA lanes x 2 flop x 1.965 GHz (guide: B200_PROFILING.md clocks)
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of one C4 batch-1 launch (4410 steps), profiles/r1_c4_b1.md
+C4_DRAM_BYTES_PER_LAUNCH = 21.12e6
 
 
 def peaks():
@@ -255,11 +257,18 @@ def main():
             roof = tensor_roofline(wl, B, n_steps, per_launch, bf16_peak, peak_src)
         elif wl["model"] == "vk":
             ach = hbytes * n_steps / per_launch / 1e9
+            tiles, nz = (int(x) for x in plan.query(mb.Q_TILE_STATS))
+            read = nz * 1024 * n_steps / per_launch / 1e9
             roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
-                    "traffic": 68.72e6 if (wl["name"], n_steps) == ("c4_vk_400x200_b1", 4410) else None,
+                    "traffic": C4_DRAM_BYTES_PER_LAUNCH if (wl["name"], n_steps) == ("c4_vk_400x200_b1", 4410) else None,
                     "peak_source": peak_src, "kernel": "vk_flow_kernel",
-                    "note": "algorithmic bytes = 4*n_phi*n_q(n_q+1)/2 per time step, once per step for the whole batch; "
-                            "traffic = dram read+write bytes of one launch (profiles/r1_c4_b1.md): H is read from HBM once and then served by L2"}
+                    "tiles": tiles, "tiles_nonzero": nz, "achieved_read": read, "frac_read": read / hbm_peak,
+                    "note": "achieved = ALGORITHMIC bytes (SURVEY.md 8(d): the dense packed tensor, 4*n_phi*n_q(n_q+1)/2 per time step, "
+                            "once per step for the whole batch) / time.  The kernel keeps the modes grouped by index parity and never "
+                            "reads the 16x16 tiles that hold only parity zeros (tiles_nonzero of tiles, SURVEY.md 8(f) row 4), so it can "
+                            "exceed the dense-traffic roofline; achieved_read / frac_read count the bytes it does read per step (most "
+                            "of them from shared memory, where they stay resident).  traffic = dram read+write bytes of one launch "
+                            "(profiles/r1_c4_b1.md): H crosses the HBM pins once per launch"}
         else:
             ach = flops * B * n_steps / per_launch / 1e12
             roof = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP32_PEAK_TFLOPS,

@@ -136,7 +136,12 @@ typedef enum {
     MODAL_Q_ACTIVE = 9,      /* int    [coeff_batch][n_q]   1 = active, 0 = masked (R11)            */
     MODAL_Q_H_FULL = 10,     /* double [n_phi][n_q][n_q]: the fp32 values the device holds, widened */
     MODAL_Q_COEFF_BATCH = 11,/* int    [1]                                                          */
-    MODAL_Q_KERNEL_INFO = 12 /* int    [8]: kernel family, cluster size, clusters, threads, smem    */
+    MODAL_Q_KERNEL_INFO = 12,/* int    [8]: kernel family, cluster size, clusters, threads, smem    */
+    MODAL_Q_TILE_STATS = 13  /* int    [2]: 16x16 tiles of the packed H, and how many hold a non-zero.   */
+                             /*        The device keeps the transverse modes grouped by index parity   */
+                             /*        (internal order only: every array of this API is in plan order),*/
+                             /*        so that the parity zeros of H fill whole  */
+                             /*        tiles, which the step kernel never reads.                       */
                              /*        bytes, resident flag, tiles per n, padded n_q (last launch)  */
 } modal_query;
 /* Copies the item into `dst` (capacity `dst_bytes`); returns MODAL_EINVAL if it does not fit. */

@@ -19,7 +19,7 @@ LINEAR, TENSION, VK = 0, 1, 2
 SV, FTM = 0, 1
 STRING, RECT = 0, 1
 (Q_MODE_M, Q_MODE_N, Q_PHI_M, Q_PHI_N, Q_LAMBDA, Q_OMEGA, Q_SIGMA, Q_NL_SCALE, Q_PICKUP, Q_ACTIVE,
- Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO) = range(13)
+ Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO, Q_TILE_STATS) = range(14)
 
 _dp = C.POINTER(C.c_double)
 _fp = C.POINTER(C.c_float)
@@ -158,7 +158,7 @@ class Plan:
             Q_LAMBDA: ((nq,), np.float64), Q_OMEGA: ((cb, nq), np.float64), Q_SIGMA: ((cb, nq), np.float64),
             Q_NL_SCALE: ((cb, nnl), np.float64), Q_PICKUP: ((cb, nq), np.float64),
             Q_ACTIVE: ((cb, nq), np.int32), Q_H_FULL: ((nphi, nq, nq), np.float64),
-            Q_COEFF_BATCH: ((1,), np.int32), Q_KERNEL_INFO: ((8,), np.int32)}[what]
+            Q_COEFF_BATCH: ((1,), np.int32), Q_KERNEL_INFO: ((8,), np.int32), Q_TILE_STATS: ((2,), np.int32)}[what]
         a = np.zeros(shape, dt)
         self._check(lib.modal_plan_query(self._h, what, a.ctypes.data_as(C.c_void_p), a.nbytes))
         return a

@@ -90,7 +90,9 @@ struct FlowSchedule {
     std::vector<int> cta_tiles;           // [G] tiles per CTA
 };
 
-inline FlowSchedule build_flow_schedule(int n_q, int n_phi, int G, int NW, int slot_tiles)
+// tile_nz: optional [n_phi * tpn] flags, 0 = the tile holds only zeros and is left out of the schedule (it is never read:
+// with the modes grouped by index parity ~70 % of the tiles of the sine-basis tensor vanish).
+inline FlowSchedule build_flow_schedule(int n_q, int n_phi, int G, int NW, int slot_tiles, const std::vector<uint8_t> *tile_nz = nullptr)
 {
     FlowSchedule s;
     s.G = G; s.NW = NW; s.slot_tiles = slot_tiles;
@@ -100,19 +102,56 @@ inline FlowSchedule build_flow_schedule(int n_q, int n_phi, int G, int NW, int s
     std::vector<Atom> atoms;
     for (int n = 0; n < n_phi; ++n)
         for (int I = 0; I < nt; ++I) {
-            const int len = I + 1, parts = (len + slot_tiles - 1) / slot_tiles;
-            for (int p = 0, j = 0; p < parts; ++p) {
-                const int l = len / parts + (p < len % parts ? 1 : 0);
-                atoms.push_back({n, I, j, l});
-                j += l;
+            // maximal runs of non-zero tiles of this tile row, each cut into parts of <= slot_tiles tiles
+            for (int J = 0; J <= I;) {
+                auto nz = [&](int jj) { return !tile_nz || (*tile_nz)[(size_t)n * tpn + I * (I + 1) / 2 + jj] != 0; };
+                if (!nz(J)) { ++J; continue; }
+                int e = J;
+                while (e <= I && nz(e)) ++e;
+                const int len = e - J, parts = (len + slot_tiles - 1) / slot_tiles;
+                for (int p = 0, j = J; p < parts; ++p) {
+                    const int l = len / parts + (p < len % parts ? 1 : 0);
+                    atoms.push_back({n, I, j, l});
+                    j += l;
+                }
+                J = e;
             }
         }
     const double unit_overhead = 1.5;     // tile-equivalents of per-unit epilogue work
     double total = 0;
     for (const Atom &a : atoms) total += a.ntl + unit_overhead;
-    // contiguous partition by cumulative cost
     std::vector<int> first(G + 1, 0);
-    {
+    // (a) whole in-plane modes per CTA (no mode is shared, so phase B1 needs no exchange): longest-processing-time
+    //     assignment of the modes; taken when its most loaded CTA stays within 10 % of the ideal share
+    bool whole_modes = false;
+    if (G > 1 && G <= n_phi) {
+        std::vector<double> cost(n_phi, 0.0);
+        for (const Atom &a : atoms) cost[a.n] += a.ntl + unit_overhead;
+        std::vector<int> order(n_phi);
+        for (int n = 0; n < n_phi; ++n) order[n] = n;
+        std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return cost[x] > cost[y]; });
+        std::vector<double> load(G, 0.0);
+        std::vector<int> owner(n_phi, 0);
+        for (int n : order) {
+            const int c = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+            owner[n] = c; load[c] += cost[n];
+        }
+        if (*std::max_element(load.begin(), load.end()) <= 1.10 * total / G) {
+            whole_modes = true;
+            std::vector<Atom> sorted;
+            sorted.reserve(atoms.size());
+            for (int c = 0; c < G; ++c) {
+                first[c] = (int)sorted.size();
+                for (int n = 0; n < n_phi; ++n)
+                    if (owner[n] == c)
+                        for (const Atom &a : atoms) if (a.n == n) sorted.push_back(a);
+            }
+            first[G] = (int)sorted.size();
+            atoms.swap(sorted);
+        }
+    }
+    // (b) otherwise: contiguous partition of the units by cumulative cost (modes may be shared between CTAs)
+    if (!whole_modes) {
         double acc = 0; int c = 1;
         for (size_t i = 0; i < atoms.size(); ++i) {
             const double mid = acc + 0.5 * (atoms[i].ntl + unit_overhead);

@@ -75,12 +75,17 @@ struct modal_plan {
     std::vector<double> omega, sigma, nl_scale, lambda_s, pickup;   // [coeff_batch][...]
     std::vector<int> active;                                          // [coeff_batch][n_q]
     std::vector<float> Ht;                                            // tile-packed H (VK, team kernel)
-    std::vector<float> Hf;                                            // flow-tile-packed H (VK, flow kernel)
+    std::vector<float> Hf;                                            // flow-tile-packed H (VK, flow kernel), INTERNAL mode order
+    std::vector<uint8_t> tile_nz;                                     // per flow tile: holds a non-zero entry
+    long long nz_tiles = 0;
+    // internal (device) order of the transverse modes: perm[k_internal] = k_user.  VK plates group the modes by index
+    // parity (m mod 2, n mod 2): H^n couples only parity classes c and c xor delta_n, so whole 16x16 tiles vanish.
+    std::vector<int> perm, iperm;
     bool coeffs_dirty = true, H_dirty = true;
     std::string err;
     int sm_count = 148;
     // device storage
-    DevBuf dHf, dfx, dgx, dqx, dtiming;
+    DevBuf dHf, dfx, dgx, dqx, dtiming, dperm;
     MmaConfig mma;
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dHt, dkv, dkq, dr, dast, ds, dw, dlam, dc, dq0, dv0, dgain, dbad, dout, dfbuf, dcounter;
@@ -100,6 +105,44 @@ namespace {
     } while (0)
 
 int n_nl(const modal_plan *p) { return p->d.model == MODAL_VK ? p->d.n_phi : 1; }
+
+bool use_team_kernel();
+int env_int(const char *name, int def);
+
+// Internal order of the transverse modes (see modal_plan::perm).
+void build_perm(modal_plan *p)
+{
+    const int nq = p->d.n_q;
+    p->perm.resize(nq); p->iperm.resize(nq);
+    for (int k = 0; k < nq; ++k) p->perm[k] = k;
+    if (p->d.model == MODAL_VK && p->d.geom == MODAL_RECT && !use_team_kernel() && env_int("MODAL_VK_PARITY_ORDER", 1))
+        std::stable_sort(p->perm.begin(), p->perm.end(), [&](int a, int b) {
+            return ((p->mq.m[a] & 1) * 2 + (p->mq.n[a] & 1)) < ((p->mq.m[b] & 1) * 2 + (p->mq.n[b] & 1));
+        });
+    for (int k = 0; k < nq; ++k) p->iperm[p->perm[k]] = k;
+}
+
+// Store H (given in USER mode order) as flow tiles in internal order; note which tiles are entirely zero.
+template <class Get>
+void set_H(modal_plan *p, Get get_user)
+{
+    const int nq = p->d.n_q, nphi = p->d.n_phi;
+    auto get = [&](int n, int a, int b) { return get_user(n, p->perm[a], p->perm[b]); };
+    mh::pack_flow_tiles(nq, nphi, get, p->Hf);
+    if (use_team_kernel()) mh::pack_tiles(nq, nphi, get, p->Ht);
+    const size_t ntiles = p->Hf.size() / mh::FT_FLOATS;
+    p->tile_nz.assign(ntiles, 0);
+    p->nz_tiles = 0;
+    for (size_t t = 0; t < ntiles; ++t) {
+        const float *x = &p->Hf[t * mh::FT_FLOATS];
+        uint8_t nz = 0;
+        for (int e = 0; e < mh::FT_FLOATS; ++e) if (x[e] != 0.f) { nz = 1; break; }
+        p->tile_nz[t] = nz; p->nz_tiles += nz;
+    }
+    for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
+    p->flow_cfgs.clear();                                   // schedules depend on the zero pattern
+    p->H_dirty = true;
+}
 
 bool validate_desc(const modal_plan_desc &d, std::string &err)
 {
@@ -200,7 +243,7 @@ modal_status sync_coeffs(modal_plan *p)
             p->active[(size_t)b * nq + k] = act;
             if (!act) { ++masked; continue; }
             const mh::StepCoeffs c = mh::step_coeffs(d.scheme, om, sg, p->T);
-            const size_t o = (size_t)b * P + k;
+            const size_t o = (size_t)b * P + p->iperm[k];
             kv[o] = c.kv; kq[o] = c.kq; r[o] = c.r; ast[o] = c.astart;
             w[o] = (float)p->pickup[(size_t)b * nq + k];
             if (d.model != MODAL_VK) lam[o] = (float)p->lambda_s[(size_t)b * nq + k];
@@ -256,6 +299,8 @@ modal_status sync_H(modal_plan *p)
         }
         CU(p->dHf.ensure(p->Hf.size() * 4));
         CU(cudaMemcpy(p->dHf.p, p->Hf.data(), p->Hf.size() * 4, cudaMemcpyHostToDevice));
+        CU(p->dperm.ensure(p->perm.size() * 4));
+        CU(cudaMemcpy(p->dperm.p, p->perm.data(), p->perm.size() * 4, cudaMemcpyHostToDevice));
         p->mma.tried = false; p->mma.ok = false;            // operand slabs are rebuilt from the new H on demand
     }
     p->H_dirty = false;
@@ -405,10 +450,10 @@ int flow_capacity(size_t smem, bool ring)
 }
 
 // Size one team shape: schedule, residency, ring.  Returns false if it does not fit shared memory.
-bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, FlowConfig &c)
+bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, const std::vector<uint8_t> *tile_nz, FlowConfig &c)
 {
     c.G = G; c.NW = 16; c.slot_tiles = 8;
-    c.sched = mh::build_flow_schedule(nq, nphi, G, c.NW, c.slot_tiles);
+    c.sched = mh::build_flow_schedule(nq, nphi, G, c.NW, c.slot_tiles, tile_nz);
     const mh::FlowSchedule &s = c.sched;
     if (s.NLOC_MAX > 255 || s.tp_max >= (1 << 24)) return false;
     const md::FlowSmem fixed = md::flow_smem_layout(0, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, 0);
@@ -438,9 +483,8 @@ bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, FlowConfig
 // beyond the ~187 that stay in shared memory are streamed from L2, which delivers ~3.3 KB/cycle to ALL teams together;
 // the exchange phases cost 3.5 k + 70 G + 35 k / G cycles (C2: 6.3 k at G=25, 7.1 k at 50, 9.8 k at 100; C4: 15.4 k at
 // 148), plus one more hop when in-plane modes are shared between CTAs.
-double flow_step_cost(int nq, int nphi, int G, int NT)
+double flow_step_cost(double tiles, int nphi, int G, int NT)
 {
-    const double tiles = (double)nphi * mh::flow_tiles_per_n(nq);
     const double per_cta = tiles / G;
     const double pass = 1500.0 + 28.0 * per_cta;
     const double resident_cap = 187.0;                          // tiles of shared memory
@@ -468,10 +512,10 @@ modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
     }
     for (int g : cand) {
         if (g < 1 || g > sm) continue;
-        const double tiles_cta = (double)nphi * mh::flow_tiles_per_n(nq) / g;
+        const double tiles_cta = (double)p->nz_tiles / g;
         if (force_g <= 0 && tiles_cta > 2000) continue;          // tables would not fit; skip the expensive build
         const int nt = std::max(1, std::min(batch, sm / g));
-        const double cost = std::ceil((double)batch / nt) * flow_step_cost(nq, nphi, g, nt);
+        const double cost = std::ceil((double)batch / nt) * flow_step_cost((double)p->nz_tiles, nphi, g, nt);
         if (!bestG || cost < best * 0.999) { bestG = g; best = cost; }
     }
     if (!bestG) { p->err += "no feasible team size for the vK flow kernel\n"; return MODAL_EINCOMPAT; }
@@ -480,7 +524,7 @@ modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
         const long long key = key0 | bestG;
         FlowConfig &fc = p->flow_cfgs[key];
         if (fc.uploaded) { c = &fc; break; }
-        if (flow_shape(nq, nphi, bestG, force_ns, force_res, fc)) {
+        if (flow_shape(nq, nphi, bestG, force_ns, force_res, &p->tile_nz, fc)) {
             CU(fc.dsched.ensure(fc.sched.blob.size() * 4));
             CU(cudaMemcpy(fc.dsched.p, fc.sched.blob.data(), fc.sched.blob.size() * 4, cudaMemcpyHostToDevice));
             fc.uploaded = true;
@@ -567,8 +611,8 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         for (int k = 0; k < nq; ++k) {
             if (!p->active[(size_t)(cb == 1 ? 0 : b) * nq + k]) continue;
             const double q = init->q0[(size_t)b * nq + k];
-            q0[(size_t)b * P + k] = q;
-            if (init->qm1) v0[(size_t)b * P + k] = q - init->qm1[(size_t)b * nq + k];
+            q0[(size_t)b * P + p->iperm[k]] = q;
+            if (init->qm1) v0[(size_t)b * P + p->iperm[k]] = q - init->qm1[(size_t)b * nq + k];
         }
     CU(p->dq0.ensure(q0.size() * 8)); CU(p->dv0.ensure(v0.size() * 8)); CU(p->dbad.ensure((size_t)batch * 4));
     CU(cudaMemcpyAsync(p->dq0.p, q0.data(), q0.size() * 8, cudaMemcpyHostToDevice, st));
@@ -577,7 +621,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         gain.assign((size_t)batch * P, 0.0);
         for (int b = 0; b < batch; ++b)
             for (int k = 0; k < nq; ++k)
-                if (p->active[(size_t)(cb == 1 ? 0 : b) * nq + k]) gain[(size_t)b * P + k] = init->fext_gain[(size_t)b * nq + k];
+                if (p->active[(size_t)(cb == 1 ? 0 : b) * nq + k]) gain[(size_t)b * P + p->iperm[k]] = init->fext_gain[(size_t)b * nq + k];
         CU(p->dgain.ensure(gain.size() * 8));
         CU(cudaMemcpyAsync(p->dgain.p, gain.data(), gain.size() * 8, cudaMemcpyHostToDevice, st));
     }
@@ -634,7 +678,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             a.fext = init->fext_signal ? init->fext_signal + (size_t)b0 * n_steps : nullptr;
             a.gain = init->fext_signal ? p->dgain.as<double>() + (size_t)b0 * P : nullptr;
             a.out = out_dev + (size_t)b0 * n_steps;
-            a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr;
+            a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr; a.kperm = p->dperm.as<int>();
             a.first_bad = p->dbad.as<int>() + b0;
             a.Qg = m.dQg.as<uint16_t>(); a.qf = m.dqf.as<float>(); a.Gx = m.dGx.as<uint32_t>(); a.fx = m.dfx.as<uint32_t>();
             a.qflag = m.dflags.as<unsigned>();
@@ -687,7 +731,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         a.q0 = p->dq0.as<double>(); a.v0 = p->dv0.as<double>();
         a.auto_start = auto_start; a.half_T2 = half_T2;
         a.fext = init->fext_signal; a.gain = p->dgain.as<double>();
-        a.out = out_dev; a.traj = init->traj_dev; a.first_bad = p->dbad.as<int>();
+        a.out = out_dev; a.traj = init->traj_dev; a.kperm = p->dperm.as<int>(); a.first_bad = p->dbad.as<int>();
         if ((long long)((batch + c->NT - 1) / c->NT) * n_steps >= 0xffffffffLL) { p->err += "batch x n_steps too large for one launch\n"; return MODAL_EINCOMPAT; }
         if (c->G > 1) {
             const size_t nfx = (size_t)c->NT * c->G * P * 8, ngx = (size_t)c->NT * d.n_phi * fs.MS * 8, nqx = (size_t)c->NT * md::FLOW_QREP * P * 8;
@@ -811,6 +855,7 @@ extern "C" modal_status modal_plan_create(const modal_plan_desc *desc, int cuda_
         if (d.model == MODAL_VK) p->mphi = mh::rect_modes(d.Lx, d.Ly, d.n_phi);   // reading R5
     } else p->mq = mh::string_modes(d.Lx, nq);
     p->NQP = d.model == MODAL_VK ? mh::padded_nq(nq) : ((nq + 31) / 32) * 32;
+    build_perm(p);
     p->coeff_batch = 1;
     p->omega.resize(nq); p->sigma.resize(nq); p->pickup.resize(nq); p->lambda_s.resize(nq);
     p->nl_scale.resize(n_nl(p));
@@ -822,8 +867,7 @@ extern "C" modal_status modal_plan_create(const modal_plan_desc *desc, int cuda_
         auto get = [&](int n, int a, int b) {
             return geom * mh::H_bracket(q.m[a], q.n[a], q.m[b], q.n[b], f.m[n], f.n[n]);
         };
-        mh::pack_flow_tiles(nq, d.n_phi, get, p->Hf);
-        if (use_team_kernel()) mh::pack_tiles(nq, d.n_phi, get, p->Ht);
+        set_H(p, get);
     }
     if (cuda_device >= 0) {
         cudaError_t e = cudaSetDevice(cuda_device);
@@ -891,9 +935,7 @@ extern "C" modal_status modal_coeffs_upload(modal_plan *p, const modal_coeffs *c
     if (c->H_full) {
         const double *H = c->H_full;
         auto get = [&](int n, int a, int b) { return H[((size_t)n * nq + a) * nq + b]; };
-        mh::pack_flow_tiles(nq, d.n_phi, get, p->Hf);
-        if (use_team_kernel()) mh::pack_tiles(nq, d.n_phi, get, p->Ht);
-        p->H_dirty = true;
+        set_H(p, get);
     }
     modal_status s = sync_coeffs(p);
     if (s == MODAL_OK && p->H_dirty) s = sync_H(p);
@@ -930,7 +972,7 @@ extern "C" void modal_plan_destroy(modal_plan *p)
     if (p->device >= 0) {
         cudaSetDevice(p->device);
         for (DevBuf *b : {&p->dHt, &p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dw, &p->dlam, &p->dc, &p->dq0,
-                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming, &p->mma.dslabs, &p->mma.dn0, &p->mma.dQg,
+                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming, &p->dperm, &p->mma.dslabs, &p->mma.dn0, &p->mma.dQg,
                           &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags}) b->release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         for (auto &kv : p->vk_cfgs) { kv.second.units.release(); kv.second.warp_ptr.release(); kv.second.cta_ptr.release(); kv.second.nlo.release(); }
@@ -959,11 +1001,18 @@ extern "C" modal_status modal_plan_query(const modal_plan *p, int what, void *ds
         case MODAL_Q_ACTIVE: return put(p->active.data(), p->active.size() * 4);
         case MODAL_Q_COEFF_BATCH: return put(&cb, 4);
         case MODAL_Q_KERNEL_INFO: return put(p->kinfo, sizeof p->kinfo);
+        case MODAL_Q_TILE_STATS: { const int ts[2] = {(int)p->tile_nz.size(), (int)p->nz_tiles}; return put(ts, sizeof ts); }
         case MODAL_Q_H_FULL: {
             if (d.model != MODAL_VK) return MODAL_EINVAL;
             const size_t bytes = (size_t)d.n_phi * nq * nq * 8;
             if (bytes > cap) return MODAL_EINVAL;
-            mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, reinterpret_cast<double *>(dst));
+            std::vector<double> Hi((size_t)d.n_phi * nq * nq);
+            mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, Hi.data());
+            double *Hu = reinterpret_cast<double *>(dst);                      // internal -> user order
+            for (int n = 0; n < d.n_phi; ++n)
+                for (int a = 0; a < nq; ++a)
+                    for (int b = 0; b < nq; ++b)
+                        Hu[((size_t)n * nq + p->perm[a]) * nq + p->perm[b]] = Hi[((size_t)n * nq + a) * nq + b];
             return MODAL_OK;
         }
         default: return MODAL_EINVAL;

@@ -42,7 +42,7 @@ struct FlowArgs {
     const double *q0, *v0;                        // [batch][NQP]
     int auto_start; double half_T2;
     const float *fext; const double *gain;
-    float *out; double *traj; int *first_bad;
+    float *out; double *traj; const int *kperm; int *first_bad;   // kperm[k]: user index of internal mode k (trajectory rows)
     unsigned long long *fx;     // [NT][G][NQP]   partial forces
     unsigned long long *gx;     // [NT][n_phi][MS] partial G_n of shared modes
     unsigned long long *qx;     // [NT][FLOW_QREP][NQP]  new state
@@ -393,7 +393,7 @@ __global__ void __launch_bounds__(RING ? 544 : 512, 1) vk_flow_kernel(const Flow
             }
             if (a.traj)
                 for (int j = tid; j < slice_len; j += NC)
-                    if (slice0 + j < a.n_q) a.traj[((size_t)b * a.n_steps + n) * a.n_q + slice0 + j] = sq[j];
+                    if (slice0 + j < a.n_q) a.traj[((size_t)b * a.n_steps + n) * a.n_q + a.kperm[slice0 + j]] = sq[j];
 
             // ---- A: one pass over this warp's units ----
             for (int u = warp; u < U; u += NW) {

@@ -48,7 +48,7 @@ struct MmaArgs {
     const double *q0, *v0;
     int auto_start; double half_T2;
     const float *fext; const double *gain;
-    float *out; double *traj; int *first_bad;
+    float *out; double *traj; const int *kperm; int *first_bad;
     // exchange (global, L2 resident)
     uint16_t *Qg;               // [2][KC][2][4096 B]   q as bf16 hi/lo operand chunks
     float *qf;                  // [256][QS]            q fp32
@@ -376,7 +376,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 const size_t co = (size_t)(a.coeff_stride_q ? be[h] : 0) * a.NQP + k[h];
                 const double fd = (double)f[h], rr = csm ? sr[e] : a.r[co], kvv = csm ? skv[e] : a.kv[co], kqq = csm ? skq[e] : a.kq[co];
                 double q = sq[e], v = sv[e];
-                if (a.traj) a.traj[((size_t)be[h] * a.n_steps + n) * a.n_q + k[h]] = q;
+                if (a.traj) a.traj[((size_t)be[h] * a.n_steps + n) * a.n_q + a.kperm[k[h]]] = q;
                 if (n == 0 && a.auto_start)
                     v = (rr != 0.0) ? a.astart[co] * q + a.half_T2 * fd : 0.0;
                 const double fe = a.fext ? (double)a.fext[(size_t)be[h] * a.n_steps + n] * a.gain[(size_t)be[h] * a.NQP + k[h]] : 0.0;

@@ -160,3 +160,38 @@ def test_berger_plate_plan_defaults_match_oracle():
     for b in range(3):
         q0 = plan.project_bump(wl["Lx"][b], wl["Ly"][b], wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
         assert np.max(np.abs(q0 - case.q0[b])) <= 1e-7 * np.max(np.abs(case.q0[b]))
+
+
+def test_parity_grouped_modes_leave_whole_tiles_empty_and_queries_stay_in_plan_order():
+    """The device order of the transverse modes (grouped by index parity) is internal: H read back through the API is
+    in plan order and equals the oracle's closed form; most 16x16 tiles of the packed tensor hold no non-zero entry
+    (parity rule m_p+m_q+m_n odd and n_p+n_q+n_n odd), and an uploaded dense H has none."""
+    wl = wlmod.c2()
+    wl["n_q"], wl["n_phi"] = 100, 20
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    m, n, _ = orc.rect_modes(0.6, 0.4, 100)
+    mp, np_, _ = orc.rect_modes(0.6, 0.4, 20)
+    H = orc.H_closed(0.6, 0.4, m, n, mp, np_)
+    Hq = plan.query(mb.Q_H_FULL)
+    assert np.max(np.abs(Hq - H)) <= 1e-6 * np.max(np.abs(H))          # fp32 storage
+    total, nz = plan.query(mb.Q_TILE_STATS)
+    assert total == 20 * 28 and nz <= 0.55 * total
+    # brute-force count of the tiles that can be non-zero when the modes are grouped by parity class
+    cls = (np.asarray(m) % 2) * 2 + (np.asarray(n) % 2)
+    order = np.argsort(cls, kind="stable")
+    Hp = H[:, order][:, :, order]
+    cnt = 0
+    for k in range(20):
+        for I in range(7):
+            for J in range(I + 1):
+                blk = Hp[k, 16 * I:16 * I + 16, 16 * J:16 * J + 16]
+                if I == J:
+                    blk = np.tril(blk)
+                cnt += bool(np.any(np.float32(blk) != 0))
+    assert cnt == nz
+    rng = np.random.default_rng(3)
+    D = rng.normal(size=(20, 100, 100)); D = D + D.transpose(0, 2, 1)
+    plan.coeffs_upload(1, H_full=D)
+    assert np.max(np.abs(plan.query(mb.Q_H_FULL) - D)) <= 1e-6 * np.max(np.abs(D))
+    total2, nz2 = plan.query(mb.Q_TILE_STATS)
+    assert total2 == total and nz2 == total
