@@ -4,6 +4,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <numeric>
 #include <string>
 #include <vector>
 
@@ -556,8 +557,12 @@ modal_status configure_mma(modal_plan *p)
     if (m.tried) return MODAL_OK;
     m.tried = true; m.ok = false;
     const int nq = p->d.n_q, nphi = p->d.n_phi;
+    // in-plane modes of one CTA share the index parity (then the slab is zero in most K chunks, which are skipped)
+    std::vector<int> mode_class(nphi, 0);
+    if (p->d.geom == MODAL_RECT && env_int("MODAL_VK_PARITY_ORDER", 1))
+        for (int n = 0; n < nphi; ++n) mode_class[n] = (p->mphi.m[n] & 1) * 2 + (p->mphi.n[n] & 1);
     if (!mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, md::mma_smem_fixed(), env_int("MODAL_MMA_NKB", 0),
-                        env_int("MODAL_MMA_RBALIGN", 16) == 4 ? 4 : 16, m.L)) return MODAL_OK;
+                        env_int("MODAL_MMA_RBALIGN", 16) == 4 ? 4 : 16, &mode_class, m.L)) return MODAL_OK;
     m.smem = md::mma_smem_layout((int)m.L.slab_bytes, m.L.nel_max).total;
     if (m.smem > SMEM_LIMIT) return MODAL_OK;
     if (cudaFuncSetAttribute(md::vk_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
@@ -577,8 +582,11 @@ modal_status configure_mma(modal_plan *p)
     const mh::MmaLayout &L = m.L;
     CU(m.dslabs.ensure(slabs.size() * 2));
     CU(cudaMemcpy(m.dslabs.p, slabs.data(), slabs.size() * 2, cudaMemcpyHostToDevice));
-    CU(m.dn0.ensure(L.n0.size() * 4));
-    CU(cudaMemcpy(m.dn0.p, L.n0.data(), L.n0.size() * 4, cudaMemcpyHostToDevice));
+    std::vector<int> tab(L.nlist);                                  // nlist | klist | kcnt in one buffer
+    tab.insert(tab.end(), L.klist.begin(), L.klist.end());
+    tab.insert(tab.end(), L.kcnt.begin(), L.kcnt.end());
+    CU(m.dn0.ensure(tab.size() * 4));
+    CU(cudaMemcpy(m.dn0.p, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice));
     CU(m.dQg.ensure((size_t)2 * L.KC * 8192));
     CU(m.dqf.ensure((size_t)256 * L.QS * 4));
     CU(m.dGx.ensure((size_t)L.G * 2 * 128 * 4 * L.NG4 * 4));
@@ -667,7 +675,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)L.slab_bytes;
             a.NKB = L.NKB; a.RB = L.RB; a.NGRP = L.NGRP; a.NG = L.NG; a.NG4 = L.NG4; a.NC = L.NC; a.KC = L.KC; a.KP = L.KP; a.QS = L.QS;
             a.G = L.G; a.nel_max = L.nel_max;
-            a.n0 = m.dn0.as<int>(); a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P;
+            a.nlist = m.dn0.as<int>(); a.klist = a.nlist + L.nlist.size(); a.kcnt = a.klist + L.klist.size(); a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P;
             a.batch = nb; a.n_steps = n_steps; a.MT = (nb + 127) / 128;
             a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
             const size_t oq = cb == 1 ? 0 : (size_t)b0 * P, on = cb == 1 ? 0 : (size_t)b0 * d.n_phi;
@@ -705,8 +713,9 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
                 for (size_t x = 0; x < tm.size(); ++x) acc[x & 7] += (double)tm[x];
                 const double den = (double)L.G * n_steps;
                 fprintf(stderr, "[modal mma timing] G=%d NGRPxNKB=%dx%d RB=%d NG=%d NC=%d cycles/step (tile 0): wait q %.0f | wait mma %.0f | epi1 %.0f | G hop %.0f | "
-                        "epi2 %.0f | f hop+update %.0f | bar+flag %.0f\n", L.G, L.NGRP, L.NKB, L.RB, L.NG, L.NC, acc[0] / den, acc[1] / den, acc[2] / den,
-                        acc[3] / den, acc[4] / den, acc[5] / den, acc[6] / den);
+                        "epi2 %.0f | f hop+update %.0f | bar+flag %.0f | K chunks used %.1f of %d\n", L.G, L.NGRP, L.NKB, L.RB, L.NG, L.NC, acc[0] / den, acc[1] / den, acc[2] / den,
+                        acc[3] / den, acc[4] / den, acc[5] / den, acc[6] / den,
+                        (double)std::accumulate(L.kcnt.begin(), L.kcnt.end(), 0) / L.G, L.KC);
             }
         }
         p->kinfo[0] = 4; p->kinfo[1] = L.G; p->kinfo[2] = L.NGRP; p->kinfo[3] = md::MMA_THREADS;

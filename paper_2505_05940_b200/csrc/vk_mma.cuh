@@ -33,13 +33,17 @@ namespace modal_dev {
 constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
 constexpr int MMA_THREADS = 384;     // warpgroup 0: warp 0 TMA producer, warp 1 MMA issuer (40 registers after setmaxnreg);
                                      // warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (232 registers)
-constexpr int MMA_FB = 20;           // partial-force words in flight per owned element while polling
+#ifndef MODAL_MMA_FB
+#define MODAL_MMA_FB 22
+#endif
+constexpr int MMA_FB = MODAL_MMA_FB;           // partial-force words in flight per owned element while polling
 
 struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H
     int slab_bytes;
     int NKB, RB, NGRP, NG, NG4, NC, KC, KP, QS, G, nel_max;
-    const int *n0;              // [NGRP+1]
+    const int *nlist;           // [NGRP][NG] in-plane modes of each group (-1: empty)
+    const int *klist, *kcnt;    // [G][KC], [G]: K chunks with a non-zero slab part (all others are skipped)
     int n_q, n_phi, NQP;
     int batch, n_steps, MT;     // batch <= 256; MT = M tiles in use
     int coeff_stride_q, coeff_stride_phi;
@@ -145,11 +149,11 @@ __device__ __forceinline__ bool tags_ok(const uint4 &w, uint32_t tag)
 
 __host__ __device__ inline int mma_own_bytes(int nel_max) { return nel_max <= 512 ? 40 : 16; }
 struct MmaSmem { size_t bars, own, sbad, cst, slab, ring, total; };
-__host__ __device__ inline size_t mma_smem_fixed() { return 256 + 256 * 4 + 256 * 64 + (size_t)MMA_NSTG * 8192 + 384; }
+__host__ __device__ inline size_t mma_smem_fixed() { return 512 + 256 * 4 + 256 * 64 + (size_t)MMA_NSTG * 8192 + 384; }
 __host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int nel_max)
 {
     MmaSmem L; size_t o = 0;
-    L.bars = o; o += 256;                                  // mbarriers, tmem pointer, abort word
+    L.bars = o; o += 512;                                  // mbarriers, tmem pointer, abort word; K-chunk list at +192 (64 ints)
     L.own = o;  o += (size_t)2 * nel_max * mma_own_bytes(nel_max);   // owner state per tile: q, v (+ kv, kq, r if they fit), fp64 [nel_max] each
     L.sbad = o; o += 256 * 4;
     L.cst = o;  o += 256 * 64;                             // per epilogue thread: s_n[16] floats
@@ -171,7 +175,6 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
     const int nch = (RB + 15) >> 4;
     const int b = mt * 128 + r;
     const bool valid = b < B;
-    const int n0 = a.n0[i];
     const float *sb = a.s + (size_t)(a.coeff_stride_phi ? (valid ? b : 0) : 0) * a.n_phi;
     // the (sample, k) elements this group owns for the update: rows r0..r1 of the tile, RB modes of block j
     const int r0 = 128 * i / NGRP, r1 = 128 * (i + 1) / NGRP, nel = (r1 - r0) * RB;
@@ -199,7 +202,10 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
     }
     bar_named(2 + mt, 128);
     if (r == 0) set_flag(a.qflag + (size_t)mt * a.G + c, 1u);
-    for (int u = 0; u < 16; ++u) sreg[u * 256] = (u < NG && n0 + u < a.n_phi) ? sb[n0 + u] : 0.f;   // [16][256]: conflict-free
+    for (int u = 0; u < 16; ++u) {                                                // [16][256]: conflict-free
+        const int nn = u < NG ? a.nlist[i * NG + u] : -1;
+        sreg[u * 256] = nn >= 0 ? sb[nn] : 0.f;
+    }
 
     const uint32_t taddr0 = tbase + ((uint32_t)lane_base << 16) + (uint32_t)(mt * NC);
     const bool tmg = a.timing && r == 0 && mt == 0;
@@ -425,6 +431,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int x = tid; x < 256; x += blockDim.x) sbad[x] = -1;
+    if (tid < a.KC && tid < 64) reinterpret_cast<int *>(bars + 24)[tid] = a.klist[(size_t)c * a.KC + tid];   // KC <= 64 (mma_layout)
     {   // H slab of this CTA: loaded once, resident for the whole run
         const uint4 *src = reinterpret_cast<const uint4 *>(a.slabs + (size_t)c * a.slab_bytes / 2);
         uint4 *dst = reinterpret_cast<uint4 *>(slab);
@@ -441,7 +448,9 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     const uint32_t tbase = *tptr;
     const int MT = a.MT, KC = a.KC, NC = a.NC;
 
-    const int kc0 = c % KC;                        // K chunks are walked from a per-CTA offset: spreads the q reads over the L2 slices
+    const int KCA = a.kcnt[c];                     // K chunks with a non-zero slab part: the others are neither loaded nor multiplied
+    const int *kl = reinterpret_cast<const int *>(bars + 24);      // this CTA's chunk list, copied to shared memory above
+    const int kc0 = c % KCA;                       // the chunks are walked from a per-CTA offset: spreads the q reads over the L2 slices
     if (warp >= 4) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
         const int mt = (warp - 4) >> 2, gw = warp & 3;
@@ -460,8 +469,8 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                 if (lane == 0) {
                     mbar_arrive(smem_u32(bars + 16 + mt));
                     asm volatile("fence.proxy.async.global;" ::: "memory");
-                    for (int kx = 0; kx < KC; ++kx) {
-                        const int kc = kx + kc0 < KC ? kx + kc0 : kx + kc0 - KC;
+                    for (int kx = 0; kx < KCA; ++kx) {
+                        const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
                         mbar_wait(smem_u32(bars + 6 + stage), ph ^ 1, s_abort);
                         mbar_expect_tx(smem_u32(bars + stage), 8192);
                         tma_bulk_g2s(smem_u32(ring + stage * 8192), a.Qg + ((size_t)mt * KC + kc) * 4096, 8192, smem_u32(bars + stage));
@@ -480,8 +489,8 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                     mbar_wait(smem_u32(bars + 14 + mt), (n & 1) ^ 1, s_abort);              // epilogues of step n-1 left the tile
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint32_t td = tbase + (uint32_t)(mt * NC);
-                    for (int kx = 0; kx < KC; ++kx) {
-                        const int kc = kx + kc0 < KC ? kx + kc0 : kx + kc0 - KC;
+                    for (int kx = 0; kx < KCA; ++kx) {
+                        const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
                         mbar_wait(smem_u32(bars + stage), ph, s_abort);
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t qa = smem_u32(ring + stage * 8192), hb = smem_u32(slab + (size_t)kc * 2 * NC * 32);
