@@ -33,10 +33,7 @@ namespace modal_dev {
 constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
 constexpr int MMA_THREADS = 384;     // warpgroup 0: warp 0 TMA producer, warp 1 MMA issuer (40 registers after setmaxnreg);
                                      // warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (232 registers)
-#ifndef MODAL_MMA_FB
-#define MODAL_MMA_FB 22
-#endif
-constexpr int MMA_FB = MODAL_MMA_FB;           // partial-force words in flight per owned element while polling
+constexpr int MMA_FB = 11;                     // 16-byte partial-force loads in flight per thread while polling
 
 struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H
@@ -337,64 +334,69 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
         mbar_arrive(smem_u32(bars + 14 + mt));                                      // TMEM tile may be overwritten
         if (tmg) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; }
         // ---- f hop + owner update: group-ordered sum of the partial forces, a5 linear update (fp64, delta form) ----
-        for (int e0 = r; e0 < nel; e0 += 256) {
-            int ee[2], re[2], k[2], be[2];
-            bool act[2];
-            const uint32_t *fp[2];
+        // A warp handles 16 quads (4 consecutive k of one owned row) per pass: lanes 0-15 gather the first half of the
+        // groups, lanes 16-31 the second half, as 16-byte strong loads (few wide requests: a thread keeps only ~16 strong
+        // loads in flight, so the 4-byte version needed three L2 round trips); the halves meet through one shuffle, then
+        // every lane updates two elements of its quad.
+        for (int qbase = 0; qbase < nel; qbase += 256) {
+            const int hh = lane >> 4, e4 = qbase + 4 * (16 * gw + (lane & 15));
+            const int rr_ = e4 / RB, kk = e4 - rr_ * RB, re = r0 + rr_, be = mt * 128 + re, kq0 = j * RB + kk;
+            const bool qact = e4 < nel && be < B && kq0 < a.n_q;
+            const int NH = (NGRP + 1) >> 1, g0 = hh * NH, g1 = min(NGRP, g0 + NH);
+            const uint32_t *fq = a.fx + ((size_t)mt * 128 + (qact ? re : 0)) * QS + (qact ? kq0 : 0);
+            float4 fs = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int ii0 = g0; ii0 < g1; ii0 += MMA_FB) {                           // group order (deterministic)
+                uint4 x[MMA_FB];
+                const int cnt = min(MMA_FB, g1 - ii0);
+                unsigned pend = qact ? (1u << cnt) - 1u : 0u, spins = 0;
+                {   // first round: every word, addresses by pointer increments
+                    const uint32_t *p0 = fq + (size_t)ii0 * fstride;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                ee[h] = e0 + 128 * h;
-                const int rr_ = ee[h] / RB, kk = ee[h] - rr_ * RB;
-                re[h] = r0 + rr_; k[h] = j * RB + kk; be[h] = mt * 128 + re[h];
-                act[h] = ee[h] < nel && be[h] < B && k[h] < a.n_q;
-                fp[h] = a.fx + ((size_t)mt * 128 + (act[h] ? re[h] : 0)) * QS + (act[h] ? k[h] : 0);
-            }
-            float f[2] = {0.f, 0.f};
-            for (int ii0 = 0; ii0 < NGRP; ii0 += MMA_FB) {                          // group order (deterministic)
-                uint32_t x[2][MMA_FB];
-                const int cnt = min(MMA_FB, NGRP - ii0);
-                const unsigned full = (1u << cnt) - 1u;
-                unsigned pend0 = act[0] ? full : 0u, pend1 = act[1] ? full : 0u, spins = 0;
-                while (pend0 | pend1) {
+                    for (int u = 0; u < MMA_FB; ++u)
+                        if (u < cnt) { x[u] = ld_relaxed4(p0); p0 += fstride; }
 #pragma unroll
-                    for (int u = 0; u < MMA_FB; ++u) {
-                        if (pend0 >> u & 1) x[0][u] = ld_relaxed1(fp[0] + (size_t)(ii0 + u) * fstride);
-                        if (pend1 >> u & 1) x[1][u] = ld_relaxed1(fp[1] + (size_t)(ii0 + u) * fstride);
-                    }
+                    for (int u = 0; u < MMA_FB; ++u)
+                        if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
+                }
+                while (pend) {                                                      // stragglers only
 #pragma unroll
-                    for (int u = 0; u < MMA_FB; ++u) {
-                        if ((pend0 >> u & 1) && (x[0][u] & 3u) == tag) pend0 &= ~(1u << u);
-                        if ((pend1 >> u & 1) && (x[1][u] & 3u) == tag) pend1 &= ~(1u << u);
-                    }
-                    if ((pend0 | pend1) && (++spins & 1023u) == 0 && (*s_abort || spins > (1u << 21))) { *s_abort = 1; flow_timeout_flag = 1; break; }
+                    for (int u = 0; u < MMA_FB; ++u)
+                        if (pend >> u & 1) x[u] = ld_relaxed4(fq + (size_t)(ii0 + u) * fstride);
+#pragma unroll
+                    for (int u = 0; u < MMA_FB; ++u)
+                        if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
+                    if (pend && (++spins & 1023u) == 0 && (*s_abort || spins > (1u << 21))) { *s_abort = 1; flow_timeout_flag = 1; break; }
                 }
 #pragma unroll
                 for (int u = 0; u < MMA_FB; ++u)
-                    if (u < cnt) {
-                        if (act[0]) f[0] += untag(x[0][u]);
-                        if (act[1]) f[1] += untag(x[1][u]);
-                    }
+                    if (u < cnt) { fs.x += untag(x[u].x); fs.y += untag(x[u].y); fs.z += untag(x[u].z); fs.w += untag(x[u].w); }
             }
+            __syncwarp();
+            float4 fo;
+            fo.x = __shfl_xor_sync(FLOW_FULL, fs.x, 16); fo.y = __shfl_xor_sync(FLOW_FULL, fs.y, 16);
+            fo.z = __shfl_xor_sync(FLOW_FULL, fs.z, 16); fo.w = __shfl_xor_sync(FLOW_FULL, fs.w, 16);
+            // first half + second half, in that order on both lanes; lane half hh updates elements 2hh, 2hh+1 of the quad
+            const float f2[2] = {hh ? fo.z + fs.z : fs.x + fo.x, hh ? fo.w + fs.w : fs.y + fo.y};
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                if (!act[h]) continue;
-                const int e = ee[h];
-                const size_t co = (size_t)(a.coeff_stride_q ? be[h] : 0) * a.NQP + k[h];
-                const double fd = (double)f[h], rr = csm ? sr[e] : a.r[co], kvv = csm ? skv[e] : a.kv[co], kqq = csm ? skq[e] : a.kq[co];
+                const int e = e4 + 2 * hh + h, k = kq0 + 2 * hh + h;
+                if (!(qact && k < a.n_q)) continue;
+                const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
+                const double fd = (double)f2[h], rr = csm ? sr[e] : a.r[co], kvv = csm ? skv[e] : a.kv[co], kqq = csm ? skq[e] : a.kq[co];
                 double q = sq[e], v = sv[e];
-                if (a.traj) a.traj[((size_t)be[h] * a.n_steps + n) * a.n_q + a.kperm[k[h]]] = q;
+                if (a.traj) a.traj[((size_t)be * a.n_steps + n) * a.n_q + a.kperm[k]] = q;
                 if (n == 0 && a.auto_start)
                     v = (rr != 0.0) ? a.astart[co] * q + a.half_T2 * fd : 0.0;
-                const double fe = a.fext ? (double)a.fext[(size_t)be[h] * a.n_steps + n] * a.gain[(size_t)be[h] * a.NQP + k[h]] : 0.0;
+                const double fe = a.fext ? (double)a.fext[(size_t)be * a.n_steps + n] * a.gain[(size_t)be * a.NQP + k] : 0.0;
                 v = kvv * v - kqq * q + rr * (fe - fd);
                 q += v;
                 sq[e] = q; sv[e] = v;
                 const float qfl = (float)q;
-                a.qf[(size_t)be[h] * QS + k[h]] = qfl;
+                a.qf[(size_t)be * QS + k] = qfl;
                 const uint16_t hi = bf16_rn_dev(qfl), lo = bf16_rn_dev(qfl - __uint_as_float((uint32_t)hi << 16));
-                const int k16 = k[h] & 15;
-                const int off = ((re[h] >> 3) * 256 + (k16 >> 3) * 128 + (re[h] & 7) * 16 + (k16 & 7) * 2) >> 1;
-                uint16_t *Qc = Qt + (size_t)(k[h] >> 4) * 4096;
+                const int k16 = k & 15;
+                const int off = ((re >> 3) * 256 + (k16 >> 3) * 128 + (re & 7) * 16 + (k16 & 7) * 2) >> 1;
+                uint16_t *Qc = Qt + (size_t)(k >> 4) * 4096;
                 Qc[off] = hi; Qc[2048 + off] = lo;
             }
         }
