@@ -461,51 +461,55 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                                tbase, s_abort, (warp & 3) * 32, sbad, gw, lane, reinterpret_cast<float *>(cst) + (tid - 128));
     } else {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
-    if (warp == 0) {
-        // ---------------- producer: wait for q^n of a tile, stream it through the ring by TMA ----------
+    // Warps 0 / 2 are the producers of tile 0 / 1, warps 1 / 3 the MMA issuers: the two tiles are independent pipelines
+    // (own half of the ring stages when both tiles are in use), so a late q^n of one tile never holds up the other.
+    const int mt = warp >> 1;
+    const int NSH = MT > 1 ? MMA_NSTG / 2 : MMA_NSTG;
+    if (mt < MT && (warp & 1) == 0) {
+        // ---------------- producer: wait for q^n of the tile, stream it through the ring by TMA ----------
         int stage = 0; unsigned ph = 0;
-        for (int n = 0; n < a.n_steps; ++n)
-            for (int mt = 0; mt < MT; ++mt) {
-                poll_flags(a.qflag + (size_t)mt * a.G, lane, a.G, (unsigned)n + 1u, s_abort);
-                __syncwarp();
-                if (lane == 0) {
-                    mbar_arrive(smem_u32(bars + 16 + mt));
-                    asm volatile("fence.proxy.async.global;" ::: "memory");
-                    for (int kx = 0; kx < KCA; ++kx) {
-                        const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
-                        mbar_wait(smem_u32(bars + 6 + stage), ph ^ 1, s_abort);
-                        mbar_expect_tx(smem_u32(bars + stage), 8192);
-                        tma_bulk_g2s(smem_u32(ring + stage * 8192), a.Qg + ((size_t)mt * KC + kc) * 4096, 8192, smem_u32(bars + stage));
-                        if (++stage == MMA_NSTG) { stage = 0; ph ^= 1; }
-                    }
+        for (int n = 0; n < a.n_steps; ++n) {
+            poll_flags(a.qflag + (size_t)mt * a.G, lane, a.G, (unsigned)n + 1u, s_abort);
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(smem_u32(bars + 16 + mt));
+                asm volatile("fence.proxy.async.global;" ::: "memory");
+                for (int kx = 0; kx < KCA; ++kx) {
+                    const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
+                    const int sg = NSH * mt + stage;
+                    mbar_wait(smem_u32(bars + 6 + sg), ph ^ 1, s_abort);
+                    mbar_expect_tx(smem_u32(bars + sg), 8192);
+                    tma_bulk_g2s(smem_u32(ring + sg * 8192), a.Qg + ((size_t)mt * KC + kc) * 4096, 8192, smem_u32(bars + sg));
+                    if (++stage == NSH) { stage = 0; ph ^= 1; }
                 }
-                __syncwarp();
             }
-    } else if (warp == 1) {
-        // ---------------- MMA issuer: one thread --------------------------------------------------------
+            __syncwarp();
+        }
+    } else if (mt < MT) {
+        // ---------------- MMA issuer: one thread per tile ------------------------------------------------
         if (lane == 0) {
             const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NC >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
             int stage = 0; unsigned ph = 0;
-            for (int n = 0; n < a.n_steps; ++n)
-                for (int mt = 0; mt < MT; ++mt) {
-                    mbar_wait(smem_u32(bars + 14 + mt), (n & 1) ^ 1, s_abort);              // epilogues of step n-1 left the tile
+            const uint32_t td = tbase + (uint32_t)(mt * NC);
+            for (int n = 0; n < a.n_steps; ++n) {
+                mbar_wait(smem_u32(bars + 14 + mt), (n & 1) ^ 1, s_abort);              // epilogues of step n-1 left the tile
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                for (int kx = 0; kx < KCA; ++kx) {
+                    const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
+                    const int sg = NSH * mt + stage;
+                    mbar_wait(smem_u32(bars + sg), ph, s_abort);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const uint32_t td = tbase + (uint32_t)(mt * NC);
-                    for (int kx = 0; kx < KCA; ++kx) {
-                        const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
-                        mbar_wait(smem_u32(bars + stage), ph, s_abort);
-                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                        const uint32_t qa = smem_u32(ring + stage * 8192), hb = smem_u32(slab + (size_t)kc * 2 * NC * 32);
-                        const uint64_t qhi = umma_desc(qa), qlo = umma_desc(qa + 4096);
-                        const uint64_t hhi = umma_desc(hb), hlo = umma_desc(hb + NC * 32);
-                        umma_bf16(td, qhi, hhi, idesc, kx > 0);
-                        umma_bf16(td, qlo, hhi, idesc, 1);
-                        umma_bf16(td, qhi, hlo, idesc, 1);
-                        umma_commit(smem_u32(bars + 6 + stage));                           // ring slot free when these MMAs retire
-                        if (++stage == MMA_NSTG) { stage = 0; ph ^= 1; }
-                    }
-                    umma_commit(smem_u32(bars + 12 + mt));                                 // t of tile mt complete
+                    const uint32_t qa = smem_u32(ring + sg * 8192), hb = smem_u32(slab + (size_t)kc * 2 * NC * 32);
+                    const uint64_t qhi = umma_desc(qa), qlo = umma_desc(qa + 4096);
+                    const uint64_t hhi = umma_desc(hb), hlo = umma_desc(hb + NC * 32);
+                    umma_bf16(td, qhi, hhi, idesc, kx > 0);
+                    umma_bf16(td, qlo, hhi, idesc, 1);
+                    umma_bf16(td, qhi, hlo, idesc, 1);
+                    umma_commit(smem_u32(bars + 6 + sg));                               // ring slot free when these MMAs retire
+                    if (++stage == NSH) { stage = 0; ph ^= 1; }
                 }
+                umma_commit(smem_u32(bars + 12 + mt));                                 // t of tile mt complete
+            }
         }
     }
     }
