@@ -716,10 +716,6 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
                         "epi2 %.0f | f hop+update %.0f | bar+flag %.0f | K chunks used %.1f of %d\n", L.G, L.NGRP, L.NKB, L.RB, L.NG, L.NC, acc[0] / den, acc[1] / den, acc[2] / den,
                         acc[3] / den, acc[4] / den, acc[5] / den, acc[6] / den,
                         (double)std::accumulate(L.kcnt.begin(), L.kcnt.end(), 0) / L.G, L.KC);
-                if (env_int("MODAL_FLOW_TIMING", 0) == 2) {   // TEMP per-CTA dump
-                    FILE *fp = fopen("gpurun_out/mma_cta_timing.txt", "w");
-                    if (fp) { for (int c2 = 0; c2 < L.G; ++c2) { fprintf(fp, "%d %d %d %d", c2, c2 / L.NKB, c2 % L.NKB, L.kcnt[c2]); for (int x = 0; x < 8; ++x) fprintf(fp, " %.2f", (double)tm[(size_t)c2 * 8 + x] / n_steps); fprintf(fp, "\n"); } fclose(fp); }
-                }
             }
         }
         p->kinfo[0] = 4; p->kinfo[1] = L.G; p->kinfo[2] = L.NGRP; p->kinfo[3] = md::MMA_THREADS;
