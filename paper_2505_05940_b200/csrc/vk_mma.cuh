@@ -31,9 +31,9 @@
 namespace modal_dev {
 
 constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
-constexpr int MMA_THREADS = 384;     // warpgroup 0: warp 0 TMA producer, warp 1 MMA issuer (40 registers after setmaxnreg);
-                                     // warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (232 registers)
-constexpr int MMA_FB = 11;                     // 16-byte partial-force loads in flight per thread while polling
+constexpr int MMA_THREADS = 384;     // warpgroup 0: warps 0 / 2 TMA producers, warps 1 / 3 MMA issuers of tile 0 / 1 (56 registers
+                                     // after setmaxnreg); warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (224 registers)
+constexpr int MMA_FB = 11;           // 16-byte partial-force loads in flight per thread while polling (a thread keeps ~16 strong loads in flight)
 
 struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H
