@@ -31,7 +31,8 @@ constexpr unsigned FULL = 0xffffffffu;
 //   v^{n+1} = kv v^n - kq q^n + r (fext - fnl),   q^{n+1} = q^n + v^{n+1}
 // SV : kv = (1-gT)/(1+gT), kq = r w^2, r = T^2/(1+gT)   (== Eq. 20-23: g = 1+kv-kq, p = -kv)
 // FTM: kv = a2, kq = 1+a1+a2, r = b1                    (== Eq. 16-19 with -a1, -a2)
-// State and coefficients are fp64; the force is evaluated in fp32.
+// State and coefficients are fp64; the vK force is evaluated in fp32 (tension kernel: per-lane sums in
+// fp64, the cross-lane sums S and pickup in fp32).
 // ----------------------------------------------------------------------------------------
 
 struct TensionArgs {
@@ -55,29 +56,33 @@ __global__ void __launch_bounds__(128) tension_kernel(const TensionArgs a)
     if (b >= a.batch) return;
     const size_t co = (size_t)(a.coeff_stride ? b : 0) * a.n_modes_pad;
     const size_t so = (size_t)b * a.n_modes_pad;
-    double q[MPL], v[MPL], kv[MPL], kq[MPL], r[MPL], gain[MPL];
-    float lam[MPL], w[MPL];
+    // rl = r * lambda: the force term r f_mu = (r lambda_mu)(c S) q_mu is folded into the fp64 update, so the
+    // step has no per-mode conversion between fp32 and fp64 (only S and the pickup cross the lanes, in fp32)
+    double q[MPL], v[MPL], kv[MPL], kq[MPL], rl[MPL], rg[MPL], lam[MPL], w[MPL];
 #pragma unroll
     for (int j = 0; j < MPL; ++j) {
         const int k = lane + 32 * j;
         q[j] = a.q0[so + k]; v[j] = a.v0[so + k];
-        kv[j] = a.kv[co + k]; kq[j] = a.kq[co + k]; r[j] = a.r[co + k];
+        kv[j] = a.kv[co + k]; kq[j] = a.kq[co + k];
         lam[j] = a.lambda[co + k]; w[j] = a.w[co + k];
-        gain[j] = a.fext ? a.gain[so + k] : 0.0;
+        const double r = a.r[co + k];
+        rl[j] = r * lam[j];
+        rg[j] = a.fext ? r * a.gain[so + k] : 0.0;
     }
     const float c = a.c[a.coeff_stride ? b : 0];
     float oreg = 0.f;
     int bad = -1;
     float *out = a.out + (size_t)b * a.n_steps;
     for (int n = 0; n < a.n_steps; ++n) {
-        float qf[MPL];
-        float o = 0.f, S = 0.f;
+        // per-lane partial sums in fp64 straight from the state (no per-mode conversion; two chains each),
+        // rounded to fp32 once for the shuffle reduction
+        double od = 0.0, Sd = 0.0, od1 = 0.0, Sd1 = 0.0;
 #pragma unroll
         for (int j = 0; j < MPL; ++j) {
-            qf[j] = (float)q[j];
-            o = fmaf(w[j], qf[j], o);
-            S = fmaf(lam[j] * qf[j], qf[j], S);
+            if (j & 1) { od1 = fma(w[j], q[j], od1); Sd1 = fma(lam[j] * q[j], q[j], Sd1); }
+            else       { od = fma(w[j], q[j], od);   Sd = fma(lam[j] * q[j], q[j], Sd); }
         }
+        float o = (float)(od + od1), S = (float)(Sd + Sd1);
 #pragma unroll
         for (int m = 16; m >= 1; m >>= 1) {
             o += __shfl_xor_sync(FULL, o, m);
@@ -93,14 +98,17 @@ __global__ void __launch_bounds__(128) tension_kernel(const TensionArgs a)
                 if (k < a.n_q) a.traj[((size_t)b * a.n_steps + n) * a.n_q + k] = q[j];
             }
         }
-        const float cS = c * S;
+        const double cS = (double)(c * S);
         const double fe = a.fext ? (double)a.fext[(size_t)b * a.n_steps + n] : 0.0;
+        if (n == 0 && a.auto_start) {
+#pragma unroll
+            for (int j = 0; j < MPL; ++j)
+                v[j] = (a.r[co + lane + 32 * j] != 0.0)
+                           ? a.astart[co + lane + 32 * j] * q[j] + a.half_T2 * (cS * lam[j] * q[j]) : 0.0;
+        }
 #pragma unroll
         for (int j = 0; j < MPL; ++j) {
-            const double f = (double)(cS * lam[j] * qf[j]);
-            if (n == 0 && a.auto_start)
-                v[j] = (r[j] != 0.0) ? a.astart[co + lane + 32 * j] * q[j] + a.half_T2 * f : 0.0;
-            v[j] = kv[j] * v[j] - kq[j] * q[j] + r[j] * (fe * gain[j] - f);
+            v[j] = fma(-fma(rl[j], cS, kq[j]), q[j], fma(kv[j], v[j], fe * rg[j]));   // only the first factor waits for S
             q[j] += v[j];
         }
     }
