@@ -141,6 +141,8 @@ def run_reference(args):
     sb = min(B, max(1, cores))
     budget = 6e9 * min(sb, cores)
     n_s = int(max(16, min(n_full, budget / (flops * sb))))
+    if n_s == n_full:                      # cheap models (strings): widen the sample over the batch instead
+        sb = int(min(B, max(sb, budget / (flops * n_full) // cores * cores)))
     case = orc.assemble(wl, samples=range(sb))
     for _ in range(args.warmup):
         orc.run_case(case, min(n_s, 16))
@@ -166,6 +168,8 @@ def cpu_baseline(wl, seconds=12.0):
     cores = orc.num_threads()
     sb = min(B, max(1, cores))
     n_s = int(max(16, min(n_full, 0.8e9 * seconds * min(sb, cores) / (flops * sb))))
+    if n_s == n_full:                      # cheap models (strings): widen the sample over the batch instead
+        sb = int(min(B, max(sb, 0.8e9 * seconds * cores / (flops * n_full) // cores * cores)))
     case = orc.assemble(wl, samples=range(sb))
     orc.run_case(case, 4)
     t0 = time.perf_counter()
