@@ -259,11 +259,12 @@ def test_vk_mma_batch_beyond_one_launch(monkeypatch):
 
 def test_c3_full_shape_tensor_core_short_run():
     """C3 at its full size (200 + 100 modes, 256 geometries) in the launch configuration bench.py times,
-    checked on a sample subset spanning the amplitude range (the oracle needs ~2 s per sample here)."""
-    n_steps = 300
+    checked on 16 samples spanning the amplitude range (the oracle needs ~6 s per sample here, one
+    sample per host core)."""
+    n_steps = 768
     wl = wlmod.c3(n_steps=n_steps)
     order = np.argsort(wl["A"] / wl["h"])
-    sub = sorted(set(order[np.linspace(0, 255, 6).astype(int)].tolist()))
+    sub = sorted(set(order[np.linspace(0, 255, 16).astype(int)].tolist()))
     torch, mb = _mods()
     plan, q0 = mb.plan_from_workload(wl, 0)
     gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
@@ -277,6 +278,22 @@ def test_c3_full_shape_tensor_core_short_run():
     assert np.all(np.isfinite(gpu[fb < 0]))
 
 
+def test_c2_full_config_parity():
+    """C2 exactly as bench.py times it (100 + 50 modes, batch 1, all 44 100 steps, the plan's own coefficient
+    derivation): the paper's 100-mode benchmark point.  The oracle needs ~45 s here."""
+    wl = wlmod.c2()
+    n_steps = wl["n_steps"]
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, n_steps)
+    torch, mb = _mods()
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 3 and st == 0 and fb[0] == -1 and ref["first_bad"][0] == -1
+    assert nl_ratio(case, 0) <= 0.05
+    check_parity(gpu, ref["out"], case)
+
+
 def test_vk_ftm_scheme_and_auto_start_parity():
     wl = _small_vk_workload(37, 13, 2, 2000)
     case = orc.assemble(wl, scheme=orc.FTM)
@@ -287,15 +304,15 @@ def test_vk_ftm_scheme_and_auto_start_parity():
 
 
 def test_c4_shape_whole_gpu_team_short_run():
-    wl = wlmod.c4(batch=1, n_steps=96)
+    wl = wlmod.c4(batch=1, n_steps=320)
     case = orc.assemble(wl)
-    ref = orc.run_case(case, 96)
+    ref = orc.run_case(case, 320)
     plan = plan_with_oracle_inputs(wl, case)
-    gpu, fb, _, _ = gpu_run(plan, case.q0, case.qm1, 96)
+    gpu, fb, _, _ = gpu_run(plan, case.q0, case.qm1, 320)
     torch, mb = _mods()
     info = plan.query(mb.Q_KERNEL_INFO)
     assert info[0] == 3 and info[1] >= 100                        # one team over (most of) the GPU
-    check_parity(gpu, ref["out"], case, first=96)
+    check_parity(gpu, ref["out"], case, first=320)
 
 
 def test_c4_shape_batch_teams_side_by_side():
@@ -312,6 +329,26 @@ def test_c4_shape_batch_teams_side_by_side():
     check_parity(gpu, ref["out"], case, first=64)
 
 
+@pytest.mark.parametrize("batch", [16, 64])
+def test_c4_bench_batches_sampled(batch):
+    """C4 at the batches of the sweep (16, 64) in the launch configuration bench.py times (the plan's own derivation,
+    teams side by side), checked on four samples spanning the amplitude range; every sample finite."""
+    n_steps = 48
+    wl = wlmod.c4(batch=batch, n_steps=n_steps)
+    order = np.argsort(wl["A"])
+    sub = sorted(set(order[np.linspace(0, batch - 1, 4).astype(int)].tolist()))
+    torch, mb = _mods()
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 3 and info[2] >= 2 and st == 0 and np.all(fb == -1)
+    sub_case = orc.assemble(wl, samples=sub)
+    ref = orc.run_case(sub_case, n_steps)
+    assert np.all(ref["first_bad"] < 0)
+    check_parity(gpu[sub], ref["out"], sub_case, first=n_steps)
+    assert np.all(np.isfinite(gpu))
+
+
 # ------------------------------------------------------------------ tension / linear ----
 @pytest.mark.parametrize("batch,n_steps", [(32, 4096), (5, 333)])
 def test_c1_string_parity(batch, n_steps):
@@ -321,6 +358,23 @@ def test_c1_string_parity(batch, n_steps):
     plan = plan_with_oracle_inputs(wl, case)
     gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, n_steps)
     torch, mb = _mods()
+    assert st == (mb.EUNSTABLE if np.any(ref["first_bad"] >= 0) else 0)
+    check_parity(gpu, ref["out"], case, ref_bad=ref["first_bad"], gpu_bad=fb)
+
+
+def test_c1_full_config_parity():
+    """C1 exactly as bench.py times it: all 1024 strings, all 44 100 steps, the plan's own coefficient derivation
+    (the oracle advances the whole batch in a few seconds on the host cores).  Strings whose explicit scheme
+    blows up in the oracle must be reported by the GPU at (nearly) the same step (check_parity)."""
+    wl = wlmod.c1()
+    n_steps = wl["n_steps"]
+    case = orc.assemble(wl)
+    ref = orc.run_case(case, n_steps)
+    torch, mb = _mods()
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 1 and info[2] * 4 >= wl["batch"]
     assert st == (mb.EUNSTABLE if np.any(ref["first_bad"] >= 0) else 0)
     check_parity(gpu, ref["out"], case, ref_bad=ref["first_bad"], gpu_bad=fb)
 
