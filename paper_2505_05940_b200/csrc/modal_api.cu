@@ -1,5 +1,6 @@
 // modal_api.cu -- the C ABI of include/modal.h: plan, coefficient upload, launch logic.
 // Host-side derivations live in host_math.hpp, kernels in kernels.cuh.
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -60,7 +61,8 @@ struct FlowConfig {
 struct MmaConfig {
     bool tried = false, ok = false;
     mh::MmaLayout L;
-    size_t smem = 0;
+    size_t smem = 0, slab_c = 0;     // slab_c: bytes of a compacted slab (only the K chunks a CTA multiplies, in list order)
+    int nstg = 0;                    // q-operand ring stages that fit beside it
     DevBuf dslabs, dn0, dQg, dqf, dGx, dfx, dflags;
 };
 
@@ -563,8 +565,8 @@ modal_status configure_mma(modal_plan *p)
         for (int n = 0; n < nphi; ++n) mode_class[n] = (p->mphi.m[n] & 1) * 2 + (p->mphi.n[n] & 1);
     if (!mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, md::mma_smem_fixed(), env_int("MODAL_MMA_NKB", 0),
                         env_int("MODAL_MMA_RBALIGN", 16) == 4 ? 4 : 16, &mode_class, m.L)) return MODAL_OK;
-    m.smem = md::mma_smem_layout((int)m.L.slab_bytes, m.L.nel_max).total;
-    if (m.smem > SMEM_LIMIT) return MODAL_OK;
+    if (md::mma_smem_layout((int)m.L.slab_bytes, m.L.nel_max, md::MMA_NSTG).total > SMEM_LIMIT) return MODAL_OK;
+    m.smem = SMEM_LIMIT;             // upper bound for the occupancy check; the launch size is set after the slabs are packed
     if (cudaFuncSetAttribute(md::vk_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, md::vk_mma_kernel, md::MMA_THREADS, m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
@@ -580,6 +582,24 @@ modal_status configure_mma(modal_plan *p)
     std::vector<uint16_t> slabs;
     mh::pack_mma_slabs(m.L, get, slabs);
     const mh::MmaLayout &L = m.L;
+    {   // compact: a CTA keeps only the K chunks it multiplies, in list order; the shared memory this frees goes to the ring
+        const size_t chunk = (size_t)2 * L.NC * 32;
+        const int kcm = *std::max_element(L.kcnt.begin(), L.kcnt.end());
+        m.slab_c = (size_t)kcm * chunk;
+        std::vector<uint16_t> cs((size_t)L.G * m.slab_c / 2, 0);
+        for (int c = 0; c < L.G; ++c)
+            for (int x = 0; x < L.kcnt[c]; ++x)
+                std::memcpy(&cs[((size_t)c * m.slab_c + (size_t)x * chunk) / 2],
+                            &slabs[((size_t)c * L.slab_bytes + (size_t)L.klist[(size_t)c * L.KC + x] * chunk) / 2], chunk);
+        slabs.swap(cs);
+        const size_t base = md::mma_smem_layout((int)m.slab_c, L.nel_max, 0).total;
+        // measured on C3 (profiles/r1_c3_b256.md): 6 / 8 / 12 stages give 17.91 / 17.86 / 18.25 us per step -- the q stream is
+        // bound by L2 bandwidth (every CTA reads the same chunks), not by the bytes in flight, so the ring stays at 8
+        const int want = std::max(2, std::min(env_int("MODAL_MMA_NSTG", 8), md::MMA_NSTG_MAX));
+        const int nstg = (int)std::min<size_t>(want, (SMEM_LIMIT - base) / 8192) & ~1;
+        m.nstg = nstg;
+        m.smem = md::mma_smem_layout((int)m.slab_c, L.nel_max, nstg).total;
+    }
     CU(m.dslabs.ensure(slabs.size() * 2));
     CU(cudaMemcpy(m.dslabs.p, slabs.data(), slabs.size() * 2, cudaMemcpyHostToDevice));
     std::vector<int> tab(L.nlist);                                  // nlist | klist | kcnt in one buffer
@@ -672,7 +692,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         for (int b0 = 0; b0 < batch; b0 += 256) {       // up to two M tiles of 128 samples per launch
             const int nb = std::min(256, batch - b0);
             md::MmaArgs a{};
-            a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)L.slab_bytes;
+            a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)m.slab_c; a.NSTG = m.nstg;
             a.NKB = L.NKB; a.RB = L.RB; a.NGRP = L.NGRP; a.NG = L.NG; a.NG4 = L.NG4; a.NC = L.NC; a.KC = L.KC; a.KP = L.KP; a.QS = L.QS;
             a.G = L.G; a.nel_max = L.nel_max;
             a.nlist = m.dn0.as<int>(); a.klist = a.nlist + L.nlist.size(); a.kcnt = a.klist + L.klist.size(); a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P;

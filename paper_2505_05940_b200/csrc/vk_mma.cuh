@@ -30,14 +30,18 @@
 
 namespace modal_dev {
 
-constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
+constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo) the layout fit assumes; the
+constexpr int MMA_NSTG_MAX = 16;     // launch uses MmaArgs::NSTG stages (8 by default, <= 16) beside the compacted slab
+// mbarrier indices: full[0..15] empty[16..31] acc_full[32,33] acc_empty[34,35] qready[36,37]; tmem pointer at word 40,
+// abort word at 41, K-chunk list (64 ints) from word 44
+constexpr int MB_FULL = 0, MB_EMPTY = 16, MB_ACCF = 32, MB_ACCE = 34, MB_QRDY = 36, MB_TPTR = 40, MB_ABORT = 41, MB_KLIST = 44;
 constexpr int MMA_THREADS = 384;     // warpgroup 0: warps 0 / 2 TMA producers, warps 1 / 3 MMA issuers of tile 0 / 1 (56 registers
                                      // after setmaxnreg); warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (224 registers)
 constexpr int MMA_FB = 11;           // 16-byte partial-force loads in flight per thread while polling (a thread keeps ~16 strong loads in flight)
 
 struct MmaArgs {
-    const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H
-    int slab_bytes;
+    const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H: only the K chunks of klist, in list order
+    int slab_bytes, NSTG;       // NSTG: ring stages of this launch (even, <= 16)
     int NKB, RB, NGRP, NG, NG4, NC, KC, KP, QS, G, nel_max;
     const int *nlist;           // [NGRP][NG] in-plane modes of each group (-1: empty)
     const int *klist, *kcnt;    // [G][KC], [G]: K chunks with a non-zero slab part (all others are skipped)
@@ -89,8 +93,13 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&u)[1
                  : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// The flags p[0 .. count), each polled with ld.acquire.gpu (a separate fence.acq_rel.gpu after relaxed polls
-// measured slower: the MEMBAR stalls the epilogue warps of the other tile).
+// The flags p[0 .. count): relaxed polls with a short sleep between rounds, then one ld.acquire.gpu per flag, which orders
+// the q data behind the flags.  All CTAs poll the same few L2 lines while the owners try to store to them, so the
+// polling rate matters (C3, us per step at batch 256 / 128): ld.acquire polls back to back 17.9 / 13.8 (each is followed
+// by an L1 invalidate, which throttles them), relaxed polls back to back 21.3 / 13.3, relaxed + 400 ns sleep 16.6 / 12.8;
+// a fence.acq_rel.gpu after relaxed polls measured slower (the MEMBAR stalls the epilogue warps of the other tile).
+// (1.5 us sleep 16.3 / 12.6; sleeping through an estimate of the wait before the first poll 16.5 / 16.5: nanosleep overshoots)
+constexpr unsigned MMA_POLL_SLEEP = 400;      // ns between polling rounds
 __device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int count, unsigned epoch, volatile int *abortp)
 {
     for (int base = lane; base < count; base += 256) {
@@ -101,11 +110,18 @@ __device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int coun
             unsigned v[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u)
-                if (pend >> u & 1) asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + base + 32 * u) : "memory");
+                if (pend >> u & 1) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + base + 32 * u) : "memory");
 #pragma unroll
             for (int u = 0; u < 8; ++u) if ((pend >> u & 1) && v[u] >= epoch) pend &= ~(1u << u);
             if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
+            if (pend) __nanosleep(MMA_POLL_SLEEP);
         }
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (base + 32 * u < count) {
+                unsigned v;
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p + base + 32 * u) : "memory");
+            }
     }
 }
 __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
@@ -146,18 +162,18 @@ __device__ __forceinline__ bool tags_ok(const uint4 &w, uint32_t tag)
 
 __host__ __device__ inline int mma_own_bytes(int nel_max) { return nel_max <= 512 ? 40 : 16; }
 struct MmaSmem { size_t bars, own, sbad, cst, slab, ring, total; };
-__host__ __device__ inline size_t mma_smem_fixed() { return 512 + 256 * 4 + 256 * 64 + (size_t)MMA_NSTG * 8192 + 384; }
-__host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int nel_max)
+__host__ __device__ inline size_t mma_smem_fixed() { return 1024 + 256 * 4 + 256 * 64 + (size_t)MMA_NSTG * 8192 + 384; }
+__host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int nel_max, int nstg)
 {
     MmaSmem L; size_t o = 0;
-    L.bars = o; o += 512;                                  // mbarriers, tmem pointer, abort word; K-chunk list at +192 (64 ints)
+    L.bars = o; o += 1024;                                 // mbarriers, tmem pointer, abort word, K-chunk list (MB_* above)
     L.own = o;  o += (size_t)2 * nel_max * mma_own_bytes(nel_max);   // owner state per tile: q, v (+ kv, kq, r if they fit), fp64 [nel_max] each
     L.sbad = o; o += 256 * 4;
     L.cst = o;  o += 256 * 64;                             // per epilogue thread: s_n[16] floats
     o = flow_align(o, 128);
     L.slab = o; o += (size_t)slab_bytes;
     o = flow_align(o, 128);
-    L.ring = o; o += (size_t)MMA_NSTG * 8192;
+    L.ring = o; o += (size_t)nstg * 8192;
     L.total = o;
     return L;
 }
@@ -217,7 +233,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
     for (int n = 0; n < a.n_steps; ++n) {
         const uint32_t tag = ((uint32_t)n + 1u) & 3u;
         long long tk = tmg ? clock64() : 0;
-        mbar_wait(smem_u32(bars + 16 + mt), n & 1, s_abort);                       // q^n published by everybody
+        mbar_wait(smem_u32(bars + MB_QRDY + mt), n & 1, s_abort);                  // q^n published by everybody
         if (tmg) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
         // ---- this sample's q over the rows of block j (operand of epilogue 1) ----
         float qb[32];
@@ -243,7 +259,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 if (sbad[m] < 0 && !(isfinite(o) && isfinite(nrm))) sbad[m] = n;
             }
         }
-        mbar_wait(smem_u32(bars + 12 + mt), n & 1, s_abort);                       // t of this tile is in TMEM
+        mbar_wait(smem_u32(bars + MB_ACCF + mt), n & 1, s_abort);                  // t of this tile is in TMEM
         if (tmg) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         // ---- epilogue 1: partial G over the RB rows k of block j, four modes per pass ----
@@ -331,7 +347,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                         st_tagged4(frow + ch * 16 + 4 * u, facc[4 * u], facc[4 * u + 1], facc[4 * u + 2], facc[4 * u + 3], tag);
             }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        mbar_arrive(smem_u32(bars + 14 + mt));                                      // TMEM tile may be overwritten
+        mbar_arrive(smem_u32(bars + MB_ACCE + mt));                                 // TMEM tile may be overwritten
         if (tmg) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; }
         // ---- f hop + owner update: group-ordered sum of the partial forces, a5 linear update (fp64, delta form) ----
         // A warp handles 16 quads (4 consecutive k of one owned row) per pass: lanes 0-15 gather the first half of the
@@ -415,25 +431,25 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     extern __shared__ __align__(128) unsigned char mma_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int c = blockIdx.x, i = c / a.NKB, j = c - i * a.NKB;
-    const MmaSmem L = mma_smem_layout(a.slab_bytes, a.nel_max);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(mma_smem + L.bars);      // full[0..5] empty[6..11] acc_full[12,13]
-    uint32_t *tptr = reinterpret_cast<uint32_t *>(bars + 20);              // acc_empty[14,15] qready[16,17]
-    volatile int *s_abort = reinterpret_cast<volatile int *>(bars + 21);
+    const MmaSmem L = mma_smem_layout(a.slab_bytes, a.nel_max, a.NSTG);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(mma_smem + L.bars);      // indices MB_*
+    uint32_t *tptr = reinterpret_cast<uint32_t *>(bars + MB_TPTR);
+    volatile int *s_abort = reinterpret_cast<volatile int *>(bars + MB_ABORT);
     double *own = reinterpret_cast<double *>(mma_smem + L.own);
     int *sbad = reinterpret_cast<int *>(mma_smem + L.sbad);
     unsigned char *cst = mma_smem + L.cst;
     unsigned char *slab = mma_smem + L.slab, *ring = mma_smem + L.ring;
 
     if (tid == 0) {
-        for (int s = 0; s < MMA_NSTG; ++s) { mbar_init(smem_u32(bars + s), 1); mbar_init(smem_u32(bars + 6 + s), 1); }
+        for (int s = 0; s < a.NSTG; ++s) { mbar_init(smem_u32(bars + MB_FULL + s), 1); mbar_init(smem_u32(bars + MB_EMPTY + s), 1); }
         for (int m = 0; m < 2; ++m) {
-            mbar_init(smem_u32(bars + 12 + m), 1); mbar_init(smem_u32(bars + 14 + m), 128); mbar_init(smem_u32(bars + 16 + m), 1);
+            mbar_init(smem_u32(bars + MB_ACCF + m), 1); mbar_init(smem_u32(bars + MB_ACCE + m), 128); mbar_init(smem_u32(bars + MB_QRDY + m), 1);
         }
         *s_abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int x = tid; x < 256; x += blockDim.x) sbad[x] = -1;
-    if (tid < a.KC && tid < 64) reinterpret_cast<int *>(bars + 24)[tid] = a.klist[(size_t)c * a.KC + tid];   // KC <= 64 (mma_layout)
+    if (tid < a.KC && tid < 64) reinterpret_cast<int *>(bars + MB_KLIST)[tid] = a.klist[(size_t)c * a.KC + tid];   // KC <= 64 (mma_layout)
     {   // H slab of this CTA: loaded once, resident for the whole run
         const uint4 *src = reinterpret_cast<const uint4 *>(a.slabs + (size_t)c * a.slab_bytes / 2);
         uint4 *dst = reinterpret_cast<uint4 *>(slab);
@@ -451,7 +467,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     const int MT = a.MT, KC = a.KC, NC = a.NC;
 
     const int KCA = a.kcnt[c];                     // K chunks with a non-zero slab part: the others are neither loaded nor multiplied
-    const int *kl = reinterpret_cast<const int *>(bars + 24);      // this CTA's chunk list, copied to shared memory above
+    const int *kl = reinterpret_cast<const int *>(bars + MB_KLIST);      // this CTA's chunk list, copied to shared memory above
     const int kc0 = c % KCA;                       // the chunks are walked from a per-CTA offset: spreads the q reads over the L2 slices
     if (warp >= 4) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
@@ -464,7 +480,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     // Warps 0 / 2 are the producers of tile 0 / 1, warps 1 / 3 the MMA issuers: the two tiles are independent pipelines
     // (own half of the ring stages when both tiles are in use), so a late q^n of one tile never holds up the other.
     const int mt = warp >> 1;
-    const int NSH = MT > 1 ? MMA_NSTG / 2 : MMA_NSTG;
+    const int NSH = MT > 1 ? a.NSTG / 2 : a.NSTG;
     if (mt < MT && (warp & 1) == 0) {
         // ---------------- producer: wait for q^n of the tile, stream it through the ring by TMA ----------
         int stage = 0; unsigned ph = 0;
@@ -472,14 +488,14 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
             poll_flags(a.qflag + (size_t)mt * a.G, lane, a.G, (unsigned)n + 1u, s_abort);
             __syncwarp();
             if (lane == 0) {
-                mbar_arrive(smem_u32(bars + 16 + mt));
+                mbar_arrive(smem_u32(bars + MB_QRDY + mt));
                 asm volatile("fence.proxy.async.global;" ::: "memory");
                 for (int kx = 0; kx < KCA; ++kx) {
                     const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
                     const int sg = NSH * mt + stage;
-                    mbar_wait(smem_u32(bars + 6 + sg), ph ^ 1, s_abort);
-                    mbar_expect_tx(smem_u32(bars + sg), 8192);
-                    tma_bulk_g2s(smem_u32(ring + sg * 8192), a.Qg + ((size_t)mt * KC + kc) * 4096, 8192, smem_u32(bars + sg));
+                    mbar_wait(smem_u32(bars + MB_EMPTY + sg), ph ^ 1, s_abort);
+                    mbar_expect_tx(smem_u32(bars + MB_FULL + sg), 8192);
+                    tma_bulk_g2s(smem_u32(ring + sg * 8192), a.Qg + ((size_t)mt * KC + kc) * 4096, 8192, smem_u32(bars + MB_FULL + sg));
                     if (++stage == NSH) { stage = 0; ph ^= 1; }
                 }
             }
@@ -492,23 +508,23 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
             int stage = 0; unsigned ph = 0;
             const uint32_t td = tbase + (uint32_t)(mt * NC);
             for (int n = 0; n < a.n_steps; ++n) {
-                mbar_wait(smem_u32(bars + 14 + mt), (n & 1) ^ 1, s_abort);              // epilogues of step n-1 left the tile
+                mbar_wait(smem_u32(bars + MB_ACCE + mt), (n & 1) ^ 1, s_abort);         // epilogues of step n-1 left the tile
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 for (int kx = 0; kx < KCA; ++kx) {
-                    const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
+                    const int kp = kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA;          // position in the list = position in the slab
                     const int sg = NSH * mt + stage;
-                    mbar_wait(smem_u32(bars + sg), ph, s_abort);
+                    mbar_wait(smem_u32(bars + MB_FULL + sg), ph, s_abort);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const uint32_t qa = smem_u32(ring + sg * 8192), hb = smem_u32(slab + (size_t)kc * 2 * NC * 32);
+                    const uint32_t qa = smem_u32(ring + sg * 8192), hb = smem_u32(slab + (size_t)kp * 2 * NC * 32);
                     const uint64_t qhi = umma_desc(qa), qlo = umma_desc(qa + 4096);
                     const uint64_t hhi = umma_desc(hb), hlo = umma_desc(hb + NC * 32);
                     umma_bf16(td, qhi, hhi, idesc, kx > 0);
                     umma_bf16(td, qlo, hhi, idesc, 1);
                     umma_bf16(td, qhi, hlo, idesc, 1);
-                    umma_commit(smem_u32(bars + 6 + sg));                               // ring slot free when these MMAs retire
+                    umma_commit(smem_u32(bars + MB_EMPTY + sg));                              // ring slot free when these MMAs retire
                     if (++stage == NSH) { stage = 0; ph ^= 1; }
                 }
-                umma_commit(smem_u32(bars + 12 + mt));                                 // t of tile mt complete
+                umma_commit(smem_u32(bars + MB_ACCF + mt));                                // t of tile mt complete
             }
         }
     }
