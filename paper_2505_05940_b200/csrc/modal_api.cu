@@ -611,7 +611,7 @@ modal_status configure_mma(modal_plan *p)
     CU(m.dqf.ensure((size_t)256 * L.QS * 4));
     CU(m.dGx.ensure((size_t)L.G * 2 * 128 * 4 * L.NG4 * 4));
     CU(m.dfx.ensure((size_t)L.NGRP * 2 * 128 * L.QS * 4));
-    CU(m.dflags.ensure((size_t)L.G * 2 * 4 * 4));
+    CU(m.dflags.ensure((size_t)L.G * 2 * 4 * md::MMA_FS));
     m.ok = true;
     return MODAL_OK;
 }
@@ -715,7 +715,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             CU(cudaMemsetAsync(m.dqf.p, 0, (size_t)256 * L.QS * 4, st));
             CU(cudaMemsetAsync(m.dGx.p, 0, (size_t)L.G * 2 * 128 * 4 * L.NG4 * 4, st));
             CU(cudaMemsetAsync(m.dfx.p, 0, (size_t)L.NGRP * 2 * 128 * L.QS * 4, st));
-            CU(cudaMemsetAsync(m.dflags.p, 0, (size_t)L.G * 2 * 4 * 4, st));
+            CU(cudaMemsetAsync(m.dflags.p, 0, (size_t)L.G * 2 * 4 * md::MMA_FS, st));
             const bool timing = env_int("MODAL_FLOW_TIMING", 0) != 0;
             if (timing) {
                 CU(p->dtiming.ensure((size_t)L.G * 64));

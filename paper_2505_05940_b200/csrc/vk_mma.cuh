@@ -37,6 +37,8 @@ constexpr int MMA_NSTG_MAX = 16;     // launch uses MmaArgs::NSTG stages (8 by d
 constexpr int MB_FULL = 0, MB_EMPTY = 16, MB_ACCF = 32, MB_ACCE = 34, MB_QRDY = 36, MB_TPTR = 40, MB_ABORT = 41, MB_KLIST = 44;
 constexpr int MMA_THREADS = 384;     // warpgroup 0: warps 0 / 2 TMA producers, warps 1 / 3 MMA issuers of tile 0 / 1 (56 registers
                                      // after setmaxnreg); warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (224 registers)
+constexpr int MMA_FS = 8;            // words between the q flags of consecutive CTAs: one flag per 32-byte sector (C3 b256: 1 / 4 /
+                                     // 8 / 16 / 32 words = 16.7 / 15.6 / 15.3 / 15.5 / 15.6 us per step; 147 stores to five lines serialise)
 constexpr int MMA_FB = 11;           // 16-byte partial-force loads in flight per thread while polling (a thread keeps ~16 strong loads in flight)
 
 struct MmaArgs {
@@ -59,7 +61,7 @@ struct MmaArgs {
     float *qf;                  // [256][QS]            q fp32
     uint32_t *Gx;               // [G][2][128][4*NG4]   partial G, tagged
     uint32_t *fx;               // [NGRP][2][128][QS]   partial f, tagged
-    unsigned *qflag;            // [2][G] epochs, one per (tile, CTA)
+    unsigned *qflag;            // [2][G][MMA_FS] epochs, one per (tile, CTA), each in its own 32-byte sector
     long long *timing;          // optional [G][8] cycle counters of tile 0 (MODAL_FLOW_TIMING)
 };
 
@@ -99,7 +101,7 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 // by an L1 invalidate, which throttles them), relaxed polls back to back 21.3 / 13.3, relaxed + 400 ns sleep 16.6 / 12.8;
 // a fence.acq_rel.gpu after relaxed polls measured slower (the MEMBAR stalls the epilogue warps of the other tile).
 // (1.5 us sleep 16.3 / 12.6; sleeping through an estimate of the wait before the first poll 16.5 / 16.5: nanosleep overshoots)
-constexpr unsigned MMA_POLL_SLEEP = 400;      // ns between polling rounds
+constexpr unsigned MMA_POLL_SLEEP = 400;      // ns between polling rounds (with one flag per sector 0 / 200 / 400 / 800 ns: 15.5 / 15.4 / 15.3 / 15.5)
 __device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int count, unsigned epoch, volatile int *abortp)
 {
     for (int base = lane; base < count; base += 256) {
@@ -110,7 +112,7 @@ __device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int coun
             unsigned v[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u)
-                if (pend >> u & 1) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + base + 32 * u) : "memory");
+                if (pend >> u & 1) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + (size_t)(base + 32 * u) * MMA_FS) : "memory");
 #pragma unroll
             for (int u = 0; u < 8; ++u) if ((pend >> u & 1) && v[u] >= epoch) pend &= ~(1u << u);
             if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
@@ -119,8 +121,8 @@ __device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int coun
 #pragma unroll
         for (int u = 0; u < 8; ++u)
             if (base + 32 * u < count) {
-                unsigned v;
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p + base + 32 * u) : "memory");
+                unsigned v;                                                        // value unused: the load is the acquire
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p + (size_t)(base + 32 * u) * MMA_FS) : "memory");
             }
     }
 }
@@ -214,7 +216,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
         if (csm) { skv[e] = kv; skq[e] = kq; sr[e] = rc; }
     }
     bar_named(2 + mt, 128);
-    if (r == 0) set_flag(a.qflag + (size_t)mt * a.G + c, 1u);
+    if (r == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * MMA_FS, 1u);
     for (int u = 0; u < 16; ++u) {                                                // [16][256]: conflict-free
         const int nn = u < NG ? a.nlist[i * NG + u] : -1;
         sreg[u * 256] = nn >= 0 ? sb[nn] : 0.f;
@@ -418,7 +420,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
         }
         if (tmg) { const long long t_ = clock64(); tm[5] += t_ - tk; tk = t_; }
         bar_named(2 + mt, 128);
-        if (r == 0) set_flag(a.qflag + (size_t)mt * a.G + c, (unsigned)n + 2u);
+        if (r == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * MMA_FS, (unsigned)n + 2u);
         if (tmg) { const long long t_ = clock64(); tm[6] += t_ - tk; tk = t_; }
     }
     if (lane == 0)
@@ -485,7 +487,7 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
         // ---------------- producer: wait for q^n of the tile, stream it through the ring by TMA ----------
         int stage = 0; unsigned ph = 0;
         for (int n = 0; n < a.n_steps; ++n) {
-            poll_flags(a.qflag + (size_t)mt * a.G, lane, a.G, (unsigned)n + 1u, s_abort);
+            poll_flags(a.qflag + (size_t)mt * a.G * MMA_FS, lane, a.G, (unsigned)n + 1u, s_abort);
             __syncwarp();
             if (lane == 0) {
                 mbar_arrive(smem_u32(bars + MB_QRDY + mt));
