@@ -395,6 +395,7 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
             fo.z = __shfl_xor_sync(FLOW_FULL, fs.z, 16); fo.w = __shfl_xor_sync(FLOW_FULL, fs.w, 16);
             // first half + second half, in that order on both lanes; lane half hh updates elements 2hh, 2hh+1 of the quad
             const float f2[2] = {hh ? fo.z + fs.z : fs.x + fo.x, hh ? fo.w + fs.w : fs.y + fo.y};
+            float qn[2] = {0.f, 0.f};                                               // the lane's two new values (0 beyond n_q: padding)
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const int e = e4 + 2 * hh + h, k = kq0 + 2 * hh + h;
@@ -409,13 +410,20 @@ __device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int m
                 v = kvv * v - kqq * q + rr * (fe - fd);
                 q += v;
                 sq[e] = q; sv[e] = v;
-                const float qfl = (float)q;
-                a.qf[(size_t)be * QS + k] = qfl;
-                const uint16_t hi = bf16_rn_dev(qfl), lo = bf16_rn_dev(qfl - __uint_as_float((uint32_t)hi << 16));
-                const int k16 = k & 15;
-                const int off = ((re >> 3) * 256 + (k16 >> 3) * 128 + (re & 7) * 16 + (k16 & 7) * 2) >> 1;
-                uint16_t *Qc = Qt + (size_t)(k >> 4) * 4096;
-                Qc[off] = hi; Qc[2048 + off] = lo;
+                qn[h] = (float)q;
+            }
+            // publish the pair (k even, k + 1 < KP): one 8-byte fp32 store and one 4-byte store each for the bf16 hi and lo halves,
+            // which are adjacent in the operand layout
+            const int k0 = kq0 + 2 * hh;
+            if (qact && k0 < a.n_q) {
+                *reinterpret_cast<float2 *>(a.qf + (size_t)be * QS + k0) = make_float2(qn[0], qn[1]);
+                const uint32_t h0 = bf16_rn_dev(qn[0]), h1 = bf16_rn_dev(qn[1]);
+                const uint32_t l0 = bf16_rn_dev(qn[0] - __uint_as_float(h0 << 16)), l1 = bf16_rn_dev(qn[1] - __uint_as_float(h1 << 16));
+                const int k16 = k0 & 15;
+                const int off = (re >> 3) * 256 + (k16 >> 3) * 128 + (re & 7) * 16 + (k16 & 7) * 2;      // bytes, 4-aligned
+                unsigned char *Qc = reinterpret_cast<unsigned char *>(Qt + (size_t)(k0 >> 4) * 4096);
+                *reinterpret_cast<uint32_t *>(Qc + off) = h0 | (h1 << 16);
+                *reinterpret_cast<uint32_t *>(Qc + 4096 + off) = l0 | (l1 << 16);
             }
         }
         if (tmg) { const long long t_ = clock64(); tm[5] += t_ - tk; tk = t_; }
