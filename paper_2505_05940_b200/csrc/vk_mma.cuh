@@ -121,8 +121,8 @@ __device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int coun
 #pragma unroll
         for (int u = 0; u < 8; ++u)
             if (base + 32 * u < count) {
-                unsigned v;                                                        // value unused: the load is the acquire
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p + (size_t)(base + 32 * u) * MMA_FS) : "memory");
+                // the value is not needed: the load is the acquire
+                asm volatile("{\n\t.reg .b32 t;\n\tld.acquire.gpu.global.u32 t, [%0];\n\t}" ::"l"(p + (size_t)(base + 32 * u) * MMA_FS) : "memory");
             }
     }
 }
