@@ -26,7 +26,10 @@
  *    from modal_last_error(); for a failed modal_plan_create (*out == NULL) pass NULL.
  *  - Modes beyond the stability limit of the scheme are masked (q_k == 0, excluded from
  *    force, projection and read-out; reading R11); masking is a warning.
- *  - Thread safety: calls on different plans may run concurrently; calls on one plan may not.
+ *  - Thread safety: calls on different plans may run concurrently; calls on one plan may not, and a plan
+ *    carries ONE simulation at a time: its exchange buffers and device state belong to the last
+ *    modal_simulate call, so a second call on the same plan must wait for the first to finish
+ *    (modal_plan_check, or a synchronised stream), also when the two use different streams.
  */
 #ifndef MODAL_H_
 #define MODAL_H_
@@ -39,7 +42,7 @@ typedef struct modal_plan modal_plan; /* opaque, owned by the library */
 
 typedef enum {
     MODAL_OK = 0,
-    MODAL_EINVAL = 1,    /* descriptor / argument validation failed                        */
+    MODAL_EINVAL = 1,    /* descriptor / argument validation failed (e.g. FTM with a mode omega <= sigma) */
     MODAL_EINCOMPAT = 2, /* valid request this build cannot run (size limits)              */
     MODAL_EUNSTABLE = 3, /* a sample went non-finite; first_bad_step says where            */
     MODAL_ECUDA = 4,     /* CUDA runtime error, or no device attached to the plan          */
@@ -108,7 +111,9 @@ typedef struct {
  * first_bad_step: host [batch] or NULL.  When non-NULL the call synchronises the stream and
  *   fills first_bad_step[b] with the first n at which sample b's state was non-finite (-1 if
  *   none) and returns MODAL_EUNSTABLE iff any is >= 0; the finite prefix of the output is valid.
- *   When NULL the work is only enqueued on `cuda_stream` (a cudaStream_t, NULL = default).
+ *   When NULL the work is only enqueued on `cuda_stream` (a cudaStream_t, NULL = default) and nothing
+ *   the kernels detect (instability, a cross-CTA exchange that timed out) can be reported by this call:
+ *   follow it with modal_plan_check.
  * Errors: MODAL_EINVAL (batch/steps outside the plan, missing q0), MODAL_ECUDA. */
 modal_status modal_simulate(modal_plan *plan, int batch, int n_steps, const modal_init *init,
                             float *out_audio_dev, int *first_bad_step, void *cuda_stream);
@@ -117,6 +122,24 @@ modal_status modal_simulate(modal_plan *plan, int batch, int n_steps, const moda
  * device memory (host<->device copies included).  Always synchronous. */
 modal_status modal_simulate_host(modal_plan *plan, int batch, int n_steps, const modal_init *init,
                                  float *out_audio_host, int *first_bad_step);
+
+/* Completes the plan's last modal_simulate call: synchronises the stream it was enqueued on, fills
+ * first_bad_step (host [batch of that call], may be NULL) and returns MODAL_EUNSTABLE / MODAL_ECUDA (a bounded
+ * wait of a persistent kernel gave up: the CTAs of a team were not co-resident) / MODAL_OK. */
+modal_status modal_plan_check(modal_plan *plan, int *first_bad_step);
+
+/* Launch-selection overrides for tests and sweeps (the defaults are automatic).  Keys:
+ *   "vk_impl"      0 automatic, 1 FP32 flow kernel, 2 tcgen05 batched kernel
+ *   "flow_g"       CTAs per team of the flow kernel (0 automatic)
+ *   "flow_ns"      TMA ring slots of the flow kernel (0: none, streamed tiles are read directly from L2)
+ *   "flow_res"     resident tiles per CTA of the flow kernel (-1 automatic)
+ *   "mma_split"    k blocks per mode class of the batched kernel (0 automatic)
+ *   "mma_ng"       in-plane modes per CTA of the batched kernel (0 automatic)
+ *   "mma_nstg"     operand ring stages of the batched kernel (0 automatic)
+ *   "parity_order" 1 (default): transverse modes grouped by index parity on the device; 0: plan order
+ *   "timing"       1: per-phase cycle counters of the persistent kernels, printed to stderr (synchronous)
+ * Returns MODAL_EINVAL for an unknown key or a value out of range. */
+modal_status modal_plan_set_option(modal_plan *plan, const char *key, int value);
 
 void modal_plan_destroy(modal_plan *plan);
 const char *modal_last_error(const modal_plan *plan);
@@ -136,13 +159,21 @@ typedef enum {
     MODAL_Q_ACTIVE = 9,      /* int    [coeff_batch][n_q]   1 = active, 0 = masked (R11)            */
     MODAL_Q_H_FULL = 10,     /* double [n_phi][n_q][n_q]: the fp32 values the device holds, widened */
     MODAL_Q_COEFF_BATCH = 11,/* int    [1]                                                          */
-    MODAL_Q_KERNEL_INFO = 12,/* int    [8]: kernel family, cluster size, clusters, threads, smem    */
+    MODAL_Q_KERNEL_INFO = 12,/* int    [8] of the last launch: kernel family (1 tension, 3 flow, 4 batched tcgen05), CTAs */
+                             /*        per team (flow) or CTAs (batched), teams (flow) or n groups (batched), threads,  */
+                             /*        dynamic shared memory bytes, flags (1: H resident in shared memory, 2: team of   */
+                             /*        several CTAs), ring slots (flow) or accumulator slots (batched), padded n_q      */
+    MODAL_Q_MMA_LAYOUT = 14, /* int    [16]: layout the batched tcgen05 kernel would use (host side, no device needed):  */
+                             /*        fits, k blocks, n groups, modes per group, TMEM columns per slot, slots, columns */
+                             /*        per mode, quads per block, K chunks, most K chunks of a CTA, CTAs, rows owned,   */
+                             /*        fewest / most K chunks of a CTA, slab KiB, most source blocks of a CTA           */
+    MODAL_Q_MMA_SLAB_CHECK = 15, /* double [3]: non-zero entries of H covered by the operand slabs, non-zero entries of */
+                             /*        H, max |hi + lo - H| / max |H| (host-side self check of the packing)             */
     MODAL_Q_TILE_STATS = 13  /* int    [2]: 16x16 tiles of the packed H, and how many hold a non-zero.   */
                              /*        The device keeps the transverse modes grouped by index parity   */
                              /*        (internal order only: every array of this API is in plan order),*/
                              /*        so that the parity zeros of H fill whole  */
                              /*        tiles, which the step kernel never reads.                       */
-                             /*        bytes, resident flag, tiles per n, padded n_q (last launch)  */
 } modal_query;
 /* Copies the item into `dst` (capacity `dst_bytes`); returns MODAL_EINVAL if it does not fit. */
 modal_status modal_plan_query(const modal_plan *plan, int what, void *dst, unsigned long long dst_bytes);

@@ -19,7 +19,7 @@ LINEAR, TENSION, VK = 0, 1, 2
 SV, FTM = 0, 1
 STRING, RECT = 0, 1
 (Q_MODE_M, Q_MODE_N, Q_PHI_M, Q_PHI_N, Q_LAMBDA, Q_OMEGA, Q_SIGMA, Q_NL_SCALE, Q_PICKUP, Q_ACTIVE,
- Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO, Q_TILE_STATS) = range(14)
+ Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO, Q_TILE_STATS, Q_MMA_LAYOUT, Q_MMA_SLAB_CHECK) = range(16)
 
 _dp = C.POINTER(C.c_double)
 _fp = C.POINTER(C.c_float)
@@ -54,8 +54,8 @@ class SampleGeom(C.Structure):
 
 
 EXPORTS = ["modal_plan_create", "modal_coeffs_upload", "modal_simulate", "modal_simulate_host",
-           "modal_plan_destroy", "modal_last_error", "modal_plan_query", "modal_derive_coeffs",
-           "modal_project_bump"]
+           "modal_plan_check", "modal_plan_set_option", "modal_plan_destroy", "modal_last_error",
+           "modal_plan_query", "modal_derive_coeffs", "modal_project_bump"]
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2505_05940_b200.build` "
@@ -65,6 +65,8 @@ lib.modal_plan_create.argtypes = [C.POINTER(PlanDesc), C.c_int, C.POINTER(C.c_vo
 lib.modal_coeffs_upload.argtypes = [C.c_void_p, C.POINTER(Coeffs)]
 lib.modal_simulate.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(Init), C.c_void_p, _ip, C.c_void_p]
 lib.modal_simulate_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(Init), _fp, _ip]
+lib.modal_plan_check.argtypes = [C.c_void_p, _ip]
+lib.modal_plan_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int]
 lib.modal_plan_destroy.argtypes = [C.c_void_p]
 lib.modal_plan_destroy.restype = None
 lib.modal_last_error.argtypes = [C.c_void_p]
@@ -135,6 +137,16 @@ class Plan:
         self._check(st, allow=(EUNSTABLE,))
         return st, fb
 
+    def check(self, batch=None):
+        """modal_plan_check: completes the last (asynchronous) simulate.  Returns (status, first_bad or None)."""
+        fb = None if batch is None else np.empty(batch, np.int32)
+        st = lib.modal_plan_check(self._h, _ptr(fb, _ip))
+        self._check(st, allow=(EUNSTABLE,))
+        return st, fb
+
+    def set_option(self, key: str, value: int):
+        return self._check(lib.modal_plan_set_option(self._h, key.encode(), int(value)))
+
     def simulate_host(self, q0, n_steps, qm1=None, out=None):
         q0 = _arr(np.atleast_2d(q0)); qm1 = None if qm1 is None else _arr(np.atleast_2d(qm1))
         batch = q0.shape[0]
@@ -158,7 +170,8 @@ class Plan:
             Q_LAMBDA: ((nq,), np.float64), Q_OMEGA: ((cb, nq), np.float64), Q_SIGMA: ((cb, nq), np.float64),
             Q_NL_SCALE: ((cb, nnl), np.float64), Q_PICKUP: ((cb, nq), np.float64),
             Q_ACTIVE: ((cb, nq), np.int32), Q_H_FULL: ((nphi, nq, nq), np.float64),
-            Q_COEFF_BATCH: ((1,), np.int32), Q_KERNEL_INFO: ((8,), np.int32), Q_TILE_STATS: ((2,), np.int32)}[what]
+            Q_COEFF_BATCH: ((1,), np.int32), Q_KERNEL_INFO: ((8,), np.int32), Q_TILE_STATS: ((2,), np.int32),
+            Q_MMA_LAYOUT: ((16,), np.int32), Q_MMA_SLAB_CHECK: ((3,), np.float64)}[what]
         a = np.zeros(shape, dt)
         self._check(lib.modal_plan_query(self._h, what, a.ctypes.data_as(C.c_void_p), a.nbytes))
         return a
@@ -199,10 +212,12 @@ def desc_from_workload(wl: dict, scheme=SV, lossless=False, max_batch=None, max_
                     max_batch=max_batch or wl["batch"], max_steps=max_steps or wl["n_steps"])
 
 
-def plan_from_workload(wl: dict, device=0, scheme=SV, lossless=False):
+def plan_from_workload(wl: dict, device=0, scheme=SV, lossless=False, options=None):
     """Create a plan for a workload dict (workloads.py), upload per-sample coefficients where the
     samples differ in geometry, and project the excitation.  Returns (plan, q0[batch][n_q])."""
     plan = Plan(desc_from_workload(wl, scheme, lossless), device)
+    for k, v in (options or {}).items():
+        plan.set_option(k, v)
     B = wl["batch"]
     q0 = np.empty((B, wl["n_q"]))
     if wl["model"] in ("vk", "berger"):

@@ -1,7 +1,6 @@
 // host_math.hpp -- host-side (fp64) derivations of the product path: mode index sets,
 // oscillator and scheme coefficients, the closed-form coupling tensor of the simply supported
-// plate, its tile-packed device layout, the work schedule of the vK kernel and the projection
-// of the excitation bump.  Independent of oracle/ (no shared code or tables).
+// plate and the projection of the excitation bump (device layouts: flow_schedule.hpp, mma_schedule.hpp).  Independent of oracle/ (no shared code or tables).
 #pragma once
 #include <algorithm>
 #include <cmath>
@@ -12,7 +11,6 @@
 namespace modal_host {
 
 constexpr double PI = 3.141592653589793238462643383279502884;
-constexpr int TILE = 16;
 
 struct ModeSet {
     std::vector<int> m, n;       // string: n[k] = 0
@@ -128,114 +126,6 @@ inline double H_bracket(int mp, int np, int mq, int nq, int mn, int nn)
     return A * S3(mp, mq, mn) * S3(np, nq, nn) - B * C3(mp, mq, mn) * C3(np, nq, nn);
 }
 inline double H_geom(double Lx, double Ly) { return 8.0 * std::pow(PI, 4) * std::pow(Lx * Ly, -2.5); }
-
-// ---- tile-packed layout ---------------------------------------------------------------
-// H^n is symmetric: only tiles (I,J), J <= I, of the 16x16 tiling of the zero-padded matrix
-// are stored, tile index I(I+1)/2 + J, row-major inside the tile.  In diagonal tiles the
-// strict upper part is zero and the diagonal is halved, so that "row pass + transposed
-// column pass" over the stored tiles yields exactly H^n q.
-inline int tiles_per_n(int n_q) { const int nt = (n_q + TILE - 1) / TILE; return nt * (nt + 1) / 2; }
-inline int padded_nq(int n_q) { return ((n_q + TILE - 1) / TILE) * TILE; }
-
-template <class Get>   // Get(n,p,q) -> double
-inline void pack_tiles(int n_q, int n_phi, Get get, std::vector<float> &Ht)
-{
-    const int nt = (n_q + TILE - 1) / TILE, tpn = nt * (nt + 1) / 2;
-    Ht.assign((size_t)n_phi * tpn * TILE * TILE, 0.f);
-    for (int n = 0; n < n_phi; ++n)
-        for (int I = 0; I < nt; ++I)
-            for (int J = 0; J <= I; ++J) {
-                float *t = &Ht[((size_t)n * tpn + I * (I + 1) / 2 + J) * TILE * TILE];
-                for (int i = 0; i < TILE; ++i)
-                    for (int j = 0; j < TILE; ++j) {
-                        const int p = I * TILE + i, q = J * TILE + j;
-                        if (p >= n_q || q >= n_q || q > p) continue;
-                        const double v = get(n, p, q);
-                        t[i * TILE + j] = (float)(p == q ? 0.5 * v : v);
-                    }
-            }
-}
-
-// inverse of pack_tiles (the fp32 values the device holds, as a full symmetric tensor)
-inline void unpack_tiles(int n_q, int n_phi, const std::vector<float> &Ht, double *H)
-{
-    const int nt = (n_q + TILE - 1) / TILE, tpn = nt * (nt + 1) / 2;
-    for (int n = 0; n < n_phi; ++n)
-        for (int p = 0; p < n_q; ++p)
-            for (int q = 0; q <= p; ++q) {
-                const int I = p / TILE, J = q / TILE;
-                const float t = Ht[((size_t)n * tpn + I * (I + 1) / 2 + J) * TILE * TILE + (p % TILE) * TILE + (q % TILE)];
-                const double v = p == q ? 2.0 * (double)t : (double)t;
-                H[((size_t)n * n_q + p) * n_q + q] = v;
-                H[((size_t)n * n_q + q) * n_q + p] = v;
-            }
-}
-
-// ---- work schedule of the vK team kernel ---------------------------------------------
-struct Unit { int n, I, nloc, tpoff, gtile0, ltile0, pad0, pad1; };   // == modal_dev::VkUnit
-
-struct Schedule {
-    int CS = 1, NCL = 1, NW = 16, NLOC_MAX = 0;
-    int max_cta_units = 0, max_tp = 0, max_cta_tiles = 0;
-    std::vector<int> nlo;            // [NCL+1]
-    std::vector<Unit> units;         // CTA-major, warp-major
-    std::vector<int> warp_ptr;       // [NCL*CS*NW][2]
-    std::vector<int> cta_ptr;        // [NCL*CS][2]
-};
-
-// In-plane modes are split into NCL contiguous ranges (one per cluster of the team); inside a
-// cluster the tile rows (n, I) are spread over CS*NW warps by longest-processing-time-first.
-inline Schedule build_schedule(int n_q, int n_phi, int CS, int NCL, int NW)
-{
-    Schedule s;
-    s.CS = CS; s.NCL = NCL; s.NW = NW;
-    const int nt = (n_q + TILE - 1) / TILE, tpn = nt * (nt + 1) / 2;
-    s.nlo.resize(NCL + 1);
-    for (int c = 0; c <= NCL; ++c) s.nlo[c] = (int)((long long)n_phi * c / NCL);
-    s.warp_ptr.assign((size_t)NCL * CS * NW * 2, 0);
-    s.cta_ptr.assign((size_t)NCL * CS * 2, 0);
-    const double unit_overhead = 1.5;   // tile-equivalents of per-unit epilogue work
-    for (int c = 0; c < NCL; ++c) {
-        s.NLOC_MAX = std::max(s.NLOC_MAX, s.nlo[c + 1] - s.nlo[c]);
-        struct U { int n, I; };
-        std::vector<U> us;
-        for (int n = s.nlo[c]; n < s.nlo[c + 1]; ++n)
-            for (int I = nt - 1; I >= 0; --I) us.push_back({n, I});
-        std::stable_sort(us.begin(), us.end(), [](const U &a, const U &b) { return a.I > b.I; });
-        const int W = CS * NW;
-        std::vector<double> load(W, 0.0);
-        std::vector<std::vector<U>> lists(W);
-        for (const U &u : us) {
-            int best = 0;
-            for (int w = 1; w < W; ++w) if (load[w] < load[best]) best = w;
-            load[best] += u.I + 1 + unit_overhead;
-            lists[best].push_back(u);
-        }
-        // warp w of the cluster -> CTA (w % CS), warp slot (w / CS): spreads heavy warps over CTAs
-        for (int r = 0; r < CS; ++r) {
-            const int cta = c * CS + r;
-            int tp = 0, lt = 0;
-            s.cta_ptr[cta * 2] = (int)s.units.size();
-            for (int wi = 0; wi < NW; ++wi) {
-                const std::vector<U> &L = lists[wi * CS + r];
-                s.warp_ptr[((size_t)cta * NW + wi) * 2] = (int)s.units.size();
-                s.warp_ptr[((size_t)cta * NW + wi) * 2 + 1] = (int)L.size();
-                for (const U &u : L) {
-                    Unit d{u.n, u.I, u.n - s.nlo[c], tp, u.n * tpn + u.I * (u.I + 1) / 2, lt, 0, 0};
-                    s.units.push_back(d);
-                    tp += (u.I + 1) * TILE;
-                    lt += u.I + 1;
-                }
-            }
-            const int cnt = (int)s.units.size() - s.cta_ptr[cta * 2];
-            s.cta_ptr[cta * 2 + 1] = cnt;
-            s.max_cta_units = std::max(s.max_cta_units, cnt);
-            s.max_tp = std::max(s.max_tp, tp);
-            s.max_cta_tiles = std::max(s.max_cta_tiles, lt);
-        }
-    }
-    return s;
-}
 
 // ---- excitation projection (reading R13) -------------------------------------------------
 // Gauss-Legendre nodes on [-1,1] by Newton iteration on P_n.

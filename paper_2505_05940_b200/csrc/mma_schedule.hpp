@@ -3,11 +3,16 @@
 //
 // Per time step and sample the kernel forms t[n][k] = sum_r H^n[k][r] q[r] (Eq. 9 in
 // one pass, C eliminated by PAPER.md:283) as a GEMM  D[b][(n,k)] = Q[b][r] * Hs[(n,k)][r]^T  on
-// tcgen05 tensor cores: M = 128 samples per tile, K = padded N_q, N = the (n,k) columns of a CTA.
-// CTA (i,j) of the NGRP x NKB grid owns in-plane modes n of group i and the RB rows k of block j
-// (B-operand row = local mode * RB + local k).
+// tcgen05 tensor cores: M = 128 samples per tile, K = the transverse modes r, N = the (n,k) columns of a CTA.
+// CTA (i,j) of the NGRP x NKB grid owns the in-plane modes n of group i and the rows k of block j.
 // Operands are bf16 split hi + lo; three MMAs (hi*hi + lo*hi + hi*lo) per K chunk give ~2^-17
 // relative accuracy, which the 1e-4 parity tolerance needs.
+//
+// Operand order of the transverse modes.  The k blocks are contiguous ranges of the plan's INTERNAL mode
+// order, aligned to its classes (for the sine-basis plate: the four index parities); every
+// block starts on a 16-element boundary of the operand K axis (koff), so a K chunk of 16 never straddles two
+// blocks.  H^n couples a parity class of k with ONE parity class of r, so a CTA's slab is non-zero in only a few K
+// chunks; the host lists them per CTA from the actual non-zeros of H (an uploaded dense H simply lists them all).
 //
 // Shared-memory operand layout (UMMA canonical K-major, no swizzle): a chunk of R rows x 16 K
 // elements (bf16) is R*32 bytes; 8-row x 8-element core matrices of 128 contiguous bytes, the two
@@ -33,115 +38,200 @@ inline float bf16_to_float(uint16_t h) { uint32_t u = (uint32_t)h << 16; float f
 // byte offset of element (row r, k in 0..15) inside a canonical chunk
 inline int umma_chunk_off(int r, int k) { return (r >> 3) * 256 + ((k >> 3) & 1) * 128 + (r & 7) * 16 + (k & 7) * 2; }
 
+constexpr int MMA_RB_MAX = 56;      // most rows k of one block (the epilogue keeps a sample's block of q in registers)
+constexpr int MMA_NG_MAX = 8;       // most in-plane modes of one group
+constexpr int MMA_KCL_MAX = 64;     // most K chunks one CTA multiplies
+constexpr int MMA_FBLK_MAX = 16;    // most k blocks whose owners a CTA waits for
+constexpr int MMA_MT_MAX = 8;       // most M tiles (of 128 samples) of one launch
+
+struct MmaBlock { int k0, nb, koff; };            // first internal mode, modes, offset on the operand K axis (multiple of 16)
+
 struct MmaLayout {
-    int n_q = 0, n_phi = 0, KP = 0, KC = 0;     // padded K, K chunks of 16
-    int NKB = 0, RB = 0;                        // k blocks, rows k per block (multiple of 4, <= 32)
-    int NGRP = 0, NG = 0, NC = 0;               // n groups, modes per group, operand columns per CTA (>= NG*RB, multiple of 16)
-    int NG4 = 0;                                // float4 per partial-G row: ceil(NG / 4)
-    int QS = 0;                                 // row stride (floats) of the q / partial-f exchange rows: max(KP, NKB*RB)
-    int G = 0;                                  // CTAs = NGRP * NKB
-    int nel_max = 0;                            // most (sample, k) elements one CTA owns per M tile
-    size_t slab_bytes = 0;                      // per CTA: KC * 2 (hi, lo) * NC * 32
+    int n_q = 0, n_phi = 0;
+    int NKB = 0;                                // k blocks
+    std::vector<MmaBlock> blocks;
+    int RBT = 0;                                // TMEM columns per in-plane mode: 32 or 64 (>= the largest block)
+    int RBQ = 0;                                // quads (4 consecutive k) per block in the exchange rows: ceil(max nb / 4)
+    int KP = 0, KC = 0;                         // operand K extent (sum of the padded blocks), chunks of 16
+    int NGRP = 0, NG = 0, NG4 = 0;              // n groups, most modes per group, float4 per partial-G row
     std::vector<int> nlist;                     // [NGRP][NG] in-plane modes of each group (-1: empty slot)
-    std::vector<int> klist, kcnt;               // [G][KC], [G]: the K chunks in which a CTA's slab holds a non-zero (pack_mma_slabs)
+    int NC = 0;                                 // TMEM columns of one accumulator slot = NG * RBT (multiple of 16, <= 256)
+    int S = 0;                                  // accumulator slots in TMEM: min(3, 512 / NC)
+    int G = 0;                                  // CTAs = NGRP * NKB
+    int rows_max = 0;                           // most sample rows of a tile one CTA owns for the update
+    int KCL = 0;                                // most K chunks of any CTA (slab size)
+    size_t slab_bytes = 0;                      // per CTA: KCL * 2 (hi, lo) * NC * 32
+    std::vector<int> klist, kcnt;               // [G][KCL], [G]: global K chunks in which a CTA's slab holds a non-zero
+    std::vector<int> fblk, fcnt;                // [G][MMA_FBLK_MAX], [G]: k blocks whose owners publish what the CTA reads (own block first)
+    double cost = 0;
 };
 
 inline int mma_rows_owned_max(int NGRP) { return (128 + NGRP - 1) / NGRP; }
 
-// One candidate shape; false if it does not fit.  smem_fixed = bytes besides the slab and the owner state.
-// mode_class (optional, [n_phi]): modes of one group share a class.  For the sine-basis tensor the class is the index
-// parity of the in-plane mode: H^n then couples a parity class of k only with one parity class of r, so most K chunks
-// of a CTA's slab are zero and are skipped.
-inline bool mma_layout_try(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, int NKB, int rb_align,
-                           const std::vector<int> *mode_class, MmaLayout &L)
+// k blocks: every class (contiguous range of the internal order; class_start has ncls+1 entries) cut into
+// `split` nearly equal parts, more if a part would exceed MMA_RB_MAX.
+inline void mma_blocks(const std::vector<int> &class_start, int split, std::vector<MmaBlock> &blocks)
 {
-    L.n_q = n_q; L.n_phi = n_phi;
-    L.KC = (n_q + 15) / 16; L.KP = L.KC * 16;
-    L.NKB = NKB;
-    L.RB = ((n_q + NKB - 1) / NKB + rb_align - 1) / rb_align * rb_align;
-    if (L.RB > 32 || NKB > sm || L.KC > 64) return false;
-    if (NKB > 1 && (NKB - 1) * L.RB >= n_q) return false;          // an empty k block
-    const int max_groups = std::min(n_phi, sm / NKB);
-    if (max_groups < 1) return false;
-    std::vector<std::vector<int>> cls(4);
-    for (int n = 0; n < n_phi; ++n) cls[mode_class ? ((*mode_class)[n] & 3) : 0].push_back(n);
-    for (L.NG = (n_phi + max_groups - 1) / max_groups; L.NG <= 16; ++L.NG) {
-        L.NGRP = 0;
-        for (const auto &v : cls) L.NGRP += ((int)v.size() + L.NG - 1) / L.NG;
-        if (L.NGRP <= max_groups) break;
+    blocks.clear();
+    int koff = 0;
+    for (size_t c = 0; c + 1 < class_start.size(); ++c) {
+        const int k0 = class_start[c], len = class_start[c + 1] - k0;
+        if (len <= 0) continue;
+        int parts = std::max(split, (len + MMA_RB_MAX - 1) / MMA_RB_MAX);
+        parts = std::min(parts, len);
+        for (int p = 0; p < parts; ++p) {
+            const int a = k0 + (int)((long long)len * p / parts), b = k0 + (int)((long long)len * (p + 1) / parts);
+            blocks.push_back({a, b - a, koff});
+            koff += (b - a + 15) / 16 * 16;
+        }
     }
-    L.NC = (L.NG * L.RB + 15) / 16 * 16;
-    if (L.NG > 16 || L.NC > 256) return false;
-    L.NG4 = (L.NG + 3) / 4;
-    L.QS = std::max(L.KP, L.NKB * L.RB);
+}
+
+// One candidate shape: blocks given, NG modes per group.  mode_class [n_phi]: modes of one group share a class.
+// `nz(n, k_int, r_int)` tells whether H^n[k][r] is non-zero.  Returns false if the shape does not fit the machine.
+template <class NZ>
+inline bool mma_layout_try(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, const std::vector<MmaBlock> &blocks,
+                           int NG, const std::vector<int> &mode_class, NZ nz, MmaLayout &L)
+{
+    L = MmaLayout();
+    L.n_q = n_q; L.n_phi = n_phi; L.blocks = blocks; L.NKB = (int)blocks.size();
+    if (L.NKB < 1 || L.NKB > MMA_FBLK_MAX - 1 || NG < 1 || NG > MMA_NG_MAX) return false;
+    int nbmax = 0;
+    for (const MmaBlock &b : blocks) nbmax = std::max(nbmax, b.nb);
+    if (nbmax > MMA_RB_MAX) return false;
+    L.RBT = nbmax <= 32 ? 32 : 64; L.RBQ = (nbmax + 3) / 4;      // the epilogue reads the accumulator in units of 32 columns
+    L.KP = blocks.back().koff + (blocks.back().nb + 15) / 16 * 16; L.KC = L.KP / 16;
+    std::vector<std::vector<int>> cls(4);
+    for (int n = 0; n < n_phi; ++n) cls[mode_class[n] & 3].push_back(n);
+    L.NG = NG; L.NG4 = (NG + 3) / 4;
+    L.NGRP = 0;
+    for (const auto &v : cls) L.NGRP += ((int)v.size() + NG - 1) / NG;
     L.G = L.NGRP * L.NKB;
-    L.nel_max = mma_rows_owned_max(L.NGRP) * L.RB;
-    L.slab_bytes = (size_t)L.KC * 2 * L.NC * 32;
-    if (L.slab_bytes + smem_fixed + (size_t)2 * L.nel_max * (L.nel_max <= 512 ? 40 : 16) > smem_limit) return false;
-    L.nlist.assign((size_t)L.NGRP * L.NG, -1);
-    int g = 0;
-    for (const auto &v : cls)
-        for (size_t x = 0; x < v.size(); x += L.NG, ++g)
-            for (int u = 0; u < L.NG && x + u < v.size(); ++u) L.nlist[(size_t)g * L.NG + u] = v[x + u];
+    if (L.G > sm || L.NGRP > 128) return false;
+    L.NC = NG * L.RBT;
+    if (L.NC > 256) return false;
+    L.S = std::min(3, 512 / L.NC);
+    L.rows_max = mma_rows_owned_max(L.NGRP);
+    L.nlist.assign((size_t)L.NGRP * NG, -1);
+    {   // groups: the modes of a class spread evenly over its groups (balanced MMA work)
+        int g = 0;
+        for (const auto &v : cls) {
+            const int ng = ((int)v.size() + NG - 1) / NG;
+            for (int x = 0; x < ng; ++x) {
+                const int a = (int)((long long)v.size() * x / ng), b = (int)((long long)v.size() * (x + 1) / ng);
+                for (int u = a; u < b; ++u) L.nlist[(size_t)(g + x) * NG + (u - a)] = v[u];
+            }
+            g += ng;
+        }
+    }
+    // K chunks and source blocks of every CTA from the non-zeros of its part of H
+    const int KC = L.KC;
+    std::vector<int> chunk_block(KC, 0);
+    for (int j = 0; j < L.NKB; ++j)
+        for (int kc = blocks[j].koff / 16; kc < (blocks[j].koff + blocks[j].nb + 15) / 16; ++kc) chunk_block[kc] = j;
+    std::vector<std::vector<int>> lists(L.G);
+    L.KCL = 1;
+    for (int i = 0; i < L.NGRP; ++i)
+        for (int j = 0; j < L.NKB; ++j) {
+            std::vector<char> used(KC, 0);
+            for (int nl = 0; nl < NG; ++nl) {
+                const int n = L.nlist[(size_t)i * NG + nl];
+                if (n < 0) continue;
+                for (int kk = 0; kk < blocks[j].nb; ++kk)
+                    for (int jr = 0; jr < L.NKB; ++jr)
+                        for (int rr = 0; rr < blocks[jr].nb; ++rr)
+                            if (!used[(blocks[jr].koff + rr) >> 4] && nz(n, blocks[j].k0 + kk, blocks[jr].k0 + rr))
+                                used[(blocks[jr].koff + rr) >> 4] = 1;
+            }
+            std::vector<int> &l = lists[(size_t)i * L.NKB + j];
+            for (int kc = 0; kc < KC; ++kc) if (used[kc]) l.push_back(kc);
+            if (l.empty()) l.push_back(blocks[j].koff / 16);     // at least one chunk, so that the accumulator is always written
+            L.KCL = std::max(L.KCL, (int)l.size());
+        }
+    if (L.KCL > MMA_KCL_MAX) return false;
+    L.slab_bytes = (size_t)L.KCL * 2 * L.NC * 32;
+    const size_t own = (size_t)MMA_MT_MAX * L.rows_max * L.RBQ * 4 * 44;          // fp64 (q, v, kv, kq, r) + fp32 w of the owned elements, every tile
+    if (L.slab_bytes + smem_fixed + own + (size_t)2 * L.KCL * 8192 > smem_limit) return false;   // ring: at least two tiles' chunks
+    L.klist.assign((size_t)L.G * L.KCL, 0); L.kcnt.assign(L.G, 0);
+    L.fblk.assign((size_t)L.G * MMA_FBLK_MAX, 0); L.fcnt.assign(L.G, 0);
+    for (int c = 0; c < L.G; ++c) {
+        const std::vector<int> &l = lists[c];
+        L.kcnt[c] = (int)l.size();
+        for (size_t x = 0; x < l.size(); ++x) L.klist[(size_t)c * L.KCL + x] = l[x];
+        int *fb = &L.fblk[(size_t)c * MMA_FBLK_MAX];
+        int cnt = 0;
+        fb[cnt++] = c % L.NKB;                                   // own block: the epilogue reads this sample's q over it
+        for (int kc : l) {
+            const int jb = chunk_block[kc];
+            bool seen = false;
+            for (int x = 0; x < cnt; ++x) seen |= fb[x] == jb;
+            if (!seen) fb[cnt++] = jb;
+        }
+        L.fcnt[c] = cnt;
+    }
+    // rough cost of one tile-step in SM cycles (per CTA): MMA issue, L2 bytes at ~32 B/clk/SM, owner gather (16 strong
+    // loads in flight per lane, 64 lanes per team) and a latency term for the hops
+    const double mma = (double)L.KCL * 3.0 * L.NC / 2.0;
+    const double bytes = (double)L.KCL * 8192 + 128.0 * L.RBQ * 16 * 2 + (double)L.NGRP * L.rows_max * L.RBQ * 16 + 128.0 * L.NG4 * 16 * L.NKB;
+    const double gather = 700.0 * std::ceil((double)L.NGRP * L.rows_max * L.RBQ / (16.0 * 64.0));
+    const double idle = (double)(sm - L.G) / sm;
+    L.cost = (std::max(mma, bytes / 32.0) + gather + 30.0 * L.NGRP) * (1.0 + idle);
     return true;
 }
 
-// Shape choice: the MMA time of a tile is ~ KC * 3 * NC / 2 cycles; the G hop reads NKB * NG4 rows per
-// thread, the f hop NGRP partials per owned element.  force_nkb > 0 pins the number of k blocks
-// (MODAL_MMA_NKB, tests / sweeps); rb_align = 16 keeps every tcgen05.ld column offset 16-aligned.
-inline bool mma_layout(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, int force_nkb, int rb_align,
-                       const std::vector<int> *mode_class, MmaLayout &L)
+// Shape choice over the class splits and group sizes.  force_split / force_ng > 0 pin them (plan options, tests / sweeps).
+template <class NZ>
+inline bool mma_layout(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, const std::vector<int> &class_start,
+                       const std::vector<int> &mode_class, NZ nz, int force_split, int force_ng, MmaLayout &L)
 {
-    double best = 1e300; bool found = false;
-    const int KC = (n_q + 15) / 16;
-    for (int NKB = 1; NKB <= std::min(4 * KC, sm); ++NKB) {
-        if (force_nkb > 0 && NKB != force_nkb) continue;
-        MmaLayout T;
-        if (!mma_layout_try(n_q, n_phi, sm, smem_limit, smem_fixed, NKB, rb_align, mode_class, T)) continue;
-        const double mma = (double)T.KC * 3.0 * T.NC / 2.0;
-        const double ghop = T.NKB > 1 ? 600.0 + 40.0 * T.NKB * T.NG4 : 0.0;
-        const double fhop = 600.0 + 12.0 * T.NGRP * ((T.nel_max + 127) / 128);
-        const double cost = mma + ghop + fhop;
-        if (cost < best) { best = cost; L = T; found = true; }
+    bool found = false;
+    for (int split = 1; split <= 4; ++split) {
+        if (force_split > 0 && split != force_split) continue;
+        std::vector<MmaBlock> blocks;
+        mma_blocks(class_start, split, blocks);
+        for (int NG = 1; NG <= MMA_NG_MAX; ++NG) {
+            if (force_ng > 0 && NG != force_ng) continue;
+            MmaLayout T;
+            if (!mma_layout_try(n_q, n_phi, sm, smem_limit, smem_fixed, blocks, NG, mode_class, nz, T)) continue;
+            if (!found || T.cost < L.cost) { L = T; found = true; }
+        }
     }
     return found;
 }
 
-// Per-CTA operand slabs: [G][KC][2][NC*32 bytes]; CTA c = i * NKB + j; operand row = nl * RB + kk.  Also lists, per CTA,
-// the K chunks whose slab part holds a non-zero (at least one entry, so that the accumulator is always written).
-template <class Get>   // Get(n,p,q) -> double (full symmetric H)
-inline void pack_mma_slabs(MmaLayout &L, Get get, std::vector<uint16_t> &slabs)
+// Per-CTA operand slabs: [G][KCL][2][NC*32 bytes], chunk x of the CTA's list at x * 2 * NC * 32 (hi, then lo at + NC*32);
+// operand row = nl * RBT + kk.  get(n, k_int, r_int) -> double (full symmetric H in internal order).
+template <class Get>
+inline void pack_mma_slabs(const MmaLayout &L, Get get, std::vector<uint16_t> &slabs)
 {
     slabs.assign((size_t)L.G * L.slab_bytes / 2, 0);
-    L.klist.assign((size_t)L.G * L.KC, 0); L.kcnt.assign(L.G, 0);
+    std::vector<int> kop(L.KP, -1);                               // operand K position -> internal mode
+    for (const MmaBlock &b : L.blocks) for (int x = 0; x < b.nb; ++x) kop[b.koff + x] = b.k0 + x;
     for (int i = 0; i < L.NGRP; ++i)
         for (int j = 0; j < L.NKB; ++j) {
             const int c = i * L.NKB + j;
             uint16_t *base = &slabs[(size_t)c * L.slab_bytes / 2];
-            std::vector<char> used(L.KC, 0);
-            for (int nl = 0; nl < L.NG; ++nl) {
-                const int n = L.nlist[(size_t)i * L.NG + nl];
-                if (n < 0) continue;
-                for (int kk = 0; kk < L.RB; ++kk) {
-                    const int k = j * L.RB + kk;
-                    if (k >= L.n_q) break;
-                    const int row = nl * L.RB + kk;
-                    for (int r = 0; r < L.n_q; ++r) {
-                        const float x = (float)get(n, k, r);
-                        if (x == 0.f) continue;
-                        used[r >> 4] = 1;
-                        const uint16_t hi = bf16_rn(x), lo = bf16_rn(x - bf16_to_float(hi));
-                        const size_t chunk = (size_t)(r >> 4) * 2 * L.NC * 32;
-                        const int off = umma_chunk_off(row, r & 15);
-                        base[(chunk + off) / 2] = hi;
-                        base[(chunk + (size_t)L.NC * 32 + off) / 2] = lo;
+            for (int x = 0; x < L.kcnt[c]; ++x) {
+                const int kc = L.klist[(size_t)c * L.KCL + x];
+                const size_t chunk = (size_t)x * 2 * L.NC * 32;
+                for (int nl = 0; nl < L.NG; ++nl) {
+                    const int n = L.nlist[(size_t)i * L.NG + nl];
+                    if (n < 0) continue;
+                    for (int kk = 0; kk < L.blocks[j].nb; ++kk) {
+                        const int row = nl * L.RBT + kk;
+                        for (int e = 0; e < 16; ++e) {
+                            const int r = kop[kc * 16 + e];
+                            if (r < 0) continue;
+                            const float v = (float)get(n, L.blocks[j].k0 + kk, r);
+                            if (v == 0.f) continue;
+                            const uint16_t hi = bf16_rn(v), lo = bf16_rn(v - bf16_to_float(hi));
+                            const int off = umma_chunk_off(row, e);
+                            base[(chunk + off) / 2] = hi;
+                            base[(chunk + (size_t)L.NC * 32 + off) / 2] = lo;
+                        }
                     }
                 }
             }
-            int cnt = 0;
-            for (int kc = 0; kc < L.KC; ++kc) if (used[kc]) L.klist[(size_t)c * L.KC + cnt++] = kc;
-            if (!cnt) { L.klist[(size_t)c * L.KC] = 0; cnt = 1; }
-            L.kcnt[c] = cnt;
         }
 }
 

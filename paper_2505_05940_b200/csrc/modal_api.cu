@@ -20,7 +20,8 @@
 namespace mh = modal_host;
 namespace md = modal_dev;
 
-static_assert(sizeof(mh::Unit) == sizeof(md::VkUnit), "schedule unit layout");
+static_assert(mh::MMA_RB_MAX == md::MMA_RB_MAX_DEV && mh::MMA_NG_MAX == md::MMA_NG_MAX_DEV && mh::MMA_MT_MAX == md::MMA_MT_MAX &&
+              mh::MMA_FBLK_MAX == 16 && mh::MMA_KCL_MAX == 64, "batched-kernel limits");
 
 namespace {
 
@@ -42,14 +43,6 @@ struct DevBuf {
     template <class T> T *as() const { return reinterpret_cast<T *>(p); }
 };
 
-struct VkConfig {
-    int CS = 1, NCL = 1, NW = 16, grid_team = 0, resident = 0, n_clusters = 1;
-    size_t smem = 0;
-    mh::Schedule sched;
-    DevBuf units, warp_ptr, cta_ptr, nlo;
-    bool uploaded = false;
-};
-
 struct FlowConfig {
     int G = 1, NT = 1, NW = 16, NS = 0, slot_tiles = 8, res_tiles = 0, direct = 0, streamed = 0;
     size_t smem = 0;
@@ -61,9 +54,13 @@ struct FlowConfig {
 struct MmaConfig {
     bool tried = false, ok = false;
     mh::MmaLayout L;
-    size_t smem = 0, slab_c = 0;     // slab_c: bytes of a compacted slab (only the K chunks a CTA multiplies, in list order)
-    int nstg = 0;                    // q-operand ring stages that fit beside it
-    DevBuf dslabs, dn0, dQg, dqf, dGx, dfx, dflags;
+    int lpq = 1;                     // lanes of an owner team that share one quad of the partial-force gather
+    size_t off_nlist = 0, off_klist = 0, off_kcnt = 0, off_fblk = 0, off_fcnt = 0, off_blk = 0;   // ints into dtab
+    DevBuf dslabs, dtab, dQop, dqf, dGx, dfx, dflags, dpx;
+};
+
+struct Options {                     // modal_plan_set_option
+    int vk_impl = 0, flow_g = 0, flow_ns = 0, flow_res = -1, mma_split = 0, mma_ng = 0, mma_nstg = 0, parity_order = 1, timing = 0;
 };
 
 }  // namespace
@@ -77,7 +74,6 @@ struct modal_plan {
     int coeff_batch = 1;
     std::vector<double> omega, sigma, nl_scale, lambda_s, pickup;   // [coeff_batch][...]
     std::vector<int> active;                                          // [coeff_batch][n_q]
-    std::vector<float> Ht;                                            // tile-packed H (VK, team kernel)
     std::vector<float> Hf;                                            // flow-tile-packed H (VK, flow kernel), INTERNAL mode order
     std::vector<uint8_t> tile_nz;                                     // per flow tile: holds a non-zero entry
     long long nz_tiles = 0;
@@ -88,12 +84,15 @@ struct modal_plan {
     std::string err;
     int sm_count = 148;
     // device storage
-    DevBuf dHf, dfx, dgx, dqx, dtiming, dperm;
+    DevBuf dHf, dfx, dgx, dqx, dtiming, dperm, dtimeout;
     MmaConfig mma;
     std::map<long long, FlowConfig> flow_cfgs;
-    DevBuf dHt, dkv, dkq, dr, dast, ds, dw, dlam, dc, dq0, dv0, dgain, dbad, dout, dfbuf, dcounter;
-    std::map<long long, VkConfig> vk_cfgs;
+    DevBuf dkv, dkq, dr, dast, ds, dsT, dw, dlam, dc, dq0, dv0, dgain, dbad, dout;      // dsT: s_n transposed [n_phi][coeff_batch] (batched kernel)
+    float *pinned_out = nullptr; size_t pinned_bytes = 0;            // staging of modal_simulate_host
+    Options opt;
     int kinfo[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    // the last modal_simulate call (modal_plan_check)
+    cudaStream_t last_stream = nullptr; int last_batch = 0; bool last_persistent = false, pending = false;
 };
 
 namespace {
@@ -109,16 +108,13 @@ namespace {
 
 int n_nl(const modal_plan *p) { return p->d.model == MODAL_VK ? p->d.n_phi : 1; }
 
-bool use_team_kernel();
-int env_int(const char *name, int def);
-
 // Internal order of the transverse modes (see modal_plan::perm).
 void build_perm(modal_plan *p)
 {
     const int nq = p->d.n_q;
     p->perm.resize(nq); p->iperm.resize(nq);
     for (int k = 0; k < nq; ++k) p->perm[k] = k;
-    if (p->d.model == MODAL_VK && p->d.geom == MODAL_RECT && !use_team_kernel() && env_int("MODAL_VK_PARITY_ORDER", 1))
+    if (p->d.model == MODAL_VK && p->d.geom == MODAL_RECT && p->opt.parity_order)
         std::stable_sort(p->perm.begin(), p->perm.end(), [&](int a, int b) {
             return ((p->mq.m[a] & 1) * 2 + (p->mq.n[a] & 1)) < ((p->mq.m[b] & 1) * 2 + (p->mq.n[b] & 1));
         });
@@ -132,7 +128,6 @@ void set_H(modal_plan *p, Get get_user)
     const int nq = p->d.n_q, nphi = p->d.n_phi;
     auto get = [&](int n, int a, int b) { return get_user(n, p->perm[a], p->perm[b]); };
     mh::pack_flow_tiles(nq, nphi, get, p->Hf);
-    if (use_team_kernel()) mh::pack_tiles(nq, nphi, get, p->Ht);
     const size_t ntiles = p->Hf.size() / mh::FT_FLOATS;
     p->tile_nz.assign(ntiles, 0);
     p->nz_tiles = 0;
@@ -144,6 +139,7 @@ void set_H(modal_plan *p, Get get_user)
     }
     for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
     p->flow_cfgs.clear();                                   // schedules depend on the zero pattern
+    p->mma.tried = false; p->mma.ok = false;
     p->H_dirty = true;
 }
 
@@ -245,6 +241,13 @@ modal_status sync_coeffs(modal_plan *p)
             const bool act = mh::mode_active(d.scheme, om, sg, p->T) && std::isfinite(om) && std::isfinite(sg);
             p->active[(size_t)b * nq + k] = act;
             if (!act) { ++masked; continue; }
+            if (d.scheme == MODAL_FTM && !(om > sg)) {        // the FTM coefficients need an underdamped mode
+                char buf[200];
+                snprintf(buf, sizeof buf, "FTM scheme: mode %d of coefficient row %d is critically damped or overdamped "
+                         "(omega = %.6g <= sigma = %.6g)\n", k, b, om, sg);
+                p->err += buf;
+                return MODAL_EINVAL;
+            }
             const mh::StepCoeffs c = mh::step_coeffs(d.scheme, om, sg, p->T);
             const size_t o = (size_t)b * P + p->iperm[k];
             kv[o] = c.kv; kq[o] = c.kq; r[o] = c.r; ast[o] = c.astart;
@@ -267,39 +270,21 @@ modal_status sync_coeffs(modal_plan *p)
     CU(up(p->dkv, kv.data(), kv.size() * 8)); CU(up(p->dkq, kq.data(), kq.size() * 8));
     CU(up(p->dr, r.data(), r.size() * 8));    CU(up(p->dast, ast.data(), ast.size() * 8));
     CU(up(p->dw, w.data(), w.size() * 4));
-    if (d.model == MODAL_VK) CU(up(p->ds, s.data(), s.size() * 4));
+    if (d.model == MODAL_VK) {
+        CU(up(p->ds, s.data(), s.size() * 4));
+        std::vector<float> sT(s.size());                          // [n_phi][cb]: consecutive samples read consecutive words
+        for (int b = 0; b < cb; ++b) for (int n = 0; n < nnl; ++n) sT[(size_t)n * cb + b] = s[(size_t)b * nnl + n];
+        CU(up(p->dsT, sT.data(), sT.size() * 4));
+    }
     else { CU(up(p->dlam, lam.data(), lam.size() * 4)); CU(up(p->dc, s.data(), s.size() * 4)); }
     p->coeffs_dirty = false;
     return MODAL_OK;
-}
-
-int env_int(const char *name, int def)
-{
-    const char *s = getenv(name);
-    return (s && *s) ? atoi(s) : def;
-}
-bool use_team_kernel()
-{
-    const char *s = getenv("MODAL_VK_IMPL");
-    return s && !strcmp(s, "team");
-}
-// 1 = forced on, 0 = forced off, -1 = automatic (batch >= 64 and the layout fits)
-int mma_kernel_mode()
-{
-    const char *s = getenv("MODAL_VK_IMPL");
-    if (s && !strcmp(s, "mma")) return 1;
-    if (s && (!strcmp(s, "flow") || !strcmp(s, "team"))) return 0;
-    return -1;
 }
 
 modal_status sync_H(modal_plan *p)
 {
     if (p->device >= 0 && p->d.model == MODAL_VK) {
         CU(cudaSetDevice(p->device));
-        if (use_team_kernel()) {
-            CU(p->dHt.ensure(p->Ht.size() * 4));
-            CU(cudaMemcpy(p->dHt.p, p->Ht.data(), p->Ht.size() * 4, cudaMemcpyHostToDevice));
-        }
         CU(p->dHf.ensure(p->Hf.size() * 4));
         CU(cudaMemcpy(p->dHf.p, p->Hf.data(), p->Hf.size() * 4, cudaMemcpyHostToDevice));
         CU(p->dperm.ensure(p->perm.size() * 4));
@@ -309,138 +294,6 @@ modal_status sync_H(modal_plan *p)
     p->H_dirty = false;
     return MODAL_OK;
 }
-
-template <bool R>
-cudaError_t launch_vk(const md::VkArgs &a, int n_clusters, int CS, int threads, size_t smem, cudaStream_t st)
-{
-    auto kern = md::vk_team_kernel<R>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    if (CS > 8) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        if (e != cudaSuccess) return e;
-    }
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(n_clusters * CS); cfg.blockDim = dim3(threads);
-    cfg.dynamicSmemBytes = smem; cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, a);
-}
-
-template <bool R>
-int max_active_clusters(int CS, int threads, size_t smem)
-{
-    auto kern = md::vk_team_kernel<R>;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
-    if (CS > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return 0;
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(CS); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    int n = 0;
-    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
-    return n;
-}
-
-size_t vk_smem_bytes(const mh::Schedule &s, int NQP, int grid_team, int resident)
-{
-    size_t f = md::vk_smem_floats(NQP, s.NLOC_MAX, s.CS, grid_team, s.max_cta_units, s.max_tp);
-    size_t bytes = f * 4;
-    if (resident) bytes += (size_t)s.max_cta_tiles * md::TILE_ELEMS * 4;
-    return bytes + 16;
-}
-
-// Choose team shape and residency for this batch.
-modal_status configure_vk(modal_plan *p, int batch, VkConfig **out)
-{
-    const int nq = p->d.n_q, nphi = p->d.n_phi, P = p->NQP;
-    const int NW = env_int("MODAL_VK_NW", 16);
-    if (P > NW * 32) { p->err += "n_q too large for the vK kernel of this build (padded n_q <= 512)\n"; return MODAL_EINCOMPAT; }
-    const int force_cs = env_int("MODAL_VK_CS", 0);
-    const char *mode = getenv("MODAL_VK_MODE");   // "resident" | "cluster" | "grid"
-    const int tiles_total = nphi * mh::tiles_per_n(nq);
-    int CS = 0, grid_team = 0, resident = 0, NCL = 1;
-    mh::Schedule sch;
-    // 1. resident in one cluster's shared memory?
-    if (!mode || !strcmp(mode, "resident")) {
-        for (int cs : {1, 2, 4, 8, 16}) {
-            if (force_cs && cs != force_cs) continue;
-            mh::Schedule s = mh::build_schedule(nq, nphi, cs, 1, NW);
-            if (vk_smem_bytes(s, P, 0, 1) > SMEM_LIMIT) continue;
-            if (max_active_clusters<true>(cs, NW * 32, vk_smem_bytes(s, P, 0, 1)) < 1) continue;
-            // widen small-batch runs while every warp still has >= 2 tiles of work
-            const bool widen = !force_cs && cs < 16 && (long long)batch * cs * 2 <= p->sm_count &&
-                               tiles_total / (cs * 2 * NW) >= 2;
-            CS = cs; resident = 1; sch = s;
-            if (!widen) break;
-        }
-    }
-    if (!CS) {
-        const bool want_grid = mode ? !strcmp(mode, "grid") : batch <= 4;
-        grid_team = want_grid;
-        if (!grid_team) {
-            CS = force_cs ? force_cs : 8;
-            sch = mh::build_schedule(nq, nphi, CS, 1, NW);
-        } else {
-            // a cluster needs its CTAs in one GPC, so the co-resident capacity depends on the
-            // cluster size: take the shape that keeps the most SMs busy (ties -> larger cluster)
-            int best_ctas = 0;
-            for (int cs : {8, 4, 2, 1}) {
-                if (force_cs && cs != force_cs) continue;
-                int ncl = std::min(p->sm_count / cs, nphi);
-                for (int it = 0; it < 2 && ncl > 0; ++it) {
-                    mh::Schedule s = mh::build_schedule(nq, nphi, cs, ncl, NW);
-                    const size_t sm = vk_smem_bytes(s, P, 1, 0);
-                    const int cap = sm <= SMEM_LIMIT ? max_active_clusters<false>(cs, NW * 32, sm) : 0;
-                    if (cap >= ncl) {
-                        if (ncl * cs > best_ctas) { best_ctas = ncl * cs; CS = cs; NCL = ncl; sch = s; }
-                        break;
-                    }
-                    ncl = cap;
-                }
-            }
-            if (!CS) { p->err += "no co-resident grid team shape for the vK kernel\n"; return MODAL_EINCOMPAT; }
-        }
-    }
-    const long long key = ((long long)CS << 40) | ((long long)NCL << 20) | (grid_team << 1) | resident;
-    VkConfig &c = p->vk_cfgs[key];
-    if (!c.uploaded) {
-        c.CS = CS; c.NCL = NCL; c.NW = NW; c.grid_team = grid_team; c.resident = resident;
-        c.sched = sch;
-        c.smem = vk_smem_bytes(sch, P, grid_team, resident);
-        if (c.smem > SMEM_LIMIT) { p->err += "vK schedule does not fit shared memory\n"; return MODAL_EINCOMPAT; }
-        auto up = [&](DevBuf &b, const void *src, size_t bytes) -> cudaError_t {
-            cudaError_t e = b.ensure(bytes);
-            return e != cudaSuccess ? e : cudaMemcpy(b.p, src, bytes, cudaMemcpyHostToDevice);
-        };
-        CU(up(c.units, sch.units.data(), sch.units.size() * sizeof(mh::Unit)));
-        CU(up(c.warp_ptr, sch.warp_ptr.data(), sch.warp_ptr.size() * 4));
-        CU(up(c.cta_ptr, sch.cta_ptr.data(), sch.cta_ptr.size() * 4));
-        CU(up(c.nlo, sch.nlo.data(), sch.nlo.size() * 4));
-        c.uploaded = true;
-    }
-    if (grid_team) {
-        const int cap = resident ? max_active_clusters<true>(CS, NW * 32, c.smem)
-                                 : max_active_clusters<false>(CS, NW * 32, c.smem);
-        if (cap < NCL) {
-            char buf[128];
-            snprintf(buf, sizeof buf, "grid team of %d clusters of %d is not co-resident (capacity %d)\n", NCL, CS, cap);
-            p->err += buf;
-            return MODAL_EINCOMPAT;
-        }
-        c.n_clusters = NCL;
-    } else {
-        c.n_clusters = batch;
-    }
-    *out = &c;
-    return MODAL_OK;
-}
-
 
 // ---- vk_flow launch selection ------------------------------
 int flow_capacity(size_t smem, bool ring)
@@ -458,7 +311,7 @@ bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, const std:
     c.G = G; c.NW = 16; c.slot_tiles = 8;
     c.sched = mh::build_flow_schedule(nq, nphi, G, c.NW, c.slot_tiles, tile_nz);
     const mh::FlowSchedule &s = c.sched;
-    if (s.NLOC_MAX > 255 || s.tp_max >= (1 << 24)) return false;
+    if (s.NLOC_MAX > 255 || s.tp_max >= (1 << 24) || s.nt > 255) return false;      // 8-bit fields of the unit descriptors
     const md::FlowSmem fixed = md::flow_smem_layout(0, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, 0);
     if (fixed.total + 1024 > SMEM_LIMIT) return false;
     const int avail_tiles = (int)((SMEM_LIMIT - fixed.total - 256) / 1024);
@@ -501,7 +354,7 @@ double flow_step_cost(double tiles, int nphi, int G, int NT)
 modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
 {
     const int nq = p->d.n_q, nphi = p->d.n_phi;
-    const int force_g = env_int("MODAL_FLOW_G", 0), force_ns = env_int("MODAL_FLOW_NS", 0), force_res = env_int("MODAL_FLOW_RES", -1);
+    const int force_g = p->opt.flow_g, force_ns = p->opt.flow_ns, force_res = p->opt.flow_res;
     const long long key0 = ((long long)force_g << 40) | ((long long)(force_ns & 0xff) << 32) | ((long long)(force_res + 1) << 8);
     // pick the team size: minimise (rounds of samples) x (step cost) over the feasible sizes
     int bestG = 0; double best = 0;
@@ -553,65 +406,69 @@ modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
 }
 
 // ---- vk_mma (batched tensor-core kernel) -------------------------------------------------------
-modal_status configure_mma(modal_plan *p)
+// Layout (mma_schedule.hpp), operand slabs and per-layout tables; the exchange buffers are sized per launch.
+// Host part: the layout and the getters of the fp32 H values the device holds (flow tiles, internal order).
+bool mma_host_layout(const modal_plan *p, mh::MmaLayout &L)
 {
-    MmaConfig &m = p->mma;
-    if (m.tried) return MODAL_OK;
-    m.tried = true; m.ok = false;
     const int nq = p->d.n_q, nphi = p->d.n_phi;
-    // in-plane modes of one CTA share the index parity (then the slab is zero in most K chunks, which are skipped)
+    if (p->d.model != MODAL_VK) return false;
+    // classes of the internal mode order (contiguous ranges) and of the in-plane modes: the index parities of the
+    // sine-basis plate, else one class.  The K chunks a CTA multiplies come from the actual non-zeros of H.
+    const bool classes = p->d.geom == MODAL_RECT && p->opt.parity_order;
+    auto cls_q = [&](int k_int) { const int k = p->perm[k_int]; return classes ? (p->mq.m[k] & 1) * 2 + (p->mq.n[k] & 1) : 0; };
+    std::vector<int> class_start{0};
+    for (int k = 1; k < nq; ++k) if (cls_q(k) != cls_q(k - 1)) class_start.push_back(k);
+    class_start.push_back(nq);
     std::vector<int> mode_class(nphi, 0);
-    if (p->d.geom == MODAL_RECT && env_int("MODAL_VK_PARITY_ORDER", 1))
-        for (int n = 0; n < nphi; ++n) mode_class[n] = (p->mphi.m[n] & 1) * 2 + (p->mphi.n[n] & 1);
-    if (!mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, md::mma_smem_fixed(), env_int("MODAL_MMA_NKB", 0),
-                        env_int("MODAL_MMA_RBALIGN", 16) == 4 ? 4 : 16, &mode_class, m.L)) return MODAL_OK;
-    if (md::mma_smem_layout((int)m.L.slab_bytes, m.L.nel_max, md::MMA_NSTG).total > SMEM_LIMIT) return MODAL_OK;
-    m.smem = SMEM_LIMIT;             // upper bound for the occupancy check; the launch size is set after the slabs are packed
-    if (cudaFuncSetAttribute(md::vk_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
-    int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, md::vk_mma_kernel, md::MMA_THREADS, m.smem) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
-    if (per_sm * p->sm_count < m.L.G) return MODAL_OK;
-    // operand slabs from the fp32 values the device holds (flow tiles)
+    if (classes) for (int n = 0; n < nphi; ++n) mode_class[n] = (p->mphi.m[n] & 1) * 2 + (p->mphi.n[n] & 1);
     const std::vector<float> &Hf = p->Hf;
     const int tpn = mh::flow_tiles_per_n(nq);
+    auto nz = [&](int n, int a, int b) -> bool {
+        const int hi = std::max(a, b), lo = std::min(a, b), I = hi / 16, J = lo / 16;
+        const size_t tile = (size_t)n * tpn + I * (I + 1) / 2 + J;
+        return p->tile_nz[tile] && Hf[tile * 256 + mh::flow_elem(hi % 16, lo % 16)] != 0.f;
+    };
+    return mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, md::mma_smem_fixed(), class_start, mode_class, nz,
+                          p->opt.mma_split, p->opt.mma_ng, L);
+}
+
+void mma_host_slabs(const modal_plan *p, const mh::MmaLayout &L, std::vector<uint16_t> &slabs)
+{
+    const std::vector<float> &Hf = p->Hf;
+    const int tpn = mh::flow_tiles_per_n(p->d.n_q);
     auto get = [&](int n, int a, int b) -> double {
         const int hi = std::max(a, b), lo = std::min(a, b), I = hi / 16, J = lo / 16;
         const float t = Hf[((size_t)n * tpn + I * (I + 1) / 2 + J) * 256 + mh::flow_elem(hi % 16, lo % 16)];
         return hi == lo ? 2.0 * (double)t : (double)t;
     };
-    std::vector<uint16_t> slabs;
-    mh::pack_mma_slabs(m.L, get, slabs);
+    mh::pack_mma_slabs(L, get, slabs);
+}
+
+modal_status configure_mma(modal_plan *p)
+{
+    MmaConfig &m = p->mma;
+    if (m.tried) return MODAL_OK;
+    m.tried = true; m.ok = false;
+    if (!mma_host_layout(p, m.L)) return MODAL_OK;
     const mh::MmaLayout &L = m.L;
-    {   // compact: a CTA keeps only the K chunks it multiplies, in list order; the shared memory this frees goes to the ring
-        const size_t chunk = (size_t)2 * L.NC * 32;
-        const int kcm = *std::max_element(L.kcnt.begin(), L.kcnt.end());
-        m.slab_c = (size_t)kcm * chunk;
-        std::vector<uint16_t> cs((size_t)L.G * m.slab_c / 2, 0);
-        for (int c = 0; c < L.G; ++c)
-            for (int x = 0; x < L.kcnt[c]; ++x)
-                std::memcpy(&cs[((size_t)c * m.slab_c + (size_t)x * chunk) / 2],
-                            &slabs[((size_t)c * L.slab_bytes + (size_t)L.klist[(size_t)c * L.KC + x] * chunk) / 2], chunk);
-        slabs.swap(cs);
-        const size_t base = md::mma_smem_layout((int)m.slab_c, L.nel_max, 0).total;
-        // measured on C3 (profiles/r1_c3_b256.md): 6 / 8 / 12 stages give 17.91 / 17.86 / 18.25 us per step -- the q stream is
-        // bound by L2 bandwidth (every CTA reads the same chunks), not by the bytes in flight, so the ring stays at 8
-        const int want = std::max(2, std::min(env_int("MODAL_MMA_NSTG", 8), md::MMA_NSTG_MAX));
-        const int nstg = (int)std::min<size_t>(want, (SMEM_LIMIT - base) / 8192) & ~1;
-        m.nstg = nstg;
-        m.smem = md::mma_smem_layout((int)m.slab_c, L.nel_max, nstg).total;
-    }
+    if (cudaFuncSetAttribute(md::vk_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, md::vk_mma_kernel<false>, md::MMA_THREADS, SMEM_LIMIT) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
+    if (per_sm * p->sm_count < L.G) return MODAL_OK;
+    std::vector<uint16_t> slabs;
+    mma_host_slabs(p, L, slabs);
     CU(m.dslabs.ensure(slabs.size() * 2));
     CU(cudaMemcpy(m.dslabs.p, slabs.data(), slabs.size() * 2, cudaMemcpyHostToDevice));
-    std::vector<int> tab(L.nlist);                                  // nlist | klist | kcnt in one buffer
-    tab.insert(tab.end(), L.klist.begin(), L.klist.end());
-    tab.insert(tab.end(), L.kcnt.begin(), L.kcnt.end());
-    CU(m.dn0.ensure(tab.size() * 4));
-    CU(cudaMemcpy(m.dn0.p, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice));
-    CU(m.dQg.ensure((size_t)2 * L.KC * 8192));
-    CU(m.dqf.ensure((size_t)256 * L.QS * 4));
-    CU(m.dGx.ensure((size_t)L.G * 2 * 128 * 4 * L.NG4 * 4));
-    CU(m.dfx.ensure((size_t)L.NGRP * 2 * 128 * L.QS * 4));
-    CU(m.dflags.ensure((size_t)L.G * 2 * 4 * md::MMA_FS));
+    std::vector<int> tab;
+    auto add = [&](const std::vector<int> &v) { const size_t o = tab.size(); tab.insert(tab.end(), v.begin(), v.end()); return o; };
+    m.off_nlist = add(L.nlist); m.off_klist = add(L.klist); m.off_kcnt = add(L.kcnt); m.off_fblk = add(L.fblk); m.off_fcnt = add(L.fcnt);
+    std::vector<int> blk;
+    for (const mh::MmaBlock &b : L.blocks) { blk.push_back(b.k0); blk.push_back(b.nb); blk.push_back(b.koff); }
+    m.off_blk = add(blk);
+    CU(m.dtab.ensure(tab.size() * 4));
+    CU(cudaMemcpy(m.dtab.p, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice));
+    // owner gather: lanes per quad so that no lane has more than 16 strong loads in flight
+    m.lpq = L.NGRP <= 16 ? 1 : L.NGRP <= 32 ? 2 : 4;
     m.ok = true;
     return MODAL_OK;
 }
@@ -623,6 +480,33 @@ cudaError_t launch_tension(const md::TensionArgs &a, cudaStream_t st)
     const int blocks = (a.batch + warps_per_block - 1) / warps_per_block;
     md::tension_kernel<MPL><<<blocks, warps_per_block * 32, 0, st>>>(a);
     return cudaGetLastError();
+}
+
+// Completes the last launch: stream synchronisation, timeout flag of the persistent kernels, first-bad steps.
+modal_status finish(modal_plan *p, int *first_bad)
+{
+    if (!p->pending) return MODAL_OK;
+    const int batch = p->last_batch;
+    std::vector<int> bad(batch, -1);
+    int flag = 0;
+    CU(cudaSetDevice(p->device));
+    CU(cudaMemcpyAsync(bad.data(), p->dbad.p, (size_t)batch * 4, cudaMemcpyDeviceToHost, p->last_stream));
+    if (p->last_persistent) CU(cudaMemcpyAsync(&flag, p->dtimeout.p, 4, cudaMemcpyDeviceToHost, p->last_stream));
+    CU(cudaStreamSynchronize(p->last_stream));
+    p->pending = false;
+    if (first_bad) memcpy(first_bad, bad.data(), (size_t)batch * 4);
+    if (flag) {
+        p->err += "a cross-CTA exchange of the persistent vK kernel timed out (team not co-resident?)\n";
+        return MODAL_ECUDA;
+    }
+    for (int b = 0; b < batch; ++b)
+        if (bad[b] >= 0) {
+            char buf[96];
+            snprintf(buf, sizeof buf, "sample %d went non-finite at step %d\n", b, bad[b]);
+            p->err += buf;
+            return MODAL_EUNSTABLE;
+        }
+    return MODAL_OK;
 }
 
 modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, float *out_dev,
@@ -654,7 +538,9 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         CU(cudaMemcpyAsync(p->dgain.p, gain.data(), gain.size() * 8, cudaMemcpyHostToDevice, st));
     }
     CU(cudaMemsetAsync(p->dbad.p, 0xff, (size_t)batch * 4, st));
-    bool flow_launched = false;
+    CU(p->dtimeout.ensure(4));
+    CU(cudaMemsetAsync(p->dtimeout.p, 0, 4, st));
+    bool persistent = false;
     const int auto_start = init->qm1 ? 0 : 1;
     const double half_T2 = 0.5 * p->T * p->T;
 
@@ -677,30 +563,47 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             case 6: e = launch_tension<6>(a, st); break;
             case 7: e = launch_tension<7>(a, st); break;
             case 8: e = launch_tension<8>(a, st); break;
+            case 9: e = launch_tension<9>(a, st); break;
+            case 10: e = launch_tension<10>(a, st); break;
+            case 11: e = launch_tension<11>(a, st); break;
             case 12: e = launch_tension<12>(a, st); break;
+            case 13: e = launch_tension<13>(a, st); break;
+            case 14: e = launch_tension<14>(a, st); break;
+            case 15: e = launch_tension<15>(a, st); break;
             case 16: e = launch_tension<16>(a, st); break;
-            default: p->err += "n_q not supported by the tension kernel (n_q <= 256, 353..384 or 481..512)\n"; return MODAL_EINCOMPAT;
+            default: p->err += "n_q too large for the tension kernel of this build (n_q <= 512)\n"; return MODAL_EINCOMPAT;
         }
         CU(e);
         p->kinfo[0] = 1; p->kinfo[1] = 1; p->kinfo[2] = (batch + 3) / 4; p->kinfo[3] = 128;
         p->kinfo[4] = 0; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
-    } else if (!use_team_kernel() && mma_kernel_mode() != 0 && (mma_kernel_mode() == 1 || batch >= 64) &&
-               configure_mma(p) == MODAL_OK && p->mma.ok) {
+    } else if (p->opt.vk_impl != 1 && (p->opt.vk_impl == 2 || batch >= 64) && configure_mma(p) == MODAL_OK && p->mma.ok) {
         MmaConfig &m = p->mma;
         const mh::MmaLayout &L = m.L;
-        CU(cudaFuncSetAttribute(md::vk_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m.smem));
-        for (int b0 = 0; b0 < batch; b0 += 256) {       // up to two M tiles of 128 samples per launch
-            const int nb = std::min(256, batch - b0);
+        const int chunk = 128 * md::MMA_MT_MAX;                 // samples per launch: up to 8 M tiles time-multiplexed in one kernel
+        size_t smem = 0;
+        for (int b0 = 0; b0 < batch; b0 += chunk) {
+            const int nb = std::min(chunk, batch - b0), MT = (nb + 127) / 128;
+            // shared memory: slab + owner state and coefficients of MT tiles + as many ring stages as fit (<= 16)
+            const size_t base = md::mma_smem_layout((int)L.slab_bytes, MT, L.rows_max, L.RBQ, 0).total;
+            int nstg = base < SMEM_LIMIT ? (int)std::min<size_t>(md::MMA_NSTG_MAX, (SMEM_LIMIT - base) / 8192) : 0;
+            if (p->opt.mma_nstg > 0) nstg = std::min(nstg, p->opt.mma_nstg);
+            if (nstg < 2) { p->err += "batched vK kernel: no room for the operand ring\n"; return MODAL_EINCOMPAT; }
+            smem = md::mma_smem_layout((int)L.slab_bytes, MT, L.rows_max, L.RBQ, nstg).total;
+            CU(cudaFuncSetAttribute(md::vk_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            CU(cudaFuncSetAttribute(md::vk_mma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             md::MmaArgs a{};
-            a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)m.slab_c; a.NSTG = m.nstg;
-            a.NKB = L.NKB; a.RB = L.RB; a.NGRP = L.NGRP; a.NG = L.NG; a.NG4 = L.NG4; a.NC = L.NC; a.KC = L.KC; a.KP = L.KP; a.QS = L.QS;
-            a.G = L.G; a.nel_max = L.nel_max;
-            a.nlist = m.dn0.as<int>(); a.klist = a.nlist + L.nlist.size(); a.kcnt = a.klist + L.klist.size(); a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P;
-            a.batch = nb; a.n_steps = n_steps; a.MT = (nb + 127) / 128;
+            a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)L.slab_bytes; a.NSTG = nstg;
+            a.NKB = L.NKB; a.NGRP = L.NGRP; a.NG = L.NG; a.NG4 = L.NG4; a.NC = L.NC; a.S = L.S; a.RBT = L.RBT; a.RBQ = L.RBQ;
+            a.KC = L.KC; a.KCL = L.KCL; a.G = L.G; a.rows_max = L.rows_max; a.LPQ = m.lpq;
+            const int *tab = m.dtab.as<int>();
+            a.nlist = tab + m.off_nlist; a.klist = tab + m.off_klist; a.kcnt = tab + m.off_kcnt; a.fblk = tab + m.off_fblk;
+            a.fcnt = tab + m.off_fcnt; a.blk = tab + m.off_blk;
+            a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P;
+            a.batch = nb; a.n_steps = n_steps; a.MT = MT;
             a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
-            const size_t oq = cb == 1 ? 0 : (size_t)b0 * P, on = cb == 1 ? 0 : (size_t)b0 * d.n_phi;
+            const size_t oq = cb == 1 ? 0 : (size_t)b0 * P;
             a.kv = p->dkv.as<double>() + oq; a.kq = p->dkq.as<double>() + oq; a.r = p->dr.as<double>() + oq;
-            a.astart = p->dast.as<double>() + oq; a.s = p->ds.as<float>() + on; a.w = p->dw.as<float>() + oq;
+            a.astart = p->dast.as<double>() + oq; a.sT = p->dsT.as<float>() + (cb == 1 ? 0 : b0); a.sT_stride = cb; a.w = p->dw.as<float>() + oq;
             a.q0 = p->dq0.as<double>() + (size_t)b0 * P; a.v0 = p->dv0.as<double>() + (size_t)b0 * P;
             a.auto_start = auto_start; a.half_T2 = half_T2;
             a.fext = init->fext_signal ? init->fext_signal + (size_t)b0 * n_steps : nullptr;
@@ -708,39 +611,44 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             a.out = out_dev + (size_t)b0 * n_steps;
             a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr; a.kperm = p->dperm.as<int>();
             a.first_bad = p->dbad.as<int>() + b0;
-            a.Qg = m.dQg.as<uint16_t>(); a.qf = m.dqf.as<float>(); a.Gx = m.dGx.as<uint32_t>(); a.fx = m.dfx.as<uint32_t>();
-            a.qflag = m.dflags.as<unsigned>();
-            // exchange buffers start at tag / epoch 0 (the first step uses 1)
-            CU(cudaMemsetAsync(m.dQg.p, 0, (size_t)2 * L.KC * 8192, st));
-            CU(cudaMemsetAsync(m.dqf.p, 0, (size_t)256 * L.QS * 4, st));
-            CU(cudaMemsetAsync(m.dGx.p, 0, (size_t)L.G * 2 * 128 * 4 * L.NG4 * 4, st));
-            CU(cudaMemsetAsync(m.dfx.p, 0, (size_t)L.NGRP * 2 * 128 * L.QS * 4, st));
-            CU(cudaMemsetAsync(m.dflags.p, 0, (size_t)L.G * 2 * 4 * md::MMA_FS, st));
-            const bool timing = env_int("MODAL_FLOW_TIMING", 0) != 0;
+            // exchange buffers (L2 resident); everything starts at tag / epoch 0 (the first step uses 1)
+            const size_t nQop = (size_t)MT * L.KC * 8192, nqf = (size_t)MT * L.NKB * L.RBQ * 128 * 16,
+                         nGx = (size_t)2 * MT * L.NGRP * L.NKB * 128 * 16 * L.NG4, nfx = (size_t)MT * L.NGRP * L.NKB * L.RBQ * 128 * 16,
+                         nfl = (size_t)MT * L.NKB * L.NGRP * md::MMA_FS * 4, npx = (size_t)2 * MT * L.NKB * 128 * 16;
+            CU(m.dQop.ensure(nQop)); CU(m.dqf.ensure(nqf)); CU(m.dGx.ensure(nGx)); CU(m.dfx.ensure(nfx)); CU(m.dflags.ensure(nfl)); CU(m.dpx.ensure(npx));
+            CU(cudaMemsetAsync(m.dQop.p, 0, nQop, st)); CU(cudaMemsetAsync(m.dqf.p, 0, nqf, st)); CU(cudaMemsetAsync(m.dGx.p, 0, nGx, st));
+            CU(cudaMemsetAsync(m.dfx.p, 0, nfx, st)); CU(cudaMemsetAsync(m.dflags.p, 0, nfl, st)); CU(cudaMemsetAsync(m.dpx.p, 0, npx, st));
+            a.Qop = m.dQop.as<uint16_t>(); a.qf = m.dqf.as<float>(); a.Gx = m.dGx.as<uint32_t>(); a.fx = m.dfx.as<uint32_t>();
+            a.qflag = m.dflags.as<unsigned>(); a.px = m.dpx.as<unsigned long long>();
+            a.timeout_flag = p->dtimeout.as<int>();
+            const bool timing = p->opt.timing != 0;
             if (timing) {
-                CU(p->dtiming.ensure((size_t)L.G * 64));
-                CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)L.G * 64, st));
+                CU(p->dtiming.ensure((size_t)L.G * 128));
+                CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)L.G * 128, st));
                 a.timing = p->dtiming.as<long long>();
             }
-            flow_launched = true;
-            md::vk_mma_kernel<<<L.G, md::MMA_THREADS, m.smem, st>>>(a);
+            persistent = true;
+            if (timing) md::vk_mma_kernel<true><<<L.G, md::MMA_THREADS, smem, st>>>(a);
+            else md::vk_mma_kernel<false><<<L.G, md::MMA_THREADS, smem, st>>>(a);
             CU(cudaGetLastError());
             if (timing) {
                 CU(cudaStreamSynchronize(st));
-                std::vector<long long> tm((size_t)L.G * 8);
+                std::vector<long long> tm((size_t)L.G * 16);
                 CU(cudaMemcpy(tm.data(), p->dtiming.p, tm.size() * 8, cudaMemcpyDeviceToHost));
-                double acc[8] = {0};
-                for (size_t x = 0; x < tm.size(); ++x) acc[x & 7] += (double)tm[x];
+                double acc[16] = {0};
+                for (size_t x = 0; x < tm.size(); ++x) acc[x & 15] += (double)tm[x];
                 const double den = (double)L.G * n_steps;
-                fprintf(stderr, "[modal mma timing] G=%d NGRPxNKB=%dx%d RB=%d NG=%d NC=%d cycles/step (tile 0): wait q %.0f | wait mma %.0f | epi1 %.0f | G hop %.0f | "
-                        "epi2 %.0f | f hop+update %.0f | bar+flag %.0f | K chunks used %.1f of %d\n", L.G, L.NGRP, L.NKB, L.RB, L.NG, L.NC, acc[0] / den, acc[1] / den, acc[2] / den,
-                        acc[3] / den, acc[4] / den, acc[5] / den, acc[6] / den,
-                        (double)std::accumulate(L.kcnt.begin(), L.kcnt.end(), 0) / L.G, L.KC);
+                fprintf(stderr, "[modal mma timing] G=%d (%d groups x %d blocks) NG=%d NC=%d S=%d KCL=%d ring=%d MT=%d  cycles/step of tile 0, mean over CTAs:\n"
+                        "   E: wait q %.0f | wait acc %.0f | epi1+send %.0f (first unit in registers after %.0f, all units after %.0f) | G hop %.0f | epi2 %.0f\n"
+                        "   O: gather %.0f | update %.0f | publish %.0f | barrier+fence+flag %.0f     P: flag poll %.0f   M: first chunk -> commit %.0f\n"
+                        "   hops: end of epilogue 2 -> forces gathered %.0f | own flag set -> all source flags seen %.0f\n",
+                        L.G, L.NGRP, L.NKB, L.NG, L.NC, L.S, L.KCL, nstg, MT, acc[0] / den, acc[1] / den, acc[2] / den, acc[5] / den, acc[6] / den, acc[3] / den, acc[4] / den,
+                        acc[8] / den, acc[11] / den, acc[9] / den, acc[10] / den, acc[12] / den, acc[13] / den, acc[14] / den, acc[15] / den);
             }
         }
         p->kinfo[0] = 4; p->kinfo[1] = L.G; p->kinfo[2] = L.NGRP; p->kinfo[3] = md::MMA_THREADS;
-        p->kinfo[4] = (int)m.smem; p->kinfo[5] = 1; p->kinfo[6] = L.NC; p->kinfo[7] = P;
-    } else if (!use_team_kernel()) {
+        p->kinfo[4] = (int)smem; p->kinfo[5] = 1 | 2; p->kinfo[6] = L.S; p->kinfo[7] = P;
+    } else {
         FlowConfig *c = nullptr;
         modal_status s = configure_flow(p, batch, &c);
         if (s != MODAL_OK) return s;
@@ -768,13 +676,14 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             CU(cudaMemsetAsync(p->dfx.p, 0, nfx, st)); CU(cudaMemsetAsync(p->dgx.p, 0, ngx, st)); CU(cudaMemsetAsync(p->dqx.p, 0, nqx, st));
             a.fx = p->dfx.as<unsigned long long>(); a.gx = p->dgx.as<unsigned long long>(); a.qx = p->dqx.as<unsigned long long>();
         }
-        const bool timing = env_int("MODAL_FLOW_TIMING", 0) != 0;
+        a.timeout_flag = p->dtimeout.as<int>();
+        const bool timing = p->opt.timing != 0;
         if (timing) {
             CU(p->dtiming.ensure((size_t)c->G * c->NT * 64));
             CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)c->G * c->NT * 64, st));
             a.timing = p->dtiming.as<long long>();
         }
-        flow_launched = true;
+        persistent = true;
         if (c->NS > 0) {
             CU(cudaFuncSetAttribute(md::vk_flow_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
             md::vk_flow_kernel<true><<<c->G * c->NT, (c->NW + 1) * 32, c->smem, st>>>(a);
@@ -795,59 +704,9 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         }
         p->kinfo[0] = 3; p->kinfo[1] = c->G; p->kinfo[2] = c->NT; p->kinfo[3] = (c->NW + (c->NS > 0 ? 1 : 0)) * 32;
         p->kinfo[4] = (int)c->smem; p->kinfo[5] = (c->streamed == 0 ? 1 : 0) | (c->G > 1 ? 2 : 0); p->kinfo[6] = c->NS; p->kinfo[7] = P;
-    } else {
-        VkConfig *c = nullptr;
-        modal_status s = configure_vk(p, batch, &c);
-        if (s != MODAL_OK) return s;
-        md::VkArgs a{};
-        a.Ht = p->dHt.as<float>(); a.units = c->units.as<md::VkUnit>();
-        a.warp_ptr = c->warp_ptr.as<int2>(); a.cta_ptr = c->cta_ptr.as<int2>(); a.nlo = c->nlo.as<int>();
-        a.NQP = P; a.n_q = nq; a.n_phi = d.n_phi; a.tiles_per_n = mh::tiles_per_n(nq);
-        a.NLOC_MAX = c->sched.NLOC_MAX; a.CS = c->CS; a.NCL = c->NCL; a.grid_team = c->grid_team; a.resident = c->resident;
-        a.max_cta_units = c->sched.max_cta_units; a.max_tp = c->sched.max_tp; a.max_cta_tiles = c->sched.max_cta_tiles;
-        a.batch = batch; a.n_steps = n_steps;
-        a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
-        a.kv = p->dkv.as<double>(); a.kq = p->dkq.as<double>(); a.r = p->dr.as<double>(); a.astart = p->dast.as<double>();
-        a.s = p->ds.as<float>(); a.w = p->dw.as<float>();
-        a.q0 = p->dq0.as<double>(); a.v0 = p->dv0.as<double>();
-        a.auto_start = auto_start; a.half_T2 = half_T2;
-        a.fext = init->fext_signal; a.gain = p->dgain.as<double>();
-        a.out = out_dev; a.traj = init->traj_dev; a.first_bad = p->dbad.as<int>();
-        if (c->grid_team) {
-            CU(p->dfbuf.ensure((size_t)2 * c->NCL * P * 4));
-            CU(p->dcounter.ensure(64));
-            CU(cudaMemsetAsync(p->dcounter.p, 0, 64, st));
-            a.fbuf = p->dfbuf.as<float>(); a.counter = p->dcounter.as<unsigned>();
-        }
-        const int threads = c->NW * 32;
-        cudaError_t e = c->resident ? launch_vk<true>(a, c->n_clusters, c->CS, threads, c->smem, st)
-                                    : launch_vk<false>(a, c->n_clusters, c->CS, threads, c->smem, st);
-        CU(e);
-        p->kinfo[0] = 2; p->kinfo[1] = c->CS; p->kinfo[2] = c->n_clusters; p->kinfo[3] = threads;
-        p->kinfo[4] = (int)c->smem; p->kinfo[5] = c->resident | (c->grid_team << 1); p->kinfo[6] = a.tiles_per_n; p->kinfo[7] = P;
     }
-    if (first_bad) {
-        CU(cudaMemcpyAsync(first_bad, p->dbad.p, (size_t)batch * 4, cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
-        if (flow_launched) {
-            int flag = 0;
-            CU(cudaMemcpyFromSymbol(&flag, md::flow_timeout_flag, sizeof(int)));
-            if (flag) {
-                const int zero = 0;
-                CU(cudaMemcpyToSymbol(md::flow_timeout_flag, &zero, sizeof(int)));
-                p->err += "vK flow kernel: a cross-CTA exchange timed out (team not co-resident?)\n";
-                return MODAL_ECUDA;
-            }
-        }
-        for (int b = 0; b < batch; ++b)
-            if (first_bad[b] >= 0) {
-                char buf[96];
-                snprintf(buf, sizeof buf, "sample %d went non-finite at step %d\n", b, first_bad[b]);
-                p->err += buf;
-                return MODAL_EUNSTABLE;
-            }
-    }
-    return MODAL_OK;
+    p->last_stream = st; p->last_batch = batch; p->last_persistent = persistent; p->pending = true;
+    return first_bad ? finish(p, first_bad) : MODAL_OK;
 }
 
 modal_status check_sim_args(modal_plan *p, int batch, int n_steps, const modal_init *init, const void *out)
@@ -883,7 +742,7 @@ extern "C" modal_status modal_plan_create(const modal_plan_desc *desc, int cuda_
         p->mq = mh::rect_modes(d.Lx, d.Ly, nq);
         if (d.model == MODAL_VK) p->mphi = mh::rect_modes(d.Lx, d.Ly, d.n_phi);   // reading R5
     } else p->mq = mh::string_modes(d.Lx, nq);
-    p->NQP = d.model == MODAL_VK ? mh::padded_nq(nq) : ((nq + 31) / 32) * 32;
+    p->NQP = d.model == MODAL_VK ? mh::flow_padded_nq(nq) : ((nq + 31) / 32) * 32;
     build_perm(p);
     p->coeff_batch = 1;
     p->omega.resize(nq); p->sigma.resize(nq); p->pickup.resize(nq); p->lambda_s.resize(nq);
@@ -987,12 +846,63 @@ extern "C" modal_status modal_simulate_host(modal_plan *p, int batch, int n_step
     const size_t bytes = (size_t)batch * n_steps * 4;
     CU(cudaSetDevice(p->device));
     CU(p->dout.ensure(bytes));
+    if (p->pinned_bytes < bytes) {                       // pinned staging: the D2H copy runs at PCIe speed
+        if (p->pinned_out) cudaFreeHost(p->pinned_out);
+        p->pinned_out = nullptr; p->pinned_bytes = 0;
+        CU(cudaMallocHost(&p->pinned_out, bytes));
+        p->pinned_bytes = bytes;
+    }
+    s = run(p, batch, n_steps, init, p->dout.as<float>(), nullptr, nullptr);
+    if (s != MODAL_OK) return s;
+    CU(cudaMemcpyAsync(p->pinned_out, p->dout.p, bytes, cudaMemcpyDeviceToHost, nullptr));
     std::vector<int> bad(batch, -1);
-    s = run(p, batch, n_steps, init, p->dout.as<float>(), bad.data(), nullptr);
+    s = finish(p, bad.data());
     if (s != MODAL_OK && s != MODAL_EUNSTABLE) return s;
-    CU(cudaMemcpy(out_audio_host, p->dout.p, bytes, cudaMemcpyDeviceToHost));
+    memcpy(out_audio_host, p->pinned_out, bytes);
     if (first_bad_step) memcpy(first_bad_step, bad.data(), (size_t)batch * 4);
     return s;
+}
+
+extern "C" modal_status modal_plan_check(modal_plan *p, int *first_bad_step)
+{
+    if (!p) return MODAL_EINVAL;
+    if (p->device < 0) { p->err = "plan has no CUDA device (host-only plan)\n"; return MODAL_ECUDA; }
+    return finish(p, first_bad_step);
+}
+
+extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, int value)
+{
+    if (!p || !key) return MODAL_EINVAL;
+    p->err.clear();
+    struct { const char *name; int *field; int lo, hi; } tab[] = {
+        {"vk_impl", &p->opt.vk_impl, 0, 2}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
+        {"flow_res", &p->opt.flow_res, -1, 1 << 20}, {"mma_split", &p->opt.mma_split, 0, 4}, {"mma_ng", &p->opt.mma_ng, 0, 8},
+        {"mma_nstg", &p->opt.mma_nstg, 0, 16}, {"parity_order", &p->opt.parity_order, 0, 1}, {"timing", &p->opt.timing, 0, 1}};
+    for (auto &t : tab)
+        if (!strcmp(key, t.name)) {
+            if (value < t.lo || value > t.hi) { p->err = std::string("option ") + key + ": value out of range\n"; return MODAL_EINVAL; }
+            if (*t.field == value) return MODAL_OK;
+            const int old = *t.field;
+            *t.field = value;
+            if (t.field == &p->opt.parity_order && p->d.model == MODAL_VK) {
+                // re-pack H in the new internal order (user-order copy through the old permutation)
+                const int nq = p->d.n_q, nphi = p->d.n_phi;
+                std::vector<double> Hi((size_t)nphi * nq * nq), Hu((size_t)nphi * nq * nq);
+                mh::unpack_flow_tiles(nq, nphi, p->Hf, Hi.data());
+                for (int n = 0; n < nphi; ++n)
+                    for (int a = 0; a < nq; ++a)
+                        for (int b = 0; b < nq; ++b)
+                            Hu[((size_t)n * nq + p->perm[a]) * nq + p->perm[b]] = Hi[((size_t)n * nq + a) * nq + b];
+                (void)old;
+                build_perm(p);
+                set_H(p, [&](int n, int a, int b) { return Hu[((size_t)n * nq + a) * nq + b]; });
+                p->coeffs_dirty = true;
+            }
+            if (t.field == &p->opt.mma_split || t.field == &p->opt.mma_ng) { p->mma.tried = false; p->mma.ok = false; }
+            return MODAL_OK;
+        }
+    p->err = std::string("unknown option ") + key + "\n";
+    return MODAL_EINVAL;
 }
 
 extern "C" void modal_plan_destroy(modal_plan *p)
@@ -1000,11 +910,12 @@ extern "C" void modal_plan_destroy(modal_plan *p)
     if (!p) return;
     if (p->device >= 0) {
         cudaSetDevice(p->device);
-        for (DevBuf *b : {&p->dHt, &p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dw, &p->dlam, &p->dc, &p->dq0,
-                          &p->dv0, &p->dgain, &p->dbad, &p->dout, &p->dfbuf, &p->dcounter, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming, &p->dperm, &p->mma.dslabs, &p->mma.dn0, &p->mma.dQg,
-                          &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags}) b->release();
+        if (p->pending) cudaStreamSynchronize(p->last_stream);
+        for (DevBuf *b : {&p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dsT, &p->dw, &p->dlam, &p->dc, &p->dq0, &p->dv0, &p->dgain, &p->dbad,
+                          &p->dout, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming, &p->dperm, &p->dtimeout, &p->mma.dslabs, &p->mma.dtab,
+                          &p->mma.dQop, &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags, &p->mma.dpx}) b->release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
-        for (auto &kv : p->vk_cfgs) { kv.second.units.release(); kv.second.warp_ptr.release(); kv.second.cta_ptr.release(); kv.second.nlo.release(); }
+        if (p->pinned_out) cudaFreeHost(p->pinned_out);
     }
     delete p;
 }
@@ -1031,6 +942,55 @@ extern "C" modal_status modal_plan_query(const modal_plan *p, int what, void *ds
         case MODAL_Q_COEFF_BATCH: return put(&cb, 4);
         case MODAL_Q_KERNEL_INFO: return put(p->kinfo, sizeof p->kinfo);
         case MODAL_Q_TILE_STATS: { const int ts[2] = {(int)p->tile_nz.size(), (int)p->nz_tiles}; return put(ts, sizeof ts); }
+        case MODAL_Q_MMA_LAYOUT: {
+            mh::MmaLayout L;
+            int v[16] = {0};
+            if (mma_host_layout(p, L)) {
+                const int w[16] = {1, L.NKB, L.NGRP, L.NG, L.NC, L.S, L.RBT, L.RBQ, L.KC, L.KCL, L.G, L.rows_max,
+                                   *std::min_element(L.kcnt.begin(), L.kcnt.end()), *std::max_element(L.kcnt.begin(), L.kcnt.end()),
+                                   (int)(L.slab_bytes / 1024), *std::max_element(L.fcnt.begin(), L.fcnt.end())};
+                memcpy(v, w, sizeof v);
+            }
+            return put(v, sizeof v);
+        }
+        case MODAL_Q_MMA_SLAB_CHECK: {
+            // host-side self check of the operand packing: rebuilds H^n[k][r] from the bf16 hi + lo slabs of every CTA and
+            // returns {entries covered, entries of H that are non-zero, max |hi + lo - H| / max |H|} as 3 doubles
+            mh::MmaLayout L;
+            double out[3] = {0, 0, 0};
+            if (mma_host_layout(p, L)) {
+                std::vector<uint16_t> slabs;
+                mma_host_slabs(p, L, slabs);
+                std::vector<double> Hi((size_t)d.n_phi * nq * nq);
+                mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, Hi.data());
+                double hmax = 0, emax = 0, covered = 0, nonzero = 0;
+                for (double x : Hi) { hmax = std::max(hmax, std::fabs(x)); nonzero += x != 0.0; }
+                std::vector<int> kop(L.KP, -1);
+                for (const mh::MmaBlock &b : L.blocks) for (int x = 0; x < b.nb; ++x) kop[b.koff + x] = b.k0 + x;
+                for (int i = 0; i < L.NGRP; ++i)
+                    for (int j = 0; j < L.NKB; ++j) {
+                        const int c = i * L.NKB + j;
+                        const uint16_t *base = &slabs[(size_t)c * L.slab_bytes / 2];
+                        for (int x = 0; x < L.kcnt[c]; ++x)
+                            for (int nl = 0; nl < L.NG; ++nl) {
+                                const int n = L.nlist[(size_t)i * L.NG + nl];
+                                if (n < 0) continue;
+                                for (int kk = 0; kk < L.blocks[j].nb; ++kk)
+                                    for (int e = 0; e < 16; ++e) {
+                                        const int r = kop[L.klist[(size_t)c * L.KCL + x] * 16 + e];
+                                        if (r < 0) continue;
+                                        const size_t off = ((size_t)x * 2 * L.NC * 32 + mh::umma_chunk_off(nl * L.RBT + kk, e)) / 2;
+                                        const double v = (double)mh::bf16_to_float(base[off]) + (double)mh::bf16_to_float(base[off + (size_t)L.NC * 16]);
+                                        const double h = Hi[((size_t)n * nq + L.blocks[j].k0 + kk) * nq + r];
+                                        emax = std::max(emax, std::fabs(v - h));
+                                        covered += h != 0.0;
+                                    }
+                            }
+                    }
+                out[0] = covered; out[1] = nonzero; out[2] = hmax > 0 ? emax / hmax : 0.0;
+            }
+            return put(out, sizeof out);
+        }
         case MODAL_Q_H_FULL: {
             if (d.model != MODAL_VK) return MODAL_EINVAL;
             const size_t bytes = (size_t)d.n_phi * nq * nq * 8;

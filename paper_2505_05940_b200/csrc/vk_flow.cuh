@@ -46,6 +46,7 @@ struct FlowArgs {
     unsigned long long *fx;     // [NT][G][NQP]   partial forces
     unsigned long long *gx;     // [NT][n_phi][MS] partial G_n of shared modes
     unsigned long long *qx;     // [NT][FLOW_QREP][NQP]  new state
+    int *timeout_flag;          // per plan: set when a bounded wait gave up
     long long *timing;          // optional [G*NT][8]: cycles in phases A, B1, B2+C+D, total (MODAL_FLOW_TIMING)
 };
 
@@ -55,10 +56,9 @@ __device__ __forceinline__ void st_tag(unsigned long long *p, float v, unsigned 
     const unsigned long long w = ((unsigned long long)epoch << 32) | (unsigned long long)__float_as_uint(v);
     asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(w) : "memory");
 }
-// Every wait is bounded (~1-2 s): a waiter that gives up raises the CTA's abort word and the global
-// flag, after which all waits of the CTA fall through and the step loop ends, so a broken exchange
-// (e.g. a team that is not co-resident) ends in an error code instead of a hung device.
-__device__ int flow_timeout_flag;
+// Every wait is bounded (~1-2 s): a waiter that gives up raises the CTA's abort word, after which all waits
+// of the CTA fall through and the step loop ends; the CTA then raises the plan's timeout flag, so a broken
+// exchange (e.g. a team that is not co-resident) ends in an error code instead of a hung device.
 __device__ __forceinline__ float ld_tag(const unsigned long long *p, unsigned epoch, volatile int *abortp)
 {
     unsigned long long w;
@@ -66,7 +66,7 @@ __device__ __forceinline__ float ld_tag(const unsigned long long *p, unsigned ep
     do {
         asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(w) : "l"(p) : "memory");
         if ((unsigned)(w >> 32) == epoch) break;
-        if ((++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
+        if ((++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; break; }
     } while (true);
     return __uint_as_float((unsigned)w);
 }
@@ -79,7 +79,7 @@ __device__ __forceinline__ float2 ld_tag2(const unsigned long long *p, unsigned 
     do {
         asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(p) : "memory");
         if ((unsigned)(w0 >> 32) == epoch && (unsigned)(w1 >> 32) == epoch) break;
-        if ((++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
+        if ((++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; break; }
     } while (true);
     return make_float2(__uint_as_float((unsigned)w0), __uint_as_float((unsigned)w1));
 }
@@ -100,7 +100,7 @@ __device__ __forceinline__ float ld_tag_sum8(const unsigned long long *p, size_t
 #pragma unroll
         for (int i = 0; i < 8; ++i)
             if ((pend >> i & 1) && (unsigned)(w[i] >> 32) == epoch) { v[i] = __uint_as_float((unsigned)w[i]); pend &= ~(1u << i); }
-        if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
+        if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; break; }
     }
     return ((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]));
 }
@@ -121,7 +121,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, volatil
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
                      "selp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-        if (!ok && (++spins & 63u) == 0 && (*abortp || clock64() - t0 > 3000000000LL)) { *abortp = 1; flow_timeout_flag = 1; break; }
+        if (!ok && (++spins & 63u) == 0 && (*abortp || clock64() - t0 > 3000000000LL)) { *abortp = 1; break; }
     } while (!ok);
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar)
@@ -341,7 +341,7 @@ __global__ void __launch_bounds__(RING ? 544 : 512, 1) vk_flow_kernel(const Flow
                     ui += step_u; if (ui >= S) ui -= S;
                 } else if ((++idle & 255u) == 0) {
                     if (idle == 256) t0 = clock64();
-                    if (*s_abort || clock64() - t0 > 3000000000LL) { *s_abort = 1; flow_timeout_flag = 1; break; }
+                    if (*s_abort || clock64() - t0 > 3000000000LL) { *s_abort = 1; break; }
                 }
             }
         }
@@ -415,7 +415,7 @@ __global__ void __launch_bounds__(RING ? 544 : 512, 1) vk_flow_kernel(const Flow
                     // use has been consumed (another warp may still be working on it)
                     if (lane == 0) {
                         unsigned spins = 0;
-                        while (done[slot] != use) if ((++spins & 1023u) == 0 && (*s_abort || spins > (1u << 24))) { *s_abort = 1; flow_timeout_flag = 1; break; }
+                        while (done[slot] != use) if ((++spins & 1023u) == 0 && (*s_abort || spins > (1u << 24))) { *s_abort = 1; break; }
                     }
                     __syncwarp();
                     mbar_wait(smem_u32(bars + slot), use & 1, s_abort);
@@ -531,6 +531,7 @@ __global__ void __launch_bounds__(RING ? 544 : 512, 1) vk_flow_kernel(const Flow
         }
         bar_consumers(NC);
     }
+    if (tid == 0 && *s_abort) *a.timeout_flag = 1;
 }
 
 }  // namespace modal_dev

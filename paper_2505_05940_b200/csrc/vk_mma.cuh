@@ -1,28 +1,39 @@
-// vk_mma.cuh -- batched MODAL_VK time loop on tcgen05 tensor cores, ONE persistent sm_100a kernel
-// (layout in mma_schedule.hpp).
+// vk_mma.cuh -- batched MODAL_VK time loop on tcgen05 tensor cores, ONE persistent sm_100a kernel for the whole
+// batch (layout in mma_schedule.hpp).
 //
-// Per time step, for up to 256 samples at once (two M tiles of 128):
+// Per time step, for every M tile of 128 samples (any number of tiles in one launch):
 //   t[b][(n,k)] = sum_r q[b][r] H^n[k][r]        tcgen05.mma kind::f16, bf16 hi/lo split, 3 MMAs per K chunk,
 //                                                A = q chunk streamed by TMA from L2, B = H slab resident in
-//                                                shared memory, D = t in TMEM (fp32), kept for both epilogues
+//                                                shared memory, D = t in a TMEM accumulator slot (fp32), kept
+//                                                for both epilogues
 //   G[b][n]  = sum_k q[b][k] t[b][(n,k)]         epilogue 1 (tcgen05.ld, one thread per sample), partial over
-//                                                the CTA's RB rows k; summed over the k blocks through L2
+//                                                the rows k of the CTA's block; summed over the k blocks through L2
 //   eta      = s_n[b] G[b][n]                    (Eq. 9, C eliminated by PAPER.md:283)
 //   f[b][k]  = sum_n eta[b][n] t[b][(n,k)]       epilogue 2, partial over the CTA's modes n; summed over
 //                                                the n groups through L2 by the owner of (b, k)
 //   fp64 delta-form update of the owner's (q, v) (Eq. 19-23), q republished as fp32 and
 //   as bf16 hi/lo in operand layout; pickup out[b][n] = w . q^n.
-// CTA (i,j) owns in-plane modes of group i and rows k of block j.
+// CTA (i,j) owns the in-plane modes of group i and the rows k of block j.
 //
-// Exchange between CTAs (no grid barrier, no atomics):
+// Roles (16 warps).  The stages of a tile-step are handled by DIFFERENT warps, each walking the tiles in the same
+// order, so several tiles are in flight and a warp that waits on an exchange never holds up the tensor pipe:
+//   warp 0      P  polls the q flags of the tile's source blocks, streams its K chunks through the ring by TMA
+//   warp 1      M  one thread issues the MMAs of the tile into accumulator slot (tile mod S) and commits
+//   warp 2      W  (block-0 CTAs) sums the pickup partials of its rows over the k blocks, writes the audio
+//   warps 4-7   O  owners: gather the partial forces of the owned (row, k) elements, fp64 update, publish q
+//   warps 8-15  E  two epilogue groups of 128 threads (thread <-> TMEM lane <-> sample), tiles alternate
+//
+// Exchange between CTAs (no grid barrier, no atomics; every wait is bounded):
 //  * partial G and partial f travel as TAGGED fp32 words: the two low mantissa bits carry (step+1) & 3, the
 //    value is rounded to a multiple of 4 ulp (2^-22 relative, far below the 2^-17 of the split products).
 //    A reader polls the data words themselves (ld.relaxed.gpu) until every tag matches: one L2 round trip,
-//    no fence, no flag.  A word is only overwritten after q of the next step has been published by every
-//    owner, i.e. after every reader of the previous value has consumed it, so a tag can never be mistaken
-//    for the one written four steps earlier.
+//    no fence, no flag.  Partial f of (tile, group, block) is rewritten only after q of the next step has been
+//    flagged by EVERY owner of that block, i.e. after every reader consumed it.  Partial G is double-buffered by
+//    step parity: a CTA can be at most one step ahead of a peer of its group (it needs the peer's next partial).
 //  * the new state q feeds the TMA (async proxy), which cannot poll: owners store, one thread per
-//    (CTA, tile) releases an epoch flag, the TMA warp of every CTA acquires the flags of all CTAs.
+//    (CTA, tile) releases an epoch flag, warp P of every CTA that reads the block acquires its owners' flags.
+//  * pickup partials (per row and k block) travel as {fp32, epoch} 64-bit words, double-buffered by step parity;
+//    an owner releases its flag only after warp W of its CTA consumed the partials of the step before.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -30,44 +41,72 @@
 
 namespace modal_dev {
 
-constexpr int MMA_NSTG = 6;          // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo) the layout fit assumes; the
-constexpr int MMA_NSTG_MAX = 16;     // launch uses MmaArgs::NSTG stages (8 by default, <= 16) beside the compacted slab
-// mbarrier indices: full[0..15] empty[16..31] acc_full[32,33] acc_empty[34,35] qready[36,37]; tmem pointer at word 40,
-// abort word at 41, K-chunk list (64 ints) from word 44
-constexpr int MB_FULL = 0, MB_EMPTY = 16, MB_ACCF = 32, MB_ACCE = 34, MB_QRDY = 36, MB_TPTR = 40, MB_ABORT = 41, MB_KLIST = 44;
-constexpr int MMA_THREADS = 384;     // warpgroup 0: warps 0 / 2 TMA producers, warps 1 / 3 MMA issuers of tile 0 / 1 (56 registers
-                                     // after setmaxnreg); warpgroups 1 / 2: epilogue + pickup of tile 0 / 1 (224 registers)
-constexpr int MMA_FS = 8;            // words between the q flags of consecutive CTAs: one flag per 32-byte sector (C3 b256: 1 / 4 /
-                                     // 8 / 16 / 32 words = 16.7 / 15.6 / 15.3 / 15.5 / 15.6 us per step; 147 stores to five lines serialise)
-constexpr int MMA_FB = 11;           // 16-byte partial-force loads in flight per thread while polling (a thread keeps ~16 strong loads in flight)
+constexpr int MMA_THREADS = 512;
+constexpr int MMA_NSTG_MAX = 16;     // q-operand ring stages (8 KiB each: 128 rows x 16 K x hi/lo)
+constexpr int MMA_MT_MAX = 8;        // M tiles per launch (== modal_host::MMA_MT_MAX): wider batches run as consecutive launches
+constexpr int MMA_FS = 8;            // words between consecutive q flags: one flag per 32-byte sector (profiles/r1_c3_b256.md)
+constexpr int MMA_GB = 16;           // 16-byte strong loads a lane keeps in flight while gathering (all n groups of the C3 layout in one round trip)
+constexpr int MMA_RB_MAX_DEV = 56;   // == modal_host::MMA_RB_MAX: rows k of a block (a sample's block of q lives in registers)
+constexpr int MMA_NG_MAX_DEV = 8;    // == modal_host::MMA_NG_MAX: in-plane modes of a group
+// mbarrier indices (64-bit words of the first shared-memory block)
+constexpr int MB_FULL = 0, MB_EMPTY = 16, MB_ACCF = 32, MB_ACCE = 35, MB_QRDY = 38, MB_TPTR = 56, MB_ABORT = 57, MB_STAMP = 58;   // QRDY: one per tile (<= 16)
+constexpr int MMA_TAB_OFF = 512;     // byte offset of the per-CTA tables inside the first block (ints): klist[64] nmode[8] fblk[16] blk[16][3]
+constexpr int MMA_BARS_BYTES = 1536;
 
 struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H: only the K chunks of klist, in list order
-    int slab_bytes, NSTG;       // NSTG: ring stages of this launch (even, <= 16)
-    int NKB, RB, NGRP, NG, NG4, NC, KC, KP, QS, G, nel_max;
+    int slab_bytes, NSTG;
+    int NKB, NGRP, NG, NG4, NC, S, RBT, RBQ, KC, KCL, G, rows_max, LPQ;
     const int *nlist;           // [NGRP][NG] in-plane modes of each group (-1: empty)
-    const int *klist, *kcnt;    // [G][KC], [G]: K chunks with a non-zero slab part (all others are skipped)
+    const int *klist, *kcnt;    // [G][KCL], [G]
+    const int *fblk, *fcnt;     // [G][16], [G]: blocks whose owners this CTA waits for (own block first)
+    const int *blk;             // [NKB][3]: k0, nb, koff
     int n_q, n_phi, NQP;
-    int batch, n_steps, MT;     // batch <= 256; MT = M tiles in use
+    int batch, n_steps, MT;
     int coeff_stride_q, coeff_stride_phi;
     const double *kv, *kq, *r, *astart;
-    const float *s, *w;
+    const float *sT, *w;        // sT: s_n transposed [n_phi][sT_stride] (sample-major inside a mode: coalesced per warp)
+    int sT_stride;
     const double *q0, *v0;
     int auto_start; double half_T2;
     const float *fext; const double *gain;
     float *out; double *traj; const int *kperm; int *first_bad;
     // exchange (global, L2 resident)
-    uint16_t *Qg;               // [2][KC][2][4096 B]   q as bf16 hi/lo operand chunks
-    float *qf;                  // [256][QS]            q fp32
-    uint32_t *Gx;               // [G][2][128][4*NG4]   partial G, tagged
-    uint32_t *fx;               // [NGRP][2][128][QS]   partial f, tagged
-    unsigned *qflag;            // [2][G][MMA_FS] epochs, one per (tile, CTA), each in its own 32-byte sector
-    long long *timing;          // optional [G][8] cycle counters of tile 0 (MODAL_FLOW_TIMING)
+    uint16_t *Qop;              // [MT][KC][8192 B]                 q as bf16 operand chunks (hi 4 KiB, lo 4 KiB)
+    float *qf;                  // [MT][NKB][RBQ][128][4]           q fp32, quads of 4 consecutive k of a block
+    uint32_t *Gx;               // [2][MT][NGRP][NKB][128][4*NG4]   partial G, tagged, by step parity
+    uint32_t *fx;               // [MT][NGRP][NKB][RBQ][128][4]     partial f, tagged
+    unsigned *qflag;            // [MT][NKB][NGRP][MMA_FS]          epochs
+    unsigned long long *px;     // [2][MT][NKB][128][2]             pickup partials {o, epoch}, {|q|^2, epoch}
+    int *timeout_flag;          // per plan: set when a bounded wait gave up
+    long long *timing;          // optional [G][16] cycle counters of tile 0
 };
+
+struct MmaSmem { size_t bars, sq, sv, coef, pk, sbad, wdone, slab, ring, total; };
+__host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int MT, int rows_max, int RBQ, int nstg)
+{
+    MmaSmem L; size_t o = 0;
+    const size_t nel = (size_t)rows_max * RBQ * 4;
+    L.bars = o;  o += MMA_BARS_BYTES;
+    L.sq = o;    o += (size_t)MT * nel * 8;
+    L.sv = o;    o += (size_t)MT * nel * 8;
+    L.coef = o;  o += (size_t)MT * nel * 28;                    // the owners' update coefficients, per tile: kv[nel], kq[nel], r[nel] fp64, w[nel] fp32
+    L.pk = o;    o += (size_t)2 * 2 * rows_max * RBQ * 8;       // [team][buffer][row][quad] float2
+    L.sbad = o;  o += (size_t)MT * rows_max * 4;
+    L.wdone = o; o += (size_t)MMA_MT_MAX * 4;
+    o = flow_align(o, 128);
+    L.slab = o;  o += (size_t)slab_bytes;
+    o = flow_align(o, 128);
+    L.ring = o;  o += (size_t)nstg * 8192;
+    L.total = o;
+    return L;
+}
+__host__ __device__ inline size_t mma_smem_fixed() { return MMA_BARS_BYTES + 4096 + 1024; }   // besides slab, ring and owner state
 
 __device__ __forceinline__ void set_flag(unsigned *p, unsigned epoch)
 {
-    asm volatile("fence.acq_rel.gpu;\n\tst.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(epoch) : "memory");
+    // st.release = MEMBAR.ALL.GPU + strong store; fence.acq_rel + st.relaxed would add a CCTL.IVALL (L1 invalidate) the owner does not need
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(epoch) : "memory");
 }
 __device__ __forceinline__ void bar_named(int id, int nthreads)
 {
@@ -95,37 +134,6 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&u)[1
                  : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// The flags p[0 .. count): relaxed polls with a short sleep between rounds, then one ld.acquire.gpu per flag, which orders
-// the q data behind the flags.  All CTAs poll the same few L2 lines while the owners try to store to them, so the
-// polling rate matters (C3, us per step at batch 256 / 128): ld.acquire polls back to back 17.9 / 13.8 (each is followed
-// by an L1 invalidate, which throttles them), relaxed polls back to back 21.3 / 13.3, relaxed + 400 ns sleep 16.6 / 12.8;
-// a fence.acq_rel.gpu after relaxed polls measured slower (the MEMBAR stalls the epilogue warps of the other tile).
-// (1.5 us sleep 16.3 / 12.6; sleeping through an estimate of the wait before the first poll 16.5 / 16.5: nanosleep overshoots)
-constexpr unsigned MMA_POLL_SLEEP = 400;      // ns between polling rounds (with one flag per sector 0 / 200 / 400 / 800 ns: 15.5 / 15.4 / 15.3 / 15.5)
-__device__ __forceinline__ void poll_flags(const unsigned *p, int lane, int count, unsigned epoch, volatile int *abortp)
-{
-    for (int base = lane; base < count; base += 256) {
-        unsigned pend = 0, spins = 0;
-#pragma unroll
-        for (int u = 0; u < 8; ++u) if (base + 32 * u < count) pend |= 1u << u;
-        while (pend) {
-            unsigned v[8];
-#pragma unroll
-            for (int u = 0; u < 8; ++u)
-                if (pend >> u & 1) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(p + (size_t)(base + 32 * u) * MMA_FS) : "memory");
-#pragma unroll
-            for (int u = 0; u < 8; ++u) if ((pend >> u & 1) && v[u] >= epoch) pend &= ~(1u << u);
-            if (pend && (++spins & 1023u) == 0 && (*abortp || spins > (1u << 21))) { *abortp = 1; flow_timeout_flag = 1; break; }
-            if (pend) __nanosleep(MMA_POLL_SLEEP);
-        }
-#pragma unroll
-        for (int u = 0; u < 8; ++u)
-            if (base + 32 * u < count) {
-                // the value is not needed: the load is the acquire
-                asm volatile("{\n\t.reg .b32 t;\n\tld.acquire.gpu.global.u32 t, [%0];\n\t}" ::"l"(p + (size_t)(base + 32 * u) * MMA_FS) : "memory");
-            }
-    }
-}
 __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
 {
     uint32_t u = __float_as_uint(x);
@@ -151,318 +159,581 @@ __device__ __forceinline__ uint4 ld_relaxed4(const uint32_t *p)
     asm volatile("ld.relaxed.gpu.global.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "l"(p) : "memory");
     return w;
 }
-__device__ __forceinline__ uint32_t ld_relaxed1(const uint32_t *p)
-{
-    uint32_t w;
-    asm volatile("ld.relaxed.gpu.global.b32 %0, [%1];" : "=r"(w) : "l"(p) : "memory");
-    return w;
-}
 __device__ __forceinline__ bool tags_ok(const uint4 &w, uint32_t tag)
 {
     return ((w.x & 3u) == tag) & ((w.y & 3u) == tag) & ((w.z & 3u) == tag) & ((w.w & 3u) == tag);
 }
+__device__ __forceinline__ void mma_give_up(volatile int *s_abort, int *gflag) { *s_abort = 1; *gflag = 1; }
 
-__host__ __device__ inline int mma_own_bytes(int nel_max) { return nel_max <= 512 ? 40 : 16; }
-struct MmaSmem { size_t bars, own, sbad, cst, slab, ring, total; };
-__host__ __device__ inline size_t mma_smem_fixed() { return 1024 + 256 * 4 + 256 * 64 + (size_t)MMA_NSTG * 8192 + 384; }
-__host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int nel_max, int nstg)
+// The flags p[f * MMA_FS], f in the lane's share of [0, count): relaxed polls with a short sleep between rounds, then
+// one ld.acquire.gpu per flag, which orders the q data behind the flags (profiles/r1_c3_b256.md: acquire polls
+// are throttled by the L1 invalidate that follows each, back-to-back relaxed polls hammer the lines the owners store to).
+constexpr unsigned MMA_POLL_SLEEP = 200;      // ns between polling rounds
+__device__ __forceinline__ void poll_flag_list(const unsigned *base, const int *fblk, int fcnt, int NGRP, int lane,
+                                               unsigned epoch, volatile int *s_abort)
 {
-    MmaSmem L; size_t o = 0;
-    L.bars = o; o += 1024;                                 // mbarriers, tmem pointer, abort word, K-chunk list (MB_* above)
-    L.own = o;  o += (size_t)2 * nel_max * mma_own_bytes(nel_max);   // owner state per tile: q, v (+ kv, kq, r if they fit), fp64 [nel_max] each
-    L.sbad = o; o += 256 * 4;
-    L.cst = o;  o += 256 * 64;                             // per epilogue thread: s_n[16] floats
-    o = flow_align(o, 128);
-    L.slab = o; o += (size_t)slab_bytes;
-    o = flow_align(o, 128);
-    L.ring = o; o += (size_t)nstg * 8192;
-    L.total = o;
-    return L;
+    const int count = fcnt * NGRP;
+    for (int f0 = 0; f0 < count; f0 += 128) {
+        const unsigned *ptr[4];
+        unsigned pend = 0, spins = 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int f = f0 + 32 * u + lane;
+            ptr[u] = base;
+            if (f < count) {
+                const int bi = f / NGRP, i = f - bi * NGRP;
+                ptr[u] = base + ((size_t)fblk[bi] * NGRP + i) * MMA_FS;
+                pend |= 1u << u;
+            }
+        }
+        const unsigned mine = pend;
+        while (pend) {
+            unsigned v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (pend >> u & 1) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v[u]) : "l"(ptr[u]) : "memory");
+#pragma unroll
+            for (int u = 0; u < 4; ++u) if ((pend >> u & 1) && v[u] >= epoch) pend &= ~(1u << u);
+            if (pend && (++spins & 255u) == 0 && (*s_abort || spins > (1u << 22))) { *s_abort = 1; break; }
+            if (pend) __nanosleep(MMA_POLL_SLEEP);
+        }
+#ifndef MMA_NO_ACQUIRE
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (mine >> u & 1)      // the value is not needed: the load is the acquire
+                asm volatile("{\n\t.reg .b32 t;\n\tld.acquire.gpu.global.u32 t, [%0];\n\t}" ::"l"(ptr[u]) : "memory");
+#else
+        (void)mine;
+#endif
+    }
 }
 
-// One epilogue group = 128 threads = one M tile of 128 samples (thread <-> TMEM lane <-> sample).
-__device__ __forceinline__ void mma_epilogue_group(const MmaArgs &a, const int mt, const int c, const int i, const int j,
-                                                   const int r, uint64_t *bars, double *own,
-                                                   const uint32_t tbase, volatile int *s_abort, const int lane_base,
-                                                   int *sbad, const int gw, const int lane, float *sreg)
+// CTA-uniform view of the kernel's shared memory and of the CTA's place in the grid
+struct MmaCta {
+    int c, i, j;                // CTA, n group, k block
+    int k0, nb, koff, RBQj;     // this block: first internal mode, modes, operand offset, quads
+    int NGa;                    // modes of this group
+    int r0, rows;               // sample rows of a tile this CTA owns for the update
+    int KCA;                    // K chunks this CTA multiplies
+    uint64_t *bars;
+    const int *kl, *nmode, *fb, *blk;     // tables in shared memory
+    volatile int *s_abort;
+    double *sq, *sv; unsigned char *coef; float2 *pk; int *sbad; volatile int *wdone;
+    unsigned char *slab, *ring;
+    uint32_t tbase;
+    size_t nel;                 // owner-state elements per tile: rows_max * RBQ * 4
+};
+
+// ------------------------------------------------------------------------------------------------------------
+// E: one epilogue group = 128 threads = the 128 samples of a tile (thread <-> TMEM lane <-> sample).
+// The accumulator is read in units of 32 columns (one tcgen05.ld.32x32b.x32 each): unit u = (mode nl, 32-column part
+// sp) with NSP parts per mode (NSP = 1: up to 8 modes of <= 32 rows; NSP = 2: up to 4 modes of <= 64 rows).  The
+// load of unit u+1 is in flight while the FMAs of unit u run (double-buffered registers; tcgen05.wait::ld waits for
+// every outstanding load of the thread, so the next load is issued right after the wait).
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t (&u)[32])
 {
-    const int NC = a.NC, NG = a.NG, NG4 = a.NG4, QS = a.QS, NKB = a.NKB, NGRP = a.NGRP, B = a.batch, RB = a.RB, KC = a.KC;
-    const int nch = (RB + 15) >> 4;
-    const int b = mt * 128 + r;
-    const bool valid = b < B;
-    const float *sb = a.s + (size_t)(a.coeff_stride_phi ? (valid ? b : 0) : 0) * a.n_phi;
-    // the (sample, k) elements this group owns for the update: rows r0..r1 of the tile, RB modes of block j
-    const int r0 = 128 * i / NGRP, r1 = 128 * (i + 1) / NGRP, nel = (r1 - r0) * RB;
-    double *sq = own, *sv = own + a.nel_max, *skv = own + 2 * a.nel_max, *skq = own + 3 * a.nel_max, *sr = own + 4 * a.nel_max;
-    const bool csm = mma_own_bytes(a.nel_max) == 40;                                // update coefficients held in shared memory
-    uint16_t *Qt = a.Qg + (size_t)mt * KC * 4096;                                  // chunk kc at + kc * 4096 (hi; lo at + 2048)
-    // ---- owner state, coefficients, publish q^0 ----
-    for (int e = r; e < nel; e += 128) {
-        const int rr_ = e / RB, kk = e - rr_ * RB, re = r0 + rr_, be = mt * 128 + re, k = j * RB + kk;
-        double q = 0.0, v = 0.0, kv = 0.0, kq = 0.0, rc = 0.0;
-        if (be < B && k < a.n_q) {
-            q = a.q0[(size_t)be * a.NQP + k]; v = a.v0[(size_t)be * a.NQP + k];
-            const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
-            kv = a.kv[co]; kq = a.kq[co]; rc = a.r[co];
-            const float qfl = (float)q;
-            a.qf[(size_t)be * QS + k] = qfl;
-            const uint16_t hi = bf16_rn_dev(qfl), lo = bf16_rn_dev(qfl - __uint_as_float((uint32_t)hi << 16));
-            const int k16 = k & 15;
-            const int off = ((re >> 3) * 256 + (k16 >> 3) * 128 + (re & 7) * 16 + (k16 & 7) * 2) >> 1;
-            uint16_t *Qc = Qt + (size_t)(k >> 4) * 4096;
-            Qc[off] = hi; Qc[2048 + off] = lo;
-        }
-        sq[e] = q; sv[e] = v;
-        if (csm) { skv[e] = kv; skq[e] = kq; sr[e] = rc; }
-    }
-    bar_named(2 + mt, 128);
-    if (r == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * MMA_FS, 1u);
-    for (int u = 0; u < 16; ++u) {                                                // [16][256]: conflict-free
-        const int nn = u < NG ? a.nlist[i * NG + u] : -1;
-        sreg[u * 256] = nn >= 0 ? sb[nn] : 0.f;
-    }
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]),
+                   "=r"(u[8]), "=r"(u[9]), "=r"(u[10]), "=r"(u[11]), "=r"(u[12]), "=r"(u[13]), "=r"(u[14]), "=r"(u[15]),
+                   "=r"(u[16]), "=r"(u[17]), "=r"(u[18]), "=r"(u[19]), "=r"(u[20]), "=r"(u[21]), "=r"(u[22]), "=r"(u[23]),
+                   "=r"(u[24]), "=r"(u[25]), "=r"(u[26]), "=r"(u[27]), "=r"(u[28]), "=r"(u[29]), "=r"(u[30]), "=r"(u[31])
+                 : "r"(taddr));
+}
 
-    const uint32_t taddr0 = tbase + ((uint32_t)lane_base << 16) + (uint32_t)(mt * NC);
-    const bool tmg = a.timing && r == 0 && mt == 0;
-    long long *tm = a.timing + (size_t)c * 8;
-    uint32_t *grow = a.Gx + ((size_t)(c * 2 + mt) * 128 + r) * (4 * NG4);
-    const uint32_t *grd = a.Gx + ((size_t)((i * NKB) * 2 + mt) * 128 + r) * (4 * NG4);
-    const size_t gstride = (size_t)2 * 128 * 4 * NG4;                               // words between consecutive k blocks
-    uint32_t *frow = a.fx + ((size_t)(i * 2 + mt) * 128 + r) * QS + j * RB;
-    const size_t fstride = (size_t)2 * 128 * QS;                                    // words between consecutive n groups
-    const float *qrow = a.qf + (size_t)(valid ? b : 0) * QS + j * RB;
-
-    for (int n = 0; n < a.n_steps; ++n) {
+// E1: q of the own block, epilogue 1 (partial G), G hop send side -- every tile, in order.
+template <int NSP, bool TIMING>
+__device__ __forceinline__ void mma_epilogue_e1_tile(const MmaArgs &a, const MmaCta &C, const int r, const int lane_base, const int n, const int t,
+                                                     const bool tmg, long long (&tm)[7])
+{
+    constexpr int NQ = 32 * NSP;                            // q values of the block a thread keeps (zero beyond the block)
+    const int NG4 = a.NG4, NKB = a.NKB, NGRP = a.NGRP, RBT = a.RBT, RBQ = a.RBQ, S = a.S, MT = a.MT;
+    const int nun = C.NGa * NSP;                            // units that hold data
+    const size_t g_words = (size_t)128 * 4 * NG4;           // words of one (tile, group, block) partial-G array
+    {
         const uint32_t tag = ((uint32_t)n + 1u) & 3u;
-        long long tk = tmg ? clock64() : 0;
-        mbar_wait(smem_u32(bars + MB_QRDY + mt), n & 1, s_abort);                  // q^n published by everybody
-        if (tmg) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
-        // ---- this sample's q over the rows of block j (operand of epilogue 1) ----
-        float qb[32];
+        {
+            const int slot = t % S, uses = (MT - slot + S - 1) / S;
+            const unsigned use = (unsigned)n * (unsigned)uses + (unsigned)(t / S);
+            long long tk = tmg && t == 0 ? clock64() : 0;
+            mbar_wait(smem_u32(C.bars + MB_QRDY + t), n & 1, C.s_abort);                 // q^n of the own block is published
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
+            // ---- this sample's q over the rows of block j (operand of epilogue 1), coalesced quads ----
+            float q[NQ];
+            {
+                const float4 *qrow = reinterpret_cast<const float4 *>(a.qf) + ((size_t)(t * NKB + C.j) * RBQ) * 128 + r;
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (4 * u < RB) x = __ldcg(reinterpret_cast<const float4 *>(qrow) + u);
-            qb[4 * u] = x.x; qb[4 * u + 1] = x.y; qb[4 * u + 2] = x.z; qb[4 * u + 3] = x.w;
-        }
-        // ---- a1 pickup + a6 write-out: out[b][n] = w . q^n for the samples b = c, c+G, ... of this tile ----
-        for (int m = gw, b2 = c + gw * a.G; b2 < B; m += 4, b2 += 4 * a.G) {
-            if (b2 / 128 != mt) continue;
-            const float *wb = a.w + (size_t)(a.coeff_stride_q ? b2 : 0) * a.NQP;
-            float o = 0.f, nrm = 0.f;
-            for (int k = lane; k < a.n_q; k += 32) {
-                const float qk = __ldcg(a.qf + (size_t)b2 * QS + k);
-                o = fmaf(wb[k], qk, o); nrm = fmaf(qk, qk, nrm);
-            }
-#pragma unroll
-            for (int sh = 16; sh >= 1; sh >>= 1) { o += __shfl_xor_sync(FLOW_FULL, o, sh); nrm += __shfl_xor_sync(FLOW_FULL, nrm, sh); }
-            if (lane == 0) {
-                a.out[(size_t)b2 * a.n_steps + n] = o;
-                if (sbad[m] < 0 && !(isfinite(o) && isfinite(nrm))) sbad[m] = n;
-            }
-        }
-        mbar_wait(smem_u32(bars + MB_ACCF + mt), n & 1, s_abort);                  // t of this tile is in TMEM
-        if (tmg) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        // ---- epilogue 1: partial G over the RB rows k of block j, four modes per pass ----
-        for (int n4 = 0; n4 < NG4; ++n4) {
-            float g4[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int nl = 4 * n4 + u;
-                if (nl < NG) {
-                    uint32_t v0[16], v1[16];
-                    tmem_ld16_nowait(taddr0 + nl * RB, v0);
-                    if (nch > 1) tmem_ld16_nowait(taddr0 + nl * RB + 16, v1);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int kk = 0; kk < 16; ++kk)
-                        if (kk < RB) g4[u] = fmaf(qb[kk], __uint_as_float(v0[kk]), g4[u]);
-                    if (nch > 1) {
-#pragma unroll
-                        for (int kk = 0; kk < 16; ++kk)
-                            if (16 + kk < RB) g4[u] = fmaf(qb[16 + kk], __uint_as_float(v1[kk]), g4[u]);
-                    }
+                for (int u = 0; u < NQ / 4; ++u) {
+                    float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (u < C.RBQj) x = __ldcg(qrow + (size_t)u * 128);
+                    q[4 * u] = x.x; q[4 * u + 1] = x.y; q[4 * u + 2] = x.z; q[4 * u + 3] = x.w;
                 }
             }
-            st_tagged4(grow + 4 * n4, g4[0], g4[1], g4[2], g4[3], tag);                   // G hop, send side
+            mbar_wait(smem_u32(C.bars + MB_ACCF + slot), use & 1u, C.s_abort);            // t of this tile is in TMEM
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t taddr0 = C.tbase + ((uint32_t)lane_base << 16) + (uint32_t)(slot * a.NC);
+            // ---- epilogue 1: partial G over the rows k of block j ----
+            float g[MMA_NG_MAX_DEV];
+#pragma unroll
+            for (int nl = 0; nl < MMA_NG_MAX_DEV; ++nl) g[nl] = 0.f;
+            {   // straight-line double buffering: every iteration handles units u, u + 1 and always issues the next loads
+                // (addresses clamped to the last unit, whose reload is harmless), so no load sits under a branch
+                uint32_t v0[32], v1[32];
+                const int ulast = nun - 1;
+                tmem_ld32_nowait(taddr0, v0);
+                if (tmg && t == 0) { tmem_ld_wait(); tm[5] += clock64() - tk; }
+                for (int u = 0; u < nun; u += 2) {
+                    const int u1 = min(u + 1, ulast), u2 = min(u + 2, ulast);
+                    tmem_ld_wait();
+                    tmem_ld32_nowait(taddr0 + (u1 / NSP) * RBT + (u1 % NSP) * 32, v1);
+                    float p0[4] = {0.f, 0.f, 0.f, 0.f}, p1[4] = {0.f, 0.f, 0.f, 0.f};      // four chains each: the FMA latency is not on the path
+#pragma unroll
+                    for (int kk = 0; kk < 32; ++kk) p0[kk & 3] = fmaf(q[kk], __uint_as_float(v0[kk]), p0[kk & 3]);
+                    tmem_ld_wait();
+                    tmem_ld32_nowait(taddr0 + (u2 / NSP) * RBT + (u2 % NSP) * 32, v0);
+#pragma unroll
+                    for (int kk = 0; kk < 32; ++kk) p1[kk & 3] = fmaf(q[(NSP - 1) * 32 + kk], __uint_as_float(v1[kk]), p1[kk & 3]);
+                    const float acc0 = (p0[0] + p0[1]) + (p0[2] + p0[3]);
+                    float acc1 = (p1[0] + p1[1]) + (p1[2] + p1[3]);
+                    if (u + 1 > ulast) acc1 = 0.f;
+                    const int m0 = u / NSP, m1 = (u + 1) / NSP;              // NSP = 2: both units belong to mode u / 2
+#pragma unroll
+                    for (int m = 0; m < MMA_NG_MAX_DEV; ++m) g[m] += (m == m0 ? acc0 : 0.f) + (m == m1 ? acc1 : 0.f);
+                }
+                tmem_ld_wait();
+            }
+            if (tmg && t == 0) tm[6] += clock64() - tk;
+            // ---- G hop, send side (buffer of this step's parity) ----
+            uint32_t *gx = a.Gx + ((size_t)(n & 1) * MT + t) * NGRP * NKB * g_words;
+            uint32_t *grow = gx + ((size_t)C.i * NKB + C.j) * g_words + (size_t)r * 4 * NG4;
+            st_tagged4(grow, g[0], g[1], g[2], g[3], tag);
+            if (NG4 > 1) st_tagged4(grow + 4, g[4], g[5], g[6], g[7], tag);
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; }
         }
-        if (tmg) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; }
-        float eta[16];
-#pragma unroll
-        for (int u = 0; u < 16; ++u) eta[u] = 0.f;
+    }
+}
+
+// E2: G hop receive side, eta, epilogue 2 (partial force), release of the accumulator slot -- every tile, in order.
+// Runs on its own warpgroup, so the wait for the peers' partial G never holds up epilogue 1 of the next tile.
+template <int NSP, bool TIMING>
+__device__ __forceinline__ void mma_epilogue_e2_tile(const MmaArgs &a, const MmaCta &C, const int r, const int lane_base, const int n, const int t,
+                                                     const bool tmg, long long (&tm)[7])
+{
+    const int NG4 = a.NG4, NKB = a.NKB, NGRP = a.NGRP, B = a.batch, RBT = a.RBT, RBQ = a.RBQ, S = a.S, MT = a.MT;
+    const size_t g_words = (size_t)128 * 4 * NG4;
+    {
+        const uint32_t tag = ((uint32_t)n + 1u) & 3u;
         {
-            // ---- G hop, receive side: gather the partial rows of all k blocks of this mode group ----
+            const int slot = t % S, uses = (MT - slot + S - 1) / S;
+            const unsigned use = (unsigned)n * (unsigned)uses + (unsigned)(t / S);
+            const int b = t * 128 + r;
+            const bool valid = b < B;
+            const uint32_t taddr0 = C.tbase + ((uint32_t)lane_base << 16) + (uint32_t)(slot * a.NC);
+            const uint32_t *gx = a.Gx + ((size_t)(n & 1) * MT + t) * NGRP * NKB * g_words;
+            mbar_wait(smem_u32(C.bars + MB_ACCF + slot), use & 1u, C.s_abort);            // t of this tile is in TMEM
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            float sc[MMA_NG_MAX_DEV];                                                      // s_n of this sample: in flight during the hop
 #pragma unroll
-            for (int m = 0; m < 2; ++m)                                           // two float4 columns of the rows per batch
-                if (2 * m < NG4)
-                    for (int jj0 = 0; jj0 < NKB; jj0 += 8) {                        // k-block order (deterministic); 8 + 8 loads in flight
-                        uint4 x[16];
-                        const int cnt = min(8, NKB - jj0);
-                        const unsigned lo8 = cnt >= 8 ? 0xffu : ((1u << cnt) - 1u);
-                        unsigned pend = lo8 | (2 * m + 1 < NG4 ? lo8 << 8 : 0u), spins = 0;
-                        while (pend) {
+            for (int u = 0; u < MMA_NG_MAX_DEV; ++u) {
+                const int nn = u < a.NG ? C.nmode[u] : -1;
+                sc[u] = nn >= 0 ? __ldg(a.sT + (size_t)nn * a.sT_stride + (a.coeff_stride_phi && valid ? b : 0)) : 0.f;
+            }
+            long long tk = tmg && t == 0 ? clock64() : 0;
+            // ---- G hop, receive side: the partial rows of the other k blocks of this mode group, block order ----
+            float eta[MMA_NG_MAX_DEV];
 #pragma unroll
-                            for (int u = 0; u < 16; ++u)
-                                if (pend >> u & 1) x[u] = ld_relaxed4(grd + (size_t)(jj0 + (u & 7)) * gstride + 4 * (2 * m + (u >> 3)));
+            for (int u = 0; u < MMA_NG_MAX_DEV; ++u) eta[u] = 0.f;
+            {
+                const uint32_t *grd = gx + (size_t)C.i * NKB * g_words + (size_t)r * 4 * NG4;
+                for (int jj0 = 0; jj0 < NKB; jj0 += 8) {
+                    uint4 x[16];
+                    const int cnt = min(8, NKB - jj0);
+                    unsigned pend = 0, spins = 0;
 #pragma unroll
-                            for (int u = 0; u < 16; ++u)
-                                if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
-                            if (pend && (++spins & 1023u) == 0 && (*s_abort || spins > (1u << 21))) { *s_abort = 1; flow_timeout_flag = 1; break; }
-                        }
+                    for (int u = 0; u < 8; ++u)
+                        if (u < cnt) pend |= (1u << u) | (NG4 > 1 ? 1u << (u + 8) : 0u);
+                    while (pend) {
 #pragma unroll
-                        for (int u = 0; u < 8; ++u)
-                            if (u < cnt) {
-                                eta[8 * m] += untag(x[u].x); eta[8 * m + 1] += untag(x[u].y);
-                                eta[8 * m + 2] += untag(x[u].z); eta[8 * m + 3] += untag(x[u].w);
-                                if (2 * m + 1 < NG4) {
-                                    eta[8 * m + 4] += untag(x[u + 8].x); eta[8 * m + 5] += untag(x[u + 8].y);
-                                    eta[8 * m + 6] += untag(x[u + 8].z); eta[8 * m + 7] += untag(x[u + 8].w);
+                        for (int u = 0; u < 16; ++u)
+                            if (pend >> u & 1) x[u] = ld_relaxed4(grd + (size_t)(jj0 + (u & 7)) * g_words + 4 * (u >> 3));
+#pragma unroll
+                        for (int u = 0; u < 16; ++u)
+                            if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
+                        if (pend && (++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 21))) { *C.s_abort = 1; break; }
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (u < cnt) {
+                            {
+                                eta[0] += untag(x[u].x); eta[1] += untag(x[u].y); eta[2] += untag(x[u].z); eta[3] += untag(x[u].w);
+                                if (NG4 > 1) {
+                                    eta[4] += untag(x[u + 8].x); eta[5] += untag(x[u + 8].y);
+                                    eta[6] += untag(x[u + 8].z); eta[7] += untag(x[u + 8].w);
                                 }
                             }
-                    }
-        }
-#pragma unroll
-        for (int u = 0; u < 16; ++u) eta[u] *= sreg[u * 256];                             // eta_n = s_n G_n
-        if (tmg) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; }
-        // ---- epilogue 2: partial force over the modes n of group i, published as tagged words ----
-        for (int ch = 0; ch < nch; ++ch) {
-                float facc[16];
-#pragma unroll
-                for (int kk = 0; kk < 16; ++kk) facc[kk] = 0.f;
-#pragma unroll
-                for (int nl = 0; nl < 16; nl += 2)
-                    if (nl < NG) {
-                        uint32_t v0[16], v1[16];
-                        tmem_ld16_nowait(taddr0 + nl * RB + ch * 16, v0);
-                        if (nl + 1 < NG) tmem_ld16_nowait(taddr0 + (nl + 1) * RB + ch * 16, v1);
-                        tmem_ld_wait();
-#pragma unroll
-                        for (int kk = 0; kk < 16; ++kk) {
-                            facc[kk] = fmaf(eta[nl], __uint_as_float(v0[kk]), facc[kk]);
-                            if (nl + 1 < NG) facc[kk] = fmaf(eta[nl + 1], __uint_as_float(v1[kk]), facc[kk]);
                         }
-                    }
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (ch * 16 + 4 * u < RB)
-                        st_tagged4(frow + ch * 16 + 4 * u, facc[4 * u], facc[4 * u + 1], facc[4 * u + 2], facc[4 * u + 3], tag);
-            }
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        mbar_arrive(smem_u32(bars + MB_ACCE + mt));                                 // TMEM tile may be overwritten
-        if (tmg) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; }
-        // ---- f hop + owner update: group-ordered sum of the partial forces, a5 linear update (fp64, delta form) ----
-        // A warp handles 16 quads (4 consecutive k of one owned row) per pass: lanes 0-15 gather the first half of the
-        // groups, lanes 16-31 the second half, as 16-byte strong loads (few wide requests: a thread keeps only ~16 strong
-        // loads in flight, so the 4-byte version needed three L2 round trips); the halves meet through one shuffle, then
-        // every lane updates two elements of its quad.
-        for (int qbase = 0; qbase < nel; qbase += 256) {
-            const int hh = lane >> 4, e4 = qbase + 4 * (16 * gw + (lane & 15));
-            const int rr_ = e4 / RB, kk = e4 - rr_ * RB, re = r0 + rr_, be = mt * 128 + re, kq0 = j * RB + kk;
-            const bool qact = e4 < nel && be < B && kq0 < a.n_q;
-            const int NH = (NGRP + 1) >> 1, g0 = hh * NH, g1 = min(NGRP, g0 + NH);
-            const uint32_t *fq = a.fx + ((size_t)mt * 128 + (qact ? re : 0)) * QS + (qact ? kq0 : 0);
-            float4 fs = make_float4(0.f, 0.f, 0.f, 0.f);
-            for (int ii0 = g0; ii0 < g1; ii0 += MMA_FB) {                           // group order (deterministic)
-                uint4 x[MMA_FB];
-                const int cnt = min(MMA_FB, g1 - ii0);
-                unsigned pend = qact ? (1u << cnt) - 1u : 0u, spins = 0;
-                {   // first round: every word, addresses by pointer increments
-                    const uint32_t *p0 = fq + (size_t)ii0 * fstride;
-#pragma unroll
-                    for (int u = 0; u < MMA_FB; ++u)
-                        if (u < cnt) { x[u] = ld_relaxed4(p0); p0 += fstride; }
-#pragma unroll
-                    for (int u = 0; u < MMA_FB; ++u)
-                        if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
                 }
-                while (pend) {                                                      // stragglers only
+            }
 #pragma unroll
-                    for (int u = 0; u < MMA_FB; ++u)
-                        if (pend >> u & 1) x[u] = ld_relaxed4(fq + (size_t)(ii0 + u) * fstride);
+            for (int u = 0; u < MMA_NG_MAX_DEV; ++u) eta[u] *= sc[u];                       // eta_n = s_n G_n
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; }
+            // ---- epilogue 2: partial force over the modes n of group i, published as tagged quads ----
+            uint32_t *frow = a.fx + ((((size_t)t * NGRP + C.i) * NKB + C.j) * RBQ) * 512 + (size_t)r * 4;
 #pragma unroll
-                    for (int u = 0; u < MMA_FB; ++u)
-                        if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
-                    if (pend && (++spins & 1023u) == 0 && (*s_abort || spins > (1u << 21))) { *s_abort = 1; flow_timeout_flag = 1; break; }
+            for (int sp = 0; sp < NSP; ++sp) {
+                float facc[32];
+#pragma unroll
+                for (int kk = 0; kk < 32; ++kk) facc[kk] = 0.f;
+                uint32_t v0[32], v1[32];
+                const int nlast = C.NGa - 1;
+                tmem_ld32_nowait(taddr0 + sp * 32, v0);
+                for (int nl = 0; nl < C.NGa; nl += 2) {
+                    const int n1 = min(nl + 1, nlast), n2 = min(nl + 2, nlast);
+                    float e0 = 0.f, e1 = 0.f;
+#pragma unroll
+                    for (int m = 0; m < MMA_NG_MAX_DEV; ++m) { e0 = m == nl ? eta[m] : e0; e1 = m == nl + 1 ? eta[m] : e1; }
+                    if (nl + 1 > nlast) e1 = 0.f;
+                    tmem_ld_wait();
+                    tmem_ld32_nowait(taddr0 + n1 * RBT + sp * 32, v1);
+#pragma unroll
+                    for (int kk = 0; kk < 32; ++kk) facc[kk] = fmaf(e0, __uint_as_float(v0[kk]), facc[kk]);
+                    tmem_ld_wait();
+                    tmem_ld32_nowait(taddr0 + n2 * RBT + sp * 32, v0);
+#pragma unroll
+                    for (int kk = 0; kk < 32; ++kk) facc[kk] = fmaf(e1, __uint_as_float(v1[kk]), facc[kk]);
                 }
+                tmem_ld_wait();
 #pragma unroll
-                for (int u = 0; u < MMA_FB; ++u)
-                    if (u < cnt) { fs.x += untag(x[u].x); fs.y += untag(x[u].y); fs.z += untag(x[u].z); fs.w += untag(x[u].w); }
+                for (int u = 0; u < 8; ++u)
+                    if (8 * sp + u < C.RBQj)
+                        st_tagged4(frow + (size_t)(8 * sp + u) * 512, facc[4 * u], facc[4 * u + 1], facc[4 * u + 2], facc[4 * u + 3], tag);
             }
-            __syncwarp();
-            float4 fo;
-            fo.x = __shfl_xor_sync(FLOW_FULL, fs.x, 16); fo.y = __shfl_xor_sync(FLOW_FULL, fs.y, 16);
-            fo.z = __shfl_xor_sync(FLOW_FULL, fs.z, 16); fo.w = __shfl_xor_sync(FLOW_FULL, fs.w, 16);
-            // first half + second half, in that order on both lanes; lane half hh updates elements 2hh, 2hh+1 of the quad
-            const float f2[2] = {hh ? fo.z + fs.z : fs.x + fo.x, hh ? fo.w + fs.w : fs.y + fo.y};
-            float qn[2] = {0.f, 0.f};                                               // the lane's two new values (0 beyond n_q: padding)
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int e = e4 + 2 * hh + h, k = kq0 + 2 * hh + h;
-                if (!(qact && k < a.n_q)) continue;
-                const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
-                const double fd = (double)f2[h], rr = csm ? sr[e] : a.r[co], kvv = csm ? skv[e] : a.kv[co], kqq = csm ? skq[e] : a.kq[co];
-                double q = sq[e], v = sv[e];
-                if (a.traj) a.traj[((size_t)be * a.n_steps + n) * a.n_q + a.kperm[k]] = q;
-                if (n == 0 && a.auto_start)
-                    v = (rr != 0.0) ? a.astart[co] * q + a.half_T2 * fd : 0.0;
-                const double fe = a.fext ? (double)a.fext[(size_t)be * a.n_steps + n] * a.gain[(size_t)be * a.NQP + k] : 0.0;
-                v = kvv * v - kqq * q + rr * (fe - fd);
-                q += v;
-                sq[e] = q; sv[e] = v;
-                qn[h] = (float)q;
-            }
-            // publish the pair (k even, k + 1 < KP): one 8-byte fp32 store and one 4-byte store each for the bf16 hi and lo halves,
-            // which are adjacent in the operand layout
-            const int k0 = kq0 + 2 * hh;
-            if (qact && k0 < a.n_q) {
-                *reinterpret_cast<float2 *>(a.qf + (size_t)be * QS + k0) = make_float2(qn[0], qn[1]);
-                const uint32_t h0 = bf16_rn_dev(qn[0]), h1 = bf16_rn_dev(qn[1]);
-                const uint32_t l0 = bf16_rn_dev(qn[0] - __uint_as_float(h0 << 16)), l1 = bf16_rn_dev(qn[1] - __uint_as_float(h1 << 16));
-                const int k16 = k0 & 15;
-                const int off = (re >> 3) * 256 + (k16 >> 3) * 128 + (re & 7) * 16 + (k16 & 7) * 2;      // bytes, 4-aligned
-                unsigned char *Qc = reinterpret_cast<unsigned char *>(Qt + (size_t)(k0 >> 4) * 4096);
-                *reinterpret_cast<uint32_t *>(Qc + off) = h0 | (h1 << 16);
-                *reinterpret_cast<uint32_t *>(Qc + 4096 + off) = l0 | (l1 << 16);
-            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            mbar_arrive(smem_u32(C.bars + MB_ACCE + slot));                              // the accumulator slot may be overwritten
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP) = t_; }
         }
-        if (tmg) { const long long t_ = clock64(); tm[5] += t_ - tk; tk = t_; }
-        bar_named(2 + mt, 128);
-        if (r == 0) set_flag(a.qflag + ((size_t)mt * a.G + c) * MMA_FS, (unsigned)n + 2u);
-        if (tmg) { const long long t_ = clock64(); tm[6] += t_ - tk; tk = t_; }
     }
-    if (lane == 0)
-        for (int m = gw, b2 = c + gw * a.G; b2 < B; m += 4, b2 += 4 * a.G)
-            if (b2 / 128 == mt) a.first_bad[b2] = sbad[m];
 }
 
+// The two epilogue warpgroups.  Up to two tiles: warpgroup 0 runs phase 1 (q, epilogue 1, G send) and warpgroup 1 phase 2 (G
+// receive, epilogue 2) of every tile, so a tile's two TMEM passes overlap the other tile's.  More tiles: warpgroup w runs both phases
+// of the tiles t = w, w + 2, ... (measured on C3, us per step at batch 128 / 256 / 1024: split 11.7 / 13.5 / 41.5, per-tile 12.2 / 14.3 / 34.4).
+template <int NSP, bool TIMING>
+__device__ __forceinline__ void mma_epilogue_warpgroup(const MmaArgs &a, const MmaCta &C, const int w, const int r, const int lane_base)
+{
+    const bool tmg = TIMING && r == 0;
+    long long tm[7] = {0, 0, 0, 0, 0, 0, 0};               // phase cycles of tile 0, kept in registers (a global update per phase would add an L2 round trip to it)
+    if (a.MT <= 2) {
+        for (int n = 0; n < a.n_steps; ++n)
+            for (int t = 0; t < a.MT; ++t) {
+                if (w == 0) mma_epilogue_e1_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg, tm);
+                else mma_epilogue_e2_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg, tm);
+            }
+    } else {
+        for (int n = 0; n < a.n_steps; ++n)
+            for (int t = w; t < a.MT; t += 2) {
+                mma_epilogue_e1_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg && w == 0, tm);
+                mma_epilogue_e2_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg && w == 0, tm);
+            }
+    }
+    if (tmg && (a.MT <= 2 || w == 0)) {
+        if (a.MT > 2 || w == 0) { for (int x = 0; x < 3; ++x) a.timing[(size_t)C.c * 16 + x] = tm[x]; a.timing[(size_t)C.c * 16 + 5] = tm[5]; a.timing[(size_t)C.c * 16 + 6] = tm[6]; }
+        if (a.MT > 2 || w == 1) { a.timing[(size_t)C.c * 16 + 3] = tm[3]; a.timing[(size_t)C.c * 16 + 4] = tm[4]; }
+    }
+}
+
+
+// ------------------------------------------------------------------------------------------------------------
+// O: owners.  A team of TS warps handles the tiles t = team, team + NTEAM, ...: for every owned (row, quad of 4 k)
+// gathers the partial forces of all n groups (16-byte strong loads, all in flight, group order), applies the a5
+// linear update in fp64 delta form and republishes q.  LPQ lanes share a quad (each gathers a part of the groups).
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mma_publish(const MmaArgs &a, const MmaCta &C, int t, int re, int qd, int h0, int cnt, const float *qn)
+{
+    // qn[0..cnt): new values of elements 4*qd + h0 .. of row re in block j (cnt = 4, 2 or 1; h0 multiple of cnt)
+    float *qf = a.qf + ((((size_t)t * a.NKB + C.j) * a.RBQ + qd) * 128 + re) * 4 + h0;
+    const int kop = C.koff + 4 * qd + h0, k16 = kop & 15;
+    unsigned char *Qc = reinterpret_cast<unsigned char *>(a.Qop) + ((size_t)t * a.KC + (kop >> 4)) * 8192 +
+                        (re >> 3) * 256 + (k16 >> 3) * 128 + (re & 7) * 16 + (k16 & 7) * 2;
+    uint32_t hi[4], lo[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const float x = u < cnt ? qn[u] : 0.f;
+        hi[u] = bf16_rn_dev(x);
+        lo[u] = bf16_rn_dev(x - __uint_as_float(hi[u] << 16));
+    }
+    if (cnt == 4) {
+        *reinterpret_cast<float4 *>(qf) = make_float4(qn[0], qn[1], qn[2], qn[3]);
+        *reinterpret_cast<uint2 *>(Qc) = make_uint2(hi[0] | (hi[1] << 16), hi[2] | (hi[3] << 16));
+        *reinterpret_cast<uint2 *>(Qc + 4096) = make_uint2(lo[0] | (lo[1] << 16), lo[2] | (lo[3] << 16));
+    } else if (cnt == 2) {
+        *reinterpret_cast<float2 *>(qf) = make_float2(qn[0], qn[1]);
+        *reinterpret_cast<uint32_t *>(Qc) = hi[0] | (hi[1] << 16);
+        *reinterpret_cast<uint32_t *>(Qc + 4096) = lo[0] | (lo[1] << 16);
+    } else {
+        *qf = qn[0];
+        *reinterpret_cast<uint16_t *>(Qc) = (uint16_t)hi[0];
+        *reinterpret_cast<uint16_t *>(Qc + 4096) = (uint16_t)lo[0];
+    }
+}
+
+// Steps [n_begin, n_end) of an owner team.  EXTRAS: trajectory output, external force or the second-order start at n = 0 are
+// in use (a separate instance keeps their registers out of the common path).
+template <int LPQ, bool TIMING, bool EXTRAS>
+__device__ __forceinline__ void mma_owner_steps(const MmaArgs &a, const MmaCta &C, const int team, const int NTEAM, const int tl, const int TL,
+                                                const int n_begin, const int n_end, unsigned &it, long long (&tm)[4], long long &tmx)
+{
+    const int NGRP = a.NGRP, NKB = a.NKB, RBQ = a.RBQ, B = a.batch, MT = a.MT;
+    const int items = C.rows * C.RBQj;
+    constexpr int EPL = 4 / LPQ;
+    const int NH = (NGRP + LPQ - 1) / LPQ;
+    const size_t fstride = (size_t)NKB * RBQ * 512;
+    const bool tmg = TIMING && team == 0 && tl == 0;
+    for (int n = n_begin; n < n_end; ++n) {
+        const uint32_t tag = ((uint32_t)n + 1u) & 3u;
+        for (int t = team; t < MT; t += NTEAM, ++it) {
+            double *sq = C.sq + (size_t)t * C.nel, *sv = C.sv + (size_t)t * C.nel;
+            // the row leaders read pk after the team barrier of this tile-step; the buffer is written again two
+            // tile-steps later, i.e. after the barrier of the next one, which the readers reach after their reads
+            float2 *pk = C.pk + (size_t)(team * 2 + (it & 1u)) * a.rows_max * RBQ;
+            long long tk = tmg && t == 0 ? clock64() : 0;
+            for (int base = 0; base < items * LPQ; base += TL) {
+                const int idx = base + tl, item = idx / LPQ, sub = idx - item * LPQ;
+                const bool act = item < items;
+                const int rr = act ? item / C.RBQj : 0, qd = act ? item - rr * C.RBQj : 0, re = C.r0 + rr, be = t * 128 + re;
+                const bool live = act && be < B;
+                const int g0 = sub * NH, g1 = min(NGRP, g0 + NH);
+                const uint32_t *fq = a.fx + ((((size_t)t * NGRP) * NKB + C.j) * RBQ + qd) * 512 + (size_t)re * 4;
+                float4 fs = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int ii0 = g0; ii0 < g1; ii0 += MMA_GB) {                       // group order (deterministic)
+                    uint4 x[MMA_GB];
+                    const int cnt = min(MMA_GB, g1 - ii0);
+                    unsigned pend = live ? (1u << cnt) - 1u : 0u, spins = 0;
+                    while (pend) {
+#pragma unroll
+                        for (int u = 0; u < MMA_GB; ++u)
+                            if (pend >> u & 1) x[u] = ld_relaxed4(fq + (size_t)(ii0 + u) * fstride);
+#pragma unroll
+                        for (int u = 0; u < MMA_GB; ++u)
+                            if ((pend >> u & 1) && tags_ok(x[u], tag)) pend &= ~(1u << u);
+                        if (pend && (++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 21))) { *C.s_abort = 1; break; }
+                    }
+                    if (live) {
+#pragma unroll
+                        for (int u = 0; u < MMA_GB; ++u)
+                            if (u < cnt) { fs.x += untag(x[u].x); fs.y += untag(x[u].y); fs.z += untag(x[u].z); fs.w += untag(x[u].w); }
+                    }
+                }
+                if (tmg && t == 0 && base == 0) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; tmx += t_ - *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP); }
+                // join the parts of the group range (fp32 addition is commutative: every lane of the quad gets the same bits)
+                if (LPQ >= 2) {
+                    fs.x += __shfl_xor_sync(FLOW_FULL, fs.x, 1); fs.y += __shfl_xor_sync(FLOW_FULL, fs.y, 1);
+                    fs.z += __shfl_xor_sync(FLOW_FULL, fs.z, 1); fs.w += __shfl_xor_sync(FLOW_FULL, fs.w, 1);
+                }
+                if (LPQ >= 4) {
+                    fs.x += __shfl_xor_sync(FLOW_FULL, fs.x, 2); fs.y += __shfl_xor_sync(FLOW_FULL, fs.y, 2);
+                    fs.z += __shfl_xor_sync(FLOW_FULL, fs.z, 2); fs.w += __shfl_xor_sync(FLOW_FULL, fs.w, 2);
+                }
+                // a5 linear update of the lane's EPL elements (fp64, delta form).  Rows beyond the batch and the padding of the last
+                // quad carry zero state and zero coefficients, so they need no special case; the rare extras (trajectory output,
+                // external force, second-order start at n = 0) go through a separate uniform branch.
+                float qn[EPL], po = 0.f, pn = 0.f;
+                const int e0 = (rr * RBQ + qd) * 4 + sub * EPL;
+                const double *cf = reinterpret_cast<const double *>(C.coef + (size_t)t * C.nel * 28);
+                const float *cw = reinterpret_cast<const float *>(cf + 3 * C.nel);
+                double qv[EPL], vv[EPL], ckv[EPL], ckq[EPL], cr[EPL];
+#pragma unroll
+                for (int h = 0; h < EPL; ++h) {
+                    qv[h] = sq[e0 + h]; vv[h] = sv[e0 + h]; ckv[h] = cf[e0 + h]; ckq[h] = cf[C.nel + e0 + h]; cr[h] = cf[2 * C.nel + e0 + h];
+                }
+                constexpr bool extras = EXTRAS;
+#pragma unroll
+                for (int h = 0; h < EPL; ++h) {
+                    const int hq = sub * EPL + h;
+                    const double fd = (double)(hq == 0 ? fs.x : hq == 1 ? fs.y : hq == 2 ? fs.z : fs.w);
+                    double fe = 0.0;
+                    if (extras && live && 4 * qd + hq < C.nb) {
+                        const int k = C.k0 + 4 * qd + hq;
+                        const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
+                        if (a.traj) a.traj[((size_t)be * a.n_steps + n) * a.n_q + a.kperm[k]] = qv[h];
+                        if (n == 0 && a.auto_start) vv[h] = (cr[h] != 0.0) ? a.astart[co] * qv[h] + a.half_T2 * fd : 0.0;
+                        if (a.fext) fe = (double)a.fext[(size_t)be * a.n_steps + n] * a.gain[(size_t)be * a.NQP + k];
+                    }
+                    vv[h] = fma(ckv[h], vv[h], fma(-ckq[h], qv[h], cr[h] * (fe - fd)));
+                    qv[h] += vv[h];
+                    qn[h] = (float)qv[h];
+                    po = fmaf(cw[e0 + h], qn[h], po); pn = fmaf(qn[h], qn[h], pn);
+                }
+                if (act) {
+#pragma unroll
+                    for (int h = 0; h < EPL; ++h) { sq[e0 + h] = qv[h]; sv[e0 + h] = vv[h]; }
+                }
+                if (tmg && t == 0 && base == 0) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; }
+                if (live) mma_publish(a, C, t, re, qd, sub * EPL, EPL, qn);
+                if (LPQ >= 2) { po += __shfl_xor_sync(FLOW_FULL, po, 1); pn += __shfl_xor_sync(FLOW_FULL, pn, 1); }
+                if (LPQ >= 4) { po += __shfl_xor_sync(FLOW_FULL, po, 2); pn += __shfl_xor_sync(FLOW_FULL, pn, 2); }
+                if (act && sub == 0) pk[item] = make_float2(po, pn);
+            }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
+            bar_named(2 + team, TL);
+            if (tl == 0) {
+                if (C.j == 0) {            // warp W must have consumed the pickup partials of q^n before any owner may go on to q^{n+2}
+                    unsigned spins = 0;
+                    while (C.wdone[t] < n + 1) if ((++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 24))) { *C.s_abort = 1; break; }
+                }
+                set_flag(a.qflag + (((size_t)t * NKB + C.j) * NGRP + C.i) * MMA_FS, (unsigned)n + 2u);
+            }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP + 1) = t_; }
+            if (tl < C.rows) {                                 // pickup partial of q^{n+1} for row tl
+                float o = 0.f, nr = 0.f;
+                for (int qd = 0; qd < C.RBQj; ++qd) { const float2 x = pk[tl * C.RBQj + qd]; o += x.x; nr += x.y; }
+                unsigned long long *pp = a.px + ((((size_t)((n + 1) & 1) * MT + t) * NKB + C.j) * 128 + C.r0 + tl) * 2;
+                const unsigned long long ep = (unsigned long long)((unsigned)n + 2u) << 32;
+                const unsigned long long w0 = ep | __float_as_uint(o), w1 = ep | __float_as_uint(nr);
+                asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(pp), "l"(w0), "l"(w1) : "memory");
+            }
+        }
+    }
+}
+
+template <int LPQ, bool TIMING>
+__device__ __forceinline__ void mma_owner_team(const MmaArgs &a, const MmaCta &C, const int team, const int NTEAM, const int tl, const int TL)
+{
+    const int NGRP = a.NGRP, NKB = a.NKB, RBQ = a.RBQ, B = a.batch, MT = a.MT;
+    const int items = C.rows * C.RBQj;
+    constexpr int EPL = 4 / LPQ;                               // elements of a quad each of its lanes updates
+    const bool tmg = TIMING && team == 0 && tl == 0;
+    long long tm[4] = {0, 0, 0, 0};
+    long long tmf = 0;
+    unsigned it = 0;                                           // tile-steps this team has handled: pk buffer = it & 1
+    // ---- owner state, publish q^0 and its pickup partials ----
+    for (int t = team; t < MT; t += NTEAM, ++it) {
+        double *sq = C.sq + (size_t)t * C.nel, *sv = C.sv + (size_t)t * C.nel;
+        float2 *pk = C.pk + (size_t)(team * 2 + (it & 1u)) * a.rows_max * RBQ;
+        for (int base = 0; base < items * LPQ; base += TL) {
+            const int idx = base + tl, item = idx / LPQ, sub = idx - item * LPQ;
+            const bool act = item < items;
+            const int rr = act ? item / C.RBQj : 0, qd = act ? item - rr * C.RBQj : 0, re = C.r0 + rr, be = t * 128 + re;
+            float qn[EPL], po = 0.f, pn = 0.f;
+#pragma unroll
+            for (int h = 0; h < EPL; ++h) {
+                const int kk = 4 * qd + sub * EPL + h, k = C.k0 + kk, e = (rr * RBQ + qd) * 4 + sub * EPL + h;
+                double q = 0.0, v = 0.0, kvv = 0.0, kqq = 0.0, rc = 0.0; float wk = 0.f;
+                if (act && be < B && kk < C.nb) {
+                    q = a.q0[(size_t)be * a.NQP + k]; v = a.v0[(size_t)be * a.NQP + k];
+                    const size_t co = (size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k;
+                    kvv = a.kv[co]; kqq = a.kq[co]; rc = a.r[co]; wk = a.w[co];
+                }
+                if (act) {
+                    sq[e] = q; sv[e] = v;
+                    double *cf = reinterpret_cast<double *>(C.coef + (size_t)t * C.nel * 28);
+                    cf[e] = kvv; cf[C.nel + e] = kqq; cf[2 * C.nel + e] = rc;
+                    reinterpret_cast<float *>(cf + 3 * C.nel)[e] = wk;
+                }
+                qn[h] = (float)q;
+                if (act && be < B && kk < C.nb) {
+                    po = fmaf(a.w[(size_t)(a.coeff_stride_q ? be : 0) * a.NQP + k], qn[h], po); pn = fmaf(qn[h], qn[h], pn);
+                }
+            }
+            if (act) mma_publish(a, C, t, re, qd, sub * EPL, EPL, qn);
+            if (LPQ >= 2) { po += __shfl_xor_sync(FLOW_FULL, po, 1); pn += __shfl_xor_sync(FLOW_FULL, pn, 1); }
+            if (LPQ >= 4) { po += __shfl_xor_sync(FLOW_FULL, po, 2); pn += __shfl_xor_sync(FLOW_FULL, pn, 2); }
+            if (act && sub == 0) pk[item] = make_float2(po, pn);
+        }
+        bar_named(2 + team, TL);
+        if (tl == 0) set_flag(a.qflag + (((size_t)t * NKB + C.j) * NGRP + C.i) * MMA_FS, 1u);
+        if (tl < C.rows) {                                     // pickup partial of q^0 for row tl: buffer 0, epoch 1
+            float o = 0.f, nr = 0.f;
+            for (int qd = 0; qd < C.RBQj; ++qd) { const float2 x = pk[tl * C.RBQj + qd]; o += x.x; nr += x.y; }
+            unsigned long long *pp = a.px + (((size_t)t * NKB + C.j) * 128 + C.r0 + tl) * 2;
+            const unsigned long long w0 = (1ull << 32) | __float_as_uint(o), w1 = (1ull << 32) | __float_as_uint(nr);
+            asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1, %2};" ::"l"(pp), "l"(w0), "l"(w1) : "memory");
+        }
+    }
+
+    const bool extras = a.traj != nullptr || a.fext != nullptr;
+    if (extras) mma_owner_steps<LPQ, TIMING, true>(a, C, team, NTEAM, tl, TL, 0, a.n_steps, it, tm, tmf);
+    else {
+        if (a.auto_start) mma_owner_steps<LPQ, TIMING, true>(a, C, team, NTEAM, tl, TL, 0, min(1, a.n_steps), it, tm, tmf);
+        mma_owner_steps<LPQ, TIMING, false>(a, C, team, NTEAM, tl, TL, a.auto_start ? 1 : 0, a.n_steps, it, tm, tmf);
+    }
+    if (tmg) { for (int x = 0; x < 4; ++x) a.timing[(size_t)C.c * 16 + 8 + x] = tm[x]; a.timing[(size_t)C.c * 16 + 14] = tmf; }
+}
+
+// W: block-0 CTAs only.  out[b][n] = sum over the k blocks of the pickup partials of q^n (a1 pickup + a6 write-out); rows of this CTA.
+__device__ __forceinline__ void mma_pickup_warp(const MmaArgs &a, const MmaCta &C, const int lane)
+{
+    const int NKB = a.NKB, MT = a.MT, B = a.batch;
+    for (int n = 0; n < a.n_steps; ++n) {
+        for (int t = 0; t < MT; ++t) {
+            for (int rr = lane; rr < C.rows; rr += 32) {
+                const int re = C.r0 + rr, be = t * 128 + re;
+                if (be >= B) continue;
+                const unsigned long long *pp = a.px + ((((size_t)(n & 1) * MT + t) * NKB) * 128 + re) * 2;
+                float o = 0.f, nr = 0.f;
+                for (int j = 0; j < NKB; ++j) {                 // block order (deterministic)
+                    unsigned long long w0, w1;
+                    unsigned spins = 0;
+                    do {
+                        asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(pp + (size_t)j * 256) : "memory");
+                        if ((unsigned)(w0 >> 32) == (unsigned)n + 1u && (unsigned)(w1 >> 32) == (unsigned)n + 1u) break;
+                        if ((++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 21))) { *C.s_abort = 1; break; }
+                        __nanosleep(100);
+                    } while (true);
+                    o += __uint_as_float((unsigned)w0); nr += __uint_as_float((unsigned)w1);
+                }
+                a.out[(size_t)be * a.n_steps + n] = o;
+                int *sb = C.sbad + t * a.rows_max + rr;
+                if (*sb < 0 && !(isfinite(o) && isfinite(nr))) *sb = n;
+            }
+            __syncwarp();
+            if (lane == 0) C.wdone[t] = n + 1;
+        }
+    }
+    for (int t = 0; t < MT; ++t)
+        for (int rr = lane; rr < C.rows; rr += 32)
+            if (t * 128 + C.r0 + rr < B) a.first_bad[t * 128 + C.r0 + rr] = C.sbad[t * a.rows_max + rr];
+}
+
+template <bool TIMING>
 __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
 {
     extern __shared__ __align__(128) unsigned char mma_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int c = blockIdx.x, i = c / a.NKB, j = c - i * a.NKB;
-    const MmaSmem L = mma_smem_layout(a.slab_bytes, a.nel_max, a.NSTG);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(mma_smem + L.bars);      // indices MB_*
-    uint32_t *tptr = reinterpret_cast<uint32_t *>(bars + MB_TPTR);
-    volatile int *s_abort = reinterpret_cast<volatile int *>(bars + MB_ABORT);
-    double *own = reinterpret_cast<double *>(mma_smem + L.own);
-    int *sbad = reinterpret_cast<int *>(mma_smem + L.sbad);
-    unsigned char *cst = mma_smem + L.cst;
-    unsigned char *slab = mma_smem + L.slab, *ring = mma_smem + L.ring;
+    const MmaSmem L = mma_smem_layout(a.slab_bytes, a.MT, a.rows_max, a.RBQ, a.NSTG);
+    MmaCta C;
+    C.c = blockIdx.x; C.i = C.c / a.NKB; C.j = C.c - C.i * a.NKB;
+    C.bars = reinterpret_cast<uint64_t *>(mma_smem + L.bars);
+    uint32_t *tptr = reinterpret_cast<uint32_t *>(C.bars + MB_TPTR);
+    C.s_abort = reinterpret_cast<volatile int *>(C.bars + MB_ABORT);
+    int *tab = reinterpret_cast<int *>(mma_smem + L.bars + MMA_TAB_OFF);
+    C.kl = tab; C.nmode = tab + 64; C.fb = tab + 72; C.blk = tab + 88;
+    C.sq = reinterpret_cast<double *>(mma_smem + L.sq); C.sv = reinterpret_cast<double *>(mma_smem + L.sv);
+    C.coef = mma_smem + L.coef;
+    C.pk = reinterpret_cast<float2 *>(mma_smem + L.pk);
+    C.sbad = reinterpret_cast<int *>(mma_smem + L.sbad);
+    C.wdone = reinterpret_cast<volatile int *>(mma_smem + L.wdone);
+    C.slab = mma_smem + L.slab; C.ring = mma_smem + L.ring;
+    C.nel = (size_t)a.rows_max * a.RBQ * 4;
 
     if (tid == 0) {
-        for (int s = 0; s < a.NSTG; ++s) { mbar_init(smem_u32(bars + MB_FULL + s), 1); mbar_init(smem_u32(bars + MB_EMPTY + s), 1); }
-        for (int m = 0; m < 2; ++m) {
-            mbar_init(smem_u32(bars + MB_ACCF + m), 1); mbar_init(smem_u32(bars + MB_ACCE + m), 128); mbar_init(smem_u32(bars + MB_QRDY + m), 1);
-        }
-        *s_abort = 0;
+        for (int s = 0; s < a.NSTG; ++s) { mbar_init(smem_u32(C.bars + MB_FULL + s), 1); mbar_init(smem_u32(C.bars + MB_EMPTY + s), 1); }
+        for (int s = 0; s < 3; ++s) { mbar_init(smem_u32(C.bars + MB_ACCF + s), 1); mbar_init(smem_u32(C.bars + MB_ACCE + s), 128); }
+        for (int t = 0; t < MMA_MT_MAX; ++t) mbar_init(smem_u32(C.bars + MB_QRDY + t), 1);
+        *C.s_abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int x = tid; x < 256; x += blockDim.x) sbad[x] = -1;
-    if (tid < a.KC && tid < 64) reinterpret_cast<int *>(bars + MB_KLIST)[tid] = a.klist[(size_t)c * a.KC + tid];   // KC <= 64 (mma_layout)
+    for (int x = tid; x < a.MT * a.rows_max; x += blockDim.x) C.sbad[x] = -1;
+    if (tid < MMA_MT_MAX) C.wdone[tid] = 0;
+    if (tid < a.KCL && tid < 64) tab[tid] = a.klist[(size_t)C.c * a.KCL + tid];
+    if (tid < MMA_NG_MAX_DEV) tab[64 + tid] = tid < a.NG ? a.nlist[C.i * a.NG + tid] : -1;
+    if (tid < 16) tab[72 + tid] = a.fblk[(size_t)C.c * 16 + tid];
+    if (tid < 3 * a.NKB && tid < 48) tab[88 + tid] = a.blk[tid];
     {   // H slab of this CTA: loaded once, resident for the whole run
-        const uint4 *src = reinterpret_cast<const uint4 *>(a.slabs + (size_t)c * a.slab_bytes / 2);
-        uint4 *dst = reinterpret_cast<uint4 *>(slab);
+        const uint4 *src = reinterpret_cast<const uint4 *>(a.slabs + (size_t)C.c * a.slab_bytes / 2);
+        uint4 *dst = reinterpret_cast<uint4 *>(C.slab);
         for (int x = tid; x < a.slab_bytes / 16; x += blockDim.x) dst[x] = __ldg(src + x);
     }
     if (warp == 0) {
@@ -473,75 +744,101 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t tbase = *tptr;
-    const int MT = a.MT, KC = a.KC, NC = a.NC;
+    C.tbase = *tptr;
+    C.k0 = C.blk[3 * C.j]; C.nb = C.blk[3 * C.j + 1]; C.koff = C.blk[3 * C.j + 2]; C.RBQj = (C.nb + 3) >> 2;
+    C.NGa = 0;
+    for (int u = 0; u < a.NG; ++u) C.NGa += C.nmode[u] >= 0;
+    C.r0 = 128 * C.i / a.NGRP; C.rows = 128 * (C.i + 1) / a.NGRP - C.r0;
+    C.KCA = a.kcnt[C.c];
+    const int MT = a.MT, S = a.S, NSTG = a.NSTG;
+    const int kc0 = C.i % C.KCA;                    // the CTAs that read the same chunks (same k block, other n groups) start at different ones:
+                                                    // spreads the reads of one tile's operand over the L2 slices instead of hammering one chunk
 
-    const int KCA = a.kcnt[c];                     // K chunks with a non-zero slab part: the others are neither loaded nor multiplied
-    const int *kl = reinterpret_cast<const int *>(bars + MB_KLIST);      // this CTA's chunk list, copied to shared memory above
-    const int kc0 = c % KCA;                       // the chunks are walked from a per-CTA offset: spreads the q reads over the L2 slices
-    if (warp >= 4) {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
-        const int mt = (warp - 4) >> 2, gw = warp & 3;
-        if (mt < MT)
-            mma_epilogue_group(a, mt, c, i, j, (warp & 3) * 32 + lane, bars, own + (size_t)mt * (mma_own_bytes(a.nel_max) / 8) * a.nel_max,
-                               tbase, s_abort, (warp & 3) * 32, sbad, gw, lane, reinterpret_cast<float *>(cst) + (tid - 128));
+    if (warp >= 8) {
+        // ---------------- E: epilogue groups ----------------------------------------------------------
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 176;");
+        const int r = (warp & 3) * 32 + lane;
+        if (a.RBT <= 32) mma_epilogue_warpgroup<1, TIMING>(a, C, (warp - 8) >> 2, r, (warp & 3) * 32);
+        else mma_epilogue_warpgroup<2, TIMING>(a, C, (warp - 8) >> 2, r, (warp & 3) * 32);
+    } else if (warp >= 4) {
+        // ---------------- O: owner teams ----------------------------------------------------------------
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 128;");
+        const int NTEAM = MT >= 2 ? 2 : 1, TS = 4 / NTEAM;
+        const int ow = warp - 4, team = ow / TS, tl = (ow - team * TS) * 32 + lane;
+        if (a.LPQ == 1) mma_owner_team<1, TIMING>(a, C, team, NTEAM, tl, TS * 32);
+        else if (a.LPQ == 2) mma_owner_team<2, TIMING>(a, C, team, NTEAM, tl, TS * 32);
+        else mma_owner_team<4, TIMING>(a, C, team, NTEAM, tl, TS * 32);
     } else {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
-    // Warps 0 / 2 are the producers of tile 0 / 1, warps 1 / 3 the MMA issuers: the two tiles are independent pipelines
-    // (own half of the ring stages when both tiles are in use), so a late q^n of one tile never holds up the other.
-    const int mt = warp >> 1;
-    const int NSH = MT > 1 ? a.NSTG / 2 : a.NSTG;
-    if (mt < MT && (warp & 1) == 0) {
-        // ---------------- producer: wait for q^n of the tile, stream it through the ring by TMA ----------
-        int stage = 0; unsigned ph = 0;
-        for (int n = 0; n < a.n_steps; ++n) {
-            poll_flags(a.qflag + (size_t)mt * a.G * MMA_FS, lane, a.G, (unsigned)n + 1u, s_abort);
-            __syncwarp();
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
+        if (warp == 0) {
+            // ---------------- P: wait for q^n of the tile's source blocks, stream its K chunks by TMA ----
+            unsigned cnt = 0;                                   // chunks issued so far: stage = cnt % NSTG
+            const int fcnt = a.fcnt[C.c];
+            const bool tmg = TIMING && lane == 0;
+            long long tmp = 0, tmq = 0;
+            for (int n = 0; n < a.n_steps; ++n)
+                for (int t = 0; t < MT; ++t) {
+                    const long long tk = tmg && t == 0 ? clock64() : 0;
+                    poll_flag_list(a.qflag + (size_t)t * a.NKB * a.NGRP * MMA_FS, C.fb, fcnt, a.NGRP, lane, (unsigned)n + 1u, C.s_abort);
+                    __syncwarp();
+                    if (tmg && t == 0) { const long long t_ = clock64(); tmp += t_ - tk; if (n > 0) tmq += t_ - *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP + 1); }
+                    if (lane == 0) {
+                        mbar_arrive(smem_u32(C.bars + MB_QRDY + t));
+                        asm volatile("fence.proxy.async.global;" ::: "memory");
+                        for (int xx = 0; xx < C.KCA; ++xx, ++cnt) {
+                            const int x = xx + kc0 < C.KCA ? xx + kc0 : xx + kc0 - C.KCA;     // walk the chunks from a per-CTA offset
+                            const unsigned sg = cnt % (unsigned)NSTG, ph = (cnt / (unsigned)NSTG) & 1u;
+                            mbar_wait(smem_u32(C.bars + MB_EMPTY + sg), ph ^ 1u, C.s_abort);
+                            mbar_expect_tx(smem_u32(C.bars + MB_FULL + sg), 8192);
+                            tma_bulk_g2s(smem_u32(C.ring + sg * 8192), a.Qop + ((size_t)t * a.KC + C.kl[x]) * 4096, 8192,
+                                         smem_u32(C.bars + MB_FULL + sg));
+                        }
+                    }
+                    __syncwarp();
+                }
+            if (tmg) { a.timing[(size_t)C.c * 16 + 12] = tmp; a.timing[(size_t)C.c * 16 + 15] = tmq; }
+        } else if (warp == 1) {
+            // ---------------- M: one thread issues the MMAs of every tile, in order ------------------------
             if (lane == 0) {
-                mbar_arrive(smem_u32(bars + MB_QRDY + mt));
-                asm volatile("fence.proxy.async.global;" ::: "memory");
-                for (int kx = 0; kx < KCA; ++kx) {
-                    const int kc = kl[kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA];
-                    const int sg = NSH * mt + stage;
-                    mbar_wait(smem_u32(bars + MB_EMPTY + sg), ph ^ 1, s_abort);
-                    mbar_expect_tx(smem_u32(bars + MB_FULL + sg), 8192);
-                    tma_bulk_g2s(smem_u32(ring + sg * 8192), a.Qg + ((size_t)mt * KC + kc) * 4096, 8192, smem_u32(bars + MB_FULL + sg));
-                    if (++stage == NSH) { stage = 0; ph ^= 1; }
-                }
+                const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(a.NC >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+                unsigned cnt = 0, uses[3] = {0u, 0u, 0u};
+                const bool tmg = TIMING;
+                long long tmm = 0;
+                for (int n = 0; n < a.n_steps; ++n)
+                    for (int t = 0; t < MT; ++t) {
+                        const int slot = t % S;
+                        const unsigned use = slot == 0 ? uses[0]++ : slot == 1 ? uses[1]++ : uses[2]++;
+                        if (use > 0) mbar_wait(smem_u32(C.bars + MB_ACCE + slot), (use - 1u) & 1u, C.s_abort);   // the slot's last tile left it
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        const uint32_t td = C.tbase + (uint32_t)(slot * a.NC);
+                        long long tk = 0;
+                        for (int xx = 0; xx < C.KCA; ++xx, ++cnt) {
+                            const int x = xx + kc0 < C.KCA ? xx + kc0 : xx + kc0 - C.KCA;     // position in the list = position in the slab
+                            const unsigned sg = cnt % (unsigned)NSTG, ph = (cnt / (unsigned)NSTG) & 1u;
+                            mbar_wait(smem_u32(C.bars + MB_FULL + sg), ph, C.s_abort);
+                            if (tmg && t == 0 && xx == 0) tk = clock64();
+                            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                            const uint32_t qa = smem_u32(C.ring + sg * 8192), hb = smem_u32(C.slab + (size_t)x * 2 * a.NC * 32);
+                            const uint64_t qhi = umma_desc(qa), qlo = umma_desc(qa + 4096);
+                            const uint64_t hhi = umma_desc(hb), hlo = umma_desc(hb + a.NC * 32);
+                            umma_bf16(td, qhi, hhi, idesc, xx > 0);
+                            umma_bf16(td, qlo, hhi, idesc, 1);
+                            umma_bf16(td, qhi, hlo, idesc, 1);
+                            umma_commit(smem_u32(C.bars + MB_EMPTY + sg));                          // ring slot free when these MMAs retire
+                        }
+                        umma_commit(smem_u32(C.bars + MB_ACCF + slot));                             // t of this tile complete
+                        if (tmg && t == 0) tmm += clock64() - tk;
+                    }
+                if (tmg) a.timing[(size_t)C.c * 16 + 13] = tmm;
             }
-            __syncwarp();
+        } else if (warp == 2 && C.j == 0) {
+            mma_pickup_warp(a, C, lane);
         }
-    } else if (mt < MT) {
-        // ---------------- MMA issuer: one thread per tile ------------------------------------------------
-        if (lane == 0) {
-            const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NC >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            int stage = 0; unsigned ph = 0;
-            const uint32_t td = tbase + (uint32_t)(mt * NC);
-            for (int n = 0; n < a.n_steps; ++n) {
-                mbar_wait(smem_u32(bars + MB_ACCE + mt), (n & 1) ^ 1, s_abort);         // epilogues of step n-1 left the tile
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                for (int kx = 0; kx < KCA; ++kx) {
-                    const int kp = kx + kc0 < KCA ? kx + kc0 : kx + kc0 - KCA;          // position in the list = position in the slab
-                    const int sg = NSH * mt + stage;
-                    mbar_wait(smem_u32(bars + MB_FULL + sg), ph, s_abort);
-                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const uint32_t qa = smem_u32(ring + sg * 8192), hb = smem_u32(slab + (size_t)kp * 2 * NC * 32);
-                    const uint64_t qhi = umma_desc(qa), qlo = umma_desc(qa + 4096);
-                    const uint64_t hhi = umma_desc(hb), hlo = umma_desc(hb + NC * 32);
-                    umma_bf16(td, qhi, hhi, idesc, kx > 0);
-                    umma_bf16(td, qlo, hhi, idesc, 1);
-                    umma_bf16(td, qhi, hlo, idesc, 1);
-                    umma_commit(smem_u32(bars + MB_EMPTY + sg));                              // ring slot free when these MMAs retire
-                    if (++stage == NSH) { stage = 0; ph ^= 1; }
-                }
-                umma_commit(smem_u32(bars + MB_ACCF + mt));                                // t of tile mt complete
-            }
-        }
-    }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tbase), "r"(512));
+    if (tid == 0 && *C.s_abort) *a.timeout_flag = 1;
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(C.tbase), "r"(512));
 }
 
 }  // namespace modal_dev

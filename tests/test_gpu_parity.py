@@ -35,11 +35,13 @@ def gpu_run(plan, q0, qm1, n_steps, want_traj=False, fext=None, fext_gain=None):
     return out.cpu().numpy().astype(np.float64), fb, (None if traj is None else traj.cpu().numpy()), st
 
 
-def plan_with_oracle_inputs(wl, case, scheme=0, lossless=False):
+def plan_with_oracle_inputs(wl, case, scheme=0, lossless=False, options=None):
     """Plan whose coefficient arrays are the oracle's (fp32-rounded where the device stores fp32),
     so that the comparison measures arithmetic, not input quantisation."""
     torch, mb = _mods()
     plan = mb.Plan(mb.desc_from_workload(wl, scheme=scheme, lossless=lossless), 0)
+    for k, v in (options or {}).items():
+        plan.set_option(k, v)
     B = case.q0.shape[0]
     # pickup: the oracle's w is already masked; the library masks again (same rule)
     if case.model == orc.VK:
@@ -166,14 +168,11 @@ def _small_vk_workload(n_q, n_phi, batch, n_steps, seed=11):
     (1, 1, 2, 0, 0, -1),           # degenerate: single mode (Duffing)
     (130, 3, 1, 40, 4, 2),         # long tile rows cut into several units, shared by many CTAs, streamed
 ])
-def test_vk_flow_team_shapes_parity(n_q, n_phi, batch, G, NS, RES, monkeypatch):
-    if G: monkeypatch.setenv("MODAL_FLOW_G", str(G))
-    if NS: monkeypatch.setenv("MODAL_FLOW_NS", str(NS))
-    if RES >= 0: monkeypatch.setenv("MODAL_FLOW_RES", str(RES))
+def test_vk_flow_team_shapes_parity(n_q, n_phi, batch, G, NS, RES):
     wl = _small_vk_workload(n_q, n_phi, batch, 1500)
     case = orc.assemble(wl)
     ref = orc.run_case(case, 1500)
-    plan = plan_with_oracle_inputs(wl, case)
+    plan = plan_with_oracle_inputs(wl, case, options=dict(flow_g=G, flow_ns=NS, flow_res=RES))
     gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, 1500)
     assert st == 0 and np.all(fb == -1)
     check_parity(gpu, ref["out"], case)
@@ -192,14 +191,13 @@ def test_vk_flow_team_shapes_parity(n_q, n_phi, batch, G, NS, RES, monkeypatch):
     (100, 50, 256, 400),           # two full M tiles, C2 shape
     (16, 1, 3, 800),               # one k block, one in-plane mode
 ])
-def test_vk_mma_tensor_core_parity(n_q, n_phi, batch, n_steps, monkeypatch):
+def test_vk_mma_tensor_core_parity(n_q, n_phi, batch, n_steps):
     """Batched step on tcgen05 (bf16 hi/lo split, 3 MMAs) against the fp64 oracle."""
-    monkeypatch.setenv("MODAL_VK_IMPL", "mma")
     wl = _small_vk_workload(n_q, n_phi, batch, n_steps)
     sub = list(range(batch)) if batch <= 8 else sorted(set(np.linspace(0, batch - 1, 12).astype(int).tolist()))
     case_all = orc.assemble(wl)
     ref = orc.run_case(orc.assemble(wl, samples=sub), n_steps)
-    plan = plan_with_oracle_inputs(wl, case_all)
+    plan = plan_with_oracle_inputs(wl, case_all, options=dict(vk_impl=2))
     gpu, fb, _, st = gpu_run(plan, case_all.q0, case_all.qm1, n_steps)
     torch, mb = _mods()
     assert plan.query(mb.Q_KERNEL_INFO)[0] == 4
@@ -210,10 +208,9 @@ def test_vk_mma_tensor_core_parity(n_q, n_phi, batch, n_steps, monkeypatch):
     assert np.array_equal(gpu, gpu2)
 
 
-def test_vk_mma_ftm_fext_traj(monkeypatch):
+def test_vk_mma_ftm_fext_traj():
     """Tensor-core kernel with the FTM coefficients, device-side second-order start, an external force signal
     and the trajectory output; lossless energy of the weakly non-linear samples tracks the oracle's."""
-    monkeypatch.setenv("MODAL_VK_IMPL", "mma")
     torch, mb = _mods()
     n_steps, batch = 1200, 9
     wl = _small_vk_workload(37, 13, batch, n_steps)
@@ -224,7 +221,7 @@ def test_vk_mma_ftm_fext_traj(monkeypatch):
     gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
     ref = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, case.q0, case.qm1, n_steps, nl_scale=case.nl_scale,
                        H=case.H, fext=orc.f32(fext), fext_gain=gain, want_traj=True)
-    plan = plan_with_oracle_inputs(wl, case, scheme=1)
+    plan = plan_with_oracle_inputs(wl, case, scheme=1, options=dict(vk_impl=2))
     gpu, fb, traj, st = gpu_run(plan, case.q0, None, n_steps, want_traj=True, fext=fext, fext_gain=gain)
     assert plan.query(mb.Q_KERNEL_INFO)[0] == 4 and st == 0 and np.all(fb == -1)
     check_parity(gpu, ref["out"], case)
@@ -234,8 +231,9 @@ def test_vk_mma_ftm_fext_traj(monkeypatch):
     wl2["A"] = 0.3 * wl2["h"]
     c2 = orc.assemble(wl2, lossless=True)
     r2 = orc.run_case(c2, 3000, want_traj=True)
-    p2 = plan_with_oracle_inputs(wl2, c2, lossless=True)
+    p2 = plan_with_oracle_inputs(wl2, c2, lossless=True, options=dict(vk_impl=2))
     _, _, tr2, _ = gpu_run(p2, c2.q0, c2.qm1, 3000, want_traj=True)
+    assert p2.query(mb.Q_KERNEL_INFO)[0] == 4
     for b in range(3):
         e_ref = orc.energy(orc.VK, c2.T, c2.omega[b], r2["traj"][b], nl_scale=c2.nl_scale[b], H=c2.H)
         e_gpu = orc.energy(orc.VK, c2.T, c2.omega[b], tr2[b], nl_scale=c2.nl_scale[b], H=c2.H)
@@ -244,15 +242,17 @@ def test_vk_mma_ftm_fext_traj(monkeypatch):
         assert np.max(np.abs(e_gpu - e_ref)) / e_ref.mean() <= TOL_E
 
 
-def test_vk_mma_batch_beyond_one_launch(monkeypatch):
-    """More than 256 samples: the library splits the batch into launches of two M tiles."""
-    monkeypatch.setenv("MODAL_VK_IMPL", "mma")
+def test_vk_mma_three_tiles_in_one_launch():
+    """More than 256 samples: three M tiles (the last one ragged) time-multiplexed through the accumulator slots
+    of ONE persistent launch."""
     wl = _small_vk_workload(16, 4, 300, 200)
     case = orc.assemble(wl)
     sub = [0, 127, 128, 255, 256, 299]
     ref = orc.run_case(orc.assemble(wl, samples=sub), 200)
-    plan = plan_with_oracle_inputs(wl, case)
+    plan = plan_with_oracle_inputs(wl, case, options=dict(vk_impl=2))
     gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, 200)
+    torch, mb = _mods()
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 4
     assert st == 0 and np.all(fb == -1)
     check_parity(gpu[sub], ref["out"], orc.assemble(wl, samples=sub), first=200)
 
