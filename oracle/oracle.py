@@ -365,9 +365,17 @@ def f32(x):
     return np.asarray(x, np.float64).astype(np.float32).astype(np.float64)
 
 
-def scheme_coeffs(scheme, omega, gamma, T):
+def scheme_coeffs(scheme, omega, gamma, T, active=None):
+    """(c1, c2, c3) of q+ = c1 q + c2 q- + c3 (fext - f): SV (g, p, r) or FTM (-a1, -a2, b1) (reading R7).
+    The FTM coefficients exist for underdamped modes only ("overdamped mode -> error naming
+    the mode"): an active mode with omega <= gamma is refused."""
     if scheme == SV:
         return sv_coeffs(omega, gamma, T)
+    bad = np.asarray(omega) <= np.asarray(gamma)
+    if active is not None:
+        bad = bad & np.asarray(active, bool)
+    if np.any(bad):
+        raise ValueError(f"FTM scheme: mode {int(np.argmax(bad))} is critically damped or overdamped (omega <= gamma)")
     a1, a2, b1 = ftm_coeffs(omega, gamma, T)
     return -a1, -a2, b1
 
@@ -424,7 +432,7 @@ def assemble(wl: dict, samples=None, *, scheme=SV, lossless=False, round_fp32=Tr
             w = rnd(np.where(act, w, 0.0))
             q0 = project_bump_rect(mq, nq, Lx, Ly, wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
             q0 = np.where(act, q0, 0.0)
-            c1, c2, c3 = scheme_coeffs(scheme, om, ga, T)
+            c1, c2, c3 = scheme_coeffs(scheme, om, ga, T, act)
             c3 = np.where(act, c3, 0.0)
             qm1 = np.where(act, start_state(VK, q0, om, T, nl_scale=s, H=H), 0.0)
             for k, v in zip(rows, (om, ga, act, c1, c2, c3, w, lam, s, q0, qm1)):
@@ -448,7 +456,7 @@ def assemble(wl: dict, samples=None, *, scheme=SV, lossless=False, round_fp32=Tr
             w = rnd(np.where(act, w, 0.0))
             q0 = project_bump_rect(mq, nq, Lx, Ly, wl["x0"][b], wl["y0"][b], wl["W"][b], wl["A"][b])
             q0 = np.where(act, q0, 0.0)
-            c1, c2, c3 = scheme_coeffs(scheme, om, ga, T)
+            c1, c2, c3 = scheme_coeffs(scheme, om, ga, T, act)
             c3 = np.where(act, c3, 0.0)
             qm1 = np.where(act, start_state(TENSION, q0, om, T, lam=lam_r, nl_scale=c), 0.0)
             for k, v in zip(rows, (om, ga, act, c1, c2, c3, w, lam_r, c, q0, qm1)):
@@ -469,7 +477,7 @@ def assemble(wl: dict, samples=None, *, scheme=SV, lossless=False, round_fp32=Tr
             w = np.array([string_mode(m, L, xp) for m in range(1, Nq + 1)])
             w = rnd(np.where(act, w, 0.0))
             q0 = np.where(act, project_bump_string(Nq, L, wl["x0"][b], wl["W"][b], wl["A"][b]), 0.0)
-            c1, c2, c3 = scheme_coeffs(scheme, om, ga, T)
+            c1, c2, c3 = scheme_coeffs(scheme, om, ga, T, act)
             c3 = np.where(act, c3, 0.0)
             qm1 = np.where(act, start_state(model, q0, om, T, lam=lam_r, nl_scale=c), 0.0)
             for k, v in zip(rows, (om, ga, act, c1, c2, c3, w, lam_r, c, q0, qm1)):

@@ -125,6 +125,10 @@ def by_name(name: str, **kw):
 def shard(wl: dict, rank: int, world: int) -> dict:
     """Batch shard for rank ``rank`` of ``world`` (independent samples, no data-path collective)."""
     B = wl["batch"]
+    if not 0 <= rank < world:
+        raise ValueError(f"rank {rank} outside [0, {world})")
+    if B < world:
+        raise ValueError(f"batch {B} < world size {world}: a rank would get no sample (run replicas instead)")
     lo, hi = (B * rank) // world, (B * (rank + 1)) // world
     out = {}
     for k, v in wl.items():

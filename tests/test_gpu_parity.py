@@ -89,6 +89,44 @@ def check_parity(gpu, ref, case, weak_only_l2=True, first=4096, ref_bad=None, gp
         assert np.all(np.isfinite(gpu[b]))
 
 
+GOLD_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def load_golden(name, wl):
+    """Long oracle runs stored by tests/golden/make_oracle_goldens.py (which calls only oracle/).  The oracle's inputs
+    for the stored samples are re-derived here and compared, so a stale file fails instead of checking old inputs."""
+    g = np.load(os.path.join(GOLD_DIR, f"oracle_{name}.npz"))
+    sub = g["sub"].tolist()
+    case = orc.assemble(wl, samples=sub)
+    for key, arr in (("q0", case.q0), ("omega", case.omega), ("nl_scale", case.nl_scale)):
+        assert np.allclose(arr, g[key], rtol=1e-12, atol=0.0), f"golden {name} is stale ({key})"
+    return g, sub, case
+
+
+def rms_envelope(x, win=1024):
+    n = x.shape[-1] // win
+    return np.sqrt(np.mean(x[..., :n * win].reshape(*x.shape[:-1], n, win) ** 2, axis=-1))
+
+
+def check_window_parity(gpu, ref, case, first=4096):
+    """BASELINE.json's tolerances over their full windows: max error <= 1e-4 of the peak over the first 4096 samples and
+    relative L2 <= 1e-3 over the whole stored run for the weakly non-linear samples (R15); strongly non-linear samples:
+    the first 256 samples point-wise and the RMS envelope in 1024-sample windows within 5 %."""
+    for x in range(ref.shape[0]):
+        peak = np.max(np.abs(ref[x]))
+        weak = nl_ratio(case, x) <= 0.05
+        k = min(first if weak else 256, ref.shape[1])
+        e_max = np.max(np.abs(gpu[x, :k] - ref[x, :k])) / peak
+        assert e_max <= TOL_MAX, (x, e_max, weak)
+        if weak:
+            e_l2 = np.linalg.norm(gpu[x] - ref[x]) / np.linalg.norm(ref[x])
+            assert e_l2 <= TOL_L2, (x, e_l2)
+        elif ref.shape[1] >= 1024:
+            er, eg = rms_envelope(ref[x]), rms_envelope(gpu[x])
+            assert np.max(np.abs(eg - er) / er) <= 0.05, (x, np.max(np.abs(eg - er) / er))
+        assert np.all(np.isfinite(gpu[x]))
+
+
 # ------------------------------------------------------------------ C0 -----------
 def test_c0_full_run_parity():
     wl = wlmod.c0()
@@ -257,27 +295,6 @@ def test_vk_mma_three_tiles_in_one_launch():
     check_parity(gpu[sub], ref["out"], orc.assemble(wl, samples=sub), first=200)
 
 
-def test_c3_full_shape_tensor_core_short_run():
-    """C3 at its full size (200 + 100 modes, 256 geometries) in the launch configuration bench.py times,
-    checked on 16 samples spanning the amplitude range (the oracle needs ~6 s per sample here, one
-    sample per host core)."""
-    n_steps = 768
-    wl = wlmod.c3(n_steps=n_steps)
-    order = np.argsort(wl["A"] / wl["h"])
-    sub = sorted(set(order[np.linspace(0, 255, 16).astype(int)].tolist()))
-    torch, mb = _mods()
-    plan, q0 = mb.plan_from_workload(wl, 0)
-    gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
-    info = plan.query(mb.Q_KERNEL_INFO)
-    assert info[0] == 4 and info[1] > 100                    # tensor-core kernel on > 100 SMs
-    sub_case = orc.assemble(wl, samples=sub)
-    ref = orc.run_case(sub_case, n_steps)
-    ok = ref["first_bad"] < 0
-    assert np.all(fb[np.array(sub)][ok] == -1)
-    check_parity(gpu[sub][ok], ref["out"][ok], orc.assemble(wl, samples=[s_ for s_, o in zip(sub, ok) if o]), first=n_steps)
-    assert np.all(np.isfinite(gpu[fb < 0]))
-
-
 def test_c2_full_config_parity():
     """C2 exactly as bench.py times it (100 + 50 modes, batch 1, all 44 100 steps, the plan's own coefficient
     derivation): the paper's 100-mode benchmark point.  The oracle needs ~45 s here."""
@@ -329,24 +346,82 @@ def test_c4_shape_batch_teams_side_by_side():
     check_parity(gpu, ref["out"], case, first=64)
 
 
-@pytest.mark.parametrize("batch", [16, 64])
-def test_c4_bench_batches_sampled(batch):
-    """C4 at the batches of the sweep (16, 64) in the launch configuration bench.py times (the plan's own derivation,
-    teams side by side), checked on four samples spanning the amplitude range; every sample finite."""
-    n_steps = 48
-    wl = wlmod.c4(batch=batch, n_steps=n_steps)
-    order = np.argsort(wl["A"])
-    sub = sorted(set(order[np.linspace(0, batch - 1, 4).astype(int)].tolist()))
+def test_c3_tolerance_window_and_full_run():
+    """C3 as bench.py times it (256 geometries x 22 050 steps, the plan's own derivation, ONE launch of the batched
+    tcgen05 kernel) against stored oracle runs: 16 samples spanning 0.1 ... 5 thicknesses over the first 4096 samples,
+    four of them over all 22 050 steps (the split-bf16 error growth over the full run is what this
+    checks).  The whole batch must stay finite and bit-reproducible."""
+    wl = wlmod.c3()
+    g, sub, case = load_golden("c3", wl)
     torch, mb = _mods()
     plan, q0 = mb.plan_from_workload(wl, 0)
-    gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
+    gpu, fb, _, st = gpu_run(plan, q0, None, wl["n_steps"])
     info = plan.query(mb.Q_KERNEL_INFO)
-    assert info[0] == 3 and info[2] >= 2 and st == 0 and np.all(fb == -1)
-    sub_case = orc.assemble(wl, samples=sub)
-    ref = orc.run_case(sub_case, n_steps)
-    assert np.all(ref["first_bad"] < 0)
-    check_parity(gpu[sub], ref["out"], sub_case, first=n_steps)
+    assert info[0] == 4 and info[1] > 100 and st == 0 and np.all(fb == -1) and np.all(g["first_bad"] == -1)
+    check_window_parity(gpu[sub][:, :4096], g["out"], case)
+    full = g["sub_full"].tolist()
+    assert np.all(g["first_bad_full"] == -1)
+    check_window_parity(gpu[full], g["out_full"], orc.assemble(wl, samples=full))
+    amp = (wl["A"] / wl["h"])[sub]
+    assert amp.min() < 0.15 and amp.max() > 4.5                  # the stored samples span linear ... strongly non-linear
     assert np.all(np.isfinite(gpu))
+    gpu2, _, _, _ = gpu_run(plan, q0, None, 2048)
+    assert np.array_equal(gpu2, gpu[:, :2048])                   # deterministic exchange order (ADVICE round 1)
+
+
+def test_c4_b1_full_run():
+    """C4 batch 1 (400 + 200 modes, whole-GPU team of the FP32 flow kernel) over all 4410 steps against the stored oracle run."""
+    wl = wlmod.c4(batch=1)
+    g, sub, case = load_golden("c4_b1", wl)
+    torch, mb = _mods()
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    gpu, fb, _, st = gpu_run(plan, q0, None, wl["n_steps"])
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 3 and info[1] >= 100 and st == 0 and fb[0] == -1 and g["first_bad"][0] == -1
+    check_window_parity(gpu[sub], g["out"], case)
+
+
+@pytest.mark.parametrize("batch", [16, 64])
+def test_c4_batches_tolerance_window(batch):
+    """C4 at the batches of the sweep in the launch configuration bench.py times, four samples spanning the amplitude range
+    over all 4410 steps (>= the 4096-sample window) against stored oracle runs; every sample finite."""
+    wl = wlmod.c4(batch=batch)
+    g, sub, case = load_golden(f"c4_b{batch}", wl)
+    torch, mb = _mods()
+    plan, q0 = mb.plan_from_workload(wl, 0)
+    gpu, fb, _, st = gpu_run(plan, q0, None, wl["n_steps"])
+    assert st == 0 and np.all(fb == -1) and np.all(g["first_bad"] == -1)
+    check_window_parity(gpu[sub], g["out"], case)
+    assert np.all(np.isfinite(gpu))
+
+
+def test_vk_flow_kernel_with_external_force():
+    """The FP32 flow kernel with an external force signal (raised-cosine strike in time) and the second-order start on
+    the device, on a team of several CTAs and on a single CTA."""
+    n_steps, batch = 1500, 3
+    wl = _small_vk_workload(37, 13, batch, n_steps)
+    case = orc.assemble(wl)
+    rng = np.random.default_rng(9)
+    fext = np.zeros((batch, n_steps)); t = np.arange(48)
+    fext[:, 30:78] = 0.5 * (1 - np.cos(2 * np.pi * t / 48))[None] * rng.uniform(0.5, 2.0, (batch, 1))
+    gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
+    ref = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, case.q0, case.qm1, n_steps, nl_scale=case.nl_scale,
+                       H=case.H, fext=orc.f32(fext), fext_gain=gain)
+    torch, mb = _mods()
+    for G in (4, 1):
+        plan = plan_with_oracle_inputs(wl, case, options=dict(vk_impl=1, flow_g=G))
+        gpu, fb, _, st = gpu_run(plan, case.q0, None, n_steps, fext=fext, fext_gain=gain)
+        info = plan.query(mb.Q_KERNEL_INFO)
+        assert info[0] == 3 and info[1] == G and st == 0 and np.all(fb == -1)
+        check_parity(gpu, ref["out"], case)
+    # zero initial state: the response is the forced one only
+    z = np.zeros_like(case.q0)
+    ref0 = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, z, z, n_steps, nl_scale=case.nl_scale,
+                        H=case.H, fext=orc.f32(fext), fext_gain=gain)
+    plan = plan_with_oracle_inputs(wl, case, options=dict(vk_impl=1))
+    gpu, _, _, _ = gpu_run(plan, z, z, n_steps, fext=fext, fext_gain=gain)
+    peak = np.abs(ref0["out"]).max(axis=1)
+    assert np.all(peak > 0) and np.all(np.max(np.abs(gpu - ref0["out"]), axis=1) <= TOL_MAX * peak)
 
 
 # ------------------------------------------------------------------ tension / linear ----

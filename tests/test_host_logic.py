@@ -195,3 +195,73 @@ def test_parity_grouped_modes_leave_whole_tiles_empty_and_queries_stay_in_plan_o
     assert np.max(np.abs(plan.query(mb.Q_H_FULL) - D)) <= 1e-6 * np.max(np.abs(D))
     total2, nz2 = plan.query(mb.Q_TILE_STATS)
     assert total2 == total and nz2 == total
+
+
+def test_ftm_plan_refuses_overdamped_mode_naming_it():
+    """FTM with omega <= sigma must be an error that names the mode, not NaN
+    coefficients; SV proceeds; the oracle applies the same rule (test_ftm_refuses_overdamped_modes)."""
+    wl, plan = _c0_plan()
+    om = plan.query(mb.Q_OMEGA)[0].copy(); sg = plan.query(mb.Q_SIGMA)[0].copy()
+    sg[3] = om[3] * 1.5
+    plan.coeffs_upload(1, omega=om, sigma=sg)                      # SV: accepted
+    d = mb.desc_from_workload(wl, scheme=mb.FTM)
+    pf = mb.Plan(d, device=-1)
+    with pytest.raises(mb.ModalError) as e:
+        pf.coeffs_upload(1, omega=om, sigma=sg)
+    assert e.value.status == mb.EINVAL and "mode 3" in e.value.message and "overdamped" in e.value.message
+    sg[3] = om[3]                                                   # critically damped: refused as well
+    with pytest.raises(mb.ModalError):
+        pf.coeffs_upload(1, omega=om, sigma=sg)
+
+
+def test_options_api_validates_keys_and_ranges():
+    wl, plan = _c0_plan()
+    plan.set_option("vk_impl", 2); plan.set_option("flow_g", 4); plan.set_option("timing", 0)
+    for key, val in (("vk_impl", 3), ("flow_ns", 99), ("nonsense", 1)):
+        with pytest.raises(mb.ModalError) as e:
+            plan.set_option(key, val)
+        assert e.value.status == mb.EINVAL
+    # parity_order re-packs H in the new internal order: the tensor seen through the API does not change
+    H1 = plan.query(mb.Q_H_FULL)
+    t1 = plan.query(mb.Q_TILE_STATS)
+    plan.set_option("parity_order", 0)
+    assert np.array_equal(plan.query(mb.Q_H_FULL), H1)
+    plan.set_option("parity_order", 1)
+    assert np.array_equal(plan.query(mb.Q_H_FULL), H1) and np.array_equal(plan.query(mb.Q_TILE_STATS), t1)
+
+
+@pytest.mark.parametrize("n_q,n_phi,opts", [(200, 100, {}), (200, 100, dict(mma_split=1)), (37, 13, {}), (16, 1, {}), (1, 1, {}),
+                                            (100, 50, dict(parity_order=0))])
+def test_batched_kernel_layout_covers_H_exactly_once(n_q, n_phi, opts):
+    """Host side of the tcgen05 kernel: the operand slabs of all CTAs together hold every non-zero H^n[k][r] exactly once,
+    as bf16 hi + lo within 2^-16 of the fp32 value; class-aligned k blocks give every CTA of the sine-basis plate the same
+    number of K chunks."""
+    wl = wlmod.c3(batch=4, n_steps=8)
+    wl["n_q"], wl["n_phi"] = n_q, n_phi
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    for k, v in opts.items():
+        plan.set_option(k, v)
+    L = plan.query(mb.Q_MMA_LAYOUT)
+    assert L[0] == 1, L
+    fits, NKB, NGRP, NG, NC, S, RBT, RBQ, KC, KCL, G, rows_max, kmin, kmax = L[:14]
+    assert G == NKB * NGRP <= 148 and NC == NG * RBT <= 256 and 1 <= S <= 3 and S * NC <= 512 and RBT in (32, 64)
+    covered, nonzero, err = plan.query(mb.Q_MMA_SLAB_CHECK)
+    H = plan.query(mb.Q_H_FULL)
+    assert covered == nonzero == np.count_nonzero(H)
+    assert err <= 2.0 ** -16
+    if n_q == 200 and not opts:
+        assert kmin == kmax == 4 and KC == 16            # four parity classes of <= 64 modes: every CTA multiplies one class
+
+
+def test_batched_kernel_layout_dense_uploaded_H():
+    """An uploaded H without the parity zeros (the paper's H-fitting case): every K chunk is listed."""
+    wl = wlmod.c3(batch=4, n_steps=8)
+    wl["n_q"], wl["n_phi"] = 48, 12
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    rng = np.random.default_rng(1)
+    H = rng.normal(size=(12, 48, 48)); H = H + H.transpose(0, 2, 1)
+    plan.coeffs_upload(1, H_full=H)
+    L = plan.query(mb.Q_MMA_LAYOUT)
+    covered, nonzero, err = plan.query(mb.Q_MMA_SLAB_CHECK)
+    assert L[0] == 1 and L[12] == L[13] == L[8]          # fewest == most K chunks == all chunks
+    assert covered == nonzero == 12 * 48 * 48 and err <= 2.0 ** -16

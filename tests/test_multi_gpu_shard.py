@@ -52,6 +52,8 @@ def test_batch_shards_cover_the_batch_once():
         assert p["batch"] == hi - lo and np.array_equal(p["L"], wl["L"][lo:hi]) and p["n_q"] == wl["n_q"]
         seen += list(range(lo, hi))
     assert seen == list(range(10))
+    with pytest.raises(ValueError):                       # fewer samples than ranks: an empty shard would be refused by the plan
+        wlmod.shard(wlmod.c1(batch=2, n_steps=8), 0, 3)
 
 
 def test_two_ranks_gloo_sharded_derivation_matches_single_rank():

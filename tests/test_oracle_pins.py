@@ -430,3 +430,76 @@ def test_plate_bump_projection_reconstructs_peak_and_is_quadrature_independent()
         phi = 2 / np.sqrt(Lx * Ly) * np.sin(m[k] * np.pi * X / Lx) * np.sin(n[k] * np.pi * Y / Ly)
         brute = np.sum(np.outer(wg, wg) * w0 * phi) * 0.25 * W * W
         assert abs(brute - q[k]) < 1e-6 * abs(q[0])
+
+
+# ---------------------------------------------- glue of assemble(): mask rule and geometry fold ----
+def test_geometry_fold_of_assemble_equals_own_geometry_tensor():
+    """Reading R14 / SURVEY.md C18: assemble() keeps ONE tensor H_ref and folds (c_b / c_ref)^2 into s_n[b].
+    Pin: the force from (H_ref, folded s) equals the force from the sample's OWN tensor, H_closed on its own
+    (Lx, Ly) at a DIFFERENT aspect ratio with the same index sets, and the plain scale E / (2 rho zeta_b^4)."""
+    wl = dict(name="fold", model="vk", n_q=14, n_phi=9, n_steps=8, batch=3, sample_rate=44100.0,
+              ref=dict(Lx=0.6, Ly=0.45, h=1e-3), T0=0.0, sigma0=0.5, sigma1=1e-3, pickup=(0.43, 0.37),
+              E=2.0e11, rho=7860.0, nu=0.3,
+              Lx=np.array([0.47, 0.8, 0.6]), Ly=np.array([0.47 * 0.52, 0.8 * 0.97, 0.45]), h=np.array([0.7e-3, 1.9e-3, 1e-3]),
+              A=np.array([1e-3, 1e-3, 1e-3]), W=np.array([0.1, 0.15, 0.1]), x0=np.array([0.2, 0.3, 0.3]), y0=np.array([0.12, 0.4, 0.2]))
+    case = orc.assemble(wl, round_fp32=False)
+    mq, nq, mphi, nphi = (case.extra[k] for k in ("mq", "nq", "mphi", "nphi"))
+    rng = np.random.default_rng(3)
+    for b in range(3):
+        Lx, Ly = wl["Lx"][b], wl["Ly"][b]
+        H_own = orc.H_closed(Lx, Ly, mq, nq, mphi, nphi)
+        s_own = wl["E"] / (2.0 * wl["rho"] * orc.rect_lambda(mphi, nphi, Lx, Ly) ** 2)
+        q = rng.normal(size=14) * 1e-3
+        f_fold = orc.vk_force(case.H, case.nl_scale[b], q)
+        f_own = orc.vk_force(H_own, s_own, q)
+        assert np.allclose(f_fold, f_own, rtol=1e-11, atol=1e-14 * np.abs(f_own).max()), b
+    # the two off-reference samples really have another aspect ratio (the pin would be vacuous otherwise)
+    assert abs(wl["Ly"][0] / wl["Lx"][0] - 0.75) > 0.2 and abs(wl["Ly"][1] / wl["Lx"][1] - 0.75) > 0.2
+
+
+def test_mask_rule_sv_keeps_what_the_scheme_carries():
+    """Reading R11 / SURVEY.md C12: SV needs omega T < 2.  A lossless linear mode at omega T = 1.89 stays bounded
+    over 1e5 steps, at omega T = 2.01 it diverges; active_mask keeps the first and drops the second."""
+    T = 1.0 / 44100.0
+    for wT, bounded in [(1.89, True), (2.01, False)]:
+        om = np.array([wT / T]); ga = np.zeros(1)
+        g, p, r = orc.sv_coeffs(om, ga, T)
+        q0 = np.array([[1.0]]); qm1 = np.array([[1.0]])
+        res = orc.simulate(orc.LINEAR, g, p, r, np.ones(1), q0, qm1, 100000)
+        peak = np.nanmax(np.abs(res["out"]))
+        assert (np.isfinite(peak) and peak < 20.0) == bounded, (wT, peak)
+        assert bool(orc.active_mask(orc.SV, om, ga, T)[0]) == bounded
+    assert orc.active_mask(orc.SV, np.array([1.8999 / T, 1.9 / T]), np.zeros(2), T).tolist() == [True, False]
+
+
+def test_mask_rule_ftm_stops_short_of_the_aliasing_limit():
+    """FTM is exact at the samples for any damped frequency, so its limit is aliasing, not stability: the sampled
+    response of a mode at w~ T = 1.06 pi is indistinguishable from that of 0.94 pi.  active_mask keeps w~ < 0.95 pi / T."""
+    T = 1.0 / 44100.0
+    ga = np.array([3.0])
+    def response(wt_T):
+        wt = wt_T * np.pi / T
+        om = np.sqrt(wt ** 2 + ga ** 2)
+        a1, a2, b1 = orc.ftm_coeffs(om, ga, T)
+        q0 = np.array([[1.0]])
+        qm1 = np.array([[np.exp(ga[0] * T) * (np.cos(wt * T) - ga[0] / wt * np.sin(wt * T))]])      # exact q(-T)
+        return om, orc.simulate(orc.LINEAR, -a1, -a2, b1, np.ones(1), q0, qm1, 4000)["out"][0]
+    om_lo, lo = response(0.94)
+    om_hi, hi = response(1.06)
+    n = np.arange(4000)
+    exact = np.exp(-ga[0] * n * T) * (np.cos(0.94 * np.pi * n) + ga[0] / (0.94 * np.pi / T) * np.sin(0.94 * np.pi * n))
+    assert np.max(np.abs(lo - exact)) < 1e-9                       # the kept mode is reproduced exactly
+    assert np.max(np.abs(hi - lo)) < 2e-3                          # the aliased one cannot be told apart from it
+    assert orc.active_mask(orc.FTM, om_lo, ga, T)[0] and not orc.active_mask(orc.FTM, om_hi, ga, T)[0]
+    w = lambda x: np.sqrt((x * np.pi / T) ** 2 + ga ** 2)
+    assert orc.active_mask(orc.FTM, w(0.9499), ga, T)[0] and not orc.active_mask(orc.FTM, w(0.9501), ga, T)[0]
+
+
+def test_ftm_refuses_overdamped_modes():
+    """the FTM coefficients need underdamped modes; an active overdamped mode is an error naming it."""
+    T = 1.0 / 44100.0
+    om = np.array([2000.0, 50.0, 3000.0]); ga = np.array([1.0, 60.0, 2.0])
+    with pytest.raises(ValueError, match="mode 1"):
+        orc.scheme_coeffs(orc.FTM, om, ga, T, np.ones(3, bool))
+    orc.scheme_coeffs(orc.FTM, om, ga, T, np.array([True, False, True]))     # a masked mode is not asked for coefficients
+    orc.scheme_coeffs(orc.SV, om, ga, T)                                      # SV proceeds (SPEC.md:270)
