@@ -7,10 +7,14 @@ modal_simulate call advancing every sample of the workload through all its time 
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c0|c1|c2|c3] [--batch B]
   python bench.py --impl reference ...      # the fp64 oracle on the host cores (bounded sample)
+  python bench.py --peaks                   # only the machine peaks measured through libmodal.so
 
-value    = sample-steps per second (batch x time steps / s), inputs resident in HBM
-e2e      = same metric through modal_simulate_host: host q0 in, host audio out
-roofline = dominant kernel against its bound (algorithmic bytes or flops per launch / CUDA-event time)
+value     = sample-steps per second (batch x time steps / s), inputs resident in HBM
+e2e       = same metric through modal_simulate_host: host q0 in, host audio out
+roofline  = dominant kernel against its bound (algorithmic bytes or flops per launch / CUDA-event time)
+secondary = every other BASELINE.json configuration (and C4 batch 1 with a dense uploaded H), device-timed
+peaks     = FP32 / FP64 FMA, L2 / HBM / shared-memory / TMEM read bandwidth and exchange-hop latencies measured
+            in this run by modal_measure_peaks (csrc/peaks.cuh)
 """
 from __future__ import annotations
 
@@ -31,13 +35,11 @@ from paper_2505_05940_b200 import workloads as wlmod  # noqa: E402
 
 METRIC = "von_karman_modal_sample_steps_per_s"
 UNIT = "sample-steps/s"
-# nominal FP32 pipe: 148 SMs x 128 FMA lanes x 2 flop x 1.965 GHz (guide: B200_PROFILING.md clocks)
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum of one C4 batch-1 launch (4410 steps), profiles/r1_c4_b1.md
-C4_DRAM_BYTES_PER_LAUNCH = 21.12e6
+# nominal FP32 pipe, used only if modal_measure_peaks is skipped: 148 SMs x 128 FMA lanes x 2 flop x 1.965 GHz
+FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
 
-def peaks():
+def driver_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
@@ -63,42 +65,6 @@ def algorithmic_work(wl):
     return 12 * nq, 0
 
 
-def tensor_roofline(wl, B, n_steps, per_launch, bf16_peak, peak_src):
-    """vk_mma_kernel: algorithmic flops (F_alg per sample-step) against the measured bf16 peak.
-    The kernel issues three bf16 MMAs per algorithmic MAC (hi*hi + lo*hi + hi*lo) to meet the 1e-4 tolerance."""
-    flops, _ = algorithmic_work(wl)
-    ach = flops * B * n_steps / per_launch / 1e12
-    return {"bound": "tensor", "achieved": ach, "peak": bf16_peak, "unit": "TFLOP/s", "frac": ach / bf16_peak, "traffic": None,
-            "peak_source": peak_src + " bf16 sustained", "kernel": "vk_mma_kernel",
-            "note": "achieved = F_alg (2 N_phi N_q^2 + ...) x batch x steps / time; the tensor pipe executes 3x that "
-                    "(split-bf16), so frac x 3 is the pipe's own utilisation on useful MACs"}
-
-
-def secondary_c3(mb, torch, steps=2, warmup=1):
-    """C3 (batch 256, tensor-core kernel), device-timed only: reported beside the headline workload."""
-    wl = wlmod.by_name("c3")
-    B, n_steps = wl["batch"], wl["n_steps"]
-    plan, q0 = mb.plan_from_workload(wl, torch.cuda.current_device())
-    out = torch.empty((B, n_steps), dtype=torch.float32, device="cuda")
-    stream = torch.cuda.current_stream().cuda_stream
-    for _ in range(warmup):
-        plan.simulate(q0, n_steps, out.data_ptr(), first_bad=False, stream=stream)
-    torch.cuda.synchronize()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-    for s_, e_ in ev:
-        s_.record(); plan.simulate(q0, n_steps, out.data_ptr(), first_bad=False, stream=stream); e_.record()
-    torch.cuda.synchronize()
-    per_launch = sum(s_.elapsed_time(e_) for s_, e_ in ev) * 1e-3 / steps
-    info = plan.query(mb.Q_KERNEL_INFO)
-    _, src, bf16_peak = peaks()
-    res = {"workload": wl["name"], "value": B * n_steps / per_launch, "unit": UNIT, "us_per_time_step": 1e6 * per_launch / n_steps,
-           "mode_steps_per_s": B * n_steps * wl["n_q"] / per_launch, "kernel_family": int(info[0]), "ctas": int(info[1])}
-    if int(info[0]) == 4:
-        res["roofline"] = tensor_roofline(wl, B, n_steps, per_launch, bf16_peak, src)
-    plan.close()
-    return res
-
-
 class ClockSampler(threading.Thread):
     def __init__(self, index=0):
         super().__init__(daemon=True)
@@ -117,14 +83,113 @@ class ClockSampler(threading.Thread):
                 pass
             time.sleep(0.1)
 
-    def summary(self):
-        if not self.rows:
+    def mark(self):
+        return len(self.rows)
+
+    def summary(self, lo=0, hi=None):
+        rows = self.rows[lo:hi]
+        if not rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
-        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        sm = sorted(int(r[0]) for r in rows if r[0].isdigit())
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i].lower().startswith("active") for r in self.rows)]
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": int(self.rows[0][1]) if self.rows[0][1].isdigit() else None,
-                "reasons": reasons, "samples": len(self.rows)}
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": int(rows[0][1]) if rows[0][1].isdigit() else None,
+                "reasons": reasons, "samples": len(rows)}
+
+
+def device_time(torch, plan, q0, n_steps, out, steps, warmup, flush=None):
+    """Seconds per modal_simulate launch: CUDA events on the launching stream, after warm-up, optional L2 flush between launches."""
+    stream = torch.cuda.current_stream().cuda_stream
+    for _ in range(max(warmup, 1)):
+        plan.simulate(q0, n_steps, out.data_ptr(), first_bad=False, stream=stream)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for s, e in ev:
+        if flush is not None:
+            flush.zero_()
+        s.record()
+        plan.simulate(q0, n_steps, out.data_ptr(), first_bad=False, stream=stream)
+        e.record()
+    torch.cuda.synchronize()
+    return sum(s.elapsed_time(e) for s, e in ev) * 1e-3 / steps
+
+
+def roofline_for(wl, B, n_steps, per_launch, info, tile_stats, pk):
+    """Roofline object of one workload: which kernel ran, what bounds it, algorithmic work / time against the measured peak."""
+    flops, hbytes = algorithmic_work(wl)
+    hbm_peak, peak_src, bf16_peak = driver_peaks()
+    fam = int(info[0])
+    if fam == 4:
+        ach = flops * B * n_steps / per_launch / 1e12
+        return {"bound": "tensor", "achieved": ach, "peak": bf16_peak, "unit": "TFLOP/s", "frac": ach / bf16_peak, "traffic": None,
+                "peak_source": peak_src + " bf16 sustained", "kernel": "vk_mma_kernel",
+                "note": "achieved = F_alg (2 N_phi N_q^2 + ...) x batch x steps / time; the kernel issues 3 bf16 MMAs per MAC (split hi/lo) "
+                        "on the K chunks that hold non-zeros only"}
+    if fam == 3:
+        ach = hbytes * n_steps / per_launch / 1e9
+        tiles, nz = tile_stats
+        read = nz * 1024 * n_steps / per_launch / 1e9
+        return {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
+                "peak_source": peak_src, "kernel": "vk_flow_kernel", "frac_dense_alg": ach / hbm_peak,
+                "tiles": tiles, "tiles_nonzero": nz, "achieved_read": read, "frac_read": read / hbm_peak,
+                "l2_read_peak_64mb": pk.get("l2_read_gbs_64mb") if pk else None,
+                "frac_read_of_l2": read / pk["l2_read_gbs_64mb"] if pk else None}
+    # tension / linear kernel: every FMA of the update is fp64 (DFMA), so the bound is the FP64 pipe
+    ach = flops * B * n_steps / per_launch / 1e12
+    peak = pk["fp64_tflops"] if pk else FP32_NOMINAL_TFLOPS
+    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+            "peak_source": "measured in this run (modal_measure_peaks, FP64 FMA)" if pk else "nominal FP32 pipe (peaks skipped)",
+            "kernel": "tension_kernel", "frac_of_fp32_pipe": ach / pk["fp32_tflops"] if pk else None}
+
+
+def run_secondary(mb, torch, sampler, pk, steps=2, warmup=1):
+    """Every other configuration of BASELINE.json plus C4 batch 1 with a dense uploaded H, device-timed."""
+    res = []
+    dev = torch.cuda.current_device()
+
+    def entry(label, wl, plan, q0, B, n_steps, extra=None):
+        out = torch.empty((B, n_steps), dtype=torch.float32, device="cuda")
+        lo = sampler.mark()
+        t = device_time(torch, plan, q0[:B], n_steps, out, steps, warmup)
+        info = plan.query(mb.Q_KERNEL_INFO)
+        ts = tuple(int(x) for x in plan.query(mb.Q_TILE_STATS)) if wl["model"] == "vk" else (0, 0)
+        st, _ = plan.check()
+        e = {"workload": label, "batch": B, "time_steps": n_steps, "value": B * n_steps / t, "unit": UNIT,
+             "us_per_time_step": 1e6 * t / n_steps, "mode_steps_per_s": B * n_steps * wl["n_q"] / t,
+             "realtime_factor_per_sample": (n_steps / wl["sample_rate"]) / t,
+             "kernel_family": int(info[0]), "ctas": int(info[1]) * (int(info[2]) if int(info[0]) == 3 else 1),
+             "status": int(st), "roofline": roofline_for(wl, B, n_steps, t, info, ts, pk), "clocks": sampler.summary(lo)}
+        if extra:
+            e.update(extra)
+        res.append(e)
+        del out
+
+    for name in ("c0", "c1", "c2"):
+        wl = wlmod.by_name(name)
+        plan, q0 = mb.plan_from_workload(wl, dev)
+        entry(wl["name"], wl, plan, q0, wl["batch"], wl["n_steps"])
+        plan.close()
+    for B in (256, 512, 1024):                              # north_star: tensor-pipe fraction "at batch >= 256"
+        wl = wlmod.c3(batch=B)
+        plan, q0 = mb.plan_from_workload(wl, dev)
+        entry(wl["name"], wl, plan, q0, B, wl["n_steps"])
+        plan.close()
+    best = max((e for e in res if e["workload"].startswith("c3_")), key=lambda e: e["roofline"]["frac"])
+    best["best_c3_batch"] = True
+    wl = wlmod.c4(batch=64)
+    plan, q0 = mb.plan_from_workload(wl, dev)
+    for B in (16, 64):
+        entry(f"c4_vk_400x200_b{B}", wl, plan, q0, B, wl["n_steps"])
+    # C4 batch 1 with a DENSE uploaded tensor (no exact zeros): the paper's H-fitting case (PAPER.md:283-285) -- nothing to skip
+    rng = np.random.default_rng(20250505)
+    H = rng.normal(size=(wl["n_phi"], wl["n_q"], wl["n_q"]))
+    H = H + H.transpose(0, 2, 1)
+    plan.coeffs_upload(1, H_full=H)
+    del H
+    entry("c4_vk_400x200_b1_dense_uploaded_H", wl, plan, q0, 1, wl["n_steps"],
+          {"note": "random symmetric H without zeros uploaded through modal_coeffs_upload: every tile is read, frac = dense-schedule fraction"})
+    plan.close()
+    return res
 
 
 def run_reference(args):
@@ -175,7 +240,7 @@ def cpu_baseline(wl, seconds=12.0):
     t0 = time.perf_counter()
     orc.run_case(case, n_s)
     dt = time.perf_counter() - t0
-    return {"value": sb * n_s / dt, "unit": UNIT, "cores": min(cores, sb), "kind": "oracle",
+    return {"value": sb * n_s / dt, "unit": UNIT, "cores": min(cores, sb), "kind": "oracle (1-core fp64 loop per sample; OpenMP over samples only)",
             "sample": f"{sb} of {B} samples x {n_s} of {n_full} time steps, {dt:.1f} s wall"}
 
 
@@ -188,8 +253,12 @@ def main():
     ap.add_argument("--workload", default="c4", choices=["c0", "c1", "c2", "c3", "c4"])
     ap.add_argument("--batch", type=int, default=0)
     ap.add_argument("--n-steps", dest="n_steps", type=int, default=0, help="time steps per simulate call (default: the config's)")
+    ap.add_argument("--option", action="append", default=[], help="plan option key=value (modal_plan_set_option), repeatable")
+    ap.add_argument("--dense-h", action="store_true", help="upload a dense random symmetric H (no parity zeros) before timing")
+    ap.add_argument("--peaks", action="store_true", help="measure and print the machine peaks only")
+    ap.add_argument("--no-peaks", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-secondary", action="store_true", help="skip the C3 (batch 256, tensor-core) line reported beside the headline")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the other configurations reported beside the headline")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -203,6 +272,9 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
+    if args.peaks:
+        print(json.dumps({"peaks": mb.measure_peaks(local)}), flush=True)
+        return
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
@@ -210,14 +282,16 @@ def main():
     # (rank r draws its excitation from the same recipe; no data-path collective).
     wl = make_workload(args.workload, args.batch, args.n_steps)
     B, n_steps = wl["batch"], wl["n_steps"]
-    plan, q0 = mb.plan_from_workload(wl, local)
+    options = {k: int(v) for k, v in (o.split("=") for o in args.option)}
+    plan, q0 = mb.plan_from_workload(wl, local, options=options)
+    if args.dense_h:
+        rng = np.random.default_rng(20250505)
+        H = rng.normal(size=(wl["n_phi"], wl["n_q"], wl["n_q"]))
+        plan.coeffs_upload(1, H_full=H + H.transpose(0, 2, 1))
+        del H
     out = torch.empty((B, n_steps), dtype=torch.float32, device="cuda")
     out_host = np.empty((B, n_steps), np.float32)
-    stream = torch.cuda.current_stream().cuda_stream
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")   # 256 MiB > 126 MB L2
-
-    def step_device():
-        plan.simulate(q0, n_steps, out.data_ptr(), first_bad=False, stream=stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -225,19 +299,13 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 1)):
-        step_device()
+    device_time(torch, plan, q0, n_steps, out, 1, max(args.warmup, 3) - 1)            # warm-up (>= 3 launches with the timed helper's own)
     barrier()
     sampler = ClockSampler(local); sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for s, e in ev:
-        flush.zero_()                         # flush L2 between timed iterations
-        s.record()
-        step_device()
-        e.record()
+    t_dev = device_time(torch, plan, q0, n_steps, out, args.steps, 1, flush) * args.steps
     barrier()
-    sampler.stop_flag = True
-    t_dev = sum(s.elapsed_time(e) for s, e in ev) * 1e-3
+    head_clocks = sampler.summary()
+    st_check, _ = plan.check()                           # one checked completion: a timed-out exchange or an instability is reported, not hidden
     # e2e: host buffers through the C ABI, H2D of the state and D2H of the audio inside the timed region
     plan.simulate_host(q0, n_steps, out=out_host)
     barrier()
@@ -252,47 +320,44 @@ def main():
     t_dev, t_e2e = tt.tolist()
     if rank == 0:
         info = plan.query(mb.Q_KERNEL_INFO)
-        flops, hbytes = algorithmic_work(wl)
+        ts = tuple(int(x) for x in plan.query(mb.Q_TILE_STATS)) if wl["model"] == "vk" else (0, 0)
+        pk = None if (args.no_peaks or world > 1) else mb.measure_peaks(local)
         units = world * B * n_steps * args.steps
         value = units / t_dev
         per_launch = t_dev / args.steps
-        hbm_peak, peak_src, bf16_peak = peaks()
-        if wl["model"] == "vk" and int(info[0]) == 4:
-            roof = tensor_roofline(wl, B, n_steps, per_launch, bf16_peak, peak_src)
-        elif wl["model"] == "vk":
-            ach = hbytes * n_steps / per_launch / 1e9
-            tiles, nz = (int(x) for x in plan.query(mb.Q_TILE_STATS))
-            read = nz * 1024 * n_steps / per_launch / 1e9
-            roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
-                    "traffic": C4_DRAM_BYTES_PER_LAUNCH if (wl["name"], n_steps) == ("c4_vk_400x200_b1", 4410) else None,
-                    "peak_source": peak_src, "kernel": "vk_flow_kernel",
-                    "tiles": tiles, "tiles_nonzero": nz, "achieved_read": read, "frac_read": read / hbm_peak,
-                    "note": "achieved = ALGORITHMIC bytes (SURVEY.md 8(d): the dense packed tensor, 4*n_phi*n_q(n_q+1)/2 per time step, "
-                            "once per step for the whole batch) / time.  The kernel keeps the modes grouped by index parity and never "
-                            "reads the 16x16 tiles that hold only parity zeros (tiles_nonzero of tiles, SURVEY.md 8(f) row 4), so it can "
-                            "exceed the dense-traffic roofline; achieved_read / frac_read count the bytes it does read per step (most "
-                            "of them from shared memory, where they stay resident).  traffic = dram read+write bytes of one launch "
-                            "(profiles/r1_c4_b1.md): H crosses the HBM pins once per launch"}
-        else:
-            ach = flops * B * n_steps / per_launch / 1e12
-            roof = {"bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP32_PEAK_TFLOPS,
-                    "traffic": None, "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz", "kernel": "tension_kernel"}
+        roof = roofline_for(wl, B, n_steps, per_launch, info, ts, pk)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": 1e3 * per_launch, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f32 force / f64 state", "data": "synthetic",
-                "config": {"workload": wl["name"], "n_q": wl["n_q"], "n_phi": wl["n_phi"], "batch": B, "time_steps": n_steps,
+                "dtype": "f32 force / f64 state" if int(info[0]) != 4 else "bf16 hi+lo operands, f32 accumulate / f64 state", "data": "synthetic",
+                "config": {"workload": wl["name"] + ("_dense_uploaded_H" if args.dense_h else ""), "n_q": wl["n_q"], "n_phi": wl["n_phi"],
+                           "batch": B, "time_steps": n_steps,
                            "sample_rate": wl["sample_rate"], "l2": "flushed between timed iterations (256 MiB write)",
-                           "kernel": {"family": int(info[0]), "cluster_size": int(info[1]), "clusters": int(info[2]),
+                           "kernel": {"family": int(info[0]), "ctas_per_team_or_ctas": int(info[1]), "teams_or_groups": int(info[2]),
                                       "threads": int(info[3]), "smem_bytes": int(info[4]), "resident": bool(info[5] & 1),
                                       "grid_team": bool(info[5] & 2)}},
                 "mode_steps_per_s": value * wl["n_q"],
                 "realtime_factor_per_sample": (n_steps / wl["sample_rate"]) / per_launch,
-                "us_per_time_step": 1e6 * per_launch / n_steps,
+                "us_per_time_step": 1e6 * per_launch / n_steps, "status_checked": int(st_check),
                 "e2e": {"value": units / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(2 * q0.size * 8),
                         "d2h_bytes_per_step": int(out_host.nbytes + 4 * B)},
-                "gpu_launches": args.steps, "clocks": sampler.summary(), "roofline": roof}
-        if not args.no_secondary and world == 1 and args.workload == "c4" and not args.batch and not args.n_steps:
-            line["secondary"] = secondary_c3(mb, torch)
+                "gpu_launches": args.steps, "clocks": head_clocks, "roofline": roof}
+        if pk:
+            line["peaks"] = pk
+        default_run = world == 1 and args.workload == "c4" and not args.batch and not args.n_steps and not args.dense_h and not options
+        if not args.no_secondary and default_run:
+            plan.close()
+            del out, flush
+            line["secondary"] = run_secondary(mb, torch, sampler, pk)
+            dense = next(e for e in line["secondary"] if e["workload"].endswith("dense_uploaded_H"))
+            roof["dense_schedule"] = {"us_per_time_step": dense["us_per_time_step"], "achieved": dense["roofline"]["achieved"],
+                                      "frac": dense["roofline"]["frac"]}
+            roof["note"] = ("frac = frac_dense_alg = ALGORITHMIC bytes (SURVEY.md 8(d): the dense packed tensor, 4 n_phi n_q (n_q+1)/2 per time step) "
+                            "/ time / measured HBM copy peak.  The sine-basis tensor is 69 % exact zeros by index parity; the kernel never reads the "
+                            "all-zero 16x16 tiles (tiles_nonzero of tiles, SURVEY.md 8(f) row 4) and keeps most of the rest in shared memory, so this "
+                            "figure can exceed 1 and is NOT a bandwidth achievement: the step is bound by its two exchange hops (DESIGN.md 7.1).  "
+                            "frac_read counts the bytes actually read; dense_schedule is the same kernel on an uploaded H without zeros, where "
+                            "every tile is read each step -- the figure to hold against north_star's 60 % for a general H.")
+        sampler.stop_flag = True
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(wl)
         print(json.dumps(line), flush=True)

@@ -198,6 +198,23 @@ modal_status modal_derive_coeffs(const modal_plan *plan, const modal_sample_geom
 modal_status modal_project_bump(const modal_plan *plan, double Lx, double Ly, double x0, double y0,
                                 double W, double A, double *q0);
 
+/* ---- machine peaks (measurement helper, not on the simulation path) ---------------------- */
+
+/* Micro-benchmarks of the denominators the roofline fractions of this build are quoted against and that the driver's
+ * MEASURED_PEAKS.json does not hold: FP32 / FP64 FMA issue peaks, L2-resident and HBM read bandwidth, shared-
+ * memory and TMEM read bandwidth, and the latency of the cross-CTA exchange primitives of the persistent kernels (one-way,
+ * SM cycles), idle and while the other SMs keep the L2 busy.  Runs ~1 s on `cuda_device`; MODAL_ECUDA on a CUDA error. */
+typedef struct {
+    double sm_clock_mhz;                 /* SM clock during the FMA test (cycles / event time)                      */
+    double fp32_tflops, fp64_tflops;     /* 2 flop per FMA                                                          */
+    double l2_read_gbs_8mb, l2_read_gbs_64mb, hbm_read_gbs;     /* ld.global.cg sweeps; 1 GiB for HBM               */
+    double smem_read_gbs, smem_bytes_per_clk_sm;                /* conflict-free LDS.128, all SMs / per SM          */
+    double tmem_read_bytes_per_clk_sm;   /* tcgen05.ld.32x32b.x32, four warps                                       */
+    double hop_cycles_idle, hop_cycles_loaded;                  /* tagged 8-byte word, st.relaxed -> polling ld.relaxed */
+    double relacq_hop_cycles_idle, relacq_hop_cycles_loaded;    /* payload + st.release flag -> poll, ld.acquire, payload */
+} modal_peaks;
+modal_status modal_measure_peaks(int cuda_device, modal_peaks *out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -55,7 +55,7 @@ class SampleGeom(C.Structure):
 
 EXPORTS = ["modal_plan_create", "modal_coeffs_upload", "modal_simulate", "modal_simulate_host",
            "modal_plan_check", "modal_plan_set_option", "modal_plan_destroy", "modal_last_error",
-           "modal_plan_query", "modal_derive_coeffs", "modal_project_bump"]
+           "modal_plan_query", "modal_derive_coeffs", "modal_project_bump", "modal_measure_peaks"]
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2505_05940_b200.build` "
@@ -74,6 +74,25 @@ lib.modal_last_error.restype = C.c_char_p
 lib.modal_plan_query.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_ulonglong]
 lib.modal_derive_coeffs.argtypes = [C.c_void_p, C.POINTER(SampleGeom), _dp, _dp, _dp, _dp, _dp]
 lib.modal_project_bump.argtypes = [C.c_void_p] + [C.c_double] * 6 + [_dp]
+
+
+class Peaks(C.Structure):
+    _fields_ = [(n, C.c_double) for n in (
+        "sm_clock_mhz", "fp32_tflops", "fp64_tflops", "l2_read_gbs_8mb", "l2_read_gbs_64mb", "hbm_read_gbs", "smem_read_gbs",
+        "smem_bytes_per_clk_sm", "tmem_read_bytes_per_clk_sm", "hop_cycles_idle", "hop_cycles_loaded",
+        "relacq_hop_cycles_idle", "relacq_hop_cycles_loaded")]
+
+
+lib.modal_measure_peaks.argtypes = [C.c_int, C.POINTER(Peaks)]
+
+
+def measure_peaks(device: int = 0) -> dict:
+    """modal_measure_peaks: FP32 / FP64 FMA, L2 / HBM / shared-memory / TMEM read bandwidth, exchange-hop latencies."""
+    pk = Peaks()
+    st = lib.modal_measure_peaks(device, C.byref(pk))
+    if st != OK:
+        raise RuntimeError(f"modal_measure_peaks: status {st}")
+    return {n: getattr(pk, n) for n, _ in Peaks._fields_}
 
 
 class ModalError(RuntimeError):

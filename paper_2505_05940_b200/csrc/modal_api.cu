@@ -16,6 +16,7 @@
 #include "kernels.cuh"
 #include "vk_flow.cuh"
 #include "vk_mma.cuh"
+#include "peaks.cuh"
 
 namespace mh = modal_host;
 namespace md = modal_dev;
@@ -1026,4 +1027,102 @@ extern "C" modal_status modal_project_bump(const modal_plan *p, double Lx, doubl
         mh::project_bump_rect(p->mq, Lx, Ly, x0, y0, W, A, q0);
     } else mh::project_bump_string(p->d.n_q, Lx, x0, W, A, q0);
     return MODAL_OK;
+}
+
+extern "C" modal_status modal_measure_peaks(int dev, modal_peaks *out)
+{
+    if (!out) return MODAL_EINVAL;
+    memset(out, 0, sizeof *out);
+#define PK(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); rc = MODAL_ECUDA; goto done; } } while (0)
+    modal_status rc = MODAL_OK;
+    cudaDeviceProp prop{};
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    void *buf = nullptr, *small = nullptr;
+    long long *cyc = nullptr;
+    std::vector<long long> hc;
+    float ms = 0;
+    int sm = 0;
+    const size_t big = (size_t)1 << 30;
+    if (cudaSetDevice(dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { cudaGetLastError(); return MODAL_ECUDA; }
+    sm = prop.multiProcessorCount;
+    PK(cudaEventCreate(&e0)); PK(cudaEventCreate(&e1));
+    PK(cudaMalloc(&buf, big)); PK(cudaMalloc(&small, 1 << 16)); PK(cudaMalloc(&cyc, (size_t)sm * 8));
+    PK(cudaMemset(buf, 1, big)); PK(cudaMemset(small, 0, 1 << 16));
+    hc.resize(sm);
+    {   // ---- FMA peaks: 8 CTAs of 256 threads per SM, 8 chains x 8 FMAs per iteration
+        const int iters = 4096;
+        auto run = [&](auto kern, auto x0, double &tf, double *clk) -> cudaError_t {
+            kern<<<sm * 8, 256>>>(reinterpret_cast<decltype(x0) *>(small), 64, x0);                      // warm-up
+            cudaEventRecord(e0); kern<<<sm * 8, 256>>>(reinterpret_cast<decltype(x0) *>(small), iters, x0); cudaEventRecord(e1);
+            cudaError_t e = cudaEventSynchronize(e1);
+            if (e != cudaSuccess) return e;
+            cudaEventElapsedTime(&ms, e0, e1);
+            const double fma = (double)sm * 8 * 256 * iters * 64.0;
+            tf = 2.0 * fma / (ms * 1e-3) / 1e12;
+            if (clk) *clk = fma / (ms * 1e-3) / ((double)sm * 128) / 1e6;                               // FP32: 128 FMA lanes per SM
+            return cudaGetLastError();
+        };
+        PK(run(md::peak_fma_kernel<float>, 1.0f, out->fp32_tflops, &out->sm_clock_mhz));
+        PK(run(md::peak_fma_kernel<double>, 1.0, out->fp64_tflops, nullptr));
+    }
+    {   // ---- read sweeps
+        auto sweep = [&](size_t bytes, int passes, double &gbs) -> cudaError_t {
+            md::peak_read_sweep_kernel<<<sm * 2, 512>>>(reinterpret_cast<const uint4 *>(buf), bytes / 16, 2, reinterpret_cast<unsigned *>(small));   // brings it into L2
+            cudaEventRecord(e0);
+            md::peak_read_sweep_kernel<<<sm * 2, 512>>>(reinterpret_cast<const uint4 *>(buf), bytes / 16, passes, reinterpret_cast<unsigned *>(small));
+            cudaEventRecord(e1);
+            cudaError_t e = cudaEventSynchronize(e1);
+            if (e != cudaSuccess) return e;
+            cudaEventElapsedTime(&ms, e0, e1);
+            gbs = (double)bytes * passes / (ms * 1e-3) / 1e9;
+            return cudaGetLastError();
+        };
+        PK(sweep((size_t)8 << 20, 400, out->l2_read_gbs_8mb));
+        PK(sweep((size_t)64 << 20, 50, out->l2_read_gbs_64mb));
+        PK(sweep(big, 4, out->hbm_read_gbs));
+    }
+    {   // ---- shared memory
+        const int iters = 4096;
+        PK(cudaFuncSetAttribute(md::peak_smem_read_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536));
+        md::peak_smem_read_kernel<<<sm, 512, 65536>>>(64, cyc, reinterpret_cast<unsigned *>(small));
+        cudaEventRecord(e0); md::peak_smem_read_kernel<<<sm, 512, 65536>>>(iters, cyc, reinterpret_cast<unsigned *>(small)); cudaEventRecord(e1);
+        PK(cudaEventSynchronize(e1));
+        cudaEventElapsedTime(&ms, e0, e1);
+        PK(cudaMemcpy(hc.data(), cyc, (size_t)sm * 8, cudaMemcpyDeviceToHost));
+        double c = 0; for (int i = 0; i < sm; ++i) c += (double)hc[i];
+        out->smem_bytes_per_clk_sm = 65536.0 * iters / (c / sm);
+        out->smem_read_gbs = 65536.0 * iters * sm / (ms * 1e-3) / 1e9;
+    }
+    {   // ---- TMEM
+        const int iters = 256;
+        md::peak_tmem_read_kernel<<<sm, 128>>>(8, cyc, reinterpret_cast<unsigned *>(small));
+        md::peak_tmem_read_kernel<<<sm, 128>>>(iters, cyc, reinterpret_cast<unsigned *>(small));
+        PK(cudaDeviceSynchronize());
+        PK(cudaMemcpy(hc.data(), cyc, (size_t)sm * 8, cudaMemcpyDeviceToHost));
+        double c = 0; for (int i = 0; i < sm; ++i) c += (double)hc[i];
+        out->tmem_read_bytes_per_clk_sm = 128.0 * 512 * 4 * iters / (c / sm);
+    }
+    {   // ---- exchange hops (one-way = half a round trip)
+        const int rounds = 2000;
+        double *dst[4] = {&out->hop_cycles_idle, &out->hop_cycles_loaded, &out->relacq_hop_cycles_idle, &out->relacq_hop_cycles_loaded};
+        for (int v = 0; v < 4; ++v) {
+            const int mode = v >> 1, load = v & 1;
+            PK(cudaMemset(small, 0, 1 << 16));
+            char *sb = reinterpret_cast<char *>(small);
+            md::peak_hop_kernel<<<sm, 512>>>(reinterpret_cast<unsigned long long *>(sb), reinterpret_cast<unsigned *>(sb + 4096), rounds, mode, load,
+                                             reinterpret_cast<const uint4 *>(buf), ((size_t)32 << 20) / 16, reinterpret_cast<volatile int *>(sb + 8192),
+                                             cyc, reinterpret_cast<unsigned *>(sb + 8256));
+            PK(cudaDeviceSynchronize());
+            PK(cudaMemcpy(hc.data(), cyc, 8, cudaMemcpyDeviceToHost));
+            *dst[v] = hc[0] > 0 ? (double)hc[0] / rounds / 2.0 : -1.0;
+        }
+    }
+done:
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (buf) cudaFree(buf);
+    if (small) cudaFree(small);
+    if (cyc) cudaFree(cyc);
+#undef PK
+    return rc;
 }
