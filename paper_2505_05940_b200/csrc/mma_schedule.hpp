@@ -56,7 +56,8 @@ struct MmaLayout {
     int NGRP = 0, NG = 0, NG4 = 0;              // n groups, most modes per group, float4 per partial-G row
     std::vector<int> nlist;                     // [NGRP][NG] in-plane modes of each group (-1: empty slot)
     int NC = 0;                                 // TMEM columns of one accumulator slot = NG * RBT (multiple of 16, <= 256)
-    int S = 0;                                  // accumulator slots in TMEM: min(3, 512 / NC)
+    int S = 0;                                  // accumulator slots in TMEM: min(3, 512 / NC); 2 in cluster mode
+    int CL = 0;                                 // 1: the NKB CTAs of a group form a thread-block cluster (partial G through distributed shared memory)
     int G = 0;                                  // CTAs = NGRP * NKB
     int rows_max = 0;                           // most sample rows of a tile one CTA owns for the update
     int KCL = 0;                                // most K chunks of any CTA (slab size)
@@ -89,9 +90,10 @@ inline void mma_blocks(const std::vector<int> &class_start, int split, std::vect
 
 // One candidate shape: blocks given, NG modes per group.  mode_class [n_phi]: modes of one group share a class.
 // `nz(n, k_int, r_int)` tells whether H^n[k][r] is non-zero.  Returns false if the shape does not fit the machine.
+// cluster_cap[s] (s = 2, 4, 8): thread-block clusters of s CTAs the device keeps co-resident with this kernel (0: none).
 template <class NZ>
 inline bool mma_layout_try(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, const std::vector<MmaBlock> &blocks,
-                           int NG, const std::vector<int> &mode_class, NZ nz, MmaLayout &L)
+                           int NG, const std::vector<int> &mode_class, NZ nz, const int *cluster_cap, MmaLayout &L)
 {
     L = MmaLayout();
     L.n_q = n_q; L.n_phi = n_phi; L.blocks = blocks; L.NKB = (int)blocks.size();
@@ -111,6 +113,8 @@ inline bool mma_layout_try(int n_q, int n_phi, int sm, size_t smem_limit, size_t
     L.NC = NG * L.RBT;
     if (L.NC > 256) return false;
     L.S = std::min(3, 512 / L.NC);
+    L.CL = (L.NKB == 2 || L.NKB == 4 || L.NKB == 8) && cluster_cap && cluster_cap[L.NKB] >= L.NGRP;
+    if (L.CL) L.S = std::min(L.S, 2);
     L.rows_max = mma_rows_owned_max(L.NGRP);
     L.nlist.assign((size_t)L.NGRP * NG, -1);
     {   // groups: the modes of a class spread evenly over its groups (balanced MMA work)
@@ -150,8 +154,8 @@ inline bool mma_layout_try(int n_q, int n_phi, int sm, size_t smem_limit, size_t
         }
     if (L.KCL > MMA_KCL_MAX) return false;
     L.slab_bytes = (size_t)L.KCL * 2 * L.NC * 32;
-    const size_t own = (size_t)MMA_MT_MAX * L.rows_max * L.RBQ * 4 * 44;          // fp64 (q, v, kv, kq, r) + fp32 w of the owned elements, every tile
-    if (L.slab_bytes + smem_fixed + own + (size_t)2 * L.KCL * 8192 > smem_limit) return false;   // ring: at least two tiles' chunks
+    const size_t own = (size_t)2 * L.rows_max * L.RBQ * 4 * 44;                    // fp64 (q, v, kv, kq, r) + fp32 w of the owned elements: at least two tiles per launch
+    if (L.slab_bytes + smem_fixed + own + (size_t)std::max(2, L.KCL) * 8192 > smem_limit) return false;   // ring: at least one tile's chunks
     L.klist.assign((size_t)L.G * L.KCL, 0); L.kcnt.assign(L.G, 0);
     L.fblk.assign((size_t)L.G * MMA_FBLK_MAX, 0); L.fcnt.assign(L.G, 0);
     for (int c = 0; c < L.G; ++c) {
@@ -175,14 +179,15 @@ inline bool mma_layout_try(int n_q, int n_phi, int sm, size_t smem_limit, size_t
     const double bytes = (double)L.KCL * 8192 + 128.0 * L.RBQ * 16 * 2 + (double)L.NGRP * L.rows_max * L.RBQ * 16 + 128.0 * L.NG4 * 16 * L.NKB;
     const double gather = 700.0 * std::ceil((double)L.NGRP * L.rows_max * L.RBQ / (16.0 * 64.0));
     const double idle = (double)(sm - L.G) / sm;
-    L.cost = (std::max(mma, bytes / 32.0) + gather + 30.0 * L.NGRP) * (1.0 + idle);
+    const double ghop = L.NKB == 1 ? 0.0 : L.CL ? 800.0 : 4500.0;          // partial-G exchange: distributed shared memory vs polling through L2
+    L.cost = (std::max(mma, bytes / 32.0) + gather + ghop + 30.0 * L.NGRP) * (1.0 + idle);
     return true;
 }
 
 // Shape choice over the class splits and group sizes.  force_split / force_ng > 0 pin them (plan options, tests / sweeps).
 template <class NZ>
 inline bool mma_layout(int n_q, int n_phi, int sm, size_t smem_limit, size_t smem_fixed, const std::vector<int> &class_start,
-                       const std::vector<int> &mode_class, NZ nz, int force_split, int force_ng, MmaLayout &L)
+                       const std::vector<int> &mode_class, NZ nz, int force_split, int force_ng, const int *cluster_cap, MmaLayout &L)
 {
     bool found = false;
     for (int split = 1; split <= 4; ++split) {
@@ -192,7 +197,7 @@ inline bool mma_layout(int n_q, int n_phi, int sm, size_t smem_limit, size_t sme
         for (int NG = 1; NG <= MMA_NG_MAX; ++NG) {
             if (force_ng > 0 && NG != force_ng) continue;
             MmaLayout T;
-            if (!mma_layout_try(n_q, n_phi, sm, smem_limit, smem_fixed, blocks, NG, mode_class, nz, T)) continue;
+            if (!mma_layout_try(n_q, n_phi, sm, smem_limit, smem_fixed, blocks, NG, mode_class, nz, cluster_cap, T)) continue;
             if (!found || T.cost < L.cost) { L = T; found = true; }
         }
     }

@@ -61,7 +61,7 @@ struct MmaConfig {
 };
 
 struct Options {                     // modal_plan_set_option
-    int vk_impl = 0, flow_g = 0, flow_ns = 0, flow_res = -1, mma_split = 0, mma_ng = 0, mma_nstg = 0, parity_order = 1, timing = 0;
+    int vk_impl = 0, flow_g = 0, flow_ns = 0, flow_res = -1, mma_split = 0, mma_ng = 0, mma_nstg = 0, mma_cluster = 1, parity_order = 1, timing = 0;
 };
 
 }  // namespace
@@ -409,7 +409,7 @@ modal_status configure_flow(modal_plan *p, int batch, FlowConfig **out)
 // ---- vk_mma (batched tensor-core kernel) -------------------------------------------------------
 // Layout (mma_schedule.hpp), operand slabs and per-layout tables; the exchange buffers are sized per launch.
 // Host part: the layout and the getters of the fp32 H values the device holds (flow tiles, internal order).
-bool mma_host_layout(const modal_plan *p, mh::MmaLayout &L)
+bool mma_host_layout(const modal_plan *p, mh::MmaLayout &L, const int *cluster_cap = nullptr)
 {
     const int nq = p->d.n_q, nphi = p->d.n_phi;
     if (p->d.model != MODAL_VK) return false;
@@ -430,7 +430,7 @@ bool mma_host_layout(const modal_plan *p, mh::MmaLayout &L)
         return p->tile_nz[tile] && Hf[tile * 256 + mh::flow_elem(hi % 16, lo % 16)] != 0.f;
     };
     return mh::mma_layout(nq, nphi, p->sm_count, SMEM_LIMIT, md::mma_smem_fixed(), class_start, mode_class, nz,
-                          p->opt.mma_split, p->opt.mma_ng, L);
+                          p->opt.mma_split, p->opt.mma_ng, p->opt.mma_cluster ? cluster_cap : nullptr, L);
 }
 
 void mma_host_slabs(const modal_plan *p, const mh::MmaLayout &L, std::vector<uint16_t> &slabs)
@@ -450,7 +450,21 @@ modal_status configure_mma(modal_plan *p)
     MmaConfig &m = p->mma;
     if (m.tried) return MODAL_OK;
     m.tried = true; m.ok = false;
-    if (!mma_host_layout(p, m.L)) return MODAL_OK;
+    // thread-block clusters of 2 / 4 / 8 CTAs of this kernel the device keeps co-resident (GPC boundaries strand some SMs)
+    int ccap[9] = {0};
+    if (cudaFuncSetAttribute(md::vk_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT) == cudaSuccess)
+        for (int cs : {2, 4, 8}) {
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3(cs * 8); cfg.blockDim = dim3(md::MMA_THREADS); cfg.dynamicSmemBytes = SMEM_LIMIT;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            int n = 0;
+            if (cudaOccupancyMaxActiveClusters(&n, md::vk_mma_kernel<false>, &cfg) == cudaSuccess) ccap[cs] = n;
+            cudaGetLastError();
+        }
+    else cudaGetLastError();
+    if (!mma_host_layout(p, m.L, ccap)) return MODAL_OK;
     const mh::MmaLayout &L = m.L;
     if (cudaFuncSetAttribute(md::vk_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT) != cudaSuccess) { cudaGetLastError(); return MODAL_OK; }
     int per_sm = 0;
@@ -580,11 +594,15 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
     } else if (p->opt.vk_impl != 1 && (p->opt.vk_impl == 2 || batch >= 64) && configure_mma(p) == MODAL_OK && p->mma.ok) {
         MmaConfig &m = p->mma;
         const mh::MmaLayout &L = m.L;
-        const int chunk = 128 * md::MMA_MT_MAX;                 // samples per launch: up to 8 M tiles time-multiplexed in one kernel
+        // M tiles per launch: as many (<= 8) as leave room for one tile's worth of ring stages beside slab and owner state; a wider batch
+        // runs as consecutive launches of equal size
+        int mt_cap = md::MMA_MT_MAX;
+        while (mt_cap > 1 && md::mma_smem_layout((int)L.slab_bytes, mt_cap, L.rows_max, L.RBQ, std::max(2, L.KCL)).total > SMEM_LIMIT) --mt_cap;
+        const int tiles = (batch + 127) / 128, launches = (tiles + mt_cap - 1) / mt_cap;
+        const int chunk = 128 * ((tiles + launches - 1) / launches);
         size_t smem = 0;
         for (int b0 = 0; b0 < batch; b0 += chunk) {
             const int nb = std::min(chunk, batch - b0), MT = (nb + 127) / 128;
-            // shared memory: slab + owner state and coefficients of MT tiles + as many ring stages as fit (<= 16)
             const size_t base = md::mma_smem_layout((int)L.slab_bytes, MT, L.rows_max, L.RBQ, 0).total;
             int nstg = base < SMEM_LIMIT ? (int)std::min<size_t>(md::MMA_NSTG_MAX, (SMEM_LIMIT - base) / 8192) : 0;
             if (p->opt.mma_nstg > 0) nstg = std::min(nstg, p->opt.mma_nstg);
@@ -595,7 +613,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             md::MmaArgs a{};
             a.slabs = m.dslabs.as<uint16_t>(); a.slab_bytes = (int)L.slab_bytes; a.NSTG = nstg;
             a.NKB = L.NKB; a.NGRP = L.NGRP; a.NG = L.NG; a.NG4 = L.NG4; a.NC = L.NC; a.S = L.S; a.RBT = L.RBT; a.RBQ = L.RBQ;
-            a.KC = L.KC; a.KCL = L.KCL; a.G = L.G; a.rows_max = L.rows_max; a.LPQ = m.lpq;
+            a.KC = L.KC; a.KCL = L.KCL; a.G = L.G; a.rows_max = L.rows_max; a.LPQ = m.lpq; a.CL = L.CL;
             const int *tab = m.dtab.as<int>();
             a.nlist = tab + m.off_nlist; a.klist = tab + m.off_klist; a.kcnt = tab + m.off_kcnt; a.fblk = tab + m.off_fblk;
             a.fcnt = tab + m.off_fcnt; a.blk = tab + m.off_blk;
@@ -624,13 +642,20 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             a.timeout_flag = p->dtimeout.as<int>();
             const bool timing = p->opt.timing != 0;
             if (timing) {
-                CU(p->dtiming.ensure((size_t)L.G * 128));
-                CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)L.G * 128, st));
+                CU(p->dtiming.ensure((size_t)L.G * (128 + 256)));
+                CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)L.G * (128 + 256), st));
                 a.timing = p->dtiming.as<long long>();
+                a.trace = a.timing + (size_t)L.G * 16;
             }
             persistent = true;
-            if (timing) md::vk_mma_kernel<true><<<L.G, md::MMA_THREADS, smem, st>>>(a);
-            else md::vk_mma_kernel<false><<<L.G, md::MMA_THREADS, smem, st>>>(a);
+            {
+                cudaLaunchConfig_t cfg{};
+                cfg.gridDim = dim3(L.G); cfg.blockDim = dim3(md::MMA_THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = L.CL ? L.NKB : 1; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                cfg.attrs = at; cfg.numAttrs = 1;
+                CU(timing ? cudaLaunchKernelEx(&cfg, md::vk_mma_kernel<true>, a) : cudaLaunchKernelEx(&cfg, md::vk_mma_kernel<false>, a));
+            }
             CU(cudaGetLastError());
             if (timing) {
                 CU(cudaStreamSynchronize(st));
@@ -639,12 +664,28 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
                 double acc[16] = {0};
                 for (size_t x = 0; x < tm.size(); ++x) acc[x & 15] += (double)tm[x];
                 const double den = (double)L.G * n_steps;
-                fprintf(stderr, "[modal mma timing] G=%d (%d groups x %d blocks) NG=%d NC=%d S=%d KCL=%d ring=%d MT=%d  cycles/step of tile 0, mean over CTAs:\n"
+                fprintf(stderr, "[modal mma timing] G=%d (%d groups x %d blocks%s) NG=%d NC=%d S=%d KCL=%d ring=%d MT=%d  cycles/step of tile 0, mean over CTAs:\n"
                         "   E: wait q %.0f | wait acc %.0f | epi1+send %.0f (first unit in registers after %.0f, all units after %.0f) | G hop %.0f | epi2 %.0f\n"
                         "   O: gather %.0f | update %.0f | publish %.0f | barrier+fence+flag %.0f     P: flag poll %.0f   M: first chunk -> commit %.0f\n"
                         "   hops: end of epilogue 2 -> forces gathered %.0f | own flag set -> all source flags seen %.0f\n",
-                        L.G, L.NGRP, L.NKB, L.NG, L.NC, L.S, L.KCL, nstg, MT, acc[0] / den, acc[1] / den, acc[2] / den, acc[5] / den, acc[6] / den, acc[3] / den, acc[4] / den,
+                        L.G, L.NGRP, L.NKB, L.CL ? ", clusters" : "", L.NG, L.NC, L.S, L.KCL, nstg, MT, acc[0] / den, acc[1] / den, acc[2] / den, acc[5] / den, acc[6] / den, acc[3] / den, acc[4] / den,
                         acc[8] / den, acc[11] / den, acc[9] / den, acc[10] / den, acc[12] / den, acc[13] / den, acc[14] / den, acc[15] / den);
+                if (n_steps >= 68) {   // spread of the phase boundaries of step 65 over the CTAs (globaltimer, ns after the earliest event of the step)
+                    std::vector<long long> tr((size_t)L.G * 32);
+                    CU(cudaMemcpy(tr.data(), p->dtiming.as<long long>() + (size_t)L.G * 16, tr.size() * 8, cudaMemcpyDeviceToHost));
+                    static const char *names[8] = {"q ready (flags seen)", "accumulator ready", "G sent", "G received", "epilogue 2 done", "forces gathered",
+                                                   "q published", "flag released"};
+                    long long t0 = -1;
+                    for (int c = 0; c < L.G; ++c) for (int e = 0; e < 8; ++e) { const long long v = tr[((size_t)c * 4 + 1) * 8 + e]; if (v > 0 && (t0 < 0 || v < t0)) t0 = v; }
+                    for (int e = 0; e < 8; ++e) {
+                        std::vector<long long> v;
+                        for (int c = 0; c < L.G; ++c) if (tr[((size_t)c * 4 + 1) * 8 + e] > 0) v.push_back(tr[((size_t)c * 4 + 1) * 8 + e] - t0);
+                        if (v.empty()) continue;
+                        std::sort(v.begin(), v.end());
+                        fprintf(stderr, "   step 65 %-20s ns after the step's first event: min %6lld  p10 %6lld  median %6lld  p90 %6lld  max %6lld\n", names[e], v.front(),
+                                v[v.size() / 10], v[v.size() / 2], v[v.size() * 9 / 10], v.back());
+                    }
+                }
             }
         }
         p->kinfo[0] = 4; p->kinfo[1] = L.G; p->kinfo[2] = L.NGRP; p->kinfo[3] = md::MMA_THREADS;
@@ -878,7 +919,7 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
     struct { const char *name; int *field; int lo, hi; } tab[] = {
         {"vk_impl", &p->opt.vk_impl, 0, 2}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
         {"flow_res", &p->opt.flow_res, -1, 1 << 20}, {"mma_split", &p->opt.mma_split, 0, 4}, {"mma_ng", &p->opt.mma_ng, 0, 8},
-        {"mma_nstg", &p->opt.mma_nstg, 0, 16}, {"parity_order", &p->opt.parity_order, 0, 1}, {"timing", &p->opt.timing, 0, 1}};
+        {"mma_nstg", &p->opt.mma_nstg, 0, 16}, {"mma_cluster", &p->opt.mma_cluster, 0, 1}, {"parity_order", &p->opt.parity_order, 0, 1}, {"timing", &p->opt.timing, 0, 1}};
     for (auto &t : tab)
         if (!strcmp(key, t.name)) {
             if (value < t.lo || value > t.hi) { p->err = std::string("option ") + key + ": value out of range\n"; return MODAL_EINVAL; }
@@ -899,7 +940,7 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
                 set_H(p, [&](int n, int a, int b) { return Hu[((size_t)n * nq + a) * nq + b]; });
                 p->coeffs_dirty = true;
             }
-            if (t.field == &p->opt.mma_split || t.field == &p->opt.mma_ng) { p->mma.tried = false; p->mma.ok = false; }
+            if (t.field == &p->opt.mma_split || t.field == &p->opt.mma_ng || t.field == &p->opt.mma_cluster) { p->mma.tried = false; p->mma.ok = false; }
             return MODAL_OK;
         }
     p->err = std::string("unknown option ") + key + "\n";

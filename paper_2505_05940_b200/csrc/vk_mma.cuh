@@ -49,7 +49,7 @@ constexpr int MMA_GB = 16;           // 16-byte strong loads a lane keeps in fli
 constexpr int MMA_RB_MAX_DEV = 56;   // == modal_host::MMA_RB_MAX: rows k of a block (a sample's block of q lives in registers)
 constexpr int MMA_NG_MAX_DEV = 8;    // == modal_host::MMA_NG_MAX: in-plane modes of a group
 // mbarrier indices (64-bit words of the first shared-memory block)
-constexpr int MB_FULL = 0, MB_EMPTY = 16, MB_ACCF = 32, MB_ACCE = 35, MB_QRDY = 38, MB_TPTR = 56, MB_ABORT = 57, MB_STAMP = 58;   // QRDY: one per tile (<= 16)
+constexpr int MB_FULL = 0, MB_EMPTY = 16, MB_ACCF = 32, MB_ACCE = 35, MB_QRDY = 38, MB_TPTR = 56, MB_ABORT = 57, MB_STAMP = 58, MB_RS = 60, MB_AG = 62;   // QRDY: one per tile (<= 16); RS / AG: cluster G exchange, one per slot
 constexpr int MMA_TAB_OFF = 512;     // byte offset of the per-CTA tables inside the first block (ints): klist[64] nmode[8] fblk[16] blk[16][3]
 constexpr int MMA_BARS_BYTES = 1536;
 
@@ -57,6 +57,7 @@ struct MmaArgs {
     const uint16_t *slabs;      // [G][slab_bytes] bf16 hi/lo operand slabs of H: only the K chunks of klist, in list order
     int slab_bytes, NSTG;
     int NKB, NGRP, NG, NG4, NC, S, RBT, RBQ, KC, KCL, G, rows_max, LPQ;
+    int CL;                     // 1: the NKB CTAs of an n group form a thread-block cluster and exchange partial G through distributed shared memory
     const int *nlist;           // [NGRP][NG] in-plane modes of each group (-1: empty)
     const int *klist, *kcnt;    // [G][KCL], [G]
     const int *fblk, *fcnt;     // [G][16], [G]: blocks whose owners this CTA waits for (own block first)
@@ -80,9 +81,10 @@ struct MmaArgs {
     unsigned long long *px;     // [2][MT][NKB][128][2]             pickup partials {o, epoch}, {|q|^2, epoch}
     int *timeout_flag;          // per plan: set when a bounded wait gave up
     long long *timing;          // optional [G][16] cycle counters of tile 0
+    long long *trace;           // optional [G][4][8] globaltimer stamps of tile 0 at steps 64..67 (phase boundaries; timing build)
 };
 
-struct MmaSmem { size_t bars, sq, sv, coef, pk, sbad, wdone, slab, ring, total; };
+struct MmaSmem { size_t bars, sq, sv, coef, pk, sbad, wdone, gex, slab, ring, total; };
 __host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int MT, int rows_max, int RBQ, int nstg)
 {
     MmaSmem L; size_t o = 0;
@@ -94,6 +96,8 @@ __host__ __device__ inline MmaSmem mma_smem_layout(int slab_bytes, int MT, int r
     L.pk = o;    o += (size_t)2 * 2 * rows_max * RBQ * 8;       // [team][buffer][row][quad] float2
     L.sbad = o;  o += (size_t)MT * rows_max * 4;
     L.wdone = o; o += (size_t)MMA_MT_MAX * 4;
+    o = flow_align(o, 16);
+    L.gex = o;   o += (size_t)2 * 2 * 128 * 32;                 // cluster G exchange: [reduce-scatter | all-gather][slot][128 x 8 floats]
     o = flow_align(o, 128);
     L.slab = o;  o += (size_t)slab_bytes;
     o = flow_align(o, 128);
@@ -134,6 +138,43 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&u)[1
                  : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// ---- distributed shared memory (thread-block cluster) ---------------------------------------------
+__device__ __forceinline__ uint32_t dsm_map(uint32_t saddr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+// st.async: the store and the signal travel together -- the bytes are counted on the destination CTA's mbarrier (complete_tx), whose
+// waiters see them when the phase completes; no fence, no separate arrive (a release-arrive per thread measured ~2 k cycles)
+__device__ __forceinline__ void dsm_st_async4(uint32_t raddr, uint32_t rbar, float a, float b, float c, float d)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1,%2,%3,%4}, [%5];"
+                 ::"r"(raddr), "r"(__float_as_uint(a)), "r"(__float_as_uint(b)), "r"(__float_as_uint(c)), "r"(__float_as_uint(d)), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ void dsm_st_async1(uint32_t raddr, uint32_t rbar, float a)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(raddr), "r"(__float_as_uint(a)), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ void dsm_wait(uint32_t bar, uint32_t parity, volatile int *abortp)
+{
+    uint32_t ok;
+    unsigned spins = 0;
+    const long long t0 = clock64();
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (!ok && (++spins & 63u) == 0 && (*abortp || clock64() - t0 > 3000000000LL)) { *abortp = 1; break; }
+    } while (!ok);
+}
+__device__ __forceinline__ void mma_trace(const MmaArgs &a, int c, int n, int ev)
+{
+    if (a.trace && n >= 64 && n < 68) {
+        long long g; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
+        a.trace[((size_t)c * 4 + (n - 64)) * 8 + ev] = g;
+    }
+}
 __device__ __forceinline__ uint16_t bf16_rn_dev(float x)
 {
     uint32_t u = __float_as_uint(x);
@@ -219,7 +260,7 @@ struct MmaCta {
     const int *kl, *nmode, *fb, *blk;     // tables in shared memory
     volatile int *s_abort;
     double *sq, *sv; unsigned char *coef; float2 *pk; int *sbad; volatile int *wdone;
-    unsigned char *slab, *ring;
+    unsigned char *slab, *ring, *gex;
     uint32_t tbase;
     size_t nel;                 // owner-state elements per tile: rows_max * RBQ * 4
 };
@@ -258,7 +299,7 @@ __device__ __forceinline__ void mma_epilogue_e1_tile(const MmaArgs &a, const Mma
             const unsigned use = (unsigned)n * (unsigned)uses + (unsigned)(t / S);
             long long tk = tmg && t == 0 ? clock64() : 0;
             mbar_wait(smem_u32(C.bars + MB_QRDY + t), n & 1, C.s_abort);                 // q^n of the own block is published
-            if (tmg && t == 0) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; mma_trace(a, C.c, n, 0); }
             // ---- this sample's q over the rows of block j (operand of epilogue 1), coalesced quads ----
             float q[NQ];
             {
@@ -271,7 +312,7 @@ __device__ __forceinline__ void mma_epilogue_e1_tile(const MmaArgs &a, const Mma
                 }
             }
             mbar_wait(smem_u32(C.bars + MB_ACCF + slot), use & 1u, C.s_abort);            // t of this tile is in TMEM
-            if (tmg && t == 0) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; mma_trace(a, C.c, n, 1); }
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t taddr0 = C.tbase + ((uint32_t)lane_base << 16) + (uint32_t)(slot * a.NC);
             // ---- epilogue 1: partial G over the rows k of block j ----
@@ -305,12 +346,23 @@ __device__ __forceinline__ void mma_epilogue_e1_tile(const MmaArgs &a, const Mma
                 tmem_ld_wait();
             }
             if (tmg && t == 0) tm[6] += clock64() - tk;
-            // ---- G hop, send side (buffer of this step's parity) ----
-            uint32_t *gx = a.Gx + ((size_t)(n & 1) * MT + t) * NGRP * NKB * g_words;
-            uint32_t *grow = gx + ((size_t)C.i * NKB + C.j) * g_words + (size_t)r * 4 * NG4;
-            st_tagged4(grow, g[0], g[1], g[2], g[3], tag);
-            if (NG4 > 1) st_tagged4(grow + 4, g[4], g[5], g[6], g[7], tag);
-            if (tmg && t == 0) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; }
+            // ---- G hop, send side ----
+            if (a.CL) {
+                // cluster of the group's k blocks: row r is summed by CTA r / RPR (reduce-scatter over the rows); the partials go
+                // straight into that CTA's shared memory, the arrival on its mbarrier releases them (no polling, no L2)
+                const int RPR = 128 / NKB, jr = r / RPR, lr = r - jr * RPR;
+                const uint32_t dst = dsm_map(smem_u32(C.gex) + (uint32_t)(((slot * NKB + C.j) * RPR + lr) * 32), (uint32_t)jr);
+                const uint32_t rbar = dsm_map(smem_u32(C.bars + MB_RS + slot), (uint32_t)jr);
+                dsm_st_async4(dst, rbar, g[0], g[1], g[2], g[3]);
+                if (NG4 > 1) dsm_st_async4(dst + 16, rbar, g[4], g[5], g[6], g[7]);
+            } else {
+                // through L2 (buffer of this step's parity): tagged words the peers poll
+                uint32_t *gx = a.Gx + ((size_t)(n & 1) * MT + t) * NGRP * NKB * g_words;
+                uint32_t *grow = gx + ((size_t)C.i * NKB + C.j) * g_words + (size_t)r * 4 * NG4;
+                st_tagged4(grow, g[0], g[1], g[2], g[3], tag);
+                if (NG4 > 1) st_tagged4(grow + 4, g[4], g[5], g[6], g[7], tag);
+            }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; mma_trace(a, C.c, n, 2); }
         }
     }
 }
@@ -319,7 +371,7 @@ __device__ __forceinline__ void mma_epilogue_e1_tile(const MmaArgs &a, const Mma
 // Runs on its own warpgroup, so the wait for the peers' partial G never holds up epilogue 1 of the next tile.
 template <int NSP, bool TIMING>
 __device__ __forceinline__ void mma_epilogue_e2_tile(const MmaArgs &a, const MmaCta &C, const int r, const int lane_base, const int n, const int t,
-                                                     const bool tmg, long long (&tm)[7])
+                                                     const bool tmg, long long (&tm)[7], const int wg)
 {
     const int NG4 = a.NG4, NKB = a.NKB, NGRP = a.NGRP, B = a.batch, RBT = a.RBT, RBQ = a.RBQ, S = a.S, MT = a.MT;
     const size_t g_words = (size_t)128 * 4 * NG4;
@@ -341,10 +393,32 @@ __device__ __forceinline__ void mma_epilogue_e2_tile(const MmaArgs &a, const Mma
                 sc[u] = nn >= 0 ? __ldg(a.sT + (size_t)nn * a.sT_stride + (a.coeff_stride_phi && valid ? b : 0)) : 0.f;
             }
             long long tk = tmg && t == 0 ? clock64() : 0;
-            // ---- G hop, receive side: the partial rows of the other k blocks of this mode group, block order ----
+            // ---- G hop, receive side: G_n of this sample summed over the k blocks of the group, block order ----
             float eta[MMA_NG_MAX_DEV];
 #pragma unroll
             for (int u = 0; u < MMA_NG_MAX_DEV; ++u) eta[u] = 0.f;
+            if (a.CL) {
+                // reduce: this CTA sums RPR rows x 8 modes over the NKB sources, broadcasts the totals into every peer's shared memory
+                const int RPR = 128 / NKB;
+                const uint32_t gex = smem_u32(C.gex);
+                if (r == 0) {      // arm this tile-step's phases: the bytes the peers send (they may already have arrived: the count is signed)
+                    mbar_expect_tx(smem_u32(C.bars + MB_RS + slot), 128u * 16u * (uint32_t)NG4);
+                    mbar_expect_tx(smem_u32(C.bars + MB_AG + slot), 4096u);
+                }
+                dsm_wait(smem_u32(C.bars + MB_RS + slot), use & 1u, C.s_abort);
+                const float *rs = reinterpret_cast<const float *>(C.gex) + (size_t)slot * 1024;
+                for (int item = r; item < RPR * 8; item += 128) {
+                    float tot = 0.f;
+                    for (int src = 0; src < NKB; ++src) tot += rs[src * RPR * 8 + item];                 // item = local row * 8 + mode
+                    const uint32_t off = (uint32_t)(8192 + slot * 4096 + (C.j * RPR * 8 + item) * 4);  // all-gather area: [slot][row][mode]
+                    for (int peer = 0; peer < NKB; ++peer)
+                        dsm_st_async1(dsm_map(gex + off, (uint32_t)peer), dsm_map(smem_u32(C.bars + MB_AG + slot), (uint32_t)peer), tot);
+                }
+                dsm_wait(smem_u32(C.bars + MB_AG + slot), use & 1u, C.s_abort);
+                const float4 *ag = reinterpret_cast<const float4 *>(C.gex + 8192 + slot * 4096 + r * 32);
+                const float4 x0 = ag[0], x1 = ag[1];
+                eta[0] = x0.x; eta[1] = x0.y; eta[2] = x0.z; eta[3] = x0.w; eta[4] = x1.x; eta[5] = x1.y; eta[6] = x1.z; eta[7] = x1.w;
+            } else
             {
                 const uint32_t *grd = gx + (size_t)C.i * NKB * g_words + (size_t)r * 4 * NG4;
                 for (int jj0 = 0; jj0 < NKB; jj0 += 8) {
@@ -378,7 +452,7 @@ __device__ __forceinline__ void mma_epilogue_e2_tile(const MmaArgs &a, const Mma
             }
 #pragma unroll
             for (int u = 0; u < MMA_NG_MAX_DEV; ++u) eta[u] *= sc[u];                       // eta_n = s_n G_n
-            if (tmg && t == 0) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[3] += t_ - tk; tk = t_; mma_trace(a, C.c, n, 3); }
             // ---- epilogue 2: partial force over the modes n of group i, published as tagged quads ----
             uint32_t *frow = a.fx + ((((size_t)t * NGRP + C.i) * NKB + C.j) * RBQ) * 512 + (size_t)r * 4;
 #pragma unroll
@@ -412,7 +486,7 @@ __device__ __forceinline__ void mma_epilogue_e2_tile(const MmaArgs &a, const Mma
             }
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             mbar_arrive(smem_u32(C.bars + MB_ACCE + slot));                              // the accumulator slot may be overwritten
-            if (tmg && t == 0) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP) = t_; }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[4] += t_ - tk; tk = t_; *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP) = t_; mma_trace(a, C.c, n, 4); }
         }
     }
 }
@@ -429,13 +503,13 @@ __device__ __forceinline__ void mma_epilogue_warpgroup(const MmaArgs &a, const M
         for (int n = 0; n < a.n_steps; ++n)
             for (int t = 0; t < a.MT; ++t) {
                 if (w == 0) mma_epilogue_e1_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg, tm);
-                else mma_epilogue_e2_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg, tm);
+                else mma_epilogue_e2_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg, tm, w);
             }
     } else {
         for (int n = 0; n < a.n_steps; ++n)
             for (int t = w; t < a.MT; t += 2) {
                 mma_epilogue_e1_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg && w == 0, tm);
-                mma_epilogue_e2_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg && w == 0, tm);
+                mma_epilogue_e2_tile<NSP, TIMING>(a, C, r, lane_base, n, t, tmg && w == 0, tm, w);
             }
     }
     if (tmg && (a.MT <= 2 || w == 0)) {
@@ -526,7 +600,7 @@ __device__ __forceinline__ void mma_owner_steps(const MmaArgs &a, const MmaCta &
                             if (u < cnt) { fs.x += untag(x[u].x); fs.y += untag(x[u].y); fs.z += untag(x[u].z); fs.w += untag(x[u].w); }
                     }
                 }
-                if (tmg && t == 0 && base == 0) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; tmx += t_ - *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP); }
+                if (tmg && t == 0 && base == 0) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; tmx += t_ - *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP); mma_trace(a, C.c, n, 5); }
                 // join the parts of the group range (fp32 addition is commutative: every lane of the quad gets the same bits)
                 if (LPQ >= 2) {
                     fs.x += __shfl_xor_sync(FLOW_FULL, fs.x, 1); fs.y += __shfl_xor_sync(FLOW_FULL, fs.y, 1);
@@ -576,7 +650,7 @@ __device__ __forceinline__ void mma_owner_steps(const MmaArgs &a, const MmaCta &
                 if (LPQ >= 4) { po += __shfl_xor_sync(FLOW_FULL, po, 2); pn += __shfl_xor_sync(FLOW_FULL, pn, 2); }
                 if (act && sub == 0) pk[item] = make_float2(po, pn);
             }
-            if (tmg && t == 0) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; mma_trace(a, C.c, n, 6); }
             bar_named(2 + team, TL);
             if (tl == 0) {
                 if (C.j == 0) {            // warp W must have consumed the pickup partials of q^n before any owner may go on to q^{n+2}
@@ -585,7 +659,7 @@ __device__ __forceinline__ void mma_owner_steps(const MmaArgs &a, const MmaCta &
                 }
                 set_flag(a.qflag + (((size_t)t * NKB + C.j) * NGRP + C.i) * MMA_FS, (unsigned)n + 2u);
             }
-            if (tmg && t == 0) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP + 1) = t_; }
+            if (tmg && t == 0) { const long long t_ = clock64(); tm[2] += t_ - tk; tk = t_; *reinterpret_cast<volatile long long *>(C.bars + MB_STAMP + 1) = t_; mma_trace(a, C.c, n, 7); }
             if (tl < C.rows) {                                 // pickup partial of q^{n+1} for row tl
                 float o = 0.f, nr = 0.f;
                 for (int qd = 0; qd < C.RBQj; ++qd) { const float2 x = pk[tl * C.RBQj + qd]; o += x.x; nr += x.y; }
@@ -715,18 +789,20 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     C.pk = reinterpret_cast<float2 *>(mma_smem + L.pk);
     C.sbad = reinterpret_cast<int *>(mma_smem + L.sbad);
     C.wdone = reinterpret_cast<volatile int *>(mma_smem + L.wdone);
-    C.slab = mma_smem + L.slab; C.ring = mma_smem + L.ring;
+    C.slab = mma_smem + L.slab; C.ring = mma_smem + L.ring; C.gex = mma_smem + L.gex;
     C.nel = (size_t)a.rows_max * a.RBQ * 4;
 
     if (tid == 0) {
         for (int s = 0; s < a.NSTG; ++s) { mbar_init(smem_u32(C.bars + MB_FULL + s), 1); mbar_init(smem_u32(C.bars + MB_EMPTY + s), 1); }
         for (int s = 0; s < 3; ++s) { mbar_init(smem_u32(C.bars + MB_ACCF + s), 1); mbar_init(smem_u32(C.bars + MB_ACCE + s), 128); }
         for (int t = 0; t < MMA_MT_MAX; ++t) mbar_init(smem_u32(C.bars + MB_QRDY + t), 1);
+        for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(C.bars + MB_RS + s), 1); mbar_init(smem_u32(C.bars + MB_AG + s), 1); }
         *C.s_abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int x = tid; x < a.MT * a.rows_max; x += blockDim.x) C.sbad[x] = -1;
     if (tid < MMA_MT_MAX) C.wdone[tid] = 0;
+    for (int x = tid; x < 4096; x += blockDim.x) reinterpret_cast<float *>(C.gex)[x] = 0.f;
     if (tid < a.KCL && tid < 64) tab[tid] = a.klist[(size_t)C.c * a.KCL + tid];
     if (tid < MMA_NG_MAX_DEV) tab[64 + tid] = tid < a.NG ? a.nlist[C.i * a.NG + tid] : -1;
     if (tid < 16) tab[72 + tid] = a.fblk[(size_t)C.c * 16 + tid];
@@ -743,6 +819,9 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (a.CL) {   // the peers' mbarriers and exchange areas are set up before anybody stores into them
+        asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    }
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     C.tbase = *tptr;
     C.k0 = C.blk[3 * C.j]; C.nb = C.blk[3 * C.j + 1]; C.koff = C.blk[3 * C.j + 2]; C.RBQj = (C.nb + 3) >> 2;
@@ -837,6 +916,9 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (a.CL) {   // no CTA of the cluster leaves while a peer may still store into its shared memory
+        asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    }
     if (tid == 0 && *C.s_abort) *a.timeout_flag = 1;
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(C.tbase), "r"(512));
 }
