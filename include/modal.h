@@ -141,6 +141,16 @@ modal_status modal_plan_check(modal_plan *plan, int *first_bad_step);
  * Returns MODAL_EINVAL for an unknown key or a value out of range. */
 modal_status modal_plan_set_option(modal_plan *plan, const char *key, int value);
 
+/* In-plane (Airy) basis of a MODAL_VK plan, PAPER.md:53, 123 (the paper gives no formula; readings R5 / R16):
+ *   MODAL_AIRY_SINE          the transverse sine products, zeta_n^4 = lambda_n^2 (default, reading R5)
+ *   MODAL_AIRY_CLAMPED_RITZ  the clamped-plate eigenfunctions Lap Lap Psi = zeta^4 Psi, Psi = dPsi/dn = 0, by Rayleigh-Ritz on
+ *                            T_i(x/Lx) T_j(y/Ly), T_i(s) = sin(pi s) sin(i pi s), i, j <= n_trial (0: chosen from n_phi)
+ * Recomputes H (closed-form integrals) and nl_scale = E / (2 rho zeta_n^4) of the reference geometry for every coefficient row;
+ * omega, sigma, pickup stay.  With the Ritz basis H does not follow the (Lx Ly)^(-5/2) law across aspect ratios, so per-sample
+ * geometries (modal_derive_coeffs) keep reading R14 only at the plan's aspect ratio.  Errors: MODAL_EINVAL, MODAL_EINCOMPAT. */
+typedef enum { MODAL_AIRY_SINE = 0, MODAL_AIRY_CLAMPED_RITZ = 1 } modal_airy_basis;
+modal_status modal_plan_set_airy_basis(modal_plan *plan, int basis, int n_trial);
+
 void modal_plan_destroy(modal_plan *plan);
 const char *modal_last_error(const modal_plan *plan);
 
@@ -169,6 +179,7 @@ typedef enum {
                              /*        fewest / most K chunks of a CTA, slab KiB, most source blocks of a CTA           */
     MODAL_Q_MMA_SLAB_CHECK = 15, /* double [3]: non-zero entries of H covered by the operand slabs, non-zero entries of */
                              /*        H, max |hi + lo - H| / max |H| (host-side self check of the packing)             */
+    MODAL_Q_AIRY_ZETA4 = 16, /* double [n_phi]: zeta_n^4 of the plan's in-plane basis (reference geometry)                    */
     MODAL_Q_TILE_STATS = 13  /* int    [2]: 16x16 tiles of the packed H, and how many hold a non-zero.   */
                              /*        The device keeps the transverse modes grouped by index parity   */
                              /*        (internal order only: every array of this API is in plan order),*/

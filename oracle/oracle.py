@@ -417,14 +417,24 @@ def assemble(wl: dict, samples=None, *, scheme=SV, lossless=False, round_fp32=Tr
         ref = wl["ref"]
         mq, nq, _ = rect_modes(ref["Lx"], ref["Ly"], Nq)            # index sets: reference geometry
         mphi, nphi, _ = rect_modes(ref["Lx"], ref["Ly"], Nphi)      # reading R5
-        H = rnd(H_closed(ref["Lx"], ref["Ly"], mq, nq, mphi, nphi))
+        ritz = wl.get("airy", "sine") == "ritz"                      # reading R16 instead of R5 (workload key, default sine)
+        if ritz:
+            z4_ref, c_airy = airy_ritz_basis(ref["Lx"], ref["Ly"], Nphi, n_trial=wl["n_trial"])
+            H = rnd(H_airy_ritz(ref["Lx"], ref["Ly"], mq, nq, c_airy))
+        else:
+            H = rnd(H_closed(ref["Lx"], ref["Ly"], mq, nq, mphi, nphi))
         c_ref = (ref["Lx"] * ref["Ly"]) ** -2.5
         for b in samples:
             Lx, Ly, h = wl["Lx"][b], wl["Ly"][b], wl["h"][b]
             lam = rect_lambda(mq, nq, Lx, Ly)
             om, ga = omega_gamma(lam, plate_D(wl["E"], h, wl["nu"]), wl["T0"], wl["rho"] * h, s0, s1)
             act = active_mask(scheme, om, ga, T)
-            zeta4 = rect_lambda(mphi, nphi, Lx, Ly) ** 2                # zeta_n^4 = lambda_n^2 (R5)
+            if ritz:
+                # the Ritz modes keep their shape only at the reference aspect ratio, where zeta^4 ~ L^-4
+                assert abs(Ly / Lx - ref["Ly"] / ref["Lx"]) < 1e-12, "reading R16: per-sample geometry at the reference aspect ratio only"
+                zeta4 = z4_ref * (ref["Lx"] / Lx) ** 4
+            else:
+                zeta4 = rect_lambda(mphi, nphi, Lx, Ly) ** 2            # zeta_n^4 = lambda_n^2 (R5)
             c_b = (Lx * Ly) ** -2.5
             s = rnd(wl["E"] / (2.0 * wl["rho"] * zeta4) * (c_b / c_ref) ** 2)   # reading R14
             xp, yp = wl["pickup"][0] * Lx, wl["pickup"][1] * Ly
@@ -494,3 +504,80 @@ def run_case(case: Case, n_steps: int, **kw):
                     lam=case.lam if case.model == TENSION else None,
                     nl_scale=case.nl_scale if case.model != LINEAR else None,
                     H=case.H, **kw)
+
+
+# ------------------------------------------------------- in-plane basis, reading B ----
+# PAPER.md:53, 123 say the in-plane (Airy) eigenfunctions Psi_n and eigenvalues zeta_n^4 come from "a separate
+# eigendecomposition of the Airy stress function" by "a Galerkin type approach" and give no formula.  For a plate whose edges
+# are free to move in the plane the Airy function obeys Psi = dPsi/dn = 0 on the boundary, i.e. the CLAMPED-plate problem
+#     Lap Lap Psi = zeta^4 Psi,   Psi = dPsi/dn = 0 on the edges                       (reading R16)
+# which has no closed form.  Rayleigh-Ritz on the trial space  T_i(x / Lx) T_j(y / Ly),  T_i(s) = sin(pi s) sin(i pi s),
+# i, j = 1 .. n_trial  (every T_i and its slope vanish at s = 0 and 1):
+#     K c = zeta^4 M c,   K = int (Lap u)(Lap v) dS,   M = int u v dS.
+# This oracle does every integral by Gauss-Legendre QUADRATURE and the eigenproblem with scipy.linalg.eigh; the library uses
+# closed-form integrals and its own eigensolver (csrc/host_math.hpp), so comparing the two is a real cross-check.
+def _ritz_trial(n_trial, s):
+    """T_i(s), T_i'(s), T_i''(s) for i = 1..n_trial at the points s (unit interval)."""
+    i = np.arange(1, n_trial + 1)[:, None]
+    a, b = np.sin(np.pi * s)[None, :], np.sin(i * np.pi * s)
+    da, db = np.pi * np.cos(np.pi * s)[None, :], i * np.pi * np.cos(i * np.pi * s)
+    dda, ddb = -np.pi ** 2 * a, -(i * np.pi) ** 2 * b
+    return a * b, da * b + a * db, dda * b + 2 * da * db + a * ddb
+
+
+def airy_ritz_basis(Lx, Ly, n_phi, n_trial=12, ng=160):
+    """The n_phi lowest clamped-plate (Airy) modes on [0, Lx] x [0, Ly]: zeta4 [n_phi] ascending and coefficients
+    c [n_phi][n_trial][n_trial] with Psi_n(x, y) = sum_ij c[n, i, j] T_i(x / Lx) T_j(y / Ly), unit L2 norm, sign fixed by
+    making the largest coefficient positive.  All integrals by ng-point Gauss-Legendre quadrature."""
+    from scipy.linalg import eigh
+    xg, wg = np.polynomial.legendre.leggauss(ng)
+    s, w = 0.5 * (xg + 1.0), 0.5 * wg
+    T, dT, ddT = _ritz_trial(n_trial, s)
+    A0, A1, A2 = (T * w) @ T.T, (dT * w) @ dT.T, (ddT * w) @ ddT.T       # int T_i T_j, T_i' T_j', T_i'' T_j'' on the unit interval
+    # int (u_xx + u_yy)(v_xx + v_yy) with int u_xx v_yy = int u_xy v_xy for clamped trial functions (two integrations by parts)
+    M = Lx * Ly * np.kron(A0, A0)
+    K = Lx * Ly * (np.kron(A2, A0) / Lx ** 4 + 2.0 * np.kron(A1, A1) / (Lx * Ly) ** 2 + np.kron(A0, A2) / Ly ** 4)
+    lam, vec = eigh(K, M)
+    zeta4 = lam[:n_phi]
+    c = vec[:, :n_phi].T.reshape(n_phi, n_trial, n_trial).copy()
+    for n in range(n_phi):
+        k = np.argmax(np.abs(c[n]))
+        if c[n].flat[k] < 0:
+            c[n] = -c[n]
+    return zeta4, c
+
+
+def airy_ritz_eval(c, Lx, Ly, x, y):
+    """Psi_n(x, y) for every n (c from airy_ritz_basis)."""
+    nt = c.shape[1]
+    Tx = _ritz_trial(nt, np.atleast_1d(x / Lx))[0][:, 0]
+    Ty = _ritz_trial(nt, np.atleast_1d(y / Ly))[0][:, 0]
+    return np.einsum("nij,i,j->n", c, Tx, Ty)
+
+
+def H_airy_ritz(Lx, Ly, mq, nq, c, ng=200):
+    """H^n_pq = int Psi_n L(Phi_p, Phi_q) dS (Eq. 10, operator of Eq. 7) for the sine transverse modes
+    (mq, nq) and the Ritz in-plane modes c, by separable Gauss-Legendre quadrature:
+        L(Phi_p, Phi_q) = Phi_p,xx Phi_q,yy + Phi_p,yy Phi_q,xx - 2 Phi_p,xy Phi_q,xy."""
+    mq = np.asarray(mq, float); nq = np.asarray(nq, float)
+    xg, wg = np.polynomial.legendre.leggauss(ng)
+    s, w = 0.5 * (xg + 1.0), 0.5 * wg
+    nt = c.shape[1]
+    T = _ritz_trial(nt, s)[0]                                               # [nt][ng]
+    sx, cx = np.sin(np.pi * mq[:, None] * s), np.cos(np.pi * mq[:, None] * s)   # transverse factors on the unit interval
+    sy, cy = np.sin(np.pi * nq[:, None] * s), np.cos(np.pi * nq[:, None] * s)
+    # 1-D integrals  int T_i sin sin  and  int T_i cos cos   -> [nt][Nq][Nq]
+    SSx = np.einsum("ig,pg,qg,g->ipq", T, sx, sx, w); CCx = np.einsum("ig,pg,qg,g->ipq", T, cx, cx, w)
+    SSy = np.einsum("jg,pg,qg,g->jpq", T, sy, sy, w); CCy = np.einsum("jg,pg,qg,g->jpq", T, cy, cy, w)
+    ax, ay = np.pi * mq / Lx, np.pi * nq / Ly                               # wavenumbers
+    # Phi = (2 / sqrt(Lx Ly)) sin sin; dS = Lx Ly ds dt
+    pref = 4.0 / (Lx * Ly) * Lx * Ly
+    A = (ax[:, None] ** 2) * (ay[None, :] ** 2)                              # Phi_p,xx Phi_q,yy -> a_xp^2 a_yq^2 (signs cancel)
+    Bc = (ax * ay)[:, None] * (ax * ay)[None, :]
+    H = np.empty((c.shape[0], len(mq), len(mq)))
+    for n in range(c.shape[0]):
+        Sx = np.einsum("ij,ipq->jpq", c[n], SSx); Cx = np.einsum("ij,ipq->jpq", c[n], CCx)
+        t1 = np.einsum("jpq,jpq->pq", Sx, SSy)                              # sum_ij c_ij SSx_i SSy_j
+        t2 = np.einsum("jpq,jpq->pq", Cx, CCy)
+        H[n] = pref * ((A + A.T) * t1 - 2.0 * Bc * t2)
+    return H

@@ -19,7 +19,8 @@ LINEAR, TENSION, VK = 0, 1, 2
 SV, FTM = 0, 1
 STRING, RECT = 0, 1
 (Q_MODE_M, Q_MODE_N, Q_PHI_M, Q_PHI_N, Q_LAMBDA, Q_OMEGA, Q_SIGMA, Q_NL_SCALE, Q_PICKUP, Q_ACTIVE,
- Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO, Q_TILE_STATS, Q_MMA_LAYOUT, Q_MMA_SLAB_CHECK) = range(16)
+ Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO, Q_TILE_STATS, Q_MMA_LAYOUT, Q_MMA_SLAB_CHECK, Q_AIRY_ZETA4) = range(17)
+AIRY_SINE, AIRY_CLAMPED_RITZ = 0, 1
 
 _dp = C.POINTER(C.c_double)
 _fp = C.POINTER(C.c_float)
@@ -54,7 +55,7 @@ class SampleGeom(C.Structure):
 
 
 EXPORTS = ["modal_plan_create", "modal_coeffs_upload", "modal_simulate", "modal_simulate_host",
-           "modal_plan_check", "modal_plan_set_option", "modal_plan_destroy", "modal_last_error",
+           "modal_plan_check", "modal_plan_set_option", "modal_plan_set_airy_basis", "modal_plan_destroy", "modal_last_error",
            "modal_plan_query", "modal_derive_coeffs", "modal_project_bump", "modal_measure_peaks"]
 
 if not os.path.exists(LIB_PATH):
@@ -67,6 +68,7 @@ lib.modal_simulate.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(Init), C.
 lib.modal_simulate_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(Init), _fp, _ip]
 lib.modal_plan_check.argtypes = [C.c_void_p, _ip]
 lib.modal_plan_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int]
+lib.modal_plan_set_airy_basis.argtypes = [C.c_void_p, C.c_int, C.c_int]
 lib.modal_plan_destroy.argtypes = [C.c_void_p]
 lib.modal_plan_destroy.restype = None
 lib.modal_last_error.argtypes = [C.c_void_p]
@@ -163,6 +165,9 @@ class Plan:
         self._check(st, allow=(EUNSTABLE,))
         return st, fb
 
+    def set_airy_basis(self, basis: int, n_trial: int = 0):
+        return self._check(lib.modal_plan_set_airy_basis(self._h, int(basis), int(n_trial)))
+
     def set_option(self, key: str, value: int):
         return self._check(lib.modal_plan_set_option(self._h, key.encode(), int(value)))
 
@@ -190,7 +195,8 @@ class Plan:
             Q_NL_SCALE: ((cb, nnl), np.float64), Q_PICKUP: ((cb, nq), np.float64),
             Q_ACTIVE: ((cb, nq), np.int32), Q_H_FULL: ((nphi, nq, nq), np.float64),
             Q_COEFF_BATCH: ((1,), np.int32), Q_KERNEL_INFO: ((8,), np.int32), Q_TILE_STATS: ((2,), np.int32),
-            Q_MMA_LAYOUT: ((16,), np.int32), Q_MMA_SLAB_CHECK: ((3,), np.float64)}[what]
+            Q_MMA_LAYOUT: ((16,), np.int32), Q_MMA_SLAB_CHECK: ((3,), np.float64),
+            Q_AIRY_ZETA4: ((nphi,), np.float64)}[what]
         a = np.zeros(shape, dt)
         self._check(lib.modal_plan_query(self._h, what, a.ctypes.data_as(C.c_void_p), a.nbytes))
         return a

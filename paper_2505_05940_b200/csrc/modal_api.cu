@@ -81,6 +81,8 @@ struct modal_plan {
     // internal (device) order of the transverse modes: perm[k_internal] = k_user.  VK plates group the modes by index
     // parity (m mod 2, n mod 2): H^n couples only parity classes c and c xor delta_n, so whole 16x16 tiles vanish.
     std::vector<int> perm, iperm;
+    int airy_basis = 0;                                               // modal_airy_basis
+    std::vector<double> zeta4;                                        // [n_phi] of the reference geometry
     bool coeffs_dirty = true, H_dirty = true;
     std::string err;
     int sm_count = 148;
@@ -798,6 +800,8 @@ extern "C" modal_status modal_plan_create(const modal_plan_desc *desc, int cuda_
             return geom * mh::H_bracket(q.m[a], q.n[a], q.m[b], q.n[b], f.m[n], f.n[n]);
         };
         set_H(p, get);
+        p->zeta4.resize(d.n_phi);
+        for (int n = 0; n < d.n_phi; ++n) p->zeta4[n] = p->mphi.lambda[n] * p->mphi.lambda[n];      // reading R5
     }
     if (cuda_device >= 0) {
         cudaError_t e = cudaSetDevice(cuda_device);
@@ -947,6 +951,45 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
     return MODAL_EINVAL;
 }
 
+extern "C" modal_status modal_plan_set_airy_basis(modal_plan *p, int basis, int n_trial)
+{
+    if (!p) return MODAL_EINVAL;
+    p->err.clear();
+    const modal_plan_desc &d = p->d;
+    if (d.model != MODAL_VK) { p->err = "the in-plane basis belongs to MODAL_VK plans\n"; return MODAL_EINVAL; }
+    if ((basis != MODAL_AIRY_SINE && basis != MODAL_AIRY_CLAMPED_RITZ) || n_trial < 0 || n_trial > 64) {
+        p->err = "basis must be MODAL_AIRY_SINE or MODAL_AIRY_CLAMPED_RITZ, n_trial in [0, 64]\n"; return MODAL_EINVAL;
+    }
+    const int nphi = d.n_phi;
+    const mh::ModeSet &q = p->mq;
+    if (basis == MODAL_AIRY_SINE) {
+        const double geom = mh::H_geom(d.Lx, d.Ly);
+        const mh::ModeSet &f = p->mphi;
+        set_H(p, [&](int n, int a, int b) { return geom * mh::H_bracket(q.m[a], q.n[a], q.m[b], q.n[b], f.m[n], f.n[n]); });
+        for (int n = 0; n < nphi; ++n) p->zeta4[n] = f.lambda[n] * f.lambda[n];
+    } else {
+        // trial functions per axis: enough for the n_phi lowest modes with a margin (the highest kept mode has ~sqrt(n_phi) half-waves per axis)
+        int nt = n_trial > 0 ? n_trial : std::max(12, 2 * (int)std::ceil(std::sqrt(1.5 * nphi * std::max(d.Lx / d.Ly, d.Ly / d.Lx))) + 6);
+        nt = std::min(nt, 64);
+        mh::AiryRitz R;
+        if (nt * nt < nphi || !mh::airy_ritz_basis(d.Lx, d.Ly, nphi, nt, R)) {
+            p->err = "Rayleigh-Ritz Airy basis: too few trial functions for n_phi, or the mass matrix is not positive definite\n";
+            return MODAL_EINCOMPAT;
+        }
+        set_H(p, [&](int n, int a, int b) {
+            return mh::airy_ritz_H_entry(nt, &R.c[(size_t)n * nt * nt], d.Lx, d.Ly, q.m[a], q.n[a], q.m[b], q.n[b]);
+        });
+        p->zeta4 = R.zeta4;
+    }
+    p->airy_basis = basis;
+    for (int b = 0; b < p->coeff_batch; ++b)
+        for (int n = 0; n < nphi; ++n) p->nl_scale[(size_t)b * nphi + n] = d.E / (2.0 * d.rho * p->zeta4[n]);
+    p->coeffs_dirty = true;
+    modal_status s = sync_coeffs(p);
+    if (s == MODAL_OK && p->H_dirty) s = sync_H(p);
+    return s;
+}
+
 extern "C" void modal_plan_destroy(modal_plan *p)
 {
     if (!p) return;
@@ -1033,6 +1076,7 @@ extern "C" modal_status modal_plan_query(const modal_plan *p, int what, void *ds
             }
             return put(out, sizeof out);
         }
+        case MODAL_Q_AIRY_ZETA4: return d.model == MODAL_VK ? put(p->zeta4.data(), p->zeta4.size() * 8) : MODAL_EINVAL;
         case MODAL_Q_H_FULL: {
             if (d.model != MODAL_VK) return MODAL_EINVAL;
             const size_t bytes = (size_t)d.n_phi * nq * nq * 8;

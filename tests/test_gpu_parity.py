@@ -424,6 +424,31 @@ def test_vk_flow_kernel_with_external_force():
     assert np.all(peak > 0) and np.all(np.max(np.abs(gpu - ref0["out"]), axis=1) <= TOL_MAX * peak)
 
 
+@pytest.mark.parametrize("n_q,n_phi,batch,impl", [(10, 10, 1, 1), (57, 23, 2, 1), (57, 23, 130, 2)])
+def test_airy_ritz_basis_parity(n_q, n_phi, batch, impl):
+    """SURVEY.md 8(f) row 2, reading R16: the plate with the clamped Rayleigh-Ritz in-plane basis -- the PLAN derives H and zeta
+    (modal_plan_set_airy_basis, closed-form route), the oracle derives them by quadrature, and the time loops are compared.
+    Same plate for every sample (the Ritz tensor does not follow the geometry law of R14 across aspect ratios)."""
+    torch, mb = _mods()
+    n_steps = 2000 if batch < 64 else 500
+    wl = wlmod.c4(batch=batch, n_steps=n_steps)
+    wl["n_q"], wl["n_phi"], wl["airy"], wl["n_trial"] = n_q, n_phi, "ritz", 12
+    wl["A"] = np.minimum(wl["A"], 1.5 * wl["h"])
+    plan, q0 = mb.plan_from_workload(wl, 0, options=dict(vk_impl=impl))
+    plan.set_airy_basis(mb.AIRY_CLAMPED_RITZ, 12)
+    gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
+    assert st == 0 and np.all(fb == -1) and plan.query(mb.Q_KERNEL_INFO)[0] == (3 if impl == 1 else 4)
+    sub = list(range(batch)) if batch <= 8 else [0, 31, 64, 127, 129]
+    case = orc.assemble(wl, samples=sub)
+    ref = orc.run_case(case, n_steps)
+    check_parity(gpu[sub], ref["out"], case, first=n_steps)
+    # and it is not the sine-basis plate: the two readings give different audio at these amplitudes
+    plan.set_airy_basis(mb.AIRY_SINE)
+    gpu_sine, _, _, _ = gpu_run(plan, q0, None, n_steps)
+    strong = int(np.argmax(wl["A"][sub]))
+    assert np.max(np.abs(gpu_sine[sub][strong] - gpu[sub][strong])) > 1e-3 * np.max(np.abs(gpu[sub][strong]))
+
+
 # ------------------------------------------------------------------ tension / linear ----
 @pytest.mark.parametrize("batch,n_steps", [(32, 4096), (5, 333)])
 def test_c1_string_parity(batch, n_steps):

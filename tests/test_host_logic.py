@@ -265,3 +265,26 @@ def test_batched_kernel_layout_dense_uploaded_H():
     covered, nonzero, err = plan.query(mb.Q_MMA_SLAB_CHECK)
     assert L[0] == 1 and L[12] == L[13] == L[8]          # fewest == most K chunks == all chunks
     assert covered == nonzero == 12 * 48 * 48 and err <= 2.0 ** -16
+
+
+def test_airy_ritz_basis_library_matches_oracle():
+    """SURVEY.md 8(f) row 2 / reading R16: the library's clamped Airy basis (closed-form integrals, symmetry-class Cholesky +
+    Jacobi) against the oracle's (Gauss-Legendre quadrature, LAPACK): zeta^4, the coupling tensor the device holds, nl_scale."""
+    wl = wlmod.c0()
+    wl["n_q"], wl["n_phi"], wl["airy"], wl["n_trial"] = 30, 14, "ritz", 12
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    H_sine = plan.query(mb.Q_H_FULL)
+    plan.set_airy_basis(mb.AIRY_CLAMPED_RITZ, 12)
+    case = orc.assemble(wl)
+    z4, _ = orc.airy_ritz_basis(0.6, 0.4, 14, n_trial=12)
+    assert np.allclose(plan.query(mb.Q_AIRY_ZETA4), z4, rtol=1e-10)
+    H = plan.query(mb.Q_H_FULL)
+    assert np.max(np.abs(H - case.H)) <= 2e-7 * np.abs(case.H).max()           # both rounded to fp32 from values that agree to 1e-10
+    assert np.allclose(plan.query(mb.Q_NL_SCALE)[0], wl["E"] / (2 * wl["rho"] * z4), rtol=1e-10)
+    assert np.max(np.abs(H - H_sine)) > 0.1 * np.abs(H_sine).max()             # it IS another tensor
+    tiles, nz = plan.query(mb.Q_TILE_STATS)
+    assert nz < tiles                                                           # reflection symmetry still empties whole tiles
+    plan.set_airy_basis(mb.AIRY_SINE)
+    assert np.array_equal(plan.query(mb.Q_H_FULL), H_sine)
+    with pytest.raises(mb.ModalError):
+        plan.set_airy_basis(mb.AIRY_CLAMPED_RITZ, 3)                            # 9 trial functions < 14 modes

@@ -503,3 +503,94 @@ def test_ftm_refuses_overdamped_modes():
         orc.scheme_coeffs(orc.FTM, om, ga, T, np.ones(3, bool))
     orc.scheme_coeffs(orc.FTM, om, ga, T, np.array([True, False, True]))     # a masked mode is not asked for coefficients
     orc.scheme_coeffs(orc.SV, om, ga, T)                                      # SV proceeds
+
+
+# ---------------------------------- in-plane basis of reading R16: clamped (Airy) modes by Rayleigh-Ritz ----
+def _ritz_fields(c_n, Lx, Ly, x, y):
+    """Psi, Psi_xx, Psi_yy, Psi_xy of one mode on the tensor grid x (x) y, from the trial functions' own derivatives."""
+    nt = c_n.shape[0]
+    Tx, dTx, ddTx = orc._ritz_trial(nt, x / Lx)
+    Ty, dTy, ddTy = orc._ritz_trial(nt, y / Ly)
+    f = lambda a, b: np.einsum("ij,ig,jh->gh", c_n, a, b)
+    return f(Tx, Ty), f(ddTx, Ty) / Lx ** 2, f(Tx, ddTy) / Ly ** 2, f(dTx, dTy) / (Lx * Ly)
+
+
+def test_airy_ritz_square_plate_textbook_value_and_upper_bounds():
+    """Clamped square plate: the fundamental frequency parameter zeta_1^2 L^2 is 35.99 in the textbooks (35.985 to five
+    figures); Rayleigh-Ritz values are upper bounds that can only fall when the trial space grows."""
+    prev = None
+    for nt in (4, 8, 12, 16):
+        z4, _ = orc.airy_ritz_basis(1.0, 1.0, 4, n_trial=nt)
+        lam = np.sqrt(z4)
+        assert lam[0] >= 35.985
+        if prev is not None:
+            assert np.all(lam <= prev * (1 + 1e-12))
+        prev = lam
+    assert prev[0] < 35.995 and abs(prev[1] - prev[2]) < 1e-6 * prev[1]          # 35.99; modes (2,1) / (1,2) degenerate on the square
+    assert abs(prev[1] - 73.40) < 0.05 and abs(prev[3] - 108.22) < 0.15            # 73.39, 108.2 in the same tables
+    # scaling: zeta^4 ~ L^-4 at fixed aspect
+    za, _ = orc.airy_ritz_basis(0.6, 0.4, 5, n_trial=10)
+    zb, _ = orc.airy_ritz_basis(1.2, 0.8, 5, n_trial=10)
+    assert np.allclose(za, 16.0 * zb, rtol=1e-10)
+
+
+def test_airy_ritz_modes_orthonormal_clamped_and_weakly_biharmonic():
+    """By 2-D Gauss-Legendre quadrature of the evaluated functions (not the Kronecker assembly): the modes are orthonormal,
+    vanish with their normal slope on the edges, and satisfy the weak eigen-equation  int Lap Psi Lap v = zeta^4 int Psi v
+    against every trial function v; the Rayleigh quotient with int (Lap Psi)^2 gives zeta^4 back."""
+    Lx, Ly, nt = 0.6, 0.4, 10
+    z4, c = orc.airy_ritz_basis(Lx, Ly, 6, n_trial=nt)
+    xg, wg = np.polynomial.legendre.leggauss(96)
+    x, wx = 0.5 * Lx * (xg + 1), 0.5 * Lx * wg
+    y, wy = 0.5 * Ly * (xg + 1), 0.5 * Ly * wg
+    W = wx[:, None] * wy[None, :]
+    F = [_ritz_fields(c[n], Lx, Ly, x, y) for n in range(6)]
+    gram = np.array([[np.sum(W * F[a][0] * F[b][0]) for b in range(6)] for a in range(6)])
+    assert np.allclose(gram, np.eye(6), atol=1e-9)
+    for n in range(6):
+        lap = F[n][1] + F[n][2]
+        assert abs(np.sum(W * lap * lap) / z4[n] - 1.0) < 1e-8
+        for (i, j) in ((1, 1), (2, 3), (5, 2)):                                   # a few trial functions as test functions
+            e = np.zeros((nt, nt)); e[i - 1, j - 1] = 1.0
+            v, vxx, vyy, _ = _ritz_fields(e, Lx, Ly, x, y)
+            lhs, rhs = np.sum(W * lap * (vxx + vyy)), z4[n] * np.sum(W * F[n][0] * v)
+            assert abs(lhs - rhs) <= 1e-7 * (abs(lhs) + abs(rhs)) + 1e-6 * np.sqrt(z4[n])
+    # boundary: value and normal derivative (finite difference of the evaluated function)
+    h = 1e-6
+    for n in range(6):
+        for yy in (0.07, 0.21, 0.33):
+            assert abs(orc.airy_ritz_eval(c, Lx, Ly, 0.0, yy)[n]) < 1e-10 and abs(orc.airy_ritz_eval(c, Lx, Ly, Lx, yy)[n]) < 1e-9
+            assert abs(orc.airy_ritz_eval(c, Lx, Ly, h, yy)[n]) / h < 1e-3 * np.abs(F[n][0]).max()
+        assert abs(orc.airy_ritz_eval(c, Lx, Ly, 0.3, h)[n]) / h < 1e-3 * np.abs(F[n][0]).max()
+
+
+def test_H_airy_ritz_vs_bruteforce_quadrature_symmetry_and_HC_identity():
+    """Eq. 10 by brute-force 2-D quadrature of Psi_n L(Phi_p, Phi_q) (operator of Eq. 7 through orc.vk_operator) against the
+    separable evaluation; symmetry in (p, q); and Eq. 11: C^s_{p,n} = int Phi_s L(Phi_p, Psi_n) equals H^n_{p,s},
+    which holds because Psi and its normal slope vanish on the edges."""
+    Lx, Ly, nt = 0.6, 0.4, 8
+    z4, c = orc.airy_ritz_basis(Lx, Ly, 5, n_trial=nt)
+    mq, nq, _ = orc.rect_modes(Lx, Ly, 6)
+    H = orc.H_airy_ritz(Lx, Ly, mq, nq, c)
+    assert np.max(np.abs(H - H.transpose(0, 2, 1))) <= 1e-9 * np.abs(H).max()
+    xg, wg = np.polynomial.legendre.leggauss(72)
+    x, wx = 0.5 * Lx * (xg + 1), 0.5 * Lx * wg
+    y, wy = 0.5 * Ly * (xg + 1), 0.5 * Ly * wg
+    W = wx[:, None] * wy[None, :]
+    amp = 2.0 / np.sqrt(Lx * Ly)
+
+    def phi(k):     # value, xx, yy, xy of transverse sine mode k on the grid
+        ax, ay = mq[k] * np.pi / Lx, nq[k] * np.pi / Ly
+        sx, cx, sy, cy = np.sin(ax * x)[:, None], np.cos(ax * x)[:, None], np.sin(ay * y)[None, :], np.cos(ay * y)[None, :]
+        return amp * sx * sy, -amp * ax ** 2 * sx * sy, -amp * ay ** 2 * sx * sy, amp * ax * ay * cx * cy
+
+    vkop = np.vectorize(orc.vk_operator)
+    for (n, p, q) in ((0, 0, 0), (0, 1, 1), (1, 0, 1), (2, 3, 0), (4, 5, 2), (3, 2, 2)):
+        psi, pxx, pyy, pxy = _ritz_fields(c[n], Lx, Ly, x, y)
+        fp, fq = phi(p), phi(q)
+        brute = np.sum(W * psi * vkop(fp[1], fp[2], fp[3], fq[1], fq[2], fq[3]))
+        assert abs(brute - H[n, p, q]) <= 1e-7 * np.abs(H).max(), (n, p, q, brute, H[n, p, q])
+        c_spn = np.sum(W * fq[0] * vkop(fp[1], fp[2], fp[3], pxx, pyy, pxy))        # s = q: C^q_{p,n}
+        assert abs(c_spn - H[n, p, q]) <= 1e-6 * np.abs(H).max(), (n, p, q, c_spn, H[n, p, q])
+    # reflection symmetry of the rectangle: ~3/4 of the entries vanish, as for the sine basis
+    assert 0.2 < np.mean(np.abs(H) > 1e-9 * np.abs(H).max()) < 0.3
