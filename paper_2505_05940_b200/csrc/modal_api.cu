@@ -13,9 +13,11 @@
 #include "host_math.hpp"
 #include "flow_schedule.hpp"
 #include "mma_schedule.hpp"
+#include "stream_schedule.hpp"
 #include "kernels.cuh"
 #include "vk_flow.cuh"
 #include "vk_mma.cuh"
+#include "vk_stream.cuh"
 #include "peaks.cuh"
 
 namespace mh = modal_host;
@@ -60,6 +62,14 @@ struct MmaConfig {
     DevBuf dslabs, dtab, dQop, dqf, dGx, dfx, dflags, dpx;
 };
 
+struct StreamConfig {                // vk_stream: layout for one NB (samples of a launch, padded to 16)
+    bool ok = false;
+    int NB = 0, lpq = 1;
+    mh::StreamLayout L;
+    size_t off_cta = 0, off_tile = 0, off_blk = 0, off_nct = 0;
+    DevBuf dA, dtab, dqx, dGx, dfx, dpx;
+};
+
 struct Options {                     // modal_plan_set_option
     int vk_impl = 0, flow_g = 0, flow_ns = 0, flow_res = -1, mma_split = 0, mma_ng = 0, mma_nstg = 0, mma_cluster = 1, parity_order = 1, timing = 0;
 };
@@ -89,6 +99,7 @@ struct modal_plan {
     // device storage
     DevBuf dHf, dfx, dgx, dqx, dtiming, dperm, dtimeout;
     MmaConfig mma;
+    StreamConfig stream;
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dkv, dkq, dr, dast, ds, dsT, dw, dlam, dc, dq0, dv0, dgain, dbad, dout;      // dsT: s_n transposed [n_phi][coeff_batch] (batched kernel)
     float *pinned_out = nullptr; size_t pinned_bytes = 0;            // staging of modal_simulate_host
@@ -142,7 +153,7 @@ void set_H(modal_plan *p, Get get_user)
     }
     for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
     p->flow_cfgs.clear();                                   // schedules depend on the zero pattern
-    p->mma.tried = false; p->mma.ok = false;
+    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0;
     p->H_dirty = true;
 }
 
@@ -292,7 +303,7 @@ modal_status sync_H(modal_plan *p)
         CU(cudaMemcpy(p->dHf.p, p->Hf.data(), p->Hf.size() * 4, cudaMemcpyHostToDevice));
         CU(p->dperm.ensure(p->perm.size() * 4));
         CU(cudaMemcpy(p->dperm.p, p->perm.data(), p->perm.size() * 4, cudaMemcpyHostToDevice));
-        p->mma.tried = false; p->mma.ok = false;            // operand slabs are rebuilt from the new H on demand
+        p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0;            // operand slabs are rebuilt from the new H on demand
     }
     p->H_dirty = false;
     return MODAL_OK;
@@ -490,6 +501,69 @@ modal_status configure_mma(modal_plan *p)
     return MODAL_OK;
 }
 
+// ---- vk_stream (streaming tensor-core kernel for small / medium batches on a large tensor) -----------------
+modal_status configure_stream(modal_plan *p, int NB)
+{
+    StreamConfig &m = p->stream;
+    if (m.NB == NB) return MODAL_OK;
+    m.NB = NB; m.ok = false;
+    if (p->d.model != MODAL_VK) return MODAL_OK;
+    const int nq = p->d.n_q;
+    const bool classes = p->d.geom == MODAL_RECT && p->opt.parity_order;
+    auto cls_q = [&](int k_int) { const int k = p->perm[k_int]; return classes ? (p->mq.m[k] & 1) * 2 + (p->mq.n[k] & 1) : 0; };
+    std::vector<int> class_start{0};
+    for (int k = 1; k < nq; ++k) if (cls_q(k) != cls_q(k - 1)) class_start.push_back(k);
+    class_start.push_back(nq);
+    const std::vector<float> &Hf = p->Hf;
+    const int tpn = mh::flow_tiles_per_n(nq);
+    auto nz = [&](int n, int a, int b) -> bool {
+        const int hi = std::max(a, b), lo = std::min(a, b), I = hi / 16, J = lo / 16;
+        const size_t tile = (size_t)n * tpn + I * (I + 1) / 2 + J;
+        return p->tile_nz[tile] && Hf[tile * 256 + mh::flow_elem(hi % 16, lo % 16)] != 0.f;
+    };
+    auto get = [&](int n, int a, int b) -> double {
+        const int hi = std::max(a, b), lo = std::min(a, b), I = hi / 16, J = lo / 16;
+        const float t = Hf[((size_t)n * tpn + I * (I + 1) / 2 + J) * 256 + mh::flow_elem(hi % 16, lo % 16)];
+        return hi == lo ? 2.0 * (double)t : (double)t;
+    };
+    if (!mh::stream_layout(nq, p->d.n_phi, p->sm_count, NB, class_start, nz, m.L)) return MODAL_OK;
+    const mh::StreamLayout &L = m.L;
+    if (md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 4).total > SMEM_LIMIT) return MODAL_OK;
+    std::vector<uint16_t> A;
+    mh::pack_stream_A(L, get, A);
+    CU(m.dA.ensure(A.size() * 2));
+    CU(cudaMemcpy(m.dA.p, A.data(), A.size() * 2, cudaMemcpyHostToDevice));
+    std::vector<int> tab;
+    auto add = [&](const std::vector<int> &v) { const size_t o = tab.size(); tab.insert(tab.end(), v.begin(), v.end()); return o; };
+    m.off_cta = add(L.cta_tab); m.off_tile = add(L.tile_tab);
+    std::vector<int> blk;
+    for (int j = 0; j < L.NKB; ++j) { blk.push_back(L.blocks[j].k0); blk.push_back(L.blocks[j].nb); blk.push_back(L.blocks[j].koff); blk.push_back(L.blk_cta0[j]); }
+    m.off_blk = add(blk); m.off_nct = add(L.blk_nctas);
+    CU(m.dtab.ensure(tab.size() * 4));
+    CU(cudaMemcpy(m.dtab.p, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice));
+    // owner gather: lanes per item so that no lane has more than 12 strong loads in flight
+    const int nct = *std::max_element(L.blk_nctas.begin(), L.blk_nctas.end());
+    m.lpq = nct <= 12 ? 1 : nct <= 24 ? 2 : nct <= 48 ? 4 : 8;
+    m.ok = true;
+    return MODAL_OK;
+}
+
+template <int NB>
+cudaError_t launch_stream(const md::StreamArgs &a, size_t smem, bool timing, cudaStream_t st)
+{
+    cudaError_t e;
+    if (timing) {
+        e = cudaFuncSetAttribute(md::vk_stream_kernel<NB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        md::vk_stream_kernel<NB, true><<<a.G, md::ST_THREADS, smem, st>>>(a);
+    } else {
+        e = cudaFuncSetAttribute(md::vk_stream_kernel<NB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        md::vk_stream_kernel<NB, false><<<a.G, md::ST_THREADS, smem, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
 template <int MPL>
 cudaError_t launch_tension(const md::TensionArgs &a, cudaStream_t st)
 {
@@ -561,6 +635,19 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
     const int auto_start = init->qm1 ? 0 : 1;
     const double half_T2 = 0.5 * p->T * p->T;
 
+    // vK kernel family: the batched tensor-core kernel when H fits the shared memory of the GPU (batch >= 64), the streaming
+    // tensor-core kernel when it does not (batch >= 8), else the FP32 flow kernel; "vk_impl" forces one
+    bool use_mma = false, use_stream = false;
+    if (d.model == MODAL_VK) {
+        const int impl = p->opt.vk_impl;
+        if ((impl == 0 && batch >= 64) || impl == 2) { modal_status s = configure_mma(p); if (s != MODAL_OK) return s; use_mma = p->mma.ok; }
+        if (!use_mma && ((impl == 0 && batch >= 8) || impl == 3)) {
+            const int NB = batch <= 16 ? 16 : batch <= 32 ? 32 : 64;
+            modal_status s = configure_stream(p, NB); if (s != MODAL_OK) return s;
+            use_stream = p->stream.ok;
+            if (impl == 3 && !use_stream) { p->err += "vk_impl=3: the streaming kernel has no layout for this plan\n"; return MODAL_EINCOMPAT; }
+        }
+    }
     if (d.model != MODAL_VK) {
         md::TensionArgs a{};
         a.batch = batch; a.n_steps = n_steps; a.n_modes_pad = P; a.coeff_stride = cb == 1 ? 0 : P;
@@ -593,7 +680,70 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         CU(e);
         p->kinfo[0] = 1; p->kinfo[1] = 1; p->kinfo[2] = (batch + 3) / 4; p->kinfo[3] = 128;
         p->kinfo[4] = 0; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
-    } else if (p->opt.vk_impl != 1 && (p->opt.vk_impl == 2 || batch >= 64) && configure_mma(p) == MODAL_OK && p->mma.ok) {
+    } else if (use_stream) {
+        StreamConfig &m = p->stream;
+        const mh::StreamLayout &L = m.L;
+        const int NB = m.NB;
+        const size_t base = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 0).total;
+        int nstg = (int)std::min<size_t>(md::ST_NSTG_MAX, (SMEM_LIMIT - base) / 8192);
+        if (p->opt.mma_nstg > 0) nstg = std::min(nstg, std::max(p->opt.mma_nstg, L.tiles_max));
+        if (nstg < L.tiles_max) { p->err += "streaming vK kernel: no room for the operand ring (one stage per tile of a CTA)\n"; return MODAL_EINCOMPAT; }
+        const size_t smem = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, nstg).total;
+        const int KOP = L.KC * 16;
+        const size_t nqx = (size_t)NB * KOP * 4, nGx = (size_t)d.n_phi * L.NKB * NB * 4, nfx = (size_t)L.G * 128 * NB * 4, npx = (size_t)4 * L.G * NB * 16;
+        CU(m.dqx.ensure(nqx)); CU(m.dGx.ensure(nGx)); CU(m.dfx.ensure(nfx)); CU(m.dpx.ensure(npx));
+        const bool timing = p->opt.timing != 0;
+        for (int b0 = 0; b0 < batch; b0 += NB) {
+            const int nb = std::min(NB, batch - b0);
+            md::StreamArgs a{};
+            const int *tab = m.dtab.as<int>();
+            a.A = m.dA.as<uint16_t>(); a.cta_tab = tab + m.off_cta; a.tile_tab = tab + m.off_tile; a.tile_stride = L.TILE_STRIDE;
+            a.blk = tab + m.off_blk; a.blk_nctas = tab + m.off_nct;
+            a.NKB = L.NKB; a.KOP = KOP; a.G = L.G; a.NSTG = nstg; a.rows_max = L.rows_max; a.bch_max = L.bch_max; a.LPQ = m.lpq;
+            a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P; a.batch = nb; a.n_steps = n_steps;
+            a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
+            const size_t oq = cb == 1 ? 0 : (size_t)b0 * P;
+            a.kv = p->dkv.as<double>() + oq; a.kq = p->dkq.as<double>() + oq; a.r = p->dr.as<double>() + oq; a.astart = p->dast.as<double>() + oq;
+            a.s = p->ds.as<float>() + (cb == 1 ? 0 : (size_t)b0 * d.n_phi); a.w = p->dw.as<float>() + oq;
+            a.q0 = p->dq0.as<double>() + (size_t)b0 * P; a.v0 = p->dv0.as<double>() + (size_t)b0 * P;
+            a.auto_start = auto_start; a.half_T2 = half_T2;
+            a.fext = init->fext_signal ? init->fext_signal + (size_t)b0 * n_steps : nullptr;
+            a.gain = init->fext_signal ? p->dgain.as<double>() + (size_t)b0 * P : nullptr;
+            a.out = out_dev + (size_t)b0 * n_steps;
+            a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr; a.kperm = p->dperm.as<int>();
+            a.first_bad = p->dbad.as<int>() + b0;
+            // exchange buffers (L2 resident); everything starts at tag / epoch 0 (the first step uses 1)
+            CU(cudaMemsetAsync(m.dqx.p, 0, nqx, st)); CU(cudaMemsetAsync(m.dGx.p, 0, nGx, st));
+            CU(cudaMemsetAsync(m.dfx.p, 0, nfx, st)); CU(cudaMemsetAsync(m.dpx.p, 0, npx, st));
+            a.qx = m.dqx.as<uint32_t>(); a.Gx = m.dGx.as<uint32_t>(); a.fx = m.dfx.as<uint32_t>(); a.px = m.dpx.as<unsigned long long>();
+            a.timeout_flag = p->dtimeout.as<int>();
+            if (timing) {
+                CU(p->dtiming.ensure((size_t)L.G * 128));
+                CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)L.G * 128, st));
+                a.timing = p->dtiming.as<long long>();
+            }
+            persistent = true;
+            CU(NB == 16 ? launch_stream<16>(a, smem, timing, st) : NB == 32 ? launch_stream<32>(a, smem, timing, st) : launch_stream<64>(a, smem, timing, st));
+            if (timing) {
+                CU(cudaStreamSynchronize(st));
+                std::vector<long long> tm((size_t)L.G * 16);
+                CU(cudaMemcpy(tm.data(), p->dtiming.p, tm.size() * 8, cudaMemcpyDeviceToHost));
+                double acc[16] = {0};
+                for (size_t x = 0; x < tm.size(); ++x) acc[x & 15] += (double)tm[x];
+                const double den = (double)L.G * n_steps;
+                double mx[16] = {0}; int amx[16] = {0};
+                for (size_t x = 0; x < tm.size(); ++x) if ((double)tm[x] > mx[x & 15]) { mx[x & 15] = (double)tm[x]; amx[x & 15] = (int)(x >> 4); }
+                static const char *names[16] = {"E q operand (wait + build)", "E own rows", "E wait acc", "E epi1 (all tiles, incl. wait)", "E G wait (sentinels)", "E epi2 (incl. G wait)",
+                                                "E f store", "E q seen (sentinels) after", "O gather", "O update + publish", "O barrier + pickup", "O wait for own E", "M step's MMAs", "M waiting for H chunks", "own f stored -> forces gathered", ""};
+                fprintf(stderr, "[modal stream timing] G=%d NB=%d blocks=%d tiles/CTA<=%d chunks/CTA<=%d rows/CTA<=%d ring=%d lpq=%d  cycles/step: mean over CTAs | max (CTA)\n",
+                        L.G, NB, L.NKB, L.tiles_max, L.bch_max, L.rows_max, nstg, m.lpq);
+                for (int x = 0; x < 16; ++x)
+                    if (names[x][0]) fprintf(stderr, "   %-32s %8.0f | %8.0f (%d: %d tiles, block %d)\n", names[x], acc[x] / den, mx[x] / n_steps, amx[x], L.cta_ntiles[amx[x]], L.cta_block[amx[x]]);
+            }
+        }
+        p->kinfo[0] = 5; p->kinfo[1] = L.G; p->kinfo[2] = NB; p->kinfo[3] = md::ST_THREADS;
+        p->kinfo[4] = (int)smem; p->kinfo[5] = 1 | 2; p->kinfo[6] = L.tiles_max; p->kinfo[7] = P;
+    } else if (use_mma) {
         MmaConfig &m = p->mma;
         const mh::MmaLayout &L = m.L;
         // M tiles per launch: as many (<= 8) as leave room for one tile's worth of ring stages beside slab and owner state; a wider batch
@@ -921,7 +1071,7 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
     if (!p || !key) return MODAL_EINVAL;
     p->err.clear();
     struct { const char *name; int *field; int lo, hi; } tab[] = {
-        {"vk_impl", &p->opt.vk_impl, 0, 2}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
+        {"vk_impl", &p->opt.vk_impl, 0, 3}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
         {"flow_res", &p->opt.flow_res, -1, 1 << 20}, {"mma_split", &p->opt.mma_split, 0, 4}, {"mma_ng", &p->opt.mma_ng, 0, 8},
         {"mma_nstg", &p->opt.mma_nstg, 0, 16}, {"mma_cluster", &p->opt.mma_cluster, 0, 1}, {"parity_order", &p->opt.parity_order, 0, 1}, {"timing", &p->opt.timing, 0, 1}};
     for (auto &t : tab)
@@ -945,6 +1095,7 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
                 p->coeffs_dirty = true;
             }
             if (t.field == &p->opt.mma_split || t.field == &p->opt.mma_ng || t.field == &p->opt.mma_cluster) { p->mma.tried = false; p->mma.ok = false; }
+            if (t.field == &p->opt.parity_order) p->stream.NB = 0;
             return MODAL_OK;
         }
     p->err = std::string("unknown option ") + key + "\n";
@@ -998,7 +1149,8 @@ extern "C" void modal_plan_destroy(modal_plan *p)
         if (p->pending) cudaStreamSynchronize(p->last_stream);
         for (DevBuf *b : {&p->dkv, &p->dkq, &p->dr, &p->dast, &p->ds, &p->dsT, &p->dw, &p->dlam, &p->dc, &p->dq0, &p->dv0, &p->dgain, &p->dbad,
                           &p->dout, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming, &p->dperm, &p->dtimeout, &p->mma.dslabs, &p->mma.dtab,
-                          &p->mma.dQop, &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags, &p->mma.dpx}) b->release();
+                          &p->mma.dQop, &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags, &p->mma.dpx, &p->stream.dA, &p->stream.dtab,
+                          &p->stream.dqx, &p->stream.dGx, &p->stream.dfx, &p->stream.dpx}) b->release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         if (p->pinned_out) cudaFreeHost(p->pinned_out);
     }
