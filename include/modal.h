@@ -129,13 +129,16 @@ modal_status modal_simulate_host(modal_plan *plan, int batch, int n_steps, const
 modal_status modal_plan_check(modal_plan *plan, int *first_bad_step);
 
 /* Launch-selection overrides for tests and sweeps (the defaults are automatic).  Keys:
- *   "vk_impl"      0 automatic, 1 FP32 flow kernel, 2 tcgen05 batched kernel
+ *   "vk_impl"      0 automatic, 1 FP32 flow kernel, 2 tcgen05 batched kernel (H resident in shared memory), 3 tcgen05
+ *                  streaming kernel (H streamed from L2; batch <= 64 per launch, wider batches run as consecutive launches)
  *   "flow_g"       CTAs per team of the flow kernel (0 automatic)
  *   "flow_ns"      TMA ring slots of the flow kernel (0: none, streamed tiles are read directly from L2)
  *   "flow_res"     resident tiles per CTA of the flow kernel (-1 automatic)
  *   "mma_split"    k blocks per mode class of the batched kernel (0 automatic)
  *   "mma_ng"       in-plane modes per CTA of the batched kernel (0 automatic)
- *   "mma_nstg"     operand ring stages of the batched kernel (0 automatic)
+ *   "mma_nstg"     operand ring stages of the batched / streaming kernel (0 automatic)
+ *   "mma_cluster"  1 (default): the CTAs of an n group of the batched kernel form a thread-block cluster and exchange partial G
+ *                  through distributed shared memory when the device keeps all clusters co-resident; 0: through L2
  *   "parity_order" 1 (default): transverse modes grouped by index parity on the device; 0: plan order
  *   "timing"       1: per-phase cycle counters of the persistent kernels, printed to stderr (synchronous)
  * Returns MODAL_EINVAL for an unknown key or a value out of range. */
@@ -169,10 +172,11 @@ typedef enum {
     MODAL_Q_ACTIVE = 9,      /* int    [coeff_batch][n_q]   1 = active, 0 = masked (R11)            */
     MODAL_Q_H_FULL = 10,     /* double [n_phi][n_q][n_q]: the fp32 values the device holds, widened */
     MODAL_Q_COEFF_BATCH = 11,/* int    [1]                                                          */
-    MODAL_Q_KERNEL_INFO = 12,/* int    [8] of the last launch: kernel family (1 tension, 3 flow, 4 batched tcgen05), CTAs */
-                             /*        per team (flow) or CTAs (batched), teams (flow) or n groups (batched), threads,  */
-                             /*        dynamic shared memory bytes, flags (1: H resident in shared memory, 2: team of   */
-                             /*        several CTAs), ring slots (flow) or accumulator slots (batched), padded n_q      */
+    MODAL_Q_KERNEL_INFO = 12,/* int    [8] of the last launch: kernel family (1 tension, 3 flow, 4 batched tcgen05, 5 streaming   */
+                             /*        tcgen05), CTAs per team (flow) or CTAs, teams (flow) / n groups (batched) / samples per  */
+                             /*        launch (streaming), threads, dynamic shared memory bytes, flags (1: H resident in shared */
+                             /*        memory or L2, 2: team of several CTAs), ring slots (flow) / accumulator slots (batched)  */
+                             /*        / most tiles of a CTA (streaming), padded n_q                                            */
     MODAL_Q_MMA_LAYOUT = 14, /* int    [16]: layout the batched tcgen05 kernel would use (host side, no device needed):  */
                              /*        fits, k blocks, n groups, modes per group, TMEM columns per slot, slots, columns */
                              /*        per mode, quads per block, K chunks, most K chunks of a CTA, CTAs, rows owned,   */
@@ -180,6 +184,12 @@ typedef enum {
     MODAL_Q_MMA_SLAB_CHECK = 15, /* double [3]: non-zero entries of H covered by the operand slabs, non-zero entries of */
                              /*        H, max |hi + lo - H| / max |H| (host-side self check of the packing)             */
     MODAL_Q_AIRY_ZETA4 = 16, /* double [n_phi]: zeta_n^4 of the plan's in-plane basis (reference geometry)                    */
+    MODAL_Q_STREAM_LAYOUT = 17, /* int [16]: layout the streaming tcgen05 kernel would use (host side): fits, CTAs, k blocks, */
+                             /*        K chunks of the operand axis, tiles, most / fewest tiles of a CTA, most q chunks of a   */
+                             /*        CTA, most / fewest rows a CTA owns, most K chunks of a tile, chunks in total, stream    */
+                             /*        MiB, most CTAs of a k block, 0, 0                                                       */
+    MODAL_Q_STREAM_CHECK = 18, /* double [4]: non-zero entries of H covered by the H stream, non-zero entries of H,            */
+                             /*        max |hi + lo - H| / max |H|, rows owned in total (== n_q)                               */
     MODAL_Q_TILE_STATS = 13  /* int    [2]: 16x16 tiles of the packed H, and how many hold a non-zero.   */
                              /*        The device keeps the transverse modes grouped by index parity   */
                              /*        (internal order only: every array of this API is in plan order),*/

@@ -502,12 +502,10 @@ modal_status configure_mma(modal_plan *p)
 }
 
 // ---- vk_stream (streaming tensor-core kernel for small / medium batches on a large tensor) -----------------
-modal_status configure_stream(modal_plan *p, int NB)
+// Host part: the layout and the H stream from the fp32 H values the device holds (flow tiles, internal order).
+bool stream_host_layout(const modal_plan *p, int NB, mh::StreamLayout &L)
 {
-    StreamConfig &m = p->stream;
-    if (m.NB == NB) return MODAL_OK;
-    m.NB = NB; m.ok = false;
-    if (p->d.model != MODAL_VK) return MODAL_OK;
+    if (p->d.model != MODAL_VK) return false;
     const int nq = p->d.n_q;
     const bool classes = p->d.geom == MODAL_RECT && p->opt.parity_order;
     auto cls_q = [&](int k_int) { const int k = p->perm[k_int]; return classes ? (p->mq.m[k] & 1) * 2 + (p->mq.n[k] & 1) : 0; };
@@ -521,16 +519,32 @@ modal_status configure_stream(modal_plan *p, int NB)
         const size_t tile = (size_t)n * tpn + I * (I + 1) / 2 + J;
         return p->tile_nz[tile] && Hf[tile * 256 + mh::flow_elem(hi % 16, lo % 16)] != 0.f;
     };
+    return mh::stream_layout(nq, p->d.n_phi, p->sm_count, NB, class_start, nz, L);
+}
+
+void stream_host_A(const modal_plan *p, const mh::StreamLayout &L, std::vector<uint16_t> &A)
+{
+    const std::vector<float> &Hf = p->Hf;
+    const int tpn = mh::flow_tiles_per_n(p->d.n_q);
     auto get = [&](int n, int a, int b) -> double {
         const int hi = std::max(a, b), lo = std::min(a, b), I = hi / 16, J = lo / 16;
         const float t = Hf[((size_t)n * tpn + I * (I + 1) / 2 + J) * 256 + mh::flow_elem(hi % 16, lo % 16)];
         return hi == lo ? 2.0 * (double)t : (double)t;
     };
-    if (!mh::stream_layout(nq, p->d.n_phi, p->sm_count, NB, class_start, nz, m.L)) return MODAL_OK;
+    mh::pack_stream_A(L, get, A);
+}
+
+modal_status configure_stream(modal_plan *p, int NB)
+{
+    StreamConfig &m = p->stream;
+    if (m.NB == NB) return MODAL_OK;
+    m.NB = NB; m.ok = false;
+    if (!stream_host_layout(p, NB, m.L)) return MODAL_OK;
     const mh::StreamLayout &L = m.L;
+    if (L.G * 4 < NB) return MODAL_OK;                   // the pickup warp of a CTA handles at most four samples
     if (md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 4).total > SMEM_LIMIT) return MODAL_OK;
     std::vector<uint16_t> A;
-    mh::pack_stream_A(L, get, A);
+    stream_host_A(p, L, A);
     CU(m.dA.ensure(A.size() * 2));
     CU(cudaMemcpy(m.dA.p, A.data(), A.size() * 2, cudaMemcpyHostToDevice));
     std::vector<int> tab;
@@ -690,7 +704,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         if (nstg < L.tiles_max) { p->err += "streaming vK kernel: no room for the operand ring (one stage per tile of a CTA)\n"; return MODAL_EINCOMPAT; }
         const size_t smem = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, nstg).total;
         const int KOP = L.KC * 16;
-        const size_t nqx = (size_t)NB * KOP * 4, nGx = (size_t)d.n_phi * L.NKB * NB * 4, nfx = (size_t)L.G * 128 * NB * 4, npx = (size_t)4 * L.G * NB * 16;
+        const size_t nqx = (size_t)NB * KOP * 4, nGx = (size_t)d.n_phi * L.NKB * NB * 4, nfx = (size_t)L.G * 128 * NB * 4, npx = (size_t)4 * L.G * NB * 16 + 256;
         CU(m.dqx.ensure(nqx)); CU(m.dGx.ensure(nGx)); CU(m.dfx.ensure(nfx)); CU(m.dpx.ensure(npx));
         const bool timing = p->opt.timing != 0;
         for (int b0 = 0; b0 < batch; b0 += NB) {
@@ -716,6 +730,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             CU(cudaMemsetAsync(m.dqx.p, 0, nqx, st)); CU(cudaMemsetAsync(m.dGx.p, 0, nGx, st));
             CU(cudaMemsetAsync(m.dfx.p, 0, nfx, st)); CU(cudaMemsetAsync(m.dpx.p, 0, npx, st));
             a.qx = m.dqx.as<uint32_t>(); a.Gx = m.dGx.as<uint32_t>(); a.fx = m.dfx.as<uint32_t>(); a.px = m.dpx.as<unsigned long long>();
+            a.wflag = reinterpret_cast<uint32_t *>(m.dpx.as<unsigned char>() + (size_t)4 * L.G * NB * 16);
             a.timeout_flag = p->dtimeout.as<int>();
             if (timing) {
                 CU(p->dtiming.ensure((size_t)L.G * 128));
@@ -1189,6 +1204,51 @@ extern "C" modal_status modal_plan_query(const modal_plan *p, int what, void *ds
                 memcpy(v, w, sizeof v);
             }
             return put(v, sizeof v);
+        }
+        case MODAL_Q_STREAM_LAYOUT: {
+            mh::StreamLayout L;
+            int v[16] = {0};
+            if (stream_host_layout(p, 64, L)) {
+                long long chunks = 0; for (const mh::StreamTile &t : L.tiles) chunks += t.nch;
+                const int w[16] = {1, L.G, L.NKB, L.KC, (int)L.tiles.size(), L.tiles_max, *std::min_element(L.cta_ntiles.begin(), L.cta_ntiles.end()), L.bch_max,
+                                   L.rows_max, *std::min_element(L.cta_rows.begin(), L.cta_rows.end()), L.nch_max, (int)chunks, (int)(L.a_bytes >> 20),
+                                   *std::max_element(L.blk_nctas.begin(), L.blk_nctas.end()), 0, 0};
+                memcpy(v, w, sizeof v);
+            }
+            return put(v, sizeof v);
+        }
+        case MODAL_Q_STREAM_CHECK: {
+            // host-side self check of the H stream: rebuilds H^n[k][r] from the bf16 hi + lo chunks of every tile and returns
+            // {non-zero entries covered, non-zero entries of H, max |hi + lo - H| / max |H|, rows owned in total} as 4 doubles
+            mh::StreamLayout L;
+            double out[4] = {0, 0, 0, 0};
+            if (stream_host_layout(p, 64, L)) {
+                std::vector<uint16_t> A;
+                stream_host_A(p, L, A);
+                std::vector<double> Hi((size_t)d.n_phi * nq * nq);
+                mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, Hi.data());
+                double hmax = 0, emax = 0, covered = 0, nonzero = 0;
+                for (double x : Hi) { hmax = std::max(hmax, std::fabs(x)); nonzero += x != 0.0; }
+                std::vector<int> kop(L.KC * 16, -1);
+                for (const mh::StreamBlock &b : L.blocks) for (int x = 0; x < b.nb; ++x) kop[b.koff + x] = b.k0 + x;
+                for (const mh::StreamTile &t : L.tiles)
+                    for (int u = 0; u < t.nch; ++u) {
+                        const uint16_t *base = &A[(t.a_off + (size_t)u * 8192) / 2];
+                        for (int kk = 0; kk < L.blocks[t.jb].nb; ++kk)
+                            for (int e = 0; e < 16; ++e) {
+                                const int r = kop[t.chunks[u] * 16 + e];
+                                if (r < 0) continue;
+                                const int o = mh::umma_chunk_off(kk, e) / 2;
+                                const double v = (double)mh::bf16_to_float(base[o]) + (double)mh::bf16_to_float(base[2048 + o]);
+                                const double h = Hi[((size_t)t.n * nq + L.blocks[t.jb].k0 + kk) * nq + r];
+                                emax = std::max(emax, std::fabs(v - h));
+                                covered += h != 0.0;
+                            }
+                    }
+                double rows = 0; for (int x : L.cta_rows) rows += x;
+                out[0] = covered; out[1] = nonzero; out[2] = hmax > 0 ? emax / hmax : 0; out[3] = rows;
+            }
+            return put(out, sizeof out);
         }
         case MODAL_Q_MMA_SLAB_CHECK: {
             // host-side self check of the operand packing: rebuilds H^n[k][r] from the bf16 hi + lo slabs of every CTA and

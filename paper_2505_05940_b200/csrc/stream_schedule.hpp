@@ -25,7 +25,7 @@ constexpr int ST_ROWS = 128;         // rows of a tile
 constexpr int ST_BCH_MAX = 16;       // most K chunks of q one CTA keeps as B operand
 constexpr int ST_TILES_MAX = 16;     // most tiles of one CTA (TMEM: tiles * NB <= 512)
 constexpr int ST_NKB_MAX = 8;        // most k blocks
-constexpr int ST_SENT_MAX = 128;     // most owner CTAs whose q one CTA waits for
+constexpr int ST_SENT_MAX = 256;     // most owner CTAs whose q one CTA waits for
 
 struct StreamBlock { int k0, nb, koff; };
 
@@ -100,13 +100,17 @@ inline bool stream_layout(int n_q, int n_phi, int sm, int NB, const std::vector<
         total += work[jb];
     }
     if (total == 0) return false;
-    std::vector<int> nct(L.NKB, 0);
+    std::vector<int> nct(L.NKB, 0), cap(L.NKB, 0);
     int used = 0;
-    for (int jb = 0; jb < L.NKB; ++jb) { nct[jb] = per_block[jb].empty() ? 0 : std::max(1, (int)((long long)sm * work[jb] / total)); used += nct[jb]; }
+    for (int jb = 0; jb < L.NKB; ++jb) {                 // a CTA has at least one tile and owns at least one row of its block
+        cap[jb] = std::min((int)per_block[jb].size(), L.blocks[jb].nb);
+        nct[jb] = std::min(cap[jb], std::max(1, (int)((long long)sm * work[jb] / total)));
+        used += nct[jb];
+    }
     while (used > sm) { int j = (int)(std::max_element(nct.begin(), nct.end()) - nct.begin()); --nct[j]; --used; }
     while (used < sm) {      // spare CTAs to the block with the most work per CTA
         int best = -1; double bw = 0;
-        for (int jb = 0; jb < L.NKB; ++jb) if (nct[jb] && (double)work[jb] / nct[jb] > bw && nct[jb] < (int)per_block[jb].size()) { bw = (double)work[jb] / nct[jb]; best = jb; }
+        for (int jb = 0; jb < L.NKB; ++jb) if (nct[jb] && (double)work[jb] / nct[jb] > bw && nct[jb] < cap[jb]) { bw = (double)work[jb] / nct[jb]; best = jb; }
         if (best < 0) break;
         ++nct[best]; ++used;
     }
@@ -123,7 +127,11 @@ inline bool stream_layout(int n_q, int n_phi, int sm, int NB, const std::vector<
             const double goal = (double)work[jb] * (x + 1) / nct[jb];
             const int t0 = (int)L.tiles.size();
             std::vector<int> bch;
-            while (i < ts.size() && (acc + 0.5 * (ts[i].nch + 2) < goal || x == nct[jb] - 1)) {
+            while (i < ts.size()) {
+                const bool must = (int)L.tiles.size() == t0;                                              // every CTA has a tile ...
+                const bool can = ts.size() - i - 1 >= (size_t)(nct[jb] - 1 - x);                          // ... and leaves one for every later CTA
+                const bool want = acc + 0.5 * (ts[i].nch + 2) < goal || x == nct[jb] - 1;
+                if (!(must || (want && can))) break;
                 L.tiles.push_back(ts[i]);
                 for (int kc : ts[i].chunks) if (std::find(bch.begin(), bch.end(), kc) == bch.end()) bch.push_back(kc);
                 acc += ts[i].nch + 2; ++i;

@@ -20,7 +20,7 @@
 namespace modal_dev {
 
 constexpr int ST_THREADS = 512;
-constexpr int ST_BCH_MAX_DEV = 16, ST_TILES_MAX_DEV = 16, ST_NKB_MAX_DEV = 8, ST_SENT_MAX_DEV = 128, ST_CTA_STRIDE = 6 + ST_BCH_MAX_DEV + 1 + ST_SENT_MAX_DEV;
+constexpr int ST_BCH_MAX_DEV = 16, ST_TILES_MAX_DEV = 16, ST_NKB_MAX_DEV = 8, ST_SENT_MAX_DEV = 256, ST_CTA_STRIDE = 6 + ST_BCH_MAX_DEV + 1 + ST_SENT_MAX_DEV;
 constexpr unsigned ST_POLL_SLEEP = 100;   // ns between polling rounds
 constexpr int SB_FULL = 0, SB_EMPTY = 16, SB_ACCF = 32, SB_ACCE = 48, SB_BRDY = 49, SB_FDONE = 50, SB_TPTR = 56, SB_ABORT = 57;
 constexpr int ST_BARS_BYTES = 512;
@@ -44,6 +44,7 @@ struct StreamArgs {
     uint32_t *Gx;               // [n_phi][NKB][NB]     partial G per k block, tagged
     uint32_t *fx;               // [G][128][NB]         partial f per CTA, tagged
     unsigned long long *px;     // [4][G][NB][2]        pickup partials {o, epoch}, {|q|^2, epoch}
+    uint32_t *wflag;            // [NB]                 steps of sample b the pickup warp has written out
     int *timeout_flag;
     long long *timing;          // optional [G][16]
 };
@@ -375,16 +376,11 @@ __device__ __forceinline__ void stream_owner_steps(const StreamArgs &a, const St
     const int items = C.rows * BQ;
     const int NH = (C.nct + LPQ - 1) / LPQ;
     const bool tmg = TIMING && tl == 0;
-    const bool wrole = C.c < a.batch;
     const double *cf = reinterpret_cast<const double *>(C.coef);
     const float *cw = reinterpret_cast<const float *>(cf + 3 * C.nel);
     for (int n = n_begin; n < n_end; ++n) {
         const uint32_t tag = ((uint32_t)n + 1u) & 3u, tag_next = ((uint32_t)n + 2u) & 3u;
         long long tk = tmg ? clock64() : 0;
-        if (wrole) {     // the pickup warp has consumed q^{n-2}: no CTA overwrites a pickup buffer it still reads (4 buffers)
-            unsigned spins = 0;
-            while (*C.wdone < n - 1) if ((++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 24))) { *C.s_abort = 1; break; }
-        }
         float2 *pk = C.pk + (size_t)(n & 1) * C.nel;
         // no force of step n is complete before the CTA's own epilogue has stored its part: sleep on a CTA barrier until then instead
         // of polling L2 through the whole MMA phase (148 x 192 lanes x 10 loads in flight would eat the bandwidth the H stream needs)
@@ -454,6 +450,13 @@ __device__ __forceinline__ void stream_owner_steps(const StreamArgs &a, const St
         if (tmg) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
         bar_named(2, TL);
         if (tl < NB) {                                                          // pickup partial of q^{n+1}, sample tl, over the CTA's rows
+            if (n >= 3 && tl < a.batch) {      // four buffers: the sample's pickup warp must have consumed q^{n-3} (it normally has, steps ago)
+                unsigned spins = 0;
+                while (ld_relaxed1(a.wflag + tl) < (unsigned)(n - 2)) {
+                    if ((++spins & 255u) == 0 && (*C.s_abort || spins > (1u << 22))) { *C.s_abort = 1; break; }
+                    __nanosleep(ST_POLL_SLEEP);
+                }
+            }
             float o = 0.f, nr = 0.f;
             for (int rr = 0; rr < C.rows; ++rr) { const float2 v = pk[rr * NB + tl]; o += v.x; nr += v.y; }
             unsigned long long *pp = a.px + (((size_t)((n + 1) & 3) * a.G + C.c) * NB + tl) * 2;
@@ -503,36 +506,46 @@ __device__ __forceinline__ void stream_owner(const StreamArgs &a, const StreamCt
     if (TIMING && tl == 0) { for (int x = 0; x < 4; ++x) a.timing[(size_t)C.c * 16 + 8 + x] = tm[x]; a.timing[(size_t)C.c * 16 + 14] = tmx; }
 }
 
-// W: CTA c < batch writes out[c][n] = sum over all CTAs of the pickup partials of q^n for sample c (a1 pickup + a6 write-out)
+// W: CTA c writes out[b][n] for the samples b = c, c + G, ...: the sum over all CTAs of the pickup partials of q^n (a1 pickup + a6 write-out)
 template <int NB>
 __device__ __forceinline__ void stream_pickup_warp(const StreamArgs &a, const StreamCta &C, const int lane)
 {
-    const int b = C.c;
-    int sbad = -1;
-    for (int n = 0; n < a.n_steps; ++n) {
-        float o = 0.f, nr = 0.f;
-        for (int x = lane; x < a.G; x += 32) {
-            const unsigned long long *pp = a.px + (((size_t)(n & 3) * a.G + x) * NB + b) * 2;
-            unsigned long long w0, w1;
-            unsigned spins = 0;
-            do {
-                asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(pp) : "memory");
-                if ((unsigned)(w0 >> 32) == (unsigned)n + 1u && (unsigned)(w1 >> 32) == (unsigned)n + 1u) break;
-                if ((++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 21))) { *C.s_abort = 1; break; }
-                __nanosleep(100);
-            } while (true);
-            o += __uint_as_float((unsigned)w0); nr += __uint_as_float((unsigned)w1);
-        }
+    constexpr int MAXS = 4;                                    // samples of one CTA: NB <= 64 samples over >= 16 CTAs; else the host refuses
+    int sbad[MAXS];
 #pragma unroll
-        for (int m = 16; m >= 1; m >>= 1) { o += __shfl_xor_sync(FLOW_FULL, o, m); nr += __shfl_xor_sync(FLOW_FULL, nr, m); }
-        if (lane == 0) {
-            a.out[(size_t)b * a.n_steps + n] = o;
-            if (sbad < 0 && !(isfinite(o) && isfinite(nr))) sbad = n;
-            *C.wdone = n + 1;
+    for (int x = 0; x < MAXS; ++x) sbad[x] = -1;
+    for (int n = 0; n < a.n_steps; ++n) {
+#pragma unroll
+        for (int x = 0; x < MAXS; ++x) {
+            const int b = C.c + x * a.G;
+            if (b >= a.batch) break;
+            float o = 0.f, nr = 0.f;
+            for (int y = lane; y < a.G; y += 32) {
+                const unsigned long long *pp = a.px + (((size_t)(n & 3) * a.G + y) * NB + b) * 2;
+                unsigned long long w0, w1;
+                unsigned spins = 0;
+                do {
+                    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(w0), "=l"(w1) : "l"(pp) : "memory");
+                    if ((unsigned)(w0 >> 32) == (unsigned)n + 1u && (unsigned)(w1 >> 32) == (unsigned)n + 1u) break;
+                    if ((++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 21))) { *C.s_abort = 1; break; }
+                    __nanosleep(ST_POLL_SLEEP);
+                } while (true);
+                o += __uint_as_float((unsigned)w0); nr += __uint_as_float((unsigned)w1);
+            }
+#pragma unroll
+            for (int m = 16; m >= 1; m >>= 1) { o += __shfl_xor_sync(FLOW_FULL, o, m); nr += __shfl_xor_sync(FLOW_FULL, nr, m); }
+            if (lane == 0) {
+                a.out[(size_t)b * a.n_steps + n] = o;
+                if (sbad[x] < 0 && !(isfinite(o) && isfinite(nr))) sbad[x] = n;
+                st_relaxed1(a.wflag + b, (uint32_t)n + 1u);                    // q^n of sample b consumed: its buffer may be reused
+            }
         }
         __syncwarp();
     }
-    if (lane == 0) a.first_bad[b] = sbad;
+    if (lane == 0) {
+#pragma unroll
+        for (int x = 0; x < MAXS; ++x) if (C.c + x * a.G < a.batch) a.first_bad[C.c + x * a.G] = sbad[x];
+    }
 }
 
 template <int NB, bool TIMING>
@@ -560,7 +573,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
         for (int s = 0; s < a.NSTG; ++s) { mbar_init(smem_u32(C.bars + SB_FULL + s), 1); mbar_init(smem_u32(C.bars + SB_EMPTY + s), 1); }
         for (int s = 0; s < ST_TILES_MAX_DEV; ++s) mbar_init(smem_u32(C.bars + SB_ACCF + s), 1);
         mbar_init(smem_u32(C.bars + SB_ACCE), 128); mbar_init(smem_u32(C.bars + SB_BRDY), 128); mbar_init(smem_u32(C.bars + SB_FDONE), 128);
-        *C.s_abort = 0; *C.wdone = 0;
+        *C.s_abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid < ST_CTA_STRIDE) tab[tid] = a.cta_tab[(size_t)C.c * ST_CTA_STRIDE + tid];

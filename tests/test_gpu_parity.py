@@ -295,6 +295,50 @@ def test_vk_mma_three_tiles_in_one_launch():
     check_parity(gpu[sub], ref["out"], orc.assemble(wl, samples=sub), first=200)
 
 
+@pytest.mark.parametrize("n_q,n_phi,batch,n_steps", [
+    (37, 13, 5, 1500),             # 16 samples per launch (11 of them padding), ragged K chunks (classes of 7..12 modes)
+    (100, 50, 20, 400),            # 32 samples per launch
+    (57, 23, 40, 600),             # 64 samples per launch
+    (130, 40, 70, 300),            # two launches (64 + 6 samples)
+    (16, 1, 9, 800),               # one in-plane mode
+])
+def test_vk_stream_tensor_core_parity(n_q, n_phi, batch, n_steps):
+    """Streaming tcgen05 kernel (rows of H on M, samples on N, H streamed from L2 every step) against the fp64 oracle."""
+    wl = _small_vk_workload(n_q, n_phi, batch, n_steps)
+    sub = list(range(batch)) if batch <= 8 else sorted(set(np.linspace(0, batch - 1, 12).astype(int).tolist()))
+    case_all = orc.assemble(wl)
+    ref = orc.run_case(orc.assemble(wl, samples=sub), n_steps)
+    plan = plan_with_oracle_inputs(wl, case_all, options=dict(vk_impl=3))
+    gpu, fb, _, st = gpu_run(plan, case_all.q0, case_all.qm1, n_steps)
+    torch, mb = _mods()
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 5 and info[2] == (16 if batch <= 16 else 32 if batch <= 32 else 64)
+    assert st == 0 and np.all(fb == -1)
+    check_parity(gpu[sub], ref["out"], orc.assemble(wl, samples=sub))
+    gpu2, _, _, _ = gpu_run(plan, case_all.q0, case_all.qm1, n_steps)
+    assert np.array_equal(gpu, gpu2)                              # fixed summation orders: bit-reproducible
+
+
+def test_vk_stream_ftm_fext_traj():
+    """Streaming kernel with the FTM coefficients, device-side second-order start, an external force signal and the
+    trajectory output."""
+    torch, mb = _mods()
+    n_steps, batch = 1200, 9
+    wl = _small_vk_workload(37, 13, batch, n_steps)
+    case = orc.assemble(wl, scheme=orc.FTM)
+    rng = np.random.default_rng(5)
+    fext = np.zeros((batch, n_steps)); t = np.arange(48)
+    fext[:, 20:68] = 0.5 * (1 - np.cos(2 * np.pi * t / 48))[None] * rng.uniform(0.5, 2.0, (batch, 1))
+    gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
+    ref = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, case.q0, case.qm1, n_steps, nl_scale=case.nl_scale,
+                       H=case.H, fext=orc.f32(fext), fext_gain=gain, want_traj=True)
+    plan = plan_with_oracle_inputs(wl, case, scheme=1, options=dict(vk_impl=3))
+    gpu, fb, traj, st = gpu_run(plan, case.q0, None, n_steps, want_traj=True, fext=fext, fext_gain=gain)
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 5 and st == 0 and np.all(fb == -1)
+    check_parity(gpu, ref["out"], case)
+    assert np.max(np.abs(traj - ref["traj"])) <= 1e-4 * np.max(np.abs(ref["traj"]))
+
+
 def test_c2_full_config_parity():
     """C2 exactly as bench.py times it (100 + 50 modes, batch 1, all 44 100 steps, the plan's own coefficient
     derivation): the paper's 100-mode benchmark point.  The oracle needs ~45 s here."""
@@ -390,6 +434,7 @@ def test_c4_batches_tolerance_window(batch):
     torch, mb = _mods()
     plan, q0 = mb.plan_from_workload(wl, 0)
     gpu, fb, _, st = gpu_run(plan, q0, None, wl["n_steps"])
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 5                  # the streaming tcgen05 kernel (the tensor does not fit shared memory)
     assert st == 0 and np.all(fb == -1) and np.all(g["first_bad"] == -1)
     check_window_parity(gpu[sub], g["out"], case)
     assert np.all(np.isfinite(gpu))

@@ -217,7 +217,7 @@ def test_ftm_plan_refuses_overdamped_mode_naming_it():
 def test_options_api_validates_keys_and_ranges():
     wl, plan = _c0_plan()
     plan.set_option("vk_impl", 2); plan.set_option("flow_g", 4); plan.set_option("timing", 0)
-    for key, val in (("vk_impl", 3), ("flow_ns", 99), ("nonsense", 1)):
+    for key, val in (("vk_impl", 4), ("flow_ns", 99), ("nonsense", 1)):
         with pytest.raises(mb.ModalError) as e:
             plan.set_option(key, val)
         assert e.value.status == mb.EINVAL
@@ -251,6 +251,28 @@ def test_batched_kernel_layout_covers_H_exactly_once(n_q, n_phi, opts):
     assert err <= 2.0 ** -16
     if n_q == 200 and not opts:
         assert kmin == kmax == 4 and KC == 16            # four parity classes of <= 64 modes: every CTA multiplies one class
+
+
+@pytest.mark.parametrize("n_q,n_phi", [(400, 200), (130, 40), (60, 80)])
+def test_streaming_kernel_layout_covers_H_exactly_once(n_q, n_phi):
+    """Host side of the streaming tcgen05 kernel (tensors too large for shared memory, batch 8..64): every non-zero H^n[k][r] sits in
+    exactly one K chunk of exactly one (mode, k block) tile, as bf16 hi + lo within 2^-16; the tiles of a CTA fit its 512 TMEM columns
+    at 64 samples; every transverse mode has exactly one owner CTA; only K chunks with a non-zero are streamed."""
+    wl = wlmod.c4(batch=16, n_steps=8)
+    wl["n_q"], wl["n_phi"] = n_q, n_phi
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    L = plan.query(mb.Q_STREAM_LAYOUT)
+    assert L[0] == 1, L
+    fits, G, NKB, KC, tiles, tmax, tmin, bch, rmax, rmin, nch, chunks, mib, nct = L[:14]
+    assert G <= 148 and tmax * 64 <= 512 and tmin >= 1 and rmin >= 1 and bch <= 16 and NKB <= 8
+    covered, nonzero, err, rows = plan.query(mb.Q_STREAM_CHECK)
+    H = plan.query(mb.Q_H_FULL)
+    assert covered == nonzero == np.count_nonzero(H)
+    assert err <= 2.0 ** -16 and rows == n_q
+    if (n_q, n_phi) == (400, 200):
+        # four parity classes of ~100 modes: a tile multiplies only the 7 chunks of its partner class, ~28 % of the dense stream
+        assert NKB == 4 and tiles == 800 and nch == 7 and chunks <= 0.3 * 800 * KC
+    plan.close()
 
 
 def test_batched_kernel_layout_dense_uploaded_H():
