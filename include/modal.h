@@ -236,6 +236,33 @@ typedef struct {
 } modal_peaks;
 modal_status modal_measure_peaks(int cuda_device, modal_peaks *out);
 
+/* The von Karman recurrence through ONE entry point that ALLOCATES NOTHING, for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it).  No plan: every array is a DEVICE pointer of the caller on
+ * the calling thread's current device; the call makes no cudaMalloc / cudaFree / allocating library call and never synchronises
+ * (it enqueues memsets and kernel launches on `cuda_stream`).  The only scratch the kernel needs -- the exchange buffer of the
+ * CTA team that shares a sample -- is a file-scope static __device__ array of MODAL_STATIC_SCRATCH_BYTES (1 MiB) that every GPU
+ * which loads the library holds until the process exits.
+ *   q^{n+1}_k = c1_k q^n_k + c2_k q^{n-1}_k - c3_k fnl_k(q^n)          PAPER.md:153-161 Eq. 19/20 (no external force)
+ *   fnl_k = sum_n eta_n sum_r H^n_kr q_r,  eta_n = s_n sum_pq H^n_pq q_p q_q      PAPER.md:112-123 Eq. 9-11, C eliminated (:283)
+ *   out_audio_dev[b][n] = sum_k w_k q^n_k,  n = 0 .. n_steps-1  (n = 0 is q0)
+ * Arguments (all row-major): H_dev fp32 [n_phi][n_q][n_q]; c1_dev, c2_dev, c3_dev fp64 and w_dev fp32 [coeff_batch][n_q];
+ * s_dev fp32 [coeff_batch][n_phi]; coeff_batch = 1 (one row for every sample) or batch; q0_dev, qm1_dev fp64 [batch][n_q]
+ * (q^0 and q^-1); out_audio_dev fp32 [batch][n_steps]; first_bad_dev int [batch] or NULL, receives -1, the first step at which
+ * the sample was non-finite, or -2 if a cross-CTA exchange timed out (the CTAs of a team were not co-resident: the GPU was shared
+ * with other work); err / err_bytes: optional host buffer for the message of a failing call.
+ * Precision as modal_simulate: force in fp32, state and update in fp64.  batch = 0 or n_steps = 0 does the per-device set-up only
+ * (cudaGetSymbolAddress of the scratch array; call it once before a graph capture).
+ * Limits: n_q <= MODAL_STATIC_MAX_NQ (256): MODAL_EINCOMPAT beyond.  Any batch: more samples than SMs run as consecutive launches.
+ * The scratch array is SHARED by every call on a device and keeps the last call's contents (each launch clears the part it uses
+ * first): calls that overlap on the GPU (different streams, no dependency) RACE and give wrong results -- order them.
+ * Errors: MODAL_EINVAL (sizes, NULL pointer), MODAL_EINCOMPAT (limits), MODAL_ECUDA. */
+#define MODAL_STATIC_MAX_NQ 256
+#define MODAL_STATIC_SCRATCH_BYTES (1u << 20)
+modal_status modal_vk_simulate_static(int n_q, int n_phi, int batch, int n_steps, int coeff_batch,
+                                      const float *H_dev, const double *c1_dev, const double *c2_dev, const double *c3_dev,
+                                      const float *s_dev, const float *w_dev, const double *q0_dev, const double *qm1_dev,
+                                      float *out_audio_dev, int *first_bad_dev, void *cuda_stream, char *err, int err_bytes);
+
 #ifdef __cplusplus
 }
 #endif

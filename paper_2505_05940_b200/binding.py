@@ -56,7 +56,7 @@ class SampleGeom(C.Structure):
 
 EXPORTS = ["modal_plan_create", "modal_coeffs_upload", "modal_simulate", "modal_simulate_host",
            "modal_plan_check", "modal_plan_set_option", "modal_plan_set_airy_basis", "modal_plan_destroy", "modal_last_error",
-           "modal_plan_query", "modal_derive_coeffs", "modal_project_bump", "modal_measure_peaks"]
+           "modal_plan_query", "modal_derive_coeffs", "modal_project_bump", "modal_measure_peaks", "modal_vk_simulate_static"]
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2505_05940_b200.build` "
@@ -86,6 +86,18 @@ class Peaks(C.Structure):
 
 
 lib.modal_measure_peaks.argtypes = [C.c_int, C.POINTER(Peaks)]
+lib.modal_vk_simulate_static.argtypes = [C.c_int] * 5 + [C.c_void_p] * 11 + [C.c_char_p, C.c_int]
+STATIC_MAX_NQ, STATIC_SCRATCH_BYTES = 256, 1 << 20
+
+
+def vk_simulate_static(n_q, n_phi, batch, n_steps, coeff_batch, H, c1, c2, c3, s, w, q0, qm1, out, first_bad=0, stream=0):
+    """modal_vk_simulate_static: every array argument is a DEVICE address (int); nothing is allocated, nothing synchronised."""
+    err = C.create_string_buffer(512)
+    st = lib.modal_vk_simulate_static(n_q, n_phi, batch, n_steps, coeff_batch, H, c1, c2, c3, s, w, q0, qm1, out,
+                                      first_bad or None, stream or None, err, 512)
+    if st != OK:
+        raise ModalError(st, err.value.decode())
+    return st
 
 
 def measure_peaks(device: int = 0) -> dict:
