@@ -165,13 +165,16 @@ def run_secondary(mb, torch, sampler, pk, steps=2, warmup=1):
         t = device_time(torch, plan, q0[:B], n_steps, out, steps, warmup)
         info = plan.query(mb.Q_KERNEL_INFO)
         ts = tuple(int(x) for x in plan.query(mb.Q_TILE_STATS)) if wl["model"] == "vk" else (0, 0)
-        st, _ = plan.check()
+        st, fbad = plan.check(B)
         e = {"workload": label, "batch": B, "time_steps": n_steps, "value": B * n_steps / t, "unit": UNIT,
              "us_per_time_step": 1e6 * t / n_steps, "mode_steps_per_s": B * n_steps * wl["n_q"] / t,
              "realtime_factor_per_sample": (n_steps / wl["sample_rate"]) / t,
              "kernel_family": int(info[0]), "ctas": int(info[1]) * (int(info[2]) if int(info[0]) == 3 else 1),
              "status": int(st), "roofline": roofline_for(wl, B, n_steps, t, info, ts, pk, plan.query(mb.Q_STREAM_LAYOUT) if int(info[0]) == 5 else None),
              "clocks": sampler.summary(lo)}
+        nbad = int((fbad >= 0).sum()) if fbad is not None else 0
+        if nbad:          # status 3: the explicit scheme itself diverges on these samples (the oracle does too, within a few steps: SPEC.md:298)
+            e["unstable_samples"] = nbad
         if extra:
             e.update(extra)
         res.append(e)

@@ -249,6 +249,21 @@ __device__ __forceinline__ void poll_flag_list(const unsigned *base, const int *
     }
 }
 
+// one try_wait on the fast path; the bounded loop only when the phase is not complete yet
+__device__ __forceinline__ void mma_wait_fast(uint32_t bar, uint32_t parity, volatile int *abortp)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (!ok) mbar_wait(bar, parity, abortp);
+}
+__device__ __forceinline__ bool mma_elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+
 // CTA-uniform view of the kernel's shared memory and of the CTA's place in the grid
 struct MmaCta {
     int c, i, j;                // CTA, n group, k block
@@ -851,7 +866,8 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
         asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");
         if (warp == 0) {
             // ---------------- P: wait for q^n of the tile's source blocks, stream its K chunks by TMA ----
-            unsigned cnt = 0;                                   // chunks issued so far: stage = cnt % NSTG
+            const uint32_t pfull0 = smem_u32(C.bars + MB_FULL), pempty0 = smem_u32(C.bars + MB_EMPTY), pring0 = smem_u32(C.ring);
+            int psg = 0; unsigned pph = 1;                       // ring stage and the parity of its EMPTY phase to wait for
             const int fcnt = a.fcnt[C.c];
             const bool tmg = TIMING && lane == 0;
             long long tmp = 0, tmq = 0;
@@ -864,23 +880,30 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                     if (lane == 0) {
                         mbar_arrive(smem_u32(C.bars + MB_QRDY + t));
                         asm volatile("fence.proxy.async.global;" ::: "memory");
-                        for (int xx = 0; xx < C.KCA; ++xx, ++cnt) {
-                            const int x = xx + kc0 < C.KCA ? xx + kc0 : xx + kc0 - C.KCA;     // walk the chunks from a per-CTA offset
-                            const unsigned sg = cnt % (unsigned)NSTG, ph = (cnt / (unsigned)NSTG) & 1u;
-                            mbar_wait(smem_u32(C.bars + MB_EMPTY + sg), ph ^ 1u, C.s_abort);
-                            mbar_expect_tx(smem_u32(C.bars + MB_FULL + sg), 8192);
-                            tma_bulk_g2s(smem_u32(C.ring + sg * 8192), a.Qop + ((size_t)t * a.KC + C.kl[x]) * 4096, 8192,
-                                         smem_u32(C.bars + MB_FULL + sg));
+                        const unsigned char *qsrc = reinterpret_cast<const unsigned char *>(a.Qop) + (size_t)t * a.KC * 8192;
+                        int x = kc0;                                                   // walk the chunks from a per-CTA offset
+                        for (int xx = 0; xx < C.KCA; ++xx) {
+                            mma_wait_fast(pempty0 + 8 * psg, pph, C.s_abort);
+                            mbar_expect_tx(pfull0 + 8 * psg, 8192);
+                            tma_bulk_g2s(pring0 + psg * 8192, qsrc + (size_t)C.kl[x] * 8192, 8192, pfull0 + 8 * psg);
+                            if (++psg == NSTG) { psg = 0; pph ^= 1u; }
+                            if (++x == C.KCA) x = 0;
                         }
                     }
                     __syncwarp();
                 }
             if (tmg) { a.timing[(size_t)C.c * 16 + 12] = tmp; a.timing[(size_t)C.c * 16 + 15] = tmq; }
         } else if (warp == 1) {
-            // ---------------- M: one thread issues the MMAs of every tile, in order ------------------------
-            if (lane == 0) {
+            // ---------------- M: the MMAs of every tile, in order --------------------------------------------
+            // The whole warp runs the (uniform) loop and one elected lane issues: inside a lane-0 branch ptxas wraps every tcgen05
+            // instruction in an ELECT / R2UR / branch loop; no division and one add per descriptor in the chunk loop.
+            {
                 const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(a.NC >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-                unsigned cnt = 0, uses[3] = {0u, 0u, 0u};
+                const uint32_t full0 = smem_u32(C.bars + MB_FULL), empty0 = smem_u32(C.bars + MB_EMPTY);
+                const uint64_t dQ0 = umma_desc(smem_u32(C.ring)), dH0 = umma_desc(smem_u32(C.slab));     // + (byte offset >> 4)
+                const uint32_t hstep = (uint32_t)(2 * a.NC * 32) >> 4, hlo = (uint32_t)(a.NC * 32) >> 4;
+                int sg = 0; unsigned ph = 0;
+                unsigned uses[3] = {0u, 0u, 0u};
                 const bool tmg = TIMING;
                 long long tmm = 0;
                 for (int n = 0; n < a.n_steps; ++n)
@@ -891,24 +914,24 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) vk_mma_kernel(const MmaArgs a)
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t td = C.tbase + (uint32_t)(slot * a.NC);
                         long long tk = 0;
-                        for (int xx = 0; xx < C.KCA; ++xx, ++cnt) {
-                            const int x = xx + kc0 < C.KCA ? xx + kc0 : xx + kc0 - C.KCA;     // position in the list = position in the slab
-                            const unsigned sg = cnt % (unsigned)NSTG, ph = (cnt / (unsigned)NSTG) & 1u;
-                            mbar_wait(smem_u32(C.bars + MB_FULL + sg), ph, C.s_abort);
+                        int x = kc0;                                                   // position in the list = position in the slab
+                        for (int xx = 0; xx < C.KCA; ++xx) {
+                            mma_wait_fast(full0 + 8 * sg, ph, C.s_abort);
                             if (tmg && t == 0 && xx == 0) tk = clock64();
-                            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                            const uint32_t qa = smem_u32(C.ring + sg * 8192), hb = smem_u32(C.slab + (size_t)x * 2 * a.NC * 32);
-                            const uint64_t qhi = umma_desc(qa), qlo = umma_desc(qa + 4096);
-                            const uint64_t hhi = umma_desc(hb), hlo = umma_desc(hb + a.NC * 32);
-                            umma_bf16(td, qhi, hhi, idesc, xx > 0);
-                            umma_bf16(td, qlo, hhi, idesc, 1);
-                            umma_bf16(td, qhi, hlo, idesc, 1);
-                            umma_commit(smem_u32(C.bars + MB_EMPTY + sg));                          // ring slot free when these MMAs retire
+                            const uint64_t qhi = dQ0 + (uint64_t)(sg * (8192 >> 4)), hhi = dH0 + (uint64_t)((uint32_t)x * hstep);
+                            if (mma_elect_one()) {
+                                umma_bf16(td, qhi, hhi, idesc, xx > 0);
+                                umma_bf16(td, qhi + (4096 >> 4), hhi, idesc, 1);
+                                umma_bf16(td, qhi, hhi + hlo, idesc, 1);
+                                umma_commit(empty0 + 8 * sg);                                             // ring slot free when these MMAs retire
+                            }
+                            if (++sg == NSTG) { sg = 0; ph ^= 1u; }
+                            if (++x == C.KCA) x = 0;
                         }
-                        umma_commit(smem_u32(C.bars + MB_ACCF + slot));                             // t of this tile complete
+                        if (mma_elect_one()) umma_commit(smem_u32(C.bars + MB_ACCF + slot));             // t of this tile complete
                         if (tmg && t == 0) tmm += clock64() - tk;
                     }
-                if (tmg) a.timing[(size_t)C.c * 16 + 13] = tmm;
+                if (tmg && lane == 0) a.timing[(size_t)C.c * 16 + 13] = tmm;
             }
         } else if (warp == 2 && C.j == 0) {
             mma_pickup_warp(a, C, lane);
