@@ -581,3 +581,74 @@ def H_airy_ritz(Lx, Ly, mq, nq, c, ng=200):
         t2 = np.einsum("jpq,jpq->pq", Cx, CCy)
         H[n] = pref * ((A + A.T) * t1 - 2.0 * Bc * t2)
     return H
+
+
+# ------------------------------------------- reverse pass ----
+def bptt_vk(c1, c2, c3, w, nl_scale, H, q0, qm1, gout):
+    """Backpropagation through time of ONE von Karman sample ("gradients ... by backpropagation through
+    the time integrator"; the paper uses autodiff, this is the same adjoint written out).
+
+    Forward, as `simulate` (Eq. 19/20, no external force), n = 0 .. N-1, N = len(gout):
+        out_n = w . q^n,     q^{n+1} = c1 q^n + c2 q^{n-1} - c3 f(q^n),
+        f_k(q) = sum_m s_m G_m t_mk,  t_m = H^m q,  G_m = q . t_m                       (Eq. 9)
+    Loss: any L(out) with gout[n] = dL/d out_n.  Adjoint a^n = dL/dq^n (total), a^N = a^{N+1} = 0:
+        a^n = w gout_n + c1 a^{n+1} + c2 a^{n+2} - J(q^n)^T (c3 a^{n+1}),
+        J_kj = df_k/dq_j = sum_m s_m [ (H^m q + H^mT q)_j t_mk + G_m H^m_kj ]
+    Returns dL/d{q0, qm1, c1, c2, c3, w, s (nl_scale), H}; H entries are treated as independent (no symmetry constraint).
+    Plain numpy fp64, one einsum per stage and step; small sizes only.
+    """
+    c1, c2, c3, w, s = (np.asarray(x, np.float64) for x in (c1, c2, c3, w, nl_scale))
+    H = np.asarray(H, np.float64); q0 = np.asarray(q0, np.float64); qm1 = np.asarray(qm1, np.float64)
+    gout = np.asarray(gout, np.float64)
+    N, Nq = gout.shape[0], q0.shape[0]
+    # forward, stored
+    q = np.empty((N + 1, Nq)); q[0] = q0
+    prev = qm1
+    for n in range(N):
+        t = np.einsum("mkr,r->mk", H, q[n])
+        G = t @ q[n]
+        f = (s * G) @ t
+        q[n + 1] = c1 * q[n] + c2 * prev - c3 * f
+        prev = q[n]
+    g = {k: np.zeros(Nq) for k in ("c1", "c2", "c3", "w")}
+    g["s"] = np.zeros_like(s); g["H"] = np.zeros_like(H)
+    a1 = np.zeros(Nq); a2 = np.zeros(Nq)            # a^{n+1}, a^{n+2}
+    for n in range(N - 1, -1, -1):
+        qn = q[n]; qp = q[n - 1] if n > 0 else qm1
+        t = np.einsum("mkr,r->mk", H, qn)           # t_m = H^m q
+        tt = np.einsum("mkr,k->mr", H, qn)          # H^mT q
+        G = t @ qn
+        f = (s * G) @ t
+        mu = c3 * a1
+        d = t @ mu                                  # t_m . mu
+        # J^T mu = sum_m s_m [ (t_m + tt_m) d_m + G_m H^mT mu ]
+        JTmu = (s * d) @ (t + tt) + np.einsum("m,mkj,k->j", s * G, H, mu)
+        g["c1"] += a1 * qn; g["c2"] += a1 * qp; g["c3"] -= a1 * f
+        g["w"] += gout[n] * qn
+        g["s"] -= d * G
+        g["H"] -= (s * d)[:, None, None] * np.multiply.outer(qn, qn)[None] + (s * G)[:, None, None] * np.multiply.outer(mu, qn)[None]
+        a0 = w * gout[n] + c1 * a1 + c2 * a2 - JTmu
+        a2, a1 = a1, a0
+    g["q0"] = a1                                     # a^0
+    g["qm1"] = c2 * a2                               # q^{-1} enters q^1 only: c2 a^1
+    return g
+
+
+def dcoeffs_domega_dgamma(scheme, omega, gamma, T):
+    """Partial derivatives of (c1, c2, c3) wrt omega and gamma, for the chain rule to the physical parameters:
+    SV (PAPER.md:162-166, Eq. 21-23): c1 = (2 - w^2 T^2)/(1 + gT), c2 = -(1 - gT)/(1 + gT), c3 = T^2/(1 + gT);
+    FTM (reading R7): c1 = 2 e^{-gT} cos(wt T), c2 = -e^{-2gT}, c3 = T e^{-gT} sin(wt T)/wt, wt = sqrt(w^2 - g^2).
+    Returns dict d{c1,c2,c3}_d{w,g}."""
+    w_, g_ = np.asarray(omega, np.float64), np.asarray(gamma, np.float64)
+    if scheme == SV:
+        den = 1.0 + g_ * T
+        return dict(c1_w=-2 * w_ * T * T / den, c1_g=-(2 - w_ ** 2 * T * T) * T / den ** 2,
+                    c2_w=np.zeros_like(w_), c2_g=2 * T / den ** 2,
+                    c3_w=np.zeros_like(w_), c3_g=-T ** 3 / den ** 2)
+    wt = np.sqrt(w_ ** 2 - g_ ** 2)
+    e = np.exp(-g_ * T); sn, cs = np.sin(wt * T), np.cos(wt * T)
+    wt_w, wt_g = w_ / wt, -g_ / wt
+    dc3_dwt = T * e * (T * cs * wt - sn) / wt ** 2
+    return dict(c1_w=-2 * e * sn * T * wt_w, c1_g=-2 * T * e * cs - 2 * e * sn * T * wt_g,
+                c2_w=np.zeros_like(w_), c2_g=2 * T * np.exp(-2 * g_ * T),
+                c3_w=dc3_dwt * wt_w, c3_g=-T * T * e * sn / wt + dc3_dwt * wt_g)

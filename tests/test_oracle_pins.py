@@ -594,3 +594,81 @@ def test_H_airy_ritz_vs_bruteforce_quadrature_symmetry_and_HC_identity():
         assert abs(c_spn - H[n, p, q]) <= 1e-6 * np.abs(H).max(), (n, p, q, c_spn, H[n, p, q])
     # reflection symmetry of the rectangle: ~3/4 of the entries vanish, as for the sine basis
     assert 0.2 < np.mean(np.abs(H) > 1e-9 * np.abs(H).max()) < 0.3
+
+
+# ------------------------------------------------ reverse pass ----
+def _bptt_problem(seed=0, Nq=7, Nphi=5, N=48):
+    rng = np.random.default_rng(seed)
+    H = rng.normal(size=(Nphi, Nq, Nq)); H = H + H.transpose(0, 2, 1)
+    T = 1 / 44100
+    om = rng.uniform(500, 9000, Nq); ga = rng.uniform(0.5, 30, Nq)
+    c1, c2, c3 = orc.scheme_coeffs(orc.SV, om, ga, T)
+    w = rng.normal(size=Nq); s = rng.uniform(1e7, 1e8, Nphi)
+    q0 = rng.normal(size=Nq) * 1e-2; qm1 = q0 + rng.normal(size=Nq) * 1e-4
+    gout = rng.normal(size=N)
+    return dict(c1=c1, c2=c2, c3=c3, w=w, s=s, H=H, q0=q0, qm1=qm1), gout, N
+
+
+def test_bptt_adjoint_matches_finite_differences_of_the_forward_oracle():
+    """PAPER.md:281-285.  The adjoint recurrence (numpy) against central differences of the INDEPENDENT forward code
+    (modal_oracle.c through `simulate`) for a linear functional L = sum_n gout_n out_n: every gradient array, including H
+    (perturbed as a symmetric pair: dL/d(pair) = g[k][r] + g[r][k]).  A wrong sign, a dropped Jacobian term, a transposed
+    index or an off-by-one in the step index fails here."""
+    P, gout, N = _bptt_problem()
+
+    def L(**over):
+        a = {**P, **over}
+        r = orc.simulate(orc.VK, a["c1"][None], a["c2"][None], a["c3"][None], a["w"][None], a["q0"][None], a["qm1"][None], N,
+                         nl_scale=a["s"][None], H=a["H"])
+        return float(gout @ r["out"][0])
+
+    g = orc.bptt_vk(P["c1"], P["c2"], P["c3"], P["w"], P["s"], P["H"], P["q0"], P["qm1"], gout)
+    # the non-linear part must matter in this problem, or the Jacobian terms would go unchecked
+    g_lin = orc.bptt_vk(P["c1"], P["c2"], P["c3"], P["w"], 0 * P["s"], P["H"], P["q0"], P["qm1"], gout)
+    assert np.linalg.norm(g["q0"] - g_lin["q0"]) > 1e-3 * np.linalg.norm(g["q0"])
+    for name, eps in (("q0", 1e-7), ("qm1", 1e-7), ("c1", 1e-7), ("c2", 1e-7), ("c3", 1e-12), ("w", 1e-6), ("s", 1e3)):
+        for idx in range(P[name].shape[0]):
+            hi = P[name].copy(); hi[idx] += eps
+            lo = P[name].copy(); lo[idx] -= eps
+            fd = (L(**{name: hi}) - L(**{name: lo})) / (2 * eps)
+            assert abs(fd - g[name][idx]) <= 2e-5 * np.max(np.abs(g[name])) + 1e-7 * abs(fd), (name, idx, fd, g[name][idx])
+    rng = np.random.default_rng(1)
+    for _ in range(12):
+        m, k, r = rng.integers(0, 5), rng.integers(0, 7), rng.integers(0, 7)
+        eps = 1e-5
+        hi = P["H"].copy(); lo = P["H"].copy()
+        for (a, b) in {(k, r), (r, k)}:
+            hi[m, a, b] += eps; lo[m, a, b] -= eps
+        fd = (L(H=hi) - L(H=lo)) / (2 * eps)
+        want = g["H"][m, k, r] + (g["H"][m, r, k] if k != r else 0.0)
+        assert abs(fd - want) <= 2e-5 * np.max(np.abs(g["H"])) + 1e-6 * abs(fd), (m, k, r, fd, want)
+
+
+def test_bptt_linear_case_is_the_transposed_impulse_response():
+    """With s = 0 the recurrence is linear and time-invariant: dL/dq0_k = sum_n gout_n w_k h_k[n], h_k the response of
+    mode k to q^0 = 1, q^-1 = 0 ... which for the homogeneous recurrence is the textbook two-term solution."""
+    P, gout, N = _bptt_problem(seed=3)
+    g = orc.bptt_vk(P["c1"], P["c2"], P["c3"], P["w"], 0 * P["s"], P["H"], P["q0"], P["qm1"], gout)
+    h0 = np.zeros((N, 7)); h1 = np.zeros((N, 7))       # responses to (q0, qm1) = (1, 0) and (0, 1)
+    a, b = np.ones(7), np.zeros(7)
+    c, d = np.zeros(7), np.ones(7)
+    for n in range(N):
+        h0[n], h1[n] = a, c
+        a, b = P["c1"] * a + P["c2"] * b, a
+        c, d = P["c1"] * c + P["c2"] * d, c
+    assert np.allclose(g["q0"], P["w"] * (gout @ h0), rtol=1e-12, atol=1e-14)
+    assert np.allclose(g["qm1"], P["w"] * (gout @ h1), rtol=1e-12, atol=1e-14)
+    assert np.all(g["s"] == 0) or np.allclose(g["H"], 0)
+
+
+@pytest.mark.parametrize("scheme", [orc.SV, orc.FTM])
+def test_scheme_coefficient_derivatives_by_finite_differences(scheme):
+    T = 1 / 44100
+    om = np.array([300.0, 2500.0, 20000.0, 60000.0]); ga = np.array([0.5, 3.0, 40.0, 200.0])
+    d = orc.dcoeffs_domega_dgamma(scheme, om, ga, T)
+    for var, eps in (("w", 1e-3), ("g", 1e-4)):
+        hi = orc.scheme_coeffs(scheme, om + (eps if var == "w" else 0), ga + (eps if var == "g" else 0), T)
+        lo = orc.scheme_coeffs(scheme, om - (eps if var == "w" else 0), ga - (eps if var == "g" else 0), T)
+        for i, c in enumerate(("c1", "c2", "c3")):
+            fd = (hi[i] - lo[i]) / (2 * eps)
+            assert np.allclose(d[f"{c}_{var}"], fd, rtol=2e-6, atol=1e-9 * np.max(np.abs(fd)) + 1e-18), (c, var, d[f"{c}_{var}"], fd)
