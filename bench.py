@@ -192,6 +192,35 @@ def run_secondary(mb, torch, sampler, pk, steps=2, warmup=1):
         plan.close()
     best = max((e for e in res if e["workload"].startswith("c3_")), key=lambda e: e["roofline"]["frac"])
     best["best_c3_batch"] = True
+    # reverse pass: C2's mode counts, forward with the trajectory kept on the device, then modal_bptt
+    for B in (1, 8):
+        wl = wlmod.c2(n_steps=4410) if B == 1 else dict(wlmod.c3(batch=B, n_steps=4410), n_q=100, n_phi=50, name=f"c2_shape_b{B}")
+        wl["A"] = np.minimum(wl["A"], 0.5 * wl["h"])
+        plan, q0 = mb.plan_from_workload(wl, dev)
+        n_steps, nq, nphi = wl["n_steps"], wl["n_q"], wl["n_phi"]
+        out = torch.empty((B, n_steps), dtype=torch.float32, device="cuda")
+        traj = torch.zeros((B, n_steps, nq), dtype=torch.float64, device="cuda")
+        stream = torch.cuda.current_stream().cuda_stream
+        qm1 = q0 * (1.0 - 1e-3)                              # any explicit q^-1: the reverse pass differentiates the recurrence it is given
+        st, _ = plan.simulate(q0, n_steps, out.data_ptr(), qm1=qm1, stream=stream, traj_dev_ptr=traj.data_ptr())
+        gout = torch.randn((B, n_steps), dtype=torch.float32, device="cuda")
+        plan.bptt(qm1, n_steps, traj.data_ptr(), gout.data_ptr(), want_H=False, stream=stream)       # warm-up
+        ts = []
+        for want_H in (False, True):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); plan.bptt(qm1, n_steps, traj.data_ptr(), gout.data_ptr(), want_H=want_H, stream=stream); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        hbm_peak, peak_src, _ = driver_peaks()
+        ach = 4.0 * nphi * nq * nq * B * n_steps / ts[0] / 1e9
+        res.append({"workload": f"bptt_vk_{nq}x{nphi}_b{B}", "batch": B, "time_steps": n_steps, "value": B * n_steps / ts[0], "unit": UNIT,
+                    "us_per_time_step": 1e6 * ts[0] / n_steps, "us_per_time_step_with_grad_H": 1e6 * ts[1] / n_steps, "kernel_family": 6, "status": int(st),
+                    "roofline": {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
+                                 "peak_source": peak_src, "kernel": "vk_bptt_kernel",
+                                 "frac_of_l2": ach / pk["l2_read_gbs_8mb"] if pk else None,
+                                 "note": "reverse step: dense fp32 H (4 N_phi N_q^2 bytes per sample) read once for both contractions, from L2; "
+                                         "time includes the gradient copies to the host (modal_bptt is synchronous)"}})
+        plan.close()
     wl = wlmod.c4(batch=256)
     plan, q0 = mb.plan_from_workload(wl, dev)
     for B in (16, 64, 256):

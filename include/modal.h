@@ -128,6 +128,31 @@ modal_status modal_simulate_host(modal_plan *plan, int batch, int n_steps, const
  * wait of a persistent kernel gave up: the CTAs of a team were not co-resident) / MODAL_OK. */
 modal_status modal_plan_check(modal_plan *plan, int *first_bad_step);
 
+/* Reverse pass (backpropagation through time) of a MODAL_VK run: SURVEY.md 8(f) row 3.  Given the trajectory of a
+ * forward run (modal_init.traj_dev of modal_simulate with the same plan, coefficients, batch and n_steps, an explicit qm1 and no
+ * external force) and gout[b][n] = dL/d out_audio[b][n] of any loss L on the audio, computes per sample
+ *   dL/dq^0, dL/dq^-1 (as independent inputs of q^{n+1} = c1 q^n + c2 q^{n-1} - c3 fnl(q^n), Eq. 19/20),
+ *   dL/dc1, dL/dc2, dL/dc3 and through them (SV Eq. 21-23 / FTM Eq. 16-18) dL/domega, dL/dsigma,
+ *   dL/dpickup, dL/dnl_scale, and dL/dH summed over the batch (entries as independent variables under t_m = H^m q: for a
+ *   symmetric parametrisation use g[n][k][r] + g[n][r][k]).  Masked modes get zero gradients.
+ * Adjoint recurrence a^n = w gout_n + c1 a^{n+1} + c2 a^{n+2} - J(q^n)^T (c3 a^{n+1}); the Jacobian product costs two contractions
+ * with H per step (csrc/vk_bptt.cuh).  Contractions in fp32, adjoint state and accumulators in fp64.  Synchronous: the gradients
+ * are copied to the HOST arrays before it returns; any gradient pointer may be NULL.  Per-sample arrays are [batch][...] even when
+ * coeff_batch is 1 (sum over the batch for shared parameters).  n_q <= 512.
+ * Errors: MODAL_EINVAL (sizes, missing qm1 / traj_dev / gout_dev), MODAL_EINCOMPAT (not a VK plan, n_q), MODAL_ECUDA. */
+typedef struct {
+    const double *qm1;        /* host   [batch][n_q]            q^-1 of the forward run                       */
+    const double *traj_dev;   /* DEVICE [batch][n_steps][n_q]   q^n of the forward run (fp64)                 */
+    const float *gout_dev;    /* DEVICE [batch][n_steps]        dL/d out_audio                                */
+    double *grad_q0, *grad_qm1;            /* host [batch][n_q]                                               */
+    double *grad_omega, *grad_sigma;       /* host [batch][n_q]                                               */
+    double *grad_c1, *grad_c2, *grad_c3;   /* host [batch][n_q]                                               */
+    double *grad_pickup;                   /* host [batch][n_q]                                               */
+    double *grad_nl_scale;                 /* host [batch][n_phi]                                             */
+    double *grad_H;                        /* host [n_phi][n_q][n_q], summed over the batch                   */
+} modal_bptt_args;
+modal_status modal_bptt(modal_plan *plan, int batch, int n_steps, const modal_bptt_args *args, void *cuda_stream);
+
 /* Launch-selection overrides for tests and sweeps (the defaults are automatic).  Keys:
  *   "vk_impl"      0 automatic, 1 FP32 flow kernel, 2 tcgen05 batched kernel (H resident in shared memory), 3 tcgen05
  *                  streaming kernel (H streamed from L2; batch <= 64 per launch, wider batches run as consecutive launches)

@@ -48,6 +48,11 @@ class Init(C.Structure):
                 ("traj_dev", C.c_void_p)]
 
 
+class BpttArgs(C.Structure):
+    _fields_ = [("qm1", _dp), ("traj_dev", C.c_void_p), ("gout_dev", C.c_void_p)] + [(n, _dp) for n in (
+        "grad_q0", "grad_qm1", "grad_omega", "grad_sigma", "grad_c1", "grad_c2", "grad_c3", "grad_pickup", "grad_nl_scale", "grad_H")]
+
+
 class SampleGeom(C.Structure):
     _fields_ = [("Lx", C.c_double), ("Ly", C.c_double), ("h", C.c_double), ("T0", C.c_double),
                 ("D", C.c_double), ("rho", C.c_double), ("area", C.c_double),
@@ -56,7 +61,7 @@ class SampleGeom(C.Structure):
 
 EXPORTS = ["modal_plan_create", "modal_coeffs_upload", "modal_simulate", "modal_simulate_host",
            "modal_plan_check", "modal_plan_set_option", "modal_plan_set_airy_basis", "modal_plan_destroy", "modal_last_error",
-           "modal_plan_query", "modal_derive_coeffs", "modal_project_bump", "modal_measure_peaks", "modal_vk_simulate_static"]
+           "modal_plan_query", "modal_derive_coeffs", "modal_project_bump", "modal_measure_peaks", "modal_vk_simulate_static", "modal_bptt"]
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2505_05940_b200.build` "
@@ -67,6 +72,7 @@ lib.modal_coeffs_upload.argtypes = [C.c_void_p, C.POINTER(Coeffs)]
 lib.modal_simulate.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(Init), C.c_void_p, _ip, C.c_void_p]
 lib.modal_simulate_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(Init), _fp, _ip]
 lib.modal_plan_check.argtypes = [C.c_void_p, _ip]
+lib.modal_bptt.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(BpttArgs), C.c_void_p]
 lib.modal_plan_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int]
 lib.modal_plan_set_airy_basis.argtypes = [C.c_void_p, C.c_int, C.c_int]
 lib.modal_plan_destroy.argtypes = [C.c_void_p]
@@ -176,6 +182,19 @@ class Plan:
         st = lib.modal_plan_check(self._h, _ptr(fb, _ip))
         self._check(st, allow=(EUNSTABLE,))
         return st, fb
+
+    def bptt(self, qm1, n_steps, traj_dev_ptr, gout_dev_ptr, want_H=False, stream=0):
+        """modal_bptt: gradients of a loss on the audio (gout = dL/d out, device) through the stored trajectory (device)."""
+        qm1 = _arr(np.atleast_2d(qm1))
+        B = qm1.shape[0]
+        g = {n: np.zeros((B, self.n_q)) for n in ("q0", "qm1", "omega", "sigma", "c1", "c2", "c3", "pickup")}
+        g["nl_scale"] = np.zeros((B, self.n_phi))
+        if want_H:
+            g["H"] = np.zeros((self.n_phi, self.n_q, self.n_q))
+        a = BpttArgs(_ptr(qm1, _dp), traj_dev_ptr, gout_dev_ptr, *[_ptr(g[n], _dp) for n in ("q0", "qm1", "omega", "sigma", "c1", "c2", "c3", "pickup", "nl_scale")],
+                     _ptr(g.get("H"), _dp))
+        self._check(lib.modal_bptt(self._h, B, int(n_steps), C.byref(a), stream or None))
+        return g
 
     def set_airy_basis(self, basis: int, n_trial: int = 0):
         return self._check(lib.modal_plan_set_airy_basis(self._h, int(basis), int(n_trial)))

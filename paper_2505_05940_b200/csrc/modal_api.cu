@@ -18,6 +18,7 @@
 #include "vk_flow.cuh"
 #include "vk_mma.cuh"
 #include "vk_stream.cuh"
+#include "vk_bptt.cuh"
 #include "peaks.cuh"
 
 namespace mh = modal_host;
@@ -100,6 +101,8 @@ struct modal_plan {
     DevBuf dHf, dfx, dgx, dqx, dtiming, dperm, dtimeout;
     MmaConfig mma;
     StreamConfig stream;
+    DevBuf bp[16];                                                    // modal_bptt: dense H, coefficients, gradients, scratch
+    bool bp_H_valid = false;
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dkv, dkq, dr, dast, ds, dsT, dw, dlam, dc, dq0, dv0, dgain, dbad, dout;      // dsT: s_n transposed [n_phi][coeff_batch] (batched kernel)
     float *pinned_out = nullptr; size_t pinned_bytes = 0;            // staging of modal_simulate_host
@@ -153,7 +156,7 @@ void set_H(modal_plan *p, Get get_user)
     }
     for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
     p->flow_cfgs.clear();                                   // schedules depend on the zero pattern
-    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0;
+    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0; p->bp_H_valid = false;
     p->H_dirty = true;
 }
 
@@ -1074,6 +1077,170 @@ extern "C" modal_status modal_simulate_host(modal_plan *p, int batch, int n_step
     return s;
 }
 
+// ---- reverse pass (vk_bptt.cuh) ---------------------------------------------------------------------
+namespace {
+// d(c1, c2, c3)/d(omega, sigma) of q+ = c1 q + c2 q- - c3 f:  SV PAPER.md:163-167 Eq. 21-23;  FTM PAPER.md:147-151 Eq. 16-18 (R7)
+struct CoeffDerivs { double c1_w, c1_g, c2_g, c3_w, c3_g; };
+CoeffDerivs coeff_derivs(int scheme, double w, double g, double T)
+{
+    CoeffDerivs d{};
+    if (scheme == MODAL_SV) {
+        const double den = 1.0 + g * T;
+        d.c1_w = -2.0 * w * T * T / den; d.c1_g = -(2.0 - w * w * T * T) * T / (den * den);
+        d.c2_g = 2.0 * T / (den * den);
+        d.c3_w = 0.0; d.c3_g = -T * T * T / (den * den);
+    } else {
+        const double wt = std::sqrt(w * w - g * g), e = std::exp(-g * T), sn = std::sin(wt * T), cs = std::cos(wt * T);
+        const double wt_w = w / wt, wt_g = -g / wt;
+        const double dc3 = T * e * (T * cs * wt - sn) / (wt * wt);
+        d.c1_w = -2.0 * e * sn * T * wt_w; d.c1_g = -2.0 * T * e * cs - 2.0 * e * sn * T * wt_g;
+        d.c2_g = 2.0 * T * std::exp(-2.0 * g * T);
+        d.c3_w = dc3 * wt_w; d.c3_g = -T * T * e * sn / wt + dc3 * wt_g;
+    }
+    return d;
+}
+}  // namespace
+
+extern "C" modal_status modal_bptt(modal_plan *p, int batch, int n_steps, const modal_bptt_args *ar, void *cuda_stream)
+{
+    if (!p) return MODAL_EINVAL;
+    p->err.clear();
+    const modal_plan_desc &d = p->d;
+    const int nq = d.n_q, nphi = d.n_phi, cb = p->coeff_batch;
+    if (d.model != MODAL_VK) { p->err += "modal_bptt: the reverse pass is built for MODAL_VK plans\n"; return MODAL_EINCOMPAT; }
+    if (p->device < 0) { p->err += "modal_bptt needs a CUDA device: there is no CPU fallback\n"; return MODAL_ECUDA; }
+    if (!ar || batch < 1 || n_steps < 1 || batch > d.max_batch || n_steps > d.max_steps || (cb != 1 && cb != batch)) {
+        p->err += "modal_bptt: batch / n_steps outside the plan, or coeff_batch neither 1 nor batch\n"; return MODAL_EINVAL;
+    }
+    if (!ar->qm1 || !ar->traj_dev || !ar->gout_dev) { p->err += "modal_bptt: qm1, traj_dev and gout_dev are required\n"; return MODAL_EINVAL; }
+    if (nq > md::BP_THREADS_MAX) { p->err += "modal_bptt: n_q <= 512 in this build\n"; return MODAL_EINCOMPAT; }
+    if (p->pending) { modal_status s = finish(p, nullptr); if (s != MODAL_OK && s != MODAL_EUNSTABLE) return s; }
+    CU(cudaSetDevice(p->device));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    enum { B_H, B_C1, B_C2, B_C3, B_S, B_W, B_QM1, B_GQ0, B_GQM1, B_GC1, B_GC2, B_GC3, B_GW, B_GS, B_AUX, B_SCR };
+    // dense fp32 H in plan order (once per H)
+    const size_t nH = (size_t)nphi * nq * nq;
+    const int ld = (nq + 3) & ~3;                                   // row stride: 16-byte loads
+    if (!p->bp_H_valid) {
+        std::vector<double> Hi(nH);
+        mh::unpack_flow_tiles(nq, nphi, p->Hf, Hi.data());
+        std::vector<float> Hu((size_t)nphi * nq * ld, 0.f);
+        for (int n = 0; n < nphi; ++n)
+            for (int a = 0; a < nq; ++a)
+                for (int b = 0; b < nq; ++b) Hu[((size_t)n * nq + p->perm[a]) * ld + p->perm[b]] = (float)Hi[((size_t)n * nq + a) * nq + b];
+        CU(p->bp[B_H].ensure(Hu.size() * 4));
+        CU(cudaMemcpy(p->bp[B_H].p, Hu.data(), Hu.size() * 4, cudaMemcpyHostToDevice));
+        p->bp_H_valid = true;
+    }
+    // canonical coefficients in plan order (masked modes: zero rows, as in the forward kernels)
+    std::vector<double> c1((size_t)cb * nq, 0.0), c2(c1), c3(c1);
+    std::vector<float> w((size_t)cb * nq, 0.f), s((size_t)cb * nphi);
+    std::vector<int> act((size_t)cb * nq, 0);
+    for (int b = 0; b < cb; ++b)
+        for (int k = 0; k < nq; ++k) {
+            const size_t o = (size_t)b * nq + k;
+            const double om = p->omega[o], sg = p->sigma[o];
+            if (!(mh::mode_active(d.scheme, om, sg, p->T) && std::isfinite(om) && std::isfinite(sg))) continue;
+            if (d.scheme == MODAL_FTM && !(om > sg)) { p->err += "modal_bptt: FTM scheme with an overdamped mode\n"; return MODAL_EINVAL; }
+            const mh::StepCoeffs c = mh::step_coeffs(d.scheme, om, sg, p->T);
+            act[o] = 1; c1[o] = 1.0 + c.kv - c.kq; c2[o] = -c.kv; c3[o] = c.r; w[o] = (float)p->pickup[o];
+        }
+    for (size_t i = 0; i < s.size(); ++i) s[i] = (float)p->nl_scale[i];
+    std::vector<double> qm1((size_t)batch * nq);
+    for (int b = 0; b < batch; ++b)
+        for (int k = 0; k < nq; ++k) qm1[(size_t)b * nq + k] = act[(size_t)(cb == 1 ? 0 : b) * nq + k] ? ar->qm1[(size_t)b * nq + k] : 0.0;
+    auto up = [&](int i, const void *src, size_t bytes) -> cudaError_t {
+        cudaError_t e = p->bp[i].ensure(bytes);
+        return e != cudaSuccess ? e : cudaMemcpyAsync(p->bp[i].p, src, bytes, cudaMemcpyHostToDevice, st);
+    };
+    CU(up(B_C1, c1.data(), c1.size() * 8)); CU(up(B_C2, c2.data(), c2.size() * 8)); CU(up(B_C3, c3.data(), c3.size() * 8));
+    CU(up(B_S, s.data(), s.size() * 4)); CU(up(B_W, w.data(), w.size() * 4)); CU(up(B_QM1, qm1.data(), qm1.size() * 8));
+    const size_t nbq = (size_t)batch * nq * 8, nbs = (size_t)batch * nphi * 8;
+    for (int i : {B_GQ0, B_GQM1, B_GC1, B_GC2, B_GC3, B_GW}) CU(p->bp[i].ensure(nbq));
+    CU(p->bp[B_GS].ensure(nbs));
+    CU(cudaMemsetAsync(p->bp[B_GS].p, 0, nbs, st));
+    const bool wantH = ar->grad_H != nullptr;
+    const size_t n_mu = (size_t)batch * n_steps * nq * 4, n_sc = (size_t)batch * n_steps * nphi * 4;
+    if (wantH) CU(p->bp[B_AUX].ensure(n_mu + 2 * n_sc + nH * 8));
+    CU(p->dtimeout.ensure(4));
+    CU(cudaMemsetAsync(p->dtimeout.p, 0, 4, st));
+    // launches of co-resident teams: G CTAs per sample, samples per launch <= SMs
+    const int per_launch = std::min(batch, p->sm_count);
+    int G = std::min({p->sm_count / per_launch, nphi, md::BP_G_MAX});
+    const size_t nscr = (size_t)2 * per_launch * G * nq * 16;
+    CU(p->bp[B_SCR].ensure(std::max<size_t>(nscr, 16)));
+    const int threads = md::BP_THREADS_MAX;
+    // the modes of a CTA stay in shared memory when they fit (C2: 4 modes x 40 KB); otherwise H streams from L2 every step
+    const int modes_max = (nphi + G - 1) / G;
+    const size_t hs_bytes = (size_t)modes_max * nq * ld * 4;
+    const int resident = hs_bytes + 28 * 1024 <= SMEM_LIMIT ? 1 : 0;
+    const int NJ = std::max(1, std::min(md::BP_THREADS_MAX / (ld / 4), nq));
+    const size_t dyn = resident ? hs_bytes : 0;
+    if (resident) CU(cudaFuncSetAttribute(md::vk_bptt_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+    for (int b0 = 0; b0 < batch; b0 += per_launch) {
+        const int nb = std::min(per_launch, batch - b0);
+        md::BpttArgs a{};
+        a.n_q = nq; a.n_phi = nphi; a.batch = nb; a.n_steps = n_steps; a.G = G; a.ld = ld; a.NJ = NJ;
+        a.cb_q = cb == 1 ? 0 : nq; a.cb_phi = cb == 1 ? 0 : nphi;
+        const size_t oq = cb == 1 ? 0 : (size_t)b0 * nq, op = cb == 1 ? 0 : (size_t)b0 * nphi;
+        a.H = p->bp[B_H].as<float>();
+        a.c1 = p->bp[B_C1].as<double>() + oq; a.c2 = p->bp[B_C2].as<double>() + oq; a.c3 = p->bp[B_C3].as<double>() + oq;
+        a.s = p->bp[B_S].as<float>() + op; a.w = p->bp[B_W].as<float>() + oq;
+        a.traj = ar->traj_dev + (size_t)b0 * n_steps * nq; a.qm1 = p->bp[B_QM1].as<double>() + (size_t)b0 * nq;
+        a.gout = ar->gout_dev + (size_t)b0 * n_steps;
+        const size_t ob = (size_t)b0 * nq;
+        a.g_q0 = p->bp[B_GQ0].as<double>() + ob; a.g_qm1 = p->bp[B_GQM1].as<double>() + ob; a.g_c1 = p->bp[B_GC1].as<double>() + ob;
+        a.g_c2 = p->bp[B_GC2].as<double>() + ob; a.g_c3 = p->bp[B_GC3].as<double>() + ob; a.g_w = p->bp[B_GW].as<double>() + ob;
+        a.g_s = p->bp[B_GS].as<double>() + (size_t)b0 * nphi;
+        if (wantH) {
+            unsigned char *aux = p->bp[B_AUX].as<unsigned char>();
+            a.mu_traj = reinterpret_cast<float *>(aux) + (size_t)b0 * n_steps * nq;
+            a.dsc = reinterpret_cast<float *>(aux + n_mu) + (size_t)b0 * n_steps * nphi;
+            a.esc = reinterpret_cast<float *>(aux + n_mu + n_sc) + (size_t)b0 * n_steps * nphi;
+        }
+        a.scratch = p->bp[B_SCR].as<unsigned long long>();
+        a.timeout_flag = p->dtimeout.as<int>();
+        if (G > 1) CU(cudaMemsetAsync(p->bp[B_SCR].p, 0, (size_t)2 * nb * G * nq * 16, st));
+        if (resident) md::vk_bptt_kernel<true><<<nb * G, threads, dyn, st>>>(a);
+        else md::vk_bptt_kernel<false><<<nb * G, threads, 0, st>>>(a);
+        CU(cudaGetLastError());
+    }
+    std::vector<double> gH;
+    if (wantH) {
+        unsigned char *aux = p->bp[B_AUX].as<unsigned char>();
+        double *dgH = reinterpret_cast<double *>(aux + n_mu + 2 * n_sc);
+        md::vk_gradH_kernel<<<dim3(nphi, (nq + 15) / 16), threads, 0, st>>>(nq, nphi, batch, n_steps, ar->traj_dev, reinterpret_cast<const float *>(aux),
+                                                                          reinterpret_cast<const float *>(aux + n_mu), reinterpret_cast<const float *>(aux + n_mu + n_sc), dgH);
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(ar->grad_H, dgH, nH * 8, cudaMemcpyDeviceToHost, st));
+    }
+    std::vector<double> gc1((size_t)batch * nq), gc2(gc1), gc3(gc1);
+    int flag = 0;
+    auto down = [&](int i, double *dst, size_t bytes) -> cudaError_t { return dst ? cudaMemcpyAsync(dst, p->bp[i].p, bytes, cudaMemcpyDeviceToHost, st) : cudaSuccess; };
+    CU(down(B_GQ0, ar->grad_q0, nbq)); CU(down(B_GQM1, ar->grad_qm1, nbq)); CU(down(B_GW, ar->grad_pickup, nbq)); CU(down(B_GS, ar->grad_nl_scale, nbs));
+    CU(down(B_GC1, gc1.data(), nbq)); CU(down(B_GC2, gc2.data(), nbq)); CU(down(B_GC3, gc3.data(), nbq));
+    CU(cudaMemcpyAsync(&flag, p->dtimeout.p, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (flag) { p->err += "modal_bptt: a cross-CTA exchange timed out (team not co-resident?)\n"; return MODAL_ECUDA; }
+    // the forward recurrence uses -c3 f: dL/dc3 as defined in modal.h (q+ = c1 q + c2 q- + c3 (fext - f)) is what the kernel accumulated
+    for (int b = 0; b < batch; ++b)
+        for (int k = 0; k < nq; ++k) {
+            const size_t o = (size_t)b * nq + k, oc = (size_t)(cb == 1 ? 0 : b) * nq + k;
+            if (ar->grad_c1) ar->grad_c1[o] = gc1[o];
+            if (ar->grad_c2) ar->grad_c2[o] = gc2[o];
+            if (ar->grad_c3) ar->grad_c3[o] = gc3[o];
+            double gw_ = 0.0, gg_ = 0.0;
+            if (act[oc]) {
+                const CoeffDerivs cd = coeff_derivs(d.scheme, p->omega[oc], p->sigma[oc], p->T);
+                gw_ = gc1[o] * cd.c1_w + gc3[o] * cd.c3_w;
+                gg_ = gc1[o] * cd.c1_g + gc2[o] * cd.c2_g + gc3[o] * cd.c3_g;
+            }
+            if (ar->grad_omega) ar->grad_omega[o] = gw_;
+            if (ar->grad_sigma) ar->grad_sigma[o] = gg_;
+        }
+    return MODAL_OK;
+}
+
 extern "C" modal_status modal_plan_check(modal_plan *p, int *first_bad_step)
 {
     if (!p) return MODAL_EINVAL;
@@ -1166,6 +1333,7 @@ extern "C" void modal_plan_destroy(modal_plan *p)
                           &p->dout, &p->dHf, &p->dfx, &p->dgx, &p->dqx, &p->dtiming, &p->dperm, &p->dtimeout, &p->mma.dslabs, &p->mma.dtab,
                           &p->mma.dQop, &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags, &p->mma.dpx, &p->stream.dA, &p->stream.dtab,
                           &p->stream.dqx, &p->stream.dGx, &p->stream.dfx, &p->stream.dpx}) b->release();
+    for (DevBuf &b : p->bp) b.release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         if (p->pinned_out) cudaFreeHost(p->pinned_out);
     }

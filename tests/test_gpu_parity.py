@@ -494,6 +494,57 @@ def test_airy_ritz_basis_parity(n_q, n_phi, batch, impl):
     assert np.max(np.abs(gpu_sine[sub][strong] - gpu[sub][strong])) > 1e-3 * np.max(np.abs(gpu[sub][strong]))
 
 
+# ------------------------------------------------------ reverse pass (8(f) row 3) ----
+@pytest.mark.parametrize("n_q,n_phi,batch,n_steps,scheme", [
+    (10, 10, 2, 400, 0),            # C0's mode counts; teams of 10 CTAs (one in-plane mode each)
+    (37, 13, 3, 300, 0),            # ragged sizes, per-sample geometries
+    (37, 13, 2, 300, 1),            # FTM coefficients (chain rule through Eq. 16-18)
+    (100, 50, 2, 120, 0),           # C2's mode counts
+])
+def test_bptt_gradients_match_oracle_adjoint(n_q, n_phi, batch, n_steps, scheme):
+    """modal_bptt (vk_bptt_kernel + vk_gradH_kernel) against oracle.bptt_vk on the same forward problem: gradients of
+    L = sum_n gout_n out_n (seeded gout) wrt q0, q^-1, c1, c2, c3, omega, sigma, pickup, nl_scale and H.  The forward trajectory
+    comes from modal_simulate itself (traj_dev), as a user would run it.  Tolerance: 2e-3 of the largest entry of each gradient
+    array (fp32 contractions on the GPU against fp64, accumulated over the run)."""
+    torch, mb = _mods()
+    wl = _small_vk_workload(n_q, n_phi, batch, n_steps)
+    wl["A"] = np.minimum(wl["A"], 0.6 * wl["h"])
+    case = orc.assemble(wl, scheme=scheme)
+    plan = plan_with_oracle_inputs(wl, case, scheme=scheme)
+    # the trajectory stays on the device between the two calls, as in a training loop
+    traj = torch.zeros((batch, n_steps, n_q), dtype=torch.float64, device="cuda")
+    out = torch.empty((batch, n_steps), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    st, fb = plan.simulate(case.q0, n_steps, out.data_ptr(), qm1=case.qm1, stream=stream, traj_dev_ptr=traj.data_ptr())
+    torch.cuda.synchronize()
+    assert st == 0
+    rng = np.random.default_rng(7)
+    gout = rng.normal(size=(batch, n_steps)).astype(np.float32)
+    gdev = torch.tensor(gout, device="cuda")
+    g = plan.bptt(case.qm1, n_steps, traj.data_ptr(), gdev.data_ptr(), want_H=True, stream=stream)
+    g2 = plan.bptt(case.qm1, n_steps, traj.data_ptr(), gdev.data_ptr(), want_H=True, stream=stream)
+    for key in g:
+        assert np.array_equal(g[key], g2[key]), key                     # fixed summation orders: bit-reproducible
+    gH_ref = np.zeros_like(g["H"])
+    T = 1.0 / wl["sample_rate"]
+    for b in range(batch):
+        cb = b if case.c1.shape[0] > 1 else 0
+        ref = orc.bptt_vk(case.c1[cb], case.c2[cb], case.c3[cb], case.w[cb], case.nl_scale[cb], case.H, case.q0[b], case.qm1[b], gout[b].astype(np.float64))
+        gH_ref += ref["H"]
+        act = case.active[cb]
+        dd = orc.dcoeffs_domega_dgamma(scheme, np.where(act, case.omega[cb], 2.0), np.where(act, case.gamma[cb], 1.0), T)
+        ref["omega"] = ref["c1"] * dd["c1_w"] + ref["c2"] * dd["c2_w"] + ref["c3"] * dd["c3_w"]
+        ref["sigma"] = ref["c1"] * dd["c1_g"] + ref["c2"] * dd["c2_g"] + ref["c3"] * dd["c3_g"]
+        for key, rk in (("q0", "q0"), ("qm1", "qm1"), ("c1", "c1"), ("c2", "c2"), ("c3", "c3"), ("omega", "omega"), ("sigma", "sigma"),
+                        ("pickup", "w"), ("nl_scale", "s")):
+            want = np.where(act, ref[rk], 0.0) if key != "nl_scale" else ref[rk]
+            scale = np.max(np.abs(want))
+            assert scale > 0, key
+            err = np.max(np.abs(g[key][b] - want)) / scale
+            assert err <= 2e-3, (key, b, err)
+    assert np.max(np.abs(g["H"] - gH_ref)) <= 2e-3 * np.max(np.abs(gH_ref))
+
+
 # ------------------------------------------------------------------ tension / linear ----
 @pytest.mark.parametrize("batch,n_steps", [(32, 4096), (5, 333)])
 def test_c1_string_parity(batch, n_steps):
