@@ -702,9 +702,9 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         const mh::StreamLayout &L = m.L;
         const int NB = m.NB;
         const size_t base = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 0).total;
-        int nstg = (int)std::min<size_t>(md::ST_NSTG_MAX, (SMEM_LIMIT - base) / 8192);
-        if (p->opt.mma_nstg > 0) nstg = std::min(nstg, std::max(p->opt.mma_nstg, L.tiles_max));
-        if (nstg < L.tiles_max) { p->err += "streaming vK kernel: no room for the operand ring (one stage per tile of a CTA)\n"; return MODAL_EINCOMPAT; }
+        int nstg = (int)std::min<size_t>(md::ST_NSTG_MAX, (SMEM_LIMIT - base) / md::ST_STAGE_BYTES);
+        if (p->opt.mma_nstg > 0) nstg = std::min(nstg, std::max(p->opt.mma_nstg, 2));
+        if (nstg < 2) { p->err += "streaming vK kernel: no room for the operand ring\n"; return MODAL_EINCOMPAT; }
         const size_t smem = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, nstg).total;
         const int KOP = L.KC * 16;
         const size_t nqx = (size_t)NB * KOP * 4, nGx = (size_t)d.n_phi * L.NKB * NB * 4, nfx = (size_t)L.G * 128 * NB * 4, npx = (size_t)4 * L.G * NB * 16 + 256;

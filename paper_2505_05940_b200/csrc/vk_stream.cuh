@@ -24,7 +24,8 @@ constexpr int ST_BCH_MAX_DEV = 16, ST_TILES_MAX_DEV = 16, ST_NKB_MAX_DEV = 8, ST
 constexpr unsigned ST_POLL_SLEEP = 100;   // ns between polling rounds
 constexpr int SB_FULL = 0, SB_EMPTY = 16, SB_ACCF = 32, SB_ACCE = 48, SB_BRDY = 49, SB_FDONE = 50, SB_TPTR = 56, SB_ABORT = 57;
 constexpr int ST_BARS_BYTES = 512;
-constexpr int ST_NSTG_MAX = 16;
+constexpr int ST_NSTG_MAX = 8;          // ring stages of ST_STAGE_BYTES
+constexpr int ST_STAGE_BYTES = 16384;   // two K chunks (hi + lo of 128 rows x 16 K each)
 
 struct StreamArgs {
     const uint16_t *A;          // H stream: per tile its K chunks, 8 KiB each (hi 4 KiB, lo 4 KiB), UMMA canonical K-major
@@ -68,7 +69,7 @@ __host__ __device__ inline StreamSmem stream_smem_layout(int NB, int rows_max, i
     o = flow_align(o, 128);
     L.bop = o;   o += (size_t)bch_max * NB * 64;               // q operand chunks: [slot][hi NB x 16 | lo NB x 16] bf16
     o = flow_align(o, 128);
-    L.ring = o;  o += (size_t)nstg * 8192;
+    L.ring = o;  o += (size_t)nstg * ST_STAGE_BYTES;
     L.total = o;
     return L;
 }
@@ -104,6 +105,14 @@ __device__ __forceinline__ uint32_t ld_relaxed1(const uint32_t *p)
 __device__ __forceinline__ void st_relaxed1(uint32_t *p, uint32_t w)
 {
     asm volatile("st.relaxed.gpu.global.b32 [%0], %1;" ::"l"(p), "r"(w) : "memory");
+}
+// one non-blocking probe of a phase
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
 }
 // one try_wait on the fast path; the bounded loop only when the phase is not complete yet
 __device__ __forceinline__ void mbar_wait_fast(uint32_t bar, uint32_t parity, volatile int *abortp)
@@ -613,6 +622,8 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
             // ---------------- P: the H stream of the CTA's tiles, every step, through the ring ----------------
             // (the loops of P and M run on one thread each: no division, no address arithmetic beyond an add per chunk --
             //  a chunk's MMAs take ~180 cycles, a careless loop iteration several hundred)
+            // A ring stage holds TWO K chunks of a tile (16 KiB; the odd last chunk of a tile travels alone): one wait, one commit and
+            // one bulk copy per six MMAs -- at N = 16 .. 64 the MMA phase is bound by these per-stage instructions, not by the math.
             if (lane == 0) {
                 const uint32_t full0 = smem_u32(C.bars + SB_FULL), empty0 = smem_u32(C.bars + SB_EMPTY), ring0 = smem_u32(C.ring);
                 const int NSTG = a.NSTG;
@@ -622,10 +633,11 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
                         const int *tt = C.ttab + i * a.tile_stride;
                         const int nch = tt[1];
                         const uint16_t *src = a.A + (size_t)tt[2] * 4096;
-                        for (int u = 0; u < nch; ++u, src += 4096) {
+                        for (int u = 0; u < nch; u += 2, src += 8192) {
+                            const uint32_t bytes = u + 1 < nch ? 16384u : 8192u;
                             mbar_wait_fast(empty0 + 8 * sg, ph, C.s_abort);
-                            mbar_expect_tx(full0 + 8 * sg, 8192);
-                            tma_bulk_g2s(ring0 + sg * 8192, src, 8192, full0 + 8 * sg);
+                            mbar_expect_tx(full0 + 8 * sg, bytes);
+                            tma_bulk_g2s(ring0 + sg * ST_STAGE_BYTES, src, bytes, full0 + 8 * sg);
                             if (++sg == NSTG) { sg = 0; ph ^= 1u; }
                         }
                     }
@@ -634,6 +646,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
             // ---------------- M: the MMAs ------------------------------------------------------------------------
             // The whole warp runs the (uniform) loop and one elected lane issues: inside a lane-0 branch ptxas wraps every
             // tcgen05 instruction in an ELECT / R2UR / branch loop, ~240 cycles per chunk instead of the ~160 its three MMAs take.
+            // The try_wait of the NEXT stage is issued before the MMAs of this one, so its ~90 cycles overlap their issue.
             {
                 const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NB >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
                 const uint32_t full0 = smem_u32(C.bars + SB_FULL), empty0 = smem_u32(C.bars + SB_EMPTY), accf0 = smem_u32(C.bars + SB_ACCF);
@@ -646,22 +659,34 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
                     if (n > 0) mbar_wait(smem_u32(C.bars + SB_ACCE), (unsigned)(n - 1) & 1u, C.s_abort);    // last step's accumulators read
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const long long tk = TIMING ? clock64() : 0;
+                    bool ready = mbar_try(full0 + 8 * sg, ph);
                     for (int i = 0; i < C.ntiles; ++i) {
                         const int *tt = C.ttab + i * a.tile_stride;
                         const int nch = tt[1];
                         const uint32_t td = C.tbase + (uint32_t)(i * NB);
-                        for (int u = 0; u < nch; ++u) {
+                        for (int u = 0; u < nch; u += 2) {
+                            const bool two = u + 1 < nch;
                             const uint64_t dB = dB0 + (uint64_t)(tt[4 + u] * (NB * 64 / 16));
-                            if (TIMING) { const long long tw = clock64(); mbar_wait_fast(full0 + 8 * sg, ph, C.s_abort); tmw += clock64() - tw; }
-                            else mbar_wait_fast(full0 + 8 * sg, ph, C.s_abort);
-                            const uint64_t dA = dA0 + (uint64_t)(sg * (8192 / 16));
+                            const uint64_t dB2 = dB0 + (uint64_t)(tt[4 + (two ? u + 1 : u)] * (NB * 64 / 16));
+                            if (!ready) {
+                                if (TIMING) { const long long tw = clock64(); mbar_wait(full0 + 8 * sg, ph, C.s_abort); tmw += clock64() - tw; }
+                                else mbar_wait(full0 + 8 * sg, ph, C.s_abort);
+                            }
+                            const int sg0 = sg;
+                            if (++sg == NSTG) { sg = 0; ph ^= 1u; }
+                            ready = mbar_try(full0 + 8 * sg, ph);                              // next stage (this or the next step's)
+                            const uint64_t dA = dA0 + (uint64_t)(sg0 * (ST_STAGE_BYTES / 16));
                             if (elect_one_sync()) {
                                 umma_bf16(td, dA, dB, idesc, u > 0);                           // hi * hi
                                 umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);                   // lo * hi
                                 umma_bf16(td, dA, dB + NB * 32 / 16, idesc, 1);                // hi * lo
-                                umma_commit(empty0 + 8 * sg);
+                                if (two) {
+                                    umma_bf16(td, dA + 8192 / 16, dB2, idesc, 1);
+                                    umma_bf16(td, dA + 12288 / 16, dB2, idesc, 1);
+                                    umma_bf16(td, dA + 8192 / 16, dB2 + NB * 32 / 16, idesc, 1);
+                                }
+                                umma_commit(empty0 + 8 * sg0);
                             }
-                            if (++sg == NSTG) { sg = 0; ph ^= 1u; }
                         }
                         if (elect_one_sync()) umma_commit(accf0 + 8 * i);
                     }
