@@ -176,6 +176,72 @@ struct StreamCta {
     size_t nel;
 };
 
+// q^n of the CTA's K chunks -> bf16 hi / lo operand chunks in shared memory (the B operand of the step's MMAs), by the 128 epilogue
+// threads and the 256 owner threads together (the owners are idle between publishing q^n and the forces of step n).
+constexpr int ST_BUILDERS = 384;
+template <int NB, int IF>   // IF: items (two 16-byte loads each) a thread keeps in flight
+__device__ __forceinline__ void stream_build_B(const StreamArgs &a, const StreamCta &C, const int first, const uint32_t tag)
+{
+    // item = (chunk slot, half of its 16 K, sample): 8 consecutive k of one sample = one 16-byte row of a core matrix;
+    // four items per round: their eight 16-byte loads are in flight together
+    for (int idx0 = first; idx0 < C.nbch * 2 * NB; idx0 += IF * ST_BUILDERS) {
+        uint4 w[IF][2];
+        int valid[IF]; const uint32_t *src[IF]; unsigned char *dst[IF];
+        unsigned pend = 0;
+#pragma unroll
+        for (int v = 0; v < IF; ++v) {
+            const int idx = idx0 + v * ST_BUILDERS;
+            valid[v] = 0; src[v] = a.qx; dst[v] = C.bop;
+            if (idx < C.nbch * 2 * NB) {
+                const int b = idx % NB, g = idx / NB, slot = g >> 1, kh = g & 1;
+                const int ent = C.ctab[6 + slot], kc = ent & 0xffff;
+                valid[v] = min(8, max(0, (ent >> 16) - 8 * kh));
+                src[v] = a.qx + (size_t)b * a.KOP + kc * 16 + kh * 8;
+                dst[v] = C.bop + (size_t)slot * NB * 64 + (b >> 3) * 256 + kh * 128 + (b & 7) * 16;
+                pend |= (valid[v] > 0 ? 1u : 0u) << v;
+                valid[v] |= 16;                                         // in range: the item is written even when it is all padding
+            }
+            w[v][0] = w[v][1] = make_uint4(0u, 0u, 0u, 0u);
+        }
+        unsigned spins = 0;
+        while (pend) {
+#pragma unroll
+            for (int v = 0; v < IF; ++v) if (pend >> v & 1) { w[v][0] = ld_relaxed4(src[v]); w[v][1] = ld_relaxed4(src[v] + 4); }
+#pragma unroll
+            for (int v = 0; v < IF; ++v)
+                if (pend >> v & 1) {
+                    const int nv = valid[v] & 15;
+                    const uint32_t ww[8] = {w[v][0].x, w[v][0].y, w[v][0].z, w[v][0].w, w[v][1].x, w[v][1].y, w[v][1].z, w[v][1].w};
+                    bool ok = true;
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) ok = ok && (e >= nv || (ww[e] & 3u) == tag);
+                    if (ok) pend &= ~(1u << v);
+                }
+            if (pend) {
+                if ((++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 21))) { *C.s_abort = 1; break; }
+                __nanosleep(ST_POLL_SLEEP);
+            }
+        }
+#pragma unroll
+        for (int v = 0; v < IF; ++v) {
+            if (!(valid[v] & 16)) continue;
+            const int nv = valid[v] & 15;
+            const uint32_t ww[8] = {w[v][0].x, w[v][0].y, w[v][0].z, w[v][0].w, w[v][1].x, w[v][1].y, w[v][1].z, w[v][1].w};
+            uint32_t hi[8], lo[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const float x = e < nv ? untag(ww[e]) : 0.f;
+                hi[e] = bf16_rn_dev(x);
+                lo[e] = bf16_rn_dev(x - __uint_as_float(hi[e] << 16));
+            }
+            *reinterpret_cast<uint4 *>(dst[v]) = make_uint4(hi[0] | (hi[1] << 16), hi[2] | (hi[3] << 16), hi[4] | (hi[5] << 16), hi[6] | (hi[7] << 16));
+            *reinterpret_cast<uint4 *>(dst[v] + NB * 32) = make_uint4(lo[0] | (lo[1] << 16), lo[2] | (lo[3] << 16), lo[4] | (lo[5] << 16), lo[6] | (lo[7] << 16));
+        }
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_arrive(smem_u32(C.bars + SB_BRDY));
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // E: 128 threads = the 128 rows of a tile (thread <-> TMEM lane <-> row k of the CTA's block).
 // ------------------------------------------------------------------------------------------------------------
@@ -192,67 +258,11 @@ __device__ __forceinline__ void stream_epilogue(const StreamArgs &a, const Strea
         long long tk = tmg ? clock64() : 0;
         // ---- wait for q^n: warp 0 polls one word of every owner CTA this CTA reads from ---------------------
         if (w4 == 0) warp_poll_sentinels(C.ctab[6 + ST_BCH_MAX_DEV], lane, tag, C.s_abort, [&](int x) { return a.qx + C.ctab[7 + ST_BCH_MAX_DEV + x]; });
+        if (w4 == 0) asm volatile("bar.arrive 4, 288;" ::: "memory");          // the owners build their share of the B operand
         bar_named(1, 128);
         if (tmg) { const long long t_ = clock64(); tm[7] += t_ - tk; }
-        // ---- (a) q^n of the CTA's K chunks -> bf16 hi / lo operand chunks in shared memory ------------------
-        // item = (chunk slot, half of its 16 K, sample): 8 consecutive k of one sample = one 16-byte row of a core matrix;
-        // four items per round: their eight 16-byte loads are in flight together
-        for (int idx0 = r; idx0 < C.nbch * 2 * NB; idx0 += 4 * 128) {
-            uint4 w[4][2];
-            int valid[4]; const uint32_t *src[4]; unsigned char *dst[4];
-            unsigned pend = 0;
-#pragma unroll
-            for (int v = 0; v < 4; ++v) {
-                const int idx = idx0 + v * 128;
-                valid[v] = 0; src[v] = a.qx; dst[v] = C.bop;
-                if (idx < C.nbch * 2 * NB) {
-                    const int b = idx % NB, g = idx / NB, slot = g >> 1, kh = g & 1;
-                    const int ent = C.ctab[6 + slot], kc = ent & 0xffff;
-                    valid[v] = min(8, max(0, (ent >> 16) - 8 * kh));
-                    src[v] = a.qx + (size_t)b * a.KOP + kc * 16 + kh * 8;
-                    dst[v] = C.bop + (size_t)slot * NB * 64 + (b >> 3) * 256 + kh * 128 + (b & 7) * 16;
-                    pend |= (valid[v] > 0 ? 1u : 0u) << v;
-                    valid[v] |= 16;                                         // in range: the item is written even when it is all padding
-                }
-                w[v][0] = w[v][1] = make_uint4(0u, 0u, 0u, 0u);
-            }
-            unsigned spins = 0;
-            while (pend) {
-#pragma unroll
-                for (int v = 0; v < 4; ++v) if (pend >> v & 1) { w[v][0] = ld_relaxed4(src[v]); w[v][1] = ld_relaxed4(src[v] + 4); }
-#pragma unroll
-                for (int v = 0; v < 4; ++v)
-                    if (pend >> v & 1) {
-                        const int nv = valid[v] & 15;
-                        const uint32_t ww[8] = {w[v][0].x, w[v][0].y, w[v][0].z, w[v][0].w, w[v][1].x, w[v][1].y, w[v][1].z, w[v][1].w};
-                        bool ok = true;
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) ok = ok && (e >= nv || (ww[e] & 3u) == tag);
-                        if (ok) pend &= ~(1u << v);
-                    }
-                if (pend) {
-                    if ((++spins & 1023u) == 0 && (*C.s_abort || spins > (1u << 21))) { *C.s_abort = 1; break; }
-                    __nanosleep(ST_POLL_SLEEP);
-                }
-            }
-#pragma unroll
-            for (int v = 0; v < 4; ++v) {
-                if (!(valid[v] & 16)) continue;
-                const int nv = valid[v] & 15;
-                const uint32_t ww[8] = {w[v][0].x, w[v][0].y, w[v][0].z, w[v][0].w, w[v][1].x, w[v][1].y, w[v][1].z, w[v][1].w};
-                uint32_t hi[8], lo[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const float x = e < nv ? untag(ww[e]) : 0.f;
-                    hi[e] = bf16_rn_dev(x);
-                    lo[e] = bf16_rn_dev(x - __uint_as_float(hi[e] << 16));
-                }
-                *reinterpret_cast<uint4 *>(dst[v]) = make_uint4(hi[0] | (hi[1] << 16), hi[2] | (hi[3] << 16), hi[4] | (hi[5] << 16), hi[6] | (hi[7] << 16));
-                *reinterpret_cast<uint4 *>(dst[v] + NB * 32) = make_uint4(lo[0] | (lo[1] << 16), lo[2] | (lo[3] << 16), lo[4] | (lo[5] << 16), lo[6] | (lo[7] << 16));
-            }
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_arrive(smem_u32(C.bars + SB_BRDY));
+        // ---- (a) the B operand of the step: this thread's share of the items (stream_build_B) ------------
+        stream_build_B<NB, 4>(a, C, r, tag);
         if (tmg) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
         // ---- (b) q^n of the thread's own row, every sample -------------------------------------------------
         float qk[NB];
@@ -390,6 +400,8 @@ __device__ __forceinline__ void stream_owner_steps(const StreamArgs &a, const St
     for (int n = n_begin; n < n_end; ++n) {
         const uint32_t tag = ((uint32_t)n + 1u) & 3u, tag_next = ((uint32_t)n + 2u) & 3u;
         long long tk = tmg ? clock64() : 0;
+        asm volatile("bar.sync 4, 288;" ::: "memory");                        // q^n complete (the epilogue warp that polls the sentinels arrives)
+        stream_build_B<NB, (NB >= 64 ? 2 : 4)>(a, C, 128 + tl, tag);
         float2 *pk = C.pk + (size_t)(n & 1) * C.nel;
         // no force of step n is complete before the CTA's own epilogue has stored its part: sleep on a CTA barrier until then instead
         // of polling L2 through the whole MMA phase (148 x 192 lanes x 10 loads in flight would eat the bandwidth the H stream needs)
@@ -581,7 +593,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
     if (tid == 0) {
         for (int s = 0; s < a.NSTG; ++s) { mbar_init(smem_u32(C.bars + SB_FULL + s), 1); mbar_init(smem_u32(C.bars + SB_EMPTY + s), 1); }
         for (int s = 0; s < ST_TILES_MAX_DEV; ++s) mbar_init(smem_u32(C.bars + SB_ACCF + s), 1);
-        mbar_init(smem_u32(C.bars + SB_ACCE), 128); mbar_init(smem_u32(C.bars + SB_BRDY), 128); mbar_init(smem_u32(C.bars + SB_FDONE), 128);
+        mbar_init(smem_u32(C.bars + SB_ACCE), 128); mbar_init(smem_u32(C.bars + SB_BRDY), ST_BUILDERS); mbar_init(smem_u32(C.bars + SB_FDONE), 128);
         *C.s_abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -607,14 +619,14 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
     C.tbase = *tptr;
 
     if (warp >= 8) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 120;");
+        if (NB >= 64) asm volatile("setmaxnreg.dec.sync.aligned.u32 120;"); else asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
         const int tl = tid - 256;
         if (a.LPQ == 1) stream_owner<NB, 1, TIMING>(a, C, tl);
         else if (a.LPQ == 2) stream_owner<NB, 2, TIMING>(a, C, tl);
         else if (a.LPQ == 4) stream_owner<NB, 4, TIMING>(a, C, tl);
         else stream_owner<NB, 8, TIMING>(a, C, tl);
     } else if (warp >= 4) {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+        if (NB >= 64) asm volatile("setmaxnreg.inc.sync.aligned.u32 232;"); else asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
         stream_epilogue<NB, TIMING>(a, C, (warp & 3) * 32 + lane, lane, warp & 3);
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
