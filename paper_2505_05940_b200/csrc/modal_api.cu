@@ -19,6 +19,7 @@
 #include "vk_mma.cuh"
 #include "vk_stream.cuh"
 #include "vk_bptt.cuh"
+#include "vk_small.cuh"
 #include "peaks.cuh"
 
 namespace mh = modal_host;
@@ -103,6 +104,7 @@ struct modal_plan {
     StreamConfig stream;
     DevBuf bp[16];                                                    // modal_bptt: dense H, coefficients, gradients, scratch
     bool bp_H_valid = false;
+    DevBuf dHsmall; bool small_H_valid = false;                       // vk_small_kernel: dense fp32 H, internal order
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dkv, dkq, dr, dast, ds, dsT, dw, dlam, dc, dq0, dv0, dgain, dbad, dout;      // dsT: s_n transposed [n_phi][coeff_batch] (batched kernel)
     float *pinned_out = nullptr; size_t pinned_bytes = 0;            // staging of modal_simulate_host
@@ -156,7 +158,7 @@ void set_H(modal_plan *p, Get get_user)
     }
     for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
     p->flow_cfgs.clear();                                   // schedules depend on the zero pattern
-    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0; p->bp_H_valid = false;
+    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0; p->bp_H_valid = false; p->small_H_valid = false;
     p->H_dirty = true;
 }
 
@@ -655,7 +657,11 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
     // vK kernel family: the batched tensor-core kernel when H fits the shared memory of the GPU (batch >= 64), the streaming
     // tensor-core kernel when it does not (batch >= 8), else the FP32 flow kernel; "vk_impl" forces one
     bool use_mma = false, use_stream = false;
-    if (d.model == MODAL_VK) {
+    // small systems (the paper's 10-mode benchmark point): one warp per sample, no barriers, no exchange (vk_small.cuh)
+    const bool use_small = d.model == MODAL_VK && nq <= 32 && d.n_phi <= 32 && (long long)d.n_phi * nq * nq <= 8192 &&
+                           (p->opt.vk_impl == 0 || p->opt.vk_impl == 4) && p->opt.flow_g == 0 && p->opt.flow_ns == 0 && p->opt.flow_res < 0;
+    if (d.model == MODAL_VK && p->opt.vk_impl == 4 && !use_small) { p->err += "vk_impl=4: the small-system kernel needs N_q, N_phi <= 32 and N_phi N_q^2 <= 8192\n"; return MODAL_EINCOMPAT; }
+    if (d.model == MODAL_VK && !use_small) {
         const int impl = p->opt.vk_impl;
         if ((impl == 0 && batch >= 64) || impl == 2) { modal_status s = configure_mma(p); if (s != MODAL_OK) return s; use_mma = p->mma.ok; }
         if (!use_mma && ((impl == 0 && batch >= 8) || impl == 3)) {
@@ -697,6 +703,36 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         CU(e);
         p->kinfo[0] = 1; p->kinfo[1] = 1; p->kinfo[2] = (batch + 3) / 4; p->kinfo[3] = 128;
         p->kinfo[4] = 0; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
+    } else if (use_small) {
+        if (!p->small_H_valid) {
+            const size_t nH = (size_t)d.n_phi * nq * nq;
+            std::vector<double> Hi(nH);
+            mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, Hi.data());
+            std::vector<float> Hd(nH);
+            for (size_t i = 0; i < nH; ++i) Hd[i] = (float)Hi[i];
+            CU(p->dHsmall.ensure(nH * 4));
+            CU(cudaMemcpy(p->dHsmall.p, Hd.data(), nH * 4, cudaMemcpyHostToDevice));
+            p->small_H_valid = true;
+        }
+        md::SmallArgs a{};
+        a.Hd = p->dHsmall.as<float>(); a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P; a.batch = batch; a.n_steps = n_steps;
+        a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
+        a.kv = p->dkv.as<double>(); a.kq = p->dkq.as<double>(); a.r = p->dr.as<double>(); a.astart = p->dast.as<double>();
+        a.s = p->ds.as<float>(); a.w = p->dw.as<float>();
+        a.q0 = p->dq0.as<double>(); a.v0 = p->dv0.as<double>();
+        a.auto_start = auto_start; a.half_T2 = half_T2;
+        a.fext = init->fext_signal; a.gain = p->dgain.as<double>();
+        a.out = out_dev; a.traj = init->traj_dev; a.kperm = p->dperm.as<int>(); a.first_bad = p->dbad.as<int>();
+        const size_t smem = md::small_smem_bytes(nq, d.n_phi);
+        const bool hreg = nq <= 16 && d.n_phi * nq <= 128;
+        CU(cudaFuncSetAttribute(md::vk_small_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaFuncSetAttribute(md::vk_small_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        const int blocks = (batch + md::SM_WARPS - 1) / md::SM_WARPS;
+        if (hreg) md::vk_small_kernel<true><<<blocks, md::SM_WARPS * 32, smem, st>>>(a);
+        else md::vk_small_kernel<false><<<blocks, md::SM_WARPS * 32, smem, st>>>(a);
+        CU(cudaGetLastError());
+        p->kinfo[0] = 2; p->kinfo[1] = 1; p->kinfo[2] = blocks; p->kinfo[3] = md::SM_WARPS * 32;
+        p->kinfo[4] = (int)smem; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
     } else if (use_stream) {
         StreamConfig &m = p->stream;
         const mh::StreamLayout &L = m.L;
@@ -1253,7 +1289,7 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
     if (!p || !key) return MODAL_EINVAL;
     p->err.clear();
     struct { const char *name; int *field; int lo, hi; } tab[] = {
-        {"vk_impl", &p->opt.vk_impl, 0, 3}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
+        {"vk_impl", &p->opt.vk_impl, 0, 4}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
         {"flow_res", &p->opt.flow_res, -1, 1 << 20}, {"mma_split", &p->opt.mma_split, 0, 4}, {"mma_ng", &p->opt.mma_ng, 0, 8},
         {"mma_nstg", &p->opt.mma_nstg, 0, 16}, {"mma_cluster", &p->opt.mma_cluster, 0, 1}, {"parity_order", &p->opt.parity_order, 0, 1}, {"timing", &p->opt.timing, 0, 1}};
     for (auto &t : tab)
@@ -1334,6 +1370,7 @@ extern "C" void modal_plan_destroy(modal_plan *p)
                           &p->mma.dQop, &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags, &p->mma.dpx, &p->stream.dA, &p->stream.dtab,
                           &p->stream.dqx, &p->stream.dGx, &p->stream.dfx, &p->stream.dpx}) b->release();
     for (DevBuf &b : p->bp) b.release();
+    p->dHsmall.release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         if (p->pinned_out) cudaFreeHost(p->pinned_out);
     }

@@ -494,6 +494,38 @@ def test_airy_ritz_basis_parity(n_q, n_phi, batch, impl):
     assert np.max(np.abs(gpu_sine[sub][strong] - gpu[sub][strong])) > 1e-3 * np.max(np.abs(gpu[sub][strong]))
 
 
+@pytest.mark.parametrize("n_q,n_phi,batch,n_steps,scheme", [
+    (10, 10, 1, 2000, 0),           # C0's mode counts
+    (10, 10, 7, 700, 1),            # FTM, ragged batch (two CTAs of four warps)
+    (32, 8, 5, 500, 0),             # the widest system of this kernel
+    (3, 1, 2, 300, 0),
+])
+def test_vk_small_kernel_parity(n_q, n_phi, batch, n_steps, scheme):
+    """Small-system kernel (one warp per sample) against the oracle, against the flow kernel on the same plan, with an external
+    force, the device-side start and the trajectory output."""
+    torch, mb = _mods()
+    wl = _small_vk_workload(n_q, n_phi, batch, n_steps)
+    case = orc.assemble(wl, scheme=scheme)
+    rng = np.random.default_rng(3)
+    fext = np.zeros((batch, n_steps)); t = np.arange(48)
+    fext[:, 10:58] = 0.5 * (1 - np.cos(2 * np.pi * t / 48))[None] * rng.uniform(0.5, 2.0, (batch, 1))
+    gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
+    ref = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, case.q0, case.qm1, n_steps, nl_scale=case.nl_scale,
+                       H=case.H, fext=orc.f32(fext), fext_gain=gain, want_traj=True)
+    plan = plan_with_oracle_inputs(wl, case, scheme=scheme)
+    gpu, fb, traj, st = gpu_run(plan, case.q0, None, n_steps, want_traj=True, fext=fext, fext_gain=gain)
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 2 and st == 0 and np.all(fb == -1)
+    check_parity(gpu, ref["out"], case)
+    assert np.max(np.abs(traj - ref["traj"])) <= 1e-4 * np.max(np.abs(ref["traj"]))
+    plan.set_option("vk_impl", 1)
+    flow, _, _, _ = gpu_run(plan, case.q0, None, n_steps, fext=fext, fext_gain=gain)
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 3
+    assert np.max(np.abs(flow - gpu)) <= 1e-5 * np.max(np.abs(gpu))
+    plan.set_option("vk_impl", 0)
+    gpu2, _, _, _ = gpu_run(plan, case.q0, None, n_steps, fext=fext, fext_gain=gain)
+    assert np.array_equal(gpu, gpu2)
+
+
 # ------------------------------------------------------ reverse pass (8(f) row 3) ----
 @pytest.mark.parametrize("n_q,n_phi,batch,n_steps,scheme", [
     (10, 10, 2, 400, 0),            # C0's mode counts; teams of 10 CTAs (one in-plane mode each)
