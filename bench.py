@@ -146,6 +146,12 @@ def roofline_for(wl, B, n_steps, per_launch, info, tile_stats, pk, stream=None):
                 "tiles": tiles, "tiles_nonzero": nz, "achieved_read": read, "frac_read": read / hbm_peak,
                 "l2_read_peak_64mb": pk.get("l2_read_gbs_64mb") if pk else None,
                 "frac_read_of_l2": read / pk["l2_read_gbs_64mb"] if pk else None}
+    if fam == 2:          # small-system kernel: one warp per sample, a dependent chain of a few hundred cycles per step (latency, not a pipe)
+        ach = flops * B * n_steps / per_launch / 1e12
+        peak = pk["fp32_tflops"] if pk else FP32_NOMINAL_TFLOPS
+        return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                "peak_source": "measured in this run (modal_measure_peaks, FP32 FMA)" if pk else "nominal FP32 pipe (peaks skipped)",
+                "kernel": "vk_small_kernel", "note": "latency-bound by construction: one warp advances one sample, no barrier, no exchange"}
     # tension / linear kernel: every FMA of the update is fp64 (DFMA), so the bound is the FP64 pipe
     ach = flops * B * n_steps / per_launch / 1e12
     peak = pk["fp64_tflops"] if pk else FP32_NOMINAL_TFLOPS

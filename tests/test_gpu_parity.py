@@ -210,7 +210,7 @@ def test_vk_flow_team_shapes_parity(n_q, n_phi, batch, G, NS, RES):
     wl = _small_vk_workload(n_q, n_phi, batch, 1500)
     case = orc.assemble(wl)
     ref = orc.run_case(case, 1500)
-    plan = plan_with_oracle_inputs(wl, case, options=dict(flow_g=G, flow_ns=NS, flow_res=RES))
+    plan = plan_with_oracle_inputs(wl, case, options=dict(vk_impl=1, flow_g=G, flow_ns=NS, flow_res=RES))       # vk_impl=1: the flow kernel also where the small-system kernel would be chosen
     gpu, fb, _, st = gpu_run(plan, case.q0, case.qm1, 1500)
     assert st == 0 and np.all(fb == -1)
     check_parity(gpu, ref["out"], case)
