@@ -1202,7 +1202,7 @@ extern "C" modal_status modal_bptt(modal_plan *p, int batch, int n_steps, const 
     CU(cudaMemsetAsync(p->dtimeout.p, 0, 4, st));
     // launches of co-resident teams: G CTAs per sample, samples per launch <= SMs
     const int per_launch = std::min(batch, p->sm_count);
-    int G = std::min({p->sm_count / per_launch, nphi, md::BP_G_MAX});
+    int G = std::min({p->sm_count / per_launch, nphi, md::BP_G_MAX, 8 * std::min(md::BP_THREADS_MAX / ((nq + 3) & ~3), 8)});
     const size_t nscr = (size_t)2 * per_launch * G * nq * 16;
     CU(p->bp[B_SCR].ensure(std::max<size_t>(nscr, 16)));
     const int threads = md::BP_THREADS_MAX;

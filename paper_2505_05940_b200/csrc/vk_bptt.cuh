@@ -22,7 +22,7 @@
 namespace modal_dev {
 
 constexpr int BP_THREADS_MAX = 512;     // one thread per transverse mode: n_q <= 512; the kernel always runs 512 threads (16 warps share the rows)
-constexpr int BP_G_MAX = 16;
+constexpr int BP_G_MAX = 32;             // CTAs of a team (also bounded by 8 x (512 / row stride): eight sources per gathering thread)
 
 struct BpttArgs {
     int n_q, n_phi, batch, n_steps, G, cb_q, cb_phi;        // cb_*: coefficient row stride per sample (0: one row for all)
@@ -146,26 +146,41 @@ __global__ void __launch_bounds__(BP_THREADS_MAX) vk_bptt_kernel(const BpttArgs 
             if (mine) {
                 st_tag(base + ((size_t)g * a.n_q + k) * 2, jacc, epoch);
                 st_tag(base + ((size_t)g * a.n_q + k) * 2 + 1, facc, epoch);
-                // all G loads in flight together (one after the other they cost an L2 round trip each); team order for the sums
-                float2 v[BP_G_MAX];
-                unsigned pend = (1u << a.G) - 1u, spins = 0;
+            }
+            // gather: thread (sub, kk) takes the sources sub, sub + NSUB, ... (at most eight, all in flight together) of mode kk; the
+            // sub-group partials are joined through shared memory in sub order: every CTA of the team adds the same numbers in the same order
+            const int NSUB = min(BP_THREADS_MAX / ld, 8);
+            const int sub = k / ld, kk = k - sub * ld;
+            if (sub < NSUB && kk < a.n_q) {
+                float2 v[8];
+                unsigned pend = 0, spins = 0;
+#pragma unroll
+                for (int u = 0; u < 8; ++u) if (sub + u * NSUB < a.G) pend |= 1u << u;
+                const unsigned have = pend;
                 while (pend) {
-                    unsigned long long w0[BP_G_MAX], w1[BP_G_MAX];
+                    unsigned long long w0[8], w1[8];
 #pragma unroll
-                    for (int gg = 0; gg < BP_G_MAX; ++gg)
-                        if (pend >> gg & 1)
-                            asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(w0[gg]), "=l"(w1[gg]) : "l"(base + ((size_t)gg * a.n_q + k) * 2) : "memory");
+                    for (int u = 0; u < 8; ++u)
+                        if (pend >> u & 1)
+                            asm volatile("ld.relaxed.gpu.global.v2.b64 {%0, %1}, [%2];" : "=l"(w0[u]), "=l"(w1[u])
+                                         : "l"(base + ((size_t)(sub + u * NSUB) * a.n_q + kk) * 2) : "memory");
 #pragma unroll
-                    for (int gg = 0; gg < BP_G_MAX; ++gg)
-                        if ((pend >> gg & 1) && (unsigned)(w0[gg] >> 32) == epoch && (unsigned)(w1[gg] >> 32) == epoch) {
-                            v[gg] = make_float2(__uint_as_float((unsigned)w0[gg]), __uint_as_float((unsigned)w1[gg]));
-                            pend &= ~(1u << gg);
+                    for (int u = 0; u < 8; ++u)
+                        if ((pend >> u & 1) && (unsigned)(w0[u] >> 32) == epoch && (unsigned)(w1[u] >> 32) == epoch) {
+                            v[u] = make_float2(__uint_as_float((unsigned)w0[u]), __uint_as_float((unsigned)w1[u]));
+                            pend &= ~(1u << u);
                         }
                     if (pend && (++spins & 1023u) == 0 && (s_abort || spins > (1u << 21))) { s_abort = 1; break; }
                 }
-                J = 0.f; f = 0.f;
+                float2 acc = make_float2(0.f, 0.f);
 #pragma unroll
-                for (int gg = 0; gg < BP_G_MAX; ++gg) if (gg < a.G) { J += v[gg].x; f += v[gg].y; }
+                for (int u = 0; u < 8; ++u) if (have >> u & 1) { acc.x += v[u].x; acc.y += v[u].y; }
+                *reinterpret_cast<float2 *>(part + 2 * (sub * ld + kk)) = acc;
+            }
+            __syncthreads();
+            if (mine) {
+                J = 0.f; f = 0.f;
+                for (int x = 0; x < NSUB; ++x) { const float2 p2 = *reinterpret_cast<const float2 *>(part + 2 * (x * ld + k)); J += p2.x; f += p2.y; }
             }
         }
         const double go = (double)go_f;
