@@ -156,7 +156,9 @@ modal_status modal_bptt(modal_plan *plan, int batch, int n_steps, const modal_bp
 /* Launch-selection overrides for tests and sweeps (the defaults are automatic).  Keys:
  *   "vk_impl"      0 automatic, 1 FP32 flow kernel, 2 tcgen05 batched kernel (H resident in shared memory), 3 tcgen05
  *                  streaming kernel (H streamed from L2; batch <= 64 per launch, wider batches run as consecutive launches),
- *                  4 small-system kernel (one warp per sample; N_q, N_phi <= 32, N_phi N_q^2 <= 8192: chosen automatically there)
+ *                  4 small-system kernel (one warp per sample; N_q, N_phi <= 32, N_phi N_q^2 <= 8192: chosen automatically there),
+ *                  5 dense-team kernel (a team of <= 32 CTAs per sample, every CTA keeps the whole state, one hop per step; chosen
+ *                  automatically at batch < 8 when the dense H of a CTA's modes fits shared memory, e.g. 100 + 50 modes)
  *   "flow_g"       CTAs per team of the flow kernel (0 automatic)
  *   "flow_ns"      TMA ring slots of the flow kernel (0: none, streamed tiles are read directly from L2)
  *   "flow_res"     resident tiles per CTA of the flow kernel (-1 automatic)
@@ -198,7 +200,8 @@ typedef enum {
     MODAL_Q_ACTIVE = 9,      /* int    [coeff_batch][n_q]   1 = active, 0 = masked (R11)            */
     MODAL_Q_H_FULL = 10,     /* double [n_phi][n_q][n_q]: the fp32 values the device holds, widened */
     MODAL_Q_COEFF_BATCH = 11,/* int    [1]                                                          */
-    MODAL_Q_KERNEL_INFO = 12,/* int    [8] of the last launch: kernel family (1 tension, 2 small-system, 3 flow, 4 batched tcgen05, 5 streaming */
+    MODAL_Q_KERNEL_INFO = 12,/* int    [8] of the last launch: kernel family (1 tension, 2 small-system, 3 flow, 4 batched tcgen05, 5 streaming, */
+                             /*        6 dense team: CTAs per team, samples per launch),                                        */
                              /*        tcgen05), CTAs per team (flow) or CTAs, teams (flow) / n groups (batched) / samples per  */
                              /*        launch (streaming), threads, dynamic shared memory bytes, flags (1: H resident in shared */
                              /*        memory or L2, 2: team of several CTAs), ring slots (flow) / accumulator slots (batched)  */

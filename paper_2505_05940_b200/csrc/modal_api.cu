@@ -20,6 +20,7 @@
 #include "vk_stream.cuh"
 #include "vk_bptt.cuh"
 #include "vk_small.cuh"
+#include "vk_dense.cuh"
 #include "peaks.cuh"
 
 namespace mh = modal_host;
@@ -104,6 +105,7 @@ struct modal_plan {
     StreamConfig stream;
     DevBuf bp[16];                                                    // modal_bptt: dense H, coefficients, gradients, scratch
     bool bp_H_valid = false;
+    DevBuf dHdense, ddscr; bool dense_H_valid = false;                // vk_dense_kernel: dense fp32 H (internal order, padded rows), exchange words
     DevBuf dHsmall; bool small_H_valid = false;                       // vk_small_kernel: dense fp32 H, internal order
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dkv, dkq, dr, dast, ds, dsT, dw, dlam, dc, dq0, dv0, dgain, dbad, dout;      // dsT: s_n transposed [n_phi][coeff_batch] (batched kernel)
@@ -158,7 +160,7 @@ void set_H(modal_plan *p, Get get_user)
     }
     for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
     p->flow_cfgs.clear();                                   // schedules depend on the zero pattern
-    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0; p->bp_H_valid = false; p->small_H_valid = false;
+    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0; p->bp_H_valid = false; p->small_H_valid = false; p->dense_H_valid = false;
     p->H_dirty = true;
 }
 
@@ -661,7 +663,21 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
     const bool use_small = d.model == MODAL_VK && nq <= 32 && d.n_phi <= 32 && (long long)d.n_phi * nq * nq <= 8192 &&
                            (p->opt.vk_impl == 0 || p->opt.vk_impl == 4) && p->opt.flow_g == 0 && p->opt.flow_ns == 0 && p->opt.flow_res < 0;
     if (d.model == MODAL_VK && p->opt.vk_impl == 4 && !use_small) { p->err += "vk_impl=4: the small-system kernel needs N_q, N_phi <= 32 and N_phi N_q^2 <= 8192\n"; return MODAL_EINCOMPAT; }
-    if (d.model == MODAL_VK && !use_small) {
+    // mid-size systems at small batch: a team of CTAs per sample with replicated state and one hop per step (vk_dense.cuh), when
+    // the dense H of a CTA's modes fits shared memory
+    bool use_dense = false;
+    int dn_G = 0, dn_per_launch = 0, dn_ld = (nq + 3) & ~3;
+    size_t dn_smem = 0;
+    if (d.model == MODAL_VK && !use_small && nq <= md::DN_THREADS && (p->opt.vk_impl == 5 || (p->opt.vk_impl == 0 && batch < 8)) &&
+        p->opt.flow_g == 0 && p->opt.flow_ns == 0 && p->opt.flow_res < 0) {
+        dn_per_launch = std::min(batch, p->sm_count);
+        dn_G = std::min({p->sm_count / dn_per_launch, d.n_phi, md::DN_G_MAX, 8 * std::min(md::DN_THREADS / dn_ld, 8)});
+        const int modes_max = (d.n_phi + dn_G - 1) / dn_G;
+        dn_smem = (size_t)modes_max * nq * dn_ld * 4;
+        use_dense = dn_G >= 2 && dn_smem + 16 * 1024 <= SMEM_LIMIT;
+        if (p->opt.vk_impl == 5 && !use_dense) { p->err += "vk_impl=5: the dense H of a CTA's modes does not fit shared memory (or one CTA per sample)\n"; return MODAL_EINCOMPAT; }
+    }
+    if (d.model == MODAL_VK && !use_small && !use_dense) {
         const int impl = p->opt.vk_impl;
         if ((impl == 0 && batch >= 64) || impl == 2) { modal_status s = configure_mma(p); if (s != MODAL_OK) return s; use_mma = p->mma.ok; }
         if (!use_mma && ((impl == 0 && batch >= 8) || impl == 3)) {
@@ -733,6 +749,52 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         CU(cudaGetLastError());
         p->kinfo[0] = 2; p->kinfo[1] = 1; p->kinfo[2] = blocks; p->kinfo[3] = md::SM_WARPS * 32;
         p->kinfo[4] = (int)smem; p->kinfo[5] = 1; p->kinfo[6] = 0; p->kinfo[7] = P;
+    } else if (use_dense) {
+        if (!p->dense_H_valid) {
+            const size_t nH = (size_t)d.n_phi * nq * nq;
+            std::vector<double> Hi(nH);
+            mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, Hi.data());
+            std::vector<float> Hd((size_t)d.n_phi * nq * dn_ld, 0.f);
+            for (int n = 0; n < d.n_phi; ++n)
+                for (int a_ = 0; a_ < nq; ++a_)
+                    for (int b_ = 0; b_ < nq; ++b_) Hd[((size_t)n * nq + a_) * dn_ld + b_] = (float)Hi[((size_t)n * nq + a_) * nq + b_];
+            CU(p->dHdense.ensure(Hd.size() * 4));
+            CU(cudaMemcpy(p->dHdense.p, Hd.data(), Hd.size() * 4, cudaMemcpyHostToDevice));
+            p->dense_H_valid = true;
+        }
+        const size_t nscr = (size_t)2 * dn_per_launch * dn_G * nq * 8;
+        CU(p->ddscr.ensure(nscr));
+        CU(cudaFuncSetAttribute(md::vk_dense_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dn_smem));
+        int out_cta = 0, fewest = 1 << 30;                     // the pickup goes to a CTA with the fewest modes
+        for (int g = 0; g < dn_G; ++g) {
+            const int cnt = (int)((long long)d.n_phi * (g + 1) / dn_G) - (int)((long long)d.n_phi * g / dn_G);
+            if (cnt < fewest) { fewest = cnt; out_cta = g; }
+        }
+        for (int b0 = 0; b0 < batch; b0 += dn_per_launch) {
+            const int nb = std::min(dn_per_launch, batch - b0);
+            md::DenseArgs a{};
+            a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P; a.batch = nb; a.n_steps = n_steps; a.G = dn_G; a.ld = dn_ld;
+            a.NJ = std::max(1, std::min(md::DN_THREADS / (dn_ld / 4), nq)); a.out_cta = out_cta;
+            a.coeff_stride_q = cb == 1 ? 0 : 1; a.coeff_stride_phi = cb == 1 ? 0 : 1;
+            const size_t oq = cb == 1 ? 0 : (size_t)b0 * P, op = cb == 1 ? 0 : (size_t)b0 * d.n_phi;
+            a.H = p->dHdense.as<float>();
+            a.kv = p->dkv.as<double>() + oq; a.kq = p->dkq.as<double>() + oq; a.r = p->dr.as<double>() + oq; a.astart = p->dast.as<double>() + oq;
+            a.s = p->ds.as<float>() + op; a.w = p->dw.as<float>() + oq;
+            a.q0 = p->dq0.as<double>() + (size_t)b0 * P; a.v0 = p->dv0.as<double>() + (size_t)b0 * P;
+            a.auto_start = auto_start; a.half_T2 = half_T2;
+            a.fext = init->fext_signal ? init->fext_signal + (size_t)b0 * n_steps : nullptr;
+            a.gain = init->fext_signal ? p->dgain.as<double>() + (size_t)b0 * P : nullptr;
+            a.out = out_dev + (size_t)b0 * n_steps;
+            a.traj = init->traj_dev ? init->traj_dev + (size_t)b0 * n_steps * nq : nullptr; a.kperm = p->dperm.as<int>();
+            a.first_bad = p->dbad.as<int>() + b0;
+            a.scratch = p->ddscr.as<unsigned long long>(); a.timeout_flag = p->dtimeout.as<int>();
+            CU(cudaMemsetAsync(p->ddscr.p, 0, (size_t)2 * nb * dn_G * nq * 8, st));
+            md::vk_dense_kernel<<<nb * dn_G, md::DN_THREADS, dn_smem, st>>>(a);
+            CU(cudaGetLastError());
+        }
+        persistent = true;
+        p->kinfo[0] = 6; p->kinfo[1] = dn_G; p->kinfo[2] = dn_per_launch; p->kinfo[3] = md::DN_THREADS;
+        p->kinfo[4] = (int)dn_smem; p->kinfo[5] = 1 | 2; p->kinfo[6] = 0; p->kinfo[7] = P;
     } else if (use_stream) {
         StreamConfig &m = p->stream;
         const mh::StreamLayout &L = m.L;
@@ -1289,7 +1351,7 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
     if (!p || !key) return MODAL_EINVAL;
     p->err.clear();
     struct { const char *name; int *field; int lo, hi; } tab[] = {
-        {"vk_impl", &p->opt.vk_impl, 0, 4}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
+        {"vk_impl", &p->opt.vk_impl, 0, 5}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
         {"flow_res", &p->opt.flow_res, -1, 1 << 20}, {"mma_split", &p->opt.mma_split, 0, 4}, {"mma_ng", &p->opt.mma_ng, 0, 8},
         {"mma_nstg", &p->opt.mma_nstg, 0, 16}, {"mma_cluster", &p->opt.mma_cluster, 0, 1}, {"parity_order", &p->opt.parity_order, 0, 1}, {"timing", &p->opt.timing, 0, 1}};
     for (auto &t : tab)
@@ -1370,7 +1432,7 @@ extern "C" void modal_plan_destroy(modal_plan *p)
                           &p->mma.dQop, &p->mma.dqf, &p->mma.dGx, &p->mma.dfx, &p->mma.dflags, &p->mma.dpx, &p->stream.dA, &p->stream.dtab,
                           &p->stream.dqx, &p->stream.dGx, &p->stream.dfx, &p->stream.dpx}) b->release();
     for (DevBuf &b : p->bp) b.release();
-    p->dHsmall.release();
+    p->dHsmall.release(); p->dHdense.release(); p->ddscr.release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         if (p->pinned_out) cudaFreeHost(p->pinned_out);
     }

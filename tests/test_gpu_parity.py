@@ -350,9 +350,13 @@ def test_c2_full_config_parity():
     plan, q0 = mb.plan_from_workload(wl, 0)
     gpu, fb, _, st = gpu_run(plan, q0, None, n_steps)
     info = plan.query(mb.Q_KERNEL_INFO)
-    assert info[0] == 3 and st == 0 and fb[0] == -1 and ref["first_bad"][0] == -1
+    assert info[0] == 6 and info[1] >= 16 and st == 0 and fb[0] == -1 and ref["first_bad"][0] == -1      # the dense-team kernel (one hop per step)
     assert nl_ratio(case, 0) <= 0.05
     check_parity(gpu, ref["out"], case)
+    plan.set_option("vk_impl", 1)                                # the flow kernel on the same plan: a shorter run, both against the oracle
+    flow, _, _, _ = gpu_run(plan, q0, None, 4096)
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 3
+    check_parity(flow, ref["out"][:, :4096], case)
 
 
 def test_vk_ftm_scheme_and_auto_start_parity():
@@ -522,6 +526,40 @@ def test_vk_small_kernel_parity(n_q, n_phi, batch, n_steps, scheme):
     assert plan.query(mb.Q_KERNEL_INFO)[0] == 3
     assert np.max(np.abs(flow - gpu)) <= 1e-5 * np.max(np.abs(gpu))
     plan.set_option("vk_impl", 0)
+    gpu2, _, _, _ = gpu_run(plan, case.q0, None, n_steps, fext=fext, fext_gain=gain)
+    assert np.array_equal(gpu, gpu2)
+
+
+@pytest.mark.parametrize("n_q,n_phi,batch,n_steps,scheme", [
+    (37, 13, 3, 1200, 0),           # teams of 13 CTAs, ragged sizes, per-sample geometries
+    (100, 50, 5, 500, 0),           # C2's mode counts, teams of 29
+    (57, 23, 2, 800, 1),            # FTM
+    (130, 3, 1, 600, 0),            # fewer in-plane modes than CTAs
+    (40, 9, 150, 200, 0),           # forced at a batch wider than the GPU: two launches, one CTA would be refused -> teams of 1 are not used
+])
+def test_vk_dense_team_kernel_parity(n_q, n_phi, batch, n_steps, scheme):
+    """Dense-team kernel (replicated state, one hop per step) against the oracle, with an external force, the device-side start and
+    the trajectory output; bit-reproducible."""
+    torch, mb = _mods()
+    wl = _small_vk_workload(n_q, n_phi, batch, n_steps)
+    case = orc.assemble(wl, scheme=scheme)
+    rng = np.random.default_rng(3)
+    fext = np.zeros((batch, n_steps)); t = np.arange(48)
+    fext[:, 10:58] = 0.5 * (1 - np.cos(2 * np.pi * t / 48))[None] * rng.uniform(0.5, 2.0, (batch, 1))
+    gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
+    sub = list(range(batch)) if batch <= 8 else [0, 1, 73, 74, 148, 149]
+    sc = orc.assemble(wl, scheme=scheme, samples=sub)
+    ref = orc.simulate(orc.VK, sc.c1, sc.c2, sc.c3, sc.w, sc.q0, sc.qm1, n_steps, nl_scale=sc.nl_scale,
+                       H=sc.H, fext=orc.f32(fext[sub]), fext_gain=gain[sub], want_traj=True)
+    if batch > 148:
+        with pytest.raises(mb.ModalError):                       # one CTA per sample is not a team: refused when forced
+            plan_with_oracle_inputs(wl, case, scheme=scheme, options=dict(vk_impl=5)).simulate(case.q0, 8, 0)
+        return
+    plan = plan_with_oracle_inputs(wl, case, scheme=scheme, options=dict(vk_impl=5))
+    gpu, fb, traj, st = gpu_run(plan, case.q0, None, n_steps, want_traj=True, fext=fext, fext_gain=gain)
+    assert plan.query(mb.Q_KERNEL_INFO)[0] == 6 and st == 0 and np.all(fb == -1)
+    check_parity(gpu[sub], ref["out"], sc)
+    assert np.max(np.abs(traj[sub] - ref["traj"])) <= 1e-4 * np.max(np.abs(ref["traj"]))
     gpu2, _, _, _ = gpu_run(plan, case.q0, None, n_steps, fext=fext, fext_gain=gain)
     assert np.array_equal(gpu, gpu2)
 

@@ -217,7 +217,7 @@ def test_ftm_plan_refuses_overdamped_mode_naming_it():
 def test_options_api_validates_keys_and_ranges():
     wl, plan = _c0_plan()
     plan.set_option("vk_impl", 2); plan.set_option("flow_g", 4); plan.set_option("timing", 0)
-    for key, val in (("vk_impl", 5), ("flow_ns", 99), ("nonsense", 1)):
+    for key, val in (("vk_impl", 6), ("flow_ns", 99), ("nonsense", 1)):
         with pytest.raises(mb.ModalError) as e:
             plan.set_option(key, val)
         assert e.value.status == mb.EINVAL
