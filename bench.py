@@ -137,6 +137,12 @@ def roofline_for(wl, B, n_steps, per_launch, info, tile_stats, pk, stream=None):
             r.update({"h_stream_mib": int(stream[12]), "h_stream_read": rd, "l2_read_peak_64mb": pk.get("l2_read_gbs_64mb") if pk else None,
                       "frac_stream_of_l2": rd / pk["l2_read_gbs_64mb"] if pk else None})
         return r
+    if fam == 6:          # dense-team kernel: H of a CTA's modes resident in shared memory, one L2 hop per step: latency-bound at batch 1
+        ach = hbytes * n_steps / per_launch / 1e9
+        return {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
+                "peak_source": peak_src, "kernel": "vk_dense_kernel", "frac_dense_alg": ach / hbm_peak,
+                "note": "algorithmic bytes = the packed H once per step (SURVEY.md 8(d)); the kernel keeps the dense fp32 H in shared memory and "
+                        "is bound by the one cross-CTA hop per step, not by bandwidth"}
     if fam == 3:
         ach = hbytes * n_steps / per_launch / 1e9
         tiles, nz = tile_stats
@@ -220,7 +226,7 @@ def run_secondary(mb, torch, sampler, pk, steps=2, warmup=1):
         hbm_peak, peak_src, _ = driver_peaks()
         ach = 4.0 * nphi * nq * nq * B * n_steps / ts[0] / 1e9
         res.append({"workload": f"bptt_vk_{nq}x{nphi}_b{B}", "batch": B, "time_steps": n_steps, "value": B * n_steps / ts[0], "unit": UNIT,
-                    "us_per_time_step": 1e6 * ts[0] / n_steps, "us_per_time_step_with_grad_H": 1e6 * ts[1] / n_steps, "kernel_family": 6, "status": int(st),
+                    "us_per_time_step": 1e6 * ts[0] / n_steps, "us_per_time_step_with_grad_H": 1e6 * ts[1] / n_steps, "kernel_family": 7, "status": int(st),
                     "roofline": {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
                                  "peak_source": peak_src, "kernel": "vk_bptt_kernel",
                                  "frac_of_l2": ach / pk["l2_read_gbs_8mb"] if pk else None,
