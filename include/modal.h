@@ -158,7 +158,8 @@ modal_status modal_bptt(modal_plan *plan, int batch, int n_steps, const modal_bp
  *                  streaming kernel (H streamed from L2; batch <= 64 per launch, wider batches run as consecutive launches),
  *                  4 small-system kernel (one warp per sample; N_q, N_phi <= 32, N_phi N_q^2 <= 8192: chosen automatically there),
  *                  5 dense-team kernel (a team of <= 32 CTAs per sample, every CTA keeps the whole state, one hop per step; chosen
- *                  automatically at batch < 8 when the dense H of a CTA's modes fits shared memory, e.g. 100 + 50 modes)
+ *                  automatically below batch 64 when the dense H of a CTA's modes fits shared memory, e.g. 100 + 50 modes, and,
+ *                  from batch 8 on, a CTA has at most 8 modes)
  *   "flow_g"       CTAs per team of the flow kernel (0 automatic)
  *   "flow_ns"      TMA ring slots of the flow kernel (0: none, streamed tiles are read directly from L2)
  *   "flow_res"     resident tiles per CTA of the flow kernel (-1 automatic)

@@ -668,13 +668,15 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
     bool use_dense = false;
     int dn_G = 0, dn_per_launch = 0, dn_ld = (nq + 3) & ~3;
     size_t dn_smem = 0;
-    if (d.model == MODAL_VK && !use_small && nq <= md::DN_THREADS && (p->opt.vk_impl == 5 || (p->opt.vk_impl == 0 && batch < 8)) &&
+    if (d.model == MODAL_VK && !use_small && nq <= md::DN_THREADS && (p->opt.vk_impl == 5 || (p->opt.vk_impl == 0 && batch < 64)) &&
         p->opt.flow_g == 0 && p->opt.flow_ns == 0 && p->opt.flow_res < 0) {
         dn_per_launch = std::min(batch, p->sm_count);
         dn_G = std::min({p->sm_count / dn_per_launch, d.n_phi, md::DN_G_MAX, 8 * std::min(md::DN_THREADS / dn_ld, 8)});
         const int modes_max = (d.n_phi + dn_G - 1) / dn_G;
         dn_smem = (size_t)modes_max * nq * dn_ld * 4;
         use_dense = dn_G >= 2 && dn_smem + 16 * 1024 <= SMEM_LIMIT;
+        // batches of 8 and more have the streaming tensor-core kernel as alternative: keep the team kernel only while a CTA has few modes
+        if (p->opt.vk_impl == 0 && batch >= 8 && modes_max > 8) use_dense = false;
         if (p->opt.vk_impl == 5 && !use_dense) { p->err += "vk_impl=5: the dense H of a CTA's modes does not fit shared memory (or one CTA per sample)\n"; return MODAL_EINCOMPAT; }
     }
     if (d.model == MODAL_VK && !use_small && !use_dense) {

@@ -535,6 +535,7 @@ def test_vk_small_kernel_parity(n_q, n_phi, batch, n_steps, scheme):
     (100, 50, 5, 500, 0),           # C2's mode counts, teams of 29
     (57, 23, 2, 800, 1),            # FTM
     (130, 3, 1, 600, 0),            # fewer in-plane modes than CTAs
+    (100, 50, 9, 300, 0),           # nine samples side by side, teams of 16
     (40, 9, 150, 200, 0),           # forced at a batch wider than the GPU: two launches, one CTA would be refused -> teams of 1 are not used
 ])
 def test_vk_dense_team_kernel_parity(n_q, n_phi, batch, n_steps, scheme):
@@ -547,7 +548,7 @@ def test_vk_dense_team_kernel_parity(n_q, n_phi, batch, n_steps, scheme):
     fext = np.zeros((batch, n_steps)); t = np.arange(48)
     fext[:, 10:58] = 0.5 * (1 - np.cos(2 * np.pi * t / 48))[None] * rng.uniform(0.5, 2.0, (batch, 1))
     gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
-    sub = list(range(batch)) if batch <= 8 else [0, 1, 73, 74, 148, 149]
+    sub = list(range(batch)) if batch <= 9 else [0, 1, 73, 74, 148, 149]
     sc = orc.assemble(wl, scheme=scheme, samples=sub)
     ref = orc.simulate(orc.VK, sc.c1, sc.c2, sc.c3, sc.w, sc.q0, sc.qm1, n_steps, nl_scale=sc.nl_scale,
                        H=sc.H, fext=orc.f32(fext[sub]), fext_gain=gain[sub], want_traj=True)
