@@ -333,7 +333,7 @@ bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, const std:
     c.sched = mh::build_flow_schedule(nq, nphi, G, c.NW, c.slot_tiles, tile_nz);
     const mh::FlowSchedule &s = c.sched;
     if (s.NLOC_MAX > 255 || s.tp_max >= (1 << 24) || s.nt > 255) return false;      // 8-bit fields of the unit descriptors
-    const md::FlowSmem fixed = md::flow_smem_layout(0, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, 0);
+    const md::FlowSmem fixed = md::flow_smem_layout(0, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, 0, G == 1);
     if (fixed.total + 1024 > SMEM_LIMIT) return false;
     const int avail_tiles = (int)((SMEM_LIMIT - fixed.total - 256) / 1024);
     if (force_ns <= 0 && force_res < 0 && s.tiles_max <= avail_tiles) { c.NS = 0; c.res_tiles = s.tiles_max; }
@@ -351,7 +351,7 @@ bool flow_shape(int nq, int nphi, int G, int force_ns, int force_res, const std:
     int rmax = 0;
     for (int g = 0; g < G; ++g) rmax = std::max(rmax, c.sched.blob[(size_t)g * s.stride + 6]);
     c.res_tiles = rmax;
-    c.smem = md::flow_smem_layout(c.NS, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, c.res_tiles).total;
+    c.smem = md::flow_smem_layout(c.NS, c.slot_tiles, s.NQP, s.NLOC_MAX, s.U_max, s.slice_max, s.tp_max, s.stride, c.res_tiles, G == 1).total;
     return c.smem <= SMEM_LIMIT;
 }
 

@@ -242,7 +242,7 @@ struct FlowSmem {
     size_t bars, q32, eta, gu, fpart, sq, sv, tp, sched, ring, res, total;
 };
 __host__ __device__ inline FlowSmem flow_smem_layout(int NS, int slot_tiles, int NQP, int NLOC_MAX, int U_max,
-                                                     int slice_max, int tp_max, int sched_stride, int res_tiles)
+                                                     int slice_max, int tp_max, int sched_stride, int res_tiles, bool single_cta = true)
 {
     FlowSmem L;
     size_t o = 0;
@@ -250,7 +250,7 @@ __host__ __device__ inline FlowSmem flow_smem_layout(int NS, int slot_tiles, int
     L.q32 = o;   o += flow_align((size_t)NQP * 4, 16);
     L.eta = o;   o += flow_align((size_t)NLOC_MAX * 4, 16);
     L.gu = o;    o += flow_align((size_t)U_max * 4, 16);
-    L.fpart = o; o += flow_align((size_t)NQP * 4, 16);
+    L.fpart = o; o += single_cta ? flow_align((size_t)NQP * 4, 16) : 0;      // the force of a one-CTA team; teams exchange it through L2 (1.6 KB that make C4's 207 tiles per CTA resident)
     L.sq = o;    o += flow_align((size_t)slice_max * 8, 16);
     L.sv = o;    o += flow_align((size_t)slice_max * 8, 16);
     L.tp = o;    o += flow_align((size_t)tp_max * 4, 16);
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(RING ? 544 : 512, 1) vk_flow_kernel(const Flow
     const int NW = a.NW, NC = NW * 32, G = a.G, NQP = a.NQP;
     const int team = blockIdx.x / G, rank = blockIdx.x - team * G;
     const FlowSmem L = flow_smem_layout(a.NS, a.slot_tiles, NQP, a.NLOC_MAX, a.U_max, a.slice_max, a.tp_max,
-                                        a.sched_stride, a.res_tiles);
+                                        a.sched_stride, a.res_tiles, a.G == 1);
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.bars);
     volatile unsigned *done = reinterpret_cast<volatile unsigned *>(bars + 2 * (a.NS > 0 ? a.NS : 1));   // uses consumed per slot
     volatile int *s_abort = reinterpret_cast<volatile int *>(done + 2 * (a.NS > 0 ? a.NS : 1));
