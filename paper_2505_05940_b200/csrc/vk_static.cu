@@ -56,7 +56,7 @@ __device__ __forceinline__ void block_sum2(float a, float b, float *red, float &
 __global__ void __launch_bounds__(ST_THREADS_S) vk_static_kernel(const StaticArgs a)
 {
     __shared__ float qf[MODAL_STATIC_MAX_NQ], tn[MODAL_STATIC_MAX_NQ], red[16];
-    __shared__ int s_abort;
+    __shared__ volatile int s_abort;
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5;
     const int bl = blockIdx.x / a.G, g = blockIdx.x - bl * a.G;           // sample of this launch, team member
     const int n0 = (int)((long long)a.n_phi * g / a.G), n1 = (int)((long long)a.n_phi * (g + 1) / a.G);
@@ -103,9 +103,24 @@ __global__ void __launch_bounds__(ST_THREADS_S) vk_static_kernel(const StaticArg
             unsigned long long *base = a.scratch + (((size_t)(n & 1) * a.batch + bl) * a.G) * MODAL_STATIC_MAX_NQ;
             if (mine) {
                 md::st_tag(base + (size_t)g * MODAL_STATIC_MAX_NQ + k, facc, (unsigned)n + 1u);
+                // all G loads in flight together (one after the other they cost an L2 round trip each); summed in team order:
+                // identical bits in every CTA of the team
+                float vv[ST_G_MAX];
+                unsigned pend = (1u << a.G) - 1u, spins = 0;
+                while (pend) {
+                    unsigned long long w0[ST_G_MAX];
+#pragma unroll
+                    for (int gg = 0; gg < ST_G_MAX; ++gg)
+                        if (pend >> gg & 1)
+                            asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(w0[gg]) : "l"(base + (size_t)gg * MODAL_STATIC_MAX_NQ + k) : "memory");
+#pragma unroll
+                    for (int gg = 0; gg < ST_G_MAX; ++gg)
+                        if ((pend >> gg & 1) && (unsigned)(w0[gg] >> 32) == (unsigned)n + 1u) { vv[gg] = __uint_as_float((unsigned)w0[gg]); pend &= ~(1u << gg); }
+                    if (pend && (++spins & 1023u) == 0 && (s_abort || spins > (1u << 21))) { s_abort = 1; break; }
+                }
                 f = 0.f;
-                for (int gg = 0; gg < a.G; ++gg)                          // team order: identical bits in every CTA of the team
-                    f += md::ld_tag(base + (size_t)gg * MODAL_STATIC_MAX_NQ + k, (unsigned)n + 1u, &s_abort);
+#pragma unroll
+                for (int gg = 0; gg < ST_G_MAX; ++gg) if (gg < a.G) f += vv[gg];
             }
         }
         v = fma(kv, v, fma(-kq, q, -r * (double)f));                      // a5
