@@ -652,3 +652,38 @@ def dcoeffs_domega_dgamma(scheme, omega, gamma, T):
     return dict(c1_w=-2 * e * sn * T * wt_w, c1_g=-2 * T * e * cs - 2 * e * sn * T * wt_g,
                 c2_w=np.zeros_like(w_), c2_g=2 * T * np.exp(-2 * g_ * T),
                 c3_w=dc3_dwt * wt_w, c3_g=-T * T * e * sn / wt + dc3_dwt * wt_g)
+
+
+def bptt_tension(c1, c2, c3, w, lam, c, q0, qm1, gout):
+    """Backpropagation through time of ONE tension-modulated sample (Kirchhoff-Carrier string / Berger plate; the paper's
+    non-linear string fits): as `bptt_vk` with f_mu = c lam_mu q_mu S, S = sum_nu lam_nu q_nu^2
+    (Eq. 8, reading R2).  J_mu,j = c [lam_mu S delta_mu,j + 2 lam_mu q_mu lam_j q_j] (symmetric), so
+    J^T mu = c [S lam mu + 2 (sum lam q mu) lam q].  Returns dL/d{q0, qm1, c1, c2, c3, w, c}; numpy fp64."""
+    c1, c2, c3, w, lam = (np.asarray(x, np.float64) for x in (c1, c2, c3, w, lam))
+    q0 = np.asarray(q0, np.float64); qm1 = np.asarray(qm1, np.float64); gout = np.asarray(gout, np.float64)
+    c = float(c)
+    N, Nq = gout.shape[0], q0.shape[0]
+    q = np.empty((N + 1, Nq)); q[0] = q0
+    prev = qm1
+    for n in range(N):
+        S = float(lam @ (q[n] ** 2))
+        q[n + 1] = c1 * q[n] + c2 * prev - c3 * (c * lam * q[n] * S)
+        prev = q[n]
+    g = {k: np.zeros(Nq) for k in ("c1", "c2", "c3", "w")}
+    g["c"] = 0.0
+    a1 = np.zeros(Nq); a2 = np.zeros(Nq)
+    for n in range(N - 1, -1, -1):
+        qn = q[n]; qp = q[n - 1] if n > 0 else qm1
+        S = float(lam @ (qn ** 2))
+        f = c * lam * qn * S
+        mu = c3 * a1
+        D = float((lam * qn) @ mu)
+        JTmu = c * (S * lam * mu + 2.0 * D * lam * qn)
+        g["c1"] += a1 * qn; g["c2"] += a1 * qp; g["c3"] -= a1 * f
+        g["w"] += gout[n] * qn
+        g["c"] -= D * S
+        a0 = w * gout[n] + c1 * a1 + c2 * a2 - JTmu
+        a2, a1 = a1, a0
+    g["q0"] = a1
+    g["qm1"] = c2 * a2
+    return g

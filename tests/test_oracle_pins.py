@@ -672,3 +672,34 @@ def test_scheme_coefficient_derivatives_by_finite_differences(scheme):
         for i, c in enumerate(("c1", "c2", "c3")):
             fd = (hi[i] - lo[i]) / (2 * eps)
             assert np.allclose(d[f"{c}_{var}"], fd, rtol=2e-6, atol=1e-9 * np.max(np.abs(fd)) + 1e-18), (c, var, d[f"{c}_{var}"], fd)
+
+
+def test_bptt_tension_adjoint_matches_finite_differences_of_the_forward_oracle():
+    """The adjoint of the tension-modulated recurrence (strings / Berger plates) against central differences of the forward C oracle."""
+    rng = np.random.default_rng(5)
+    Nq, N = 9, 60
+    T = 1 / 44100
+    om = rng.uniform(500, 9000, Nq); ga = rng.uniform(0.5, 30, Nq)
+    c1, c2, c3 = orc.scheme_coeffs(orc.SV, om, ga, T)
+    lam = np.sort(rng.uniform(10, 900, Nq)); w = rng.normal(size=Nq); cval = 4.0e6
+    q0 = rng.normal(size=Nq) * 2e-3; qm1 = q0 + rng.normal(size=Nq) * 1e-5
+    gout = rng.normal(size=N)
+    P = dict(c1=c1, c2=c2, c3=c3, w=w, q0=q0, qm1=qm1)
+
+    def L(cv=cval, **over):
+        a = {**P, **over}
+        r = orc.simulate(orc.TENSION, a["c1"][None], a["c2"][None], a["c3"][None], a["w"][None], a["q0"][None], a["qm1"][None], N,
+                         lam=lam[None], nl_scale=np.array([cv]))
+        return float(gout @ r["out"][0])
+
+    g = orc.bptt_tension(c1, c2, c3, w, lam, cval, q0, qm1, gout)
+    g_lin = orc.bptt_tension(c1, c2, c3, w, lam, 0.0, q0, qm1, gout)
+    assert np.linalg.norm(g["q0"] - g_lin["q0"]) > 1e-3 * np.linalg.norm(g["q0"])          # the non-linear terms matter here
+    for name, eps in (("q0", 1e-8), ("qm1", 1e-8), ("c1", 1e-7), ("c2", 1e-7), ("c3", 1e-13), ("w", 1e-6)):
+        for idx in range(Nq):
+            hi = P[name].copy(); hi[idx] += eps
+            lo = P[name].copy(); lo[idx] -= eps
+            fd = (L(**{name: hi}) - L(**{name: lo})) / (2 * eps)
+            assert abs(fd - g[name][idx]) <= 5e-5 * np.max(np.abs(g[name])) + 1e-7 * abs(fd), (name, idx, fd, g[name][idx])
+    fd = (L(cv=cval * (1 + 1e-5)) - L(cv=cval * (1 - 1e-5))) / (2e-5 * cval)
+    assert abs(fd - g["c"]) <= 1e-5 * abs(g["c"]), (fd, g["c"])
