@@ -128,7 +128,9 @@ modal_status modal_simulate_host(modal_plan *plan, int batch, int n_steps, const
  * wait of a persistent kernel gave up: the CTAs of a team were not co-resident) / MODAL_OK. */
 modal_status modal_plan_check(modal_plan *plan, int *first_bad_step);
 
-/* Reverse pass (backpropagation through time) of a MODAL_VK run: SURVEY.md 8(f) row 3.  Given the trajectory of a
+/* Reverse pass (backpropagation through time) of a run: SURVEY.md 8(f) row 3.  MODAL_VK as described below;
+ * MODAL_TENSION / MODAL_LINEAR plans (strings, Berger plates: the paper's non-linear string fits) the same with
+ * fnl_mu = c lam_mu q_mu sum lam q^2, grad_nl_scale [batch] = dL/dc and no grad_H.  Given the trajectory of a
  * forward run (modal_init.traj_dev of modal_simulate with the same plan, coefficients, batch and n_steps, an explicit qm1 and no
  * external force) and gout[b][n] = dL/d out_audio[b][n] of any loss L on the audio, computes per sample
  *   dL/dq^0, dL/dq^-1 (as independent inputs of q^{n+1} = c1 q^n + c2 q^{n-1} - c3 fnl(q^n), Eq. 19/20),
@@ -139,7 +141,7 @@ modal_status modal_plan_check(modal_plan *plan, int *first_bad_step);
  * with H per step (csrc/vk_bptt.cuh).  Contractions in fp32, adjoint state and accumulators in fp64.  Synchronous: the gradients
  * are copied to the HOST arrays before it returns; any gradient pointer may be NULL.  Per-sample arrays are [batch][...] even when
  * coeff_batch is 1 (sum over the batch for shared parameters).  n_q <= 512.
- * Errors: MODAL_EINVAL (sizes, missing qm1 / traj_dev / gout_dev), MODAL_EINCOMPAT (not a VK plan, n_q), MODAL_ECUDA. */
+ * Errors: MODAL_EINVAL (sizes, missing qm1 / traj_dev / gout_dev), MODAL_EINCOMPAT (n_q), MODAL_ECUDA. */
 typedef struct {
     const double *qm1;        /* host   [batch][n_q]            q^-1 of the forward run                       */
     const double *traj_dev;   /* DEVICE [batch][n_steps][n_q]   q^n of the forward run (fp64)                 */

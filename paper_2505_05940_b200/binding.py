@@ -188,8 +188,8 @@ class Plan:
         qm1 = _arr(np.atleast_2d(qm1))
         B = qm1.shape[0]
         g = {n: np.zeros((B, self.n_q)) for n in ("q0", "qm1", "omega", "sigma", "c1", "c2", "c3", "pickup")}
-        g["nl_scale"] = np.zeros((B, self.n_phi))
-        if want_H:
+        g["nl_scale"] = np.zeros((B, max(self.n_phi, 1)))            # tension / linear plans: one scale per sample
+        if want_H and self.n_phi > 0:
             g["H"] = np.zeros((self.n_phi, self.n_q, self.n_q))
         a = BpttArgs(_ptr(qm1, _dp), traj_dev_ptr, gout_dev_ptr, *[_ptr(g[n], _dp) for n in ("q0", "qm1", "omega", "sigma", "c1", "c2", "c3", "pickup", "nl_scale")],
                      _ptr(g.get("H"), _dp))

@@ -1206,8 +1206,8 @@ extern "C" modal_status modal_bptt(modal_plan *p, int batch, int n_steps, const 
     if (!p) return MODAL_EINVAL;
     p->err.clear();
     const modal_plan_desc &d = p->d;
-    const int nq = d.n_q, nphi = d.n_phi, cb = p->coeff_batch;
-    if (d.model != MODAL_VK) { p->err += "modal_bptt: the reverse pass is built for MODAL_VK plans\n"; return MODAL_EINCOMPAT; }
+    const bool vk = d.model == MODAL_VK;
+    const int nq = d.n_q, nphi = vk ? d.n_phi : 1, cb = p->coeff_batch;      // tension / linear: one non-linear scale per sample
     if (p->device < 0) { p->err += "modal_bptt needs a CUDA device: there is no CPU fallback\n"; return MODAL_ECUDA; }
     if (!ar || batch < 1 || n_steps < 1 || batch > d.max_batch || n_steps > d.max_steps || (cb != 1 && cb != batch)) {
         p->err += "modal_bptt: batch / n_steps outside the plan, or coeff_batch neither 1 nor batch\n"; return MODAL_EINVAL;
@@ -1221,7 +1221,7 @@ extern "C" modal_status modal_bptt(modal_plan *p, int batch, int n_steps, const 
     // dense fp32 H in plan order (once per H)
     const size_t nH = (size_t)nphi * nq * nq;
     const int ld = (nq + 3) & ~3;                                   // row stride: 16-byte loads
-    if (!p->bp_H_valid) {
+    if (vk && !p->bp_H_valid) {
         std::vector<double> Hi(nH);
         mh::unpack_flow_tiles(nq, nphi, p->Hf, Hi.data());
         std::vector<float> Hu((size_t)nphi * nq * ld, 0.f);
@@ -1259,11 +1259,29 @@ extern "C" modal_status modal_bptt(modal_plan *p, int batch, int n_steps, const 
     for (int i : {B_GQ0, B_GQM1, B_GC1, B_GC2, B_GC3, B_GW}) CU(p->bp[i].ensure(nbq));
     CU(p->bp[B_GS].ensure(nbs));
     CU(cudaMemsetAsync(p->bp[B_GS].p, 0, nbs, st));
-    const bool wantH = ar->grad_H != nullptr;
+    const bool wantH = vk && ar->grad_H != nullptr;
     const size_t n_mu = (size_t)batch * n_steps * nq * 4, n_sc = (size_t)batch * n_steps * nphi * 4;
     if (wantH) CU(p->bp[B_AUX].ensure(n_mu + 2 * n_sc + nH * 8));
     CU(p->dtimeout.ensure(4));
     CU(cudaMemsetAsync(p->dtimeout.p, 0, 4, st));
+    if (!vk) {
+        // tension-modulated / linear models: one warp per sample (tension_bptt_kernel); lambda travels in the dense-H buffer slot
+        std::vector<float> lam((size_t)cb * nq, 0.f);
+        if (d.model == MODAL_TENSION) for (size_t i = 0; i < lam.size(); ++i) lam[i] = act[i] ? (float)p->lambda_s[i] : 0.f;
+        if (d.model != MODAL_TENSION) for (float &x : s) x = 0.f;
+        CU(up(B_H, lam.data(), lam.size() * 4)); CU(up(B_S, s.data(), s.size() * 4));
+        md::TensionBpttArgs a{};
+        a.n_q = nq; a.batch = batch; a.n_steps = n_steps; a.cb_q = cb == 1 ? 0 : nq;
+        a.c1 = p->bp[B_C1].as<double>(); a.c2 = p->bp[B_C2].as<double>(); a.c3 = p->bp[B_C3].as<double>();
+        a.w = p->bp[B_W].as<float>(); a.lam = p->bp[B_H].as<float>(); a.c = p->bp[B_S].as<float>();
+        a.traj = ar->traj_dev; a.qm1 = p->bp[B_QM1].as<double>(); a.gout = ar->gout_dev;
+        a.g_q0 = p->bp[B_GQ0].as<double>(); a.g_qm1 = p->bp[B_GQM1].as<double>(); a.g_c1 = p->bp[B_GC1].as<double>();
+        a.g_c2 = p->bp[B_GC2].as<double>(); a.g_c3 = p->bp[B_GC3].as<double>(); a.g_w = p->bp[B_GW].as<double>(); a.g_c = p->bp[B_GS].as<double>();
+        const size_t smem = md::tension_bptt_smem(nq);
+        CU(cudaFuncSetAttribute(md::tension_bptt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        md::tension_bptt_kernel<<<(batch + md::TB_WARPS - 1) / md::TB_WARPS, md::TB_WARPS * 32, smem, st>>>(a);
+        CU(cudaGetLastError());
+    }
     // launches of co-resident teams: G CTAs per sample, samples per launch <= SMs
     const int per_launch = std::min(batch, p->sm_count);
     int G = std::min({p->sm_count / per_launch, nphi, md::BP_G_MAX, 8 * std::min(md::BP_THREADS_MAX / ((nq + 3) & ~3), 8)});
@@ -1277,7 +1295,7 @@ extern "C" modal_status modal_bptt(modal_plan *p, int batch, int n_steps, const 
     const int NJ = std::max(1, std::min(md::BP_THREADS_MAX / (ld / 4), nq));
     const size_t dyn = resident ? hs_bytes : 0;
     if (resident) CU(cudaFuncSetAttribute(md::vk_bptt_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-    for (int b0 = 0; b0 < batch; b0 += per_launch) {
+    for (int b0 = 0; vk && b0 < batch; b0 += per_launch) {
         const int nb = std::min(per_launch, batch - b0);
         md::BpttArgs a{};
         a.n_q = nq; a.n_phi = nphi; a.batch = nb; a.n_steps = n_steps; a.G = G; a.ld = ld; a.NJ = NJ;

@@ -228,3 +228,67 @@ __global__ void __launch_bounds__(BP_THREADS_MAX) vk_gradH_kernel(int n_q, int n
 }
 
 }  // namespace modal_dev
+
+namespace modal_dev {
+
+// ---- reverse pass of the tension-modulated / linear recurrence (Kirchhoff-Carrier string, Berger plate): one warp per sample --------
+//   f_mu = c lam_mu q_mu S,  S = sum lam q^2  (Eq. 8, reading R2);  J symmetric:
+//   J^T mu = c [ S lam mu + 2 (sum lam q mu) lam q ];   dL/dc -= (sum lam q mu) S;   the rest as vk_bptt_kernel.  Oracle: oracle.bptt_tension.
+// O(N) work per step: the adjoint state and the gradient accumulators of a sample live in the warp's slice of shared memory (fp64).
+constexpr int TB_WARPS = 4;
+
+struct TensionBpttArgs {
+    int n_q, batch, n_steps, cb_q;                         // cb_q: coefficient row stride per sample (0: one row for all)
+    const double *c1, *c2, *c3; const float *w, *lam, *c;  // [cb][n_q] ...; c [cb]
+    const double *traj, *qm1; const float *gout;
+    double *g_q0, *g_qm1, *g_c1, *g_c2, *g_c3, *g_w, *g_c; // [batch][n_q]; g_c [batch]
+};
+
+__host__ __device__ inline size_t tension_bptt_smem(int n_q) { return (size_t)TB_WARPS * n_q * 6 * sizeof(double); }
+
+__global__ void __launch_bounds__(TB_WARPS * 32) tension_bptt_kernel(const TensionBpttArgs a)
+{
+    extern __shared__ __align__(16) double tb_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.x * TB_WARPS + warp;
+    if (b >= a.batch) return;
+    const int nq = a.n_q;
+    double *A1 = tb_smem + (size_t)warp * nq * 6, *A2 = A1 + nq, *G1 = A2 + nq, *G2 = G1 + nq, *G3 = G2 + nq, *GW = G3 + nq;
+    for (int k = lane; k < nq; k += 32) { A1[k] = 0.0; A2[k] = 0.0; G1[k] = 0.0; G2[k] = 0.0; G3[k] = 0.0; GW[k] = 0.0; }
+    __syncwarp();
+    const size_t co = (size_t)b * a.cb_q;
+    const double *c1 = a.c1 + co, *c2 = a.c2 + co, *c3 = a.c3 + co;
+    const float *w = a.w + co, *lam = a.lam + co;
+    const double cn = (double)a.c[a.cb_q ? b : 0];
+    const double *traj = a.traj + (size_t)b * a.n_steps * nq, *qm1 = a.qm1 + (size_t)b * nq;
+    double gcn = 0.0;
+    for (int n = a.n_steps - 1; n >= 0; --n) {
+        const double *qn = traj + (size_t)n * nq;
+        const double *qp = n > 0 ? traj + (size_t)(n - 1) * nq : qm1;
+        double S = 0.0, D = 0.0;
+        for (int k = lane; k < nq; k += 32) {
+            const double q = qn[k], lq = (double)lam[k] * q;
+            S = fma(lq, q, S); D = fma(lq, c3[k] * A1[k], D);
+        }
+#pragma unroll
+        for (int m = 16; m >= 1; m >>= 1) { S += __shfl_xor_sync(FLOW_FULL, S, m); D += __shfl_xor_sync(FLOW_FULL, D, m); }
+        const double go = (double)a.gout[(size_t)b * a.n_steps + n];
+        for (int k = lane; k < nq; k += 32) {
+            const double q = qn[k], l = (double)lam[k], a1 = A1[k], mu = c3[k] * a1;
+            const double f = cn * l * q * S;
+            const double JT = cn * (S * l * mu + 2.0 * D * l * q);
+            G1[k] = fma(a1, q, G1[k]); G2[k] = fma(a1, qp[k], G2[k]); G3[k] = fma(-a1, f, G3[k]); GW[k] = fma(go, q, GW[k]);
+            const double a0 = fma((double)w[k], go, fma(c1[k], a1, fma(c2[k], A2[k], -JT)));
+            A2[k] = a1; A1[k] = a0;
+        }
+        gcn -= D * S;
+        __syncwarp();
+    }
+    for (int k = lane; k < nq; k += 32) {
+        const size_t o = (size_t)b * nq + k;
+        a.g_q0[o] = A1[k]; a.g_qm1[o] = c2[k] * A2[k]; a.g_c1[o] = G1[k]; a.g_c2[o] = G2[k]; a.g_c3[o] = G3[k]; a.g_w[o] = GW[k];
+    }
+    if (lane == 0) a.g_c[b] = gcn;
+}
+
+}  // namespace modal_dev

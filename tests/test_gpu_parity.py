@@ -616,6 +616,41 @@ def test_bptt_gradients_match_oracle_adjoint(n_q, n_phi, batch, n_steps, scheme)
     assert np.max(np.abs(g["H"] - gH_ref)) <= 2e-3 * np.max(np.abs(gH_ref))
 
 
+@pytest.mark.parametrize("batch,n_steps,scheme", [(6, 500, 0), (3, 400, 1)])
+def test_bptt_tension_gradients_match_oracle_adjoint(batch, n_steps, scheme):
+    """modal_bptt on a Kirchhoff-Carrier string plan (tension_bptt_kernel) against oracle.bptt_tension: gradients wrt q0, q^-1,
+    c1, c2, c3, omega, sigma, pickup and the tension scale; trajectory from modal_simulate."""
+    torch, mb = _mods()
+    wl = wlmod.c1(batch=batch, n_steps=n_steps)
+    wl["A"] = 0.5 * wl["A"]
+    case = orc.assemble(wl, scheme=scheme)
+    plan = plan_with_oracle_inputs(wl, case, scheme=scheme)
+    n_q = wl["n_q"]
+    traj = torch.zeros((batch, n_steps, n_q), dtype=torch.float64, device="cuda")
+    out = torch.empty((batch, n_steps), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    st, fb = plan.simulate(case.q0, n_steps, out.data_ptr(), qm1=case.qm1, stream=stream, traj_dev_ptr=traj.data_ptr())
+    torch.cuda.synchronize()
+    assert st == 0
+    rng = np.random.default_rng(9)
+    gout = rng.normal(size=(batch, n_steps)).astype(np.float32)
+    gdev = torch.tensor(gout, device="cuda")
+    g = plan.bptt(case.qm1, n_steps, traj.data_ptr(), gdev.data_ptr(), stream=stream)
+    T = 1.0 / wl["sample_rate"]
+    for b in range(batch):
+        act = case.active[b]
+        ref = orc.bptt_tension(case.c1[b], case.c2[b], case.c3[b], case.w[b], np.where(act, case.lam[b], 0.0), float(np.ravel(case.nl_scale)[b]),
+                               case.q0[b], case.qm1[b], gout[b].astype(np.float64))
+        dd = orc.dcoeffs_domega_dgamma(scheme, np.where(act, case.omega[b], 2.0), np.where(act, case.gamma[b], 1.0), T)
+        ref["omega"] = ref["c1"] * dd["c1_w"] + ref["c2"] * dd["c2_w"] + ref["c3"] * dd["c3_w"]
+        ref["sigma"] = ref["c1"] * dd["c1_g"] + ref["c2"] * dd["c2_g"] + ref["c3"] * dd["c3_g"]
+        for key, rk in (("q0", "q0"), ("qm1", "qm1"), ("c1", "c1"), ("c2", "c2"), ("c3", "c3"), ("omega", "omega"), ("sigma", "sigma"), ("pickup", "w")):
+            want = np.where(act, ref[rk], 0.0)
+            err = np.max(np.abs(g[key][b] - want)) / np.max(np.abs(want))
+            assert err <= 2e-3, (key, b, err)
+        assert abs(g["nl_scale"][b, 0] - ref["c"]) <= 2e-3 * abs(ref["c"]), (b, g["nl_scale"][b, 0], ref["c"])
+
+
 # ------------------------------------------------------------------ tension / linear ----
 @pytest.mark.parametrize("batch,n_steps", [(32, 4096), (5, 333)])
 def test_c1_string_parity(batch, n_steps):
