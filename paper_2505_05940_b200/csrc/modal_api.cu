@@ -549,7 +549,7 @@ modal_status configure_stream(modal_plan *p, int NB)
     if (!stream_host_layout(p, NB, m.L)) return MODAL_OK;
     const mh::StreamLayout &L = m.L;
     if (L.G * 4 < NB) return MODAL_OK;                   // the pickup warp of a CTA handles at most four samples
-    if (md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 4).total > SMEM_LIMIT) return MODAL_OK;
+    if (md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 2, L.nch_max * 8192).total > SMEM_LIMIT) return MODAL_OK;
     std::vector<uint16_t> A;
     stream_host_A(p, L, A);
     CU(m.dA.ensure(A.size() * 2));
@@ -801,11 +801,12 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         StreamConfig &m = p->stream;
         const mh::StreamLayout &L = m.L;
         const int NB = m.NB;
-        const size_t base = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 0).total;
-        int nstg = (int)std::min<size_t>(md::ST_NSTG_MAX, (SMEM_LIMIT - base) / md::ST_STAGE_BYTES);
+        const int stage_bytes = L.nch_max * 8192;                  // one tile per ring stage
+        const size_t base = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, 0, stage_bytes).total;
+        int nstg = (int)std::min<size_t>(md::ST_NSTG_MAX, (SMEM_LIMIT - base) / stage_bytes);
         if (p->opt.mma_nstg > 0) nstg = std::min(nstg, std::max(p->opt.mma_nstg, 2));
         if (nstg < 2) { p->err += "streaming vK kernel: no room for the operand ring\n"; return MODAL_EINCOMPAT; }
-        const size_t smem = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, nstg).total;
+        const size_t smem = md::stream_smem_layout(NB, L.rows_max, L.bch_max, L.TILE_STRIDE, nstg, stage_bytes).total;
         const int KOP = L.KC * 16;
         const size_t nqx = (size_t)NB * KOP * 4, nGx = (size_t)d.n_phi * L.NKB * NB * 4, nfx = (size_t)L.G * 128 * NB * 4, npx = (size_t)4 * L.G * NB * 16 + 256;
         CU(m.dqx.ensure(nqx)); CU(m.dGx.ensure(nGx)); CU(m.dfx.ensure(nfx)); CU(m.dpx.ensure(npx));
@@ -816,7 +817,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             const int *tab = m.dtab.as<int>();
             a.A = m.dA.as<uint16_t>(); a.cta_tab = tab + m.off_cta; a.tile_tab = tab + m.off_tile; a.tile_stride = L.TILE_STRIDE;
             a.blk = tab + m.off_blk; a.blk_nctas = tab + m.off_nct;
-            a.NKB = L.NKB; a.KOP = KOP; a.G = L.G; a.NSTG = nstg; a.rows_max = L.rows_max; a.bch_max = L.bch_max; a.LPQ = m.lpq;
+            a.NKB = L.NKB; a.KOP = KOP; a.G = L.G; a.NSTG = nstg; a.stage_bytes = stage_bytes; a.rows_max = L.rows_max; a.bch_max = L.bch_max; a.LPQ = m.lpq;
             a.n_q = nq; a.n_phi = d.n_phi; a.NQP = P; a.batch = nb; a.n_steps = n_steps;
             a.coeff_stride_q = cb == 1 ? 0 : P; a.coeff_stride_phi = cb == 1 ? 0 : d.n_phi;
             const size_t oq = cb == 1 ? 0 : (size_t)b0 * P;

@@ -117,7 +117,7 @@ inline bool stream_layout(int n_q, int n_phi, int sm, int NB, const std::vector<
     L.G = used;
     L.blk_cta0.assign(L.NKB, 0); L.blk_nctas = nct;
     L.tile_of.assign((size_t)n_phi * L.NKB, -1);
-    const int tiles_cap = std::min(ST_TILES_MAX, 512 / NB);
+    const int tiles_cap = std::min(ST_TILES_MAX, 512 / (NB <= 32 ? 2 * NB : NB));      // TMEM columns: 2 NB per tile when NB <= 32 (dual accumulator halves)
     int cta = 0;
     for (int jb = 0; jb < L.NKB; ++jb) {
         L.blk_cta0[jb] = cta;

@@ -24,8 +24,7 @@ constexpr int ST_BCH_MAX_DEV = 16, ST_TILES_MAX_DEV = 16, ST_NKB_MAX_DEV = 8, ST
 constexpr unsigned ST_POLL_SLEEP = 100;   // ns between polling rounds
 constexpr int SB_FULL = 0, SB_EMPTY = 16, SB_ACCF = 32, SB_ACCE = 48, SB_BRDY = 49, SB_FDONE = 50, SB_TPTR = 56, SB_ABORT = 57;
 constexpr int ST_BARS_BYTES = 512;
-constexpr int ST_NSTG_MAX = 8;          // ring stages of ST_STAGE_BYTES
-constexpr int ST_STAGE_BYTES = 16384;   // two K chunks (hi + lo of 128 rows x 16 K each)
+constexpr int ST_NSTG_MAX = 8;          // ring stages (one tile each)
 
 struct StreamArgs {
     const uint16_t *A;          // H stream: per tile its K chunks, 8 KiB each (hi 4 KiB, lo 4 KiB), UMMA canonical K-major
@@ -33,6 +32,7 @@ struct StreamArgs {
     const int *blk;             // [NKB][4]: k0, nb, koff, first CTA of the block
     const int *blk_nctas;       // [NKB]
     int NKB, KOP, G, NSTG, rows_max, bch_max, LPQ;
+    int stage_bytes;            // ring stage = the most K chunks of a tile x 8 KiB
     int n_q, n_phi, NQP, batch, n_steps;
     int coeff_stride_q, coeff_stride_phi;
     const double *kv, *kq, *r, *astart;
@@ -51,7 +51,7 @@ struct StreamArgs {
 };
 
 struct StreamSmem { size_t bars, tab, ss, wsum, seta, sq, sv, coef, pk, misc, bop, ring, total; };
-__host__ __device__ inline StreamSmem stream_smem_layout(int NB, int rows_max, int bch_max, int tile_stride, int nstg)
+__host__ __device__ inline StreamSmem stream_smem_layout(int NB, int rows_max, int bch_max, int tile_stride, int nstg, int stage_bytes)
 {
     StreamSmem L; size_t o = 0;
     const size_t nel = (size_t)rows_max * NB;
@@ -69,7 +69,7 @@ __host__ __device__ inline StreamSmem stream_smem_layout(int NB, int rows_max, i
     o = flow_align(o, 128);
     L.bop = o;   o += (size_t)bch_max * NB * 64;               // q operand chunks: [slot][hi NB x 16 | lo NB x 16] bf16
     o = flow_align(o, 128);
-    L.ring = o;  o += (size_t)nstg * ST_STAGE_BYTES;
+    L.ring = o;  o += (size_t)nstg * stage_bytes;
     L.total = o;
     return L;
 }
@@ -175,6 +175,34 @@ struct StreamCta {
     uint32_t tbase;
     size_t nel;
 };
+
+// DUAL (NB <= 32): a tile's accumulator has 2 NB columns -- [0, NB) = H_hi q_hi + H_lo q_hi, [NB, 2 NB) = H_hi q_lo -- so that the two MMAs
+// that use H_hi (against q_hi and q_lo) are ONE instruction with the B operand [q_hi ; q_lo] of 2 NB rows (the two halves are adjacent
+// in the operand layout): two MMAs and 8 KiB of shared-memory operand reads per K chunk instead of three and 12 KiB.  The epilogues
+// add the halves.  At NB = 64 the tiles of a CTA would not fit the 512 TMEM columns, so the three-MMA form stays.
+template <int NB> struct StreamDual { static constexpr bool value = NB <= 32; static constexpr int TSTR = NB <= 32 ? 2 * NB : NB; };
+template <int NB, int U, int NU>
+__device__ __forceinline__ void stream_load_t(const uint32_t lane_addr, const int i, uint32_t (&tu)[NU][U])
+{
+    constexpr int TSTR = StreamDual<NB>::TSTR;
+    if (StreamDual<NB>::value) {
+        uint32_t lo[NU][U];
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            TmemUnit<U>::ld(lane_addr + (uint32_t)(i * TSTR + u * U), tu[u]);
+            TmemUnit<U>::ld(lane_addr + (uint32_t)(i * TSTR + NB + u * U), lo[u]);
+        }
+        tmem_ld_wait();
+#pragma unroll
+        for (int u = 0; u < NU; ++u)
+#pragma unroll
+            for (int c = 0; c < U; ++c) tu[u][c] = __float_as_uint(__uint_as_float(tu[u][c]) + __uint_as_float(lo[u][c]));
+    } else {
+#pragma unroll
+        for (int u = 0; u < NU; ++u) TmemUnit<U>::ld(lane_addr + (uint32_t)(i * TSTR + u * U), tu[u]);
+        tmem_ld_wait();
+    }
+}
 
 // q^n of the CTA's K chunks -> bf16 hi / lo operand chunks in shared memory (the B operand of the step's MMAs), by the 128 epilogue
 // threads and the 256 owner threads together (the owners are idle between publishing q^n and the forces of step n).
@@ -292,9 +320,7 @@ __device__ __forceinline__ void stream_epilogue(const StreamArgs &a, const Strea
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             if (tmg) tm[2] += clock64() - tw;
             uint32_t tu[NU][U];
-#pragma unroll
-            for (int u = 0; u < NU; ++u) TmemUnit<U>::ld(lane_addr + (uint32_t)(i * NB + u * U), tu[u]);
-            tmem_ld_wait();
+            stream_load_t<NB, U, NU>(lane_addr, i, tu);
             float *ws = C.wsum + (size_t)(i & 1) * 4 * NB + w4 * NB;
 #pragma unroll
             for (int u = 0; u < NU; ++u) {
@@ -352,9 +378,7 @@ __device__ __forceinline__ void stream_epilogue(const StreamArgs &a, const Strea
         for (int b = 0; b < NB; ++b) facc[b] = 0.f;
         for (int i = 0; i < C.ntiles; ++i) {
             uint32_t tu[NU][U];
-#pragma unroll
-            for (int u = 0; u < NU; ++u) TmemUnit<U>::ld(lane_addr + (uint32_t)(i * NB + u * U), tu[u]);
-            tmem_ld_wait();
+            stream_load_t<NB, U, NU>(lane_addr, i, tu);
             const float4 *ep = reinterpret_cast<const float4 *>(C.seta + i * NB);
 #pragma unroll
             for (int u = 0; u < NU; ++u)
@@ -574,7 +598,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
 {
     extern __shared__ __align__(128) unsigned char st_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const StreamSmem L = stream_smem_layout(NB, a.rows_max, a.bch_max, a.tile_stride, a.NSTG);
+    const StreamSmem L = stream_smem_layout(NB, a.rows_max, a.bch_max, a.tile_stride, a.NSTG, a.stage_bytes);
     StreamCta C;
     C.c = blockIdx.x;
     C.bars = reinterpret_cast<uint64_t *>(st_smem + L.bars);
@@ -632,10 +656,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
         if (warp == 0) {
             // ---------------- P: the H stream of the CTA's tiles, every step, through the ring ----------------
-            // (the loops of P and M run on one thread each: no division, no address arithmetic beyond an add per chunk --
-            //  a chunk's MMAs take ~180 cycles, a careless loop iteration several hundred)
-            // A ring stage holds TWO K chunks of a tile (16 KiB; the odd last chunk of a tile travels alone): one wait, one commit and
-            // one bulk copy per six MMAs -- at N = 16 .. 64 the MMA phase is bound by these per-stage instructions, not by the math.
+            // ONE bulk copy per tile (its K chunks are contiguous in the stream: <= 56 KiB at C4): a cp.async.bulk costs ~670 cycles of the
+            // SM's copy engine whatever its size (measured: 2 KiB and 32 KiB copies take the same time), so 8 or 16 KiB stages capped the
+            // stream at 12-24 B/clk per SM and the step's MMAs waited for it (the whole MMA phase was this stream).
             if (lane == 0) {
                 const uint32_t full0 = smem_u32(C.bars + SB_FULL), empty0 = smem_u32(C.bars + SB_EMPTY), ring0 = smem_u32(C.ring);
                 const int NSTG = a.NSTG;
@@ -643,24 +666,20 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
                 for (int n = 0; n < a.n_steps; ++n)
                     for (int i = 0; i < C.ntiles; ++i) {
                         const int *tt = C.ttab + i * a.tile_stride;
-                        const int nch = tt[1];
-                        const uint16_t *src = a.A + (size_t)tt[2] * 4096;
-                        for (int u = 0; u < nch; u += 2, src += 8192) {
-                            const uint32_t bytes = u + 1 < nch ? 16384u : 8192u;
-                            mbar_wait_fast(empty0 + 8 * sg, ph, C.s_abort);
-                            mbar_expect_tx(full0 + 8 * sg, bytes);
-                            tma_bulk_g2s(ring0 + sg * ST_STAGE_BYTES, src, bytes, full0 + 8 * sg);
-                            if (++sg == NSTG) { sg = 0; ph ^= 1u; }
-                        }
+                        const uint32_t bytes = (uint32_t)tt[1] * 8192u;
+                        mbar_wait_fast(empty0 + 8 * sg, ph, C.s_abort);
+                        mbar_expect_tx(full0 + 8 * sg, bytes);
+                        tma_bulk_g2s(ring0 + sg * a.stage_bytes, a.A + (size_t)tt[2] * 4096, bytes, full0 + 8 * sg);
+                        if (++sg == NSTG) { sg = 0; ph ^= 1u; }
                     }
             }
         } else if (warp == 1) {
             // ---------------- M: the MMAs ------------------------------------------------------------------------
             // The whole warp runs the (uniform) loop and one elected lane issues: inside a lane-0 branch ptxas wraps every
             // tcgen05 instruction in an ELECT / R2UR / branch loop, ~240 cycles per chunk instead of the ~160 its three MMAs take.
-            // The try_wait of the NEXT stage is issued before the MMAs of this one, so its ~90 cycles overlap their issue.
             {
                 const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NB >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+                const uint32_t idesc2 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((2 * NB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // N = 2 NB
                 const uint32_t full0 = smem_u32(C.bars + SB_FULL), empty0 = smem_u32(C.bars + SB_EMPTY), accf0 = smem_u32(C.bars + SB_ACCF);
                 const uint64_t dA0 = umma_desc(smem_u32(C.ring)), dB0 = umma_desc(smem_u32(C.bop));   // + (byte offset >> 4)
                 const int NSTG = a.NSTG;
@@ -671,36 +690,32 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
                     if (n > 0) mbar_wait(smem_u32(C.bars + SB_ACCE), (unsigned)(n - 1) & 1u, C.s_abort);    // last step's accumulators read
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const long long tk = TIMING ? clock64() : 0;
-                    bool ready = mbar_try(full0 + 8 * sg, ph);
                     for (int i = 0; i < C.ntiles; ++i) {
                         const int *tt = C.ttab + i * a.tile_stride;
                         const int nch = tt[1];
-                        const uint32_t td = C.tbase + (uint32_t)(i * NB);
-                        for (int u = 0; u < nch; u += 2) {
-                            const bool two = u + 1 < nch;
+                        const uint32_t td = C.tbase + (uint32_t)(i * StreamDual<NB>::TSTR);
+                        {
+                            const long long tw = TIMING ? clock64() : 0;
+                            mbar_wait(full0 + 8 * sg, ph, C.s_abort);                          // the tile's chunks have landed
+                            if (TIMING) tmw += clock64() - tw;
+                        }
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        uint64_t dA = dA0 + (uint64_t)(sg * (a.stage_bytes >> 4));
+                        for (int u = 0; u < nch; ++u, dA += 8192 / 16) {
                             const uint64_t dB = dB0 + (uint64_t)(tt[4 + u] * (NB * 64 / 16));
-                            const uint64_t dB2 = dB0 + (uint64_t)(tt[4 + (two ? u + 1 : u)] * (NB * 64 / 16));
-                            if (!ready) {
-                                if (TIMING) { const long long tw = clock64(); mbar_wait(full0 + 8 * sg, ph, C.s_abort); tmw += clock64() - tw; }
-                                else mbar_wait(full0 + 8 * sg, ph, C.s_abort);
-                            }
-                            const int sg0 = sg;
-                            if (++sg == NSTG) { sg = 0; ph ^= 1u; }
-                            ready = mbar_try(full0 + 8 * sg, ph);                              // next stage (this or the next step's)
-                            const uint64_t dA = dA0 + (uint64_t)(sg0 * (ST_STAGE_BYTES / 16));
                             if (elect_one_sync()) {
-                                umma_bf16(td, dA, dB, idesc, u > 0);                           // hi * hi
-                                umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);                   // lo * hi
-                                umma_bf16(td, dA, dB + NB * 32 / 16, idesc, 1);                // hi * lo
-                                if (two) {
-                                    umma_bf16(td, dA + 8192 / 16, dB2, idesc, 1);
-                                    umma_bf16(td, dA + 12288 / 16, dB2, idesc, 1);
-                                    umma_bf16(td, dA + 8192 / 16, dB2 + NB * 32 / 16, idesc, 1);
+                                if (StreamDual<NB>::value) {
+                                    umma_bf16(td, dA, dB, idesc2, u > 0);                      // H_hi * [q_hi ; q_lo]  -> both column halves
+                                    umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);               // H_lo * q_hi           -> first half
+                                } else {
+                                    umma_bf16(td, dA, dB, idesc, u > 0);                       // hi * hi
+                                    umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);               // lo * hi
+                                    umma_bf16(td, dA, dB + NB * 32 / 16, idesc, 1);            // hi * lo
                                 }
-                                umma_commit(empty0 + 8 * sg0);
                             }
                         }
-                        if (elect_one_sync()) umma_commit(accf0 + 8 * i);
+                        if (elect_one_sync()) { umma_commit(empty0 + 8 * sg); umma_commit(accf0 + 8 * i); }
+                        if (++sg == NSTG) { sg = 0; ph ^= 1u; }
                     }
                     if (TIMING) tmm += clock64() - tk;
                 }
