@@ -700,10 +700,12 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
                             if (TIMING) tmw += clock64() - tw;
                         }
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                        uint64_t dA = dA0 + (uint64_t)(sg * (a.stage_bytes >> 4));
-                        for (int u = 0; u < nch; ++u, dA += 8192 / 16) {
-                            const uint64_t dB = dB0 + (uint64_t)(tt[4 + u] * (NB * 64 / 16));
-                            if (elect_one_sync()) {
+                        // one elected lane issues the whole tile: an elect block of its own per chunk costs ~130 cycles of issue latency
+                        // (ELECT, the R2UR moves, the branch), a loop inside the block ~47 per MMA (the shared-memory read of A)
+                        if (elect_one_sync()) {
+                            uint64_t dA = dA0 + (uint64_t)(sg * (a.stage_bytes >> 4));
+                            for (int u = 0; u < nch; ++u, dA += 8192 / 16) {
+                                const uint64_t dB = dB0 + (uint64_t)(tt[4 + u] * (NB * 64 / 16));
                                 if (StreamDual<NB>::value) {
                                     umma_bf16(td, dA, dB, idesc2, u > 0);                      // H_hi * [q_hi ; q_lo]  -> both column halves
                                     umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);               // H_lo * q_hi           -> first half
@@ -713,8 +715,9 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
                                     umma_bf16(td, dA, dB + NB * 32 / 16, idesc, 1);            // hi * lo
                                 }
                             }
+                            umma_commit(empty0 + 8 * sg); umma_commit(accf0 + 8 * i);
                         }
-                        if (elect_one_sync()) { umma_commit(empty0 + 8 * sg); umma_commit(accf0 + 8 * i); }
+                        __syncwarp();
                         if (++sg == NSTG) { sg = 0; ph ^= 1u; }
                     }
                     if (TIMING) tmm += clock64() - tk;
