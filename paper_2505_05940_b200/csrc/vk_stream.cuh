@@ -675,9 +675,10 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
             }
         } else if (warp == 1) {
             // ---------------- M: the MMAs ------------------------------------------------------------------------
-            // The whole warp runs the (uniform) loop and one elected lane issues: inside a lane-0 branch ptxas wraps every
-            // tcgen05 instruction in an ELECT / R2UR / branch loop, ~240 cycles per chunk instead of the ~160 its three MMAs take.
-            {
+            // ONE elected lane runs the whole role.  (A lane-0 branch makes ptxas wrap every tcgen05 instruction in an ELECT / R2UR /
+            // branch loop; under elect.sync it knows a single thread is active.  An elect block per chunk or per tile costs ~130 and
+            // ~300 cycles of issue latency each time it is entered -- measured beside ~45 cycles per MMA inside one.)
+            if (elect_one_sync()) {
                 const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(NB >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
                 const uint32_t idesc2 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((2 * NB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // N = 2 NB
                 const uint32_t full0 = smem_u32(C.bars + SB_FULL), empty0 = smem_u32(C.bars + SB_EMPTY), accf0 = smem_u32(C.bars + SB_ACCF);
@@ -700,30 +701,26 @@ __global__ void __launch_bounds__(ST_THREADS, 1) vk_stream_kernel(const StreamAr
                             if (TIMING) tmw += clock64() - tw;
                         }
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                        // one elected lane issues the whole tile: an elect block of its own per chunk costs ~130 cycles of issue latency
-                        // (ELECT, the R2UR moves, the branch), a loop inside the block ~47 per MMA (the shared-memory read of A)
-                        if (elect_one_sync()) {
-                            uint64_t dA = dA0 + (uint64_t)(sg * (a.stage_bytes >> 4));
-                            for (int u = 0; u < nch; ++u, dA += 8192 / 16) {
-                                const uint64_t dB = dB0 + (uint64_t)(tt[4 + u] * (NB * 64 / 16));
-                                if (StreamDual<NB>::value) {
-                                    umma_bf16(td, dA, dB, idesc2, u > 0);                      // H_hi * [q_hi ; q_lo]  -> both column halves
-                                    umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);               // H_lo * q_hi           -> first half
-                                } else {
-                                    umma_bf16(td, dA, dB, idesc, u > 0);                       // hi * hi
-                                    umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);               // lo * hi
-                                    umma_bf16(td, dA, dB + NB * 32 / 16, idesc, 1);            // hi * lo
-                                }
+                        uint64_t dA = dA0 + (uint64_t)(sg * (a.stage_bytes >> 4));
+                        for (int u = 0; u < nch; ++u, dA += 8192 / 16) {
+                            const uint64_t dB = dB0 + (uint64_t)(tt[4 + u] * (NB * 64 / 16));
+                            if (StreamDual<NB>::value) {
+                                umma_bf16(td, dA, dB, idesc2, u > 0);                      // H_hi * [q_hi ; q_lo]  -> both column halves
+                                umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);               // H_lo * q_hi           -> first half
+                            } else {
+                                umma_bf16(td, dA, dB, idesc, u > 0);                       // hi * hi
+                                umma_bf16(td, dA + 4096 / 16, dB, idesc, 1);               // lo * hi
+                                umma_bf16(td, dA, dB + NB * 32 / 16, idesc, 1);            // hi * lo
                             }
-                            umma_commit(empty0 + 8 * sg); umma_commit(accf0 + 8 * i);
                         }
-                        __syncwarp();
+                        umma_commit(empty0 + 8 * sg); umma_commit(accf0 + 8 * i);
                         if (++sg == NSTG) { sg = 0; ph ^= 1u; }
                     }
                     if (TIMING) tmm += clock64() - tk;
                 }
-                if (TIMING && lane == 0) { a.timing[(size_t)C.c * 16 + 12] = tmm; a.timing[(size_t)C.c * 16 + 13] = tmw; }
+                if (TIMING) { a.timing[(size_t)C.c * 16 + 12] = tmm; a.timing[(size_t)C.c * 16 + 13] = tmw; }
             }
+            __syncwarp();
         } else if (warp == 2 && C.c < a.batch) {
             stream_pickup_warp<NB>(a, C, lane);
         }
