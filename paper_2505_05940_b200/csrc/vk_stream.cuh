@@ -3,8 +3,10 @@
 //
 // Per step (Eq. 9 with C eliminated; update PAPER.md:120-124 Eq. 10 in delta form, R4):
 //   t[(n,k)][b] = sum_r H^n[k][r] q[b][r]          tcgen05.mma, M = 128 rows k of one (mode n, k block) tile, N = NB samples, K = r;
-//                                                  H streamed from L2 by TMA as bf16 hi + lo, q rebuilt in shared memory as bf16 hi + lo,
-//                                                  three MMAs per K chunk (hi*hi + lo*hi + hi*lo), fp32 accumulators of ALL tiles of the CTA in TMEM
+//                                                  H streamed from L2 by TMA as bf16 hi + lo (one bulk copy per tile into a ring of tile-sized
+//                                                  stages), q rebuilt in shared memory as bf16 hi + lo; per K chunk three MMAs (hi*hi + lo*hi +
+//                                                  hi*lo) at NB = 64, two at NB <= 32 (H_hi * [q_hi ; q_lo] with N = 2 NB, then H_lo * q_hi: the
+//                                                  epilogues add the two column halves); fp32 accumulators of ALL tiles of the CTA in TMEM
 //   G_n[b] = sum_k q[b][k] t[(n,k)][b]             epilogue 1: thread <-> row k; products reduced over the 128 rows by a butterfly that leaves
 //                                                  each lane with one sample, partial G per k block exchanged through L2 (tagged words)
 //   f[b][k] = sum_n s_n[b] G_n[b] t[(n,k)][b]      epilogue 2: the thread's row accumulates over the CTA's tiles in registers
