@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmodal.so")
 SOURCES = [os.path.join(CSRC, "modal_api.cu"), os.path.join(CSRC, "vk_static.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "host_math.hpp", "vk_flow.cuh", "flow_schedule.hpp", "vk_mma.cuh", "mma_schedule.hpp", "peaks.cuh", "vk_stream.cuh", "stream_schedule.hpp", "vk_bptt.cuh", "vk_small.cuh", "vk_dense.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "host_math.hpp", "vk_flow.cuh", "flow_schedule.hpp", "vk_mma.cuh", "mma_schedule.hpp", "peaks.cuh", "vk_stream.cuh", "stream_schedule.hpp", "vk_bptt.cuh", "vk_small.cuh", "vk_dense.cuh", "vk_repl.cuh", "repl_schedule.hpp")] + [
     os.path.join(os.path.dirname(HERE), "include", "modal.h")]
 
 

@@ -21,6 +21,8 @@
 #include "vk_bptt.cuh"
 #include "vk_small.cuh"
 #include "vk_dense.cuh"
+#include "vk_repl.cuh"
+#include "repl_schedule.hpp"
 #include "peaks.cuh"
 
 namespace mh = modal_host;
@@ -65,6 +67,14 @@ struct MmaConfig {
     DevBuf dslabs, dtab, dQop, dqf, dGx, dfx, dflags, dpx;
 };
 
+struct ReplConfig {                  // vk_repl: replicated state, whole in-plane modes per CTA (one sample)
+    bool tried = false, ok = false;
+    int CL = 1, NCL = 1, SL = 0, NQ2 = 0;
+    size_t smem = 0;
+    mh::ReplLayout L;
+    DevBuf dHp, dtab, dcls, dX;
+};
+
 struct StreamConfig {                // vk_stream: layout for one NB (samples of a launch, padded to 16)
     bool ok = false;
     int NB = 0, lpq = 1;
@@ -107,6 +117,7 @@ struct modal_plan {
     bool bp_H_valid = false;
     DevBuf dHdense, ddscr; bool dense_H_valid = false;                // vk_dense_kernel: dense fp32 H (internal order, padded rows), exchange words
     DevBuf dHsmall; bool small_H_valid = false;                       // vk_small_kernel: dense fp32 H, internal order
+    ReplConfig repl;
     std::map<long long, FlowConfig> flow_cfgs;
     DevBuf dkv, dkq, dr, dast, ds, dsT, dw, dlam, dc, dq0, dv0, dgain, dbad, dout;      // dsT: s_n transposed [n_phi][coeff_batch] (batched kernel)
     float *pinned_out = nullptr; size_t pinned_bytes = 0;            // staging of modal_simulate_host
@@ -160,7 +171,7 @@ void set_H(modal_plan *p, Get get_user)
     }
     for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
     p->flow_cfgs.clear();                                   // schedules depend on the zero pattern
-    p->mma.tried = false; p->mma.ok = false; p->stream.NB = 0; p->bp_H_valid = false; p->small_H_valid = false; p->dense_H_valid = false;
+    p->mma.tried = false; p->mma.ok = false; p->repl.tried = false; p->repl.ok = false; p->stream.NB = 0; p->bp_H_valid = false; p->small_H_valid = false; p->dense_H_valid = false;
     p->H_dirty = true;
 }
 
@@ -510,6 +521,62 @@ modal_status configure_mma(modal_plan *p)
 
 // ---- vk_stream (streaming tensor-core kernel for small / medium batches on a large tensor) -----------------
 // Host part: the layout and the H stream from the fp32 H values the device holds (flow tiles, internal order).
+// vk_repl: layout + device tables, once per plan and H.  Needs the parity-class structure and a symmetric H (repl_schedule.hpp); the
+// grid is as many thread-block clusters as the GPU holds at once (every CTA spins on its peers: all must be resident).
+modal_status configure_repl(modal_plan *p)
+{
+    ReplConfig &m = p->repl;
+    if (m.tried) return MODAL_OK;
+    m.tried = true; m.ok = false;
+    if (p->d.model != MODAL_VK || p->d.n_q > md::RP_THREADS) return MODAL_OK;
+    const int nq = p->d.n_q, nphi = p->d.n_phi;
+    const bool classes = p->d.geom == MODAL_RECT && p->opt.parity_order;
+    auto cls_q = [&](int k_int) { const int k = p->perm[k_int]; return classes ? (p->mq.m[k] & 1) * 2 + (p->mq.n[k] & 1) : 0; };
+    std::vector<int> class_start{0}, cls(nq, 0);
+    for (int k = 1; k < nq; ++k) if (cls_q(k) != cls_q(k - 1)) class_start.push_back(k);
+    class_start.push_back(nq);
+    if ((int)class_start.size() - 1 > md::RP_MAXCLS) return MODAL_OK;
+    for (int c = 0; c + 1 < (int)class_start.size(); ++c) for (int k = class_start[c]; k < class_start[c + 1]; ++k) cls[k] = c;
+    cudaFuncAttributes fa{};
+    CU(cudaFuncGetAttributes(&fa, md::vk_repl_kernel<false>));
+    cudaFuncAttributes fb{};
+    CU(cudaFuncGetAttributes(&fb, md::vk_repl_kernel<true>));
+    const size_t dyn_max = SMEM_LIMIT - std::max(fa.sharedSizeBytes, fb.sharedSizeBytes) - 1024;
+    CU(cudaFuncSetAttribute(md::vk_repl_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
+    CU(cudaFuncSetAttribute(md::vk_repl_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
+    std::vector<double> Hi;
+    const int NQ2 = (nq + 1) & ~1;
+    for (int CL : {8, 4}) {
+        const int SL = (((NQ2 + CL - 1) / CL) + 1) & ~1;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(CL); cfg.blockDim = dim3(md::RP_THREADS); cfg.dynamicSmemBytes = dyn_max;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int nc = 0;
+        if (cudaOccupancyMaxActiveClusters(&nc, md::vk_repl_kernel<false>, &cfg) != cudaSuccess) { cudaGetLastError(); continue; }
+        nc = std::min(nc, (nphi + CL - 1) / CL);
+        if (nc < 1) continue;
+        const size_t fixed = (size_t)4 + 2 * CL * SL + 16;
+        if (dyn_max / 4 <= fixed) continue;
+        if (Hi.empty()) { Hi.resize((size_t)nphi * nq * nq); mh::unpack_flow_tiles(nq, nphi, p->Hf, Hi.data()); }
+        if (!mh::repl_layout(nq, nphi, nc * CL, dyn_max / 4 - fixed, class_start, Hi.data(), m.L)) continue;
+        m.CL = CL; m.NCL = nc; m.SL = SL; m.NQ2 = NQ2;
+        m.smem = md::repl_smem_bytes(m.L.hfloats_max, m.L.cp_max, m.L.rp_max, CL, SL);
+        CU(m.dHp.ensure(std::max<size_t>(m.L.Hp.size(), 4) * 4));
+        CU(cudaMemcpy(m.dHp.p, m.L.Hp.data(), m.L.Hp.size() * 4, cudaMemcpyHostToDevice));
+        CU(m.dtab.ensure(m.L.tab.size() * 4));
+        CU(cudaMemcpy(m.dtab.p, m.L.tab.data(), m.L.tab.size() * 4, cudaMemcpyHostToDevice));
+        CU(m.dcls.ensure(cls.size() * 4));
+        CU(cudaMemcpy(m.dcls.p, cls.data(), cls.size() * 4, cudaMemcpyHostToDevice));
+        CU(m.dX.ensure((size_t)2 * nc * NQ2 * 8));
+        std::vector<float>().swap(m.L.Hp);                  // the packed copy lives on the device now
+        m.ok = true;
+        break;
+    }
+    return MODAL_OK;
+}
+
 bool stream_host_layout(const modal_plan *p, int NB, mh::StreamLayout &L)
 {
     if (p->d.model != MODAL_VK) return false;
@@ -679,7 +746,14 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         if (p->opt.vk_impl == 0 && batch >= 8 && modes_max > 8) use_dense = false;
         if (p->opt.vk_impl == 5 && !use_dense) { p->err += "vk_impl=5: the dense H of a CTA's modes does not fit shared memory (or one CTA per sample)\n"; return MODAL_EINCOMPAT; }
     }
-    if (d.model == MODAL_VK && !use_small && !use_dense) {
+    // one sample of a plate too large for the team kernel: replicated state, whole in-plane modes per CTA, one hop per step (vk_repl.cuh)
+    bool use_repl = false;
+    if (d.model == MODAL_VK && !use_small && !use_dense && (p->opt.vk_impl == 6 || (p->opt.vk_impl == 0 && batch == 1)) &&
+        p->opt.flow_g == 0 && p->opt.flow_ns == 0 && p->opt.flow_res < 0) {
+        if (batch == 1) { modal_status s = configure_repl(p); if (s != MODAL_OK) return s; use_repl = p->repl.ok; }
+        if (p->opt.vk_impl == 6 && !use_repl) { p->err += "vk_impl=6: the replicated-state kernel takes one sample of a plan whose H has the parity-class structure and fits shared memory\n"; return MODAL_EINCOMPAT; }
+    }
+    if (d.model == MODAL_VK && !use_small && !use_dense && !use_repl) {
         const int impl = p->opt.vk_impl;
         if ((impl == 0 && batch >= 64) || impl == 2) { modal_status s = configure_mma(p); if (s != MODAL_OK) return s; use_mma = p->mma.ok; }
         if (!use_mma && ((impl == 0 && batch >= 8) || impl == 3)) {
@@ -797,6 +871,50 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
         persistent = true;
         p->kinfo[0] = 6; p->kinfo[1] = dn_G; p->kinfo[2] = dn_per_launch; p->kinfo[3] = md::DN_THREADS;
         p->kinfo[4] = (int)dn_smem; p->kinfo[5] = 1 | 2; p->kinfo[6] = 0; p->kinfo[7] = P;
+    } else if (use_repl) {
+        ReplConfig &m = p->repl;
+        md::ReplArgs a{};
+        a.n_q = nq; a.NQ2 = m.NQ2; a.n_phi = d.n_phi; a.NQP = P; a.n_steps = n_steps; a.G = m.L.G; a.CL = m.CL; a.NCL = m.NCL; a.SL = m.SL;
+        a.out_cta = m.L.out_cta; a.hfloats_max = m.L.hfloats_max; a.cp_max = m.L.cp_max; a.rp_max = m.L.rp_max;
+        a.Hp = m.dHp.as<float>(); a.tab = m.dtab.as<int>(); a.cls = m.dcls.as<int>();
+        a.kv = p->dkv.as<double>(); a.kq = p->dkq.as<double>(); a.r = p->dr.as<double>(); a.astart = p->dast.as<double>();
+        a.s = p->ds.as<float>(); a.w = p->dw.as<float>();
+        a.q0 = p->dq0.as<double>(); a.v0 = p->dv0.as<double>();
+        a.auto_start = auto_start; a.half_T2 = half_T2;
+        a.fext = init->fext_signal; a.gain = init->fext_signal ? p->dgain.as<double>() : nullptr;
+        a.out = out_dev; a.traj = init->traj_dev; a.kperm = p->dperm.as<int>(); a.first_bad = p->dbad.as<int>();
+        a.X = m.dX.as<unsigned long long>(); a.timeout_flag = p->dtimeout.as<int>();
+        CU(cudaMemsetAsync(m.dX.p, 0, (size_t)2 * m.NCL * m.NQ2 * 8, st));
+        const bool timing = p->opt.timing != 0;
+        if (timing) {
+            CU(p->dtiming.ensure((size_t)m.L.G * 64));
+            CU(cudaMemsetAsync(p->dtiming.p, 0, (size_t)m.L.G * 64, st));
+            a.timing = p->dtiming.as<long long>();
+        }
+        {
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3(m.L.G); cfg.blockDim = dim3(md::RP_THREADS); cfg.dynamicSmemBytes = m.smem; cfg.stream = st;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = m.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            CU(timing ? cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<true>, a) : cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<false>, a));
+        }
+        CU(cudaGetLastError());
+        if (timing) {
+            CU(cudaStreamSynchronize(st));
+            std::vector<long long> tm((size_t)m.L.G * 8);
+            CU(cudaMemcpy(tm.data(), p->dtiming.p, tm.size() * 8, cudaMemcpyDeviceToHost));
+            double acc[8] = {0}, mx[8] = {0};
+            for (size_t x = 0; x < tm.size(); ++x) { acc[x & 7] += (double)tm[x]; mx[x & 7] = std::max(mx[x & 7], (double)tm[x]); }
+            const double den = (double)m.L.G * n_steps;
+            fprintf(stderr, "[modal repl timing] G=%d clusters of %d, H <= %d KiB per CTA, rows per item <= %d  cycles/step mean | max over CTAs:\n"
+                            "   items (t = H q partials) %.0f | %.0f   join + block sums %.0f | %.0f   cluster reduce-scatter + publish %.0f | %.0f   gather %.0f | %.0f\n",
+                    m.L.G, m.CL, m.L.hfloats_max / 256, m.L.rows_max, acc[0] / den, mx[0] / n_steps, acc[1] / den, mx[1] / n_steps,
+                    acc[2] / den, mx[2] / n_steps, acc[3] / den, mx[3] / n_steps);
+        }
+        persistent = true;
+        p->kinfo[0] = 8; p->kinfo[1] = m.L.G; p->kinfo[2] = m.CL; p->kinfo[3] = md::RP_THREADS;
+        p->kinfo[4] = (int)m.smem; p->kinfo[5] = 1 | 2; p->kinfo[6] = m.L.rows_max; p->kinfo[7] = P;
     } else if (use_stream) {
         StreamConfig &m = p->stream;
         const mh::StreamLayout &L = m.L;
@@ -1372,7 +1490,7 @@ extern "C" modal_status modal_plan_set_option(modal_plan *p, const char *key, in
     if (!p || !key) return MODAL_EINVAL;
     p->err.clear();
     struct { const char *name; int *field; int lo, hi; } tab[] = {
-        {"vk_impl", &p->opt.vk_impl, 0, 5}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
+        {"vk_impl", &p->opt.vk_impl, 0, 6}, {"flow_g", &p->opt.flow_g, 0, 1024}, {"flow_ns", &p->opt.flow_ns, 0, 32},
         {"flow_res", &p->opt.flow_res, -1, 1 << 20}, {"mma_split", &p->opt.mma_split, 0, 4}, {"mma_ng", &p->opt.mma_ng, 0, 8},
         {"mma_nstg", &p->opt.mma_nstg, 0, 16}, {"mma_cluster", &p->opt.mma_cluster, 0, 1}, {"parity_order", &p->opt.parity_order, 0, 1}, {"timing", &p->opt.timing, 0, 1}};
     for (auto &t : tab)
@@ -1454,6 +1572,7 @@ extern "C" void modal_plan_destroy(modal_plan *p)
                           &p->stream.dqx, &p->stream.dGx, &p->stream.dfx, &p->stream.dpx}) b->release();
     for (DevBuf &b : p->bp) b.release();
     p->dHsmall.release(); p->dHdense.release(); p->ddscr.release();
+    p->repl.dHp.release(); p->repl.dtab.release(); p->repl.dcls.release(); p->repl.dX.release();
         for (auto &kv : p->flow_cfgs) kv.second.dsched.release();
         if (p->pinned_out) cudaFreeHost(p->pinned_out);
     }
