@@ -908,7 +908,7 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             for (size_t x = 0; x < tm.size(); ++x) { acc[x & 7] += (double)tm[x]; mx[x & 7] = std::max(mx[x & 7], (double)tm[x]); }
             const double den = (double)m.L.G * n_steps;
             fprintf(stderr, "[modal repl timing] G=%d clusters of %d, H <= %d KiB per CTA, rows per item <= %d  cycles/step mean | max over CTAs:\n"
-                            "   items (t = H q partials) %.0f | %.0f   join + block sums %.0f | %.0f   cluster reduce-scatter + publish %.0f | %.0f   gather %.0f | %.0f\n",
+                            "   items (partials of t = H q) %.0f | %.0f   join + block sums %.0f | %.0f   cluster reduce-scatter + publish %.0f | %.0f   gather %.0f | %.0f\n",
                     m.L.G, m.CL, m.L.hfloats_max / 256, m.L.rows_max, acc[0] / den, mx[0] / n_steps, acc[1] / den, mx[1] / n_steps,
                     acc[2] / den, mx[2] / n_steps, acc[3] / den, mx[3] / n_steps);
         }

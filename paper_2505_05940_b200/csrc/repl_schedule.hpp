@@ -42,8 +42,8 @@ struct ReplLayout {
     std::vector<float> Hp;                        // packed blocks, CTA after CTA
     // device table, RP_CTA_STRIDE ints per CTA:
     //   [0] hoff / 4 (float4 units into Hp)  [1] hfloats  [2] nmodes  [3] items  [4..8) mode ids
-    //   items [t]: {hoff (floats into the CTA's H), ld, qa0, nrows, qb0, rp_off (-1: none), rp_stride, cp_off}
-    //   joins [m][class]: {kind 0 none / 1 column sums / 2 row sums, base, count, stride}
+    //   items [t]: {hoff (floats into the CTA's H), ld | mode slot << 16, qa0, nrows, qb0, rp_off (-1: none), rp_stride, cp_off}
+    //   joins [m][class]: {kind 0 none / 1 column sums / 2 row sums, base, count, stride of the partials (1) or pitch of a row (2)}
     std::vector<int> tab;
 };
 
@@ -111,22 +111,23 @@ inline bool repl_layout(int n_q, int n_phi, int G, size_t cap_floats, const std:
                 for (int j = 0; j < ldb; ++j)
                     L.Hp.push_back(j < lb ? (float)Hn[(size_t)(class_start[b.a] + i) * n_q + class_start[b.b] + j] : 0.f);
             const bool rows = b.a != b.b;
+            int slot = 0;
+            while (L.cta_modes[(size_t)g * RP_MAXM + slot] != b.n) ++slot;
+            const int rpitch = nq4 | 1;                                            // odd: thread k reads row k of rpart without bank conflicts
             const int RC = (la + nchunks - 1) / nchunks, nc = (la + RC - 1) / RC;
             L.rows_max = std::max(L.rows_max, RC);
             for (int j = 0; j < nc; ++j)
                 for (int cq = 0; cq < nq4; ++cq, ++t) {
                     int *I = items + t * RP_ITEM;
                     const int r0 = j * RC, nr = std::min(RC, la - r0);
-                    I[0] = hoff + r0 * ldb + 4 * cq; I[1] = ldb; I[2] = class_start[b.a] + r0; I[3] = nr; I[4] = class_start[b.b] + 4 * cq;
-                    I[5] = rows ? rp + r0 * nq4 + cq : -1; I[6] = nq4; I[7] = cp + j * ldb + 4 * cq;
+                    I[0] = hoff + r0 * ldb + 4 * cq; I[1] = ldb | (slot << 16); I[2] = class_start[b.a] + r0; I[3] = nr; I[4] = class_start[b.b] + 4 * cq;
+                    I[5] = rows ? rp + r0 * rpitch + cq : -1; I[6] = rpitch; I[7] = cp + j * ldb + 4 * cq;
                 }
-            int slot = 0;
-            while (L.cta_modes[(size_t)g * RP_MAXM + slot] != b.n) ++slot;
             int *Jb = joins + (slot * RP_MAXCLS + b.b) * RP_JOIN;                  // the column class: column sums
             if (Jb[0]) return false;                                               // a class with two partner classes in one mode: not this kernel's case
             Jb[0] = 1; Jb[1] = cp; Jb[2] = nc; Jb[3] = ldb;
-            if (rows) { int *Ja = joins + (slot * RP_MAXCLS + b.a) * RP_JOIN; if (Ja[0]) return false; Ja[0] = 2; Ja[1] = rp; Ja[2] = nq4; Ja[3] = 1; }
-            hoff += la * ldb; cp += nc * ldb; if (rows) rp += la * nq4;
+            if (rows) { int *Ja = joins + (slot * RP_MAXCLS + b.a) * RP_JOIN; if (Ja[0]) return false; Ja[0] = 2; Ja[1] = rp; Ja[2] = nq4; Ja[3] = rpitch; }
+            hoff += la * ldb; cp += nc * ldb; if (rows) rp += la * rpitch;
         }
         if (t > RP_THREADS) return false;
         T[0] = (int)(L.cta_hoff[g] / 4); T[1] = hoff; T[2] = L.cta_nmodes[g]; T[3] = t;

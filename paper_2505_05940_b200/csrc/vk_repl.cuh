@@ -48,33 +48,43 @@ __host__ __device__ inline size_t repl_smem_bytes(int hfloats_max, int cp_max, i
     return ((size_t)hfloats_max + cp_max + rp_max + 4 + (size_t)2 * CL * SL) * 4 + 64;
 }
 
-// sums of M values over the block, fixed order; every thread gets them.  red: M * 16 floats.  Two barriers.
-template <int M>
-__device__ __forceinline__ void rp_block_sum(float (&a)[M], float *red)
+// sums of nv <= 8 values over the block, fixed order; every thread gets them.  red: [16 warps][8] floats of THIS step's parity (the
+// caller double-buffers, so one barrier is enough: the buffer is rewritten two steps later, behind several barriers).
+__device__ __forceinline__ void rp_block_sum8(float (&a)[8], int nv, float *red)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
-    for (int x = 0; x < M; ++x) {
+    for (int x = 0; x < 8; ++x)
+        if (x < nv) {
 #pragma unroll
-        for (int m = 16; m >= 1; m >>= 1) a[x] += __shfl_xor_sync(0xffffffffu, a[x], m);
-        if (lane == 0) red[x * 16 + warp] = a[x];
+            for (int m = 16; m >= 1; m >>= 1) a[x] += __shfl_xor_sync(0xffffffffu, a[x], m);
+        }
+    if (lane == 0) {
+        *reinterpret_cast<float4 *>(red + warp * 8) = make_float4(a[0], a[1], a[2], a[3]);
+        if (nv > 4) *reinterpret_cast<float4 *>(red + warp * 8 + 4) = make_float4(a[4], a[5], a[6], a[7]);
     }
     __syncthreads();
+    float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-    for (int x = 0; x < M; ++x) {
-        float A = 0.f;
-#pragma unroll
-        for (int y = 0; y < RP_THREADS / 32; ++y) A += red[x * 16 + y];
-        a[x] = A;
+    for (int y = 0; y < RP_THREADS / 32; ++y) {
+        const float4 u = *reinterpret_cast<const float4 *>(red + y * 8);
+        A.x += u.x; A.y += u.y; A.z += u.z; A.w += u.w;
     }
-    __syncthreads();
+    if (nv > 4) {
+#pragma unroll
+        for (int y = 0; y < RP_THREADS / 32; ++y) {
+            const float4 u = *reinterpret_cast<const float4 *>(red + y * 8 + 4);
+            B.x += u.x; B.y += u.y; B.z += u.z; B.w += u.w;
+        }
+    }
+    a[0] = A.x; a[1] = A.y; a[2] = A.z; a[3] = A.w; a[4] = B.x; a[5] = B.y; a[6] = B.z; a[7] = B.w;
 }
 
 template <bool TIMING>
 __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a)
 {
     __shared__ __align__(16) float qs[RP_THREADS + 8];
-    __shared__ float red[(RP_MAXM + 2) * 16];
+    __shared__ __align__(16) float red[2 * 16 * 8];
     __shared__ __align__(16) float part2[RP_NSUB_MAX * RP_THREADS];     // partial sums of the gather sub-groups
     __shared__ __align__(8) uint64_t rsbar[2];
     __shared__ volatile int s_abort;
@@ -102,7 +112,8 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
             J[m] = make_int4(0, 0, 0, 0);
             if (mine && m < nmodes) {
                 J[m] = *reinterpret_cast<const int4 *>(T + RP_HDR + RP_THREADS * RP_ITEM + (m * RP_MAXCLS + c) * RP_JOIN);
-                J[m].y += (k - first) * (J[m].x == 2 ? J[m].z : 1);   // row sums: the row's quads are consecutive; column sums: the column
+                if (J[m].x == 2) { J[m].y += (k - first) * J[m].w; J[m].w = 1; }      // row sums: the row's quads are consecutive (odd row pitch)
+                else J[m].y += k - first;                                              // column sums: one partial per chunk of rows
             }
         }
     }
@@ -155,7 +166,7 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
         // ---- a2: the thread's item ----------------------------------------------------------------------------
         if (has_item) {
             const float4 *hp = reinterpret_cast<const float4 *>(Hs + I0.x);
-            const int ld4 = I0.y >> 2;
+            const int ld4 = (I0.y & 0xffff) >> 2;
             const float4 qb = make_float4(qs[I1.x], qs[I1.x + 1], qs[I1.x + 2], qs[I1.x + 3]);   // a class need not start at a multiple of 4
             const float *qa = qs + I0.z;
             float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -178,33 +189,32 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
         }
         __syncthreads();
         if (TIMING) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
-        // ---- join, a3, a4 ------------------------------------------------------------------------------------------
-        float t[RP_MAXM], G[RP_MAXM];
+        // ---- join (thread k: t_m[k] of every mode of the CTA), a3, a4 ---------------------------------------------------
+        float t[RP_MAXM], vals[8];
 #pragma unroll
         for (int m = 0; m < RP_MAXM; ++m) {
-            float acc = 0.f;
+            float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
             if (J[m].x) {
                 const float *src = (J[m].x == 2 ? rpart : cpart) + J[m].y;
-                for (int i = 0; i < J[m].z; ++i) acc += src[i * J[m].w];
+                const int cnt = J[m].z, st_ = J[m].w;
+                int i = 0;
+                for (; i + 3 < cnt; i += 4) { a0 += src[i * st_]; a1 += src[(i + 1) * st_]; a2 += src[(i + 2) * st_]; a3 += src[(i + 3) * st_]; }
+                for (; i < cnt; ++i) a0 += src[i * st_];
             }
-            t[m] = acc; G[m] = x * acc;
+            t[m] = (a0 + a1) + (a2 + a3); vals[m] = x * t[m];
         }
-        if (out_cta) {                                         // a1 pickup + a6 write-out ride on the same block sum
-            float o[RP_MAXM + 2];
 #pragma unroll
-            for (int m = 0; m < RP_MAXM; ++m) o[m] = G[m];
-            o[RP_MAXM] = wk * x; o[RP_MAXM + 1] = x * x;
-            rp_block_sum<RP_MAXM + 2>(o, red);
-#pragma unroll
-            for (int m = 0; m < RP_MAXM; ++m) G[m] = o[m];
-            if (k == 0) { a.out[n] = o[RP_MAXM]; if (bad < 0 && !(isfinite(o[RP_MAXM]) && isfinite(o[RP_MAXM + 1]))) bad = n; }
+        for (int m = RP_MAXM; m < 8; ++m) vals[m] = 0.f;
+        // a1 pickup + a6 write-out ride on the same block sum (slots RP_MAXM, RP_MAXM + 1; only the CTA out_cta)
+        if (out_cta) { vals[RP_MAXM] = wk * x; vals[RP_MAXM + 1] = x * x; }
+        rp_block_sum8(vals, out_cta ? RP_MAXM + 2 : nmodes, red + (n & 1) * 128);
+        if (out_cta) {
+            if (k == 0) { a.out[n] = vals[RP_MAXM]; if (bad < 0 && !(isfinite(vals[RP_MAXM]) && isfinite(vals[RP_MAXM + 1]))) bad = n; }
             if (a.traj && mine) a.traj[(size_t)n * a.n_q + kp] = q;
-        } else {
-            rp_block_sum<RP_MAXM>(G, red);
         }
         float facc = 0.f;
 #pragma unroll
-        for (int m = 0; m < RP_MAXM; ++m) facc = fmaf(sm_[m] * G[m], t[m], facc);
+        for (int m = 0; m < RP_MAXM; ++m) facc = fmaf(sm_[m] * vals[m], t[m], facc);
         if (TIMING) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
         // ---- exchange ----------------------------------------------------------------------------------------------
         const unsigned par = (unsigned)n & 1u, epoch = (unsigned)n + 1u;
