@@ -162,6 +162,10 @@ modal_status modal_bptt(modal_plan *plan, int batch, int n_steps, const modal_bp
  *                  5 dense-team kernel (a team of <= 32 CTAs per sample, every CTA keeps the whole state, one hop per step; chosen
  *                  automatically below batch 64 when the dense H of a CTA's modes fits shared memory, e.g. 100 + 50 modes, and,
  *                  from batch 8 on, a CTA has at most 8 modes)
+ *                  6 replicated-state kernel (ONE sample; every CTA keeps the whole state and whole in-plane modes whose H^n sits in
+ *                  shared memory as the dense blocks of the parity-class structure, stored once per symmetric pair; thread-block
+ *                  clusters reduce the partial forces through distributed shared memory, one L2 hop per step; chosen automatically
+ *                  at batch 1 when the dense-team kernel does not fit and the blocks do: the 400 + 200 mode plate of the headline)
  *   "flow_g"       CTAs per team of the flow kernel (0 automatic)
  *   "flow_ns"      TMA ring slots of the flow kernel (0: none, streamed tiles are read directly from L2)
  *   "flow_res"     resident tiles per CTA of the flow kernel (-1 automatic)
@@ -205,6 +209,7 @@ typedef enum {
     MODAL_Q_COEFF_BATCH = 11,/* int    [1]                                                          */
     MODAL_Q_KERNEL_INFO = 12,/* int    [8] of the last launch: kernel family (1 tension, 2 small-system, 3 flow, 4 batched tcgen05, 5 streaming, */
                              /*        6 dense team: CTAs per team, samples per launch),                                        */
+                             /*        8 replicated state: CTAs, CTAs per cluster; [6] most rows of an item),                   */
                              /*        tcgen05), CTAs per team (flow) or CTAs, teams (flow) / n groups (batched) / samples per  */
                              /*        launch (streaming), threads, dynamic shared memory bytes, flags (1: H resident in shared */
                              /*        memory or L2, 2: team of several CTAs), ring slots (flow) / accumulator slots (batched)  */
@@ -222,6 +227,10 @@ typedef enum {
                              /*        MiB, most CTAs of a k block, 0, 0                                                       */
     MODAL_Q_STREAM_CHECK = 18, /* double [4]: non-zero entries of H covered by the H stream, non-zero entries of H,            */
                              /*        max |hi + lo - H| / max |H|, rows owned in total (== n_q)                               */
+    MODAL_Q_REPL_CHECK = 19, /* double [8]: host-side check of the replicated-state kernel's layout on 132 CTAs: layout found,      */
+                             /*        non-zero entries of H rebuilt exactly once from the packed blocks (negative: mismatches), */
+                             /*        non-zero entries of H, largest H of a CTA in KiB, most modes of a CTA, most rows of an item, */
+                             /*        packed floats in total, CTAs that hold a mode                                            */
     MODAL_Q_TILE_STATS = 13  /* int    [2]: 16x16 tiles of the packed H, and how many hold a non-zero.   */
                              /*        The device keeps the transverse modes grouped by index parity   */
                              /*        (internal order only: every array of this API is in plan order),*/

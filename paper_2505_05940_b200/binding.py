@@ -19,7 +19,7 @@ LINEAR, TENSION, VK = 0, 1, 2
 SV, FTM = 0, 1
 STRING, RECT = 0, 1
 (Q_MODE_M, Q_MODE_N, Q_PHI_M, Q_PHI_N, Q_LAMBDA, Q_OMEGA, Q_SIGMA, Q_NL_SCALE, Q_PICKUP, Q_ACTIVE,
- Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO, Q_TILE_STATS, Q_MMA_LAYOUT, Q_MMA_SLAB_CHECK, Q_AIRY_ZETA4, Q_STREAM_LAYOUT, Q_STREAM_CHECK) = range(19)
+ Q_H_FULL, Q_COEFF_BATCH, Q_KERNEL_INFO, Q_TILE_STATS, Q_MMA_LAYOUT, Q_MMA_SLAB_CHECK, Q_AIRY_ZETA4, Q_STREAM_LAYOUT, Q_STREAM_CHECK, Q_REPL_CHECK) = range(20)
 AIRY_SINE, AIRY_CLAMPED_RITZ = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -227,7 +227,8 @@ class Plan:
             Q_ACTIVE: ((cb, nq), np.int32), Q_H_FULL: ((nphi, nq, nq), np.float64),
             Q_COEFF_BATCH: ((1,), np.int32), Q_KERNEL_INFO: ((8,), np.int32), Q_TILE_STATS: ((2,), np.int32),
             Q_MMA_LAYOUT: ((16,), np.int32), Q_MMA_SLAB_CHECK: ((3,), np.float64),
-            Q_AIRY_ZETA4: ((nphi,), np.float64), Q_STREAM_LAYOUT: ((16,), np.int32), Q_STREAM_CHECK: ((4,), np.float64)}[what]
+            Q_AIRY_ZETA4: ((nphi,), np.float64), Q_STREAM_LAYOUT: ((16,), np.int32), Q_STREAM_CHECK: ((4,), np.float64),
+            Q_REPL_CHECK: ((8,), np.float64)}[what]
         a = np.zeros(shape, dt)
         self._check(lib.modal_plan_query(self._h, what, a.ctypes.data_as(C.c_void_p), a.nbytes))
         return a

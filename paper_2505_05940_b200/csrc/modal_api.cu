@@ -1624,6 +1624,53 @@ extern "C" modal_status modal_plan_query(const modal_plan *p, int what, void *ds
             }
             return put(v, sizeof v);
         }
+        case MODAL_Q_REPL_CHECK: {
+            // host-side self check of the replicated-state kernel's layout on a grid of 132 CTAs (33 clusters of 4): rebuilds H^n[k][r]
+            // from the packed blocks through the item descriptors (and their mirror images for the blocks stored once) and returns
+            // {layout found, non-zero entries covered exactly once with the right value, non-zero entries of H, largest H of a CTA in KiB,
+            //  most modes of a CTA, most rows of an item, packed floats in total, CTAs with a mode} as 8 doubles
+            double out[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            if (d.model == MODAL_VK && nq <= md::RP_THREADS) {
+                const bool classes = d.geom == MODAL_RECT && p->opt.parity_order;
+                auto cls_q = [&](int k_int) { const int k = p->perm[k_int]; return classes ? (p->mq.m[k] & 1) * 2 + (p->mq.n[k] & 1) : 0; };
+                std::vector<int> class_start{0};
+                for (int k = 1; k < nq; ++k) if (cls_q(k) != cls_q(k - 1)) class_start.push_back(k);
+                class_start.push_back(nq);
+                std::vector<double> Hi((size_t)d.n_phi * nq * nq);
+                mh::unpack_flow_tiles(nq, d.n_phi, p->Hf, Hi.data());
+                mh::ReplLayout L;
+                if ((int)class_start.size() - 1 <= md::RP_MAXCLS && mh::repl_layout(nq, d.n_phi, 132, (size_t)212 * 256, class_start, Hi.data(), L)) {
+                    out[0] = 1;
+                    std::vector<unsigned char> seen(Hi.size(), 0);
+                    double covered = 0, nonzero = 0, bad = 0;
+                    for (double x : Hi) nonzero += x != 0.0;
+                    int mm = 0;
+                    for (int g = 0; g < L.G; ++g) {
+                        const int *T = L.tab.data() + (size_t)g * mh::RP_CTA_STRIDE;
+                        mm = std::max(mm, T[2]);
+                        for (int t = 0; t < T[3]; ++t) {
+                            const int *I = T + mh::RP_HDR + t * mh::RP_ITEM;
+                            const int ld = I[1] & 0xffff, n = T[4 + (I[1] >> 16)];
+                            for (int i = 0; i < I[3]; ++i)
+                                for (int c = 0; c < 4; ++c) {
+                                    const float v = L.Hp[L.cta_hoff[g] + I[0] + (size_t)i * ld + c];
+                                    const int row = I[2] + i, col = I[4] + c;
+                                    if (v == 0.f) continue;
+                                    if (col >= nq) { bad += 1; continue; }
+                                    for (int mirror = 0; mirror < (I[5] >= 0 ? 2 : 1); ++mirror) {
+                                        const size_t e = ((size_t)n * nq + (mirror ? col : row)) * nq + (mirror ? row : col);
+                                        if (seen[e] || (float)Hi[e] != v) bad += 1; else { seen[e] = 1; covered += 1; }
+                                    }
+                                }
+                        }
+                    }
+                    out[1] = bad ? -bad : covered; out[2] = nonzero; out[3] = L.hfloats_max / 256.0; out[4] = mm; out[5] = L.rows_max;
+                    out[6] = (double)L.Hp.size();
+                    for (int g = 0; g < L.G; ++g) out[7] += L.cta_nmodes[g] > 0;
+                }
+            }
+            return put(out, sizeof out);
+        }
         case MODAL_Q_STREAM_CHECK: {
             // host-side self check of the H stream: rebuilds H^n[k][r] from the bf16 hi + lo chunks of every tile and returns
             // {non-zero entries covered, non-zero entries of H, max |hi + lo - H| / max |H|, rows owned in total} as 4 doubles

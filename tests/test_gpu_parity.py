@@ -368,15 +368,18 @@ def test_vk_ftm_scheme_and_auto_start_parity():
     check_parity(gpu, ref["out"], case)
 
 
-def test_c4_shape_whole_gpu_team_short_run():
+@pytest.mark.parametrize("impl,family", [(0, 8), (1, 3)])
+def test_c4_shape_whole_gpu_team_short_run(impl, family):
+    """C4, one sample, against the oracle on the oracle's inputs: the replicated-state kernel (the default at batch 1: clusters over
+    most of the GPU) and the FP32 flow kernel (one team over most of the GPU)."""
     wl = wlmod.c4(batch=1, n_steps=320)
     case = orc.assemble(wl)
     ref = orc.run_case(case, 320)
-    plan = plan_with_oracle_inputs(wl, case)
+    plan = plan_with_oracle_inputs(wl, case, options=dict(vk_impl=impl))
     gpu, fb, _, _ = gpu_run(plan, case.q0, case.qm1, 320)
     torch, mb = _mods()
     info = plan.query(mb.Q_KERNEL_INFO)
-    assert info[0] == 3 and info[1] >= 100                        # one team over (most of) the GPU
+    assert info[0] == family and info[1] >= 100
     check_parity(gpu, ref["out"], case, first=320)
 
 
@@ -417,16 +420,20 @@ def test_c3_tolerance_window_and_full_run():
     assert np.array_equal(gpu2, gpu[:, :2048])                   # deterministic exchange order
 
 
-def test_c4_b1_full_run():
-    """C4 batch 1 (400 + 200 modes, whole-GPU team of the FP32 flow kernel) over all 4410 steps against the stored oracle run."""
+@pytest.mark.parametrize("impl,family", [(0, 8), (1, 3)])
+def test_c4_b1_full_run(impl, family):
+    """C4 batch 1 (400 + 200 modes) as bench.py times it -- the replicated-state kernel, the default -- and through the FP32 flow
+    kernel, over all 4410 steps against the stored oracle run."""
     wl = wlmod.c4(batch=1)
     g, sub, case = load_golden("c4_b1", wl)
     torch, mb = _mods()
-    plan, q0 = mb.plan_from_workload(wl, 0)
+    plan, q0 = mb.plan_from_workload(wl, 0, options=dict(vk_impl=impl))
     gpu, fb, _, st = gpu_run(plan, q0, None, wl["n_steps"])
     info = plan.query(mb.Q_KERNEL_INFO)
-    assert info[0] == 3 and info[1] >= 100 and st == 0 and fb[0] == -1 and g["first_bad"][0] == -1
+    assert info[0] == family and info[1] >= 100 and st == 0 and fb[0] == -1 and g["first_bad"][0] == -1
     check_window_parity(gpu[sub], g["out"], case)
+    gpu2, _, _, _ = gpu_run(plan, q0, None, 1024)
+    assert np.array_equal(gpu2, gpu[:, :1024])                   # fixed summation order: bit-reproducible
 
 
 @pytest.mark.parametrize("batch", [16, 64])
@@ -563,6 +570,41 @@ def test_vk_dense_team_kernel_parity(n_q, n_phi, batch, n_steps, scheme):
     assert np.max(np.abs(traj[sub] - ref["traj"])) <= 1e-4 * np.max(np.abs(ref["traj"]))
     gpu2, _, _, _ = gpu_run(plan, case.q0, None, n_steps, fext=fext, fext_gain=gain)
     assert np.array_equal(gpu, gpu2)
+
+
+@pytest.mark.parametrize("n_q,n_phi,n_steps,scheme", [
+    (57, 23, 500, 1),               # odd N_q (the exchange runs over pairs: one pad word), FTM, classes of 16 / 15 / 13 / 13 modes
+    (130, 40, 300, 0),              # two or three in-plane modes per CTA
+    (100, 50, 400, 0),              # C2's mode counts
+    (10, 10, 300, 0),               # fewer in-plane modes than CTAs of the largest grid: clusters with idle CTAs
+])
+def test_vk_repl_kernel_parity(n_q, n_phi, n_steps, scheme):
+    """Replicated-state kernel (whole in-plane modes per CTA, symmetric parity blocks in shared memory, cluster reduce-scatter + one
+    L2 hop per step) against the oracle, with an external force, the device-side start and the trajectory output; bit-reproducible;
+    refused for a batch."""
+    torch, mb = _mods()
+    wl = _small_vk_workload(n_q, n_phi, 1, n_steps)
+    case = orc.assemble(wl, scheme=scheme)
+    rng = np.random.default_rng(5)
+    fext = np.zeros((1, n_steps)); t = np.arange(48)
+    fext[:, 10:58] = 0.5 * (1 - np.cos(2 * np.pi * t / 48))[None] * rng.uniform(0.5, 2.0, (1, 1))
+    gain = np.where(case.active, rng.normal(size=case.q0.shape), 0.0) * 1e-2
+    ref = orc.simulate(orc.VK, case.c1, case.c2, case.c3, case.w, case.q0, case.qm1, n_steps, nl_scale=case.nl_scale,
+                       H=case.H, fext=orc.f32(fext), fext_gain=gain, want_traj=True)
+    plan = plan_with_oracle_inputs(wl, case, scheme=scheme, options=dict(vk_impl=6))
+    gpu, fb, traj, st = gpu_run(plan, case.q0, None, n_steps, want_traj=True, fext=fext, fext_gain=gain)
+    info = plan.query(mb.Q_KERNEL_INFO)
+    assert info[0] == 8 and info[2] in (4, 8) and st == 0 and np.all(fb == -1)
+    check_parity(gpu, ref["out"], case)
+    assert np.max(np.abs(traj - ref["traj"])) <= 1e-4 * np.max(np.abs(ref["traj"]))
+    gpu2, _, _, _ = gpu_run(plan, case.q0, None, n_steps, fext=fext, fext_gain=gain)
+    assert np.array_equal(gpu, gpu2)
+    gpu3, _, _, _ = gpu_run(plan, case.q0, case.qm1, n_steps, fext=fext, fext_gain=gain)     # explicit q^-1: same run
+    check_parity(gpu3, ref["out"], case)
+    wl2 = _small_vk_workload(n_q, n_phi, 3, 16)
+    case2 = orc.assemble(wl2, scheme=scheme)
+    with pytest.raises(mb.ModalError):                           # one sample only
+        plan_with_oracle_inputs(wl2, case2, scheme=scheme, options=dict(vk_impl=6)).simulate(case2.q0, 8, 0)
 
 
 # ------------------------------------------------------ reverse pass (8(f) row 3) ----

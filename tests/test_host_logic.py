@@ -217,7 +217,7 @@ def test_ftm_plan_refuses_overdamped_mode_naming_it():
 def test_options_api_validates_keys_and_ranges():
     wl, plan = _c0_plan()
     plan.set_option("vk_impl", 2); plan.set_option("flow_g", 4); plan.set_option("timing", 0)
-    for key, val in (("vk_impl", 6), ("flow_ns", 99), ("nonsense", 1)):
+    for key, val in (("vk_impl", 7), ("flow_ns", 99), ("nonsense", 1)):
         with pytest.raises(mb.ModalError) as e:
             plan.set_option(key, val)
         assert e.value.status == mb.EINVAL
@@ -272,6 +272,34 @@ def test_streaming_kernel_layout_covers_H_exactly_once(n_q, n_phi):
     if (n_q, n_phi) == (400, 200):
         # four parity classes of ~100 modes: a tile multiplies only the 7 chunks of its partner class, ~28 % of the dense stream
         assert NKB == 4 and tiles == 800 and nch == 7 and chunks <= 0.3 * 800 * KC
+    plan.close()
+
+
+@pytest.mark.parametrize("n_q,n_phi", [(400, 200), (57, 23), (130, 40)])
+def test_replicated_state_kernel_layout_rebuilds_H(n_q, n_phi):
+    """Host side of the replicated-state kernel (one sample of a large plate, whole in-plane modes per CTA): the packed blocks --
+    one per symmetric pair of parity classes -- and the item descriptors of the threads rebuild every non-zero H^n[k][r] exactly once
+    with its fp32 value, mirror images included; at C4 a CTA holds <= 2 modes in <= 160 KiB."""
+    wl = wlmod.c4(batch=1, n_steps=8)
+    wl["n_q"], wl["n_phi"] = n_q, n_phi
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    found, covered, nonzero, kib, modes, rows, floats, ctas = plan.query(mb.Q_REPL_CHECK)
+    H = plan.query(mb.Q_H_FULL)
+    assert found == 1 and covered == nonzero == np.count_nonzero(H.astype(np.float32))
+    if (n_q, n_phi) == (400, 200):
+        assert kib <= 160 and modes == 2 and rows <= 27 and 128 <= ctas <= 132 and floats * 4 < 21e6
+    plan.close()
+
+
+def test_replicated_state_kernel_refuses_a_dense_uploaded_H():
+    """An uploaded H without the parity zeros has one block per class pair: it does not fit, and the layout says so."""
+    wl = wlmod.c4(batch=1, n_steps=8)
+    wl["n_q"], wl["n_phi"] = 96, 24
+    plan = mb.Plan(mb.desc_from_workload(wl), device=-1)
+    rng = np.random.default_rng(2)
+    H = rng.normal(size=(24, 96, 96)); H = H + H.transpose(0, 2, 1)
+    plan.coeffs_upload(1, H_full=H)
+    assert plan.query(mb.Q_REPL_CHECK)[0] == 0
     plan.close()
 
 
