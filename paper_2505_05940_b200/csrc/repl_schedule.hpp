@@ -30,7 +30,7 @@ constexpr int RP_ITEM = 8;           // ints per item descriptor
 constexpr int RP_JOIN = 4;           // ints per join descriptor
 constexpr int RP_CTA_STRIDE = RP_HDR + RP_THREADS * RP_ITEM + RP_MAXM * RP_MAXCLS * RP_JOIN;
 
-struct ReplBlock { int n, a, b; };   // mode, row class, column class (a <= b)
+struct ReplBlock { int n, a, b; };   // mode, row class, column class (found with a <= b; a CTA may store it the other way round)
 
 struct ReplLayout {
     int n_q = 0, n_phi = 0, G = 0, ncls = 0;
@@ -91,8 +91,18 @@ inline bool repl_layout(int n_q, int n_phi, int G, size_t cap_floats, const std:
     size_t least = (size_t)-1;
     for (int g = 0; g < G; ++g) {
         int *T = L.tab.data() + (size_t)g * RP_CTA_STRIDE;
+        // a block with a != b may be stored either way round (it is its own mirror image): the ROW class pays the long join (one partial
+        // per quad of columns, the column class one per chunk of rows), so the roles are dealt out evenly over the classes of the CTA
         std::vector<ReplBlock> blocks;
-        for (int m = 0; m < L.cta_nmodes[g]; ++m) for (const ReplBlock &b : mblocks[L.cta_modes[(size_t)g * RP_MAXM + m]]) blocks.push_back(b);
+        std::vector<int> rowjoins(ncls, 0);
+        for (int m = 0; m < L.cta_nmodes[g]; ++m)
+            for (ReplBlock b : mblocks[L.cta_modes[(size_t)g * RP_MAXM + m]]) {
+                if (b.a != b.b) {
+                    if (rowjoins[b.b] < rowjoins[b.a]) std::swap(b.a, b.b);
+                    rowjoins[b.a] += ld(b.b) / 4;
+                }
+                blocks.push_back(b);
+            }
         int quads = 0;
         for (const ReplBlock &b : blocks) quads += ld(b.b) / 4;
         int nchunks = quads ? RP_THREADS / quads : 1;
