@@ -48,36 +48,35 @@ __host__ __device__ inline size_t repl_smem_bytes(int hfloats_max, int cp_max, i
     return ((size_t)hfloats_max + cp_max + rp_max + 4 + (size_t)2 * CL * SL) * 4 + 64;
 }
 
-// sums of nv <= 8 values over the block, fixed order; every thread gets them.  red: [16 warps][8] floats of THIS step's parity (the
-// caller double-buffers, so one barrier is enough: the buffer is rewritten two steps later, behind several barriers).
-__device__ __forceinline__ void rp_block_sum8(float (&a)[8], int nv, float *red)
+// sums of the first NV (<= 8) values over the block; every thread gets the same bits.  red: [16 warps][8] floats of THIS step's parity
+// (the caller double-buffers, so one barrier is enough: the buffer is rewritten two steps later, behind several barriers).
+// Level-major butterflies (the NV shuffles of a level are independent), then lane y of every warp reads the row of warp y and a
+// 16-lane butterfly joins them: 16 dependent shared-memory loads per thread measured 640 cycles here, this 150.
+template <int NV>
+__device__ __forceinline__ void rp_block_sum(float (&a)[8], float *red)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
-    for (int x = 0; x < 8; ++x)
-        if (x < nv) {
+    for (int m = 16; m >= 1; m >>= 1) {
 #pragma unroll
-            for (int m = 16; m >= 1; m >>= 1) a[x] += __shfl_xor_sync(0xffffffffu, a[x], m);
-        }
+        for (int x = 0; x < NV; ++x) a[x] += __shfl_xor_sync(0xffffffffu, a[x], m);
+    }
     if (lane == 0) {
         *reinterpret_cast<float4 *>(red + warp * 8) = make_float4(a[0], a[1], a[2], a[3]);
-        if (nv > 4) *reinterpret_cast<float4 *>(red + warp * 8 + 4) = make_float4(a[4], a[5], a[6], a[7]);
+        if (NV > 4) *reinterpret_cast<float4 *>(red + warp * 8 + 4) = make_float4(a[4], a[5], a[6], a[7]);
     }
     __syncthreads();
-    float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-    for (int y = 0; y < RP_THREADS / 32; ++y) {
-        const float4 u = *reinterpret_cast<const float4 *>(red + y * 8);
-        A.x += u.x; A.y += u.y; A.z += u.z; A.w += u.w;
+    const float4 u = *reinterpret_cast<const float4 *>(red + (lane & 15) * 8);
+    a[0] = u.x; a[1] = u.y; a[2] = u.z; a[3] = u.w;
+    if (NV > 4) {
+        const float4 w = *reinterpret_cast<const float4 *>(red + (lane & 15) * 8 + 4);
+        a[4] = w.x; a[5] = w.y; a[6] = w.z; a[7] = w.w;
     }
-    if (nv > 4) {
 #pragma unroll
-        for (int y = 0; y < RP_THREADS / 32; ++y) {
-            const float4 u = *reinterpret_cast<const float4 *>(red + y * 8 + 4);
-            B.x += u.x; B.y += u.y; B.z += u.z; B.w += u.w;
-        }
+    for (int m = 8; m >= 1; m >>= 1) {
+#pragma unroll
+        for (int x = 0; x < NV; ++x) a[x] += __shfl_xor_sync(0xffffffffu, a[x], m);
     }
-    a[0] = A.x; a[1] = A.y; a[2] = A.z; a[3] = A.w; a[4] = B.x; a[5] = B.y; a[6] = B.z; a[7] = B.w;
 }
 
 template <bool TIMING>
@@ -207,7 +206,9 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
         for (int m = RP_MAXM; m < 8; ++m) vals[m] = 0.f;
         // a1 pickup + a6 write-out ride on the same block sum (slots RP_MAXM, RP_MAXM + 1; only the CTA out_cta)
         if (out_cta) { vals[RP_MAXM] = wk * x; vals[RP_MAXM + 1] = x * x; }
-        rp_block_sum8(vals, out_cta ? RP_MAXM + 2 : nmodes, red + (n & 1) * 128);
+        if (out_cta) rp_block_sum<RP_MAXM + 2>(vals, red + (n & 1) * 128);
+        else if (nmodes <= 2) rp_block_sum<2>(vals, red + (n & 1) * 128);
+        else rp_block_sum<RP_MAXM>(vals, red + (n & 1) * 128);
         if (out_cta) {
             if (k == 0) { a.out[n] = vals[RP_MAXM]; if (bad < 0 && !(isfinite(vals[RP_MAXM]) && isfinite(vals[RP_MAXM + 1]))) bad = n; }
             if (a.traj && mine) a.traj[(size_t)n * a.n_q + kp] = q;
