@@ -48,8 +48,11 @@ __device__ __forceinline__ void bp_block_sum2(float a, float b, float *red, int 
     for (int m = 16; m >= 1; m >>= 1) { a += __shfl_xor_sync(FLOW_FULL, a, m); b += __shfl_xor_sync(FLOW_FULL, b, m); }
     if (lane == 0) { red[warp] = a; red[16 + warp] = b; }
     __syncthreads();
-    A = 0.f; B = 0.f;
-    for (int x = 0; x < nwarps; ++x) { A += red[x]; B += red[16 + x]; }
+    // lane y reads the sums of warp y, a 16-lane butterfly joins them (a loop of dependent shared-memory loads cost ~500 cycles here)
+    const int y = lane & 15;
+    A = y < nwarps ? red[y] : 0.f; B = y < nwarps ? red[16 + y] : 0.f;
+#pragma unroll
+    for (int m = 8; m >= 1; m >>= 1) { A += __shfl_xor_sync(FLOW_FULL, A, m); B += __shfl_xor_sync(FLOW_FULL, B, m); }
     __syncthreads();
 }
 
