@@ -544,6 +544,7 @@ modal_status configure_repl(modal_plan *p)
     const size_t dyn_max = SMEM_LIMIT - std::max(fa.sharedSizeBytes, fb.sharedSizeBytes) - 1024;
     CU(cudaFuncSetAttribute(md::vk_repl_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
     CU(cudaFuncSetAttribute(md::vk_repl_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
+    CU(cudaFuncSetAttribute(md::vk_repl_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
     std::vector<double> Hi;
     const int NQ2 = (nq + 1) & ~1;
     for (int CL : {8, 4}) {
@@ -897,7 +898,11 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             cudaLaunchAttribute at[1];
             at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = m.CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
             cfg.attrs = at; cfg.numAttrs = 1;
-            CU(timing ? cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<true>, a) : cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<false>, a));
+            int mm = 0;
+            for (int nm : m.L.cta_nmodes) mm = std::max(mm, nm);
+            if (timing) CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<true, md::RP_MAXM>, a));
+            else if (mm <= 2) CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<false, 2>, a));
+            else CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<false, md::RP_MAXM>, a));
         }
         CU(cudaGetLastError());
         if (timing) {

@@ -79,7 +79,8 @@ __device__ __forceinline__ void rp_block_sum(float (&a)[8], float *red)
     }
 }
 
-template <bool TIMING>
+// MM: mode slots the instance carries (2 when no CTA holds more than two in-plane modes, as at C4: half the unrolled join code)
+template <bool TIMING, int MM = RP_MAXM>
 __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a)
 {
     __shared__ __align__(16) float qs[RP_THREADS + 8];
@@ -101,13 +102,13 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
     const int4 I0 = *reinterpret_cast<const int4 *>(T + RP_HDR + k * RP_ITEM), I1 = *reinterpret_cast<const int4 *>(T + RP_HDR + k * RP_ITEM + 4);
     const bool has_item = k < T[3];
     const bool mine = k < a.n_q;
-    int4 J[RP_MAXM];
+    int4 J[MM];
     {
         const int c = mine ? a.cls[k] : 0, c0 = mine ? k : 0;
         int first = c0;                                        // first mode of the class: walk down while the class is the same
         while (first > 0 && a.cls[first - 1] == c) --first;
 #pragma unroll
-        for (int m = 0; m < RP_MAXM; ++m) {
+        for (int m = 0; m < MM; ++m) {
             J[m] = make_int4(0, 0, 0, 0);
             if (mine && m < nmodes) {
                 J[m] = *reinterpret_cast<const int4 *>(T + RP_HDR + RP_THREADS * RP_ITEM + (m * RP_MAXCLS + c) * RP_JOIN);
@@ -116,9 +117,9 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
             }
         }
     }
-    float sm_[RP_MAXM];
+    float sm_[MM];
 #pragma unroll
-    for (int m = 0; m < RP_MAXM; ++m) sm_[m] = m < nmodes ? a.s[T[4 + m]] : 0.f;
+    for (int m = 0; m < MM; ++m) sm_[m] = m < nmodes ? a.s[T[4 + m]] : 0.f;
     double q = 0.0, v = 0.0, kv = 0.0, kq = 0.0, r = 0.0, ast = 0.0, gn = 0.0; float wk = 0.f;
     if (mine) {
         q = a.q0[k]; v = a.v0[k]; kv = a.kv[k]; kq = a.kq[k]; r = a.r[k]; ast = a.astart[k]; wk = a.w[k];
@@ -189,9 +190,9 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
         __syncthreads();
         if (TIMING) { const long long t_ = clock64(); tm[0] += t_ - tk; tk = t_; }
         // ---- join (thread k: t_m[k] of every mode of the CTA), a3, a4 ---------------------------------------------------
-        float t[RP_MAXM], vals[8];
+        float t[MM], vals[8];
 #pragma unroll
-        for (int m = 0; m < RP_MAXM; ++m) {
+        for (int m = 0; m < MM; ++m) {
             float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
             if (J[m].x) {
                 const float *src = (J[m].x == 2 ? rpart : cpart) + J[m].y;
@@ -203,19 +204,19 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
             t[m] = (a0 + a1) + (a2 + a3); vals[m] = x * t[m];
         }
 #pragma unroll
-        for (int m = RP_MAXM; m < 8; ++m) vals[m] = 0.f;
-        // a1 pickup + a6 write-out ride on the same block sum (slots RP_MAXM, RP_MAXM + 1; only the CTA out_cta)
-        if (out_cta) { vals[RP_MAXM] = wk * x; vals[RP_MAXM + 1] = x * x; }
-        if (out_cta) rp_block_sum<RP_MAXM + 2>(vals, red + (n & 1) * 128);
-        else if (nmodes <= 2) rp_block_sum<2>(vals, red + (n & 1) * 128);
-        else rp_block_sum<RP_MAXM>(vals, red + (n & 1) * 128);
+        for (int m = MM; m < 8; ++m) vals[m] = 0.f;
+        // a1 pickup + a6 write-out ride on the same block sum (slots MM, MM + 1; only the CTA out_cta)
+        if (out_cta) { vals[MM] = wk * x; vals[MM + 1] = x * x; }
+        if (out_cta) rp_block_sum<MM + 2>(vals, red + (n & 1) * 128);
+        else if (MM == 2 || nmodes <= 2) rp_block_sum<2>(vals, red + (n & 1) * 128);
+        else rp_block_sum<MM>(vals, red + (n & 1) * 128);
         if (out_cta) {
-            if (k == 0) { a.out[n] = vals[RP_MAXM]; if (bad < 0 && !(isfinite(vals[RP_MAXM]) && isfinite(vals[RP_MAXM + 1]))) bad = n; }
+            if (k == 0) { a.out[n] = vals[MM]; if (bad < 0 && !(isfinite(vals[MM]) && isfinite(vals[MM + 1]))) bad = n; }
             if (a.traj && mine) a.traj[(size_t)n * a.n_q + kp] = q;
         }
         float facc = 0.f;
 #pragma unroll
-        for (int m = 0; m < RP_MAXM; ++m) facc = fmaf(sm_[m] * vals[m], t[m], facc);
+        for (int m = 0; m < MM; ++m) facc = fmaf(sm_[m] * vals[m], t[m], facc);
         if (TIMING) { const long long t_ = clock64(); tm[1] += t_ - tk; tk = t_; }
         // ---- exchange ----------------------------------------------------------------------------------------------
         const unsigned par = (unsigned)n & 1u, epoch = (unsigned)n + 1u;
