@@ -545,6 +545,7 @@ modal_status configure_repl(modal_plan *p)
     CU(cudaFuncSetAttribute(md::vk_repl_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
     CU(cudaFuncSetAttribute(md::vk_repl_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
     CU(cudaFuncSetAttribute(md::vk_repl_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
+    CU(cudaFuncSetAttribute(md::vk_repl_kernel<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_max));
     std::vector<double> Hi;
     const int NQ2 = (nq + 1) & ~1;
     for (int CL : {8, 4}) {
@@ -900,7 +901,8 @@ modal_status run(modal_plan *p, int batch, int n_steps, const modal_init *init, 
             cfg.attrs = at; cfg.numAttrs = 1;
             int mm = 0;
             for (int nm : m.L.cta_nmodes) mm = std::max(mm, nm);
-            if (timing) CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<true, md::RP_MAXM>, a));
+            if (timing && mm <= 2) CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<true, 2>, a));
+            else if (timing) CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<true, md::RP_MAXM>, a));
             else if (mm <= 2) CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<false, 2>, a));
             else CU(cudaLaunchKernelEx(&cfg, md::vk_repl_kernel<false, md::RP_MAXM>, a));
         }
