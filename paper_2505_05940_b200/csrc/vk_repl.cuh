@@ -172,14 +172,14 @@ __global__ void __launch_bounds__(RP_THREADS, 1) vk_repl_kernel(const ReplArgs a
             float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
             if (I1.y >= 0) {
                 float *rp = rpart + I1.y;
-#pragma unroll 4
+#pragma unroll 2
                 for (int i = 0; i < I0.w; ++i, hp += ld4, rp += I1.z) {
                     const float4 h = *hp; const float qr = qa[i];
                     c4.x = fmaf(h.x, qr, c4.x); c4.y = fmaf(h.y, qr, c4.y); c4.z = fmaf(h.z, qr, c4.z); c4.w = fmaf(h.w, qr, c4.w);
                     *rp = fmaf(h.x, qb.x, fmaf(h.y, qb.y, fmaf(h.z, qb.z, h.w * qb.w)));
                 }
             } else {
-#pragma unroll 4
+#pragma unroll 2
                 for (int i = 0; i < I0.w; ++i, hp += ld4) {
                     const float4 h = *hp; const float qr = qa[i];
                     c4.x = fmaf(h.x, qr, c4.x); c4.y = fmaf(h.y, qr, c4.y); c4.z = fmaf(h.z, qr, c4.z); c4.w = fmaf(h.w, qr, c4.w);
